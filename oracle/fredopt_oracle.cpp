@@ -1,0 +1,408 @@
+// fredopt_oracle.cpp -- TEST INFRASTRUCTURE, NOT THE PRODUCT.
+//
+// Plain, slow, single-threaded fp64 CPU restatement of the hot path of FREDopt's plan
+// optimisation, written from the paper (/root/reference/PAPER.md, arxiv 2509.20012) and the
+// readings recorded in DESIGN.md ("Readings of the paper", R0..R22 = SURVEY.md sec. 8c A0..A22).
+// Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference leg may use
+// it.  It shares no code with the CUDA path (paper_2509_20012_b200/csrc) and neither includes the
+// other.
+//
+// What it computes, step by step in the paper's order and notation:
+//   * AMSrelaxDLET (Fig. 2) in its SIMULTANEOUS (Cimmino) form (reading R1): every
+//     residual is taken at the same fluence x and one summed, weighted, relaxed step is applied, then
+//     the clamp fluence_j < 0 -> 0;
+//   * SuperiorDLET (Fig. 3): before each AMS step, `reductionsN` perturbations
+//     x' = x - beta * grad_cost(x), beta = beta0 * a^s, accepted only if cost(x') < cost(x);
+//   * cost chi^2(x) of Eq. (2) and its gradient;
+//   * LETd = l / d voxel-wise (Eq. (1) with the dose as denominator);
+//   * the OAR LETd limit linearised as <L_i - LETmax*D_i, x> <= 0, the proximity function and the
+//     violation count (not in the paper: BASELINE.json north_star; reading R18).
+//
+// Everything is double; the fp32 inputs are widened once.  Rows are visited in index order; the
+// back-projection is an ordered scatter-add through the forward CSR (no transposed copy).  There is
+// no blocking, fusion or reordering.
+//
+// Parity pins: tests/test_oracle_pins.py checks this file against dense brute force, closed forms
+// and invariants (SURVEY.md sec. 8c pins 1-12).  The paper prints no worked numbers of an iteration
+// and never states lambda, alpha, eta, reductionsN or the matrix sizes, so parity with the PAPER'S OWN
+// RUNS is unpinned; the algorithmic content is pinned by those mathematical checks.
+
+#include <cmath>
+#include <cstdint>
+#include <cstring>
+#include <vector>
+
+namespace {
+
+struct Csr {
+    int64_t n_rows = 0, n_cols = 0;
+    std::vector<int64_t> ptr;
+    std::vector<int32_t> col;
+    std::vector<double> val;   // widened once from fp32
+};
+
+struct Bounds {   // all widened from the fp32 bit patterns the caller passed; NaN = absent
+    double weight, dose_lo, dose_hi, dl_lo, dl_hi, letd_max, dose_ref, dl_ref;
+};
+
+inline bool present(double v) { return !std::isnan(v); }
+
+struct Plan {
+    Csr D, L;
+    std::vector<int32_t> label;        // per voxel; 0 = unconstrained
+    std::vector<Bounds> bounds;        // index s-1 for label s
+    std::vector<double> nD, nL, nT;    // squared norms of D_i, L_i, L_i - letd_max*D_i  (per voxel)
+    std::vector<double> what;          // normalised weight per structure (index s-1)
+    double W = 0.0;
+    int64_t n_sets = 0, n_zero_norm_sets = 0;
+    std::vector<double> x;             // fluence
+    // state of Fig. 3
+    int64_t k = 0, s = 0, trials = 0;
+    bool started = false;
+    double beta_next = 0.0, eta_pow = 1.0, last_beta = 0.0;
+    // options
+    double eta = 1.0;
+    int64_t reductionsN = 1, max_trials = 200;
+    bool accept_check = true;
+};
+
+// <A_i, x>
+inline double row_dot(const Csr& A, int64_t i, const std::vector<double>& x) {
+    double acc = 0.0;
+    for (int64_t p = A.ptr[i]; p < A.ptr[i + 1]; ++p) acc += A.val[p] * x[A.col[p]];
+    return acc;
+}
+
+bool has_dose_slab(const Bounds& b) { return present(b.dose_lo) || present(b.dose_hi); }
+bool has_dl_slab(const Bounds& b) { return present(b.dl_lo) || present(b.dl_hi); }
+bool has_letd(const Bounds& b) { return present(b.letd_max); }
+
+// Signed residual of a hyperslab lo <= val <= hi (reading R5: one set per (row, quantity); R2: sign):
+// upper violations positive, lower violations negative, 0 inside.
+inline double slab_residual(double val, double lo, double hi) {
+    if (present(hi) && val > hi) return val - hi;
+    if (present(lo) && val < lo) return val - lo;
+    return 0.0;
+}
+
+// <L_i - letd_max * D_i, x> over the union pattern of rows i of L and D (merge of two sorted rows).
+double letd_row_dot(const Plan& P, int64_t i, double letd_max, const std::vector<double>& x, double* norm2) {
+    const Csr &D = P.D, &L = P.L;
+    int64_t p = D.ptr[i], pe = D.ptr[i + 1], q = L.ptr[i], qe = L.ptr[i + 1];
+    double acc = 0.0, n2 = 0.0;
+    while (p < pe || q < qe) {
+        int32_t cd = p < pe ? D.col[p] : INT32_MAX, cl = q < qe ? L.col[q] : INT32_MAX;
+        double a;
+        int32_t c;
+        if (cd == cl) { a = L.val[q] - letd_max * D.val[p]; c = cd; ++p; ++q; }
+        else if (cd < cl) { a = -letd_max * D.val[p]; c = cd; ++p; }
+        else { a = L.val[q]; c = cl; ++q; }
+        acc += a * x[c];
+        n2 += a * a;
+    }
+    if (norm2) *norm2 = n2;
+    return acc;
+}
+
+void setup(Plan& P) {
+    const int64_t V = P.D.n_rows;
+    P.nD.assign(V, 0.0); P.nL.assign(V, 0.0); P.nT.assign(V, 0.0);
+    std::vector<int64_t> part(P.bounds.size(), 0);   // participating sets per structure
+    std::vector<double> zero(P.D.n_cols, 0.0);
+    P.n_sets = 0; P.n_zero_norm_sets = 0;
+    for (int64_t i = 0; i < V; ++i) {
+        int32_t s = P.label[i];
+        if (s == 0) continue;
+        const Bounds& b = P.bounds[s - 1];
+        double n = 0.0;
+        for (int64_t p = P.D.ptr[i]; p < P.D.ptr[i + 1]; ++p) n += P.D.val[p] * P.D.val[p];
+        P.nD[i] = n;
+        n = 0.0;
+        for (int64_t p = P.L.ptr[i]; p < P.L.ptr[i + 1]; ++p) n += P.L.val[p] * P.L.val[p];
+        P.nL[i] = n;
+        if (has_letd(b)) { letd_row_dot(P, i, b.letd_max, zero, &n); P.nT[i] = n; }
+        if (has_dose_slab(b)) { ++P.n_sets; if (P.nD[i] > 0) ++part[s - 1]; else ++P.n_zero_norm_sets; }
+        if (has_dl_slab(b))   { ++P.n_sets; if (P.nL[i] > 0) ++part[s - 1]; else ++P.n_zero_norm_sets; }
+        if (has_letd(b))      { ++P.n_sets; if (P.nT[i] > 0) ++part[s - 1]; else ++P.n_zero_norm_sets; }
+    }
+    // reading R3: w^_s = w_s / W,  W = sum over participating sets of w_{s(k)} (grouped by structure, s ascending)
+    P.W = 0.0;
+    for (size_t s = 0; s < P.bounds.size(); ++s) P.W += P.bounds[s].weight * (double)part[s];
+    P.what.assign(P.bounds.size(), 0.0);
+    for (size_t s = 0; s < P.bounds.size(); ++s) P.what[s] = P.W > 0 ? P.bounds[s].weight / P.W : 0.0;
+}
+
+// chi^2(x), Eq. (2): sum_i w^_i (Dref_i - D(x)_i)^2 + sum_i w^_i (cDLref_i - cDL(x)_i)^2
+double cost(const Plan& P, const std::vector<double>& x) {
+    double phi = 0.0;
+    for (int64_t i = 0; i < P.D.n_rows; ++i) {
+        int32_t s = P.label[i];
+        if (s == 0) continue;
+        const Bounds& b = P.bounds[s - 1];
+        if (present(b.dose_ref)) { double e = b.dose_ref - row_dot(P.D, i, x); phi += P.what[s - 1] * e * e; }
+        if (present(b.dl_ref))   { double e = b.dl_ref - row_dot(P.L, i, x);   phi += P.what[s - 1] * e * e; }
+    }
+    return phi;
+}
+
+// grad chi^2(x) = 2 [ sum_i w^_i (D(x)_i - Dref_i) D_i + sum_i w^_i (cDL(x)_i - cDLref_i) L_i ]
+void grad_cost(const Plan& P, const std::vector<double>& x, std::vector<double>& g) {
+    g.assign(P.D.n_cols, 0.0);
+    for (int64_t i = 0; i < P.D.n_rows; ++i) {
+        int32_t s = P.label[i];
+        if (s == 0) continue;
+        const Bounds& b = P.bounds[s - 1];
+        if (present(b.dose_ref)) {
+            double c = 2.0 * P.what[s - 1] * (row_dot(P.D, i, x) - b.dose_ref);
+            for (int64_t p = P.D.ptr[i]; p < P.D.ptr[i + 1]; ++p) g[P.D.col[p]] += c * P.D.val[p];
+        }
+        if (present(b.dl_ref)) {
+            double c = 2.0 * P.what[s - 1] * (row_dot(P.L, i, x) - b.dl_ref);
+            for (int64_t p = P.L.ptr[i]; p < P.L.ptr[i + 1]; ++p) g[P.L.col[p]] += c * P.L.val[p];
+        }
+    }
+}
+
+// One pass over all declared sets at x.  If `step` is non-null it receives
+//   sum_{k in P} w^_k (r_k / n_k) a_k      (the summed Fig. 2 step fractions)
+// prox = 1/2 sum_{k in P} w^_k r_k^2 / n_k ;  n_viol = #{declared sets with r_k != 0}.
+void constraint_pass(const Plan& P, const std::vector<double>& x, std::vector<double>* step,
+                     double* prox, int64_t* n_viol) {
+    if (step) step->assign(P.D.n_cols, 0.0);
+    double pr = 0.0;
+    int64_t nv = 0;
+    for (int64_t i = 0; i < P.D.n_rows; ++i) {
+        int32_t s = P.label[i];
+        if (s == 0) continue;
+        const Bounds& b = P.bounds[s - 1];
+        const double w = P.what[s - 1];
+        if (has_dose_slab(b)) {                                   // dose block of Fig. 2 (R4)
+            double r = slab_residual(row_dot(P.D, i, x), b.dose_lo, b.dose_hi);
+            if (r != 0.0) ++nv;
+            if (P.nD[i] > 0 && r != 0.0) {
+                pr += 0.5 * w * r * r / P.nD[i];
+                if (step) { double c = w * r / P.nD[i];
+                    for (int64_t p = P.D.ptr[i]; p < P.D.ptr[i + 1]; ++p) (*step)[P.D.col[p]] += c * P.D.val[p]; }
+            }
+        }
+        if (has_dl_slab(b)) {                                     // cDLET block of Fig. 2
+            double r = slab_residual(row_dot(P.L, i, x), b.dl_lo, b.dl_hi);
+            if (r != 0.0) ++nv;
+            if (P.nL[i] > 0 && r != 0.0) {
+                pr += 0.5 * w * r * r / P.nL[i];
+                if (step) { double c = w * r / P.nL[i];
+                    for (int64_t p = P.L.ptr[i]; p < P.L.ptr[i + 1]; ++p) (*step)[P.L.col[p]] += c * P.L.val[p]; }
+            }
+        }
+        if (has_letd(b)) {                                        // <L_i - LETmax D_i, x> <= 0 (north_star)
+            double val = letd_row_dot(P, i, b.letd_max, x, nullptr);
+            double r = val > 0.0 ? val : 0.0;
+            if (r != 0.0) ++nv;
+            if (P.nT[i] > 0 && r != 0.0) {
+                pr += 0.5 * w * r * r / P.nT[i];
+                if (step) { double c = w * r / P.nT[i];
+                    for (int64_t p = P.L.ptr[i]; p < P.L.ptr[i + 1]; ++p) (*step)[P.L.col[p]] += c * P.L.val[p];
+                    for (int64_t p = P.D.ptr[i]; p < P.D.ptr[i + 1]; ++p) (*step)[P.D.col[p]] -= c * b.letd_max * P.D.val[p]; }
+            }
+        }
+    }
+    if (prox) *prox = pr;
+    if (n_viol) *n_viol = nv;
+}
+
+void fill_csr(Csr& A, int64_t V, int64_t S, const int64_t* ptr, const int32_t* col, const float* val) {
+    A.n_rows = V; A.n_cols = S;
+    A.ptr.assign(ptr, ptr + V + 1);
+    int64_t nnz = ptr[V];
+    A.col.assign(col, col + nnz);
+    A.val.resize(nnz);
+    for (int64_t p = 0; p < nnz; ++p) A.val[p] = (double)val[p];
+}
+
+}  // namespace
+
+extern "C" {
+
+void* oracle_create(int64_t V, int64_t S, const int64_t* ptrD, const int32_t* colD, const float* valD,
+                    const int64_t* ptrL, const int32_t* colL, const float* valL, const int32_t* labels,
+                    const float* bounds /* n_struct x 8: weight, dose_lo, dose_hi, dl_lo, dl_hi, letd_max, dose_ref, dl_ref */,
+                    int32_t n_struct) {
+    Plan* P = new Plan();
+    fill_csr(P->D, V, S, ptrD, colD, valD);
+    fill_csr(P->L, V, S, ptrL, colL, valL);
+    P->label.assign(labels, labels + V);
+    for (int32_t s = 0; s < n_struct; ++s) {
+        const float* b = bounds + 8 * s;
+        P->bounds.push_back(Bounds{(double)b[0], (double)b[1], (double)b[2], (double)b[3], (double)b[4],
+                                   (double)b[5], (double)b[6], (double)b[7]});
+    }
+    P->x.assign(S, 0.0);
+    setup(*P);
+    return P;
+}
+
+void oracle_destroy(void* h) { delete (Plan*)h; }
+
+void oracle_set_x(void* h, const float* x) { Plan* P = (Plan*)h; for (size_t j = 0; j < P->x.size(); ++j) P->x[j] = (double)x[j]; }
+void oracle_set_x64(void* h, const double* x) { Plan* P = (Plan*)h; P->x.assign(x, x + P->x.size()); }
+void oracle_get_x(void* h, double* x) { Plan* P = (Plan*)h; std::memcpy(x, P->x.data(), P->x.size() * sizeof(double)); }
+
+// keys: 0 eta, 1 reductionsN, 2 accept_check, 3 max_trials, 4 reset (k, s, beta)
+void oracle_set_option(void* h, int32_t key, double v) {
+    Plan* P = (Plan*)h;
+    switch (key) {
+        case 0: P->eta = v; break;
+        case 1: P->reductionsN = (int64_t)v; break;
+        case 2: P->accept_check = v != 0.0; break;
+        case 3: P->max_trials = (int64_t)v; break;
+        case 4: P->k = 0; P->s = 0; P->trials = 0; P->started = false; P->eta_pow = 1.0; P->last_beta = 0.0; break;
+        default: break;
+    }
+}
+
+// d = D x, l = L x over ALL rows; LETd_i = l_i / d_i where d_i > 0, else 0 (Eq. (1); R15)
+void oracle_dose_let(void* h, const double* xin, double* dose, double* l_out, double* letd) {
+    Plan* P = (Plan*)h;
+    std::vector<double> x = xin ? std::vector<double>(xin, xin + P->x.size()) : P->x;
+    for (int64_t i = 0; i < P->D.n_rows; ++i) {
+        double d = row_dot(P->D, i, x), l = row_dot(P->L, i, x);
+        if (dose) dose[i] = d;
+        if (l_out) l_out[i] = l;
+        if (letd) letd[i] = d > 0.0 ? l / d : 0.0;
+    }
+}
+
+// Same as oracle_dose_let but only for the listed rows (full-size sampled parity).
+void oracle_dose_let_rows(void* h, const double* xin, const int64_t* rows, int64_t n, double* dose, double* l_out, double* letd) {
+    Plan* P = (Plan*)h;
+    std::vector<double> x = xin ? std::vector<double>(xin, xin + P->x.size()) : P->x;
+    for (int64_t t = 0; t < n; ++t) {
+        int64_t i = rows[t];
+        double d = row_dot(P->D, i, x), l = row_dot(P->L, i, x);
+        dose[t] = d; l_out[t] = l; letd[t] = d > 0.0 ? l / d : 0.0;
+    }
+}
+
+// out_j = sum_i D_ij u_i + L_ij v_i over all rows (active_only: rows with label != 0), ordered scatter-add.
+// out_abs_j = sum_i |D_ij u_i| + |L_ij v_i|  (the scale the per-element tolerance refers to).
+void oracle_transpose(void* h, const double* u, const double* v, int32_t active_only, double* out, double* out_abs) {
+    Plan* P = (Plan*)h;
+    const int64_t S = P->D.n_cols;
+    for (int64_t j = 0; j < S; ++j) { out[j] = 0.0; if (out_abs) out_abs[j] = 0.0; }
+    for (int64_t i = 0; i < P->D.n_rows; ++i) {
+        if (active_only && P->label[i] == 0) continue;
+        if (u) for (int64_t p = P->D.ptr[i]; p < P->D.ptr[i + 1]; ++p) {
+            double t = P->D.val[p] * u[i]; out[P->D.col[p]] += t; if (out_abs) out_abs[P->D.col[p]] += std::fabs(t); }
+        if (v) for (int64_t p = P->L.ptr[i]; p < P->L.ptr[i + 1]; ++p) {
+            double t = P->L.val[p] * v[i]; out[P->L.col[p]] += t; if (out_abs) out_abs[P->L.col[p]] += std::fabs(t); }
+    }
+}
+
+double oracle_cost(void* h, const double* xin) {
+    Plan* P = (Plan*)h;
+    std::vector<double> x = xin ? std::vector<double>(xin, xin + P->x.size()) : P->x;
+    return cost(*P, x);
+}
+
+void oracle_grad(void* h, const double* xin, double* g) {
+    Plan* P = (Plan*)h;
+    std::vector<double> x = xin ? std::vector<double>(xin, xin + P->x.size()) : P->x, gv;
+    grad_cost(*P, x, gv);
+    std::memcpy(g, gv.data(), gv.size() * sizeof(double));
+}
+
+void oracle_proximity(void* h, const double* xin, double* prox, int64_t* n_viol) {
+    Plan* P = (Plan*)h;
+    std::vector<double> x = xin ? std::vector<double>(xin, xin + P->x.size()) : P->x;
+    constraint_pass(*P, x, nullptr, prox, n_viol);
+}
+
+// SuperiorDLET (Fig. 3) around the simultaneous AMSrelaxDLET step (Fig. 2).
+// lambda, beta0, a arrive as the fp32 bit patterns the caller passes to the C-ABI and are widened here.
+void oracle_iterate(void* h, int32_t n_iter, float lambda_f, float beta0_f, float a_f) {
+    Plan* P = (Plan*)h;
+    const double lambda = (double)lambda_f, beta0 = (double)beta0_f, a = (double)a_f;
+    const int64_t S = P->D.n_cols;
+    if (!P->started) { P->beta_next = beta0; P->eta_pow = 1.0; P->started = true; }   // beta_0 = beta0; eta^0 = 1
+    std::vector<double> g, xn(S), step;
+    for (int32_t it = 0; it < n_iter; ++it) {
+        // ---- perturbation phase; skipped entirely when beta0 == 0 (pure AMS)
+        if (beta0 != 0.0) {
+            for (int64_t t = 0; t < P->reductionsN; ++t) {
+                const double phi0 = cost(*P, P->x);
+                grad_cost(*P, P->x, g);
+                bool zero = true;
+                for (int64_t j = 0; j < S; ++j) if (g[j] != 0.0) { zero = false; break; }
+                if (zero) break;                                              // R10: nothing to reduce
+                for (int64_t trial = 0; trial < P->max_trials; ++trial) {     // `while loop do`; R10 cap
+                    const double beta = P->beta_next;                        // s = s + 1; beta = alpha^s (R8: beta0 * a^s)
+                    P->beta_next *= a; ++P->s; ++P->trials;
+                    for (int64_t j = 0; j < S; ++j) xn[j] = P->x[j] - beta * g[j];
+                    if (!P->accept_check || cost(*P, xn) < phi0) {            // strict decrease
+                        P->x = xn; P->last_beta = beta; break;
+                    }
+                }
+            }
+        }
+        // ---- feasibility-seeking step with w_k = eta^k w, simultaneous form (R1)
+        constraint_pass(*P, P->x, &step, nullptr, nullptr);
+        const double relax = lambda * P->eta_pow;
+        for (int64_t j = 0; j < S; ++j) {
+            double v = P->x[j] - relax * step[j];
+            P->x[j] = v < 0.0 ? 0.0 : v;                                       // clamp (R6)
+        }
+        P->eta_pow *= P->eta;
+        ++P->k;
+    }
+}
+
+// out: k, s, trials, n_sets, n_zero_norm_sets ; dout: last_beta, W, beta_next
+void oracle_stats(void* h, int64_t* out, double* dout) {
+    Plan* P = (Plan*)h;
+    out[0] = P->k; out[1] = P->s; out[2] = P->trials; out[3] = P->n_sets; out[4] = P->n_zero_norm_sets;
+    dout[0] = P->last_beta; dout[1] = P->W; dout[2] = P->beta_next;
+}
+
+void oracle_norms(void* h, double* nD, double* nL, double* nT) {
+    Plan* P = (Plan*)h;
+    std::memcpy(nD, P->nD.data(), P->nD.size() * sizeof(double));
+    std::memcpy(nL, P->nL.data(), P->nL.size() * sizeof(double));
+    std::memcpy(nT, P->nT.data(), P->nT.size() * sizeof(double));
+}
+
+void oracle_what(void* h, double* what) { Plan* P = (Plan*)h; std::memcpy(what, P->what.data(), P->what.size() * sizeof(double)); }
+
+// Fully sequential Fig. 2 sweep exactly as the listing reads (in-place updates voxel by voxel, dose block then
+// cDLET block, then the LETd rows, then the clamp) with per-row relaxation lambda * weight_s (un-normalised):
+// tiny-case sanity reference only (SURVEY pin 12); NOT the method under test.
+void oracle_sequential_sweep(void* h, float lambda_f) {
+    Plan* P = (Plan*)h;
+    const double lambda = (double)lambda_f;
+    std::vector<double>& x = P->x;
+    for (int pass = 0; pass < 3; ++pass)
+        for (int64_t i = 0; i < P->D.n_rows; ++i) {
+            int32_t s = P->label[i];
+            if (s == 0) continue;
+            const Bounds& b = P->bounds[s - 1];
+            const double w = b.weight < 1.0 ? b.weight : 1.0;
+            if (pass == 0 && has_dose_slab(b) && P->nD[i] > 0) {
+                double r = slab_residual(row_dot(P->D, i, x), b.dose_lo, b.dose_hi);
+                if (r != 0.0) { double c = lambda * w * r / P->nD[i];
+                    for (int64_t p = P->D.ptr[i]; p < P->D.ptr[i + 1]; ++p) x[P->D.col[p]] -= c * P->D.val[p]; }
+            }
+            if (pass == 1 && has_dl_slab(b) && P->nL[i] > 0) {
+                double r = slab_residual(row_dot(P->L, i, x), b.dl_lo, b.dl_hi);
+                if (r != 0.0) { double c = lambda * w * r / P->nL[i];
+                    for (int64_t p = P->L.ptr[i]; p < P->L.ptr[i + 1]; ++p) x[P->L.col[p]] -= c * P->L.val[p]; }
+            }
+            if (pass == 2 && has_letd(b) && P->nT[i] > 0) {
+                double val = letd_row_dot(*P, i, b.letd_max, x, nullptr);
+                if (val > 0.0) { double c = lambda * w * val / P->nT[i];
+                    for (int64_t p = P->L.ptr[i]; p < P->L.ptr[i + 1]; ++p) x[P->L.col[p]] -= c * P->L.val[p];
+                    for (int64_t p = P->D.ptr[i]; p < P->D.ptr[i + 1]; ++p) x[P->D.col[p]] += c * b.letd_max * P->D.val[p]; }
+            }
+        }
+    for (size_t j = 0; j < x.size(); ++j) if (x[j] < 0.0) x[j] = 0.0;
+}
+
+}  // extern "C"

@@ -1,0 +1,177 @@
+"""ctypes wrapper of the fp64 CPU oracle (oracle/fredopt_oracle.cpp) -- TEST INFRASTRUCTURE.
+
+Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference leg may import
+this.  It imports nothing from the CUDA package.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+import subprocess
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, "fredopt_oracle.cpp")
+_LIB = os.path.join(_HERE, "libfredopt_oracle.so")
+
+OPT_ETA, OPT_REDUCTIONS, OPT_ACCEPT_CHECK, OPT_MAX_TRIALS, OPT_RESET = 0, 1, 2, 3, 4
+
+
+def build(force: bool = False) -> str:
+    """Compile the oracle with plain g++ -O2 (no OpenMP, no fast-math)."""
+    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
+        subprocess.check_call(["g++", "-O2", "-std=c++17", "-fPIC", "-shared", "-ffp-contract=off",
+                               "-o", _LIB, _SRC])
+    return _LIB
+
+
+_lib = None
+
+
+def _load():
+    global _lib
+    if _lib is None:
+        lib = C.CDLL(build())
+        vp, i64, i32, f32, f64 = C.c_void_p, C.c_int64, C.c_int32, C.c_float, C.c_double
+        lib.oracle_create.restype = vp
+        lib.oracle_create.argtypes = [i64, i64, vp, vp, vp, vp, vp, vp, vp, vp, i32]
+        lib.oracle_destroy.argtypes = [vp]
+        lib.oracle_set_x.argtypes = [vp, vp]
+        lib.oracle_set_x64.argtypes = [vp, vp]
+        lib.oracle_get_x.argtypes = [vp, vp]
+        lib.oracle_set_option.argtypes = [vp, i32, f64]
+        lib.oracle_dose_let.argtypes = [vp, vp, vp, vp, vp]
+        lib.oracle_dose_let_rows.argtypes = [vp, vp, vp, i64, vp, vp, vp]
+        lib.oracle_transpose.argtypes = [vp, vp, vp, i32, vp, vp]
+        lib.oracle_cost.restype = f64
+        lib.oracle_cost.argtypes = [vp, vp]
+        lib.oracle_grad.argtypes = [vp, vp, vp]
+        lib.oracle_proximity.argtypes = [vp, vp, vp, vp]
+        lib.oracle_iterate.argtypes = [vp, i32, f32, f32, f32]
+        lib.oracle_stats.argtypes = [vp, vp, vp]
+        lib.oracle_norms.argtypes = [vp, vp, vp, vp]
+        lib.oracle_what.argtypes = [vp, vp]
+        lib.oracle_sequential_sweep.argtypes = [vp, f32]
+        _lib = lib
+    return _lib
+
+
+def _p(a):
+    return None if a is None else a.ctypes.data_as(C.c_void_p)
+
+
+class Oracle:
+    """fp64 CPU restatement of the hot path.  Inputs are numpy arrays (fp32 values, int32 cols, int64 ptrs)."""
+
+    def __init__(self, D, L, labels, bounds):
+        lib = _load()
+        rpD, ciD, vD = D
+        rpL, ciL, vL = L
+        self.V = len(rpD) - 1
+        self.n_struct = int(np.asarray(bounds).shape[0])
+        self._keep = [np.ascontiguousarray(rpD, np.int64), np.ascontiguousarray(ciD, np.int32),
+                      np.ascontiguousarray(vD, np.float32), np.ascontiguousarray(rpL, np.int64),
+                      np.ascontiguousarray(ciL, np.int32), np.ascontiguousarray(vL, np.float32),
+                      np.ascontiguousarray(labels, np.int32), np.ascontiguousarray(bounds, np.float32)]
+        self._lib = lib
+
+    @classmethod
+    def create(cls, V, S, D, L, labels, bounds):
+        self = cls(D, L, labels, bounds)
+        self.V, self.S = int(V), int(S)
+        k = self._keep
+        assert len(k[0]) == V + 1 and len(k[3]) == V + 1 and len(k[6]) == V
+        self._h = self._lib.oracle_create(V, S, _p(k[0]), _p(k[1]), _p(k[2]), _p(k[3]), _p(k[4]), _p(k[5]),
+                                          _p(k[6]), _p(k[7]), self.n_struct)
+        self._keep = None   # the oracle copied everything
+        return self
+
+    def __del__(self):
+        h = getattr(self, "_h", None)
+        if h:
+            self._lib.oracle_destroy(h)
+            self._h = None
+
+    # ---- state
+    def set_x(self, x):
+        x = np.ascontiguousarray(x)
+        if x.dtype == np.float32:
+            self._lib.oracle_set_x(self._h, _p(x))
+        else:
+            x = np.ascontiguousarray(x, np.float64)
+            self._lib.oracle_set_x64(self._h, _p(x))
+
+    def get_x(self):
+        x = np.empty(self.S, np.float64)
+        self._lib.oracle_get_x(self._h, _p(x))
+        return x
+
+    def set_option(self, key, value):
+        self._lib.oracle_set_option(self._h, key, float(value))
+
+    # ---- the calls of the boundary
+    def dose_let(self, x=None):
+        d = np.empty(self.V, np.float64); l = np.empty(self.V, np.float64); t = np.empty(self.V, np.float64)
+        xx = None if x is None else np.ascontiguousarray(x, np.float64)
+        self._lib.oracle_dose_let(self._h, _p(xx), _p(d), _p(l), _p(t))
+        return d, l, t
+
+    def dose_let_rows(self, rows, x=None):
+        rows = np.ascontiguousarray(rows, np.int64)
+        n = len(rows)
+        d = np.empty(n, np.float64); l = np.empty(n, np.float64); t = np.empty(n, np.float64)
+        xx = None if x is None else np.ascontiguousarray(x, np.float64)
+        self._lib.oracle_dose_let_rows(self._h, _p(xx), _p(rows), n, _p(d), _p(l), _p(t))
+        return d, l, t
+
+    def transpose(self, u, v, active_only=False):
+        uu = None if u is None else np.ascontiguousarray(u, np.float64)
+        vv = None if v is None else np.ascontiguousarray(v, np.float64)
+        out = np.empty(self.S, np.float64); oa = np.empty(self.S, np.float64)
+        self._lib.oracle_transpose(self._h, _p(uu), _p(vv), int(active_only), _p(out), _p(oa))
+        return out, oa
+
+    def cost(self, x=None):
+        xx = None if x is None else np.ascontiguousarray(x, np.float64)
+        return float(self._lib.oracle_cost(self._h, _p(xx)))
+
+    def grad(self, x=None):
+        xx = None if x is None else np.ascontiguousarray(x, np.float64)
+        g = np.empty(self.S, np.float64)
+        self._lib.oracle_grad(self._h, _p(xx), _p(g))
+        return g
+
+    def proximity(self, x=None):
+        xx = None if x is None else np.ascontiguousarray(x, np.float64)
+        pr = C.c_double(0.0); nv = C.c_int64(0)
+        self._lib.oracle_proximity(self._h, _p(xx), C.byref(pr), C.byref(nv))
+        return pr.value, nv.value
+
+    def iterate(self, n_iter, lam, beta0, a):
+        self._lib.oracle_iterate(self._h, int(n_iter), float(lam), float(beta0), float(a))
+
+    def stats(self):
+        o = np.zeros(5, np.int64); d = np.zeros(3, np.float64)
+        self._lib.oracle_stats(self._h, _p(o), _p(d))
+        return dict(k=int(o[0]), s=int(o[1]), trials=int(o[2]), n_sets=int(o[3]), n_zero_norm_sets=int(o[4]),
+                    last_beta=float(d[0]), W=float(d[1]), beta_next=float(d[2]))
+
+    def norms(self):
+        a = np.empty(self.V, np.float64); b = np.empty(self.V, np.float64); c = np.empty(self.V, np.float64)
+        self._lib.oracle_norms(self._h, _p(a), _p(b), _p(c))
+        return a, b, c
+
+    def what(self):
+        w = np.empty(self.n_struct, np.float64)
+        self._lib.oracle_what(self._h, _p(w))
+        return w
+
+    def sequential_sweep(self, lam):
+        self._lib.oracle_sequential_sweep(self._h, float(lam))
+
+
+def from_plan(plan) -> "Oracle":
+    """Oracle over a plangen.Plan (tensors are copied to host numpy)."""
+    rp, ci, vd, vl, lab = plan.to_numpy()
+    return Oracle.create(plan.n_rows, plan.n_cols, (rp, ci, vd), (rp, ci, vl), lab, plan.bounds)

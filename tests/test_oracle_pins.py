@@ -1,0 +1,482 @@
+"""Pins of the fp64 oracle against what the paper and the mathematics fix (CPU only).
+
+The paper prints no worked numbers for an iteration, so the oracle is pinned by
+dense brute force, closed forms, invariants and reductions to textbook/library routines (SURVEY.md
+sec. 8c pins 1-12).  Each test names the part of oracle/fredopt_oracle.cpp a plausible mistake in
+which would make it fail.
+"""
+import os
+
+import numpy as np
+import pytest
+
+from oracle import oracle as orc
+from paper_2509_20012_b200 import plangen as pg
+
+NAN = np.nan
+F32 = np.float32
+
+
+# ----------------------------------------------------------------------------- helpers
+def dense_to_csr(M):
+    V, _ = M.shape
+    rp = np.zeros(V + 1, np.int64)
+    ci, vv = [], []
+    for i in range(V):
+        js = np.nonzero(M[i])[0]
+        rp[i + 1] = rp[i] + len(js)
+        ci.append(js.astype(np.int32))
+        vv.append(M[i, js].astype(F32))
+    return rp, np.concatenate(ci) if len(ci) else np.zeros(0, np.int32), \
+        np.concatenate(vv) if len(vv) else np.zeros(0, F32)
+
+
+def csr_to_dense(csr, S):
+    rp, ci, vv = csr
+    M = np.zeros((len(rp) - 1, S))
+    for i in range(len(rp) - 1):
+        M[i, ci[rp[i]:rp[i + 1]]] = vv[rp[i]:rp[i + 1]].astype(np.float64)
+    return M
+
+
+def bounds_rows(*rows):
+    """rows: dicts with keys of plangen.Bounds."""
+    return np.array([pg.Bounds(**r).as_row() for r in rows], dtype=F32)
+
+
+class DenseReference:
+    """Dense restatement of SURVEY.md sec. 8c, written separately from the oracle (numpy mat-vecs)."""
+
+    def __init__(self, Dd, Ld, labels, bounds):
+        self.D, self.L, self.lab = Dd, Ld, labels
+        self.b = np.asarray(bounds, dtype=F32).astype(np.float64)
+        sets = []   # (row vector a, lo, hi, structure)
+        for i, s in enumerate(labels):
+            if s == 0:
+                continue
+            w, dlo, dhi, llo, lhi, tmax, _, _ = self.b[s - 1]
+            if not (np.isnan(dlo) and np.isnan(dhi)):
+                sets.append((Dd[i], dlo, dhi, s))
+            if not (np.isnan(llo) and np.isnan(lhi)):
+                sets.append((Ld[i], llo, lhi, s))
+            if not np.isnan(tmax):
+                sets.append((Ld[i] - tmax * Dd[i], NAN, 0.0, s))
+        self.sets = sets
+        self.W = sum(self.b[s - 1, 0] for a, lo, hi, s in sets if a @ a > 0)
+        self.what = self.b[:, 0] / self.W if self.W > 0 else self.b[:, 0] * 0
+
+    @staticmethod
+    def resid(val, lo, hi):
+        if not np.isnan(hi) and val > hi:
+            return val - hi
+        if not np.isnan(lo) and val < lo:
+            return val - lo
+        return 0.0
+
+    def proximity(self, x):
+        p, nv = 0.0, 0
+        for a, lo, hi, s in self.sets:
+            r = self.resid(a @ x, lo, hi)
+            nv += r != 0
+            if a @ a > 0:
+                p += 0.5 * self.what[s - 1] * r * r / (a @ a)
+        return p, nv
+
+    def cost(self, x):
+        phi = 0.0
+        d, l = self.D @ x, self.L @ x
+        for i, s in enumerate(self.lab):
+            if s == 0:
+                continue
+            dref, lref = self.b[s - 1, 6], self.b[s - 1, 7]
+            if not np.isnan(dref):
+                phi += self.what[s - 1] * (dref - d[i]) ** 2
+            if not np.isnan(lref):
+                phi += self.what[s - 1] * (lref - l[i]) ** 2
+        return phi
+
+    def grad(self, x):
+        g = np.zeros_like(x)
+        d, l = self.D @ x, self.L @ x
+        for i, s in enumerate(self.lab):
+            if s == 0:
+                continue
+            dref, lref = self.b[s - 1, 6], self.b[s - 1, 7]
+            if not np.isnan(dref):
+                g += 2 * self.what[s - 1] * (d[i] - dref) * self.D[i]
+            if not np.isnan(lref):
+                g += 2 * self.what[s - 1] * (l[i] - lref) * self.L[i]
+        return g
+
+    def iterate(self, x, n, lam, beta0, a, max_trials=200):
+        lam, beta0, a = float(F32(lam)), float(F32(beta0)), float(F32(a))
+        beta = beta0
+        s_count = 0
+        for _ in range(n):
+            if beta0 != 0:
+                phi0, g = self.cost(x), self.grad(x)
+                if np.any(g != 0):
+                    for _t in range(max_trials):
+                        b = beta
+                        beta *= a
+                        s_count += 1
+                        xn = x - b * g
+                        if self.cost(xn) < phi0:
+                            x = xn
+                            break
+            step = np.zeros_like(x)
+            for av, lo, hi, s in self.sets:
+                n2 = av @ av
+                if n2 > 0:
+                    step += self.what[s - 1] * self.resid(av @ x, lo, hi) / n2 * av
+            x = np.maximum(x - lam * step, 0.0)
+        return x, s_count
+
+
+def make_oracle(Dd, Ld, labels, bounds):
+    V, S = Dd.shape
+    return orc.Oracle.create(V, S, dense_to_csr(Dd), dense_to_csr(Ld), np.asarray(labels, np.int32), bounds)
+
+
+def f32mat(M):
+    return M.astype(F32).astype(np.float64)
+
+
+# ----------------------------------------------------------------------------- pin 1: dense brute force
+@pytest.mark.parametrize("seed,same", [(1, True), (2, True), (3, False), (4, False)])
+def test_pin1_dense_brute_force(seed, same):
+    """Whole iteration, CSR traversal, scatter back-projection, union-pattern LETd rows."""
+    D, L, labels, x0 = pg.random_small_plan(seed, V=45, S=9, n_struct=3, same_pattern=same)
+    S = 9
+    Dd, Ld = csr_to_dense(D, S), csr_to_dense(L, S)
+    b = bounds_rows(dict(weight=1.0, dose_lo=1.2, dose_hi=1.6, dose_ref=1.4),
+                    dict(weight=2.5, dose_hi=0.9, dl_hi=4.0, dl_lo=0.5, letd_max=5.0, dl_ref=3.0),
+                    dict(weight=0.5, letd_max=4.0, dose_lo=0.3))
+    o = orc.Oracle.create(45, S, D, L, labels, b)
+    ref = DenseReference(Dd, Ld, labels, b)
+    x0d = x0.astype(np.float64)
+    o.set_x(x0)
+    assert o.stats()["n_sets"] == len(ref.sets)
+    assert np.isclose(o.stats()["W"], ref.W, rtol=1e-14)
+    d, l, t = o.dose_let()
+    np.testing.assert_allclose(d, Dd @ x0d, rtol=1e-13)
+    np.testing.assert_allclose(l, Ld @ x0d, rtol=1e-13)
+    p, nv = o.proximity()
+    pr, nvr = ref.proximity(x0d)
+    assert nv == nvr and np.isclose(p, pr, rtol=1e-12)
+    assert np.isclose(o.cost(), ref.cost(x0d), rtol=1e-12)
+    np.testing.assert_allclose(o.grad(), ref.grad(x0d), rtol=1e-11, atol=1e-15)
+    for lam, beta0 in [(1.0, 0.0), (1.3, 1.0), (0.7, 0.5)]:
+        o.set_option(orc.OPT_RESET, 1)
+        o.set_x(x0)
+        o.iterate(7, lam, beta0, 0.9)
+        xr, s_ref = ref.iterate(x0d.copy(), 7, lam, beta0, 0.9)
+        np.testing.assert_allclose(o.get_x(), xr, rtol=1e-10, atol=1e-13)
+        assert o.stats()["s"] == s_ref
+        assert o.proximity()[1] == ref.proximity(xr)[1]
+
+
+# ----------------------------------------------------------------------------- pin 2: single half-space
+@pytest.mark.parametrize("side", ["upper", "lower"])
+def test_pin2_single_halfspace_closed_form(side):
+    """Projection formula, sign of the lower branch (reading R2), norms: lambda=1 lands ON the boundary,
+    is idempotent; general lambda: <a,x+> - b = (1 - lambda)(<a,x> - b)."""
+    a = f32mat(np.array([[0.3, 1.1, 0.0, 0.7, 2.0]]))
+    x0 = np.array([1.0, 2.0, 3.0, 0.5, 1.5], F32)
+    val0 = float(a[0] @ x0.astype(np.float64))
+    bnd = F32(val0 - 1.7) if side == "upper" else F32(val0 + 0.9)
+    kw = dict(dose_hi=float(bnd)) if side == "upper" else dict(dose_lo=float(bnd))
+    o = make_oracle(a, a * 3.0, [1], bounds_rows(dict(weight=3.0, **kw)))
+    for lam in (1.0, 0.4, 1.7):
+        o.set_x(x0)
+        o.iterate(1, lam, 0.0, 0.5)
+        x1 = o.get_x()
+        assert np.all(x1 > 0)   # clamp inactive in this construction
+        lhs = a[0] @ x1 - float(bnd)
+        rhs = (1.0 - float(F32(lam))) * (val0 - float(bnd))
+        assert abs(lhs - rhs) <= 1e-13 * max(1.0, abs(val0))
+        if lam == 1.0:
+            assert abs(lhs) < 1e-13
+            # the move is along a (orthogonal projection)
+            dx = x1 - x0.astype(np.float64)
+            assert abs(abs(dx @ a[0]) - np.linalg.norm(dx) * np.linalg.norm(a[0])) < 1e-12
+            o.iterate(1, lam, 0.0, 0.5)
+            assert np.max(np.abs(o.get_x() - x1)) < 1e-14      # idempotent
+            assert o.proximity()[0] < 1e-25
+
+
+def test_pin2b_cdl_and_letd_halfspace():
+    """Same closed form through the cDLET block and the linearised LETd row (a = L - LETmax D)."""
+    Dd = f32mat(np.array([[0.5, 0.2, 0.9, 0.4]]))
+    Ld = f32mat(np.array([[2.5, 2.2, 1.0, 3.1]]))
+    x0 = np.array([1.0, 1.0, 1.0, 1.0], F32)
+    # cDL upper
+    o = make_oracle(Dd, Ld, [1], bounds_rows(dict(dl_hi=5.0)))
+    o.set_x(x0); o.iterate(1, 1.0, 0.0, 0.5)
+    assert abs(Ld[0] @ o.get_x() - 5.0) < 1e-13
+    # LETd: <L - 3 D, x> <= 0
+    o = make_oracle(Dd, Ld, [1], bounds_rows(dict(letd_max=3.0)))
+    o.set_x(x0)
+    a = Ld[0] - 3.0 * Dd[0]
+    assert a @ x0 > 0
+    o.iterate(1, 1.0, 0.0, 0.5)
+    x1 = o.get_x()
+    assert abs(a @ x1) < 1e-13
+    d, l, t = o.dose_let()
+    assert abs(t[0] - 3.0) < 1e-12          # LETd sits exactly at LETmax after the projection
+    assert o.proximity() == (0.0, 0) or o.proximity()[0] < 1e-25
+
+
+# ----------------------------------------------------------------------------- pin 3: diagonal system
+def test_pin3_diagonal_geometric_decay():
+    """w^ normalisation (R3) and multi-iteration bookkeeping: D = I, upper bounds, x0 above them:
+    residual_i(k) = (1 - lambda/S)^k residual_i(0)."""
+    S = 6
+    I = np.eye(S)
+    o = make_oracle(I, 2 * I, [1] * S, bounds_rows(dict(weight=7.0, dose_hi=1.0)))
+    x0 = (2.0 + np.arange(S)).astype(F32)
+    lam = 1.5
+    o.set_x(x0)
+    for k in range(1, 6):
+        o.iterate(1, lam, 0.0, 0.5)
+        np.testing.assert_allclose(o.get_x() - 1.0, (1 - float(F32(lam)) / S) ** k * (x0 - 1.0), rtol=1e-13)
+
+
+# ----------------------------------------------------------------------------- pin 4: Cimmino averaging
+def test_pin4_two_orthogonal_halfspaces_mean_of_projections():
+    Dd = f32mat(np.array([[1.0, 0.0, 0.0], [0.0, 2.0, 0.0]]))
+    o = make_oracle(Dd, Dd, [1, 1], bounds_rows(dict(dose_hi=1.0)))
+    x0 = np.array([3.0, 4.0, 5.0], F32)
+    o.set_x(x0); o.iterate(1, 1.0, 0.0, 0.5)
+    p1 = np.array([1.0, 4.0, 5.0]); p2 = np.array([3.0, 0.5, 5.0])
+    np.testing.assert_allclose(o.get_x(), 0.5 * (p1 + p2), rtol=1e-14)
+
+
+def test_pin4b_copies_of_one_halfspace_equal_that_halfspace():
+    a = f32mat(np.array([[0.3, 1.1, 0.7]]))
+    x0 = np.array([2.0, 2.0, 2.0], F32)
+    o1 = make_oracle(a, a, [1], bounds_rows(dict(dose_hi=1.0)))
+    oM = make_oracle(np.repeat(a, 5, 0), np.repeat(a, 5, 0), [1] * 5, bounds_rows(dict(dose_hi=1.0)))
+    for o in (o1, oM):
+        o.set_x(x0); o.iterate(3, 0.8, 0.0, 0.5)
+    np.testing.assert_allclose(oM.get_x(), o1.get_x(), rtol=1e-14)
+    assert np.isclose(oM.proximity()[0], o1.proximity()[0], rtol=1e-13)
+
+
+# ----------------------------------------------------------------------------- pin 5: monotone proximity
+@pytest.mark.parametrize("lam", [0.5, 1.0, 1.5, 1.9])
+def test_pin5_monotone_proximity_config0(plan0, lam):
+    """Step direction/scale, clamp, proximity definition: beta0 = 0, lambda in (0,2) => p nonincreasing."""
+    o = orc.from_plan(plan0)
+    o.set_x(plan0.x0)
+    prev = o.proximity()[0]
+    for _ in range(25):
+        o.iterate(1, lam, 0.0, 0.99)
+        cur = o.proximity()[0]
+        assert cur <= prev * (1 + 1e-12)
+        prev = cur
+
+
+# ----------------------------------------------------------------------------- pin 6: known feasible point / least squares
+def test_pin6_known_feasible_point_converges():
+    u = pg.uniform01_array(11, 30 * 6 + 6)
+    A = f32mat((u[:180].reshape(30, 6) < 0.6) * (0.2 + u[:180].reshape(30, 6)))
+    A[0, 0] = 0.5     # no empty row 0
+    xs = 0.5 + u[180:186]
+    Lm = f32mat(A * 3.0)
+    d, l = A @ xs, Lm @ xs
+    labels = np.arange(30) % 2 + 1
+    # per-structure scalar bounds that xs satisfies
+    b = bounds_rows(dict(dose_lo=float(F32(d[labels == 1].min() * 0.999)), dose_hi=float(F32(d[labels == 1].max() * 1.001))),
+                    dict(dose_hi=float(F32(d[labels == 2].max() * 1.001)), dl_hi=float(F32(l[labels == 2].max() * 1.001)),
+                         letd_max=3.001))
+    o = make_oracle(A, Lm, labels, b)
+    assert o.proximity(xs) == (0.0, 0)
+    o.set_x((xs * 3 + 1).astype(F32))
+    p0, n0 = o.proximity()
+    assert n0 > 0
+    o.iterate(4000, 1.9, 0.0, 0.5)
+    p1, n1 = o.proximity()
+    assert p1 < 1e-24 * p0 and n1 < n0    # on the feasible set to rounding (sets met on their boundary keep ulp-level residuals)
+
+
+def test_pin6b_equalities_reduce_to_weighted_least_squares():
+    """lo = hi = b with the clamp inactive: Landweber on min sum_k w^ (a_k x - b_k)^2 / n_k  ->  numpy lstsq."""
+    u = pg.uniform01_array(5, 12 * 4 + 12)
+    A = f32mat(0.2 + u[:48].reshape(12, 4))
+    xs = np.array([1.0, 2.0, 1.5, 0.7])
+    # one structure per row so each row has its own (equality) bound; noisy right-hand side
+    rhs = (A @ xs + 0.05 * (u[48:60] - 0.5)).astype(F32)
+    b = bounds_rows(*[dict(weight=1.0 + (i % 3), dose_lo=float(rhs[i]), dose_hi=float(rhs[i])) for i in range(12)])
+    o = make_oracle(A, A, np.arange(12) + 1, b)
+    o.set_x(np.ones(4, F32))
+    o.iterate(60000, 1.9, 0.0, 0.5)
+    w = np.array([1.0 + (i % 3) for i in range(12)])
+    sc = np.sqrt(w / (A * A).sum(1))
+    xl = np.linalg.lstsq(A * sc[:, None], rhs.astype(np.float64) * sc, rcond=None)[0]
+    assert np.all(xl > 0)
+    np.testing.assert_allclose(o.get_x(), xl, rtol=1e-8)
+
+
+# ----------------------------------------------------------------------------- pin 7: cost / gradient / accept loop
+def test_pin7_gradient_and_accept_loop(plan0):
+    o = orc.from_plan(plan0)
+    x = plan0.x0.astype(np.float64) * (1 + 0.3 * (pg.uniform01_array(3, plan0.n_cols) - 0.5))
+    g = o.grad(x)
+    # central differences of Eq. (2) on a few coordinates (phi is quadratic => exact up to rounding)
+    for j in (0, 137, 455, 799):
+        e = np.zeros_like(x); e[j] = 1e-3
+        fd = (o.cost(x + e) - o.cost(x - e)) / 2e-3
+        assert abs(fd - g[j]) <= 1e-8 * max(1.0, abs(g[j]))
+    # phi(x - beta g) = phi - beta |g|^2 + beta^2 c  with  c = sum w^ (Dg)^2 (+ cDL terms)
+    phi0, gg = o.cost(x), g @ g
+    c = (o.cost(x - 1.0 * g) - phi0 + gg)
+    for beta in (0.5, 0.1, 2.0):
+        assert np.isclose(o.cost(x - beta * g), phi0 - beta * gg + beta * beta * c, rtol=1e-10)
+    # every accepted perturbation strictly lowers phi; s grows by the number of trials; sum beta <= beta0/(1-a)
+    o.set_x(x)
+    s_prev, tot_beta = 0, 0.0
+    for _ in range(10):
+        xb = o.get_x(); phib = o.cost(xb)
+        gb = o.grad(xb)
+        o.set_option(orc.OPT_MAX_TRIALS, 200)
+        o.iterate(1, 1.0, 1.0, 0.9)
+        st = o.stats()
+        assert st["s"] > s_prev
+        # the accepted beta is beta0 * a^(s-1) by recursion
+        beta = 1.0
+        for _k in range(st["s"] - 1):
+            beta *= float(F32(0.9))
+        assert st["last_beta"] == beta
+        assert o.cost(xb - beta * gb) < phib
+        # the rejected ones did not lower phi
+        b2 = 1.0
+        for _k in range(s_prev):
+            b2 *= float(F32(0.9))
+        for _k in range(s_prev, st["s"] - 1):
+            assert not (o.cost(xb - b2 * gb) < phib)
+            b2 *= float(F32(0.9))
+        tot_beta += beta
+        s_prev = st["s"]
+    assert tot_beta <= 1.0 / (1 - float(F32(0.9)))
+
+
+# ----------------------------------------------------------------------------- pin 8: control flow / state
+def test_pin8_state_and_control_flow(plan0):
+    a = orc.from_plan(plan0); b = orc.from_plan(plan0); c = orc.from_plan(plan0)
+    for o in (a, b, c):
+        o.set_x(plan0.x0)
+    a.iterate(20, 1.0, 1.0, 0.99)
+    b.iterate(10, 1.0, 1.0, 0.99); b.iterate(10, 1.0, 1.0, 0.99)
+    assert np.array_equal(a.get_x(), b.get_x()) and a.stats() == b.stats()
+    # beta0 = 0 => SA == AMS bit for bit, whatever a is; s stays 0
+    c.iterate(5, 1.0, 0.0, 0.5)
+    d = orc.from_plan(plan0); d.set_x(plan0.x0); d.iterate(5, 1.0, 0.0, 0.99)
+    assert np.array_equal(c.get_x(), d.get_x()) and c.stats()["s"] == 0
+    # accept_check = 0 => unconditional beta0 a^k steps, s == k
+    e = orc.from_plan(plan0); e.set_x(plan0.x0); e.set_option(orc.OPT_ACCEPT_CHECK, 0); e.iterate(7, 1.0, 0.3, 0.9)
+    assert e.stats()["s"] == 7 and e.stats()["k"] == 7
+
+
+# ----------------------------------------------------------------------------- pin 9: exact row scaling, permutations
+def test_pin9_row_scaling_and_permutation_invariance():
+    D, L, labels, x0 = pg.random_small_plan(21, V=36, S=7, n_struct=2)
+    S = 7
+    Dd, Ld = csr_to_dense(D, S), csr_to_dense(L, S)
+    labels = np.where(labels == 0, 0, labels)
+    b1 = bounds_rows(dict(dose_lo=1.0, dose_hi=1.5), dict(dose_hi=0.75))
+    o1 = make_oracle(Dd, Ld, labels, b1)
+    # scale every row of D by 2 (exact in binary) and the dose bounds by 2: iterates bit-identical
+    b2 = bounds_rows(dict(dose_lo=2.0, dose_hi=3.0), dict(dose_hi=1.5))
+    o2 = make_oracle(2 * Dd, Ld, labels, b2)
+    for o in (o1, o2):
+        o.set_x(x0); o.iterate(6, 1.2, 0.0, 0.5)
+    assert np.array_equal(o1.get_x(), o2.get_x())
+    # voxel permutation / spot permutation: same result up to summation order
+    pv = np.argsort(pg.uniform01_array(8, 36)); ps = np.argsort(pg.uniform01_array(9, S))
+    o3 = make_oracle(Dd[pv][:, ps], Ld[pv][:, ps], labels[pv], b1)
+    o3.set_x(x0[ps]); o3.iterate(6, 1.2, 0.0, 0.5)
+    np.testing.assert_allclose(o3.get_x(), o1.get_x()[ps], rtol=1e-12, atol=1e-15)
+
+
+# ----------------------------------------------------------------------------- pin 10: transpose identity
+def test_pin10_transpose_identity(plan0):
+    o = orc.from_plan(plan0)
+    x = pg.uniform01_array(5, plan0.n_cols)
+    r = pg.uniform01_array(6, plan0.n_rows) - 0.5
+    q = pg.uniform01_array(7, plan0.n_rows) - 0.5
+    d, l, _ = o.dose_let(x)
+    out, oabs = o.transpose(r, q)
+    assert np.isclose(d @ r + l @ q, x @ out, rtol=1e-11)
+    assert np.all(oabs >= np.abs(out) - 1e-12)
+    lab = plan0.labels.numpy()
+    outa, _ = o.transpose(r, None, active_only=True)
+    assert np.isclose(d[lab != 0] @ r[lab != 0], x @ outa, rtol=1e-11)
+
+
+# ----------------------------------------------------------------------------- pin 11: analytic LETd, generator
+def test_pin11_analytic_letd_single_spot(plan0):
+    """x = e_j => LETd_i = L_ij/D_ij = 2 + 10 exp(-max(R_j - z_i, 0)/5 mm) on every voxel the spot touches;
+    uniform x0 => mean PTV dose = 2 Gy.  (Pins dose_let and the generator's depth convention.)"""
+    o = orc.from_plan(plan0)
+    nx, ny, nz = plan0.spec.grid
+    h = plan0.spec.h
+    for j in (0, 417, 799):
+        x = np.zeros(plan0.n_cols); x[j] = 1.0
+        d, l, t = o.dose_let(x)
+        rows = np.nonzero(d > 0)[0]
+        assert len(rows) > 500
+        z = ((rows // (nx * ny)) + 0.5) * h               # beam along +z entering at z = 0
+        R = plan0.spot_range[j]
+        np.testing.assert_allclose(t[rows], 2 + 10 * np.exp(-np.maximum(R - z, 0) / 5.0), rtol=3e-7)   # fp32 storage
+        assert np.all(t[d == 0] == 0)
+    d, _, _ = o.dose_let(plan0.x0.astype(np.float64))
+    lab = plan0.labels.numpy()
+    assert abs(d[lab == 1].mean() - 2.0) < 1e-6
+
+
+# ----------------------------------------------------------------------------- pin 12: sequential Fig. 2 sweep
+def test_pin12_sequential_sweep_reaches_feasible_point_of_same_system():
+    u = pg.uniform01_array(31, 24 * 5 + 5)
+    A = f32mat(0.1 + u[:120].reshape(24, 5))
+    xs = 0.5 + u[120:125]
+    d = A @ xs
+    labels = np.arange(24) % 2 + 1
+    b = bounds_rows(dict(dose_lo=float(F32(d[labels == 1].min() * 0.99)), dose_hi=float(F32(d[labels == 1].max() * 1.01))),
+                    dict(dose_hi=float(F32(d[labels == 2].max() * 1.01)), dl_hi=float(F32(2 * d[labels == 2].max() * 1.01))))
+    o = make_oracle(A, 2 * A, labels, b)
+    o.set_x((xs * 2).astype(F32))
+    assert o.proximity()[1] > 0
+    for _ in range(300):
+        o.sequential_sweep(1.0)
+    assert o.proximity()[1] == 0
+
+
+# ----------------------------------------------------------------------------- external fixture (SURVEY probe)
+def test_config0_matches_survey_probe_trajectory(plan0):
+    path = os.path.join(os.path.dirname(__file__), "golden", "config0_trajectory.txt")
+    gold = {}
+    for line in open(path):
+        if line.startswith("#") or not line.strip():
+            continue
+        k, v = line.split()
+        gold[k] = float(v)
+    o = orc.from_plan(plan0)
+    st = o.stats()
+    assert st["n_sets"] == gold["n_sets"] and st["n_sets"] - st["n_zero_norm_sets"] == gold["n_participating"]
+    assert np.isclose(plan0.x0[0], gold["x0"], rtol=2e-7)
+    o.set_x(plan0.x0)
+    assert np.isclose(o.cost(), gold["phi0"], rtol=2e-6)
+    assert np.isclose(np.linalg.norm(o.grad()), gold["gnorm0"], rtol=2e-6)
+    p, nv = o.proximity()
+    assert np.isclose(p, gold["prox0"], rtol=2e-6) and nv == gold["viol0"]
+    for tag, beta0 in (("sa", 1.0), ("ams", 0.0)):
+        o = orc.from_plan(plan0); o.set_x(plan0.x0)
+        done = 0
+        for n in (1, 10, 20, 50):
+            o.iterate(n - done, 1.0, beta0, 0.99); done = n
+            p, nv = o.proximity()
+            assert np.isclose(p, gold[f"{tag}_prox_{n}"], rtol=2e-6), (tag, n, p)
+            assert nv == gold[f"{tag}_viol_{n}"], (tag, n, nv)
+        if tag == "sa":
+            assert o.stats()["s"] == 50       # single beam: no rejections
