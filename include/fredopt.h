@@ -1,0 +1,176 @@
+/* fredopt.h -- C-ABI of the B200-native (sm_100a) hot path of FREDopt's plan optimisation.
+ *
+ * The library implements ONE thing: the superiorized, simultaneous (Cimmino-type) feasibility-seeking
+ * iteration over the sparse spot->voxel influence matrices D (dose) and L (LET-weighted dose) of
+ * "GPU-accelerated FREDopt package for simultaneous dose and LETd proton radiotherapy plan optimization via
+ * superiorization methods" (arxiv 2509.20012; cited below as PAPER.md:<line>), i.e.
+ *
+ *   AMSrelaxDLET  (Fig. 2)  relaxed projections onto per-voxel dose / cDL half-spaces,
+ *                                             then the clamp fluence_j < 0 -> 0;
+ *   SuperiorDLET  (Fig. 3)  perturbations x' = x - beta * grad chi^2(x), beta = beta0*a^s,
+ *                                             accepted iff chi^2 decreases, interleaved with AMS steps;
+ *   chi^2         (Eq. 2,  PAPER.md:207)      sum_PTV w (Dref - D(x))^2 + sum_OAR w (cDLref - cDL(x))^2;
+ *   LETd = l / d  (Eq. 1,  PAPER.md:56-64)    with the dose as denominator;
+ *   plus the OAR LETd limit linearised as <L_i - LETmax * D_i, x> <= 0, the proximity function and the
+ *   violation count (BASELINE.json north_star; not in the paper).
+ *
+ * The readings of the paper that fix every detail (simultaneous form, sign of the lower-bound branch, weight
+ * normalisation, ...) are listed in DESIGN.md, "Readings of the paper".
+ *
+ * Conventions
+ *   - rows = voxels (V = n_rows), columns = spots (S = n_cols); x in R^S is the spot-weight ("fluence") vector.
+ *   - every pointer argument may be a HOST or a DEVICE pointer (detected with cudaPointerGetAttributes) unless
+ *     stated otherwise; caller arrays are BORROWED for the duration of the call only; outputs are
+ *     caller-allocated.  fredopt_create copies what it needs: inputs may be freed on return.
+ *   - one plan = one GPU, one CUDA stream (given at creation; NULL = the legacy default stream).  Calls enqueue
+ *     on that stream; a call that writes host memory synchronises the stream before returning, a call with
+ *     device outputs only does not.
+ *   - arithmetic: matrix values are stored as given (fp32), indices int32, offsets int64; every vector the
+ *     iteration keeps (x, d, l, g, u, v) and every accumulator / scalar / decision is fp64 on the device.
+ *     fp32 scalars cross the ABI as their bit patterns and are widened, never recomputed.
+ *   - every function returns FREDOPT_OK (0) or a negative error code; no exception or abort crosses the ABI;
+ *     on failure outputs and plan state are untouched (fredopt_create: *out = NULL).
+ *   - requires a device of compute capability 10.x (built for sm_100a only): FREDOPT_UNSUPPORTED_ARCH otherwise.
+ *     There is no CPU fallback.
+ */
+#ifndef FREDOPT_H
+#define FREDOPT_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define FREDOPT_OK                 0
+#define FREDOPT_INVALID_ARG       -1
+#define FREDOPT_OUT_OF_MEMORY     -2
+#define FREDOPT_CUDA_ERROR        -3
+#define FREDOPT_UNSUPPORTED_ARCH  -4
+#define FREDOPT_UNSUPPORTED       -5
+
+typedef struct fredopt_plan fredopt_plan;   /* opaque */
+
+/* Compressed sparse rows.  row_ptr: n_rows+1 entries, non-decreasing, row_ptr[0] = 0, row_ptr[n_rows] = nnz.
+ * col_idx / values: nnz entries; within a row the columns are strictly increasing and < n_cols; values finite. */
+typedef struct {
+    int64_t n_rows, n_cols, nnz;
+    const int64_t *row_ptr;
+    const int32_t *col_idx;
+    const float   *values;
+} fredopt_csr;
+
+/* Bounds of one structure (label s = 1..n_struct uses bounds[s-1]); NaN = absent.
+ * Inputs of Figs. 2-3: U_D, L_D, U_cDLET, L_cDLET, w; Dref, cDLref of Eq. (2). */
+typedef struct {
+    float weight;               /* w_s > 0: weight / priority of the structure              */
+    float dose_lo, dose_hi;     /* L_D <= <D_i, x> <= U_D                                                  */
+    float dl_lo, dl_hi;         /* L_cDLET <= <L_i, x> <= U_cDLET                                          */
+    float letd_max;             /* <L_i - letd_max * D_i, x> <= 0      (north_star)                        */
+    float dose_ref, dl_ref;     /* Dref, cDLref of Eq. (2): cost terms w (ref - value)^2                   */
+} fredopt_bounds;
+
+/* Filled by fredopt_get_stats (synchronises). */
+typedef struct {
+    int64_t k;                  /* iterations done (Fig. 3's k)                                            */
+    int64_t s;                  /* step-size exponent consumed so far (Fig. 3's s + 1)                     */
+    int64_t trials;             /* perturbation trials evaluated so far (= s)                              */
+    int64_t n_violated;         /* declared sets with a non-zero residual at the point the last AMS step   */
+                                /*   of fredopt_iterate was taken from, or at the last fredopt_proximity   */
+    int64_t n_sets;             /* declared constraint sets                                                */
+    int64_t n_zero_norm_sets;   /* declared sets whose row has zero norm (take no part in the step)        */
+    int64_t n_active_rows;      /* voxels with label != 0                                                  */
+    int64_t nnz;                /* non-zeros per matrix (union pattern)                                    */
+    int64_t nnz_active;         /* non-zeros in active rows                                                */
+    int64_t alg_bytes_iter;     /* algorithmic bytes of ONE superiorized iteration ("Bytes")    */
+    double  last_beta;          /* last accepted beta (0 if none)                                          */
+    double  phi;                /* chi^2 at the perturbed point of the last iteration                      */
+    double  prox;               /* proximity 1/2 sum w^ r^2/|a|^2 at that same point / last proximity call */
+    double  weight_sum;         /* W: sum of the weights of the participating sets                         */
+} fredopt_stats;
+
+/* Options (fredopt_set_option). */
+#define FREDOPT_OPT_ETA            0   /* eta of Fig. 3: lambda_k = lambda * eta^k; default 1      */
+#define FREDOPT_OPT_REDUCTIONS     1   /* reductionsN of Fig. 3; default 1                         */
+#define FREDOPT_OPT_ACCEPT_CHECK   2   /* 1 (default): accept a perturbation iff chi^2 decreases; 0: always      */
+#define FREDOPT_OPT_MAX_TRIALS     3   /* cap of the `while loop` of Fig. 3 per reduction; default 200            */
+#define FREDOPT_OPT_RESET          4   /* any value: k = s = 0, beta restarts at beta0                            */
+#define FREDOPT_OPT_USE_GRAPH      5   /* 1 (default): replay one captured iteration as a CUDA graph; 0: launch   */
+#define FREDOPT_OPT_TIME_PASSES    6   /* 1: bracket every kernel of fredopt_iterate with CUDA events (implies no */
+                                       /*    graph); read with fredopt_get_pass_times; default 0                  */
+
+/* Row selectors of the per-pass exports. */
+#define FREDOPT_ROWS_ALL     0
+#define FREDOPT_ROWS_ACTIVE  1
+
+/* Pass indices of fredopt_get_pass_times / fredopt_get_pass_bytes. */
+#define FREDOPT_PASS_FORWARD_X   0   /* d = D x, l = L x on active rows     */
+#define FREDOPT_PASS_TRANSPOSE_G 1   /* g = 2 (D^T p + L^T q)                                 (a3)            */
+#define FREDOPT_PASS_FORWARD_G   2   /* D g, L g: the perturbed values and the accept test    (a5, a6)        */
+#define FREDOPT_PASS_SELECT      3   /* beta selection + x' = x - beta g (scalar kernel)      (a4, a6)        */
+#define FREDOPT_PASS_RESIDUAL    4   /* residuals / violations / u, v                         (a7)            */
+#define FREDOPT_PASS_TRANSPOSE_B 5   /* back-projection + update + clamp                      (a8, a9)        */
+#define FREDOPT_N_PASSES         6
+
+/* Build a plan.  D, L: same n_rows, n_cols (patterns may differ; the union is used).  voxel_labels: n_rows
+ * entries in 0..n_struct, 0 = unconstrained.  bounds: n_struct entries (HOST pointer).  cuda_stream: a
+ * cudaStream_t (or NULL).  The plan's x starts at 0: call fredopt_set_weights.
+ * Errors: INVALID_ARG (null pointer, shape mismatch, bad row_ptr, unsorted / duplicate / out-of-range column,
+ * non-finite value, label outside 0..n_struct, weight <= 0 or non-finite, lo > hi, nnz >= 2^32),
+ * OUT_OF_MEMORY, CUDA_ERROR, UNSUPPORTED_ARCH. */
+int fredopt_create(const fredopt_csr *D, const fredopt_csr *L, const int32_t *voxel_labels,
+                   const fredopt_bounds *bounds, int32_t n_struct, void *cuda_stream, fredopt_plan **out);
+void fredopt_destroy(fredopt_plan *plan);
+
+/* Spot weights x (n_cols floats).  set: widened to fp64; get: the plan's fp64 x rounded to fp32.
+ * fredopt_get_weights_f64 returns the fp64 state itself (n_cols doubles). */
+int fredopt_set_weights(fredopt_plan *plan, const float *x);
+int fredopt_get_weights(fredopt_plan *plan, float *x);
+int fredopt_get_weights_f64(fredopt_plan *plan, double *x);
+
+/* dose = D x, LETd_i = (L x)_i / (D x)_i (0 where dose_i = 0) over ALL n_rows voxels (Eq. 1).
+ * x: n_cols floats or NULL = the plan's x.  dose, letd: n_rows floats each; either may be NULL. */
+int fredopt_dose_let(fredopt_plan *plan, const float *x, float *dose, float *letd);
+
+/* n_iter iterations of SuperiorDLET (Fig. 3) around the simultaneous AMSrelaxDLET step (Fig. 2), from the plan's
+ * x; advances the plan's x, k, s.  lambda in (0, 2]; beta0 >= 0 (0 = pure feasibility-seeking,
+ * the paper's "AMS" runs); a in (0, 1).  beta_s = beta0 * a^s by repeated multiplication in fp64;
+ * beta0 and a are latched at the first call after create / RESET.  Asynchronous (device work only). */
+int fredopt_iterate(fredopt_plan *plan, int32_t n_iter, float lambda, float beta0, float a);
+
+/* Proximity p(x) = 1/2 sum_{k in P} w^_k r_k^2 / |a_k|^2 and the number of declared sets with r_k != 0.
+ * x: n_cols floats or NULL = the plan's x.  prox, n_violated: HOST pointers.  Synchronises. */
+int fredopt_proximity(fredopt_plan *plan, const float *x, double *prox, int64_t *n_violated);
+
+int fredopt_set_option(fredopt_plan *plan, int32_t key, double value);
+int fredopt_get_stats(fredopt_plan *plan, fredopt_stats *out);
+
+/* ---- per-pass exports: per-SpMV parity tests and the isolated-pass sweep (BASELINE.json configs[4]) ----
+ * forward:   d = D x, l = L x over the selected rows; d, l: n_rows floats, voxel-indexed (rows outside the
+ *            selection are written as 0); either may be NULL (that matrix's values are then not read).
+ * transpose: out = D^T u + L^T v over the selected rows; u, v: n_rows floats, voxel-indexed; either may be NULL;
+ *            out: n_cols floats.  ROWS_ALL builds a transposed copy of the whole matrix on first use. */
+int fredopt_spmv_forward(fredopt_plan *plan, int32_t rows, const float *x, float *d, float *l);
+int fredopt_spmv_transpose(fredopt_plan *plan, int32_t rows, const float *u, const float *v, float *out);
+
+/* Accumulated device time [ms] and launch count of each pass of fredopt_iterate since TIME_PASSES was set to 1
+ * (ms, launches: FREDOPT_N_PASSES entries each, HOST pointers).  Synchronises. */
+int fredopt_get_pass_times(fredopt_plan *plan, double *ms, int64_t *launches);
+/* Algorithmic bytes of ONE launch of each pass ("Bytes"): FREDOPT_N_PASSES entries, HOST pointer. */
+int fredopt_get_pass_bytes(fredopt_plan *plan, int64_t *bytes);
+
+/* Number of kernels this library has launched on behalf of `plan` since creation. */
+int64_t fredopt_launch_count(fredopt_plan *plan);
+
+/* Read-only streaming-sum kernel over `bytes` bytes of device memory (multiple of 16): the practical ceiling of
+ * a 100%-read pass on this GPU.  Enqueues `reps` launches on the plan's stream; asynchronous. */
+int fredopt_stream_read(fredopt_plan *plan, const void *device_buf, int64_t bytes, int32_t reps);
+
+const char *fredopt_strerror(int code);
+/* Text of the last CUDA error seen by this thread inside the library ("" if none). */
+const char *fredopt_last_cuda_error(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* FREDOPT_H */

@@ -1,0 +1,1076 @@
+// fredopt_api.cu -- C-ABI (include/fredopt.h), create-time plan builder and pass orchestration.
+// The hot kernels are in fredopt_kernels.cuh.  Nothing here touches the CPU oracle; there is no CPU fallback.
+#include "../../include/fredopt.h"
+#include "fredopt_kernels.cuh"
+
+#include <cub/cub.cuh>
+
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <string>
+#include <vector>
+
+using namespace fredopt;
+
+// ============================================================================================ errors
+static thread_local std::string g_last_cuda_error;
+
+#define CK(expr)                                                                                   \
+    do {                                                                                           \
+        cudaError_t e__ = (expr);                                                                  \
+        if (e__ != cudaSuccess) {                                                                  \
+            g_last_cuda_error = std::string(#expr) + ": " + cudaGetErrorString(e__);               \
+            cudaGetLastError();                                                                    \
+            return e__ == cudaErrorMemoryAllocation ? FREDOPT_OUT_OF_MEMORY : FREDOPT_CUDA_ERROR;  \
+        }                                                                                          \
+    } while (0)
+#define CKR(expr)                         \
+    do {                                  \
+        int r__ = (expr);                 \
+        if (r__ != FREDOPT_OK) return r__; \
+    } while (0)
+
+// ============================================================================================ plan
+struct RowSet {
+    long long n = 0;                 // rows
+    int n_seg = 1;
+    int32_t* vox = nullptr;          // [n]
+    int32_t* seg = nullptr;          // [n] or nullptr
+    long long* start = nullptr;      // [n]
+    int32_t* len = nullptr;          // [n] padded
+    int32_t* ulen = nullptr;         // [n] unpadded
+    long long nnz = 0;               // unpadded entries in the set
+    // CSR of the transposes restricted to this set: rows = spots, per-segment runs, columns = list index
+    bool t_built = false;
+    long long* t_ptr = nullptr;      // [S*n_seg + 1]
+    int32_t* t_col = nullptr;
+    float* t_valD = nullptr;
+    float* t_valL = nullptr;
+    long long t_nnz_padded = 0;
+    RowList view() const { return RowList{n, start, len, seg, vox}; }
+};
+
+struct EventPair { cudaEvent_t a, b; int pass; };
+
+struct fredopt_plan {
+    cudaStream_t stream = nullptr;
+    int device = 0;
+    long long V = 0, S = 0, nnz = 0, nnz_padded = 0;
+    int n_struct = 0;
+    std::vector<void*> allocs;
+    // padded matrix (union pattern), all non-empty rows
+    int32_t* col = nullptr;
+    float* valD = nullptr;
+    float* valL = nullptr;
+    RowSet full, act;
+    // per active row
+    double *nD = nullptr, *nL = nullptr, *nT = nullptr;
+    // tables
+    StructInfo* tab = nullptr;             // [n_struct]
+    std::vector<StructInfo> h_tab;
+    uint8_t *mode_union = nullptr, *mode_con = nullptr, *mode_cost = nullptr, *mode_fixed = nullptr;  // mode_fixed: [4][max_seg]
+    int max_seg = 1;
+    SegCoef *coef_cost = nullptr, *coef_unit = nullptr;
+    DevState* st = nullptr;
+    // vectors (fp64)
+    double *x = nullptr, *g = nullptr, *xtmp = nullptr;                       // [S]
+    double *d = nullptr, *l = nullptr, *Dg = nullptr, *Lg = nullptr, *u = nullptr, *v = nullptr;   // [VA]
+    double *fullD = nullptr, *fullL = nullptr;                                 // lazily: [full.n] gather vectors for ROWS_ALL transposes
+    double* cpart = nullptr;
+    double *part_prox = nullptr, *part_phi = nullptr;
+    long long* part_cnt = nullptr;
+    int* sink = nullptr;
+    // options / host state
+    double eta = 1.0;
+    long long reductionsN = 1, max_trials = 200;
+    int accept_check = 1, use_graph = 1, time_passes = 0;
+    bool started = false;
+    float latched_beta0 = 0.f;
+    long long launches = 0;
+    // graphs: [0] = AMS iteration, [1] = SA iteration (for the current reductionsN)
+    cudaGraphExec_t gexec[2] = {nullptr, nullptr};
+    long long gexec_red[2] = {0, 0};
+    int gexec_kernels[2] = {0, 0};
+    // timing
+    std::vector<EventPair> events;
+    double pass_ms[FREDOPT_N_PASSES] = {0};
+    long long pass_launches[FREDOPT_N_PASSES] = {0};
+    long long pass_bytes[FREDOPT_N_PASSES] = {0};
+    int sm_count = 148;
+};
+
+template <class T>
+static int dmalloc(fredopt_plan* P, T** p, size_t n) {
+    *p = nullptr;
+    if (n == 0) n = 1;
+    CK(cudaMalloc((void**)p, n * sizeof(T)));
+    P->allocs.push_back((void*)*p);
+    return FREDOPT_OK;
+}
+static void dfree(fredopt_plan* P, void* p) {
+    if (!p) return;
+    for (size_t i = 0; i < P->allocs.size(); ++i)
+        if (P->allocs[i] == p) { P->allocs[i] = P->allocs.back(); P->allocs.pop_back(); break; }
+    cudaFree(p);
+}
+
+static bool is_device_ptr(const void* p) {
+    cudaPointerAttributes at;
+    if (cudaPointerGetAttributes(&at, p) != cudaSuccess) { cudaGetLastError(); return false; }
+    return at.type == cudaMemoryTypeDevice || at.type == cudaMemoryTypeManaged;
+}
+
+static inline int grid_for(long long n, int threads, int cap) {
+    long long g = (n + threads - 1) / threads;
+    if (g < 1) g = 1;
+    if (g > cap) g = cap;
+    return (int)g;
+}
+
+// ============================================================================================ create-time kernels
+namespace {
+
+__global__ void k_check_ptr(const long long* ptr, long long V, long long nnz, int* bad) {
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i <= V; i += (long long)gridDim.x * blockDim.x) {
+        const long long a = ptr[i];
+        if (a < 0 || a > nnz) *bad = 1;
+        if (i == 0 && a != 0) *bad = 1;
+        if (i == V && a != nnz) *bad = 1;
+        if (i < V && ptr[i + 1] < a) *bad = 1;
+    }
+}
+
+// warp per row: columns strictly increasing and in range, values finite
+__global__ void k_check_rows(const long long* ptr, const int32_t* col, const float* val, long long V, long long S, int* bad) {
+    const int lane = threadIdx.x & 31;
+    const long long w0 = ((long long)blockIdx.x * blockDim.x + threadIdx.x) >> 5, nw = ((long long)gridDim.x * blockDim.x) >> 5;
+    for (long long i = w0; i < V; i += nw) {
+        const long long b = ptr[i], e = ptr[i + 1];
+        for (long long p = b + lane; p < e; p += 32) {
+            const int c = col[p];
+            if (c < 0 || c >= S) *bad = 2;
+            if (p > b && col[p - 1] >= c) *bad = 2;
+            if (!isfinite(val[p])) *bad = 3;
+        }
+    }
+}
+
+__global__ void k_check_labels(const int32_t* lab, long long V, int n_struct, int* bad) {
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < V; i += (long long)gridDim.x * blockDim.x)
+        if (lab[i] < 0 || lab[i] > n_struct) *bad = 4;
+}
+
+__global__ void k_cmp_i64(const long long* a, const long long* b, long long n, int* diff) {
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (long long)gridDim.x * blockDim.x)
+        if (a[i] != b[i]) *diff = 1;
+}
+__global__ void k_cmp_i32(const int32_t* a, const int32_t* b, long long n, int* diff) {
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (long long)gridDim.x * blockDim.x)
+        if (a[i] != b[i]) *diff = 1;
+}
+
+// union pattern of two sorted rows: count, then fill (thread per row; rare path)
+__global__ void k_union_count(const long long* pD, const int32_t* cD, const long long* pL, const int32_t* cL, long long V,
+                              long long* cnt) {
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < V; i += (long long)gridDim.x * blockDim.x) {
+        long long p = pD[i], pe = pD[i + 1], q = pL[i], qe = pL[i + 1], n = 0;
+        while (p < pe || q < qe) {
+            const int a = p < pe ? cD[p] : INT32_MAX, b = q < qe ? cL[q] : INT32_MAX;
+            if (a == b) { ++p; ++q; } else if (a < b) ++p; else ++q;
+            ++n;
+        }
+        cnt[i] = n;
+    }
+}
+__global__ void k_union_fill(const long long* pD, const int32_t* cD, const float* vD, const long long* pL, const int32_t* cL,
+                             const float* vL, long long V, const long long* pU, int32_t* cU, float* uD, float* uL) {
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < V; i += (long long)gridDim.x * blockDim.x) {
+        long long p = pD[i], pe = pD[i + 1], q = pL[i], qe = pL[i + 1], o = pU[i];
+        while (p < pe || q < qe) {
+            const int a = p < pe ? cD[p] : INT32_MAX, b = q < qe ? cL[q] : INT32_MAX;
+            if (a == b) { cU[o] = a; uD[o] = vD[p]; uL[o] = vL[q]; ++p; ++q; }
+            else if (a < b) { cU[o] = a; uD[o] = vD[p]; uL[o] = 0.f; ++p; }
+            else { cU[o] = b; uD[o] = 0.f; uL[o] = vL[q]; ++q; }
+            ++o;
+        }
+    }
+}
+
+// per voxel: unpadded length, padded length (as int64 for the scan), flags
+__global__ void k_row_lengths(const long long* ptr, const int32_t* lab, long long V, long long* plen64, int32_t* nonempty,
+                              int32_t* active) {
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < V; i += (long long)gridDim.x * blockDim.x) {
+        const long long n = ptr[i + 1] - ptr[i];
+        plen64[i] = (n + 3) & ~3LL;
+        nonempty[i] = n > 0;
+        active[i] = lab[i] != 0;
+    }
+}
+
+// compact the flagged voxels (pos = exclusive scan of flag) into a row list
+__global__ void k_compact_rows(const int32_t* flag, const int32_t* pos, const long long* ptr, const long long* pstart,
+                               const int32_t* lab, long long V, int32_t* vox, long long* start, int32_t* len, int32_t* ulen,
+                               int32_t* key) {
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < V; i += (long long)gridDim.x * blockDim.x) {
+        if (!flag[i]) continue;
+        const int o = pos[i];
+        vox[o] = (int32_t)i;
+        if (start) {
+            const long long n = ptr[i + 1] - ptr[i];
+            start[o] = pstart[i];
+            len[o] = (int32_t)((n + 3) & ~3LL);
+            ulen[o] = (int32_t)n;
+        }
+        if (key) key[o] = lab[i];
+    }
+}
+
+// after sorting the active voxels by label: fill the list from the voxel ids
+__global__ void k_fill_active(const int32_t* vox, const int32_t* lab_sorted, const long long* ptr, const long long* pstart,
+                              long long n, long long* start, int32_t* len, int32_t* ulen, int32_t* seg) {
+    for (long long a = (long long)blockIdx.x * blockDim.x + threadIdx.x; a < n; a += (long long)gridDim.x * blockDim.x) {
+        const long long i = vox[a];
+        const long long m = ptr[i + 1] - ptr[i];
+        start[a] = pstart[i];
+        len[a] = (int32_t)((m + 3) & ~3LL);
+        ulen[a] = (int32_t)m;
+        seg[a] = lab_sorted[a] - 1;
+    }
+}
+
+// copy the rows into the padded arrays (warp per non-empty row); padding stays {col 0, value 0}
+__global__ void k_copy_padded(long long n, const int32_t* vox, const long long* start, const long long* ptr, const int32_t* cU,
+                              const float* uD, const float* uL, int32_t* col, float* vD, float* vL) {
+    const int lane = threadIdx.x & 31;
+    const long long w0 = ((long long)blockIdx.x * blockDim.x + threadIdx.x) >> 5, nw = ((long long)gridDim.x * blockDim.x) >> 5;
+    for (long long r = w0; r < n; r += nw) {
+        const long long i = vox[r], b = ptr[i], e = ptr[i + 1], o = start[r];
+        for (long long p = b + lane; p < e; p += 32) {
+            col[o + (p - b)] = cU[p];
+            vD[o + (p - b)] = uD[p];
+            vL[o + (p - b)] = uL[p];
+        }
+    }
+}
+
+// squared norms of D_i, L_i and L_i - LETmax D_i in fp64 (warp per active row)
+__global__ void k_norms(RowList rl, const int32_t* col, const float* vD, const float* vL, const StructInfo* tab, double* nD,
+                        double* nL, double* nT) {
+    const int lane = threadIdx.x & 31;
+    const long long w0 = ((long long)blockIdx.x * blockDim.x + threadIdx.x) >> 5, nw = ((long long)gridDim.x * blockDim.x) >> 5;
+    for (long long r = w0; r < rl.n; r += nw) {
+        const long long s = rl.start[r];
+        const int L = rl.len[r];
+        const StructInfo& T = tab[rl.seg[r]];
+        const double tm = (T.flags & F_LETD) ? T.letd_max : 0.0;
+        double a = 0.0, b = 0.0, c = 0.0;
+        for (int p = lane; p < L; p += 32) {
+            const double dv = (double)vD[s + p], lv = (double)vL[s + p];
+            a = fma(dv, dv, a);
+            b = fma(lv, lv, b);
+            const double t = lv - tm * dv;
+            c = fma(t, t, c);
+        }
+        a = warp_sum(a); b = warp_sum(b); c = warp_sum(c);
+        if (lane == 0) { nD[r] = a; nL[r] = b; nT[r] = (T.flags & F_LETD) ? c : 0.0; }
+    }
+}
+
+// integer bookkeeping per structure (atomics on integers: order-independent result)
+__global__ void k_count_sets(long long n, const int32_t* seg, const int32_t* ulen, const double* nD, const double* nL,
+                             const double* nT, StructInfo* tab) {
+    for (long long a = (long long)blockIdx.x * blockDim.x + threadIdx.x; a < n; a += (long long)gridDim.x * blockDim.x) {
+        StructInfo& T = tab[seg[a]];
+        const int f = T.flags;
+        unsigned long long sets = 0, part = 0;
+        if (f & F_DOSE_SLAB) { ++sets; part += nD[a] > 0.0; }
+        if (f & F_DL_SLAB) { ++sets; part += nL[a] > 0.0; }
+        if (f & F_LETD) { ++sets; part += nT[a] > 0.0; }
+        atomicAdd(&T.n_sets, sets);
+        atomicAdd(&T.part, part);
+        atomicAdd(&T.n_zero, sets - part);
+        atomicAdd(&T.rows, 1ULL);
+        atomicAdd(&T.nnz, (unsigned long long)ulen[a]);
+    }
+}
+
+// W = sum_s w_s * part_s (s ascending), w^_s = w_s / W; pass modes and transposed-pass coefficients
+__global__ void k_finish_tables(StructInfo* tab, int n_struct, DevState* st, uint8_t* mode_union, uint8_t* mode_con,
+                                uint8_t* mode_cost, uint8_t* mode_fixed, int max_seg, SegCoef* coef_cost, SegCoef* coef_unit) {
+    if (threadIdx.x != 0 || blockIdx.x != 0) return;
+    double W = 0.0;
+    long long ns = 0, nz = 0;
+    for (int s = 0; s < n_struct; ++s) { W += tab[s].w * (double)tab[s].part; ns += tab[s].n_sets; nz += tab[s].n_zero; }
+    for (int s = 0; s < n_struct; ++s) {
+        StructInfo& T = tab[s];
+        T.what = W > 0.0 ? T.w / W : 0.0;
+        const int f = T.flags;
+        const int cost = ((f & F_DOSE_REF) ? 1 : 0) | ((f & F_DL_REF) ? 2 : 0);
+        const int con = ((f & (F_DOSE_SLAB | F_LETD)) ? 1 : 0) | ((f & (F_DL_SLAB | F_LETD)) ? 2 : 0);
+        mode_cost[s] = (uint8_t)cost;
+        mode_con[s] = (uint8_t)con;
+        mode_union[s] = (uint8_t)(cost | con);
+        coef_cost[s] = SegCoef{(f & F_DOSE_REF) ? 2.0 * T.what : 0.0, (f & F_DOSE_REF) ? T.dose_ref : 0.0,
+                               (f & F_DL_REF) ? 2.0 * T.what : 0.0, (f & F_DL_REF) ? T.dl_ref : 0.0};
+    }
+    for (int s = 0; s < max_seg; ++s) {
+        coef_unit[s] = SegCoef{1.0, 0.0, 1.0, 0.0};
+        for (int m = 0; m < 4; ++m) mode_fixed[m * max_seg + s] = (uint8_t)m;
+    }
+    st->W = W; st->n_sets = ns; st->n_zero = nz;
+}
+
+// ---- transposition of a row set
+__global__ void k_tr_keys(RowList rl, const int32_t* ulen, const long long* off, const int32_t* col, int n_seg,
+                          uint32_t* keys, uint32_t* vals) {
+    const int lane = threadIdx.x & 31;
+    const long long w0 = ((long long)blockIdx.x * blockDim.x + threadIdx.x) >> 5, nw = ((long long)gridDim.x * blockDim.x) >> 5;
+    for (long long r = w0; r < rl.n; r += nw) {
+        const long long s = rl.start[r], o = off[r];
+        const int L = ulen[r];
+        const int sg = rl.seg ? rl.seg[r] : 0;
+        for (int p = lane; p < L; p += 32) {
+            keys[o + p] = (uint32_t)col[s + p] * (uint32_t)n_seg + (uint32_t)sg;
+            vals[o + p] = (uint32_t)(o + p);
+        }
+    }
+}
+// ustart[k] = first sorted position with key >= k, k = 0..K
+__global__ void k_tr_bounds(const uint32_t* keys, long long E, long long K, long long* ustart, long long* pcount) {
+    for (long long k = (long long)blockIdx.x * blockDim.x + threadIdx.x; k <= K; k += (long long)gridDim.x * blockDim.x) {
+        long long lo = 0, hi = E;
+        while (lo < hi) { const long long mid = (lo + hi) >> 1; if ((long long)keys[mid] < k) lo = mid + 1; else hi = mid; }
+        ustart[k] = lo;
+    }
+}
+__global__ void k_tr_pcount(const long long* ustart, long long K, long long* pcount) {
+    for (long long k = (long long)blockIdx.x * blockDim.x + threadIdx.x; k < K; k += (long long)gridDim.x * blockDim.x)
+        pcount[k] = (ustart[k + 1] - ustart[k] + 3) & ~3LL;
+}
+__global__ void k_tr_fill(const uint32_t* keys, const uint32_t* vals, long long E, const long long* ustart, const long long* t_ptr,
+                          const long long* off, long long n_rows, const long long* start, const float* vD, const float* vL,
+                          int32_t* t_col, float* tD, float* tL) {
+    for (long long r = (long long)blockIdx.x * blockDim.x + threadIdx.x; r < E; r += (long long)gridDim.x * blockDim.x) {
+        const long long k = keys[r], e = vals[r];
+        // row a with off[a] <= e < off[a+1]
+        long long lo = 0, hi = n_rows;
+        while (lo < hi) { const long long mid = (lo + hi) >> 1; if (off[mid + 1] <= e) lo = mid + 1; else hi = mid; }
+        const long long a = lo, p = start[a] + (e - off[a]);
+        const long long dst = t_ptr[k] + (r - ustart[k]);
+        t_col[dst] = (int32_t)a;
+        tD[dst] = vD[p];
+        tL[dst] = vL[p];
+    }
+}
+__global__ void k_i32_to_i64(const int32_t* in, long long* out, long long n) {
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (long long)gridDim.x * blockDim.x) out[i] = in[i];
+}
+
+}  // namespace
+
+// ============================================================================================ helpers
+template <class T>
+static int scan_exclusive(fredopt_plan* P, const T* in, T* out, long long n) {
+    size_t tb = 0;
+    CK(cub::DeviceScan::ExclusiveSum(nullptr, tb, in, out, n, P->stream));
+    void* tmp = nullptr;
+    CK(cudaMalloc(&tmp, tb ? tb : 1));
+    cudaError_t e = cub::DeviceScan::ExclusiveSum(tmp, tb, in, out, n, P->stream);
+    cudaError_t e2 = cudaStreamSynchronize(P->stream);
+    cudaFree(tmp);
+    CK(e);
+    CK(e2);
+    return FREDOPT_OK;
+}
+
+static int build_transpose(fredopt_plan* P, RowSet& R) {
+    cudaStream_t st = P->stream;
+    const long long n = R.n, S = P->S, K = S * R.n_seg;
+    // unpadded offsets
+    long long *len64 = nullptr, *off = nullptr;
+    CK(cudaMalloc(&len64, (n + 1) * sizeof(long long)));
+    CK(cudaMalloc(&off, (n + 2) * sizeof(long long)));
+    CK(cudaMemsetAsync(len64, 0, (n + 1) * sizeof(long long), st));
+    if (n) k_i32_to_i64<<<grid_for(n, 256, 4096), 256, 0, st>>>(R.ulen, len64, n);
+    int rc = scan_exclusive(P, len64, off, n + 1);
+    cudaFree(len64);
+    if (rc) { cudaFree(off); return rc; }
+    long long E = 0;
+    CK(cudaMemcpyAsync(&E, off + n, sizeof(long long), cudaMemcpyDeviceToHost, st));
+    CK(cudaStreamSynchronize(st));
+    R.nnz = E;
+    if (E >= (1LL << 32) || K >= (1LL << 32)) { cudaFree(off); return FREDOPT_INVALID_ARG; }
+    uint32_t *keys = nullptr, *vals = nullptr, *keys2 = nullptr, *vals2 = nullptr;
+    long long *ustart = nullptr, *pcount = nullptr;
+    void* tmp = nullptr;
+    int ret = FREDOPT_OK;
+    auto cleanup = [&]() {
+        cudaFree(keys); cudaFree(vals); cudaFree(keys2); cudaFree(vals2); cudaFree(ustart); cudaFree(pcount); cudaFree(tmp); cudaFree(off);
+    };
+#define CKC(expr)                                                                                   \
+    do {                                                                                            \
+        cudaError_t e__ = (expr);                                                                   \
+        if (e__ != cudaSuccess) {                                                                   \
+            g_last_cuda_error = std::string(#expr) + ": " + cudaGetErrorString(e__);                \
+            cudaGetLastError();                                                                     \
+            cleanup();                                                                              \
+            return e__ == cudaErrorMemoryAllocation ? FREDOPT_OUT_OF_MEMORY : FREDOPT_CUDA_ERROR;   \
+        }                                                                                           \
+    } while (0)
+    const size_t En = E ? (size_t)E : 1;
+    CKC(cudaMalloc(&keys, En * 4)); CKC(cudaMalloc(&vals, En * 4));
+    CKC(cudaMalloc(&keys2, En * 4)); CKC(cudaMalloc(&vals2, En * 4));
+    CKC(cudaMalloc(&ustart, (K + 2) * sizeof(long long))); CKC(cudaMalloc(&pcount, (K + 2) * sizeof(long long)));
+    if (n) k_tr_keys<<<grid_for(n * 32, 256, 1 << 16), 256, 0, st>>>(R.view(), R.ulen, off, P->col, R.n_seg, keys, vals);
+    int bits = 1;
+    while ((1LL << bits) < K) ++bits;
+    size_t tb = 0;
+    CKC(cub::DeviceRadixSort::SortPairs(nullptr, tb, keys, keys2, vals, vals2, E, 0, bits, st));
+    CKC(cudaMalloc(&tmp, tb ? tb : 1));
+    CKC(cub::DeviceRadixSort::SortPairs(tmp, tb, keys, keys2, vals, vals2, E, 0, bits, st));   // stable: list order kept inside a key
+    k_tr_bounds<<<grid_for(K + 1, 256, 4096), 256, 0, st>>>(keys2, E, K, ustart, pcount);
+    CKC(cudaMemsetAsync(pcount, 0, (K + 2) * sizeof(long long), st));
+    k_tr_pcount<<<grid_for(K, 256, 4096), 256, 0, st>>>(ustart, K, pcount);
+    CKC(cudaGetLastError());
+    ret = dmalloc(P, &R.t_ptr, (size_t)K + 2);
+    if (ret) { cleanup(); return ret; }
+    ret = scan_exclusive(P, pcount, R.t_ptr, K + 1);
+    if (ret) { cleanup(); return ret; }
+    CKC(cudaMemcpyAsync(&R.t_nnz_padded, R.t_ptr + K, sizeof(long long), cudaMemcpyDeviceToHost, st));
+    CKC(cudaStreamSynchronize(st));
+    const size_t Tn = R.t_nnz_padded ? (size_t)R.t_nnz_padded : 4;
+    if ((ret = dmalloc(P, &R.t_col, Tn)) || (ret = dmalloc(P, &R.t_valD, Tn)) || (ret = dmalloc(P, &R.t_valL, Tn))) { cleanup(); return ret; }
+    CKC(cudaMemsetAsync(R.t_col, 0, Tn * 4, st));
+    CKC(cudaMemsetAsync(R.t_valD, 0, Tn * 4, st));
+    CKC(cudaMemsetAsync(R.t_valL, 0, Tn * 4, st));
+    if (E) k_tr_fill<<<grid_for(E, 256, 1 << 16), 256, 0, st>>>(keys2, vals2, E, ustart, R.t_ptr, off, n, R.start, P->valD, P->valL,
+                                                             R.t_col, R.t_valD, R.t_valL);
+    CKC(cudaGetLastError());
+    CKC(cudaStreamSynchronize(st));
+    cleanup();
+#undef CKC
+    R.t_built = true;
+    return FREDOPT_OK;
+}
+
+// bytes the method must move in one launch of a pass: per non-zero 4 B index + 4 B per value array
+// the row needs; 8 B per row offset; fp64 vectors read / written once.
+static void compute_pass_bytes(fredopt_plan* P) {
+    long long fwd_union = 0, fwd_con = 0, tr_cost = 0, tr_con = 0, rows_union = 0, rows_con = 0, rows_cost = 0;
+    for (int s = 0; s < P->n_struct; ++s) {
+        const StructInfo& T = P->h_tab[s];
+        const int f = T.flags;
+        const int cost = ((f & F_DOSE_REF) ? 1 : 0) | ((f & F_DL_REF) ? 2 : 0);
+        const int con = ((f & (F_DOSE_SLAB | F_LETD)) ? 1 : 0) | ((f & (F_DL_SLAB | F_LETD)) ? 2 : 0);
+        auto per = [](int m) { return m ? 4 + 4 * ((m & 1) + ((m >> 1) & 1)) : 0; };
+        fwd_union += (long long)T.nnz * per(cost | con);
+        fwd_con += (long long)T.nnz * per(con);
+        tr_cost += (long long)T.nnz * per(cost);
+        tr_con += (long long)T.nnz * per(con);
+        if (cost | con) rows_union += T.rows;
+        if (con) rows_con += T.rows;
+        if (cost) rows_cost += T.rows;
+    }
+    const long long S = P->S, VA = P->act.n;
+    P->pass_bytes[FREDOPT_PASS_FORWARD_X] = fwd_union + rows_union * (8 + 16) + S * 8;
+    P->pass_bytes[FREDOPT_PASS_FORWARD_G] = fwd_union + rows_union * (8 + 16) + S * 8;
+    P->pass_bytes[FREDOPT_PASS_TRANSPOSE_G] = tr_cost + S * P->act.n_seg * 8 + rows_cost * 16 + S * 8;
+    P->pass_bytes[FREDOPT_PASS_TRANSPOSE_B] = tr_con + S * P->act.n_seg * 8 + rows_con * 16 + S * 16;
+    P->pass_bytes[FREDOPT_PASS_SELECT] = S * 24;
+    P->pass_bytes[FREDOPT_PASS_RESIDUAL] = VA * (4 + 8 * 9);
+    (void)fwd_con;
+}
+
+// ============================================================================================ launches
+static void ev_begin(fredopt_plan* P, int pass) {
+    if (!P->time_passes) return;
+    EventPair ep;
+    cudaEventCreate(&ep.a); cudaEventCreate(&ep.b);
+    ep.pass = pass;
+    cudaEventRecord(ep.a, P->stream);
+    P->events.push_back(ep);
+}
+static void ev_end(fredopt_plan* P) {
+    if (!P->time_passes) return;
+    cudaEventRecord(P->events.back().b, P->stream);
+}
+
+static int fwd_grid(fredopt_plan* P, long long n) {
+    const int cap = P->sm_count * 8 < MAX_PARTIALS ? P->sm_count * 8 : MAX_PARTIALS;
+    return grid_for(n, FWD_WARPS, cap);
+}
+
+static void launch_forward_store(fredopt_plan* P, const RowSet& R, const uint8_t* mode, const double* x, double* oD, double* oL,
+                                 bool cpart) {
+    if (R.n == 0) { if (cpart) cudaMemsetAsync(P->cpart, 0, sizeof(double) * MAX_PARTIALS, P->stream); return; }
+    const int g = fwd_grid(P, R.n);
+    if (cpart) {
+        k_forward<EPI_CPART><<<g, FWD_THREADS, 0, P->stream>>>(R.view(), mode, P->col, P->valD, P->valL, x, oD, oL, P->tab, P->cpart,
+                                                               nullptr, nullptr, 0);
+    } else
+        k_forward<EPI_STORE><<<g, FWD_THREADS, 0, P->stream>>>(R.view(), mode, P->col, P->valD, P->valL, x, oD, oL, nullptr, nullptr,
+                                                               nullptr, nullptr, 0);
+    ++P->launches;
+}
+
+template <int EPI>
+static void launch_transpose(fredopt_plan* P, const RowSet& R, const uint8_t* mode, const SegCoef* coef, const double* vecD,
+                             const double* vecL, double* g_out, double* x, float* f_out) {
+    if (P->S == 0) return;
+    k_transpose<EPI><<<(unsigned)P->S, TR_THREADS, 0, P->stream>>>(R.n_seg, R.t_ptr, R.t_col, R.t_valD, R.t_valL, mode, coef, vecD,
+                                                                  vecL, g_out, x, P->st, f_out);
+    ++P->launches;
+}
+
+static int res_grid(fredopt_plan* P) {
+    const int cap = P->sm_count * 4 < MAX_PARTIALS ? P->sm_count * 4 : MAX_PARTIALS;
+    return grid_for(P->act.n, ROW_THREADS, cap);
+}
+
+static void launch_residual(fredopt_plan* P, double* d, double* l, int use_beta, int final, int write_uv) {
+    const int g = res_grid(P);
+    k_residual<<<g, ROW_THREADS, 0, P->stream>>>(P->act.n, P->act.seg, P->tab, P->st, d, l, P->Dg, P->Lg, P->nD, P->nL, P->nT, P->u,
+                                                 P->v, P->part_prox, P->part_phi, P->part_cnt, use_beta, final, write_uv);
+    ++P->launches;
+}
+
+static void launch_finalize(fredopt_plan* P) {
+    k_finalize_stats<<<1, 1024, 0, P->stream>>>(P->st, P->part_prox, P->part_phi, P->part_cnt, res_grid(P));
+    ++P->launches;
+}
+
+// one iteration of Fig. 3 around the simultaneous Fig. 2 step; returns the number of kernels enqueued
+static int enqueue_iteration(fredopt_plan* P, bool sa) {
+    const long long before = P->launches;
+    if (sa) {
+        ev_begin(P, FREDOPT_PASS_FORWARD_X);
+        launch_forward_store(P, P->act, P->mode_union, P->x, P->d, P->l, false);                       // a1: d = Dx, l = Lx
+        ev_end(P);
+        for (long long t = 0; t < P->reductionsN; ++t) {
+            ev_begin(P, FREDOPT_PASS_TRANSPOSE_G);
+            launch_transpose<TEPI_GRAD>(P, P->act, P->mode_cost, P->coef_cost, P->d, P->l, P->g, nullptr, nullptr);   // a3: g
+            ev_end(P);
+            ev_begin(P, FREDOPT_PASS_FORWARD_G);
+            launch_forward_store(P, P->act, P->mode_union, P->g, P->Dg, P->Lg, true);                  // a5: Dg, Lg, c
+            ev_end(P);
+            ev_begin(P, FREDOPT_PASS_SELECT);
+            k_select<<<1, 1024, 0, P->stream>>>(P->st, P->g, P->x, P->S, P->cpart, MAX_PARTIALS);      // a4, a6
+            ++P->launches;
+            ev_end(P);
+            ev_begin(P, FREDOPT_PASS_RESIDUAL);
+            const int last = t == P->reductionsN - 1;
+            launch_residual(P, P->d, P->l, 1, last, last);                                             // a7 (and d', l')
+            ev_end(P);
+        }
+    } else {
+        ev_begin(P, FREDOPT_PASS_FORWARD_X);
+        launch_forward_store(P, P->act, P->mode_con, P->x, P->d, P->l, false);
+        ev_end(P);
+        ev_begin(P, FREDOPT_PASS_RESIDUAL);
+        launch_residual(P, P->d, P->l, 0, 1, 1);
+        ev_end(P);
+    }
+    ev_begin(P, FREDOPT_PASS_TRANSPOSE_B);
+    launch_transpose<TEPI_UPDATE>(P, P->act, P->mode_con, P->coef_unit, P->u, P->v, nullptr, P->x, nullptr);   // a8, a9
+    ev_end(P);
+    return (int)(P->launches - before);
+}
+
+// ============================================================================================ API
+extern "C" {
+
+const char* fredopt_strerror(int code) {
+    switch (code) {
+        case FREDOPT_OK: return "ok";
+        case FREDOPT_INVALID_ARG: return "invalid argument";
+        case FREDOPT_OUT_OF_MEMORY: return "out of device memory";
+        case FREDOPT_CUDA_ERROR: return "CUDA error";
+        case FREDOPT_UNSUPPORTED_ARCH: return "unsupported GPU architecture (needs compute capability 10.x, built for sm_100a)";
+        case FREDOPT_UNSUPPORTED: return "unsupported";
+        default: return "unknown error";
+    }
+}
+const char* fredopt_last_cuda_error(void) { return g_last_cuda_error.c_str(); }
+
+void fredopt_destroy(fredopt_plan* P) {
+    if (!P) return;
+    cudaStreamSynchronize(P->stream);
+    for (auto& ep : P->events) { cudaEventDestroy(ep.a); cudaEventDestroy(ep.b); }
+    for (int i = 0; i < 2; ++i) if (P->gexec[i]) cudaGraphExecDestroy(P->gexec[i]);
+    for (void* p : P->allocs) cudaFree(p);
+    delete P;
+}
+
+static int create_impl(fredopt_plan* P, const fredopt_csr* D, const fredopt_csr* L, const int32_t* labels,
+                       const fredopt_bounds* bounds, int32_t n_struct) {
+    cudaStream_t st = P->stream;
+    const long long V = D->n_rows, S = D->n_cols;
+    P->V = V; P->S = S; P->n_struct = n_struct;
+    // ---- host-side table of structures
+    P->h_tab.resize(n_struct > 0 ? n_struct : 1);
+    for (int s = 0; s < n_struct; ++s) {
+        const fredopt_bounds& b = bounds[s];
+        if (!(b.weight > 0.f) || !std::isfinite(b.weight)) return FREDOPT_INVALID_ARG;
+        if (b.dose_lo > b.dose_hi || b.dl_lo > b.dl_hi) return FREDOPT_INVALID_ARG;
+        if (std::isinf(b.dose_lo) || std::isinf(b.dose_hi) || std::isinf(b.dl_lo) || std::isinf(b.dl_hi) || std::isinf(b.letd_max) ||
+            std::isinf(b.dose_ref) || std::isinf(b.dl_ref))
+            return FREDOPT_INVALID_ARG;
+        StructInfo T;
+        memset(&T, 0, sizeof(T));
+        T.w = (double)b.weight;
+        T.dose_lo = (double)b.dose_lo; T.dose_hi = (double)b.dose_hi; T.dl_lo = (double)b.dl_lo; T.dl_hi = (double)b.dl_hi;
+        T.letd_max = (double)b.letd_max; T.dose_ref = (double)b.dose_ref; T.dl_ref = (double)b.dl_ref;
+        T.flags = ((!std::isnan(b.dose_lo) || !std::isnan(b.dose_hi)) ? F_DOSE_SLAB : 0) |
+                  ((!std::isnan(b.dl_lo) || !std::isnan(b.dl_hi)) ? F_DL_SLAB : 0) | (!std::isnan(b.letd_max) ? F_LETD : 0) |
+                  (!std::isnan(b.dose_ref) ? F_DOSE_REF : 0) | (!std::isnan(b.dl_ref) ? F_DL_REF : 0);
+        P->h_tab[s] = T;
+    }
+    // ---- inputs on the device (borrowed if already there)
+    std::vector<void*> tmp;   // temporaries of this call
+    auto tfree = [&]() { for (void* p : tmp) cudaFree(p); tmp.clear(); };
+    struct Guard { decltype(tfree)& f; ~Guard() { f(); } } guard{tfree};
+    auto to_dev = [&](const void* src, size_t bytes, const void** out) -> int {
+        if (bytes == 0) { void* p; CK(cudaMalloc(&p, 16)); tmp.push_back(p); *out = p; return FREDOPT_OK; }
+        if (is_device_ptr(src)) { *out = src; return FREDOPT_OK; }
+        void* p = nullptr;
+        CK(cudaMalloc(&p, bytes));
+        tmp.push_back(p);
+        CK(cudaMemcpyAsync(p, src, bytes, cudaMemcpyHostToDevice, st));
+        *out = p;
+        return FREDOPT_OK;
+    };
+    const long long *pD, *pL; const int32_t *cD, *cL, *lab; const float *vD, *vL;
+    CKR(to_dev(D->row_ptr, (V + 1) * 8, (const void**)&pD));
+    CKR(to_dev(D->col_idx, D->nnz * 4, (const void**)&cD));
+    CKR(to_dev(D->values, D->nnz * 4, (const void**)&vD));
+    CKR(to_dev(L->row_ptr, (V + 1) * 8, (const void**)&pL));
+    CKR(to_dev(L->col_idx, L->nnz * 4, (const void**)&cL));
+    CKR(to_dev(L->values, L->nnz * 4, (const void**)&vL));
+    CKR(to_dev(labels, V * 4, (const void**)&lab));
+    // ---- validate
+    int* flag = nullptr;
+    CK(cudaMalloc(&flag, 2 * sizeof(int))); tmp.push_back(flag);
+    CK(cudaMemsetAsync(flag, 0, 2 * sizeof(int), st));
+    k_check_ptr<<<grid_for(V + 1, 256, 4096), 256, 0, st>>>(pD, V, D->nnz, flag);
+    k_check_ptr<<<grid_for(V + 1, 256, 4096), 256, 0, st>>>(pL, V, L->nnz, flag);
+    k_check_labels<<<grid_for(V, 256, 4096), 256, 0, st>>>(lab, V, n_struct, flag);
+    int hflag[2] = {0, 0};
+    CK(cudaMemcpyAsync(hflag, flag, 2 * sizeof(int), cudaMemcpyDeviceToHost, st));
+    CK(cudaStreamSynchronize(st));
+    if (hflag[0]) return FREDOPT_INVALID_ARG;
+    k_check_rows<<<grid_for(V * 32, 256, 1 << 16), 256, 0, st>>>(pD, cD, vD, V, S, flag);
+    k_check_rows<<<grid_for(V * 32, 256, 1 << 16), 256, 0, st>>>(pL, cL, vL, V, S, flag);
+    // ---- same pattern?
+    int same = D->nnz == L->nnz;
+    if (same) {
+        k_cmp_i64<<<grid_for(V + 1, 256, 4096), 256, 0, st>>>(pD, pL, V + 1, flag + 1);
+        k_cmp_i32<<<grid_for(D->nnz, 256, 1 << 16), 256, 0, st>>>(cD, cL, D->nnz, flag + 1);
+    }
+    CK(cudaMemcpyAsync(hflag, flag, 2 * sizeof(int), cudaMemcpyDeviceToHost, st));
+    CK(cudaStreamSynchronize(st));
+    CK(cudaGetLastError());
+    if (hflag[0]) return FREDOPT_INVALID_ARG;
+    if (hflag[1]) same = 0;
+    const long long* pU = pD; const int32_t* cU = cD; const float *uD = vD, *uL = vL;
+    long long nnzU = D->nnz;
+    if (!same) {   // union pattern (rare path)
+        long long *cnt = nullptr, *pu = nullptr;
+        CK(cudaMalloc(&cnt, (V + 1) * 8)); tmp.push_back(cnt);
+        CK(cudaMalloc(&pu, (V + 2) * 8)); tmp.push_back(pu);
+        CK(cudaMemsetAsync(cnt, 0, (V + 1) * 8, st));
+        k_union_count<<<grid_for(V, 128, 1 << 16), 128, 0, st>>>(pD, cD, pL, cL, V, cnt);
+        CKR(scan_exclusive(P, cnt, pu, V + 1));
+        CK(cudaMemcpyAsync(&nnzU, pu + V, 8, cudaMemcpyDeviceToHost, st));
+        CK(cudaStreamSynchronize(st));
+        int32_t* cu; float *ud, *ul;
+        CK(cudaMalloc(&cu, (nnzU ? nnzU : 1) * 4)); tmp.push_back(cu);
+        CK(cudaMalloc(&ud, (nnzU ? nnzU : 1) * 4)); tmp.push_back(ud);
+        CK(cudaMalloc(&ul, (nnzU ? nnzU : 1) * 4)); tmp.push_back(ul);
+        k_union_fill<<<grid_for(V, 128, 1 << 16), 128, 0, st>>>(pD, cD, vD, pL, cL, vL, V, pu, cu, ud, ul);
+        pU = pu; cU = cu; uD = ud; uL = ul;
+    }
+    if (nnzU >= (1LL << 32)) return FREDOPT_INVALID_ARG;
+    P->nnz = nnzU;
+    // ---- row lengths, non-empty list, active list
+    long long *plen64, *pstart; int32_t *f_ne, *f_act, *pos_ne, *pos_act;
+    CK(cudaMalloc(&plen64, (V + 1) * 8)); tmp.push_back(plen64);
+    CK(cudaMalloc(&pstart, (V + 2) * 8)); tmp.push_back(pstart);
+    CK(cudaMalloc(&f_ne, (V + 1) * 4)); tmp.push_back(f_ne);
+    CK(cudaMalloc(&f_act, (V + 1) * 4)); tmp.push_back(f_act);
+    CK(cudaMalloc(&pos_ne, (V + 2) * 4)); tmp.push_back(pos_ne);
+    CK(cudaMalloc(&pos_act, (V + 2) * 4)); tmp.push_back(pos_act);
+    CK(cudaMemsetAsync(plen64, 0, (V + 1) * 8, st));
+    CK(cudaMemsetAsync(f_ne, 0, (V + 1) * 4, st));
+    CK(cudaMemsetAsync(f_act, 0, (V + 1) * 4, st));
+    if (V) k_row_lengths<<<grid_for(V, 256, 1 << 16), 256, 0, st>>>(pU, lab, V, plen64, f_ne, f_act);
+    CKR(scan_exclusive(P, plen64, pstart, V + 1));
+    CKR(scan_exclusive(P, f_ne, pos_ne, V + 1));
+    CKR(scan_exclusive(P, f_act, pos_act, V + 1));
+    int32_t n_ne = 0, n_act = 0;
+    CK(cudaMemcpyAsync(&P->nnz_padded, pstart + V, 8, cudaMemcpyDeviceToHost, st));
+    CK(cudaMemcpyAsync(&n_ne, pos_ne + V, 4, cudaMemcpyDeviceToHost, st));
+    CK(cudaMemcpyAsync(&n_act, pos_act + V, 4, cudaMemcpyDeviceToHost, st));
+    CK(cudaStreamSynchronize(st));
+    // ---- full row set + padded arrays
+    RowSet& F = P->full;
+    F.n = n_ne; F.n_seg = 1; F.nnz = nnzU;
+    CKR(dmalloc(P, &F.vox, (size_t)n_ne)); CKR(dmalloc(P, &F.start, (size_t)n_ne));
+    CKR(dmalloc(P, &F.len, (size_t)n_ne)); CKR(dmalloc(P, &F.ulen, (size_t)n_ne));
+    if (V) k_compact_rows<<<grid_for(V, 256, 1 << 16), 256, 0, st>>>(f_ne, pos_ne, pU, pstart, lab, V, F.vox, F.start, F.len, F.ulen, nullptr);
+    const size_t np = P->nnz_padded ? (size_t)P->nnz_padded : 4;
+    CKR(dmalloc(P, &P->col, np)); CKR(dmalloc(P, &P->valD, np)); CKR(dmalloc(P, &P->valL, np));
+    CK(cudaMemsetAsync(P->col, 0, np * 4, st)); CK(cudaMemsetAsync(P->valD, 0, np * 4, st)); CK(cudaMemsetAsync(P->valL, 0, np * 4, st));
+    if (n_ne) k_copy_padded<<<grid_for((long long)n_ne * 32, 256, 1 << 16), 256, 0, st>>>(F.n, F.vox, F.start, pU, cU, uD, uL, P->col, P->valD, P->valL);
+    // ---- active row set, ordered by (label, voxel)
+    RowSet& A = P->act;
+    A.n = n_act; A.n_seg = n_struct > 0 ? n_struct : 1;
+    CKR(dmalloc(P, &A.vox, (size_t)n_act)); CKR(dmalloc(P, &A.start, (size_t)n_act)); CKR(dmalloc(P, &A.len, (size_t)n_act));
+    CKR(dmalloc(P, &A.ulen, (size_t)n_act)); CKR(dmalloc(P, &A.seg, (size_t)n_act));
+    {
+        int32_t *vox0, *key0, *key1;
+        CK(cudaMalloc(&vox0, (n_act + 1) * 4)); tmp.push_back(vox0);
+        CK(cudaMalloc(&key0, (n_act + 1) * 4)); tmp.push_back(key0);
+        CK(cudaMalloc(&key1, (n_act + 1) * 4)); tmp.push_back(key1);
+        if (V) k_compact_rows<<<grid_for(V, 256, 1 << 16), 256, 0, st>>>(f_act, pos_act, pU, pstart, lab, V, vox0, nullptr, nullptr, nullptr, key0);
+        int bits = 1;
+        while ((1 << bits) <= n_struct) ++bits;
+        size_t tb = 0;
+        CK(cub::DeviceRadixSort::SortPairs(nullptr, tb, key0, key1, vox0, A.vox, n_act, 0, bits, st));
+        void* t2; CK(cudaMalloc(&t2, tb ? tb : 1)); tmp.push_back(t2);
+        CK(cub::DeviceRadixSort::SortPairs(t2, tb, key0, key1, vox0, A.vox, n_act, 0, bits, st));
+        if (n_act) k_fill_active<<<grid_for(n_act, 256, 1 << 16), 256, 0, st>>>(A.vox, key1, pU, pstart, n_act, A.start, A.len, A.ulen, A.seg);
+    }
+    // ---- tables, norms, w^
+    const int ns = n_struct > 0 ? n_struct : 1;
+    P->max_seg = ns;
+    CKR(dmalloc(P, &P->tab, (size_t)ns));
+    CK(cudaMemcpyAsync(P->tab, P->h_tab.data(), sizeof(StructInfo) * ns, cudaMemcpyHostToDevice, st));
+    CKR(dmalloc(P, &P->nD, (size_t)n_act)); CKR(dmalloc(P, &P->nL, (size_t)n_act)); CKR(dmalloc(P, &P->nT, (size_t)n_act));
+    CKR(dmalloc(P, &P->mode_union, (size_t)ns)); CKR(dmalloc(P, &P->mode_con, (size_t)ns)); CKR(dmalloc(P, &P->mode_cost, (size_t)ns));
+    CKR(dmalloc(P, &P->mode_fixed, (size_t)ns * 4));
+    CKR(dmalloc(P, &P->coef_cost, (size_t)ns)); CKR(dmalloc(P, &P->coef_unit, (size_t)ns));
+    CKR(dmalloc(P, &P->st, 1));
+    CK(cudaMemsetAsync(P->st, 0, sizeof(DevState), st));
+    if (n_act) {
+        k_norms<<<grid_for((long long)n_act * 32, 256, 1 << 16), 256, 0, st>>>(A.view(), P->col, P->valD, P->valL, P->tab, P->nD, P->nL, P->nT);
+        k_count_sets<<<grid_for(n_act, 256, 4096), 256, 0, st>>>(n_act, A.seg, A.ulen, P->nD, P->nL, P->nT, P->tab);
+    }
+    k_finish_tables<<<1, 1, 0, st>>>(P->tab, n_struct, P->st, P->mode_union, P->mode_con, P->mode_cost, P->mode_fixed, ns, P->coef_cost,
+                                    P->coef_unit);
+    k_set_params<<<1, 1, 0, st>>>(P->st, 1.0, 0.0, 0.5, 1.0, 200, 1, 1);
+    CK(cudaMemcpyAsync(P->h_tab.data(), P->tab, sizeof(StructInfo) * ns, cudaMemcpyDeviceToHost, st));
+    CK(cudaStreamSynchronize(st));
+    CK(cudaGetLastError());
+    // ---- vectors
+    CKR(dmalloc(P, &P->x, (size_t)S)); CKR(dmalloc(P, &P->g, (size_t)S)); CKR(dmalloc(P, &P->xtmp, (size_t)S));
+    CK(cudaMemsetAsync(P->x, 0, (S ? S : 1) * 8, st)); CK(cudaMemsetAsync(P->g, 0, (S ? S : 1) * 8, st));
+    double** vecs[] = {&P->d, &P->l, &P->Dg, &P->Lg, &P->u, &P->v};
+    for (auto pp : vecs) { CKR(dmalloc(P, pp, (size_t)n_act)); CK(cudaMemsetAsync(*pp, 0, (n_act ? n_act : 1) * 8, st)); }
+    CKR(dmalloc(P, &P->cpart, (size_t)MAX_PARTIALS)); CKR(dmalloc(P, &P->part_prox, (size_t)MAX_PARTIALS));
+    CKR(dmalloc(P, &P->part_phi, (size_t)MAX_PARTIALS)); CKR(dmalloc(P, &P->part_cnt, (size_t)MAX_PARTIALS));
+    CKR(dmalloc(P, &P->sink, 4));
+    CK(cudaMemsetAsync(P->cpart, 0, MAX_PARTIALS * 8, st));
+    CK(cudaMemsetAsync(P->part_prox, 0, MAX_PARTIALS * 8, st)); CK(cudaMemsetAsync(P->part_phi, 0, MAX_PARTIALS * 8, st));
+    CK(cudaMemsetAsync(P->part_cnt, 0, MAX_PARTIALS * 8, st));
+    // ---- CSR of the transposes restricted to the active rows
+    CKR(build_transpose(P, A));
+    compute_pass_bytes(P);
+    CK(cudaStreamSynchronize(st));
+    return FREDOPT_OK;
+}
+
+int fredopt_create(const fredopt_csr* D, const fredopt_csr* L, const int32_t* voxel_labels, const fredopt_bounds* bounds,
+                   int32_t n_struct, void* cuda_stream, fredopt_plan** out) {
+    if (!out) return FREDOPT_INVALID_ARG;
+    *out = nullptr;
+    if (!D || !L || n_struct < 0 || (n_struct > 0 && !bounds)) return FREDOPT_INVALID_ARG;
+    if (D->n_rows != L->n_rows || D->n_cols != L->n_cols || D->n_rows < 0 || D->n_cols < 0 || D->nnz < 0 || L->nnz < 0)
+        return FREDOPT_INVALID_ARG;
+    if (D->n_rows >= (1LL << 31) - 1 || D->n_cols >= (1LL << 31) - 1 || D->nnz >= (1LL << 32) || L->nnz >= (1LL << 32))
+        return FREDOPT_INVALID_ARG;
+    if (!D->row_ptr || !L->row_ptr || (D->n_rows > 0 && !voxel_labels)) return FREDOPT_INVALID_ARG;
+    if ((D->nnz > 0 && (!D->col_idx || !D->values)) || (L->nnz > 0 && (!L->col_idx || !L->values))) return FREDOPT_INVALID_ARG;
+    int dev = 0;
+    CK(cudaGetDevice(&dev));
+    cudaDeviceProp prop;
+    CK(cudaGetDeviceProperties(&prop, dev));
+    if (prop.major != 10) return FREDOPT_UNSUPPORTED_ARCH;
+    fredopt_plan* P = new (std::nothrow) fredopt_plan();
+    if (!P) return FREDOPT_OUT_OF_MEMORY;
+    P->stream = (cudaStream_t)cuda_stream;
+    P->device = dev;
+    P->sm_count = prop.multiProcessorCount;
+    int rc = create_impl(P, D, L, voxel_labels, bounds, n_struct);
+    if (rc != FREDOPT_OK) { fredopt_destroy(P); return rc; }
+    *out = P;
+    return FREDOPT_OK;
+}
+
+// ---- host/device staging of small vectors
+static int stage_in_f32(fredopt_plan* P, const float* src, size_t n, const float** dev, void** to_free) {
+    *to_free = nullptr;
+    if (is_device_ptr(src)) { *dev = src; return FREDOPT_OK; }
+    void* p = nullptr;
+    CK(cudaMalloc(&p, (n ? n : 1) * 4));
+    cudaError_t e = cudaMemcpyAsync(p, src, n * 4, cudaMemcpyHostToDevice, P->stream);
+    if (e != cudaSuccess) { cudaFree(p); CK(e); }
+    *dev = (const float*)p; *to_free = p;
+    return FREDOPT_OK;
+}
+
+int fredopt_set_weights(fredopt_plan* P, const float* x) {
+    if (!P || !x) return FREDOPT_INVALID_ARG;
+    const float* dx; void* fr;
+    CKR(stage_in_f32(P, x, P->S, &dx, &fr));
+    k_f32_to_f64<<<grid_for(P->S, 256, 1024), 256, 0, P->stream>>>(dx, P->x, P->S);
+    ++P->launches;
+    if (fr) { cudaStreamSynchronize(P->stream); cudaFree(fr); }
+    CK(cudaGetLastError());
+    return FREDOPT_OK;
+}
+
+int fredopt_get_weights_f64(fredopt_plan* P, double* x) {
+    if (!P || !x) return FREDOPT_INVALID_ARG;
+    const bool dev = is_device_ptr(x);
+    CK(cudaMemcpyAsync(x, P->x, P->S * 8, dev ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost, P->stream));
+    if (!dev) CK(cudaStreamSynchronize(P->stream));
+    return FREDOPT_OK;
+}
+
+int fredopt_get_weights(fredopt_plan* P, float* x) {
+    if (!P || !x) return FREDOPT_INVALID_ARG;
+    if (is_device_ptr(x)) {
+        k_f64_to_f32<<<grid_for(P->S, 256, 1024), 256, 0, P->stream>>>(P->x, x, P->S);
+        ++P->launches;
+        CK(cudaGetLastError());
+        return FREDOPT_OK;
+    }
+    float* tmp = (float*)P->xtmp;   // S doubles of scratch hold S floats
+    k_f64_to_f32<<<grid_for(P->S, 256, 1024), 256, 0, P->stream>>>(P->x, tmp, P->S);
+    ++P->launches;
+    CK(cudaMemcpyAsync(x, tmp, P->S * 4, cudaMemcpyDeviceToHost, P->stream));
+    CK(cudaStreamSynchronize(P->stream));
+    return FREDOPT_OK;
+}
+
+// x argument of dose_let / proximity / spmv_forward: NULL = plan's x, else widened into xtmp
+static int resolve_x(fredopt_plan* P, const float* x, const double** xd) {
+    if (!x) { *xd = P->x; return FREDOPT_OK; }
+    const float* dx; void* fr;
+    CKR(stage_in_f32(P, x, P->S, &dx, &fr));
+    k_f32_to_f64<<<grid_for(P->S, 256, 1024), 256, 0, P->stream>>>(dx, P->xtmp, P->S);
+    ++P->launches;
+    if (fr) { cudaStreamSynchronize(P->stream); cudaFree(fr); }
+    *xd = P->xtmp;
+    return FREDOPT_OK;
+}
+
+static int forward_f32(fredopt_plan* P, const RowSet& R, int m, const double* xd, float* d, float* l, int letd_out) {
+    // d, l: caller outputs (host or device), voxel-indexed, n_rows floats; rows outside R are 0
+    float *dd = d, *dl = l;
+    void *fr_d = nullptr, *fr_l = nullptr;
+    const size_t nb = (size_t)(P->V ? P->V : 1) * 4;
+    if (d && !is_device_ptr(d)) { CK(cudaMalloc(&fr_d, nb)); dd = (float*)fr_d; }
+    if (l && !is_device_ptr(l)) { cudaError_t e = cudaMalloc(&fr_l, nb); if (e != cudaSuccess) { cudaFree(fr_d); CK(e); } dl = (float*)fr_l; }
+    if (dd) cudaMemsetAsync(dd, 0, (size_t)P->V * 4, P->stream);
+    if (dl) cudaMemsetAsync(dl, 0, (size_t)P->V * 4, P->stream);
+    if (R.n) {
+        k_forward<EPI_F32VOX><<<fwd_grid(P, R.n), FWD_THREADS, 0, P->stream>>>(R.view(), P->mode_fixed + (size_t)m * P->max_seg, P->col,
+                                                                               P->valD, P->valL, xd, nullptr, nullptr, nullptr, nullptr,
+                                                                               dd, dl, letd_out);
+        ++P->launches;
+    }
+    int rc = FREDOPT_OK;
+    cudaError_t e = cudaGetLastError();
+    if (e == cudaSuccess && fr_d) e = cudaMemcpyAsync(d, dd, (size_t)P->V * 4, cudaMemcpyDeviceToHost, P->stream);
+    if (e == cudaSuccess && fr_l) e = cudaMemcpyAsync(l, dl, (size_t)P->V * 4, cudaMemcpyDeviceToHost, P->stream);
+    if (fr_d || fr_l) { cudaError_t e2 = cudaStreamSynchronize(P->stream); if (e == cudaSuccess) e = e2; }
+    cudaFree(fr_d); cudaFree(fr_l);
+    if (e != cudaSuccess) { g_last_cuda_error = cudaGetErrorString(e); cudaGetLastError(); rc = FREDOPT_CUDA_ERROR; }
+    return rc;
+}
+
+int fredopt_dose_let(fredopt_plan* P, const float* x, float* dose, float* letd) {
+    if (!P || (!dose && !letd)) return FREDOPT_INVALID_ARG;
+    const double* xd;
+    CKR(resolve_x(P, x, &xd));
+    return forward_f32(P, P->full, letd ? 3 : 1, xd, dose, letd, 1);
+}
+
+int fredopt_spmv_forward(fredopt_plan* P, int32_t rows, const float* x, float* d, float* l) {
+    if (!P || (!d && !l) || (rows != FREDOPT_ROWS_ALL && rows != FREDOPT_ROWS_ACTIVE)) return FREDOPT_INVALID_ARG;
+    const double* xd;
+    CKR(resolve_x(P, x, &xd));
+    const RowSet& R = rows == FREDOPT_ROWS_ALL ? P->full : P->act;
+    return forward_f32(P, R, (d ? 1 : 0) | (l ? 2 : 0), xd, d, l, 0);
+}
+
+int fredopt_spmv_transpose(fredopt_plan* P, int32_t rows, const float* u, const float* v, float* out) {
+    if (!P || !out || (!u && !v) || (rows != FREDOPT_ROWS_ALL && rows != FREDOPT_ROWS_ACTIVE)) return FREDOPT_INVALID_ARG;
+    RowSet& R = rows == FREDOPT_ROWS_ALL ? P->full : P->act;
+    double *vecD = P->u, *vecL = P->v;
+    if (rows == FREDOPT_ROWS_ALL) {
+        if (!R.t_built) CKR(build_transpose(P, R));
+        if (!P->fullD) { CKR(dmalloc(P, &P->fullD, (size_t)R.n)); CKR(dmalloc(P, &P->fullL, (size_t)R.n)); }
+        vecD = P->fullD; vecL = P->fullL;
+    }
+    const float *du = nullptr, *dv = nullptr; void *fu = nullptr, *fv = nullptr;
+    if (u) CKR(stage_in_f32(P, u, P->V, &du, &fu));
+    if (v) { int rc = stage_in_f32(P, v, P->V, &dv, &fv); if (rc) { cudaFree(fu); return rc; } }
+    if (R.n) {
+        if (u) { k_gather_f32_to_f64<<<grid_for(R.n, 256, 4096), 256, 0, P->stream>>>(du, R.vox, vecD, R.n); ++P->launches; }
+        if (v) { k_gather_f32_to_f64<<<grid_for(R.n, 256, 4096), 256, 0, P->stream>>>(dv, R.vox, vecL, R.n); ++P->launches; }
+    }
+    float* dout = out; void* fo = nullptr;
+    if (!is_device_ptr(out)) { cudaError_t e = cudaMalloc(&fo, (P->S ? P->S : 1) * 4); if (e != cudaSuccess) { cudaFree(fu); cudaFree(fv); CK(e); } dout = (float*)fo; }
+    const int m = (u ? 1 : 0) | (v ? 2 : 0);
+    launch_transpose<TEPI_F32>(P, R, P->mode_fixed + (size_t)m * P->max_seg, P->coef_unit, vecD, vecL, nullptr, nullptr, dout);
+    cudaError_t e = cudaGetLastError();
+    if (e == cudaSuccess && fo) e = cudaMemcpyAsync(out, dout, P->S * 4, cudaMemcpyDeviceToHost, P->stream);
+    if (fo || fu || fv) { cudaError_t e2 = cudaStreamSynchronize(P->stream); if (e == cudaSuccess) e = e2; }
+    cudaFree(fo); cudaFree(fu); cudaFree(fv);
+    CK(e);
+    return FREDOPT_OK;
+}
+
+int fredopt_proximity(fredopt_plan* P, const float* x, double* prox, int64_t* n_violated) {
+    if (!P || (!prox && !n_violated)) return FREDOPT_INVALID_ARG;
+    const double* xd;
+    CKR(resolve_x(P, x, &xd));
+    // scratch: Dg / Lg hold the products so that the iteration's d, l are left alone
+    launch_forward_store(P, P->act, P->mode_con, xd, P->Dg, P->Lg, false);
+    launch_residual(P, P->Dg, P->Lg, 0, 1, 0);
+    launch_finalize(P);
+    DevState h;
+    CK(cudaMemcpyAsync(&h, P->st, sizeof(DevState), cudaMemcpyDeviceToHost, P->stream));
+    CK(cudaStreamSynchronize(P->stream));
+    CK(cudaGetLastError());
+    if (prox) *prox = h.prox;
+    if (n_violated) *n_violated = h.n_viol;
+    return FREDOPT_OK;
+}
+
+int fredopt_set_option(fredopt_plan* P, int32_t key, double value) {
+    if (!P) return FREDOPT_INVALID_ARG;
+    switch (key) {
+        case FREDOPT_OPT_ETA: if (!(value > 0.0) || value > 1.0) return FREDOPT_INVALID_ARG; P->eta = value; break;
+        case FREDOPT_OPT_REDUCTIONS:
+            if (value < 1.0 || value > 1000.0) return FREDOPT_INVALID_ARG;
+            P->reductionsN = (long long)value;
+            break;
+        case FREDOPT_OPT_ACCEPT_CHECK: P->accept_check = value != 0.0; break;
+        case FREDOPT_OPT_MAX_TRIALS: if (value < 1.0) return FREDOPT_INVALID_ARG; P->max_trials = (long long)value; break;
+        case FREDOPT_OPT_RESET: {
+            P->started = false;
+            DevState h;
+            CK(cudaMemcpyAsync(&h, P->st, sizeof(DevState), cudaMemcpyDeviceToHost, P->stream));
+            CK(cudaStreamSynchronize(P->stream));
+            h.k = 0; h.s = 0; h.trials = 0; h.last_beta = 0.0; h.eta_pow = 1.0; h.beta_acc = 0.0;
+            CK(cudaMemcpyAsync(P->st, &h, sizeof(DevState), cudaMemcpyHostToDevice, P->stream));
+            CK(cudaStreamSynchronize(P->stream));
+            break;
+        }
+        case FREDOPT_OPT_USE_GRAPH: P->use_graph = value != 0.0; break;
+        case FREDOPT_OPT_TIME_PASSES:
+            P->time_passes = value != 0.0;
+            if (P->time_passes) {
+                for (auto& ep : P->events) { cudaEventDestroy(ep.a); cudaEventDestroy(ep.b); }
+                P->events.clear();
+                for (int i = 0; i < FREDOPT_N_PASSES; ++i) { P->pass_ms[i] = 0; P->pass_launches[i] = 0; }
+            }
+            break;
+        default: return FREDOPT_INVALID_ARG;
+    }
+    return FREDOPT_OK;
+}
+
+int fredopt_iterate(fredopt_plan* P, int32_t n_iter, float lambda, float beta0, float a) {
+    if (!P || n_iter < 0) return FREDOPT_INVALID_ARG;
+    if (!(lambda > 0.f) || !(lambda <= 2.f) || !(beta0 >= 0.f) || !std::isfinite(beta0) || !(a > 0.f) || !(a < 1.f))
+        return FREDOPT_INVALID_ARG;
+    const int latch = !P->started;
+    if (latch) { P->latched_beta0 = beta0; P->started = true; }
+    k_set_params<<<1, 1, 0, P->stream>>>(P->st, (double)lambda, (double)beta0, (double)a, P->eta, P->max_trials, P->accept_check, latch);
+    ++P->launches;
+    const bool sa = beta0 != 0.f;
+    if (n_iter > 0) {
+        const bool graph = P->use_graph && !P->time_passes && n_iter > 1;
+        if (graph) {
+            const int gi = sa ? 1 : 0;
+            if (!P->gexec[gi] || P->gexec_red[gi] != P->reductionsN) {
+                if (P->gexec[gi]) { cudaGraphExecDestroy(P->gexec[gi]); P->gexec[gi] = nullptr; }
+                cudaGraph_t gr = nullptr;
+                CK(cudaStreamBeginCapture(P->stream, cudaStreamCaptureModeThreadLocal));
+                const long long l0 = P->launches;
+                const int nk = enqueue_iteration(P, sa);
+                P->launches = l0;
+                cudaError_t e = cudaStreamEndCapture(P->stream, &gr);
+                CK(e);
+                e = cudaGraphInstantiate(&P->gexec[gi], gr, 0);
+                cudaGraphDestroy(gr);
+                CK(e);
+                P->gexec_red[gi] = P->reductionsN;
+                P->gexec_kernels[gi] = nk;
+            }
+            for (int it = 0; it < n_iter; ++it) CK(cudaGraphLaunch(P->gexec[gi], P->stream));
+            P->launches += (long long)n_iter * P->gexec_kernels[gi];
+        } else {
+            for (int it = 0; it < n_iter; ++it) enqueue_iteration(P, sa);
+        }
+        launch_finalize(P);
+    }
+    CK(cudaGetLastError());
+    return FREDOPT_OK;
+}
+
+int fredopt_get_stats(fredopt_plan* P, fredopt_stats* out) {
+    if (!P || !out) return FREDOPT_INVALID_ARG;
+    DevState h;
+    CK(cudaMemcpyAsync(&h, P->st, sizeof(DevState), cudaMemcpyDeviceToHost, P->stream));
+    CK(cudaStreamSynchronize(P->stream));
+    out->k = h.k; out->s = h.s; out->trials = h.trials; out->n_violated = h.n_viol;
+    out->n_sets = h.n_sets; out->n_zero_norm_sets = h.n_zero;
+    out->n_active_rows = P->act.n; out->nnz = P->nnz; out->nnz_active = P->act.nnz;
+    long long b = 0;
+    const int sa_passes[] = {FREDOPT_PASS_FORWARD_X, FREDOPT_PASS_TRANSPOSE_G, FREDOPT_PASS_FORWARD_G, FREDOPT_PASS_SELECT,
+                             FREDOPT_PASS_RESIDUAL, FREDOPT_PASS_TRANSPOSE_B};
+    for (int p : sa_passes) b += P->pass_bytes[p];
+    out->alg_bytes_iter = b;
+    out->last_beta = h.last_beta; out->phi = h.phi; out->prox = h.prox; out->weight_sum = h.W;
+    return FREDOPT_OK;
+}
+
+int fredopt_get_pass_times(fredopt_plan* P, double* ms, int64_t* launches) {
+    if (!P || !ms || !launches) return FREDOPT_INVALID_ARG;
+    CK(cudaStreamSynchronize(P->stream));
+    for (auto& ep : P->events) {
+        float t = 0.f;
+        if (cudaEventElapsedTime(&t, ep.a, ep.b) == cudaSuccess) { P->pass_ms[ep.pass] += t; P->pass_launches[ep.pass] += 1; }
+        cudaEventDestroy(ep.a); cudaEventDestroy(ep.b);
+    }
+    cudaGetLastError();
+    P->events.clear();
+    for (int i = 0; i < FREDOPT_N_PASSES; ++i) { ms[i] = P->pass_ms[i]; launches[i] = P->pass_launches[i]; }
+    return FREDOPT_OK;
+}
+
+int fredopt_get_pass_bytes(fredopt_plan* P, int64_t* bytes) {
+    if (!P || !bytes) return FREDOPT_INVALID_ARG;
+    for (int i = 0; i < FREDOPT_N_PASSES; ++i) bytes[i] = P->pass_bytes[i];
+    return FREDOPT_OK;
+}
+
+int64_t fredopt_launch_count(fredopt_plan* P) { return P ? P->launches : 0; }
+
+int fredopt_stream_read(fredopt_plan* P, const void* device_buf, int64_t bytes, int32_t reps) {
+    if (!P || !device_buf || bytes < 16 || (bytes & 15) || reps < 1 || !is_device_ptr(device_buf)) return FREDOPT_INVALID_ARG;
+    for (int i = 0; i < reps; ++i) {
+        k_stream_read<<<P->sm_count * 4, 512, 0, P->stream>>>((const int4*)device_buf, bytes / 16, P->sink);
+        ++P->launches;
+    }
+    CK(cudaGetLastError());
+    return FREDOPT_OK;
+}
+
+}  // extern "C"
