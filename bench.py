@@ -1,0 +1,296 @@
+#!/usr/bin/env python
+"""bench.py -- superiorized feasibility-seeking iterations/s of the FREDopt hot path on B200.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config I] [--impl ours|reference]
+
+A STEP is one superiorized iteration (forward pass at x, transposed pass ->
+gradient, forward pass on g + accept test, residual / violation epilogue, transposed back-projection + update +
+clamp) on the synthetic plan BASELINE.json configs[I] describes.  `value` = iterations/s with the plan resident in
+HBM, timed with CUDA events on the plan's stream around one `fredopt_iterate(K)` call.  `e2e` is the same metric
+through the C-ABI with HOST buffers: every step uploads the spot weights from pinned host memory
+(fredopt_set_weights), runs fredopt_iterate(1) and reads the weights and the proximity / violation count back.
+`roofline` is for the dominant kernel: its algorithmic bytes per launch (fredopt_get_pass_bytes; DESIGN.md
+"Bytes") / its mean launch duration measured with CUDA events inside the library (FREDOPT_OPT_TIME_PASSES).
+`cpu_baseline` is the fp64 oracle (oracle/), as it stands, timed on the host cores on a bounded sample.
+
+N > 1 (torchrun): the path's units here are independent plans; every rank optimises its own copy of the plan
+(weak scaling, no data-path collective), value = all ranks' iterations / max time.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+import torch
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+METRIC = "superiorization iterations/sec"
+UNIT = "iterations/s"
+DEFAULT_CONFIG = 1
+DEFAULT_STEPS = {0: 50, 1: 200, 2: 100, 3: 50}
+
+
+def _peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        try:
+            return float(json.load(open(p))["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+        except Exception:
+            pass
+    return 6650.0, "fallback (B200_PROFILING.md: 6.65 TB/s)"
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons during the timed region (B200_PROFILING.md recipe)."""
+    Q = ("clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.rows, self.proc, self.index = [], None, index
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.Q}",
+                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.t = threading.Thread(target=self._read, daemon=True)
+            self.t.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([c.strip() for c in line.split(",")])
+
+    def stop(self):
+        if not self.proc:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except Exception:
+            self.proc.kill()
+        sm, mx, reasons = [], None, set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in self.rows:
+            try:
+                sm.append(float(r[0])); mx = float(r[1])
+            except Exception:
+                continue
+            for n, v in zip(names, r[2:6]):
+                if v.lower().startswith("active"):
+                    reasons.add(n)
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": mx, "reasons": sorted(reasons),
+                "samples": len(sm)}
+
+
+def _dist_init():
+    ws = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    lr = int(os.environ.get("LOCAL_RANK", "0"))
+    return ws, rank, lr
+
+
+# ------------------------------------------------------------------------------------------------ reference arm
+def run_reference(args):
+    """The oracle, as it stands, on the host cores: a bounded sample of the same workload per step."""
+    ws, rank, _ = _dist_init()
+    if rank != 0:
+        return
+    from oracle import oracle
+    from paper_2509_20012_b200 import plangen as pg
+    spec = pg.config_spec(args.config)
+    plan = pg.build_plan(spec, device="cuda" if torch.cuda.is_available() else "cpu")
+    orc = oracle.from_plan(plan)
+    orc.set_x(plan.x0)
+    K, W = args.steps, args.warmup
+    orc.iterate(W, spec.lam, spec.beta0, spec.a)
+    t0 = time.perf_counter()
+    orc.iterate(K, spec.lam, spec.beta0, spec.a)
+    dt = time.perf_counter() - t0
+    v = K / dt
+    sample = f"{K} superiorized iterations of configs[{args.config}] ({spec.name}), full plan, after {W} warm-up iterations"
+    print(json.dumps({
+        "impl": "reference", "metric": METRIC, "value": v, "unit": UNIT, "n_gpus": args.gpus, "steps": K, "warmup": W,
+        "ms_per_step": 1e3 * dt / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+        "data": "synthetic", "config": {"workload": f"configs[{args.config}] {spec.name}", "nnz": plan.nnz,
+                                        "n_spots": plan.n_cols, "n_voxels": plan.n_rows},
+        "cpu_baseline": {"value": v, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
+        "e2e": {"value": v, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0}))
+
+
+# ------------------------------------------------------------------------------------------------ our arm
+def run_ours(args):
+    ws, rank, lr = _dist_init()
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the hot path has no CPU fallback")
+    torch.cuda.set_device(lr)
+    dist = None
+    if ws > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", lr))
+    from paper_2509_20012_b200 import fredopt, plangen as pg
+
+    spec = pg.config_spec(args.config)
+    t0 = time.perf_counter()
+    plan = pg.build_plan(spec, device="cuda")
+    torch.cuda.synchronize()
+    t_gen = time.perf_counter() - t0
+    stream = torch.cuda.current_stream()
+    t0 = time.perf_counter()
+    gp = fredopt.from_plan(plan, stream=stream.cuda_stream)
+    torch.cuda.synchronize()
+    t_create = time.perf_counter() - t0
+    st0 = gp.stats()
+    K, W = args.steps, args.warmup
+    lam, beta0, a = spec.lam, spec.beta0, spec.a
+    pass_bytes = gp.pass_bytes()
+    iter_bytes = st0["alg_bytes_iter"]
+    l2_bytes = torch.cuda.get_device_properties(lr).L2_cache_size
+    flush = None
+    if iter_bytes < 2 * l2_bytes:
+        flush = torch.empty(int(1.5 * l2_bytes), dtype=torch.uint8, device="cuda")
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    # ---- device-resident timing: W warm-up iterations, then K iterations in one fredopt_iterate call
+    gp.set_weights(plan.x0)
+    gp.iterate(W, lam, beta0, a)
+    if flush is not None:
+        flush.zero_()
+    barrier()
+    sampler = ClockSampler(lr)
+    sampler.start()
+    l0 = gp.launch_count()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record(stream)
+    gp.iterate(K, lam, beta0, a)
+    e1.record(stream)
+    barrier()
+    launches = gp.launch_count() - l0
+    ms = e0.elapsed_time(e1)
+    # ---- end to end: host buffers, copies inside the timed region, every step
+    xh = torch.from_numpy(plan.x0.copy()).pin_memory()
+    xo = torch.empty_like(xh).pin_memory()
+    gp.set_option(fredopt.OPT_RESET, 1)
+    for _ in range(W):
+        gp.set_weights(xh); gp.iterate(1, lam, beta0, a); gp.get_weights(xo); xh.copy_(xo)
+    barrier()
+    t0 = time.perf_counter()
+    for _ in range(K):
+        gp.set_weights(xh)                    # H2D: S floats from pinned host memory
+        gp.iterate(1, lam, beta0, a)
+        gp.get_weights(xo)                    # D2H: S floats (synchronises)
+        prox, nviol = gp.proximity(None)      # D2H: the step's metric (fp64 + int64)
+        xh.copy_(xo)
+    barrier()
+    e2e_s = time.perf_counter() - t0
+    clocks = sampler.stop()
+    # ---- per-kernel durations (CUDA events inside the library, on the plan's stream)
+    gp.set_option(fredopt.OPT_RESET, 1)
+    gp.set_weights(plan.x0)
+    gp.iterate(W, lam, beta0, a)
+    gp.set_option(fredopt.OPT_TIME_PASSES, 1)
+    gp.iterate(min(K, 50), lam, beta0, a)
+    pt = gp.pass_times()
+    gp.set_option(fredopt.OPT_TIME_PASSES, 0)
+    top = max(pt, key=lambda n: pt[n][0])
+    top_ms = pt[top][0] / max(pt[top][1], 1)
+    peak, peak_src = _peaks()
+    achieved = pass_bytes[top] / (top_ms * 1e-3) / 1e9
+    passes = {n: {"ms": pt[n][0] / max(pt[n][1], 1), "alg_bytes": pass_bytes[n],
+                  "gbs": pass_bytes[n] / max(pt[n][0] / max(pt[n][1], 1), 1e-9) / 1e6} for n in pt}
+    stats = gp.stats()
+
+    if dist is not None:
+        t = torch.tensor([ms, e2e_s], dtype=torch.float64, device="cuda")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms, e2e_s = float(t[0]), float(t[1])
+    if rank != 0:
+        if dist is not None:
+            dist.destroy_process_group()
+        return
+    value = ws * K / (ms * 1e-3)
+    out = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": ws, "steps": K, "warmup": W, "ms_per_step": ms / K,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64 accumulate / f32 matrix values",
+        "data": "synthetic",
+        "config": {"workload": f"configs[{args.config}] {spec.name}", "n_voxels": plan.n_rows, "n_spots": plan.n_cols,
+                   "nnz_per_matrix": plan.nnz, "nnz_active": stats["nnz_active"], "n_active_rows": stats["n_active_rows"],
+                   "n_sets": stats["n_sets"], "lambda": lam, "beta0": beta0, "a": a,
+                   "passes_per_iteration": 4, "alg_bytes_per_iteration": iter_bytes,
+                   "l2": ("L2-resident working set (%.1f MB < 2 x L2): L2 flushed once before the timed region; "
+                          "HBM fraction not meaningful" % (iter_bytes / 1e6)) if flush is not None else
+                         "inputs larger than L2 (%.2f GB streamed per iteration)" % (iter_bytes / 1e9),
+                   "parallelism": "1 plan per GPU"},
+        "iter_gbs": iter_bytes * K / (ms * 1e-3) / 1e9,
+        "e2e": {"value": ws * K / e2e_s, "unit": UNIT, "h2d_bytes_per_step": plan.n_cols * 4,
+                "d2h_bytes_per_step": plan.n_cols * 4 + 16},
+        "gpu_launches": int(launches),
+        "clocks": clocks,
+        "roofline": {"bound": "hbm", "kernel": top, "achieved": achieved, "peak": peak, "unit": "GB/s",
+                     "frac": achieved / peak, "traffic": None, "peak_source": peak_src,
+                     "alg_bytes_per_launch": pass_bytes[top], "ms_per_launch": top_ms},
+        "passes": passes,
+        "setup": {"generate_s": t_gen, "create_s": t_create},
+        "final": {"prox": prox, "n_violated": nviol, "trials": stats["trials"]},
+    }
+    if ws == 1 and not args.no_cpu_baseline:
+        out["cpu_baseline"] = cpu_baseline(plan, spec, args)
+    print(json.dumps(out))
+    if dist is not None:
+        dist.destroy_process_group()
+
+
+def cpu_baseline(plan, spec, args):
+    """The oracle as it stands, single thread, on a bounded sample (about 10-30 s) of the same workload."""
+    from oracle import oracle
+    orc = oracle.from_plan(plan)
+    orc.set_x(plan.x0)
+    t0 = time.perf_counter()
+    orc.iterate(1, spec.lam, spec.beta0, spec.a)
+    t1 = time.perf_counter() - t0
+    n = int(max(1, min(200, 15.0 / max(t1, 1e-6))))
+    t0 = time.perf_counter()
+    orc.iterate(n, spec.lam, spec.beta0, spec.a)
+    dt = time.perf_counter() - t0
+    return {"value": n / dt, "unit": UNIT, "cores": 1, "kind": "oracle",
+            "sample": f"{n} superiorized iterations of the same plan (after 1 warm-up iteration), fp64, single thread"}
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=None)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", type=int, default=DEFAULT_CONFIG)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.warmup < 3:
+        args.warmup = 3
+    if args.impl == "reference":
+        if args.steps is None:
+            args.steps = 5
+        run_reference(args)
+    else:
+        if args.steps is None:
+            args.steps = DEFAULT_STEPS.get(args.config, 50)
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

@@ -22,8 +22,9 @@
  *   - every pointer argument may be a HOST or a DEVICE pointer (detected with cudaPointerGetAttributes) unless
  *     stated otherwise; caller arrays are BORROWED for the duration of the call only; outputs are
  *     caller-allocated.  fredopt_create copies what it needs: inputs may be freed on return.
- *   - one plan = one GPU, one CUDA stream (given at creation; NULL = the legacy default stream).  Calls enqueue
- *     on that stream; a call that writes host memory synchronises the stream before returning, a call with
+ *   - one plan = one GPU, one CUDA stream (given at creation; NULL = a stream the plan creates and owns, with
+ *     cudaStreamDefault flags, i.e. ordered against the legacy default stream as any blocking stream is -- the
+ *     legacy stream itself cannot be captured into a CUDA graph).  Calls enqueue on that stream; a call that writes host memory synchronises the stream before returning, a call with
  *     device outputs only does not.
  *   - arithmetic: matrix values are stored as given (fp32), indices int32, offsets int64; every vector the
  *     iteration keeps (x, d, l, g, u, v) and every accumulator / scalar / decision is fp64 on the device.

@@ -55,6 +55,7 @@ struct EventPair { cudaEvent_t a, b; int pass; };
 
 struct fredopt_plan {
     cudaStream_t stream = nullptr;
+    bool owns_stream = false;
     int device = 0;
     long long V = 0, S = 0, nnz = 0, nnz_padded = 0;
     int n_struct = 0;
@@ -599,6 +600,7 @@ void fredopt_destroy(fredopt_plan* P) {
     for (auto& ep : P->events) { cudaEventDestroy(ep.a); cudaEventDestroy(ep.b); }
     for (int i = 0; i < 2; ++i) if (P->gexec[i]) cudaGraphExecDestroy(P->gexec[i]);
     for (void* p : P->allocs) cudaFree(p);
+    if (P->owns_stream) cudaStreamDestroy(P->stream);
     delete P;
 }
 
@@ -799,6 +801,11 @@ int fredopt_create(const fredopt_csr* D, const fredopt_csr* L, const int32_t* vo
     fredopt_plan* P = new (std::nothrow) fredopt_plan();
     if (!P) return FREDOPT_OUT_OF_MEMORY;
     P->stream = (cudaStream_t)cuda_stream;
+    if (!P->stream) {   // the legacy default stream cannot be captured into a graph: own a blocking stream instead
+        cudaError_t e = cudaStreamCreateWithFlags(&P->stream, cudaStreamDefault);
+        if (e != cudaSuccess) { delete P; CK(e); }
+        P->owns_stream = true;
+    }
     P->device = dev;
     P->sm_count = prop.multiProcessorCount;
     int rc = create_impl(P, D, L, voxel_labels, bounds, n_struct);

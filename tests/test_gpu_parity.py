@@ -1,0 +1,333 @@
+"""GPU-vs-oracle parity through the C-ABI (include/fredopt.h) on the same seeded inputs.
+
+Tolerances (BASELINE.json north_star): per SpMV relative error <= 1e-5; after 20 iterations relative L2
+error in w <= 1e-4 and an IDENTICAL constraint-violation count.  Transposed passes carry signed
+coefficients, so they are judged element-wise relative to sum_i |A_ij r_i| (parity rule).
+"""
+import numpy as np
+import pytest
+import torch
+
+from paper_2509_20012_b200 import plangen as pg
+
+pytestmark = pytest.mark.gpu
+
+TOL_SPMV = 1e-5
+TOL_X20 = 1e-4
+
+
+@pytest.fixture(scope="module")
+def fredopt():
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    from paper_2509_20012_b200 import fredopt as f
+    return f
+
+
+def _oracle(plan):
+    from oracle import oracle
+    return oracle.from_plan(plan)
+
+
+def _oracle_np(V, S, D, L, lab, bounds):
+    from oracle import oracle
+    return oracle.Oracle.create(V, S, D, L, lab, bounds)
+
+
+def _gpu_x(gp):
+    return gp.get_weights_f64(np.empty(gp.n_cols, np.float64))
+
+
+def _rel_l2(a, b):
+    return float(np.linalg.norm(a - b) / max(np.linalg.norm(b), 1e-300))
+
+
+def _assert_fwd(got, ref, what):
+    got = got.astype(np.float64)
+    # fp32 output rounding: half an ulp = 6e-8 relative; the bar is 1e-5
+    err = np.abs(got - ref)
+    bad = err > TOL_SPMV * np.abs(ref)
+    assert not bad.any(), f"{what}: max rel err {np.max(err[ref != 0] / np.abs(ref[ref != 0])):.3e}"
+    assert np.all(got[ref == 0] == 0)
+
+
+# ------------------------------------------------------------------------------------------ per pass
+def test_forward_all_rows_and_dose_let_config0(fredopt, plan0):
+    orc = _oracle(plan0)
+    gp = fredopt.from_plan(plan0)
+    x = pg.log_uniform_weights(7, plan0.n_cols)
+    d_ref, l_ref, t_ref = orc.dose_let(x.astype(np.float64))
+    d = np.full(plan0.n_rows, -1, np.float32); l = np.full(plan0.n_rows, -1, np.float32)
+    gp.spmv_forward(fredopt.ROWS_ALL, x, d, l)
+    _assert_fwd(d, d_ref, "D x")
+    _assert_fwd(l, l_ref, "L x")
+    # single-matrix passes
+    d1 = np.empty_like(d); gp.spmv_forward(fredopt.ROWS_ALL, x, d1, None)
+    l1 = np.empty_like(l); gp.spmv_forward(fredopt.ROWS_ALL, x, None, l1)
+    assert np.array_equal(d1, d) and np.array_equal(l1, l)
+    # dose_let: LETd = l / d, 0 where d = 0 (Eq. 1; reading R15)
+    dose = np.empty_like(d); letd = np.empty_like(d)
+    gp.dose_let(x, dose, letd)
+    assert np.array_equal(dose, d)
+    _assert_fwd(letd, t_ref, "LETd")
+    # device pointers give the same bits as host pointers; x = NULL uses the plan's x
+    gp.set_weights(x)
+    dd = torch.empty(plan0.n_rows, dtype=torch.float32, device="cuda"); tt = torch.empty_like(dd)
+    gp.dose_let(None, dd, tt)
+    torch.cuda.synchronize()
+    assert np.array_equal(dd.cpu().numpy(), dose) and np.array_equal(tt.cpu().numpy(), letd)
+
+
+def test_forward_active_rows_config0(fredopt, plan0):
+    orc = _oracle(plan0)
+    gp = fredopt.from_plan(plan0)
+    x = plan0.x0
+    lab = plan0.labels.numpy()
+    d_ref, l_ref, _ = orc.dose_let(x.astype(np.float64))
+    d = np.empty(plan0.n_rows, np.float32); l = np.empty(plan0.n_rows, np.float32)
+    gp.spmv_forward(fredopt.ROWS_ACTIVE, x, d, l)
+    _assert_fwd(d, np.where(lab != 0, d_ref, 0.0), "D x (active)")
+    _assert_fwd(l, np.where(lab != 0, l_ref, 0.0), "L x (active)")
+
+
+@pytest.mark.parametrize("rows", ["all", "active"])
+def test_transpose_config0(fredopt, plan0, rows):
+    orc = _oracle(plan0)
+    gp = fredopt.from_plan(plan0)
+    V = plan0.n_rows
+    # signed, dense coefficient vectors (lower-bound violations are negative)
+    u = (pg.uniform01_array(11, V) - 0.4).astype(np.float32)
+    v = (pg.uniform01_array(12, V) - 0.6).astype(np.float32)
+    sel = fredopt.ROWS_ALL if rows == "all" else fredopt.ROWS_ACTIVE
+    for uu, vv in ((u, v), (u, None), (None, v)):
+        ref, ref_abs = orc.transpose(None if uu is None else uu.astype(np.float64),
+                                     None if vv is None else vv.astype(np.float64), active_only=(rows == "active"))
+        out = np.empty(plan0.n_cols, np.float32)
+        gp.spmv_transpose(sel, uu, vv, out)
+        err = np.abs(out.astype(np.float64) - ref)
+        assert np.all(err <= TOL_SPMV * ref_abs + 1e-300), f"max {np.max(err / np.maximum(ref_abs, 1e-300)):.3e}"
+        assert _rel_l2(out.astype(np.float64), ref) <= TOL_SPMV
+
+
+def test_proximity_config0(fredopt, plan0):
+    orc = _oracle(plan0)
+    gp = fredopt.from_plan(plan0)
+    for x in (plan0.x0, pg.log_uniform_weights(3, plan0.n_cols)):
+        p_ref, n_ref = orc.proximity(x.astype(np.float64))
+        p, n = gp.proximity(x)
+        assert n == n_ref
+        assert abs(p - p_ref) <= 1e-12 * abs(p_ref)
+    st = gp.stats()
+    os_ = orc.stats()
+    assert st["n_sets"] == os_["n_sets"] and st["n_zero_norm_sets"] == os_["n_zero_norm_sets"]
+    assert abs(st["weight_sum"] - os_["W"]) <= 1e-12 * os_["W"]
+    assert st["nnz"] == plan0.nnz and st["n_active_rows"] == int((plan0.labels != 0).sum())
+
+
+# ------------------------------------------------------------------------------------------ iteration
+def _run_pair(fredopt, plan, n_iter, lam, beta0, a, opts=(), gp=None, orc=None):
+    orc = orc or _oracle(plan)
+    gp = gp or fredopt.from_plan(plan)
+    for k, v in opts:
+        orc.set_option(k, v); gp.set_option(k, v)
+    orc.set_x(plan.x0); gp.set_weights(plan.x0)
+    orc.iterate(n_iter, lam, beta0, a); gp.iterate(n_iter, lam, beta0, a)
+    return gp, orc
+
+
+def _assert_state(gp, orc, tol=TOL_X20):
+    xg, xo = _gpu_x(gp), orc.get_x()
+    assert _rel_l2(xg, xo) <= tol, f"rel L2 {_rel_l2(xg, xo):.3e}"
+    pg_, ng = gp.proximity(None)
+    po, no = orc.proximity(None)
+    assert ng == no, f"violation count {ng} vs oracle {no}"
+    assert abs(pg_ - po) <= 1e-6 * abs(po) + 1e-300
+    sg, so = gp.stats(), orc.stats()
+    assert sg["k"] == so["k"] and sg["s"] == so["s"] and sg["trials"] == so["trials"]
+    if so["last_beta"]:
+        assert abs(sg["last_beta"] - so["last_beta"]) <= 1e-15 * so["last_beta"]
+
+
+@pytest.mark.parametrize("n_iter", [1, 20, 50])
+def test_superiorized_iterations_config0(fredopt, plan0, n_iter):
+    sp = plan0.spec
+    gp, orc = _run_pair(fredopt, plan0, n_iter, sp.lam, sp.beta0, sp.a)
+    _assert_state(gp, orc)
+    assert (_gpu_x(gp) >= 0).all()
+
+
+@pytest.mark.parametrize("lam", [0.5, 1.0, 1.9, 2.0])
+def test_pure_feasibility_seeking_config0(fredopt, plan0, lam):
+    gp, orc = _run_pair(fredopt, plan0, 20, lam, 0.0, 0.5)
+    _assert_state(gp, orc)
+    assert gp.stats()["s"] == 0
+
+
+def test_violation_count_identical_every_iteration_config0(fredopt, plan0):
+    orc = _oracle(plan0); gp = fredopt.from_plan(plan0)
+    orc.set_x(plan0.x0); gp.set_weights(plan0.x0)
+    for _ in range(30):
+        orc.iterate(1, 1.0, 1.0, 0.99); gp.iterate(1, 1.0, 1.0, 0.99)
+        assert gp.proximity(None)[1] == orc.proximity(None)[1]
+
+
+def test_options_eta_reductions_accept_maxtrials(fredopt, plan0):
+    f = fredopt
+    for opts in ([(f.OPT_ETA, 0.9)], [(f.OPT_REDUCTIONS, 3)], [(f.OPT_ACCEPT_CHECK, 0)],
+                 [(f.OPT_ETA, 0.95), (f.OPT_REDUCTIONS, 2)]):
+        gp, orc = _run_pair(fredopt, plan0, 12, 1.3, 1.0, 0.9, opts)
+        _assert_state(gp, orc)
+    # a cost step far too large: every trial up to the cap is rejected, x is kept, s still advances (R10)
+    gp, orc = _run_pair(fredopt, plan0, 2, 1.0, 1.0e6, 0.999, [(f.OPT_MAX_TRIALS, 5)])
+    _assert_state(gp, orc)
+    assert gp.stats()["s"] == 10
+
+
+def test_state_two_calls_equal_one_and_graph_equals_launches(fredopt, plan0):
+    f = fredopt
+    a = f.from_plan(plan0); a.set_weights(plan0.x0); a.iterate(20, 1.0, 1.0, 0.99)
+    b = f.from_plan(plan0); b.set_weights(plan0.x0); b.iterate(10, 1.0, 1.0, 0.99); b.iterate(10, 1.0, 1.0, 0.99)
+    c = f.from_plan(plan0); c.set_option(f.OPT_USE_GRAPH, 0); c.set_weights(plan0.x0); c.iterate(20, 1.0, 1.0, 0.99)
+    xa, xb, xc = _gpu_x(a), _gpu_x(b), _gpu_x(c)
+    assert np.array_equal(xa, xb) and np.array_equal(xa, xc)      # no atomics: bitwise reproducible
+    # RESET restarts beta at beta0
+    a.set_option(f.OPT_RESET, 1); a.set_weights(plan0.x0); a.iterate(20, 1.0, 1.0, 0.99)
+    assert np.array_equal(_gpu_x(a), xa)
+    assert a.launch_count() > 0
+
+
+def test_rejected_trials_multi_beam(fredopt):
+    """Three beams: the first iterations reject many step sizes (reading R8); the device-side accept loop must
+    consume exactly the trials the oracle's literal re-evaluation consumes."""
+    plan = pg.build_plan(pg.config_spec(2, scale=0.25), device="cuda")
+    gp, orc = _run_pair(fredopt, plan, 20, 1.0, 1.0, 0.99)
+    assert orc.stats()["trials"] > 20
+    _assert_state(gp, orc)
+
+
+# ------------------------------------------------------------------------------------------ small / ragged / degenerate
+@pytest.mark.parametrize("seed,same", [(1, True), (2, False), (5, False)])
+def test_random_small_plans_union_pattern(fredopt, seed, same):
+    V, S = 300, 37
+    D, L, lab, x0 = pg.random_small_plan(seed, V=V, S=S, n_struct=3, density=0.3, same_pattern=same)
+    nan = np.nan
+    bounds = np.array([[1.0, 0.5, 0.9, nan, nan, nan, 0.7, nan],
+                       [2.0, nan, 0.4, nan, 1.5, 3.0, nan, 1.5],
+                       [0.5, 0.1, nan, 0.2, 2.0, nan, 0.3, 1.0]], np.float32)
+    orc = _oracle_np(V, S, D, L, lab, bounds)
+    gp = fredopt.Plan(V, S, D, L, lab, bounds)
+    x = x0
+    d_ref, l_ref, _ = orc.dose_let(x.astype(np.float64))
+    d = np.empty(V, np.float32); l = np.empty(V, np.float32)
+    gp.spmv_forward(fredopt.ROWS_ALL, x, d, l)
+    _assert_fwd(d, d_ref, "D x"); _assert_fwd(l, l_ref, "L x")
+    orc.set_x(x0); gp.set_weights(x0)
+    orc.iterate(20, 1.5, 0.5, 0.8); gp.iterate(20, 1.5, 0.5, 0.8)
+    _assert_state(gp, orc)
+
+
+def test_degenerate_inputs(fredopt):
+    f = fredopt
+    nan = np.nan
+    b1 = np.array([[1.0, nan, 1.0, nan, nan, nan, nan, nan]], np.float32)
+    # all rows empty: nothing participates, x is unchanged, a violated lower bound on an unreachable voxel is counted (R14)
+    V, S = 5, 3
+    rp = np.zeros(V + 1, np.int64); ci = np.zeros(0, np.int32); vv = np.zeros(0, np.float32)
+    lab = np.array([0, 1, 1, 0, 1], np.int32)
+    blo = np.array([[1.0, 0.5, nan, nan, nan, nan, nan, nan]], np.float32)
+    gp = f.Plan(V, S, (rp, ci, vv), (rp, ci, vv), lab, blo)
+    x = np.array([1, 2, 3], np.float32)
+    gp.set_weights(x); gp.iterate(3, 1.0, 1.0, 0.5)
+    assert np.array_equal(_gpu_x(gp), x.astype(np.float64))
+    assert gp.proximity(None) == (0.0, 3)
+    orc = _oracle_np(V, S, (rp, ci, vv), (rp, ci, vv), lab, blo)
+    orc.set_x(x); orc.iterate(3, 1.0, 1.0, 0.5)
+    assert orc.proximity(None) == (0.0, 3)
+    # no labelled voxel / no structure
+    rp = np.array([0, 2, 2, 3], np.int64); ci = np.array([0, 1, 1], np.int32); vv = np.array([1, 2, 3], np.float32)
+    gp = f.Plan(3, 2, (rp, ci, vv), (rp, ci, vv), np.zeros(3, np.int32), np.zeros((0, 8), np.float32))
+    gp.set_weights(np.array([1, 1], np.float32)); gp.iterate(2, 1.0, 0.0, 0.5)
+    d = np.empty(3, np.float32); gp.spmv_forward(f.ROWS_ALL, None, d, None)
+    assert np.array_equal(d, np.array([3, 0, 3], np.float32))
+    # one very long row (several 256-entry tiles and a ragged tail) and rows of length 1..9
+    S = 3001
+    lens = [S, 1, 2, 3, 4, 5, 6, 7, 8, 9, 0, 257, 511]
+    rp = np.concatenate([[0], np.cumsum(lens)]).astype(np.int64)
+    ci = np.concatenate([np.arange(n, dtype=np.int32) * (S // max(n, 1)) for n in lens]).astype(np.int32)
+    vv = (0.1 + pg.uniform01_array(9, int(rp[-1]))).astype(np.float32)
+    vl = (vv * (2 + pg.uniform01_array(10, int(rp[-1])))).astype(np.float32)
+    lab = np.ones(len(lens), np.int32)
+    b = np.array([[1.0, 1.0, 2.0, nan, 30.0, 3.0, 1.5, nan]], np.float32)
+    gp = f.Plan(len(lens), S, (rp, ci, vv), (rp, ci, vl), lab, b)
+    orc = _oracle_np(len(lens), S, (rp, ci, vv), (rp, ci, vl), lab, b)
+    x0 = pg.log_uniform_weights(4, S)
+    orc.set_x(x0); gp.set_weights(x0)
+    orc.iterate(20, 1.0, 0.3, 0.9); gp.iterate(20, 1.0, 0.3, 0.9)
+    _assert_state(gp, orc)
+
+
+def test_invalid_arguments(fredopt):
+    f = fredopt
+    nan = np.nan
+    rp = np.array([0, 2, 3], np.int64); ci = np.array([0, 1, 1], np.int32); vv = np.array([1, 2, 3], np.float32)
+    lab = np.array([1, 0], np.int32)
+    b = np.array([[1.0, nan, 1.0, nan, nan, nan, nan, nan]], np.float32)
+
+    def bad(**kw):
+        a = dict(rp=rp, ci=ci, vv=vv, lab=lab, b=b)
+        a.update(kw)
+        with pytest.raises(f.FredoptError) as e:
+            f.Plan(2, 2, (a["rp"], a["ci"], a["vv"]), (a["rp"], a["ci"], a["vv"]), a["lab"], a["b"])
+        assert e.value.code == f.INVALID_ARG
+
+    bad(rp=np.array([0, 3, 2], np.int64))                      # decreasing row_ptr
+    bad(rp=np.array([1, 2, 3], np.int64))                      # row_ptr[0] != 0
+    bad(ci=np.array([1, 0, 1], np.int32))                      # unsorted columns
+    bad(ci=np.array([0, 0, 1], np.int32))                      # duplicate column
+    bad(ci=np.array([0, 2, 1], np.int32))                      # column out of range
+    bad(vv=np.array([1, np.inf, 3], np.float32))               # non-finite value
+    bad(lab=np.array([2, 0], np.int32))                        # label outside 0..n_struct
+    bad(b=np.array([[0.0, nan, 1.0, nan, nan, nan, nan, nan]], np.float32))    # weight <= 0
+    bad(b=np.array([[1.0, 2.0, 1.0, nan, nan, nan, nan, nan]], np.float32))    # lo > hi
+    gp = f.Plan(2, 2, (rp, ci, vv), (rp, ci, vv), lab, b)
+    x = np.array([1, 1], np.float32); gp.set_weights(x)
+    for args in ((-1, 1.0, 1.0, 0.5), (1, 0.0, 1.0, 0.5), (1, 2.5, 1.0, 0.5), (1, 1.0, -1.0, 0.5), (1, 1.0, 1.0, 1.0),
+                 (1, 1.0, 1.0, 0.0)):
+        with pytest.raises(f.FredoptError):
+            gp.iterate(*args)
+    assert np.array_equal(_gpu_x(gp), x.astype(np.float64))    # state untouched on failure
+    with pytest.raises(f.FredoptError):
+        gp.set_option(99, 1.0)
+
+
+# ------------------------------------------------------------------------------------------ BASELINE configs[1]: the bench workload
+@pytest.fixture(scope="module")
+def plan1_dev():
+    return pg.build_plan(pg.config_spec(1), device="cuda")
+
+
+def test_config1_20_iterations_in_bench_configuration(fredopt, plan1_dev):
+    """Full size of the workload bench.py times (configs[1]), same launch configuration (graph replay)."""
+    plan = plan1_dev
+    gp = fredopt.from_plan(plan, stream=torch.cuda.current_stream().cuda_stream)
+    orc = _oracle(plan)
+    sp = plan.spec
+    orc.set_x(plan.x0); gp.set_weights(plan.x0)
+    orc.iterate(20, sp.lam, sp.beta0, sp.a); gp.iterate(20, sp.lam, sp.beta0, sp.a)
+    _assert_state(gp, orc)
+    # sampled outputs of the full forward pass, computed one by one by the oracle
+    x = pg.log_uniform_weights(21, plan.n_cols)
+    dose = torch.empty(plan.n_rows, dtype=torch.float32, device="cuda"); letd = torch.empty_like(dose)
+    gp.dose_let(torch.from_numpy(x).cuda(), dose, letd)
+    torch.cuda.synchronize()
+    nz = (plan.row_ptr[1:] > plan.row_ptr[:-1]).nonzero().reshape(-1).cpu().numpy()
+    rows = nz[(pg.uniform01_array(22, 4000) * len(nz)).astype(np.int64)]
+    d_ref, _, t_ref = orc.dose_let_rows(rows, x.astype(np.float64))
+    _assert_fwd(dose.cpu().numpy()[rows], d_ref, "dose (sampled)")
+    _assert_fwd(letd.cpu().numpy()[rows], t_ref, "LETd (sampled)")
+    # transposed pass over all rows, full size
+    V = plan.n_rows
+    u = (pg.uniform01_array(31, V) - 0.4).astype(np.float32); v = (pg.uniform01_array(32, V) - 0.6).astype(np.float32)
+    ref, ref_abs = orc.transpose(u.astype(np.float64), v.astype(np.float64))
+    out = np.empty(plan.n_cols, np.float32)
+    gp.spmv_transpose(fredopt.ROWS_ALL, u, v, out)
+    assert np.all(np.abs(out - ref) <= TOL_SPMV * ref_abs)
