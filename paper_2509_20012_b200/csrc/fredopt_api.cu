@@ -32,14 +32,28 @@ static thread_local std::string g_last_cuda_error;
     } while (0)
 
 // ============================================================================================ plan
+// view of a row set for the create-time kernels
+struct RowList {
+    long long n;                 // rows in the list
+    const long long* start;      // [n] offset of the row in the set's padded arrays (multiple of 4)
+    const int32_t* len;          // [n] padded length (multiple of 4)
+    const int32_t* seg;          // [n] segment (structure - 1), or nullptr = segment 0
+    const int32_t* vox;          // [n] voxel index of the row
+};
+
 struct RowSet {
     long long n = 0;                 // rows
     int n_seg = 1;
+    // padded index / value arrays of the set (rows stored back to back in list order)
+    int32_t* col = nullptr;
+    float* valD = nullptr;
+    float* valL = nullptr;
     int32_t* vox = nullptr;          // [n]
     int32_t* seg = nullptr;          // [n] or nullptr
     long long* start = nullptr;      // [n]
     int32_t* len = nullptr;          // [n] padded
     int32_t* ulen = nullptr;         // [n] unpadded
+    Item* items = nullptr;           // [n] {start, len, seg}: what the forward kernel reads
     long long nnz = 0;               // unpadded entries in the set
     // CSR of the transposes restricted to this set: rows = spots, per-segment runs, columns = list index
     bool t_built = false;
@@ -48,6 +62,13 @@ struct RowSet {
     float* t_valD = nullptr;
     float* t_valL = nullptr;
     long long t_nnz_padded = 0;
+    // work items of the transposed pass: runs cut into pieces of at most TR_ITEM_MAX entries
+    long long t_n_items = 0;
+    Item* t_items = nullptr;         // [t_n_items]
+    int32_t* t_item_spot = nullptr;  // [t_n_items]
+    long long* t_item_ptr = nullptr; // [S+1] items of spot j: t_item_ptr[j] .. t_item_ptr[j+1]-1
+    double* t_partial = nullptr;     // [t_n_items]
+    unsigned int* t_counter = nullptr;  // [S] arrival counters (0 between launches)
     RowList view() const { return RowList{n, start, len, seg, vox}; }
 };
 
@@ -60,10 +81,8 @@ struct fredopt_plan {
     long long V = 0, S = 0, nnz = 0, nnz_padded = 0;
     int n_struct = 0;
     std::vector<void*> allocs;
-    // padded matrix (union pattern), all non-empty rows
-    int32_t* col = nullptr;
-    float* valD = nullptr;
-    float* valL = nullptr;
+    // full: all non-empty rows of the padded matrix (union pattern); act: a compact copy of the rows with a label,
+    // ordered by (structure, voxel)
     RowSet full, act;
     // per active row
     double *nD = nullptr, *nL = nullptr, *nT = nullptr;
@@ -72,12 +91,12 @@ struct fredopt_plan {
     std::vector<StructInfo> h_tab;
     uint8_t *mode_union = nullptr, *mode_con = nullptr, *mode_cost = nullptr, *mode_fixed = nullptr;  // mode_fixed: [4][max_seg]
     int max_seg = 1;
-    SegCoef *coef_cost = nullptr, *coef_unit = nullptr;
     DevState* st = nullptr;
     // vectors (fp64)
     double *x = nullptr, *g = nullptr, *xtmp = nullptr;                       // [S]
-    double *d = nullptr, *l = nullptr, *Dg = nullptr, *Lg = nullptr, *u = nullptr, *v = nullptr;   // [VA]
-    double *fullD = nullptr, *fullL = nullptr;                                 // lazily: [full.n] gather vectors for ROWS_ALL transposes
+    double *d = nullptr, *l = nullptr, *Dg = nullptr, *Lg = nullptr;          // [VA]
+    double2 *pq = nullptr, *uv = nullptr;                                      // [VA] gather vectors of the transposed passes
+    double2* fullUV = nullptr;                                                 // lazily: [full.n] gather vector for ROWS_ALL transposes
     double* cpart = nullptr;
     double *part_prox = nullptr, *part_phi = nullptr;
     long long* part_cnt = nullptr;
@@ -298,7 +317,7 @@ __global__ void k_count_sets(long long n, const int32_t* seg, const int32_t* ule
 
 // W = sum_s w_s * part_s (s ascending), w^_s = w_s / W; pass modes and transposed-pass coefficients
 __global__ void k_finish_tables(StructInfo* tab, int n_struct, DevState* st, uint8_t* mode_union, uint8_t* mode_con,
-                                uint8_t* mode_cost, uint8_t* mode_fixed, int max_seg, SegCoef* coef_cost, SegCoef* coef_unit) {
+                                uint8_t* mode_cost, uint8_t* mode_fixed, int max_seg) {
     if (threadIdx.x != 0 || blockIdx.x != 0) return;
     double W = 0.0;
     long long ns = 0, nz = 0;
@@ -312,11 +331,8 @@ __global__ void k_finish_tables(StructInfo* tab, int n_struct, DevState* st, uin
         mode_cost[s] = (uint8_t)cost;
         mode_con[s] = (uint8_t)con;
         mode_union[s] = (uint8_t)(cost | con);
-        coef_cost[s] = SegCoef{(f & F_DOSE_REF) ? 2.0 * T.what : 0.0, (f & F_DOSE_REF) ? T.dose_ref : 0.0,
-                               (f & F_DL_REF) ? 2.0 * T.what : 0.0, (f & F_DL_REF) ? T.dl_ref : 0.0};
     }
     for (int s = 0; s < max_seg; ++s) {
-        coef_unit[s] = SegCoef{1.0, 0.0, 1.0, 0.0};
         for (int m = 0; m < 4; ++m) mode_fixed[m * max_seg + s] = (uint8_t)m;
     }
     st->W = W; st->n_sets = ns; st->n_zero = nz;
@@ -363,6 +379,36 @@ __global__ void k_tr_fill(const uint32_t* keys, const uint32_t* vals, long long 
         tD[dst] = vD[p];
         tL[dst] = vL[p];
     }
+}
+// {start, len, seg} -> the 16-byte item the hot kernels read
+__global__ void k_pack_items(long long n, const long long* start, const int32_t* len, const int32_t* seg, Item* items) {
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (long long)gridDim.x * blockDim.x) {
+        Item it;
+        it.start = start[i]; it.len = len[i]; it.seg = seg ? seg[i] : 0;
+        items[i] = it;
+    }
+}
+// items per (spot, segment) run: ceil(padded length / TR_ITEM_MAX)
+__global__ void k_tr_item_count(const long long* t_ptr, long long K, long long* cnt) {
+    for (long long k = (long long)blockIdx.x * blockDim.x + threadIdx.x; k < K; k += (long long)gridDim.x * blockDim.x)
+        cnt[k] = (t_ptr[k + 1] - t_ptr[k] + TR_ITEM_MAX - 1) / TR_ITEM_MAX;
+}
+__global__ void k_tr_item_fill(const long long* t_ptr, const long long* ibase, long long K, int n_seg, Item* items,
+                               int32_t* item_spot) {
+    for (long long k = (long long)blockIdx.x * blockDim.x + threadIdx.x; k < K; k += (long long)gridDim.x * blockDim.x) {
+        const long long b = t_ptr[k], e = t_ptr[k + 1];
+        long long i = ibase[k];
+        for (long long p = b; p < e; p += TR_ITEM_MAX, ++i) {
+            Item it;
+            it.start = p; it.len = (int32_t)((e - p) < TR_ITEM_MAX ? (e - p) : TR_ITEM_MAX); it.seg = (int32_t)(k % n_seg);
+            items[i] = it;
+            item_spot[i] = (int32_t)(k / n_seg);
+        }
+    }
+}
+__global__ void k_tr_item_ptr(const long long* ibase, long long S, int n_seg, long long* item_ptr) {
+    for (long long j = (long long)blockIdx.x * blockDim.x + threadIdx.x; j <= S; j += (long long)gridDim.x * blockDim.x)
+        item_ptr[j] = ibase[j * n_seg];
 }
 __global__ void k_i32_to_i64(const int32_t* in, long long* out, long long n) {
     for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (long long)gridDim.x * blockDim.x) out[i] = in[i];
@@ -423,7 +469,7 @@ static int build_transpose(fredopt_plan* P, RowSet& R) {
     CKC(cudaMalloc(&keys, En * 4)); CKC(cudaMalloc(&vals, En * 4));
     CKC(cudaMalloc(&keys2, En * 4)); CKC(cudaMalloc(&vals2, En * 4));
     CKC(cudaMalloc(&ustart, (K + 2) * sizeof(long long))); CKC(cudaMalloc(&pcount, (K + 2) * sizeof(long long)));
-    if (n) k_tr_keys<<<grid_for(n * 32, 256, 1 << 16), 256, 0, st>>>(R.view(), R.ulen, off, P->col, R.n_seg, keys, vals);
+    if (n) k_tr_keys<<<grid_for(n * 32, 256, 1 << 16), 256, 0, st>>>(R.view(), R.ulen, off, R.col, R.n_seg, keys, vals);
     int bits = 1;
     while ((1LL << bits) < K) ++bits;
     size_t tb = 0;
@@ -445,8 +491,22 @@ static int build_transpose(fredopt_plan* P, RowSet& R) {
     CKC(cudaMemsetAsync(R.t_col, 0, Tn * 4, st));
     CKC(cudaMemsetAsync(R.t_valD, 0, Tn * 4, st));
     CKC(cudaMemsetAsync(R.t_valL, 0, Tn * 4, st));
-    if (E) k_tr_fill<<<grid_for(E, 256, 1 << 16), 256, 0, st>>>(keys2, vals2, E, ustart, R.t_ptr, off, n, R.start, P->valD, P->valL,
+    if (E) k_tr_fill<<<grid_for(E, 256, 1 << 16), 256, 0, st>>>(keys2, vals2, E, ustart, R.t_ptr, off, n, R.start, R.valD, R.valL,
                                                              R.t_col, R.t_valD, R.t_valL);
+    CKC(cudaGetLastError());
+    // ---- work items: every (spot, segment) run cut into pieces of at most TR_ITEM_MAX entries
+    CKC(cudaMemsetAsync(pcount, 0, (K + 2) * sizeof(long long), st));
+    k_tr_item_count<<<grid_for(K, 256, 4096), 256, 0, st>>>(R.t_ptr, K, pcount);
+    ret = scan_exclusive(P, pcount, ustart, K + 1);      // ustart now = first item of each run
+    if (ret) { cleanup(); return ret; }
+    CKC(cudaMemcpyAsync(&R.t_n_items, ustart + K, sizeof(long long), cudaMemcpyDeviceToHost, st));
+    CKC(cudaStreamSynchronize(st));
+    if ((ret = dmalloc(P, &R.t_items, (size_t)R.t_n_items)) || (ret = dmalloc(P, &R.t_item_spot, (size_t)R.t_n_items)) ||
+        (ret = dmalloc(P, &R.t_item_ptr, (size_t)S + 1)) || (ret = dmalloc(P, &R.t_partial, (size_t)R.t_n_items)) ||
+        (ret = dmalloc(P, &R.t_counter, (size_t)S))) { cleanup(); return ret; }
+    CKC(cudaMemsetAsync(R.t_counter, 0, (S ? S : 1) * sizeof(unsigned int), st));
+    k_tr_item_fill<<<grid_for(K, 256, 4096), 256, 0, st>>>(R.t_ptr, ustart, K, R.n_seg, R.t_items, R.t_item_spot);
+    k_tr_item_ptr<<<grid_for(S + 1, 256, 4096), 256, 0, st>>>(ustart, S, R.n_seg, R.t_item_ptr);
     CKC(cudaGetLastError());
     CKC(cudaStreamSynchronize(st));
     cleanup();
@@ -497,42 +557,51 @@ static void ev_end(fredopt_plan* P) {
     cudaEventRecord(P->events.back().b, P->stream);
 }
 
+// grid of the item kernels: one warp per item up to FWD_CTAS_PER_SM resident-CTA-fulls per SM (then round-robin)
+constexpr int FWD_CTAS_PER_SM = 6;   // 2 waves of the 3 CTAs an SM holds (launch bounds of k_forward / k_transpose)
 static int fwd_grid(fredopt_plan* P, long long n) {
-    const int cap = P->sm_count * 8 < MAX_PARTIALS ? P->sm_count * 8 : MAX_PARTIALS;
+    const int cap = P->sm_count * FWD_CTAS_PER_SM < MAX_PARTIALS ? P->sm_count * FWD_CTAS_PER_SM : MAX_PARTIALS;
     return grid_for(n, FWD_WARPS, cap);
 }
 
-static void launch_forward_store(fredopt_plan* P, const RowSet& R, const uint8_t* mode, const double* x, double* oD, double* oL,
-                                 bool cpart) {
-    if (R.n == 0) { if (cpart) cudaMemsetAsync(P->cpart, 0, sizeof(double) * MAX_PARTIALS, P->stream); return; }
+// epi: EPI_STORE (d, l), EPI_STORE_PQ (d, l and the cost residuals p, q), EPI_CPART (Dg, Lg and partial sums of c)
+static void launch_forward(fredopt_plan* P, const RowSet& R, const uint8_t* mode, const double* x, double* oD, double* oL, int epi) {
+    if (R.n == 0) { if (epi == EPI_CPART) cudaMemsetAsync(P->cpart, 0, sizeof(double) * MAX_PARTIALS, P->stream); return; }
     const int g = fwd_grid(P, R.n);
-    if (cpart) {
-        k_forward<EPI_CPART><<<g, FWD_THREADS, 0, P->stream>>>(R.view(), mode, P->col, P->valD, P->valL, x, oD, oL, P->tab, P->cpart,
-                                                               nullptr, nullptr, 0);
-    } else
-        k_forward<EPI_STORE><<<g, FWD_THREADS, 0, P->stream>>>(R.view(), mode, P->col, P->valD, P->valL, x, oD, oL, nullptr, nullptr,
-                                                               nullptr, nullptr, 0);
+    if (epi == EPI_CPART)
+        k_forward<EPI_CPART><<<g, FWD_THREADS, 0, P->stream>>>(R.n, R.items, R.vox, mode, R.col, R.valD, R.valL, x, oD, oL, nullptr,
+                                                               P->tab, P->cpart, nullptr, nullptr, 0);
+    else if (epi == EPI_STORE_PQ)
+        k_forward<EPI_STORE_PQ><<<g, FWD_THREADS, 0, P->stream>>>(R.n, R.items, R.vox, mode, R.col, R.valD, R.valL, x, oD, oL, P->pq,
+                                                                  P->tab, nullptr, nullptr, nullptr, 0);
+    else
+        k_forward<EPI_STORE><<<g, FWD_THREADS, 0, P->stream>>>(R.n, R.items, R.vox, mode, R.col, R.valD, R.valL, x, oD, oL, nullptr,
+                                                               nullptr, nullptr, nullptr, nullptr, 0);
     ++P->launches;
 }
+static int cpart_count(fredopt_plan* P) { return P->act.n ? fwd_grid(P, P->act.n) : MAX_PARTIALS; }
 
 template <int EPI>
-static void launch_transpose(fredopt_plan* P, const RowSet& R, const uint8_t* mode, const SegCoef* coef, const double* vecD,
-                             const double* vecL, double* g_out, double* x, float* f_out) {
-    if (P->S == 0) return;
-    k_transpose<EPI><<<(unsigned)P->S, TR_THREADS, 0, P->stream>>>(R.n_seg, R.t_ptr, R.t_col, R.t_valD, R.t_valL, mode, coef, vecD,
-                                                                  vecL, g_out, x, P->st, f_out);
+static void launch_transpose(fredopt_plan* P, const RowSet& R, const uint8_t* mode, const double2* vec, double* g_out, double* x,
+                             float* f_out) {
+    if (R.t_n_items == 0) return;
+    k_transpose<EPI><<<fwd_grid(P, R.t_n_items), FWD_THREADS, 0, P->stream>>>(R.t_n_items, R.t_items, R.t_item_spot, R.t_item_ptr, mode,
+                                                                             R.t_col, R.t_valD, R.t_valL, vec, R.t_partial, R.t_counter,
+                                                                             g_out, x, P->st, f_out);
     ++P->launches;
 }
 
 static int res_grid(fredopt_plan* P) {
     const int cap = P->sm_count * 4 < MAX_PARTIALS ? P->sm_count * 4 : MAX_PARTIALS;
-    return grid_for(P->act.n, ROW_THREADS, cap);
+    const long long n = P->act.n > P->S ? P->act.n : P->S;
+    return grid_for(n, ROW_THREADS, cap);
 }
 
 static void launch_residual(fredopt_plan* P, double* d, double* l, int use_beta, int final, int write_uv) {
     const int g = res_grid(P);
-    k_residual<<<g, ROW_THREADS, 0, P->stream>>>(P->act.n, P->act.seg, P->tab, P->st, d, l, P->Dg, P->Lg, P->nD, P->nL, P->nT, P->u,
-                                                 P->v, P->part_prox, P->part_phi, P->part_cnt, use_beta, final, write_uv);
+    k_residual<<<g, ROW_THREADS, 0, P->stream>>>(P->act.n, P->act.items, P->tab, P->st, d, l, P->Dg, P->Lg, P->nD, P->nL, P->nT, P->uv,
+                                                 P->pq, P->x, P->g, P->S, P->part_prox, P->part_phi, P->part_cnt, use_beta, final,
+                                                 write_uv);
     ++P->launches;
 }
 
@@ -546,34 +615,34 @@ static int enqueue_iteration(fredopt_plan* P, bool sa) {
     const long long before = P->launches;
     if (sa) {
         ev_begin(P, FREDOPT_PASS_FORWARD_X);
-        launch_forward_store(P, P->act, P->mode_union, P->x, P->d, P->l, false);                       // a1: d = Dx, l = Lx
+        launch_forward(P, P->act, P->mode_union, P->x, P->d, P->l, EPI_STORE_PQ);                      // a1, a2: d, l, p, q
         ev_end(P);
         for (long long t = 0; t < P->reductionsN; ++t) {
             ev_begin(P, FREDOPT_PASS_TRANSPOSE_G);
-            launch_transpose<TEPI_GRAD>(P, P->act, P->mode_cost, P->coef_cost, P->d, P->l, P->g, nullptr, nullptr);   // a3: g
+            launch_transpose<TEPI_GRAD>(P, P->act, P->mode_cost, P->pq, P->g, nullptr, nullptr);       // a3: g = D^T p + L^T q
             ev_end(P);
             ev_begin(P, FREDOPT_PASS_FORWARD_G);
-            launch_forward_store(P, P->act, P->mode_union, P->g, P->Dg, P->Lg, true);                  // a5: Dg, Lg, c
+            launch_forward(P, P->act, P->mode_union, P->g, P->Dg, P->Lg, EPI_CPART);                   // a5: Dg, Lg, c
             ev_end(P);
             ev_begin(P, FREDOPT_PASS_SELECT);
-            k_select<<<1, 1024, 0, P->stream>>>(P->st, P->g, P->x, P->S, P->cpart, MAX_PARTIALS);      // a4, a6
+            k_select<<<1, 1024, 0, P->stream>>>(P->st, P->g, P->S, P->cpart, cpart_count(P));          // a4, a6: beta
             ++P->launches;
             ev_end(P);
             ev_begin(P, FREDOPT_PASS_RESIDUAL);
             const int last = t == P->reductionsN - 1;
-            launch_residual(P, P->d, P->l, 1, last, last);                                             // a7 (and d', l')
+            launch_residual(P, P->d, P->l, 1, last, last);                                             // x', d', l'; a7
             ev_end(P);
         }
     } else {
         ev_begin(P, FREDOPT_PASS_FORWARD_X);
-        launch_forward_store(P, P->act, P->mode_con, P->x, P->d, P->l, false);
+        launch_forward(P, P->act, P->mode_con, P->x, P->d, P->l, EPI_STORE);
         ev_end(P);
         ev_begin(P, FREDOPT_PASS_RESIDUAL);
         launch_residual(P, P->d, P->l, 0, 1, 1);
         ev_end(P);
     }
     ev_begin(P, FREDOPT_PASS_TRANSPOSE_B);
-    launch_transpose<TEPI_UPDATE>(P, P->act, P->mode_con, P->coef_unit, P->u, P->v, nullptr, P->x, nullptr);   // a8, a9
+    launch_transpose<TEPI_UPDATE>(P, P->act, P->mode_con, P->uv, nullptr, P->x, nullptr);              // a8, a9
     ev_end(P);
     return (int)(P->launches - before);
 }
@@ -718,22 +787,29 @@ static int create_impl(fredopt_plan* P, const fredopt_csr* D, const fredopt_csr*
     RowSet& F = P->full;
     F.n = n_ne; F.n_seg = 1; F.nnz = nnzU;
     CKR(dmalloc(P, &F.vox, (size_t)n_ne)); CKR(dmalloc(P, &F.start, (size_t)n_ne));
-    CKR(dmalloc(P, &F.len, (size_t)n_ne)); CKR(dmalloc(P, &F.ulen, (size_t)n_ne));
+    CKR(dmalloc(P, &F.len, (size_t)n_ne)); CKR(dmalloc(P, &F.ulen, (size_t)n_ne)); CKR(dmalloc(P, &F.items, (size_t)n_ne));
     if (V) k_compact_rows<<<grid_for(V, 256, 1 << 16), 256, 0, st>>>(f_ne, pos_ne, pU, pstart, lab, V, F.vox, F.start, F.len, F.ulen, nullptr);
     const size_t np = P->nnz_padded ? (size_t)P->nnz_padded : 4;
-    CKR(dmalloc(P, &P->col, np)); CKR(dmalloc(P, &P->valD, np)); CKR(dmalloc(P, &P->valL, np));
-    CK(cudaMemsetAsync(P->col, 0, np * 4, st)); CK(cudaMemsetAsync(P->valD, 0, np * 4, st)); CK(cudaMemsetAsync(P->valL, 0, np * 4, st));
-    if (n_ne) k_copy_padded<<<grid_for((long long)n_ne * 32, 256, 1 << 16), 256, 0, st>>>(F.n, F.vox, F.start, pU, cU, uD, uL, P->col, P->valD, P->valL);
-    // ---- active row set, ordered by (label, voxel)
+    CKR(dmalloc(P, &F.col, np)); CKR(dmalloc(P, &F.valD, np)); CKR(dmalloc(P, &F.valL, np));
+    CK(cudaMemsetAsync(F.col, 0, np * 4, st)); CK(cudaMemsetAsync(F.valD, 0, np * 4, st)); CK(cudaMemsetAsync(F.valL, 0, np * 4, st));
+    if (n_ne) {
+        k_copy_padded<<<grid_for((long long)n_ne * 32, 256, 1 << 16), 256, 0, st>>>(F.n, F.vox, F.start, pU, cU, uD, uL, F.col, F.valD, F.valL);
+        k_pack_items<<<grid_for(n_ne, 256, 4096), 256, 0, st>>>(n_ne, F.start, F.len, nullptr, F.items);
+    }
+    // ---- active row set, ordered by (label, voxel), with its own compact copy of the rows: the iteration then
+    //      streams contiguous arrays (no unconstrained rows in between)
     RowSet& A = P->act;
     A.n = n_act; A.n_seg = n_struct > 0 ? n_struct : 1;
-    CKR(dmalloc(P, &A.vox, (size_t)n_act)); CKR(dmalloc(P, &A.start, (size_t)n_act)); CKR(dmalloc(P, &A.len, (size_t)n_act));
-    CKR(dmalloc(P, &A.ulen, (size_t)n_act)); CKR(dmalloc(P, &A.seg, (size_t)n_act));
+    CKR(dmalloc(P, &A.vox, (size_t)n_act)); CKR(dmalloc(P, &A.start, (size_t)n_act + 1)); CKR(dmalloc(P, &A.len, (size_t)n_act));
+    CKR(dmalloc(P, &A.ulen, (size_t)n_act)); CKR(dmalloc(P, &A.seg, (size_t)n_act)); CKR(dmalloc(P, &A.items, (size_t)n_act));
     {
         int32_t *vox0, *key0, *key1;
+        long long *alen64, *fstart;
         CK(cudaMalloc(&vox0, (n_act + 1) * 4)); tmp.push_back(vox0);
         CK(cudaMalloc(&key0, (n_act + 1) * 4)); tmp.push_back(key0);
         CK(cudaMalloc(&key1, (n_act + 1) * 4)); tmp.push_back(key1);
+        CK(cudaMalloc(&alen64, ((size_t)n_act + 1) * 8)); tmp.push_back(alen64);
+        CK(cudaMalloc(&fstart, ((size_t)n_act + 1) * 8)); tmp.push_back(fstart);
         if (V) k_compact_rows<<<grid_for(V, 256, 1 << 16), 256, 0, st>>>(f_act, pos_act, pU, pstart, lab, V, vox0, nullptr, nullptr, nullptr, key0);
         int bits = 1;
         while ((1 << bits) <= n_struct) ++bits;
@@ -741,7 +817,21 @@ static int create_impl(fredopt_plan* P, const fredopt_csr* D, const fredopt_csr*
         CK(cub::DeviceRadixSort::SortPairs(nullptr, tb, key0, key1, vox0, A.vox, n_act, 0, bits, st));
         void* t2; CK(cudaMalloc(&t2, tb ? tb : 1)); tmp.push_back(t2);
         CK(cub::DeviceRadixSort::SortPairs(t2, tb, key0, key1, vox0, A.vox, n_act, 0, bits, st));
-        if (n_act) k_fill_active<<<grid_for(n_act, 256, 1 << 16), 256, 0, st>>>(A.vox, key1, pU, pstart, n_act, A.start, A.len, A.ulen, A.seg);
+        // fstart = the row's offset in the full arrays (unused afterwards), A.len / A.ulen / A.seg; then A.start by a scan
+        if (n_act) k_fill_active<<<grid_for(n_act, 256, 1 << 16), 256, 0, st>>>(A.vox, key1, pU, pstart, n_act, fstart, A.len, A.ulen, A.seg);
+        CK(cudaMemsetAsync(alen64, 0, ((size_t)n_act + 1) * 8, st));
+        if (n_act) k_i32_to_i64<<<grid_for(n_act, 256, 4096), 256, 0, st>>>(A.len, alen64, n_act);
+        CKR(scan_exclusive(P, alen64, A.start, (long long)n_act + 1));
+        long long a_padded = 0;
+        CK(cudaMemcpyAsync(&a_padded, A.start + n_act, 8, cudaMemcpyDeviceToHost, st));
+        CK(cudaStreamSynchronize(st));
+        const size_t na = a_padded ? (size_t)a_padded : 4;
+        CKR(dmalloc(P, &A.col, na)); CKR(dmalloc(P, &A.valD, na)); CKR(dmalloc(P, &A.valL, na));
+        CK(cudaMemsetAsync(A.col, 0, na * 4, st)); CK(cudaMemsetAsync(A.valD, 0, na * 4, st)); CK(cudaMemsetAsync(A.valL, 0, na * 4, st));
+        if (n_act) {
+            k_copy_padded<<<grid_for((long long)n_act * 32, 256, 1 << 16), 256, 0, st>>>(A.n, A.vox, A.start, pU, cU, uD, uL, A.col, A.valD, A.valL);
+            k_pack_items<<<grid_for(n_act, 256, 4096), 256, 0, st>>>(n_act, A.start, A.len, A.seg, A.items);
+        }
     }
     // ---- tables, norms, w^
     const int ns = n_struct > 0 ? n_struct : 1;
@@ -751,15 +841,13 @@ static int create_impl(fredopt_plan* P, const fredopt_csr* D, const fredopt_csr*
     CKR(dmalloc(P, &P->nD, (size_t)n_act)); CKR(dmalloc(P, &P->nL, (size_t)n_act)); CKR(dmalloc(P, &P->nT, (size_t)n_act));
     CKR(dmalloc(P, &P->mode_union, (size_t)ns)); CKR(dmalloc(P, &P->mode_con, (size_t)ns)); CKR(dmalloc(P, &P->mode_cost, (size_t)ns));
     CKR(dmalloc(P, &P->mode_fixed, (size_t)ns * 4));
-    CKR(dmalloc(P, &P->coef_cost, (size_t)ns)); CKR(dmalloc(P, &P->coef_unit, (size_t)ns));
     CKR(dmalloc(P, &P->st, 1));
     CK(cudaMemsetAsync(P->st, 0, sizeof(DevState), st));
     if (n_act) {
-        k_norms<<<grid_for((long long)n_act * 32, 256, 1 << 16), 256, 0, st>>>(A.view(), P->col, P->valD, P->valL, P->tab, P->nD, P->nL, P->nT);
+        k_norms<<<grid_for((long long)n_act * 32, 256, 1 << 16), 256, 0, st>>>(A.view(), A.col, A.valD, A.valL, P->tab, P->nD, P->nL, P->nT);
         k_count_sets<<<grid_for(n_act, 256, 4096), 256, 0, st>>>(n_act, A.seg, A.ulen, P->nD, P->nL, P->nT, P->tab);
     }
-    k_finish_tables<<<1, 1, 0, st>>>(P->tab, n_struct, P->st, P->mode_union, P->mode_con, P->mode_cost, P->mode_fixed, ns, P->coef_cost,
-                                    P->coef_unit);
+    k_finish_tables<<<1, 1, 0, st>>>(P->tab, n_struct, P->st, P->mode_union, P->mode_con, P->mode_cost, P->mode_fixed, ns);
     k_set_params<<<1, 1, 0, st>>>(P->st, 1.0, 0.0, 0.5, 1.0, 200, 1, 1);
     CK(cudaMemcpyAsync(P->h_tab.data(), P->tab, sizeof(StructInfo) * ns, cudaMemcpyDeviceToHost, st));
     CK(cudaStreamSynchronize(st));
@@ -767,8 +855,10 @@ static int create_impl(fredopt_plan* P, const fredopt_csr* D, const fredopt_csr*
     // ---- vectors
     CKR(dmalloc(P, &P->x, (size_t)S)); CKR(dmalloc(P, &P->g, (size_t)S)); CKR(dmalloc(P, &P->xtmp, (size_t)S));
     CK(cudaMemsetAsync(P->x, 0, (S ? S : 1) * 8, st)); CK(cudaMemsetAsync(P->g, 0, (S ? S : 1) * 8, st));
-    double** vecs[] = {&P->d, &P->l, &P->Dg, &P->Lg, &P->u, &P->v};
+    double** vecs[] = {&P->d, &P->l, &P->Dg, &P->Lg};
     for (auto pp : vecs) { CKR(dmalloc(P, pp, (size_t)n_act)); CK(cudaMemsetAsync(*pp, 0, (n_act ? n_act : 1) * 8, st)); }
+    CKR(dmalloc(P, &P->pq, (size_t)n_act)); CKR(dmalloc(P, &P->uv, (size_t)n_act));
+    CK(cudaMemsetAsync(P->pq, 0, (n_act ? n_act : 1) * 16, st)); CK(cudaMemsetAsync(P->uv, 0, (n_act ? n_act : 1) * 16, st));
     CKR(dmalloc(P, &P->cpart, (size_t)MAX_PARTIALS)); CKR(dmalloc(P, &P->part_prox, (size_t)MAX_PARTIALS));
     CKR(dmalloc(P, &P->part_phi, (size_t)MAX_PARTIALS)); CKR(dmalloc(P, &P->part_cnt, (size_t)MAX_PARTIALS));
     CKR(dmalloc(P, &P->sink, 4));
@@ -883,9 +973,9 @@ static int forward_f32(fredopt_plan* P, const RowSet& R, int m, const double* xd
     if (dd) cudaMemsetAsync(dd, 0, (size_t)P->V * 4, P->stream);
     if (dl) cudaMemsetAsync(dl, 0, (size_t)P->V * 4, P->stream);
     if (R.n) {
-        k_forward<EPI_F32VOX><<<fwd_grid(P, R.n), FWD_THREADS, 0, P->stream>>>(R.view(), P->mode_fixed + (size_t)m * P->max_seg, P->col,
-                                                                               P->valD, P->valL, xd, nullptr, nullptr, nullptr, nullptr,
-                                                                               dd, dl, letd_out);
+        k_forward<EPI_F32VOX><<<fwd_grid(P, R.n), FWD_THREADS, 0, P->stream>>>(R.n, R.items, R.vox, P->mode_fixed + (size_t)m * P->max_seg,
+                                                                               R.col, R.valD, R.valL, xd, nullptr, nullptr, nullptr,
+                                                                               nullptr, nullptr, dd, dl, letd_out);
         ++P->launches;
     }
     int rc = FREDOPT_OK;
@@ -916,23 +1006,21 @@ int fredopt_spmv_forward(fredopt_plan* P, int32_t rows, const float* x, float* d
 int fredopt_spmv_transpose(fredopt_plan* P, int32_t rows, const float* u, const float* v, float* out) {
     if (!P || !out || (!u && !v) || (rows != FREDOPT_ROWS_ALL && rows != FREDOPT_ROWS_ACTIVE)) return FREDOPT_INVALID_ARG;
     RowSet& R = rows == FREDOPT_ROWS_ALL ? P->full : P->act;
-    double *vecD = P->u, *vecL = P->v;
+    double2* vec = P->uv;
     if (rows == FREDOPT_ROWS_ALL) {
         if (!R.t_built) CKR(build_transpose(P, R));
-        if (!P->fullD) { CKR(dmalloc(P, &P->fullD, (size_t)R.n)); CKR(dmalloc(P, &P->fullL, (size_t)R.n)); }
-        vecD = P->fullD; vecL = P->fullL;
+        if (!P->fullUV) CKR(dmalloc(P, &P->fullUV, (size_t)R.n));
+        vec = P->fullUV;
     }
     const float *du = nullptr, *dv = nullptr; void *fu = nullptr, *fv = nullptr;
     if (u) CKR(stage_in_f32(P, u, P->V, &du, &fu));
     if (v) { int rc = stage_in_f32(P, v, P->V, &dv, &fv); if (rc) { cudaFree(fu); return rc; } }
-    if (R.n) {
-        if (u) { k_gather_f32_to_f64<<<grid_for(R.n, 256, 4096), 256, 0, P->stream>>>(du, R.vox, vecD, R.n); ++P->launches; }
-        if (v) { k_gather_f32_to_f64<<<grid_for(R.n, 256, 4096), 256, 0, P->stream>>>(dv, R.vox, vecL, R.n); ++P->launches; }
-    }
+    if (R.n) { k_gather_uv<<<grid_for(R.n, 256, 4096), 256, 0, P->stream>>>(du, dv, R.vox, vec, R.n); ++P->launches; }
     float* dout = out; void* fo = nullptr;
     if (!is_device_ptr(out)) { cudaError_t e = cudaMalloc(&fo, (P->S ? P->S : 1) * 4); if (e != cudaSuccess) { cudaFree(fu); cudaFree(fv); CK(e); } dout = (float*)fo; }
     const int m = (u ? 1 : 0) | (v ? 2 : 0);
-    launch_transpose<TEPI_F32>(P, R, P->mode_fixed + (size_t)m * P->max_seg, P->coef_unit, vecD, vecL, nullptr, nullptr, dout);
+    cudaMemsetAsync(dout, 0, (size_t)(P->S ? P->S : 1) * 4, P->stream);     // spots without entries are never visited
+    launch_transpose<TEPI_F32>(P, R, P->mode_fixed + (size_t)m * P->max_seg, vec, nullptr, nullptr, dout);
     cudaError_t e = cudaGetLastError();
     if (e == cudaSuccess && fo) e = cudaMemcpyAsync(out, dout, P->S * 4, cudaMemcpyDeviceToHost, P->stream);
     if (fo || fu || fv) { cudaError_t e2 = cudaStreamSynchronize(P->stream); if (e == cudaSuccess) e = e2; }
@@ -946,7 +1034,7 @@ int fredopt_proximity(fredopt_plan* P, const float* x, double* prox, int64_t* n_
     const double* xd;
     CKR(resolve_x(P, x, &xd));
     // scratch: Dg / Lg hold the products so that the iteration's d, l are left alone
-    launch_forward_store(P, P->act, P->mode_con, xd, P->Dg, P->Lg, false);
+    launch_forward(P, P->act, P->mode_con, xd, P->Dg, P->Lg, EPI_STORE);
     launch_residual(P, P->Dg, P->Lg, 0, 1, 0);
     launch_finalize(P);
     DevState h;
@@ -1073,7 +1161,7 @@ int64_t fredopt_launch_count(fredopt_plan* P) { return P ? P->launches : 0; }
 int fredopt_stream_read(fredopt_plan* P, const void* device_buf, int64_t bytes, int32_t reps) {
     if (!P || !device_buf || bytes < 16 || (bytes & 15) || reps < 1 || !is_device_ptr(device_buf)) return FREDOPT_INVALID_ARG;
     for (int i = 0; i < reps; ++i) {
-        k_stream_read<<<P->sm_count * 4, 512, 0, P->stream>>>((const int4*)device_buf, bytes / 16, P->sink);
+        k_stream_read<<<(unsigned)((bytes / 16 + 2047) / 2048), 256, 0, P->stream>>>((const int4*)device_buf, bytes / 16, P->sink);
         ++P->launches;
     }
     CK(cudaGetLastError());

@@ -1,13 +1,19 @@
 // fredopt_kernels.cuh -- the hot kernels of the superiorized feasibility-seeking iteration (sm_100a).
 //
 // Passes of one iteration:
-//   k_forward    d = D x, l = L x   over a row list (warp per row, 128-bit streamed index/value loads, fp64
-//                accumulation, shuffle reduction).  Rows read only the value arrays their structure needs.
-//   k_transpose  out_j = sum_i D_ij cD_i + L_ij cL_i   over the stored CSR of the transposes (CTA per spot,
-//                per-structure segments, no atomics, fixed-order reduction) with the gradient / update+clamp
-//                epilogues fused.
-//   k_select     |g|^2, c = sum w^ (Dg)^2 + w^ (Lg)^2, the accept loop of Fig. 3 on device scalars, x' = x - beta g.
-//   k_residual   d' = d - beta Dg, l' = l - beta Lg, residuals / violations of Fig. 2 -> u, v, partial sums.
+//   k_forward    d = D x, l = L x over a list of work items (one item = one voxel row; one warp per item,
+//                round-robin, 128-bit streamed index/value loads kept out of L1, fp64 accumulation, shuffle
+//                reduction).  A row reads only the value arrays its structure needs.  Epilogues: store d, l
+//                (+ the cost residuals p, q of Eq. 2), the quadratic coefficient c of the accept test, or fp32
+//                dose / LETd per voxel.
+//   k_transpose  out_j = sum_i D_ij u_i + L_ij v_i over the stored CSR of the transposes (one item = at most
+//                TR_ITEM_MAX entries of one (spot, structure) run; one warp per item; no floating-point
+//                atomics: every item writes its partial sum and the LAST item of a spot to finish adds the
+//                spot's partials in item order, so the result does not depend on the schedule) with the
+//                gradient / update+clamp epilogues fused.
+//   k_select     |g|^2, c = sum w^ (Dg)^2 + w^ (Lg)^2 and the accept loop of Fig. 3 on device scalars.
+//   k_residual   d' = d - beta Dg, l' = l - beta Lg, x' = x - beta g, residuals / violations of Fig. 2 -> u, v,
+//                partial sums of proximity, cost and violation count.
 // All vectors and accumulators are fp64; matrix values fp32; indices int32; offsets int64.
 #pragma once
 #include <cuda_runtime.h>
@@ -17,9 +23,9 @@ namespace fredopt {
 
 constexpr int FWD_THREADS = 256;
 constexpr int FWD_WARPS = FWD_THREADS / 32;
-constexpr int TR_THREADS = 256;
-constexpr int MAX_PARTIALS = 1184;          // 148 SMs x 8 resident CTAs of 256 threads
+constexpr int MAX_PARTIALS = 2368;          // 148 SMs x 16 CTAs: upper bound of any partial-sum grid
 constexpr int ROW_THREADS = 256;
+constexpr int TR_ITEM_MAX = 2048;           // entries per transposed work item (multiple of 4)
 
 // flags of a structure
 enum : int { F_DOSE_SLAB = 1, F_DL_SLAB = 2, F_LETD = 4, F_DOSE_REF = 8, F_DL_REF = 16 };
@@ -31,8 +37,6 @@ struct StructInfo {
     unsigned long long part, n_sets, n_zero, rows, nnz;   // participating sets, declared sets, zero-norm sets, rows, nnz
 };
 
-struct SegCoef { double scaleD, shiftD, scaleL, shiftL; };   // coefficient = scale * (vec[a] - shift)
-
 struct DevState {
     double lambda, beta0, a, eta;
     double beta_next, eta_pow, relax, last_beta, beta_acc;
@@ -40,6 +44,14 @@ struct DevState {
     long long k, s, trials, n_viol, max_trials;
     long long n_sets, n_zero;
     int accept_check, pad;
+};
+
+// One work item: `len` entries (multiple of 4) starting at entry `start` (multiple of 4) of the index / value
+// arrays; `seg` = structure - 1 (selects which value arrays are read).  16 bytes: fetched with one 128-bit load.
+struct __align__(16) Item {
+    long long start;
+    int32_t len;
+    int32_t seg;
 };
 
 // ------------------------------------------------------------------------------------------ loads
@@ -54,6 +66,20 @@ __device__ __forceinline__ float4 ld_stream_f4(const float* p) {
     float4 r;
     asm volatile("ld.global.nc.L1::no_allocate.v4.f32 {%0,%1,%2,%3}, [%4];"
                  : "=f"(r.x), "=f"(r.y), "=f"(r.z), "=f"(r.w) : "l"(p));
+    return r;
+}
+__device__ __forceinline__ Item ld_item(const Item* p) {
+    const int4 v = __ldg((const int4*)p);
+    Item it;
+    it.start = (long long)(((unsigned long long)(unsigned)v.y << 32) | (unsigned)v.x);
+    it.len = v.z;
+    it.seg = v.w;
+    return it;
+}
+// partial sums written by other CTAs of the same launch: bypass L1
+__device__ __forceinline__ double ld_cg_f64(const double* p) {
+    double r;
+    asm volatile("ld.global.cg.f64 %0, [%1];" : "=d"(r) : "l"(p));
     return r;
 }
 
@@ -75,17 +101,6 @@ __device__ __forceinline__ double block_sum(double v, double* sm) {
     return r;
 }
 
-// ------------------------------------------------------------------------------------------ forward
-struct RowList {
-    long long n;                 // rows in the list
-    const long long* start;      // [n] offset of the row in the padded arrays (multiple of 4)
-    const int32_t* len;          // [n] padded length (multiple of 4)
-    const int32_t* seg;          // [n] segment (structure - 1), or nullptr = segment 0
-    const int32_t* vox;          // [n] voxel index of the row
-};
-
-enum : int { EPI_STORE = 0, EPI_CPART = 1, EPI_F32VOX = 2 };
-
 __device__ __forceinline__ void fma4(double& acc, const float4& a, double x0, double x1, double x2, double x3) {
     acc = fma((double)a.x, x0, acc);
     acc = fma((double)a.y, x1, acc);
@@ -93,68 +108,99 @@ __device__ __forceinline__ void fma4(double& acc, const float4& a, double x0, do
     acc = fma((double)a.w, x3, acc);
 }
 
-// One warp per row, rows r = warp, warp + W, ... (static mapping: deterministic partial sums).
+// ------------------------------------------------------------------------------------------ forward
+enum : int { EPI_STORE = 0, EPI_STORE_PQ = 1, EPI_CPART = 2, EPI_F32VOX = 3 };
+
+// <D_i, x> and / or <L_i, x> of one row by one warp.  M: bit 0 = D, bit 1 = L.  Four 128-entry chunks per trip:
+// up to 12 independent 128-bit loads per lane in flight before the first gather.
+template <int M>
+__device__ __forceinline__ void fwd_row(const int32_t* __restrict__ cp, const float* __restrict__ dp,
+                                        const float* __restrict__ lp, int L, int lane, const double* __restrict__ x,
+                                        double& aD, double& aL) {
+    constexpr int U = 4;
+    int p = lane * 4;
+    for (; p + 128 * (U - 1) < L; p += 128 * U) {
+        int4 c[U];
+        float4 d[U], l[U];
+#pragma unroll
+        for (int u = 0; u < U; ++u) {
+            c[u] = ld_stream_i4(cp + p + 128 * u);
+            if (M & 1) d[u] = ld_stream_f4(dp + p + 128 * u);
+            if (M & 2) l[u] = ld_stream_f4(lp + p + 128 * u);
+        }
+#pragma unroll
+        for (int u = 0; u < U; ++u) {
+            const double x0 = __ldg(x + c[u].x), x1 = __ldg(x + c[u].y), x2 = __ldg(x + c[u].z), x3 = __ldg(x + c[u].w);
+            if (M & 1) fma4(aD, d[u], x0, x1, x2, x3);
+            if (M & 2) fma4(aL, l[u], x0, x1, x2, x3);
+        }
+    }
+    for (; p < L; p += 128) {
+        const int4 c0 = ld_stream_i4(cp + p);
+        float4 d0, l0;
+        if (M & 1) d0 = ld_stream_f4(dp + p);
+        if (M & 2) l0 = ld_stream_f4(lp + p);
+        const double x0 = __ldg(x + c0.x), x1 = __ldg(x + c0.y), x2 = __ldg(x + c0.z), x3 = __ldg(x + c0.w);
+        if (M & 1) fma4(aD, d0, x0, x1, x2, x3);
+        if (M & 2) fma4(aL, l0, x0, x1, x2, x3);
+    }
+}
+
+// One warp per item, items r = warp, warp + W, ... (static mapping: deterministic partial sums; the warps of the
+// grid read one contiguous window of the arrays at any time).  The next item's descriptor is fetched one item ahead.
 // mode[seg]: bit 0 = read valD, bit 1 = read valL.
 template <int EPI>
-__global__ void __launch_bounds__(FWD_THREADS)
-k_forward(RowList rl, const uint8_t* __restrict__ mode, const int32_t* __restrict__ col,
-          const float* __restrict__ vD, const float* __restrict__ vL, const double* __restrict__ x,
-          double* __restrict__ oD, double* __restrict__ oL,               // EPI_STORE / EPI_CPART: list-indexed
-          const StructInfo* __restrict__ tab, double* __restrict__ cpart,  // EPI_CPART
+__global__ void __launch_bounds__(FWD_THREADS, 3)
+k_forward(long long n, const Item* __restrict__ items, const int32_t* __restrict__ vox, const uint8_t* __restrict__ mode,
+          const int32_t* __restrict__ col, const float* __restrict__ vD, const float* __restrict__ vL,
+          const double* __restrict__ x,
+          double* __restrict__ oD, double* __restrict__ oL,                // EPI_STORE*, EPI_CPART: item-indexed
+          double2* __restrict__ pq,                                        // EPI_STORE_PQ: cost residuals (Eq. 2)
+          const StructInfo* __restrict__ tab, double* __restrict__ cpart,  // EPI_STORE_PQ / EPI_CPART
           float* __restrict__ fD, float* __restrict__ fL, int letd_out)    // EPI_F32VOX: voxel-indexed
 {
     const int lane = threadIdx.x & 31;
-    const long long warp0 = (long long)blockIdx.x * FWD_WARPS + (threadIdx.x >> 5);
     const long long nwarps = (long long)gridDim.x * FWD_WARPS;
+    long long r = (long long)blockIdx.x * FWD_WARPS + (threadIdx.x >> 5);
     double csum = 0.0;
-    for (long long r = warp0; r < rl.n; r += nwarps) {
-        const long long s = rl.start[r];
-        const int L = rl.len[r];
-        const int sg = rl.seg ? rl.seg[r] : 0;
-        const int m = mode[sg];
+    Item it;
+    if (r < n) it = ld_item(items + r);
+    while (r < n) {
+        const long long rn = r + nwarps;
+        Item nx;
+        if (rn < n) nx = ld_item(items + rn);
+        const int m = mode[it.seg];
         double aD = 0.0, aL = 0.0;
-        if (m != 0) {
-            const int32_t* cp = col + s;
-            const float* dp = vD + s;
-            const float* lp = vL + s;
-            int p = lane * 4;
-            for (; p + 128 < L; p += 256) {
-                const int4 c0 = ld_stream_i4(cp + p), c1 = ld_stream_i4(cp + p + 128);
-                float4 d0, d1, l0, l1;
-                if (m & 1) { d0 = ld_stream_f4(dp + p); d1 = ld_stream_f4(dp + p + 128); }
-                if (m & 2) { l0 = ld_stream_f4(lp + p); l1 = ld_stream_f4(lp + p + 128); }
-                const double x0 = __ldg(x + c0.x), x1 = __ldg(x + c0.y), x2 = __ldg(x + c0.z), x3 = __ldg(x + c0.w);
-                const double y0 = __ldg(x + c1.x), y1 = __ldg(x + c1.y), y2 = __ldg(x + c1.z), y3 = __ldg(x + c1.w);
-                if (m & 1) { fma4(aD, d0, x0, x1, x2, x3); fma4(aD, d1, y0, y1, y2, y3); }
-                if (m & 2) { fma4(aL, l0, x0, x1, x2, x3); fma4(aL, l1, y0, y1, y2, y3); }
-            }
-            if (p < L) {
-                const int4 c0 = ld_stream_i4(cp + p);
-                float4 d0, l0;
-                if (m & 1) d0 = ld_stream_f4(dp + p);
-                if (m & 2) l0 = ld_stream_f4(lp + p);
-                const double x0 = __ldg(x + c0.x), x1 = __ldg(x + c0.y), x2 = __ldg(x + c0.z), x3 = __ldg(x + c0.w);
-                if (m & 1) fma4(aD, d0, x0, x1, x2, x3);
-                if (m & 2) fma4(aL, l0, x0, x1, x2, x3);
-            }
-            aD = warp_sum(aD);
-            aL = warp_sum(aL);
-        }
+        const int32_t* cp = col + it.start;
+        if (m == 3) fwd_row<3>(cp, vD + it.start, vL + it.start, it.len, lane, x, aD, aL);
+        else if (m == 1) fwd_row<1>(cp, vD + it.start, nullptr, it.len, lane, x, aD, aL);
+        else if (m == 2) fwd_row<2>(cp, nullptr, vL + it.start, it.len, lane, x, aD, aL);
+        if (m & 1) aD = warp_sum(aD);
+        if (m & 2) aL = warp_sum(aL);
         if (lane == 0) {
             if (EPI == EPI_F32VOX) {
-                const int v = rl.vox[r];
+                const int v = vox[r];
                 if (fD) fD[v] = (float)aD;
                 if (fL) fL[v] = letd_out ? (aD > 0.0 ? (float)(aL / aD) : 0.0f) : (float)aL;
             } else {
                 oD[r] = aD;
                 oL[r] = aL;
+                if (EPI == EPI_STORE_PQ) {      // p_i = 2 w^ (d_i - Dref), q_i = 2 w^ (l_i - cDLref): grad chi^2 = D^T p + L^T q
+                    const StructInfo& T = tab[it.seg];
+                    double2 v;
+                    v.x = (T.flags & F_DOSE_REF) ? 2.0 * T.what * (aD - T.dose_ref) : 0.0;
+                    v.y = (T.flags & F_DL_REF) ? 2.0 * T.what * (aL - T.dl_ref) : 0.0;
+                    pq[r] = v;
+                }
                 if (EPI == EPI_CPART) {
-                    const StructInfo& T = tab[sg];
+                    const StructInfo& T = tab[it.seg];
                     if (T.flags & F_DOSE_REF) csum += T.what * aD * aD;
                     if (T.flags & F_DL_REF) csum += T.what * aL * aL;
                 }
             }
         }
+        r = rn;
+        it = nx;
     }
     if (EPI == EPI_CPART) {
         __shared__ double sm[FWD_WARPS];
@@ -167,65 +213,114 @@ k_forward(RowList rl, const uint8_t* __restrict__ mode, const int32_t* __restric
 // ------------------------------------------------------------------------------------------ transposed
 enum : int { TEPI_F32 = 0, TEPI_GRAD = 1, TEPI_UPDATE = 2 };
 
-// One CTA per spot j.  The spot's entries are stored per structure segment (t_ptr[j*n_seg + s]), columns =
-// compact active-row indices in ascending order; entry coefficient = scale_s * (vec[a] - shift_s).
-template <int EPI>
-__global__ void __launch_bounds__(TR_THREADS)
-k_transpose(int n_seg, const long long* __restrict__ t_ptr, const int32_t* __restrict__ t_col,
-            const float* __restrict__ tD, const float* __restrict__ tL, const uint8_t* __restrict__ mode,
-            const SegCoef* __restrict__ coef, const double* __restrict__ vecD, const double* __restrict__ vecL,
-            double* __restrict__ g_out,                    // TEPI_GRAD
-            double* __restrict__ x, const DevState* __restrict__ st,   // TEPI_UPDATE
-            float* __restrict__ f_out)                     // TEPI_F32
-{
-    __shared__ double sm[TR_THREADS / 32];
-    const long long j = blockIdx.x;
-    double acc = 0.0;
-    for (int sg = 0; sg < n_seg; ++sg) {
-        const int m = mode[sg];
-        if (m == 0) continue;
-        const long long b = t_ptr[j * n_seg + sg], e = t_ptr[j * n_seg + sg + 1];
-        if (b == e) continue;
-        const SegCoef cf = coef[sg];
-        double aD = 0.0, aL = 0.0;
-        long long p = b + threadIdx.x * 4;
-        for (; p + TR_THREADS * 4 < e; p += TR_THREADS * 8) {
-            const int4 c0 = ld_stream_i4(t_col + p), c1 = ld_stream_i4(t_col + p + TR_THREADS * 4);
-            if (m & 1) {
-                const float4 a0 = ld_stream_f4(tD + p), a1 = ld_stream_f4(tD + p + TR_THREADS * 4);
-                const double s = cf.shiftD;
-                fma4(aD, a0, __ldg(vecD + c0.x) - s, __ldg(vecD + c0.y) - s, __ldg(vecD + c0.z) - s, __ldg(vecD + c0.w) - s);
-                fma4(aD, a1, __ldg(vecD + c1.x) - s, __ldg(vecD + c1.y) - s, __ldg(vecD + c1.z) - s, __ldg(vecD + c1.w) - s);
-            }
-            if (m & 2) {
-                const float4 a0 = ld_stream_f4(tL + p), a1 = ld_stream_f4(tL + p + TR_THREADS * 4);
-                const double s = cf.shiftL;
-                fma4(aL, a0, __ldg(vecL + c0.x) - s, __ldg(vecL + c0.y) - s, __ldg(vecL + c0.z) - s, __ldg(vecL + c0.w) - s);
-                fma4(aL, a1, __ldg(vecL + c1.x) - s, __ldg(vecL + c1.y) - s, __ldg(vecL + c1.z) - s, __ldg(vecL + c1.w) - s);
+// sum_i D_ij vec[i].x + L_ij vec[i].y over one item by one warp (vec is L2-resident; entries of a spot run over
+// ascending compact row indices, so neighbouring lanes gather neighbouring elements)
+template <int M>
+__device__ __forceinline__ double tr_item(const int32_t* __restrict__ cp, const float* __restrict__ dp,
+                                          const float* __restrict__ lp, int L, int lane, const double2* __restrict__ vec) {
+    constexpr int U = 4;
+    const double* vs = (const double*)vec;
+    double aD = 0.0, aL = 0.0;
+    int p = lane * 4;
+    for (; p + 128 * (U - 1) < L; p += 128 * U) {
+        int4 c[U];
+        float4 d[U], l[U];
+#pragma unroll
+        for (int u = 0; u < U; ++u) {
+            c[u] = ld_stream_i4(cp + p + 128 * u);
+            if (M & 1) d[u] = ld_stream_f4(dp + p + 128 * u);
+            if (M & 2) l[u] = ld_stream_f4(lp + p + 128 * u);
+        }
+#pragma unroll
+        for (int u = 0; u < U; ++u) {
+            if (M == 3) {
+                const double2 g0 = __ldg(vec + c[u].x), g1 = __ldg(vec + c[u].y), g2 = __ldg(vec + c[u].z), g3 = __ldg(vec + c[u].w);
+                fma4(aD, d[u], g0.x, g1.x, g2.x, g3.x);
+                fma4(aL, l[u], g0.y, g1.y, g2.y, g3.y);
+            } else {
+                constexpr int o = (M == 2) ? 1 : 0;
+                const double g0 = __ldg(vs + 2 * (long long)c[u].x + o), g1 = __ldg(vs + 2 * (long long)c[u].y + o);
+                const double g2 = __ldg(vs + 2 * (long long)c[u].z + o), g3 = __ldg(vs + 2 * (long long)c[u].w + o);
+                if (M == 1) fma4(aD, d[u], g0, g1, g2, g3); else fma4(aL, l[u], g0, g1, g2, g3);
             }
         }
-        if (p < e) {
-            const int4 c0 = ld_stream_i4(t_col + p);
-            if (m & 1) {
-                const float4 a0 = ld_stream_f4(tD + p);
-                const double s = cf.shiftD;
-                fma4(aD, a0, __ldg(vecD + c0.x) - s, __ldg(vecD + c0.y) - s, __ldg(vecD + c0.z) - s, __ldg(vecD + c0.w) - s);
-            }
-            if (m & 2) {
-                const float4 a0 = ld_stream_f4(tL + p);
-                const double s = cf.shiftL;
-                fma4(aL, a0, __ldg(vecL + c0.x) - s, __ldg(vecL + c0.y) - s, __ldg(vecL + c0.z) - s, __ldg(vecL + c0.w) - s);
-            }
-        }
-        acc += cf.scaleD * aD + cf.scaleL * aL;
     }
-    const double tot = block_sum(acc, sm);
-    if (threadIdx.x == 0) {
-        if (EPI == TEPI_GRAD) g_out[j] = tot;
-        else if (EPI == TEPI_UPDATE) {
-            const double v = x[j] - st->relax * tot;          // x <- x' - lambda eta^k * sum w^ (r/|a|^2) a
-            x[j] = v < 0.0 ? 0.0 : v;                          // clamp
-        } else f_out[j] = (float)tot;
+    for (; p < L; p += 128) {
+        const int4 c0 = ld_stream_i4(cp + p);
+        if (M == 3) {
+            const float4 d0 = ld_stream_f4(dp + p), l0 = ld_stream_f4(lp + p);
+            const double2 g0 = __ldg(vec + c0.x), g1 = __ldg(vec + c0.y), g2 = __ldg(vec + c0.z), g3 = __ldg(vec + c0.w);
+            fma4(aD, d0, g0.x, g1.x, g2.x, g3.x);
+            fma4(aL, l0, g0.y, g1.y, g2.y, g3.y);
+        } else {
+            constexpr int o = (M == 2) ? 1 : 0;
+            const float4 a0 = ld_stream_f4((M == 1 ? dp : lp) + p);
+            const double g0 = __ldg(vs + 2 * (long long)c0.x + o), g1 = __ldg(vs + 2 * (long long)c0.y + o);
+            const double g2 = __ldg(vs + 2 * (long long)c0.z + o), g3 = __ldg(vs + 2 * (long long)c0.w + o);
+            fma4(aD, a0, g0, g1, g2, g3);
+        }
+    }
+    return aD + aL;
+}
+
+// One warp per item (round-robin).  The items of spot j are item_ptr[j] .. item_ptr[j+1]-1 (ascending structure,
+// then ascending position).  Every item stores its partial sum; the warp that completes the LAST outstanding item
+// of a spot (per-spot arrival counter, integer atomics only) adds the spot's partials in item order and runs the
+// epilogue, then re-arms the counter.  The value is therefore independent of which warp finishes last.
+// Spots without items are never visited: their g / output stays 0 (set at creation / by the caller), their x is
+// already >= 0.
+template <int EPI>
+__global__ void __launch_bounds__(FWD_THREADS, 3)
+k_transpose(long long n, const Item* __restrict__ items, const int32_t* __restrict__ item_spot,
+            const long long* __restrict__ item_ptr, const uint8_t* __restrict__ mode, const int32_t* __restrict__ t_col,
+            const float* __restrict__ tD, const float* __restrict__ tL, const double2* __restrict__ vec,
+            double* __restrict__ partial, unsigned int* __restrict__ counter,
+            double* __restrict__ g_out,                                 // TEPI_GRAD
+            double* __restrict__ x, const DevState* __restrict__ st,   // TEPI_UPDATE
+            float* __restrict__ f_out)                                  // TEPI_F32
+{
+    const int lane = threadIdx.x & 31;
+    const long long nwarps = (long long)gridDim.x * FWD_WARPS;
+    long long r = (long long)blockIdx.x * FWD_WARPS + (threadIdx.x >> 5);
+    Item it;
+    if (r < n) it = ld_item(items + r);
+    while (r < n) {
+        const long long rn = r + nwarps;
+        Item nx;
+        if (rn < n) nx = ld_item(items + rn);
+        const int m = mode[it.seg];
+        double tot = 0.0;
+        const int32_t* cp = t_col + it.start;
+        if (m == 3) tot = tr_item<3>(cp, tD + it.start, tL + it.start, it.len, lane, vec);
+        else if (m == 1) tot = tr_item<1>(cp, tD + it.start, nullptr, it.len, lane, vec);
+        else if (m == 2) tot = tr_item<2>(cp, nullptr, tL + it.start, it.len, lane, vec);
+        if (m) tot = warp_sum(tot);
+        if (lane == 0) {
+            const int j = item_spot[r];
+            const long long ib = item_ptr[j], ie = item_ptr[j + 1];
+            bool last = true;
+            if (ie - ib > 1) {
+                partial[r] = tot;
+                __threadfence();
+                const unsigned int old = atomicAdd(counter + j, 1u);
+                last = old == (unsigned int)(ie - ib - 1);
+                if (last) {
+                    __threadfence();
+                    tot = 0.0;
+                    for (long long i = ib; i < ie; ++i) tot += ld_cg_f64(partial + i);
+                    counter[j] = 0u;
+                }
+            }
+            if (last) {
+                if (EPI == TEPI_GRAD) g_out[j] = tot;
+                else if (EPI == TEPI_UPDATE) {
+                    const double v = x[j] - st->relax * tot;          // x <- x' - lambda eta^k * sum w^ (r/|a|^2) a
+                    x[j] = v < 0.0 ? 0.0 : v;                          // clamp
+                } else f_out[j] = (float)tot;
+            }
+        }
+        r = rn;
+        it = nx;
     }
 }
 
@@ -241,15 +336,18 @@ __global__ void k_set_params(DevState* st, double lambda, double beta0, double a
 
 // |g|^2 and c by fixed-order sums, then the `while loop` of Fig. 3 on scalars:
 // chi^2(x - beta g) = chi^2(x) - beta |g|^2 + beta^2 c   =>   accept  <=>  beta c < |g|^2.
-// Then x <- x - beta g.  One CTA.
+// The accepted beta (0 if none) goes to st->beta_acc; k_residual applies it.  One CTA.
 __global__ void __launch_bounds__(1024)
-k_select(DevState* st, const double* __restrict__ g, double* __restrict__ x, long long S,
-         const double* __restrict__ cpart, int n_part) {
+k_select(DevState* st, const double* __restrict__ g, long long S, const double* __restrict__ cpart, int n_part) {
     __shared__ double sm[32];
-    __shared__ double s_beta;
-    double a = 0.0;
-    for (long long j = threadIdx.x; j < S; j += blockDim.x) a = fma(g[j], g[j], a);
-    const double gg = block_sum(a, sm);
+    double a0 = 0.0, a1 = 0.0, a2 = 0.0, a3 = 0.0;
+    long long j = threadIdx.x;
+    for (; j + 3 * 1024 < S; j += 4 * 1024) {       // 4 independent loads in flight; fixed order of addition
+        const double g0 = g[j], g1 = g[j + 1024], g2 = g[j + 2048], g3 = g[j + 3072];
+        a0 = fma(g0, g0, a0); a1 = fma(g1, g1, a1); a2 = fma(g2, g2, a2); a3 = fma(g3, g3, a3);
+    }
+    for (; j < S; j += 1024) a0 = fma(g[j], g[j], a0);
+    const double gg = block_sum((a0 + a1) + (a2 + a3), sm);
     double c = 0.0;
     for (int i = threadIdx.x; i < n_part; i += blockDim.x) c += cpart[i];
     const double cc = block_sum(c, sm);
@@ -269,12 +367,7 @@ k_select(DevState* st, const double* __restrict__ g, double* __restrict__ x, lon
             st->beta_next = bn; st->s = s; st->trials = tr;
         }
         st->beta_acc = acc; st->gg = gg; st->c = cc;
-        s_beta = acc;
     }
-    __syncthreads();
-    const double beta = s_beta;
-    if (beta != 0.0)
-        for (long long j = threadIdx.x; j < S; j += blockDim.x) x[j] = fma(-beta, g[j], x[j]);
 }
 
 // signed residual of a hyperslab lo <= val <= hi (NaN = absent): upper violations > 0, lower < 0
@@ -284,33 +377,43 @@ __device__ __forceinline__ double slab_residual(double val, double lo, double hi
     return 0.0;
 }
 
-// Per active row: apply the accepted perturbation to the stored products (d' = d - beta Dg, l' = l - beta Lg),
-// then, if `final`, the residuals of Fig. 2 in simultaneous form at that point:
+// Per active row: apply the accepted perturbation to the stored products (d' = d - beta Dg, l' = l - beta Lg) and
+// per spot to the weights (x' = x - beta g); then, if `final`, the residuals of Fig. 2 in simultaneous form at x':
 //   u_i = w^ r_dose/|D_i|^2 - LETmax w^ r_letd/|L_i - LETmax D_i|^2 ,  v_i = w^ r_dl/|L_i|^2 + w^ r_letd/|...|^2
-// plus partial sums of the proximity, chi^2 and the violation count (fixed grid, fixed order).
+// plus partial sums of the proximity, chi^2 and the violation count (fixed grid, fixed order); if not final
+// (another reduction of Fig. 3 follows), the cost residuals p, q at x'.
 __global__ void __launch_bounds__(ROW_THREADS)
-k_residual(long long n, const int32_t* __restrict__ seg, const StructInfo* __restrict__ tab, DevState* st,
+k_residual(long long n, const Item* __restrict__ items, const StructInfo* __restrict__ tab, DevState* st,
            double* __restrict__ d, double* __restrict__ l, const double* __restrict__ Dg, const double* __restrict__ Lg,
            const double* __restrict__ nD, const double* __restrict__ nL, const double* __restrict__ nT,
-           double* __restrict__ u, double* __restrict__ v,
+           double2* __restrict__ uv, double2* __restrict__ pq, double* __restrict__ x, const double* __restrict__ g, long long S,
            double* __restrict__ part_prox, double* __restrict__ part_phi, long long* __restrict__ part_cnt,
            int use_beta, int final, int write_uv) {
     __shared__ double sm[ROW_THREADS / 32];
     __shared__ long long smc[ROW_THREADS / 32];
     const double beta = use_beta ? st->beta_acc : 0.0;
+    const long long tid = (long long)blockIdx.x * blockDim.x + threadIdx.x, nth = (long long)gridDim.x * blockDim.x;
+    if (beta != 0.0)
+        for (long long j = tid; j < S; j += nth) x[j] = fma(-beta, g[j], x[j]);
     double prox = 0.0, phi = 0.0;
     long long cnt = 0;
-    for (long long a = (long long)blockIdx.x * blockDim.x + threadIdx.x; a < n; a += (long long)gridDim.x * blockDim.x) {
+    for (long long a = tid; a < n; a += nth) {
         double dv = d[a], lv = l[a];
         if (beta != 0.0) {
             dv = fma(-beta, Dg[a], dv);
             lv = fma(-beta, Lg[a], lv);
             d[a] = dv; l[a] = lv;
         }
-        if (!final) continue;
-        const StructInfo& T = tab[seg[a]];
+        const StructInfo& T = tab[items[a].seg];
         const int f = T.flags;
         const double w = T.what;
+        if (!final) {
+            double2 v;
+            v.x = (f & F_DOSE_REF) ? 2.0 * w * (dv - T.dose_ref) : 0.0;
+            v.y = (f & F_DL_REF) ? 2.0 * w * (lv - T.dl_ref) : 0.0;
+            pq[a] = v;
+            continue;
+        }
         double cD = 0.0, cL = 0.0, cT = 0.0;
         if (f & (F_DOSE_SLAB)) {
             const double r = slab_residual(dv, T.dose_lo, T.dose_hi);
@@ -327,8 +430,10 @@ k_residual(long long n, const int32_t* __restrict__ seg, const StructInfo* __res
         if (f & F_DOSE_REF) { const double e = T.dose_ref - dv; phi += w * e * e; }
         if (f & F_DL_REF) { const double e = T.dl_ref - lv; phi += w * e * e; }
         if (write_uv) {
-            u[a] = (f & F_LETD) ? cD - T.letd_max * cT : cD;     // row of the LETd set is L_i - LETmax D_i
-            v[a] = cL + cT;
+            double2 o;
+            o.x = (f & F_LETD) ? cD - T.letd_max * cT : cD;     // row of the LETd set is L_i - LETmax D_i
+            o.y = cL + cT;
+            uv[a] = o;
         }
     }
     if (final) {
@@ -383,25 +488,31 @@ __global__ void k_f64_to_f32(const double* __restrict__ in, float* __restrict__ 
     for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (long long)gridDim.x * blockDim.x)
         out[i] = (float)in[i];
 }
-// out[a] = (double) in[vox[a]]   (voxel-indexed fp32 -> list-indexed fp64)
-__global__ void k_gather_f32_to_f64(const float* __restrict__ in, const int32_t* __restrict__ vox,
-                                    double* __restrict__ out, long long n) {
-    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (long long)gridDim.x * blockDim.x)
-        out[i] = (double)in[vox[i]];
+// out[a] = {u[vox[a]], v[vox[a]]}   (voxel-indexed fp32 -> item-indexed fp64 pairs; a null input reads as 0)
+__global__ void k_gather_uv(const float* __restrict__ u, const float* __restrict__ v, const int32_t* __restrict__ vox,
+                            double2* __restrict__ out, long long n) {
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (long long)gridDim.x * blockDim.x) {
+        const int vx = vox[i];
+        double2 o;
+        o.x = u ? (double)u[vx] : 0.0;
+        o.y = v ? (double)v[vx] : 0.0;
+        out[i] = o;
+    }
 }
 
-// read-only streaming sum (practical ceiling of a 100%-read pass)
-__global__ void __launch_bounds__(512)
+// read-only streaming sum (practical ceiling of a 100%-read pass): 8 independent 128-bit loads per thread
+__global__ void __launch_bounds__(256)
 k_stream_read(const int4* __restrict__ p, long long n16, int* __restrict__ sink) {
-    int acc = 0;
-    long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-    const long long stride = (long long)gridDim.x * blockDim.x;
-    for (; i + 3 * stride < n16; i += 4 * stride) {
-        const int4 a = ld_stream_i4((const int32_t*)(p + i)), b = ld_stream_i4((const int32_t*)(p + i + stride));
-        const int4 c = ld_stream_i4((const int32_t*)(p + i + 2 * stride)), d = ld_stream_i4((const int32_t*)(p + i + 3 * stride));
-        acc += a.x ^ a.y ^ a.z ^ a.w ^ b.x ^ b.y ^ b.z ^ b.w ^ c.x ^ c.y ^ c.z ^ c.w ^ d.x ^ d.y ^ d.z ^ d.w;
+    const long long base = (long long)blockIdx.x * 2048 + threadIdx.x;
+    int4 v[8];
+#pragma unroll
+    for (int u = 0; u < 8; ++u) {
+        const long long i = base + u * 256;
+        v[u] = i < n16 ? ld_stream_i4((const int32_t*)(p + i)) : make_int4(0, 0, 0, 0);
     }
-    for (; i < n16; i += stride) { const int4 a = ld_stream_i4((const int32_t*)(p + i)); acc += a.x ^ a.y ^ a.z ^ a.w; }
+    int acc = 0;
+#pragma unroll
+    for (int u = 0; u < 8; ++u) acc += v[u].x ^ v[u].y ^ v[u].z ^ v[u].w;
     if (acc == 0x7fffffff) *sink = acc;      // never true in practice; keeps the loads alive
 }
 
