@@ -259,6 +259,17 @@ __global__ void k_fill_active(const int32_t* vox, const int32_t* lab_sorted, con
     }
 }
 
+// Storage order inside a row (or a transposed run) of padded length Lp: every chunk of n <= 128 entries (n a
+// multiple of 4, q = n/4 lanes) is interleaved so that memory position 4t+k of the chunk holds the chunk's logical
+// entry t + q*k.  A lane's 128-bit load then yields entries t, t+q, t+2q, t+3q, and the k-th gather instruction of
+// the warp covers q CONSECUTIVE entries: few cache lines of the gathered vector per instruction.
+__device__ __forceinline__ long long perm_pos(long long e, long long Lp) {
+    const long long cb = e & ~127LL;
+    const long long rem = Lp - cb;
+    const int n = rem < 128 ? (int)rem : 128, q = n >> 2, r = (int)(e - cb);
+    return cb + 4 * (r % q) + r / q;
+}
+
 // copy the rows into the padded arrays (warp per non-empty row); padding stays {col 0, value 0}
 __global__ void k_copy_padded(long long n, const int32_t* vox, const long long* start, const long long* ptr, const int32_t* cU,
                               const float* uD, const float* uL, int32_t* col, float* vD, float* vL) {
@@ -266,10 +277,12 @@ __global__ void k_copy_padded(long long n, const int32_t* vox, const long long* 
     const long long w0 = ((long long)blockIdx.x * blockDim.x + threadIdx.x) >> 5, nw = ((long long)gridDim.x * blockDim.x) >> 5;
     for (long long r = w0; r < n; r += nw) {
         const long long i = vox[r], b = ptr[i], e = ptr[i + 1], o = start[r];
+        const long long Lp = (e - b + 3) & ~3LL;
         for (long long p = b + lane; p < e; p += 32) {
-            col[o + (p - b)] = cU[p];
-            vD[o + (p - b)] = uD[p];
-            vL[o + (p - b)] = uL[p];
+            const long long m = o + perm_pos(p - b, Lp);
+            col[m] = cU[p];
+            vD[m] = uD[p];
+            vL[m] = uL[p];
         }
     }
 }
@@ -347,8 +360,9 @@ __global__ void k_tr_keys(RowList rl, const int32_t* ulen, const long long* off,
         const long long s = rl.start[r], o = off[r];
         const int L = ulen[r];
         const int sg = rl.seg ? rl.seg[r] : 0;
+        const int Lp = rl.len[r];
         for (int p = lane; p < L; p += 32) {
-            keys[o + p] = (uint32_t)col[s + p] * (uint32_t)n_seg + (uint32_t)sg;
+            keys[o + p] = (uint32_t)col[s + perm_pos(p, Lp)] * (uint32_t)n_seg + (uint32_t)sg;
             vals[o + p] = (uint32_t)(o + p);
         }
     }
@@ -366,15 +380,15 @@ __global__ void k_tr_pcount(const long long* ustart, long long K, long long* pco
         pcount[k] = (ustart[k + 1] - ustart[k] + 3) & ~3LL;
 }
 __global__ void k_tr_fill(const uint32_t* keys, const uint32_t* vals, long long E, const long long* ustart, const long long* t_ptr,
-                          const long long* off, long long n_rows, const long long* start, const float* vD, const float* vL,
-                          int32_t* t_col, float* tD, float* tL) {
+                          const long long* off, long long n_rows, const long long* start, const int32_t* len, const float* vD,
+                          const float* vL, int32_t* t_col, float* tD, float* tL) {
     for (long long r = (long long)blockIdx.x * blockDim.x + threadIdx.x; r < E; r += (long long)gridDim.x * blockDim.x) {
         const long long k = keys[r], e = vals[r];
         // row a with off[a] <= e < off[a+1]
         long long lo = 0, hi = n_rows;
         while (lo < hi) { const long long mid = (lo + hi) >> 1; if (off[mid + 1] <= e) lo = mid + 1; else hi = mid; }
-        const long long a = lo, p = start[a] + (e - off[a]);
-        const long long dst = t_ptr[k] + (r - ustart[k]);
+        const long long a = lo, p = start[a] + perm_pos(e - off[a], len[a]);
+        const long long dst = t_ptr[k] + perm_pos(r - ustart[k], t_ptr[k + 1] - t_ptr[k]);
         t_col[dst] = (int32_t)a;
         tD[dst] = vD[p];
         tL[dst] = vL[p];
@@ -491,7 +505,7 @@ static int build_transpose(fredopt_plan* P, RowSet& R) {
     CKC(cudaMemsetAsync(R.t_col, 0, Tn * 4, st));
     CKC(cudaMemsetAsync(R.t_valD, 0, Tn * 4, st));
     CKC(cudaMemsetAsync(R.t_valL, 0, Tn * 4, st));
-    if (E) k_tr_fill<<<grid_for(E, 256, 1 << 16), 256, 0, st>>>(keys2, vals2, E, ustart, R.t_ptr, off, n, R.start, R.valD, R.valL,
+    if (E) k_tr_fill<<<grid_for(E, 256, 1 << 16), 256, 0, st>>>(keys2, vals2, E, ustart, R.t_ptr, off, n, R.start, R.len, R.valD, R.valL,
                                                              R.t_col, R.t_valD, R.t_valL);
     CKC(cudaGetLastError());
     // ---- work items: every (spot, segment) run cut into pieces of at most TR_ITEM_MAX entries
