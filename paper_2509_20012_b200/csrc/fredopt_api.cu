@@ -55,9 +55,9 @@ struct RowSet {
     int32_t* ulen = nullptr;         // [n] unpadded
     Item* items = nullptr;           // [n] {start, len, seg}: what the forward kernel reads
     long long nnz = 0;               // unpadded entries in the set
-    // CSR of the transposes restricted to this set: rows = spots, per-segment runs, columns = list index
+    // CSR of the transposes restricted to this set, SEGMENT-major: run k = seg*S + spot; columns = list index
     bool t_built = false;
-    long long* t_ptr = nullptr;      // [S*n_seg + 1]
+    long long* t_ptr = nullptr;      // [n_seg*S + 1]
     int32_t* t_col = nullptr;
     float* t_valD = nullptr;
     float* t_valL = nullptr;
@@ -65,8 +65,8 @@ struct RowSet {
     // work items of the transposed pass: runs cut into pieces of at most TR_ITEM_MAX entries
     long long t_n_items = 0;
     Item* t_items = nullptr;         // [t_n_items]
-    int32_t* t_item_spot = nullptr;  // [t_n_items]
-    long long* t_item_ptr = nullptr; // [S+1] items of spot j: t_item_ptr[j] .. t_item_ptr[j+1]-1
+    int2* t_item_js = nullptr;       // [t_n_items] {spot, slot of the item's partial sum}
+    long long* t_item_ptr = nullptr; // [S+1] partial-sum slots of spot j: t_item_ptr[j] .. t_item_ptr[j+1]-1
     double* t_partial = nullptr;     // [t_n_items]
     unsigned int* t_counter = nullptr;  // [S] arrival counters (0 between launches)
     RowList view() const { return RowList{n, start, len, seg, vox}; }
@@ -95,8 +95,8 @@ struct fredopt_plan {
     // vectors (fp64)
     double *x = nullptr, *g = nullptr, *xtmp = nullptr;                       // [S]
     double *d = nullptr, *l = nullptr, *Dg = nullptr, *Lg = nullptr;          // [VA]
-    double2 *pq = nullptr, *uv = nullptr;                                      // [VA] gather vectors of the transposed passes
-    double2* fullUV = nullptr;                                                 // lazily: [full.n] gather vector for ROWS_ALL transposes
+    GatherVec pq{nullptr, nullptr, nullptr}, uv{nullptr, nullptr, nullptr};    // [VA] gather vectors of the transposed passes
+    GatherVec fullUV{nullptr, nullptr, nullptr};                               // lazily: [full.n] gather vector for ROWS_ALL transposes
     double* cpart = nullptr;
     double *part_prox = nullptr, *part_phi = nullptr;
     long long* part_cnt = nullptr;
@@ -133,6 +133,14 @@ static void dfree(fredopt_plan* P, void* p) {
     for (size_t i = 0; i < P->allocs.size(); ++i)
         if (P->allocs[i] == p) { P->allocs[i] = P->allocs.back(); P->allocs.pop_back(); break; }
     cudaFree(p);
+}
+
+static int gv_alloc(fredopt_plan* P, GatherVec* g, size_t n) {
+    CKR(dmalloc(P, &g->pair, n)); CKR(dmalloc(P, &g->cD, n)); CKR(dmalloc(P, &g->cL, n));
+    CK(cudaMemsetAsync(g->pair, 0, (n ? n : 1) * 16, P->stream));
+    CK(cudaMemsetAsync(g->cD, 0, (n ? n : 1) * 8, P->stream));
+    CK(cudaMemsetAsync(g->cL, 0, (n ? n : 1) * 8, P->stream));
+    return FREDOPT_OK;
 }
 
 static bool is_device_ptr(const void* p) {
@@ -352,7 +360,7 @@ __global__ void k_finish_tables(StructInfo* tab, int n_struct, DevState* st, uin
 }
 
 // ---- transposition of a row set
-__global__ void k_tr_keys(RowList rl, const int32_t* ulen, const long long* off, const int32_t* col, int n_seg,
+__global__ void k_tr_keys(RowList rl, const int32_t* ulen, const long long* off, const int32_t* col, long long S,
                           uint32_t* keys, uint32_t* vals) {
     const int lane = threadIdx.x & 31;
     const long long w0 = ((long long)blockIdx.x * blockDim.x + threadIdx.x) >> 5, nw = ((long long)gridDim.x * blockDim.x) >> 5;
@@ -362,7 +370,7 @@ __global__ void k_tr_keys(RowList rl, const int32_t* ulen, const long long* off,
         const int sg = rl.seg ? rl.seg[r] : 0;
         const int Lp = rl.len[r];
         for (int p = lane; p < L; p += 32) {
-            keys[o + p] = (uint32_t)col[s + perm_pos(p, Lp)] * (uint32_t)n_seg + (uint32_t)sg;
+            keys[o + p] = (uint32_t)sg * (uint32_t)S + (uint32_t)col[s + perm_pos(p, Lp)];
             vals[o + p] = (uint32_t)(o + p);
         }
     }
@@ -407,22 +415,28 @@ __global__ void k_tr_item_count(const long long* t_ptr, long long K, long long* 
     for (long long k = (long long)blockIdx.x * blockDim.x + threadIdx.x; k < K; k += (long long)gridDim.x * blockDim.x)
         cnt[k] = (t_ptr[k + 1] - t_ptr[k] + TR_ITEM_MAX - 1) / TR_ITEM_MAX;
 }
-__global__ void k_tr_item_fill(const long long* t_ptr, const long long* ibase, long long K, int n_seg, Item* items,
-                               int32_t* item_spot) {
-    for (long long k = (long long)blockIdx.x * blockDim.x + threadIdx.x; k < K; k += (long long)gridDim.x * blockDim.x) {
+// the same counts in spot-major order (the order of a spot's partial-sum slots)
+__global__ void k_tr_item_count_sm(const long long* cnt, long long S, int n_seg, long long* cnt_sm) {
+    for (long long k = (long long)blockIdx.x * blockDim.x + threadIdx.x; k < S * n_seg; k += (long long)gridDim.x * blockDim.x)
+        cnt_sm[(k % S) * n_seg + k / S] = cnt[k];
+}
+__global__ void k_tr_item_fill(const long long* t_ptr, const long long* ibase, const long long* sbase, long long S, int n_seg,
+                               Item* items, int2* item_js) {
+    for (long long k = (long long)blockIdx.x * blockDim.x + threadIdx.x; k < S * n_seg; k += (long long)gridDim.x * blockDim.x) {
         const long long b = t_ptr[k], e = t_ptr[k + 1];
-        long long i = ibase[k];
-        for (long long p = b; p < e; p += TR_ITEM_MAX, ++i) {
+        const long long j = k % S, sg = k / S;
+        long long i = ibase[k], slot = sbase[j * n_seg + sg];
+        for (long long p = b; p < e; p += TR_ITEM_MAX, ++i, ++slot) {
             Item it;
-            it.start = p; it.len = (int32_t)((e - p) < TR_ITEM_MAX ? (e - p) : TR_ITEM_MAX); it.seg = (int32_t)(k % n_seg);
+            it.start = p; it.len = (int32_t)((e - p) < TR_ITEM_MAX ? (e - p) : TR_ITEM_MAX); it.seg = (int32_t)sg;
             items[i] = it;
-            item_spot[i] = (int32_t)(k / n_seg);
+            item_js[i] = make_int2((int)j, (int)slot);
         }
     }
 }
-__global__ void k_tr_item_ptr(const long long* ibase, long long S, int n_seg, long long* item_ptr) {
+__global__ void k_tr_item_ptr(const long long* sbase, long long S, int n_seg, long long* item_ptr) {
     for (long long j = (long long)blockIdx.x * blockDim.x + threadIdx.x; j <= S; j += (long long)gridDim.x * blockDim.x)
-        item_ptr[j] = ibase[j * n_seg];
+        item_ptr[j] = sbase[j * n_seg];
 }
 __global__ void k_i32_to_i64(const int32_t* in, long long* out, long long n) {
     for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (long long)gridDim.x * blockDim.x) out[i] = in[i];
@@ -483,7 +497,7 @@ static int build_transpose(fredopt_plan* P, RowSet& R) {
     CKC(cudaMalloc(&keys, En * 4)); CKC(cudaMalloc(&vals, En * 4));
     CKC(cudaMalloc(&keys2, En * 4)); CKC(cudaMalloc(&vals2, En * 4));
     CKC(cudaMalloc(&ustart, (K + 2) * sizeof(long long))); CKC(cudaMalloc(&pcount, (K + 2) * sizeof(long long)));
-    if (n) k_tr_keys<<<grid_for(n * 32, 256, 1 << 16), 256, 0, st>>>(R.view(), R.ulen, off, R.col, R.n_seg, keys, vals);
+    if (n) k_tr_keys<<<grid_for(n * 32, 256, 1 << 16), 256, 0, st>>>(R.view(), R.ulen, off, R.col, S, keys, vals);
     int bits = 1;
     while ((1LL << bits) < K) ++bits;
     size_t tb = 0;
@@ -508,19 +522,29 @@ static int build_transpose(fredopt_plan* P, RowSet& R) {
     if (E) k_tr_fill<<<grid_for(E, 256, 1 << 16), 256, 0, st>>>(keys2, vals2, E, ustart, R.t_ptr, off, n, R.start, R.len, R.valD, R.valL,
                                                              R.t_col, R.t_valD, R.t_valL);
     CKC(cudaGetLastError());
-    // ---- work items: every (spot, segment) run cut into pieces of at most TR_ITEM_MAX entries
+    // ---- work items: every (segment, spot) run cut into pieces of at most TR_ITEM_MAX entries, in run order
+    //      (neighbouring items = neighbouring spots of one structure: overlapping voxel footprints share L1 lines)
     CKC(cudaMemsetAsync(pcount, 0, (K + 2) * sizeof(long long), st));
     k_tr_item_count<<<grid_for(K, 256, 4096), 256, 0, st>>>(R.t_ptr, K, pcount);
-    ret = scan_exclusive(P, pcount, ustart, K + 1);      // ustart now = first item of each run
-    if (ret) { cleanup(); return ret; }
-    CKC(cudaMemcpyAsync(&R.t_n_items, ustart + K, sizeof(long long), cudaMemcpyDeviceToHost, st));
-    CKC(cudaStreamSynchronize(st));
-    if ((ret = dmalloc(P, &R.t_items, (size_t)R.t_n_items)) || (ret = dmalloc(P, &R.t_item_spot, (size_t)R.t_n_items)) ||
+    long long *cnt_sm = nullptr, *sbase = nullptr;
+    CKC(cudaMalloc(&cnt_sm, (K + 2) * sizeof(long long)));
+    { cudaError_t e_ = cudaMalloc(&sbase, (K + 2) * sizeof(long long)); if (e_ != cudaSuccess) { cudaFree(cnt_sm); CKC(e_); } }
+    auto cleanup2 = [&]() { cudaFree(cnt_sm); cudaFree(sbase); cleanup(); };
+    cudaMemsetAsync(cnt_sm, 0, (K + 2) * sizeof(long long), st);
+    k_tr_item_count_sm<<<grid_for(K, 256, 4096), 256, 0, st>>>(pcount, S, R.n_seg, cnt_sm);
+    ret = scan_exclusive(P, pcount, ustart, K + 1);      // ustart now = first item of each run (execution order)
+    if (!ret) ret = scan_exclusive(P, cnt_sm, sbase, K + 1);   // first partial-sum slot of each (spot, segment)
+    if (ret) { cleanup2(); return ret; }
+    if (cudaMemcpyAsync(&R.t_n_items, ustart + K, sizeof(long long), cudaMemcpyDeviceToHost, st) != cudaSuccess ||
+        cudaStreamSynchronize(st) != cudaSuccess) { cleanup2(); return FREDOPT_CUDA_ERROR; }
+    if ((ret = dmalloc(P, &R.t_items, (size_t)R.t_n_items)) || (ret = dmalloc(P, &R.t_item_js, (size_t)R.t_n_items)) ||
         (ret = dmalloc(P, &R.t_item_ptr, (size_t)S + 1)) || (ret = dmalloc(P, &R.t_partial, (size_t)R.t_n_items)) ||
-        (ret = dmalloc(P, &R.t_counter, (size_t)S))) { cleanup(); return ret; }
-    CKC(cudaMemsetAsync(R.t_counter, 0, (S ? S : 1) * sizeof(unsigned int), st));
-    k_tr_item_fill<<<grid_for(K, 256, 4096), 256, 0, st>>>(R.t_ptr, ustart, K, R.n_seg, R.t_items, R.t_item_spot);
-    k_tr_item_ptr<<<grid_for(S + 1, 256, 4096), 256, 0, st>>>(ustart, S, R.n_seg, R.t_item_ptr);
+        (ret = dmalloc(P, &R.t_counter, (size_t)S))) { cleanup2(); return ret; }
+    cudaMemsetAsync(R.t_counter, 0, (S ? S : 1) * sizeof(unsigned int), st);
+    k_tr_item_fill<<<grid_for(K, 256, 4096), 256, 0, st>>>(R.t_ptr, ustart, sbase, S, R.n_seg, R.t_items, R.t_item_js);
+    k_tr_item_ptr<<<grid_for(S + 1, 256, 4096), 256, 0, st>>>(sbase, S, R.n_seg, R.t_item_ptr);
+    if (cudaGetLastError() != cudaSuccess || cudaStreamSynchronize(st) != cudaSuccess) { cleanup2(); return FREDOPT_CUDA_ERROR; }
+    cudaFree(cnt_sm); cudaFree(sbase);
     CKC(cudaGetLastError());
     CKC(cudaStreamSynchronize(st));
     cleanup();
@@ -583,23 +607,23 @@ static void launch_forward(fredopt_plan* P, const RowSet& R, const uint8_t* mode
     if (R.n == 0) { if (epi == EPI_CPART) cudaMemsetAsync(P->cpart, 0, sizeof(double) * MAX_PARTIALS, P->stream); return; }
     const int g = fwd_grid(P, R.n);
     if (epi == EPI_CPART)
-        k_forward<EPI_CPART><<<g, FWD_THREADS, 0, P->stream>>>(R.n, R.items, R.vox, mode, R.col, R.valD, R.valL, x, oD, oL, nullptr,
+        k_forward<EPI_CPART><<<g, FWD_THREADS, 0, P->stream>>>(R.n, R.items, R.vox, mode, R.col, R.valD, R.valL, x, oD, oL, GatherVec{nullptr, nullptr, nullptr},
                                                                P->tab, P->cpart, nullptr, nullptr, 0);
     else if (epi == EPI_STORE_PQ)
         k_forward<EPI_STORE_PQ><<<g, FWD_THREADS, 0, P->stream>>>(R.n, R.items, R.vox, mode, R.col, R.valD, R.valL, x, oD, oL, P->pq,
                                                                   P->tab, nullptr, nullptr, nullptr, 0);
     else
-        k_forward<EPI_STORE><<<g, FWD_THREADS, 0, P->stream>>>(R.n, R.items, R.vox, mode, R.col, R.valD, R.valL, x, oD, oL, nullptr,
+        k_forward<EPI_STORE><<<g, FWD_THREADS, 0, P->stream>>>(R.n, R.items, R.vox, mode, R.col, R.valD, R.valL, x, oD, oL, GatherVec{nullptr, nullptr, nullptr},
                                                                nullptr, nullptr, nullptr, nullptr, 0);
     ++P->launches;
 }
 static int cpart_count(fredopt_plan* P) { return P->act.n ? fwd_grid(P, P->act.n) : MAX_PARTIALS; }
 
 template <int EPI>
-static void launch_transpose(fredopt_plan* P, const RowSet& R, const uint8_t* mode, const double2* vec, double* g_out, double* x,
+static void launch_transpose(fredopt_plan* P, const RowSet& R, const uint8_t* mode, const GatherVec& vec, double* g_out, double* x,
                              float* f_out) {
     if (R.t_n_items == 0) return;
-    k_transpose<EPI><<<fwd_grid(P, R.t_n_items), FWD_THREADS, 0, P->stream>>>(R.t_n_items, R.t_items, R.t_item_spot, R.t_item_ptr, mode,
+    k_transpose<EPI><<<fwd_grid(P, R.t_n_items), FWD_THREADS, 0, P->stream>>>(R.t_n_items, R.t_items, R.t_item_js, R.t_item_ptr, mode,
                                                                              R.t_col, R.t_valD, R.t_valL, vec, R.t_partial, R.t_counter,
                                                                              g_out, x, P->st, f_out);
     ++P->launches;
@@ -871,8 +895,7 @@ static int create_impl(fredopt_plan* P, const fredopt_csr* D, const fredopt_csr*
     CK(cudaMemsetAsync(P->x, 0, (S ? S : 1) * 8, st)); CK(cudaMemsetAsync(P->g, 0, (S ? S : 1) * 8, st));
     double** vecs[] = {&P->d, &P->l, &P->Dg, &P->Lg};
     for (auto pp : vecs) { CKR(dmalloc(P, pp, (size_t)n_act)); CK(cudaMemsetAsync(*pp, 0, (n_act ? n_act : 1) * 8, st)); }
-    CKR(dmalloc(P, &P->pq, (size_t)n_act)); CKR(dmalloc(P, &P->uv, (size_t)n_act));
-    CK(cudaMemsetAsync(P->pq, 0, (n_act ? n_act : 1) * 16, st)); CK(cudaMemsetAsync(P->uv, 0, (n_act ? n_act : 1) * 16, st));
+    CKR(gv_alloc(P, &P->pq, (size_t)n_act)); CKR(gv_alloc(P, &P->uv, (size_t)n_act));
     CKR(dmalloc(P, &P->cpart, (size_t)MAX_PARTIALS)); CKR(dmalloc(P, &P->part_prox, (size_t)MAX_PARTIALS));
     CKR(dmalloc(P, &P->part_phi, (size_t)MAX_PARTIALS)); CKR(dmalloc(P, &P->part_cnt, (size_t)MAX_PARTIALS));
     CKR(dmalloc(P, &P->sink, 4));
@@ -988,8 +1011,8 @@ static int forward_f32(fredopt_plan* P, const RowSet& R, int m, const double* xd
     if (dl) cudaMemsetAsync(dl, 0, (size_t)P->V * 4, P->stream);
     if (R.n) {
         k_forward<EPI_F32VOX><<<fwd_grid(P, R.n), FWD_THREADS, 0, P->stream>>>(R.n, R.items, R.vox, P->mode_fixed + (size_t)m * P->max_seg,
-                                                                               R.col, R.valD, R.valL, xd, nullptr, nullptr, nullptr,
-                                                                               nullptr, nullptr, dd, dl, letd_out);
+                                                                               R.col, R.valD, R.valL, xd, nullptr, nullptr,
+                                                                               GatherVec{nullptr, nullptr, nullptr}, nullptr, nullptr, dd, dl, letd_out);
         ++P->launches;
     }
     int rc = FREDOPT_OK;
@@ -1020,10 +1043,10 @@ int fredopt_spmv_forward(fredopt_plan* P, int32_t rows, const float* x, float* d
 int fredopt_spmv_transpose(fredopt_plan* P, int32_t rows, const float* u, const float* v, float* out) {
     if (!P || !out || (!u && !v) || (rows != FREDOPT_ROWS_ALL && rows != FREDOPT_ROWS_ACTIVE)) return FREDOPT_INVALID_ARG;
     RowSet& R = rows == FREDOPT_ROWS_ALL ? P->full : P->act;
-    double2* vec = P->uv;
+    GatherVec vec = P->uv;
     if (rows == FREDOPT_ROWS_ALL) {
         if (!R.t_built) CKR(build_transpose(P, R));
-        if (!P->fullUV) CKR(dmalloc(P, &P->fullUV, (size_t)R.n));
+        if (!P->fullUV.pair) CKR(gv_alloc(P, &P->fullUV, (size_t)R.n));
         vec = P->fullUV;
     }
     const float *du = nullptr, *dv = nullptr; void *fu = nullptr, *fv = nullptr;

@@ -54,6 +54,18 @@ struct __align__(16) Item {
     int32_t seg;
 };
 
+// Gather vector of a transposed pass, item-indexed, kept in two layouts: runs that need both matrices gather one
+// 16-byte pair per entry; runs that need one matrix gather from the dense 8-byte array (four rows per 32-byte sector).
+struct GatherVec {
+    double2* pair;   // {coefficient of D_i, coefficient of L_i}
+    double* cD;
+    double* cL;
+};
+__device__ __forceinline__ void gv_store(const GatherVec& g, long long a, double vd, double vl) {
+    double2 v; v.x = vd; v.y = vl;
+    g.pair[a] = v; g.cD[a] = vd; g.cL[a] = vl;
+}
+
 // ------------------------------------------------------------------------------------------ loads
 // streamed arrays (index / value): read once, keep them out of L1 so that L1 holds the gathered vector
 __device__ __forceinline__ int4 ld_stream_i4(const int32_t* p) {
@@ -155,7 +167,7 @@ k_forward(long long n, const Item* __restrict__ items, const int32_t* __restrict
           const int32_t* __restrict__ col, const float* __restrict__ vD, const float* __restrict__ vL,
           const double* __restrict__ x,
           double* __restrict__ oD, double* __restrict__ oL,                // EPI_STORE*, EPI_CPART: item-indexed
-          double2* __restrict__ pq,                                        // EPI_STORE_PQ: cost residuals (Eq. 2)
+          const GatherVec pq,                                              // EPI_STORE_PQ: cost residuals (Eq. 2)
           const StructInfo* __restrict__ tab, double* __restrict__ cpart,  // EPI_STORE_PQ / EPI_CPART
           float* __restrict__ fD, float* __restrict__ fL, int letd_out)    // EPI_F32VOX: voxel-indexed
 {
@@ -187,10 +199,8 @@ k_forward(long long n, const Item* __restrict__ items, const int32_t* __restrict
                 oL[r] = aL;
                 if (EPI == EPI_STORE_PQ) {      // p_i = 2 w^ (d_i - Dref), q_i = 2 w^ (l_i - cDLref): grad chi^2 = D^T p + L^T q
                     const StructInfo& T = tab[it.seg];
-                    double2 v;
-                    v.x = (T.flags & F_DOSE_REF) ? 2.0 * T.what * (aD - T.dose_ref) : 0.0;
-                    v.y = (T.flags & F_DL_REF) ? 2.0 * T.what * (aL - T.dl_ref) : 0.0;
-                    pq[r] = v;
+                    gv_store(pq, r, (T.flags & F_DOSE_REF) ? 2.0 * T.what * (aD - T.dose_ref) : 0.0,
+                             (T.flags & F_DL_REF) ? 2.0 * T.what * (aL - T.dl_ref) : 0.0);
                 }
                 if (EPI == EPI_CPART) {
                     const StructInfo& T = tab[it.seg];
@@ -217,9 +227,10 @@ enum : int { TEPI_F32 = 0, TEPI_GRAD = 1, TEPI_UPDATE = 2 };
 // ascending compact row indices, so neighbouring lanes gather neighbouring elements)
 template <int M>
 __device__ __forceinline__ double tr_item(const int32_t* __restrict__ cp, const float* __restrict__ dp,
-                                          const float* __restrict__ lp, int L, int lane, const double2* __restrict__ vec) {
+                                          const float* __restrict__ lp, int L, int lane, const GatherVec& gv) {
     constexpr int U = 4;
-    const double* vs = (const double*)vec;
+    const double2* __restrict__ vec = gv.pair;
+    const double* __restrict__ vs = (M == 2) ? gv.cL : gv.cD;
     double aD = 0.0, aL = 0.0;
     int p = lane * 4;
     for (; p + 128 * (U - 1) < L; p += 128 * U) {
@@ -238,9 +249,7 @@ __device__ __forceinline__ double tr_item(const int32_t* __restrict__ cp, const 
                 fma4(aD, d[u], g0.x, g1.x, g2.x, g3.x);
                 fma4(aL, l[u], g0.y, g1.y, g2.y, g3.y);
             } else {
-                constexpr int o = (M == 2) ? 1 : 0;
-                const double g0 = __ldg(vs + 2 * (long long)c[u].x + o), g1 = __ldg(vs + 2 * (long long)c[u].y + o);
-                const double g2 = __ldg(vs + 2 * (long long)c[u].z + o), g3 = __ldg(vs + 2 * (long long)c[u].w + o);
+                const double g0 = __ldg(vs + c[u].x), g1 = __ldg(vs + c[u].y), g2 = __ldg(vs + c[u].z), g3 = __ldg(vs + c[u].w);
                 if (M == 1) fma4(aD, d[u], g0, g1, g2, g3); else fma4(aL, l[u], g0, g1, g2, g3);
             }
         }
@@ -253,27 +262,27 @@ __device__ __forceinline__ double tr_item(const int32_t* __restrict__ cp, const 
             fma4(aD, d0, g0.x, g1.x, g2.x, g3.x);
             fma4(aL, l0, g0.y, g1.y, g2.y, g3.y);
         } else {
-            constexpr int o = (M == 2) ? 1 : 0;
             const float4 a0 = ld_stream_f4((M == 1 ? dp : lp) + p);
-            const double g0 = __ldg(vs + 2 * (long long)c0.x + o), g1 = __ldg(vs + 2 * (long long)c0.y + o);
-            const double g2 = __ldg(vs + 2 * (long long)c0.z + o), g3 = __ldg(vs + 2 * (long long)c0.w + o);
+            const double g0 = __ldg(vs + c0.x), g1 = __ldg(vs + c0.y), g2 = __ldg(vs + c0.z), g3 = __ldg(vs + c0.w);
             fma4(aD, a0, g0, g1, g2, g3);
         }
     }
     return aD + aL;
 }
 
-// One warp per item (round-robin).  The items of spot j are item_ptr[j] .. item_ptr[j+1]-1 (ascending structure,
-// then ascending position).  Every item stores its partial sum; the warp that completes the LAST outstanding item
+// One warp per item (round-robin; items are in (structure, spot) order so that the warps of a CTA work on
+// neighbouring spots of one structure).  Item r belongs to spot item_js[r].x and owns partial-sum slot item_js[r].y;
+// the slots of spot j are item_ptr[j] .. item_ptr[j+1]-1 (ascending structure, then ascending position).
+// Every item stores its partial sum; the warp that completes the LAST outstanding item
 // of a spot (per-spot arrival counter, integer atomics only) adds the spot's partials in item order and runs the
 // epilogue, then re-arms the counter.  The value is therefore independent of which warp finishes last.
 // Spots without items are never visited: their g / output stays 0 (set at creation / by the caller), their x is
 // already >= 0.
 template <int EPI>
 __global__ void __launch_bounds__(FWD_THREADS, 3)
-k_transpose(long long n, const Item* __restrict__ items, const int32_t* __restrict__ item_spot,
+k_transpose(long long n, const Item* __restrict__ items, const int2* __restrict__ item_js,
             const long long* __restrict__ item_ptr, const uint8_t* __restrict__ mode, const int32_t* __restrict__ t_col,
-            const float* __restrict__ tD, const float* __restrict__ tL, const double2* __restrict__ vec,
+            const float* __restrict__ tD, const float* __restrict__ tL, const GatherVec vec,
             double* __restrict__ partial, unsigned int* __restrict__ counter,
             double* __restrict__ g_out,                                 // TEPI_GRAD
             double* __restrict__ x, const DevState* __restrict__ st,   // TEPI_UPDATE
@@ -296,11 +305,12 @@ k_transpose(long long n, const Item* __restrict__ items, const int32_t* __restri
         else if (m == 2) tot = tr_item<2>(cp, nullptr, tL + it.start, it.len, lane, vec);
         if (m) tot = warp_sum(tot);
         if (lane == 0) {
-            const int j = item_spot[r];
+            const int2 js = item_js[r];
+            const int j = js.x;
             const long long ib = item_ptr[j], ie = item_ptr[j + 1];
             bool last = true;
             if (ie - ib > 1) {
-                partial[r] = tot;
+                partial[js.y] = tot;
                 __threadfence();
                 const unsigned int old = atomicAdd(counter + j, 1u);
                 last = old == (unsigned int)(ie - ib - 1);
@@ -386,7 +396,7 @@ __global__ void __launch_bounds__(ROW_THREADS)
 k_residual(long long n, const Item* __restrict__ items, const StructInfo* __restrict__ tab, DevState* st,
            double* __restrict__ d, double* __restrict__ l, const double* __restrict__ Dg, const double* __restrict__ Lg,
            const double* __restrict__ nD, const double* __restrict__ nL, const double* __restrict__ nT,
-           double2* __restrict__ uv, double2* __restrict__ pq, double* __restrict__ x, const double* __restrict__ g, long long S,
+           const GatherVec uv, const GatherVec pq, double* __restrict__ x, const double* __restrict__ g, long long S,
            double* __restrict__ part_prox, double* __restrict__ part_phi, long long* __restrict__ part_cnt,
            int use_beta, int final, int write_uv) {
     __shared__ double sm[ROW_THREADS / 32];
@@ -408,10 +418,7 @@ k_residual(long long n, const Item* __restrict__ items, const StructInfo* __rest
         const int f = T.flags;
         const double w = T.what;
         if (!final) {
-            double2 v;
-            v.x = (f & F_DOSE_REF) ? 2.0 * w * (dv - T.dose_ref) : 0.0;
-            v.y = (f & F_DL_REF) ? 2.0 * w * (lv - T.dl_ref) : 0.0;
-            pq[a] = v;
+            gv_store(pq, a, (f & F_DOSE_REF) ? 2.0 * w * (dv - T.dose_ref) : 0.0, (f & F_DL_REF) ? 2.0 * w * (lv - T.dl_ref) : 0.0);
             continue;
         }
         double cD = 0.0, cL = 0.0, cT = 0.0;
@@ -430,10 +437,8 @@ k_residual(long long n, const Item* __restrict__ items, const StructInfo* __rest
         if (f & F_DOSE_REF) { const double e = T.dose_ref - dv; phi += w * e * e; }
         if (f & F_DL_REF) { const double e = T.dl_ref - lv; phi += w * e * e; }
         if (write_uv) {
-            double2 o;
-            o.x = (f & F_LETD) ? cD - T.letd_max * cT : cD;     // row of the LETd set is L_i - LETmax D_i
-            o.y = cL + cT;
-            uv[a] = o;
+            gv_store(uv, a, (f & F_LETD) ? cD - T.letd_max * cT : cD,      // row of the LETd set is L_i - LETmax D_i
+                     cL + cT);
         }
     }
     if (final) {
@@ -490,13 +495,10 @@ __global__ void k_f64_to_f32(const double* __restrict__ in, float* __restrict__ 
 }
 // out[a] = {u[vox[a]], v[vox[a]]}   (voxel-indexed fp32 -> item-indexed fp64 pairs; a null input reads as 0)
 __global__ void k_gather_uv(const float* __restrict__ u, const float* __restrict__ v, const int32_t* __restrict__ vox,
-                            double2* __restrict__ out, long long n) {
+                            const GatherVec out, long long n) {
     for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (long long)gridDim.x * blockDim.x) {
         const int vx = vox[i];
-        double2 o;
-        o.x = u ? (double)u[vx] : 0.0;
-        o.y = v ? (double)v[vx] : 0.0;
-        out[i] = o;
+        gv_store(out, i, u ? (double)u[vx] : 0.0, v ? (double)v[vx] : 0.0);
     }
 }
 
