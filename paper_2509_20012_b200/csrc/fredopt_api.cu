@@ -7,6 +7,7 @@
 
 #include <cmath>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <string>
 #include <vector>
@@ -434,6 +435,20 @@ __global__ void k_tr_item_fill(const long long* t_ptr, const long long* ibase, c
         }
     }
 }
+// longest-first execution order: key = length class (256-entry bins, longest = 0); a stable sort keeps the
+// (structure, spot) order inside a class
+__global__ void k_tr_item_key(const Item* items, long long n, uint32_t* key, uint32_t* idx) {
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (long long)gridDim.x * blockDim.x) {
+        key[i] = (uint32_t)((TR_ITEM_MAX - items[i].len) / 256);
+        idx[i] = (uint32_t)i;
+    }
+}
+__global__ void k_tr_item_permute(const uint32_t* idx, long long n, const Item* items, const int2* js, Item* items2, int2* js2) {
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (long long)gridDim.x * blockDim.x) {
+        items2[i] = items[idx[i]];
+        js2[i] = js[idx[i]];
+    }
+}
 __global__ void k_tr_item_ptr(const long long* sbase, long long S, int n_seg, long long* item_ptr) {
     for (long long j = (long long)blockIdx.x * blockDim.x + threadIdx.x; j <= S; j += (long long)gridDim.x * blockDim.x)
         item_ptr[j] = sbase[j * n_seg];
@@ -545,6 +560,37 @@ static int build_transpose(fredopt_plan* P, RowSet& R) {
     k_tr_item_ptr<<<grid_for(S + 1, 256, 4096), 256, 0, st>>>(sbase, S, R.n_seg, R.t_item_ptr);
     if (cudaGetLastError() != cudaSuccess || cudaStreamSynchronize(st) != cudaSuccess) { cleanup2(); return FREDOPT_CUDA_ERROR; }
     cudaFree(cnt_sm); cudaFree(sbase);
+    // ---- longest items first: with the static round-robin mapping every round of the grid then holds items of
+    //      one length class, so the warps stay balanced to within one class width per round
+    if (R.t_n_items > 1) {
+        const long long ni = R.t_n_items;
+        uint32_t *ik = nullptr, *ik2 = nullptr, *ii = nullptr, *ii2 = nullptr;
+        Item* it2 = nullptr; int2* js2 = nullptr; void* stmp = nullptr;
+        auto cleanup3 = [&]() { cudaFree(ik); cudaFree(ik2); cudaFree(ii); cudaFree(ii2); cudaFree(it2); cudaFree(js2); cudaFree(stmp); cleanup(); };
+#define CK3(expr) do { cudaError_t e__ = (expr); if (e__ != cudaSuccess) { g_last_cuda_error = std::string(#expr) + ": " + cudaGetErrorString(e__); cudaGetLastError(); cleanup3(); return e__ == cudaErrorMemoryAllocation ? FREDOPT_OUT_OF_MEMORY : FREDOPT_CUDA_ERROR; } } while (0)
+        CK3(cudaMalloc(&ik, ni * 4)); CK3(cudaMalloc(&ik2, ni * 4)); CK3(cudaMalloc(&ii, ni * 4)); CK3(cudaMalloc(&ii2, ni * 4));
+        CK3(cudaMalloc(&it2, ni * sizeof(Item))); CK3(cudaMalloc(&js2, ni * sizeof(int2)));
+        k_tr_item_key<<<grid_for(ni, 256, 4096), 256, 0, st>>>(R.t_items, ni, ik, ii);
+        size_t sb = 0;
+        CK3(cub::DeviceRadixSort::SortPairs(nullptr, sb, ik, ik2, ii, ii2, ni, 0, 4, st));
+        CK3(cudaMalloc(&stmp, sb ? sb : 1));
+        CK3(cub::DeviceRadixSort::SortPairs(stmp, sb, ik, ik2, ii, ii2, ni, 0, 4, st));
+        k_tr_item_permute<<<grid_for(ni, 256, 4096), 256, 0, st>>>(ii2, ni, R.t_items, R.t_item_js, it2, js2);
+        CK3(cudaMemcpyAsync(R.t_items, it2, ni * sizeof(Item), cudaMemcpyDeviceToDevice, st));
+        CK3(cudaMemcpyAsync(R.t_item_js, js2, ni * sizeof(int2), cudaMemcpyDeviceToDevice, st));
+        CK3(cudaStreamSynchronize(st));
+#undef CK3
+        cudaFree(ik); cudaFree(ik2); cudaFree(ii); cudaFree(ii2); cudaFree(it2); cudaFree(js2); cudaFree(stmp);
+    }
+    if (getenv("FREDOPT_DEBUG")) {   // shape of the transposed work list (stderr; debugging aid only)
+        std::vector<Item> h((size_t)R.t_n_items);
+        cudaMemcpy(h.data(), R.t_items, sizeof(Item) * h.size(), cudaMemcpyDeviceToHost);
+        long long hist[8] = {0}, ent[8] = {0};
+        for (auto& it : h) { int b = it.len <= 32 ? 0 : it.len <= 128 ? 1 : it.len <= 256 ? 2 : it.len <= 512 ? 3 : it.len <= 1024 ? 4 : it.len < 2048 ? 5 : 6; ++hist[b]; ent[b] += it.len; }
+        fprintf(stderr, "[fredopt] transposed set: rows %lld spots %lld segs %d entries %lld padded %lld items %lld\n", n, S, R.n_seg, E, R.t_nnz_padded, R.t_n_items);
+        const char* nm[7] = {"<=32", "<=128", "<=256", "<=512", "<=1024", "<2048", "=2048"};
+        for (int b = 0; b < 7; ++b) fprintf(stderr, "[fredopt]   len %-6s items %8lld entries %10lld\n", nm[b], hist[b], ent[b]);
+    }
     CKC(cudaGetLastError());
     CKC(cudaStreamSynchronize(st));
     cleanup();
