@@ -33,9 +33,14 @@ ROOT = os.path.dirname(os.path.abspath(__file__))
 sys.path.insert(0, ROOT)
 
 METRIC = "superiorization iterations/sec"
+STATE_BYTES = 176           # sizeof(DevState): what fredopt_get_stats copies back
 UNIT = "iterations/s"
-DEFAULT_CONFIG = 1
+DEFAULT_CONFIG = 3          # BASELINE.json configs[3]: the clinical-size plan the metric is quoted on (fits one B200)
 DEFAULT_STEPS = {0: 50, 1: 200, 2: 100, 3: 50}
+NOMINAL_HBM_GBS = 8000.0    # north_star's "~8 TB/s peak" (context; the roofline denominator is the measured copy figure)
+# dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel from the committed `ncu --set full`
+# capture (profiles/r01_ncu_full_config3.md); keyed by (config, pass)
+NCU_TRAFFIC = {}
 
 
 def _peaks():
@@ -59,10 +64,13 @@ class ClockSampler:
     def start(self):
         try:
             self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.Q}",
-                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                          "--format=csv,noheader,nounits", "-lms", "20"],
                                          stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
             self.t = threading.Thread(target=self._read, daemon=True)
             self.t.start()
+            t0 = time.time()
+            while not self.rows and time.time() - t0 < 3.0:      # first sample before the timed region starts
+                time.sleep(0.01)
         except Exception:
             self.proc = None
 
@@ -167,13 +175,13 @@ def run_ours(args):
         torch.cuda.synchronize()
 
     # ---- device-resident timing: W warm-up iterations, then K iterations in one fredopt_iterate call
+    sampler = ClockSampler(lr)
+    sampler.start()
     gp.set_weights(plan.x0)
     gp.iterate(W, lam, beta0, a)
     if flush is not None:
         flush.zero_()
     barrier()
-    sampler = ClockSampler(lr)
-    sampler.start()
     l0 = gp.launch_count()
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     e0.record(stream)
@@ -194,8 +202,9 @@ def run_ours(args):
         gp.set_weights(xh)                    # H2D: S floats from pinned host memory
         gp.iterate(1, lam, beta0, a)
         gp.get_weights(xo)                    # D2H: S floats (synchronises)
-        prox, nviol = gp.proximity(None)      # D2H: the step's metric (fp64 + int64)
+        st_e = gp.stats()                     # D2H: the step's metrics (proximity, chi^2, violation count, k, s, beta)
         xh.copy_(xo)
+    prox, nviol = st_e["prox"], st_e["n_violated"]
     barrier()
     e2e_s = time.perf_counter() - t0
     clocks = sampler.stop()
@@ -207,6 +216,16 @@ def run_ours(args):
     gp.iterate(min(K, 50), lam, beta0, a)
     pt = gp.pass_times()
     gp.set_option(fredopt.OPT_TIME_PASSES, 0)
+    # ---- practical ceiling of a 100%-read pass: the library's streaming-read kernel over a buffer larger than L2
+    nb = 1 << 31
+    buf = torch.empty(nb, dtype=torch.uint8, device="cuda")
+    buf.zero_()
+    gp.stream_read(buf, nb, 3)
+    r0, r1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    r0.record(stream); gp.stream_read(buf, nb, 10); r1.record(stream)
+    torch.cuda.synchronize()
+    read_gbs = 10 * nb / (r0.elapsed_time(r1) * 1e-3) / 1e9
+    del buf
     top = max(pt, key=lambda n: pt[n][0])
     top_ms = pt[top][0] / max(pt[top][1], 1)
     peak, peak_src = _peaks()
@@ -214,6 +233,8 @@ def run_ours(args):
     passes = {n: {"ms": pt[n][0] / max(pt[n][1], 1), "alg_bytes": pass_bytes[n],
                   "gbs": pass_bytes[n] / max(pt[n][0] / max(pt[n][1], 1), 1e-9) / 1e6} for n in pt}
     stats = gp.stats()
+    spmv = ("forward_x", "transpose_g", "forward_g", "transpose_b")
+    four_gbs = sum(pass_bytes[n] for n in spmv) / max(sum(passes[n]["ms"] for n in spmv), 1e-9) / 1e6
 
     if dist is not None:
         t = torch.tensor([ms, e2e_s], dtype=torch.float64, device="cuda")
@@ -238,12 +259,15 @@ def run_ours(args):
                    "parallelism": "1 plan per GPU"},
         "iter_gbs": iter_bytes * K / (ms * 1e-3) / 1e9,
         "e2e": {"value": ws * K / e2e_s, "unit": UNIT, "h2d_bytes_per_step": plan.n_cols * 4,
-                "d2h_bytes_per_step": plan.n_cols * 4 + 16},
+                "d2h_bytes_per_step": plan.n_cols * 4 + STATE_BYTES},
         "gpu_launches": int(launches),
         "clocks": clocks,
         "roofline": {"bound": "hbm", "kernel": top, "achieved": achieved, "peak": peak, "unit": "GB/s",
-                     "frac": achieved / peak, "traffic": None, "peak_source": peak_src,
-                     "alg_bytes_per_launch": pass_bytes[top], "ms_per_launch": top_ms},
+                     "frac": achieved / peak, "traffic": NCU_TRAFFIC.get((args.config, top)), "peak_source": peak_src,
+                     "alg_bytes_per_launch": pass_bytes[top], "ms_per_launch": top_ms,
+                     "frac_of_nominal_8TBs": achieved / NOMINAL_HBM_GBS, "read_ceiling_gbs": read_gbs,
+                     "frac_of_read_ceiling": achieved / read_gbs,
+                     "four_spmv_passes_gbs": four_gbs, "four_spmv_passes_frac": four_gbs / peak},
         "passes": passes,
         "setup": {"generate_s": t_gen, "create_s": t_create},
         "final": {"prox": prox, "n_violated": nviol, "trials": stats["trials"]},

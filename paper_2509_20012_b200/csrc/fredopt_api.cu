@@ -66,10 +66,9 @@ struct RowSet {
     // work items of the transposed pass: runs cut into pieces of at most TR_ITEM_MAX entries
     long long t_n_items = 0;
     Item* t_items = nullptr;         // [t_n_items]
-    int2* t_item_js = nullptr;       // [t_n_items] {spot, slot of the item's partial sum}
+    int32_t* t_item_slot = nullptr;  // [t_n_items] slot of the item's partial sum
     long long* t_item_ptr = nullptr; // [S+1] partial-sum slots of spot j: t_item_ptr[j] .. t_item_ptr[j+1]-1
     double* t_partial = nullptr;     // [t_n_items]
-    unsigned int* t_counter = nullptr;  // [S] arrival counters (0 between launches)
     RowList view() const { return RowList{n, start, len, seg, vox}; }
 };
 
@@ -422,7 +421,7 @@ __global__ void k_tr_item_count_sm(const long long* cnt, long long S, int n_seg,
         cnt_sm[(k % S) * n_seg + k / S] = cnt[k];
 }
 __global__ void k_tr_item_fill(const long long* t_ptr, const long long* ibase, const long long* sbase, long long S, int n_seg,
-                               Item* items, int2* item_js) {
+                               Item* items, int32_t* item_slot) {
     for (long long k = (long long)blockIdx.x * blockDim.x + threadIdx.x; k < S * n_seg; k += (long long)gridDim.x * blockDim.x) {
         const long long b = t_ptr[k], e = t_ptr[k + 1];
         const long long j = k % S, sg = k / S;
@@ -431,7 +430,7 @@ __global__ void k_tr_item_fill(const long long* t_ptr, const long long* ibase, c
             Item it;
             it.start = p; it.len = (int32_t)((e - p) < TR_ITEM_MAX ? (e - p) : TR_ITEM_MAX); it.seg = (int32_t)sg;
             items[i] = it;
-            item_js[i] = make_int2((int)j, (int)slot);
+            item_slot[i] = (int32_t)slot;
         }
     }
 }
@@ -443,7 +442,7 @@ __global__ void k_tr_item_key(const Item* items, long long n, uint32_t* key, uin
         idx[i] = (uint32_t)i;
     }
 }
-__global__ void k_tr_item_permute(const uint32_t* idx, long long n, const Item* items, const int2* js, Item* items2, int2* js2) {
+__global__ void k_tr_item_permute(const uint32_t* idx, long long n, const Item* items, const int32_t* js, Item* items2, int32_t* js2) {
     for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (long long)gridDim.x * blockDim.x) {
         items2[i] = items[idx[i]];
         js2[i] = js[idx[i]];
@@ -552,11 +551,9 @@ static int build_transpose(fredopt_plan* P, RowSet& R) {
     if (ret) { cleanup2(); return ret; }
     if (cudaMemcpyAsync(&R.t_n_items, ustart + K, sizeof(long long), cudaMemcpyDeviceToHost, st) != cudaSuccess ||
         cudaStreamSynchronize(st) != cudaSuccess) { cleanup2(); return FREDOPT_CUDA_ERROR; }
-    if ((ret = dmalloc(P, &R.t_items, (size_t)R.t_n_items)) || (ret = dmalloc(P, &R.t_item_js, (size_t)R.t_n_items)) ||
-        (ret = dmalloc(P, &R.t_item_ptr, (size_t)S + 1)) || (ret = dmalloc(P, &R.t_partial, (size_t)R.t_n_items)) ||
-        (ret = dmalloc(P, &R.t_counter, (size_t)S))) { cleanup2(); return ret; }
-    cudaMemsetAsync(R.t_counter, 0, (S ? S : 1) * sizeof(unsigned int), st);
-    k_tr_item_fill<<<grid_for(K, 256, 4096), 256, 0, st>>>(R.t_ptr, ustart, sbase, S, R.n_seg, R.t_items, R.t_item_js);
+    if ((ret = dmalloc(P, &R.t_items, (size_t)R.t_n_items)) || (ret = dmalloc(P, &R.t_item_slot, (size_t)R.t_n_items)) ||
+        (ret = dmalloc(P, &R.t_item_ptr, (size_t)S + 1)) || (ret = dmalloc(P, &R.t_partial, (size_t)R.t_n_items))) { cleanup2(); return ret; }
+    k_tr_item_fill<<<grid_for(K, 256, 4096), 256, 0, st>>>(R.t_ptr, ustart, sbase, S, R.n_seg, R.t_items, R.t_item_slot);
     k_tr_item_ptr<<<grid_for(S + 1, 256, 4096), 256, 0, st>>>(sbase, S, R.n_seg, R.t_item_ptr);
     if (cudaGetLastError() != cudaSuccess || cudaStreamSynchronize(st) != cudaSuccess) { cleanup2(); return FREDOPT_CUDA_ERROR; }
     cudaFree(cnt_sm); cudaFree(sbase);
@@ -565,19 +562,19 @@ static int build_transpose(fredopt_plan* P, RowSet& R) {
     if (R.t_n_items > 1) {
         const long long ni = R.t_n_items;
         uint32_t *ik = nullptr, *ik2 = nullptr, *ii = nullptr, *ii2 = nullptr;
-        Item* it2 = nullptr; int2* js2 = nullptr; void* stmp = nullptr;
+        Item* it2 = nullptr; int32_t* js2 = nullptr; void* stmp = nullptr;
         auto cleanup3 = [&]() { cudaFree(ik); cudaFree(ik2); cudaFree(ii); cudaFree(ii2); cudaFree(it2); cudaFree(js2); cudaFree(stmp); cleanup(); };
 #define CK3(expr) do { cudaError_t e__ = (expr); if (e__ != cudaSuccess) { g_last_cuda_error = std::string(#expr) + ": " + cudaGetErrorString(e__); cudaGetLastError(); cleanup3(); return e__ == cudaErrorMemoryAllocation ? FREDOPT_OUT_OF_MEMORY : FREDOPT_CUDA_ERROR; } } while (0)
         CK3(cudaMalloc(&ik, ni * 4)); CK3(cudaMalloc(&ik2, ni * 4)); CK3(cudaMalloc(&ii, ni * 4)); CK3(cudaMalloc(&ii2, ni * 4));
-        CK3(cudaMalloc(&it2, ni * sizeof(Item))); CK3(cudaMalloc(&js2, ni * sizeof(int2)));
+        CK3(cudaMalloc(&it2, ni * sizeof(Item))); CK3(cudaMalloc(&js2, ni * sizeof(int32_t)));
         k_tr_item_key<<<grid_for(ni, 256, 4096), 256, 0, st>>>(R.t_items, ni, ik, ii);
         size_t sb = 0;
         CK3(cub::DeviceRadixSort::SortPairs(nullptr, sb, ik, ik2, ii, ii2, ni, 0, 4, st));
         CK3(cudaMalloc(&stmp, sb ? sb : 1));
         CK3(cub::DeviceRadixSort::SortPairs(stmp, sb, ik, ik2, ii, ii2, ni, 0, 4, st));
-        k_tr_item_permute<<<grid_for(ni, 256, 4096), 256, 0, st>>>(ii2, ni, R.t_items, R.t_item_js, it2, js2);
+        k_tr_item_permute<<<grid_for(ni, 256, 4096), 256, 0, st>>>(ii2, ni, R.t_items, R.t_item_slot, it2, js2);
         CK3(cudaMemcpyAsync(R.t_items, it2, ni * sizeof(Item), cudaMemcpyDeviceToDevice, st));
-        CK3(cudaMemcpyAsync(R.t_item_js, js2, ni * sizeof(int2), cudaMemcpyDeviceToDevice, st));
+        CK3(cudaMemcpyAsync(R.t_item_slot, js2, ni * sizeof(int32_t), cudaMemcpyDeviceToDevice, st));
         CK3(cudaStreamSynchronize(st));
 #undef CK3
         cudaFree(ik); cudaFree(ik2); cudaFree(ii); cudaFree(ii2); cudaFree(it2); cudaFree(js2); cudaFree(stmp);
@@ -669,10 +666,10 @@ template <int EPI>
 static void launch_transpose(fredopt_plan* P, const RowSet& R, const uint8_t* mode, const GatherVec& vec, double* g_out, double* x,
                              float* f_out) {
     if (R.t_n_items == 0) return;
-    k_transpose<EPI><<<fwd_grid(P, R.t_n_items), FWD_THREADS, 0, P->stream>>>(R.t_n_items, R.t_items, R.t_item_js, R.t_item_ptr, mode,
-                                                                             R.t_col, R.t_valD, R.t_valL, vec, R.t_partial, R.t_counter,
-                                                                             g_out, x, P->st, f_out);
-    ++P->launches;
+    k_transpose<<<fwd_grid(P, R.t_n_items), FWD_THREADS, 0, P->stream>>>(R.t_n_items, R.t_items, R.t_item_slot, mode, R.t_col, R.t_valD,
+                                                                           R.t_valL, vec, R.t_partial);
+    k_combine<EPI><<<grid_for(P->S, 256, 1 << 30), 256, 0, P->stream>>>(P->S, R.t_item_ptr, R.t_partial, g_out, x, P->st, f_out);
+    P->launches += 2;
 }
 
 static int res_grid(fredopt_plan* P) {

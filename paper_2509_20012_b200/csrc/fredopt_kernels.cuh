@@ -7,10 +7,9 @@
 //                (+ the cost residuals p, q of Eq. 2), the quadratic coefficient c of the accept test, or fp32
 //                dose / LETd per voxel.
 //   k_transpose  out_j = sum_i D_ij u_i + L_ij v_i over the stored CSR of the transposes (one item = at most
-//                TR_ITEM_MAX entries of one (spot, structure) run; one warp per item; no floating-point
-//                atomics: every item writes its partial sum and the LAST item of a spot to finish adds the
-//                spot's partials in item order, so the result does not depend on the schedule) with the
-//                gradient / update+clamp epilogues fused.
+//                TR_ITEM_MAX entries of one (structure, spot) run; one warp per item; every item writes its
+//                partial sum to a fixed slot: no atomics, no fences).
+//   k_combine    adds the slots of every spot in slot order and runs the gradient / update+clamp epilogue.
 //   k_select     |g|^2, c = sum w^ (Dg)^2 + w^ (Lg)^2 and the accept loop of Fig. 3 on device scalars.
 //   k_residual   d' = d - beta Dg, l' = l - beta Lg, x' = x - beta g, residuals / violations of Fig. 2 -> u, v,
 //                partial sums of proximity, cost and violation count.
@@ -87,12 +86,6 @@ __device__ __forceinline__ Item ld_item(const Item* p) {
     it.len = v.z;
     it.seg = v.w;
     return it;
-}
-// partial sums written by other CTAs of the same launch: bypass L1
-__device__ __forceinline__ double ld_cg_f64(const double* p) {
-    double r;
-    asm volatile("ld.global.cg.f64 %0, [%1];" : "=d"(r) : "l"(p));
-    return r;
 }
 
 __device__ __forceinline__ double warp_sum(double v) {
@@ -270,23 +263,14 @@ __device__ __forceinline__ double tr_item(const int32_t* __restrict__ cp, const 
     return aD + aL;
 }
 
-// One warp per item (round-robin; items are in (structure, spot) order so that the warps of a CTA work on
-// neighbouring spots of one structure).  Item r belongs to spot item_js[r].x and owns partial-sum slot item_js[r].y;
-// the slots of spot j are item_ptr[j] .. item_ptr[j+1]-1 (ascending structure, then ascending position).
-// Every item stores its partial sum; the warp that completes the LAST outstanding item
-// of a spot (per-spot arrival counter, integer atomics only) adds the spot's partials in item order and runs the
-// epilogue, then re-arms the counter.  The value is therefore independent of which warp finishes last.
-// Spots without items are never visited: their g / output stays 0 (set at creation / by the caller), their x is
-// already >= 0.
-template <int EPI>
+// One warp per item, round-robin.  Items are in longest-first order (ties in (structure, spot) order, so the warps
+// of a CTA mostly work on neighbouring spots of one structure and share L1 lines of the gather vector).  Item r
+// stores its partial sum in slot item_slot[r]; k_combine adds the slots of every spot in slot order.  No
+// floating-point atomics, no fences: the result does not depend on the schedule.
 __global__ void __launch_bounds__(FWD_THREADS, 3)
-k_transpose(long long n, const Item* __restrict__ items, const int2* __restrict__ item_js,
-            const long long* __restrict__ item_ptr, const uint8_t* __restrict__ mode, const int32_t* __restrict__ t_col,
-            const float* __restrict__ tD, const float* __restrict__ tL, const GatherVec vec,
-            double* __restrict__ partial, unsigned int* __restrict__ counter,
-            double* __restrict__ g_out,                                 // TEPI_GRAD
-            double* __restrict__ x, const DevState* __restrict__ st,   // TEPI_UPDATE
-            float* __restrict__ f_out)                                  // TEPI_F32
+k_transpose(long long n, const Item* __restrict__ items, const int32_t* __restrict__ item_slot,
+            const uint8_t* __restrict__ mode, const int32_t* __restrict__ t_col, const float* __restrict__ tD,
+            const float* __restrict__ tL, const GatherVec vec, double* __restrict__ partial)
 {
     const int lane = threadIdx.x & 31;
     const long long nwarps = (long long)gridDim.x * FWD_WARPS;
@@ -304,34 +288,31 @@ k_transpose(long long n, const Item* __restrict__ items, const int2* __restrict_
         else if (m == 1) tot = tr_item<1>(cp, tD + it.start, nullptr, it.len, lane, vec);
         else if (m == 2) tot = tr_item<2>(cp, nullptr, tL + it.start, it.len, lane, vec);
         if (m) tot = warp_sum(tot);
-        if (lane == 0) {
-            const int2 js = item_js[r];
-            const int j = js.x;
-            const long long ib = item_ptr[j], ie = item_ptr[j + 1];
-            bool last = true;
-            if (ie - ib > 1) {
-                partial[js.y] = tot;
-                __threadfence();
-                const unsigned int old = atomicAdd(counter + j, 1u);
-                last = old == (unsigned int)(ie - ib - 1);
-                if (last) {
-                    __threadfence();
-                    tot = 0.0;
-                    for (long long i = ib; i < ie; ++i) tot += ld_cg_f64(partial + i);
-                    counter[j] = 0u;
-                }
-            }
-            if (last) {
-                if (EPI == TEPI_GRAD) g_out[j] = tot;
-                else if (EPI == TEPI_UPDATE) {
-                    const double v = x[j] - st->relax * tot;          // x <- x' - lambda eta^k * sum w^ (r/|a|^2) a
-                    x[j] = v < 0.0 ? 0.0 : v;                          // clamp
-                } else f_out[j] = (float)tot;
-            }
-        }
+        if (lane == 0) partial[item_slot[r]] = tot;
         r = rn;
         it = nx;
     }
+}
+
+// Second stage of a transposed pass: one thread per spot adds the spot's partial sums in slot order (ascending
+// structure, then ascending position in the run) and runs the epilogue: gradient store (a3), update + clamp (a9), or
+// fp32 output.  Spots without entries are skipped: their g / output stays 0 (set at creation / by the caller) and
+// their x is already >= 0.
+template <int EPI>
+__global__ void __launch_bounds__(256)
+k_combine(long long S, const long long* __restrict__ item_ptr, const double* __restrict__ partial,
+          double* __restrict__ g_out, double* __restrict__ x, const DevState* __restrict__ st, float* __restrict__ f_out) {
+    const long long j = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (j >= S) return;
+    const long long ib = item_ptr[j], ie = item_ptr[j + 1];
+    if (ib == ie) return;
+    double tot = 0.0;
+    for (long long i = ib; i < ie; ++i) tot += partial[i];
+    if (EPI == TEPI_GRAD) g_out[j] = tot;
+    else if (EPI == TEPI_UPDATE) {
+        const double v = x[j] - st->relax * tot;          // x <- x' - lambda eta^k * sum w^ (r/|a|^2) a
+        x[j] = v < 0.0 ? 0.0 : v;                          // clamp
+    } else f_out[j] = (float)tot;
 }
 
 // ------------------------------------------------------------------------------------------ scalar kernels
