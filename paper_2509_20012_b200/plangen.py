@@ -469,9 +469,9 @@ def config_spec(i: int, seed: int = 0, scale: float = 1.0) -> PlanSpec:
         g = (int(300 * scale), int(300 * scale), int(200 * scale))
         return PlanSpec(
             name="config3_large", grid=g, h=2.0,
-            beams=[Beam(u=(0.0, 1.0, 0.25), d_iso=200.0, pitch=5.0, n_layers=22, sigma_lo=4.0, sigma_hi=7.0),
-                   Beam(u=(0.9, 0.3, -0.3), d_iso=200.0, pitch=5.0, n_layers=22, sigma_lo=4.0, sigma_hi=7.0),
-                   Beam(u=(-0.85, 0.35, 0.4), d_iso=200.0, pitch=5.0, n_layers=22, sigma_lo=4.0, sigma_hi=7.0)],
+            beams=[Beam(u=(0.0, 1.0, 0.25), d_iso=200.0, pitch=5.0, n_layers=22, sigma_lo=5.5, sigma_hi=9.5),
+                   Beam(u=(0.9, 0.3, -0.3), d_iso=200.0, pitch=5.0, n_layers=22, sigma_lo=5.5, sigma_hi=9.5),
+                   Beam(u=(-0.85, 0.35, 0.4), d_iso=200.0, pitch=5.0, n_layers=22, sigma_lo=5.5, sigma_hi=9.5)],
             structures=[[Shape("bumpy", (0, 0, 0), (60, 55, 43), bump=bump)],
                         [Shape("cylinder", (0, -72, 0), (12, 12, 40), axis=2)],
                         [Shape("ellipsoid", (78, 0, 0), (14, 20, 16))],
