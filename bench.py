@@ -39,8 +39,9 @@ DEFAULT_CONFIG = 3          # BASELINE.json configs[3]: the clinical-size plan t
 DEFAULT_STEPS = {0: 50, 1: 200, 2: 100, 3: 50}
 NOMINAL_HBM_GBS = 8000.0    # north_star's "~8 TB/s peak" (context; the roofline denominator is the measured copy figure)
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel from the committed `ncu --set full`
-# capture (profiles/r01_ncu_full_config3.md); keyed by (config, pass)
-NCU_TRAFFIC = {}
+# capture (profiles/r01_ncu_full_config3.md); keyed by (config, pass); a transposed pass = k_transpose + k_combine
+NCU_TRAFFIC = {(3, "forward_x"): 1246998776, (3, "transpose_g"): 1192556112, (3, "forward_g"): 1247750520,
+               (3, "transpose_b"): 1261692064}
 
 
 def _peaks():
