@@ -20,6 +20,7 @@ from __future__ import annotations
 
 import argparse
 import json
+import math
 import os
 import subprocess
 import sys
@@ -296,6 +297,75 @@ def cpu_baseline(plan, spec, args):
             "sample": f"{n} superiorized iterations of the same plan (after 1 warm-up iteration), fp64, single thread"}
 
 
+
+# ------------------------------------------------------------------------------------------------ configs[4]: pass sweep
+def run_sweep(args):
+    """BASELINE.json configs[4]: isolated SpMV passes on configs[2]-geometry matrices with every voxel labelled; spot sigma
+    3 -> 10 mm, non-zeros 1e7 -> 1.2e9 (through pitch and layer count); x log-uniform on [1e-3, 1].  One JSON line per
+    (sigma, nnz) point with GB/s (algorithmic bytes: 4 B index + 4 B per value array per non-zero) of every pass, timed
+    with CUDA events around the C-ABI call (its vector conversions included), median of `--steps` repetitions."""
+    import gc
+    from paper_2509_20012_b200 import fredopt, plangen as pg
+    torch.cuda.set_device(0)
+    stream = torch.cuda.current_stream()
+    peak, peak_src = _peaks()
+    l2 = torch.cuda.get_device_properties(0).L2_cache_size
+    flush = torch.empty(int(1.5 * l2), dtype=torch.uint8, device="cuda")
+    reps = args.steps or 10
+    sigmas = [3.0, 5.0, 7.0, 10.0]
+    targets = [1e7, 3e7, 1e8, 3e8, 1.2e9]
+    if args.quick:
+        sigmas, targets = [5.0], [1e7, 1e8]
+
+    def timed(fn, nbytes, resident):
+        ts = []
+        for i in range(reps + 3):
+            if resident:
+                flush.zero_()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(stream); fn(); e1.record(stream)
+            torch.cuda.synchronize()
+            if i >= 3:
+                ts.append(e0.elapsed_time(e1))
+        ms = float(np.median(ts))
+        return {"ms": ms, "gbs": nbytes / ms / 1e6, "frac_of_measured_peak": nbytes / ms / 1e6 / peak}
+
+    for sigma in sigmas:
+        # probe: non-zeros at a coarse lattice, then scale the spot count (pitch) and layer count to the target
+        probe = pg.build_plan(pg.sweep_spec(sigma, 12.0, 6), device="cuda")
+        nnz0 = probe.nnz
+        del probe
+        for target in targets:
+            ratio = target / nnz0                                  # nnz ~ layers / pitch^2
+            layers = int(min(40, max(6, round(6 * ratio ** 0.4))))
+            pitch = 12.0 / math.sqrt(max(ratio * 6 / layers, 1e-9))
+            pitch = min(max(pitch, 1.5), 40.0)
+            plan = pg.build_plan(pg.sweep_spec(sigma, pitch, layers), device="cuda")
+            gp = fredopt.from_plan(plan, stream=stream.cuda_stream)
+            V, S, nnz = plan.n_rows, plan.n_cols, plan.nnz
+            x = torch.from_numpy(pg.log_uniform_weights(5, S)).cuda()
+            r = torch.from_numpy(pg.log_uniform_weights(6, V)).cuda()
+            d = torch.empty(V, dtype=torch.float32, device="cuda"); l = torch.empty_like(d)
+            o = torch.empty(S, dtype=torch.float32, device="cuda")
+            resident = 12 * nnz < 2 * l2
+            gp.spmv_transpose(fredopt.ROWS_ALL, r, None, o)        # builds the transposed copy of the full matrix
+            res = {
+                "forward_D": timed(lambda: gp.spmv_forward(fredopt.ROWS_ALL, x, d, None), 8 * nnz, resident),
+                "forward_DL_fused": timed(lambda: gp.spmv_forward(fredopt.ROWS_ALL, x, d, l), 12 * nnz, resident),
+                "transpose_D": timed(lambda: gp.spmv_transpose(fredopt.ROWS_ALL, r, None, o), 8 * nnz, resident),
+                "transpose_L": timed(lambda: gp.spmv_transpose(fredopt.ROWS_ALL, None, r, o), 8 * nnz, resident),
+                "transpose_DL_fused": timed(lambda: gp.spmv_transpose(fredopt.ROWS_ALL, r, r, o), 12 * nnz, resident),
+            }
+            rows_ne = int((plan.row_ptr[1:] > plan.row_ptr[:-1]).sum().item())
+            print(json.dumps({"sweep": "configs[4]", "sigma_mm": sigma, "pitch_mm": round(pitch, 3), "layers": layers,
+                              "n_voxels": V, "n_spots": S, "nnz": nnz, "mean_row": nnz / max(rows_ne, 1),
+                              "mean_col": nnz / max(S, 1), "l2": "L2 flushed before every repetition" if resident
+                              else "larger than L2", "peak_gbs": peak, "passes": res}), flush=True)
+            gp.destroy()
+            del plan, gp, x, r, d, l, o
+            gc.collect(); torch.cuda.empty_cache()
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -304,9 +374,14 @@ def main():
     ap.add_argument("--config", type=int, default=DEFAULT_CONFIG)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--sweep", action="store_true", help="BASELINE.json configs[4]: isolated-pass sweep (1 GPU)")
+    ap.add_argument("--quick", action="store_true", help="with --sweep: two points only")
     args = ap.parse_args()
     if args.warmup < 3:
         args.warmup = 3
+    if args.sweep:
+        run_sweep(args)
+        return
     if args.impl == "reference":
         if args.steps is None:
             args.steps = 5

@@ -299,15 +299,10 @@ def test_invalid_arguments(fredopt):
         gp.set_option(99, 1.0)
 
 
-# ------------------------------------------------------------------------------------------ BASELINE configs[1]: the bench workload
-@pytest.fixture(scope="module")
-def plan1_dev():
-    return pg.build_plan(pg.config_spec(1), device="cuda")
-
-
-def test_config1_20_iterations_in_bench_configuration(fredopt, plan1_dev):
-    """Full size of the workload bench.py times (configs[1]), same launch configuration (graph replay)."""
-    plan = plan1_dev
+# ------------------------------------------------------------------------------------------ full-size configurations
+def _full_size_parity(fredopt, plan, n_sample_rows):
+    """20 superiorized iterations in the launch configuration bench.py times (one fredopt_iterate call = graph replay),
+    sampled outputs of the full forward pass computed one by one by the oracle, and the full transposed pass."""
     gp = fredopt.from_plan(plan, stream=torch.cuda.current_stream().cuda_stream)
     orc = _oracle(plan)
     sp = plan.spec
@@ -320,10 +315,13 @@ def test_config1_20_iterations_in_bench_configuration(fredopt, plan1_dev):
     gp.dose_let(torch.from_numpy(x).cuda(), dose, letd)
     torch.cuda.synchronize()
     nz = (plan.row_ptr[1:] > plan.row_ptr[:-1]).nonzero().reshape(-1).cpu().numpy()
-    rows = nz[(pg.uniform01_array(22, 4000) * len(nz)).astype(np.int64)]
+    rows = nz[(pg.uniform01_array(22, n_sample_rows) * len(nz)).astype(np.int64)]
     d_ref, _, t_ref = orc.dose_let_rows(rows, x.astype(np.float64))
     _assert_fwd(dose.cpu().numpy()[rows], d_ref, "dose (sampled)")
     _assert_fwd(letd.cpu().numpy()[rows], t_ref, "LETd (sampled)")
+    # rows no spot reaches are exactly 0
+    empty = (plan.row_ptr[1:] == plan.row_ptr[:-1])
+    assert float(dose[empty].abs().max().item() if bool(empty.any()) else 0.0) == 0.0
     # transposed pass over all rows, full size
     V = plan.n_rows
     u = (pg.uniform01_array(31, V) - 0.4).astype(np.float32); v = (pg.uniform01_array(32, V) - 0.6).astype(np.float32)
@@ -331,3 +329,22 @@ def test_config1_20_iterations_in_bench_configuration(fredopt, plan1_dev):
     out = np.empty(plan.n_cols, np.float32)
     gp.spmv_transpose(fredopt.ROWS_ALL, u, v, out)
     assert np.all(np.abs(out - ref) <= TOL_SPMV * ref_abs)
+    # and over the labelled rows only, with the D-only and L-only forms
+    for uu, vv in ((u, v), (u, None), (None, v)):
+        ref, ref_abs = orc.transpose(None if uu is None else uu.astype(np.float64),
+                                     None if vv is None else vv.astype(np.float64), active_only=True)
+        gp.spmv_transpose(fredopt.ROWS_ACTIVE, uu, vv, out)
+        assert np.all(np.abs(out - ref) <= TOL_SPMV * ref_abs)
+    gp.destroy()
+
+
+def test_config1_20_iterations_full_size(fredopt):
+    """BASELINE.json configs[1] (mid-size phantom, L2-resident working set)."""
+    _full_size_parity(fredopt, pg.build_plan(pg.config_spec(1), device="cuda"), 4000)
+
+
+def test_config3_20_iterations_in_bench_configuration(fredopt):
+    """BASELINE.json configs[3]: the workload bench.py times (1.15e9 non-zeros per matrix), at full size."""
+    plan = pg.build_plan(pg.config_spec(3), device="cuda")
+    assert plan.nnz > 1.0e9
+    _full_size_parity(fredopt, plan, 20000)
