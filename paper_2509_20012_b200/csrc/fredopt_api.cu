@@ -84,6 +84,7 @@ struct fredopt_plan {
     // full: all non-empty rows of the padded matrix (union pattern); act: a compact copy of the rows with a label,
     // ordered by (structure, voxel)
     RowSet full, act;
+    long long full_class[5] = {0, 0, 0, 0, 0};   // rows of length class c of `full`: full_class[c] .. full_class[c+1]-1
     // per active row
     double *nD = nullptr, *nL = nullptr, *nT = nullptr;
     // tables
@@ -254,6 +255,18 @@ __global__ void k_compact_rows(const int32_t* flag, const int32_t* pos, const lo
     }
 }
 
+// length class of a row of the full set: 0 = more than 64 entries (whole warp per row), 1 = 33..64 (16 lanes per row),
+// 2 = 17..32 (8 lanes), 3 = at most 16 (4 lanes)
+__host__ __device__ inline int len_class(long long padded) { return padded > 64 ? 0 : padded > 32 ? 1 : padded > 16 ? 2 : 3; }
+__global__ void k_class_keys(const int32_t* vox, const long long* ptr, long long n, int32_t* key, unsigned long long* hist) {
+    for (long long a = (long long)blockIdx.x * blockDim.x + threadIdx.x; a < n; a += (long long)gridDim.x * blockDim.x) {
+        const long long i = vox[a];
+        const int c = len_class((ptr[i + 1] - ptr[i] + 3) & ~3LL);
+        key[a] = c;
+        atomicAdd(hist + c, 1ULL);
+    }
+}
+
 // after sorting the active voxels by label: fill the list from the voxel ids
 __global__ void k_fill_active(const int32_t* vox, const int32_t* lab_sorted, const long long* ptr, const long long* pstart,
                               long long n, long long* start, int32_t* len, int32_t* ulen, int32_t* seg) {
@@ -263,7 +276,7 @@ __global__ void k_fill_active(const int32_t* vox, const int32_t* lab_sorted, con
         start[a] = pstart[i];
         len[a] = (int32_t)((m + 3) & ~3LL);
         ulen[a] = (int32_t)m;
-        seg[a] = lab_sorted[a] - 1;
+        if (seg) seg[a] = lab_sorted[a] - 1;
     }
 }
 
@@ -864,18 +877,45 @@ static int create_impl(fredopt_plan* P, const fredopt_csr* D, const fredopt_csr*
     CK(cudaMemcpyAsync(&n_ne, pos_ne + V, 4, cudaMemcpyDeviceToHost, st));
     CK(cudaMemcpyAsync(&n_act, pos_act + V, 4, cudaMemcpyDeviceToHost, st));
     CK(cudaStreamSynchronize(st));
-    // ---- full row set + padded arrays
+    // ---- full row set: non-empty rows ordered by (length class, voxel) and stored in that order, so that short rows
+    //      (entrance channels, few spots per voxel) are handled by sub-warps over contiguous memory
     RowSet& F = P->full;
     F.n = n_ne; F.n_seg = 1; F.nnz = nnzU;
-    CKR(dmalloc(P, &F.vox, (size_t)n_ne)); CKR(dmalloc(P, &F.start, (size_t)n_ne));
+    CKR(dmalloc(P, &F.vox, (size_t)n_ne)); CKR(dmalloc(P, &F.start, (size_t)n_ne + 1));
     CKR(dmalloc(P, &F.len, (size_t)n_ne)); CKR(dmalloc(P, &F.ulen, (size_t)n_ne)); CKR(dmalloc(P, &F.items, (size_t)n_ne));
-    if (V) k_compact_rows<<<grid_for(V, 256, 1 << 16), 256, 0, st>>>(f_ne, pos_ne, pU, pstart, lab, V, F.vox, F.start, F.len, F.ulen, nullptr);
     const size_t np = P->nnz_padded ? (size_t)P->nnz_padded : 4;
     CKR(dmalloc(P, &F.col, np)); CKR(dmalloc(P, &F.valD, np)); CKR(dmalloc(P, &F.valL, np));
     CK(cudaMemsetAsync(F.col, 0, np * 4, st)); CK(cudaMemsetAsync(F.valD, 0, np * 4, st)); CK(cudaMemsetAsync(F.valL, 0, np * 4, st));
-    if (n_ne) {
-        k_copy_padded<<<grid_for((long long)n_ne * 32, 256, 1 << 16), 256, 0, st>>>(F.n, F.vox, F.start, pU, cU, uD, uL, F.col, F.valD, F.valL);
-        k_pack_items<<<grid_for(n_ne, 256, 4096), 256, 0, st>>>(n_ne, F.start, F.len, nullptr, F.items);
+    {
+        int32_t *vox0, *key0, *key1;
+        long long *flen64, *fstart;
+        unsigned long long* hist;
+        CK(cudaMalloc(&vox0, ((size_t)n_ne + 1) * 4)); tmp.push_back(vox0);
+        CK(cudaMalloc(&key0, ((size_t)n_ne + 1) * 4)); tmp.push_back(key0);
+        CK(cudaMalloc(&key1, ((size_t)n_ne + 1) * 4)); tmp.push_back(key1);
+        CK(cudaMalloc(&flen64, ((size_t)n_ne + 1) * 8)); tmp.push_back(flen64);
+        CK(cudaMalloc(&fstart, ((size_t)n_ne + 1) * 8)); tmp.push_back(fstart);
+        CK(cudaMalloc(&hist, 4 * 8)); tmp.push_back(hist);
+        CK(cudaMemsetAsync(hist, 0, 4 * 8, st));
+        if (V) k_compact_rows<<<grid_for(V, 256, 1 << 16), 256, 0, st>>>(f_ne, pos_ne, pU, pstart, lab, V, vox0, nullptr, nullptr, nullptr, nullptr);
+        if (n_ne) k_class_keys<<<grid_for(n_ne, 256, 1 << 16), 256, 0, st>>>(vox0, pU, n_ne, key0, hist);
+        size_t tb = 0;
+        CK(cub::DeviceRadixSort::SortPairs(nullptr, tb, key0, key1, vox0, F.vox, n_ne, 0, 2, st));
+        void* t2; CK(cudaMalloc(&t2, tb ? tb : 1)); tmp.push_back(t2);
+        CK(cub::DeviceRadixSort::SortPairs(t2, tb, key0, key1, vox0, F.vox, n_ne, 0, 2, st));   // stable: voxel order inside a class
+        if (n_ne) k_fill_active<<<grid_for(n_ne, 256, 1 << 16), 256, 0, st>>>(F.vox, nullptr, pU, pstart, n_ne, fstart, F.len, F.ulen, nullptr);
+        CK(cudaMemsetAsync(flen64, 0, ((size_t)n_ne + 1) * 8, st));
+        if (n_ne) k_i32_to_i64<<<grid_for(n_ne, 256, 4096), 256, 0, st>>>(F.len, flen64, n_ne);
+        CKR(scan_exclusive(P, flen64, F.start, (long long)n_ne + 1));
+        unsigned long long hh[4];
+        CK(cudaMemcpyAsync(hh, hist, 4 * 8, cudaMemcpyDeviceToHost, st));
+        CK(cudaStreamSynchronize(st));
+        P->full_class[0] = 0;
+        for (int c = 0; c < 4; ++c) P->full_class[c + 1] = P->full_class[c] + (long long)hh[c];
+        if (n_ne) {
+            k_copy_padded<<<grid_for((long long)n_ne * 32, 256, 1 << 16), 256, 0, st>>>(F.n, F.vox, F.start, pU, cU, uD, uL, F.col, F.valD, F.valL);
+            k_pack_items<<<grid_for(n_ne, 256, 4096), 256, 0, st>>>(n_ne, F.start, F.len, nullptr, F.items);
+        }
     }
     // ---- active row set, ordered by (label, voxel), with its own compact copy of the rows: the iteration then
     //      streams contiguous arrays (no unconstrained rows in between)
@@ -1053,10 +1093,21 @@ static int forward_f32(fredopt_plan* P, const RowSet& R, int m, const double* xd
     if (dd) cudaMemsetAsync(dd, 0, (size_t)P->V * 4, P->stream);
     if (dl) cudaMemsetAsync(dl, 0, (size_t)P->V * 4, P->stream);
     if (R.n) {
-        k_forward<EPI_F32VOX><<<fwd_grid(P, R.n), FWD_THREADS, 0, P->stream>>>(R.n, R.items, R.vox, P->mode_fixed + (size_t)m * P->max_seg,
-                                                                               R.col, R.valD, R.valL, xd, nullptr, nullptr,
-                                                                               GatherVec{nullptr, nullptr, nullptr}, nullptr, nullptr, dd, dl, letd_out);
-        ++P->launches;
+        const uint8_t* md = P->mode_fixed + (size_t)m * P->max_seg;
+        long long n_long = R.n;
+        if (&R == &P->full) {   // short rows by sub-warps (4 / 8 / 16 lanes per row), long rows by whole warps
+            n_long = P->full_class[1];
+            const long long b1 = P->full_class[1], b2 = P->full_class[2], b3 = P->full_class[3], b4 = P->full_class[4];
+            if (b2 > b1) { k_forward_short<16><<<fwd_grid(P, (b2 - b1 + 1) / 2), FWD_THREADS, 0, P->stream>>>(b2 - b1, R.items + b1, R.vox + b1, m, R.col, R.valD, R.valL, xd, dd, dl, letd_out); ++P->launches; }
+            if (b3 > b2) { k_forward_short<8><<<fwd_grid(P, (b3 - b2 + 3) / 4), FWD_THREADS, 0, P->stream>>>(b3 - b2, R.items + b2, R.vox + b2, m, R.col, R.valD, R.valL, xd, dd, dl, letd_out); ++P->launches; }
+            if (b4 > b3) { k_forward_short<4><<<fwd_grid(P, (b4 - b3 + 7) / 8), FWD_THREADS, 0, P->stream>>>(b4 - b3, R.items + b3, R.vox + b3, m, R.col, R.valD, R.valL, xd, dd, dl, letd_out); ++P->launches; }
+        }
+        if (n_long) {
+            k_forward<EPI_F32VOX><<<fwd_grid(P, n_long), FWD_THREADS, 0, P->stream>>>(n_long, R.items, R.vox, md, R.col, R.valD, R.valL, xd,
+                                                                                  nullptr, nullptr, GatherVec{nullptr, nullptr, nullptr},
+                                                                                  nullptr, nullptr, dd, dl, letd_out);
+            ++P->launches;
+        }
     }
     int rc = FREDOPT_OK;
     cudaError_t e = cudaGetLastError();

@@ -140,14 +140,25 @@ __device__ __forceinline__ void fwd_row(const int32_t* __restrict__ cp, const fl
             if (M & 2) fma4(aL, l[u], x0, x1, x2, x3);
         }
     }
-    for (; p < L; p += 128) {
-        const int4 c0 = ld_stream_i4(cp + p);
-        float4 d0, l0;
-        if (M & 1) d0 = ld_stream_f4(dp + p);
-        if (M & 2) l0 = ld_stream_f4(lp + p);
-        const double x0 = __ldg(x + c0.x), x1 = __ldg(x + c0.y), x2 = __ldg(x + c0.z), x3 = __ldg(x + c0.w);
-        if (M & 1) fma4(aD, d0, x0, x1, x2, x3);
-        if (M & 2) fma4(aL, l0, x0, x1, x2, x3);
+    if (p < L) {   // remainder (fewer than U chunks): ONE predicated trip, all loads in flight together; a lane without
+                   // an entry behaves like padding (column 0, value 0)
+        int4 c[U - 1];
+        float4 d[U - 1], l[U - 1];
+#pragma unroll
+        for (int u = 0; u < U - 1; ++u) {
+            const bool ok = p + 128 * u < L;
+            c[u] = ok ? ld_stream_i4(cp + p + 128 * u) : make_int4(0, 0, 0, 0);
+            if (M & 1) d[u] = ok ? ld_stream_f4(dp + p + 128 * u) : make_float4(0.f, 0.f, 0.f, 0.f);
+            if (M & 2) l[u] = ok ? ld_stream_f4(lp + p + 128 * u) : make_float4(0.f, 0.f, 0.f, 0.f);
+        }
+#pragma unroll
+        for (int u = 0; u < U - 1; ++u) {
+            if (p + 128 * u < L) {
+                const double x0 = __ldg(x + c[u].x), x1 = __ldg(x + c[u].y), x2 = __ldg(x + c[u].z), x3 = __ldg(x + c[u].w);
+                if (M & 1) fma4(aD, d[u], x0, x1, x2, x3);
+                if (M & 2) fma4(aL, l[u], x0, x1, x2, x3);
+            }
+        }
     }
 }
 
@@ -213,6 +224,44 @@ k_forward(long long n, const Item* __restrict__ items, const int32_t* __restrict
     }
 }
 
+// Short rows (at most 4*G entries, G = 4, 8 or 16): G lanes per row, 32/G rows per warp at a time, one 128-bit load per
+// lane and array, shuffle reduction inside the lane group.  Rows of one length class are stored back to back, so the
+// warp's loads are contiguous.  fp32 voxel-indexed outputs only (fredopt_dose_let / fredopt_spmv_forward over all rows).
+template <int G>
+__global__ void __launch_bounds__(FWD_THREADS)
+k_forward_short(long long n, const Item* __restrict__ items, const int32_t* __restrict__ vox, int m,
+                const int32_t* __restrict__ col, const float* __restrict__ vD, const float* __restrict__ vL,
+                const double* __restrict__ x, float* __restrict__ fD, float* __restrict__ fL, int letd_out)
+{
+    constexpr int RPW = 32 / G;                       // rows per warp and trip
+    const int lane = threadIdx.x & 31, t = lane % G, grp = lane / G;
+    const long long nwarps = (long long)gridDim.x * FWD_WARPS;
+    for (long long base = ((long long)blockIdx.x * FWD_WARPS + (threadIdx.x >> 5)) * RPW; base < n; base += nwarps * RPW) {
+        const long long r = base + grp;
+        double aD = 0.0, aL = 0.0;
+        if (r < n) {
+            const Item it = ld_item(items + r);
+            if (4 * t < it.len) {
+                const long long p = it.start + 4 * t;
+                const int4 c = ld_stream_i4(col + p);
+                const double x0 = __ldg(x + c.x), x1 = __ldg(x + c.y), x2 = __ldg(x + c.z), x3 = __ldg(x + c.w);
+                if (m & 1) fma4(aD, ld_stream_f4(vD + p), x0, x1, x2, x3);
+                if (m & 2) fma4(aL, ld_stream_f4(vL + p), x0, x1, x2, x3);
+            }
+        }
+#pragma unroll
+        for (int o = G / 2; o > 0; o >>= 1) {
+            aD += __shfl_down_sync(0xffffffffu, aD, o, G);
+            aL += __shfl_down_sync(0xffffffffu, aL, o, G);
+        }
+        if (t == 0 && r < n) {
+            const int v = vox[r];
+            if (fD) fD[v] = (float)aD;
+            if (fL) fL[v] = letd_out ? (aD > 0.0 ? (float)(aL / aD) : 0.0f) : (float)aL;
+        }
+    }
+}
+
 // ------------------------------------------------------------------------------------------ transposed
 enum : int { TEPI_F32 = 0, TEPI_GRAD = 1, TEPI_UPDATE = 2 };
 
@@ -247,17 +296,28 @@ __device__ __forceinline__ double tr_item(const int32_t* __restrict__ cp, const 
             }
         }
     }
-    for (; p < L; p += 128) {
-        const int4 c0 = ld_stream_i4(cp + p);
-        if (M == 3) {
-            const float4 d0 = ld_stream_f4(dp + p), l0 = ld_stream_f4(lp + p);
-            const double2 g0 = __ldg(vec + c0.x), g1 = __ldg(vec + c0.y), g2 = __ldg(vec + c0.z), g3 = __ldg(vec + c0.w);
-            fma4(aD, d0, g0.x, g1.x, g2.x, g3.x);
-            fma4(aL, l0, g0.y, g1.y, g2.y, g3.y);
-        } else {
-            const float4 a0 = ld_stream_f4((M == 1 ? dp : lp) + p);
-            const double g0 = __ldg(vs + c0.x), g1 = __ldg(vs + c0.y), g2 = __ldg(vs + c0.z), g3 = __ldg(vs + c0.w);
-            fma4(aD, a0, g0, g1, g2, g3);
+    if (p < L) {   // remainder: one predicated trip (see fwd_row)
+        int4 c[U - 1];
+        float4 d[U - 1], l[U - 1];
+#pragma unroll
+        for (int u = 0; u < U - 1; ++u) {
+            const bool ok = p + 128 * u < L;
+            c[u] = ok ? ld_stream_i4(cp + p + 128 * u) : make_int4(0, 0, 0, 0);
+            if (M & 1) d[u] = ok ? ld_stream_f4(dp + p + 128 * u) : make_float4(0.f, 0.f, 0.f, 0.f);
+            if (M & 2) l[u] = ok ? ld_stream_f4(lp + p + 128 * u) : make_float4(0.f, 0.f, 0.f, 0.f);
+        }
+#pragma unroll
+        for (int u = 0; u < U - 1; ++u) {
+            if (p + 128 * u < L) {
+                if (M == 3) {
+                    const double2 g0 = __ldg(vec + c[u].x), g1 = __ldg(vec + c[u].y), g2 = __ldg(vec + c[u].z), g3 = __ldg(vec + c[u].w);
+                    fma4(aD, d[u], g0.x, g1.x, g2.x, g3.x);
+                    fma4(aL, l[u], g0.y, g1.y, g2.y, g3.y);
+                } else {
+                    const double g0 = __ldg(vs + c[u].x), g1 = __ldg(vs + c[u].y), g2 = __ldg(vs + c[u].z), g3 = __ldg(vs + c[u].w);
+                    if (M == 1) fma4(aD, d[u], g0, g1, g2, g3); else fma4(aL, l[u], g0, g1, g2, g3);
+                }
+            }
         }
     }
     return aD + aL;
