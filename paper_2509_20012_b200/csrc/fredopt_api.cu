@@ -46,7 +46,8 @@ struct RowSet {
     long long n = 0;                 // rows
     int n_seg = 1;
     // padded index / value arrays of the set (rows stored back to back in list order)
-    int32_t* col = nullptr;
+    int32_t* col = nullptr;          // int32 column indices (kept for transposition; the hot kernels read col16 if set)
+    uint16_t* col16 = nullptr;       // the same indices as 16 bits when n_cols <= 65536 (2 B instead of 4 B per non-zero)
     float* valD = nullptr;
     float* valL = nullptr;
     int32_t* vox = nullptr;          // [n]
@@ -59,7 +60,9 @@ struct RowSet {
     // CSR of the transposes restricted to this set, SEGMENT-major: run k = seg*S + spot; columns = list index
     bool t_built = false;
     long long* t_ptr = nullptr;      // [n_seg*S + 1]
-    int32_t* t_col = nullptr;
+    int32_t* t_col = nullptr;        // compact row index (32-bit form: only if the 16-bit form does not apply)
+    uint16_t* t_col16 = nullptr;     // low 16 bits of the compact row index; runs are cut where the high bits change
+    int t_H = 1;                     // number of 65536-row blocks of the list (1 in the 32-bit form)
     float* t_valD = nullptr;
     float* t_valL = nullptr;
     long long t_nnz_padded = 0;
@@ -373,7 +376,8 @@ __global__ void k_finish_tables(StructInfo* tab, int n_struct, DevState* st, uin
 }
 
 // ---- transposition of a row set
-__global__ void k_tr_keys(RowList rl, const int32_t* ulen, const long long* off, const int32_t* col, long long S,
+// key of an entry = ((segment * S + spot) * H + block) with block = row index >> 16 (H = 1: no blocks)
+__global__ void k_tr_keys(RowList rl, const int32_t* ulen, const long long* off, const int32_t* col, long long S, int H,
                           uint32_t* keys, uint32_t* vals) {
     const int lane = threadIdx.x & 31;
     const long long w0 = ((long long)blockIdx.x * blockDim.x + threadIdx.x) >> 5, nw = ((long long)gridDim.x * blockDim.x) >> 5;
@@ -383,7 +387,7 @@ __global__ void k_tr_keys(RowList rl, const int32_t* ulen, const long long* off,
         const int sg = rl.seg ? rl.seg[r] : 0;
         const int Lp = rl.len[r];
         for (int p = lane; p < L; p += 32) {
-            keys[o + p] = (uint32_t)sg * (uint32_t)S + (uint32_t)col[s + perm_pos(p, Lp)];
+            keys[o + p] = ((uint32_t)sg * (uint32_t)S + (uint32_t)col[s + perm_pos(p, Lp)]) * (uint32_t)H + (H > 1 ? (uint32_t)(r >> 16) : 0u);
             vals[o + p] = (uint32_t)(o + p);
         }
     }
@@ -402,7 +406,7 @@ __global__ void k_tr_pcount(const long long* ustart, long long K, long long* pco
 }
 __global__ void k_tr_fill(const uint32_t* keys, const uint32_t* vals, long long E, const long long* ustart, const long long* t_ptr,
                           const long long* off, long long n_rows, const long long* start, const int32_t* len, const float* vD,
-                          const float* vL, int32_t* t_col, float* tD, float* tL) {
+                          const float* vL, int32_t* t_col, uint16_t* t_col16, float* tD, float* tL) {
     for (long long r = (long long)blockIdx.x * blockDim.x + threadIdx.x; r < E; r += (long long)gridDim.x * blockDim.x) {
         const long long k = keys[r], e = vals[r];
         // row a with off[a] <= e < off[a+1]
@@ -410,7 +414,7 @@ __global__ void k_tr_fill(const uint32_t* keys, const uint32_t* vals, long long 
         while (lo < hi) { const long long mid = (lo + hi) >> 1; if (off[mid + 1] <= e) lo = mid + 1; else hi = mid; }
         const long long a = lo, p = start[a] + perm_pos(e - off[a], len[a]);
         const long long dst = t_ptr[k] + perm_pos(r - ustart[k], t_ptr[k + 1] - t_ptr[k]);
-        t_col[dst] = (int32_t)a;
+        if (t_col16) t_col16[dst] = (uint16_t)(a & 0xFFFF); else t_col[dst] = (int32_t)a;
         tD[dst] = vD[p];
         tL[dst] = vL[p];
     }
@@ -429,16 +433,20 @@ __global__ void k_tr_item_count(const long long* t_ptr, long long K, long long* 
         cnt[k] = (t_ptr[k + 1] - t_ptr[k] + TR_ITEM_MAX - 1) / TR_ITEM_MAX;
 }
 // the same counts in spot-major order (the order of a spot's partial-sum slots)
-__global__ void k_tr_item_count_sm(const long long* cnt, long long S, int n_seg, long long* cnt_sm) {
-    for (long long k = (long long)blockIdx.x * blockDim.x + threadIdx.x; k < S * n_seg; k += (long long)gridDim.x * blockDim.x)
-        cnt_sm[(k % S) * n_seg + k / S] = cnt[k];
+__global__ void k_tr_item_count_sm(const long long* cnt, long long S, int n_seg, int H, long long* cnt_sm) {
+    for (long long k = (long long)blockIdx.x * blockDim.x + threadIdx.x; k < S * n_seg * H; k += (long long)gridDim.x * blockDim.x) {
+        const long long hi = k % H, js = k / H, j = js % S, sg = js / S;
+        cnt_sm[(j * n_seg + sg) * H + hi] = cnt[k];
+    }
 }
-__global__ void k_tr_item_fill(const long long* t_ptr, const long long* ibase, const long long* sbase, long long S, int n_seg,
+// item.seg = segment | (block << 8): the kernel adds block << 16 to the 16-bit row indices
+__global__ void k_tr_item_fill(const long long* t_ptr, const long long* ibase, const long long* sbase, long long S, int n_seg, int H,
                                Item* items, int32_t* item_slot) {
-    for (long long k = (long long)blockIdx.x * blockDim.x + threadIdx.x; k < S * n_seg; k += (long long)gridDim.x * blockDim.x) {
+    for (long long k = (long long)blockIdx.x * blockDim.x + threadIdx.x; k < S * n_seg * H; k += (long long)gridDim.x * blockDim.x) {
         const long long b = t_ptr[k], e = t_ptr[k + 1];
-        const long long j = k % S, sg = k / S;
-        long long i = ibase[k], slot = sbase[j * n_seg + sg];
+        const long long hi = k % H, js = k / H, j = js % S, sg0 = js / S;
+        const long long sg = sg0 | (hi << 8);
+        long long i = ibase[k], slot = sbase[(j * n_seg + sg0) * H + hi];
         for (long long p = b; p < e; p += TR_ITEM_MAX, ++i, ++slot) {
             Item it;
             it.start = p; it.len = (int32_t)((e - p) < TR_ITEM_MAX ? (e - p) : TR_ITEM_MAX); it.seg = (int32_t)sg;
@@ -461,9 +469,13 @@ __global__ void k_tr_item_permute(const uint32_t* idx, long long n, const Item* 
         js2[i] = js[idx[i]];
     }
 }
-__global__ void k_tr_item_ptr(const long long* sbase, long long S, int n_seg, long long* item_ptr) {
+__global__ void k_tr_item_ptr(const long long* sbase, long long S, long long runs_per_spot, long long* item_ptr) {
     for (long long j = (long long)blockIdx.x * blockDim.x + threadIdx.x; j <= S; j += (long long)gridDim.x * blockDim.x)
-        item_ptr[j] = sbase[j * n_seg];
+        item_ptr[j] = sbase[j * runs_per_spot];
+}
+__global__ void k_narrow_u16(const int32_t* in, uint16_t* out, long long n) {
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (long long)gridDim.x * blockDim.x)
+        out[i] = (uint16_t)in[i];
 }
 __global__ void k_i32_to_i64(const int32_t* in, long long* out, long long n) {
     for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (long long)gridDim.x * blockDim.x) out[i] = in[i];
@@ -488,7 +500,14 @@ static int scan_exclusive(fredopt_plan* P, const T* in, T* out, long long n) {
 
 static int build_transpose(fredopt_plan* P, RowSet& R) {
     cudaStream_t st = P->stream;
-    const long long n = R.n, S = P->S, K = S * R.n_seg;
+    const long long n = R.n, S = P->S;
+    // 16-bit row indices: cut every (segment, spot) run where the row index crosses a multiple of 65536
+    int H = (int)((n + 65535) >> 16);
+    if (H < 1) H = 1;
+    bool idx16 = R.n_seg < 256 && H < (1 << 23) && (double)S * R.n_seg * H < 4.0e9 && !getenv("FREDOPT_IDX32");
+    if (!idx16) H = 1;
+    R.t_H = H;
+    const long long K = S * R.n_seg * H;
     // unpadded offsets
     long long *len64 = nullptr, *off = nullptr;
     CK(cudaMalloc(&len64, (n + 1) * sizeof(long long)));
@@ -524,7 +543,7 @@ static int build_transpose(fredopt_plan* P, RowSet& R) {
     CKC(cudaMalloc(&keys, En * 4)); CKC(cudaMalloc(&vals, En * 4));
     CKC(cudaMalloc(&keys2, En * 4)); CKC(cudaMalloc(&vals2, En * 4));
     CKC(cudaMalloc(&ustart, (K + 2) * sizeof(long long))); CKC(cudaMalloc(&pcount, (K + 2) * sizeof(long long)));
-    if (n) k_tr_keys<<<grid_for(n * 32, 256, 1 << 16), 256, 0, st>>>(R.view(), R.ulen, off, R.col, S, keys, vals);
+    if (n) k_tr_keys<<<grid_for(n * 32, 256, 1 << 16), 256, 0, st>>>(R.view(), R.ulen, off, R.col, S, H, keys, vals);
     int bits = 1;
     while ((1LL << bits) < K) ++bits;
     size_t tb = 0;
@@ -542,12 +561,14 @@ static int build_transpose(fredopt_plan* P, RowSet& R) {
     CKC(cudaMemcpyAsync(&R.t_nnz_padded, R.t_ptr + K, sizeof(long long), cudaMemcpyDeviceToHost, st));
     CKC(cudaStreamSynchronize(st));
     const size_t Tn = R.t_nnz_padded ? (size_t)R.t_nnz_padded : 4;
-    if ((ret = dmalloc(P, &R.t_col, Tn)) || (ret = dmalloc(P, &R.t_valD, Tn)) || (ret = dmalloc(P, &R.t_valL, Tn))) { cleanup(); return ret; }
+    if ((ret = idx16 ? dmalloc(P, &R.t_col16, Tn) : dmalloc(P, &R.t_col, Tn)) || (ret = dmalloc(P, &R.t_valD, Tn)) ||
+        (ret = dmalloc(P, &R.t_valL, Tn))) { cleanup(); return ret; }
+    if (idx16) CKC(cudaMemsetAsync(R.t_col16, 0, Tn * 2, st)); else
     CKC(cudaMemsetAsync(R.t_col, 0, Tn * 4, st));
     CKC(cudaMemsetAsync(R.t_valD, 0, Tn * 4, st));
     CKC(cudaMemsetAsync(R.t_valL, 0, Tn * 4, st));
     if (E) k_tr_fill<<<grid_for(E, 256, 1 << 16), 256, 0, st>>>(keys2, vals2, E, ustart, R.t_ptr, off, n, R.start, R.len, R.valD, R.valL,
-                                                             R.t_col, R.t_valD, R.t_valL);
+                                                             R.t_col, R.t_col16, R.t_valD, R.t_valL);
     CKC(cudaGetLastError());
     // ---- work items: every (segment, spot) run cut into pieces of at most TR_ITEM_MAX entries, in run order
     //      (neighbouring items = neighbouring spots of one structure: overlapping voxel footprints share L1 lines)
@@ -558,7 +579,7 @@ static int build_transpose(fredopt_plan* P, RowSet& R) {
     { cudaError_t e_ = cudaMalloc(&sbase, (K + 2) * sizeof(long long)); if (e_ != cudaSuccess) { cudaFree(cnt_sm); CKC(e_); } }
     auto cleanup2 = [&]() { cudaFree(cnt_sm); cudaFree(sbase); cleanup(); };
     cudaMemsetAsync(cnt_sm, 0, (K + 2) * sizeof(long long), st);
-    k_tr_item_count_sm<<<grid_for(K, 256, 4096), 256, 0, st>>>(pcount, S, R.n_seg, cnt_sm);
+    k_tr_item_count_sm<<<grid_for(K, 256, 4096), 256, 0, st>>>(pcount, S, R.n_seg, H, cnt_sm);
     ret = scan_exclusive(P, pcount, ustart, K + 1);      // ustart now = first item of each run (execution order)
     if (!ret) ret = scan_exclusive(P, cnt_sm, sbase, K + 1);   // first partial-sum slot of each (spot, segment)
     if (ret) { cleanup2(); return ret; }
@@ -566,8 +587,8 @@ static int build_transpose(fredopt_plan* P, RowSet& R) {
         cudaStreamSynchronize(st) != cudaSuccess) { cleanup2(); return FREDOPT_CUDA_ERROR; }
     if ((ret = dmalloc(P, &R.t_items, (size_t)R.t_n_items)) || (ret = dmalloc(P, &R.t_item_slot, (size_t)R.t_n_items)) ||
         (ret = dmalloc(P, &R.t_item_ptr, (size_t)S + 1)) || (ret = dmalloc(P, &R.t_partial, (size_t)R.t_n_items))) { cleanup2(); return ret; }
-    k_tr_item_fill<<<grid_for(K, 256, 4096), 256, 0, st>>>(R.t_ptr, ustart, sbase, S, R.n_seg, R.t_items, R.t_item_slot);
-    k_tr_item_ptr<<<grid_for(S + 1, 256, 4096), 256, 0, st>>>(sbase, S, R.n_seg, R.t_item_ptr);
+    k_tr_item_fill<<<grid_for(K, 256, 4096), 256, 0, st>>>(R.t_ptr, ustart, sbase, S, R.n_seg, H, R.t_items, R.t_item_slot);
+    k_tr_item_ptr<<<grid_for(S + 1, 256, 4096), 256, 0, st>>>(sbase, S, (long long)R.n_seg * H, R.t_item_ptr);
     if (cudaGetLastError() != cudaSuccess || cudaStreamSynchronize(st) != cudaSuccess) { cleanup2(); return FREDOPT_CUDA_ERROR; }
     cudaFree(cnt_sm); cudaFree(sbase);
     // ---- longest items first: with the static round-robin mapping every round of the grid then holds items of
@@ -618,11 +639,12 @@ static void compute_pass_bytes(fredopt_plan* P) {
         const int f = T.flags;
         const int cost = ((f & F_DOSE_REF) ? 1 : 0) | ((f & F_DL_REF) ? 2 : 0);
         const int con = ((f & (F_DOSE_SLAB | F_LETD)) ? 1 : 0) | ((f & (F_DL_SLAB | F_LETD)) ? 2 : 0);
-        auto per = [](int m) { return m ? 4 + 4 * ((m & 1) + ((m >> 1) & 1)) : 0; };
-        fwd_union += (long long)T.nnz * per(cost | con);
-        fwd_con += (long long)T.nnz * per(con);
-        tr_cost += (long long)T.nnz * per(cost);
-        tr_con += (long long)T.nnz * per(con);
+        auto per = [](int m, int ib) { return m ? ib + 4 * ((m & 1) + ((m >> 1) & 1)) : 0; };
+        const int ibf = P->act.col16 ? 2 : 4, ibt = P->act.t_col16 ? 2 : 4;     // index bytes as stored
+        fwd_union += (long long)T.nnz * per(cost | con, ibf);
+        fwd_con += (long long)T.nnz * per(con, ibf);
+        tr_cost += (long long)T.nnz * per(cost, ibt);
+        tr_con += (long long)T.nnz * per(con, ibt);
         if (cost | con) rows_union += T.rows;
         if (con) rows_con += T.rows;
         if (cost) rows_cost += T.rows;
@@ -662,15 +684,20 @@ static int fwd_grid(fredopt_plan* P, long long n) {
 static void launch_forward(fredopt_plan* P, const RowSet& R, const uint8_t* mode, const double* x, double* oD, double* oL, int epi) {
     if (R.n == 0) { if (epi == EPI_CPART) cudaMemsetAsync(P->cpart, 0, sizeof(double) * MAX_PARTIALS, P->stream); return; }
     const int g = fwd_grid(P, R.n);
-    if (epi == EPI_CPART)
-        k_forward<EPI_CPART><<<g, FWD_THREADS, 0, P->stream>>>(R.n, R.items, R.vox, mode, R.col, R.valD, R.valL, x, oD, oL, GatherVec{nullptr, nullptr, nullptr},
-                                                               P->tab, P->cpart, nullptr, nullptr, 0);
-    else if (epi == EPI_STORE_PQ)
-        k_forward<EPI_STORE_PQ><<<g, FWD_THREADS, 0, P->stream>>>(R.n, R.items, R.vox, mode, R.col, R.valD, R.valL, x, oD, oL, P->pq,
-                                                                  P->tab, nullptr, nullptr, nullptr, 0);
-    else
-        k_forward<EPI_STORE><<<g, FWD_THREADS, 0, P->stream>>>(R.n, R.items, R.vox, mode, R.col, R.valD, R.valL, x, oD, oL, GatherVec{nullptr, nullptr, nullptr},
-                                                               nullptr, nullptr, nullptr, nullptr, 0);
+    const GatherVec none{nullptr, nullptr, nullptr};
+#define FWD_LAUNCH(E, I16, COL, PQ, TAB, CP)                                                                                   \
+    k_forward<E, I16><<<g, FWD_THREADS, 0, P->stream>>>(R.n, R.items, R.vox, mode, COL, R.valD, R.valL, x, oD, oL, PQ, TAB, CP, \
+                                                       nullptr, nullptr, 0)
+    if (R.col16) {
+        if (epi == EPI_CPART) FWD_LAUNCH(EPI_CPART, true, R.col16, none, P->tab, P->cpart);
+        else if (epi == EPI_STORE_PQ) FWD_LAUNCH(EPI_STORE_PQ, true, R.col16, P->pq, P->tab, nullptr);
+        else FWD_LAUNCH(EPI_STORE, true, R.col16, none, nullptr, nullptr);
+    } else {
+        if (epi == EPI_CPART) FWD_LAUNCH(EPI_CPART, false, R.col, none, P->tab, P->cpart);
+        else if (epi == EPI_STORE_PQ) FWD_LAUNCH(EPI_STORE_PQ, false, R.col, P->pq, P->tab, nullptr);
+        else FWD_LAUNCH(EPI_STORE, false, R.col, none, nullptr, nullptr);
+    }
+#undef FWD_LAUNCH
     ++P->launches;
 }
 static int cpart_count(fredopt_plan* P) { return P->act.n ? fwd_grid(P, P->act.n) : MAX_PARTIALS; }
@@ -679,8 +706,12 @@ template <int EPI>
 static void launch_transpose(fredopt_plan* P, const RowSet& R, const uint8_t* mode, const GatherVec& vec, double* g_out, double* x,
                              float* f_out) {
     if (R.t_n_items == 0) return;
-    k_transpose<<<fwd_grid(P, R.t_n_items), FWD_THREADS, 0, P->stream>>>(R.t_n_items, R.t_items, R.t_item_slot, mode, R.t_col, R.t_valD,
-                                                                           R.t_valL, vec, R.t_partial);
+    if (R.t_col16)
+        k_transpose<true><<<fwd_grid(P, R.t_n_items), FWD_THREADS, 0, P->stream>>>(R.t_n_items, R.t_items, R.t_item_slot, mode, R.t_col16,
+                                                                                     R.t_valD, R.t_valL, vec, R.t_partial);
+    else
+        k_transpose<false><<<fwd_grid(P, R.t_n_items), FWD_THREADS, 0, P->stream>>>(R.t_n_items, R.t_items, R.t_item_slot, mode, R.t_col,
+                                                                                      R.t_valD, R.t_valL, vec, R.t_partial);
     k_combine<EPI><<<grid_for(P->S, 256, 1 << 30), 256, 0, P->stream>>>(P->S, R.t_item_ptr, R.t_partial, g_out, x, P->st, f_out);
     P->launches += 2;
 }
@@ -916,6 +947,10 @@ static int create_impl(fredopt_plan* P, const fredopt_csr* D, const fredopt_csr*
             k_copy_padded<<<grid_for((long long)n_ne * 32, 256, 1 << 16), 256, 0, st>>>(F.n, F.vox, F.start, pU, cU, uD, uL, F.col, F.valD, F.valL);
             k_pack_items<<<grid_for(n_ne, 256, 4096), 256, 0, st>>>(n_ne, F.start, F.len, nullptr, F.items);
         }
+        if (S <= 65536 && !getenv("FREDOPT_IDX32")) {   // 16-bit column indices for the hot kernels
+            CKR(dmalloc(P, &F.col16, np));
+            k_narrow_u16<<<grid_for((long long)np, 256, 1 << 16), 256, 0, st>>>(F.col, F.col16, (long long)np);
+        }
     }
     // ---- active row set, ordered by (label, voxel), with its own compact copy of the rows: the iteration then
     //      streams contiguous arrays (no unconstrained rows in between)
@@ -952,6 +987,10 @@ static int create_impl(fredopt_plan* P, const fredopt_csr* D, const fredopt_csr*
         if (n_act) {
             k_copy_padded<<<grid_for((long long)n_act * 32, 256, 1 << 16), 256, 0, st>>>(A.n, A.vox, A.start, pU, cU, uD, uL, A.col, A.valD, A.valL);
             k_pack_items<<<grid_for(n_act, 256, 4096), 256, 0, st>>>(n_act, A.start, A.len, A.seg, A.items);
+        }
+        if (S <= 65536 && !getenv("FREDOPT_IDX32")) {
+            CKR(dmalloc(P, &A.col16, na));
+            k_narrow_u16<<<grid_for((long long)na, 256, 1 << 16), 256, 0, st>>>(A.col, A.col16, (long long)na);
         }
     }
     // ---- tables, norms, w^
@@ -1094,18 +1133,28 @@ static int forward_f32(fredopt_plan* P, const RowSet& R, int m, const double* xd
     if (dl) cudaMemsetAsync(dl, 0, (size_t)P->V * 4, P->stream);
     if (R.n) {
         const uint8_t* md = P->mode_fixed + (size_t)m * P->max_seg;
+        const GatherVec none{nullptr, nullptr, nullptr};
+        const bool i16 = R.col16 != nullptr;
+        const void* colp = i16 ? (const void*)R.col16 : (const void*)R.col;
         long long n_long = R.n;
         if (&R == &P->full) {   // short rows by sub-warps (4 / 8 / 16 lanes per row), long rows by whole warps
             n_long = P->full_class[1];
-            const long long b1 = P->full_class[1], b2 = P->full_class[2], b3 = P->full_class[3], b4 = P->full_class[4];
-            if (b2 > b1) { k_forward_short<16><<<fwd_grid(P, (b2 - b1 + 1) / 2), FWD_THREADS, 0, P->stream>>>(b2 - b1, R.items + b1, R.vox + b1, m, R.col, R.valD, R.valL, xd, dd, dl, letd_out); ++P->launches; }
-            if (b3 > b2) { k_forward_short<8><<<fwd_grid(P, (b3 - b2 + 3) / 4), FWD_THREADS, 0, P->stream>>>(b3 - b2, R.items + b2, R.vox + b2, m, R.col, R.valD, R.valL, xd, dd, dl, letd_out); ++P->launches; }
-            if (b4 > b3) { k_forward_short<4><<<fwd_grid(P, (b4 - b3 + 7) / 8), FWD_THREADS, 0, P->stream>>>(b4 - b3, R.items + b3, R.vox + b3, m, R.col, R.valD, R.valL, xd, dd, dl, letd_out); ++P->launches; }
+            const long long b[4] = {P->full_class[1], P->full_class[2], P->full_class[3], P->full_class[4]};
+#define SHORT_LAUNCH(G, LO, HI)                                                                                                  \
+    if (HI > LO) {                                                                                                               \
+        const int gg = fwd_grid(P, ((HI) - (LO) + (32 / G) - 1) / (32 / G));                                                    \
+        if (i16) k_forward_short<G, true><<<gg, FWD_THREADS, 0, P->stream>>>((HI) - (LO), R.items + (LO), R.vox + (LO), m, colp, R.valD, R.valL, xd, dd, dl, letd_out); \
+        else k_forward_short<G, false><<<gg, FWD_THREADS, 0, P->stream>>>((HI) - (LO), R.items + (LO), R.vox + (LO), m, colp, R.valD, R.valL, xd, dd, dl, letd_out);    \
+        ++P->launches;                                                                                                           \
+    }
+            SHORT_LAUNCH(16, b[0], b[1])
+            SHORT_LAUNCH(8, b[1], b[2])
+            SHORT_LAUNCH(4, b[2], b[3])
+#undef SHORT_LAUNCH
         }
         if (n_long) {
-            k_forward<EPI_F32VOX><<<fwd_grid(P, n_long), FWD_THREADS, 0, P->stream>>>(n_long, R.items, R.vox, md, R.col, R.valD, R.valL, xd,
-                                                                                  nullptr, nullptr, GatherVec{nullptr, nullptr, nullptr},
-                                                                                  nullptr, nullptr, dd, dl, letd_out);
+            if (i16) k_forward<EPI_F32VOX, true><<<fwd_grid(P, n_long), FWD_THREADS, 0, P->stream>>>(n_long, R.items, R.vox, md, colp, R.valD, R.valL, xd, nullptr, nullptr, none, nullptr, nullptr, dd, dl, letd_out);
+            else k_forward<EPI_F32VOX, false><<<fwd_grid(P, n_long), FWD_THREADS, 0, P->stream>>>(n_long, R.items, R.vox, md, colp, R.valD, R.valL, xd, nullptr, nullptr, none, nullptr, nullptr, dd, dl, letd_out);
             ++P->launches;
         }
     }

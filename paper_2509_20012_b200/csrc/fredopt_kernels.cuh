@@ -46,7 +46,8 @@ struct DevState {
 };
 
 // One work item: `len` entries (multiple of 4) starting at entry `start` (multiple of 4) of the index / value
-// arrays; `seg` = structure - 1 (selects which value arrays are read).  16 bytes: fetched with one 128-bit load.
+// arrays; `seg` = structure - 1 (selects which value arrays are read); transposed items carry the 65536-row block of
+// their 16-bit row indices in seg >> 8.  16 bytes: fetched with one 128-bit load.
 struct __align__(16) Item {
     long long start;
     int32_t len;
@@ -78,6 +79,17 @@ __device__ __forceinline__ float4 ld_stream_f4(const float* p) {
     asm volatile("ld.global.nc.L1::no_allocate.v4.f32 {%0,%1,%2,%3}, [%4];"
                  : "=f"(r.x), "=f"(r.y), "=f"(r.z), "=f"(r.w) : "l"(p));
     return r;
+}
+// four consecutive stored indices starting at entry e (multiple of 4): 32-bit form or 16-bit form (+ `add`)
+template <bool I16>
+__device__ __forceinline__ int4 ld_idx4(const void* __restrict__ base, long long e, int add) {
+    if (I16) {
+        unsigned int lo, hi;
+        asm volatile("ld.global.nc.L1::no_allocate.v2.u32 {%0,%1}, [%2];" : "=r"(lo), "=r"(hi) : "l"((const uint16_t*)base + e));
+        return make_int4((int)(lo & 0xFFFFu) + add, (int)(lo >> 16) + add, (int)(hi & 0xFFFFu) + add, (int)(hi >> 16) + add);
+    } else {
+        return ld_stream_i4((const int32_t*)base + e);
+    }
 }
 __device__ __forceinline__ Item ld_item(const Item* p) {
     const int4 v = __ldg((const int4*)p);
@@ -118,8 +130,8 @@ enum : int { EPI_STORE = 0, EPI_STORE_PQ = 1, EPI_CPART = 2, EPI_F32VOX = 3 };
 
 // <D_i, x> and / or <L_i, x> of one row by one warp.  M: bit 0 = D, bit 1 = L.  Four 128-entry chunks per trip:
 // up to 12 independent 128-bit loads per lane in flight before the first gather.
-template <int M>
-__device__ __forceinline__ void fwd_row(const int32_t* __restrict__ cp, const float* __restrict__ dp,
+template <int M, bool I16>
+__device__ __forceinline__ void fwd_row(const void* __restrict__ cbase, long long e0, const float* __restrict__ dp,
                                         const float* __restrict__ lp, int L, int lane, const double* __restrict__ x,
                                         double& aD, double& aL) {
     constexpr int U = 4;
@@ -129,7 +141,7 @@ __device__ __forceinline__ void fwd_row(const int32_t* __restrict__ cp, const fl
         float4 d[U], l[U];
 #pragma unroll
         for (int u = 0; u < U; ++u) {
-            c[u] = ld_stream_i4(cp + p + 128 * u);
+            c[u] = ld_idx4<I16>(cbase, e0 + p + 128 * u, 0);
             if (M & 1) d[u] = ld_stream_f4(dp + p + 128 * u);
             if (M & 2) l[u] = ld_stream_f4(lp + p + 128 * u);
         }
@@ -147,7 +159,7 @@ __device__ __forceinline__ void fwd_row(const int32_t* __restrict__ cp, const fl
 #pragma unroll
         for (int u = 0; u < U - 1; ++u) {
             const bool ok = p + 128 * u < L;
-            c[u] = ok ? ld_stream_i4(cp + p + 128 * u) : make_int4(0, 0, 0, 0);
+            c[u] = ok ? ld_idx4<I16>(cbase, e0 + p + 128 * u, 0) : make_int4(0, 0, 0, 0);
             if (M & 1) d[u] = ok ? ld_stream_f4(dp + p + 128 * u) : make_float4(0.f, 0.f, 0.f, 0.f);
             if (M & 2) l[u] = ok ? ld_stream_f4(lp + p + 128 * u) : make_float4(0.f, 0.f, 0.f, 0.f);
         }
@@ -165,10 +177,10 @@ __device__ __forceinline__ void fwd_row(const int32_t* __restrict__ cp, const fl
 // One warp per item, items r = warp, warp + W, ... (static mapping: deterministic partial sums; the warps of the
 // grid read one contiguous window of the arrays at any time).  The next item's descriptor is fetched one item ahead.
 // mode[seg]: bit 0 = read valD, bit 1 = read valL.
-template <int EPI>
+template <int EPI, bool I16>
 __global__ void __launch_bounds__(FWD_THREADS, 3)
 k_forward(long long n, const Item* __restrict__ items, const int32_t* __restrict__ vox, const uint8_t* __restrict__ mode,
-          const int32_t* __restrict__ col, const float* __restrict__ vD, const float* __restrict__ vL,
+          const void* __restrict__ col, const float* __restrict__ vD, const float* __restrict__ vL,
           const double* __restrict__ x,
           double* __restrict__ oD, double* __restrict__ oL,                // EPI_STORE*, EPI_CPART: item-indexed
           const GatherVec pq,                                              // EPI_STORE_PQ: cost residuals (Eq. 2)
@@ -187,10 +199,9 @@ k_forward(long long n, const Item* __restrict__ items, const int32_t* __restrict
         if (rn < n) nx = ld_item(items + rn);
         const int m = mode[it.seg];
         double aD = 0.0, aL = 0.0;
-        const int32_t* cp = col + it.start;
-        if (m == 3) fwd_row<3>(cp, vD + it.start, vL + it.start, it.len, lane, x, aD, aL);
-        else if (m == 1) fwd_row<1>(cp, vD + it.start, nullptr, it.len, lane, x, aD, aL);
-        else if (m == 2) fwd_row<2>(cp, nullptr, vL + it.start, it.len, lane, x, aD, aL);
+        if (m == 3) fwd_row<3, I16>(col, it.start, vD + it.start, vL + it.start, it.len, lane, x, aD, aL);
+        else if (m == 1) fwd_row<1, I16>(col, it.start, vD + it.start, nullptr, it.len, lane, x, aD, aL);
+        else if (m == 2) fwd_row<2, I16>(col, it.start, nullptr, vL + it.start, it.len, lane, x, aD, aL);
         if (m & 1) aD = warp_sum(aD);
         if (m & 2) aL = warp_sum(aL);
         if (lane == 0) {
@@ -227,10 +238,10 @@ k_forward(long long n, const Item* __restrict__ items, const int32_t* __restrict
 // Short rows (at most 4*G entries, G = 4, 8 or 16): G lanes per row, 32/G rows per warp at a time, one 128-bit load per
 // lane and array, shuffle reduction inside the lane group.  Rows of one length class are stored back to back, so the
 // warp's loads are contiguous.  fp32 voxel-indexed outputs only (fredopt_dose_let / fredopt_spmv_forward over all rows).
-template <int G>
+template <int G, bool I16>
 __global__ void __launch_bounds__(FWD_THREADS)
 k_forward_short(long long n, const Item* __restrict__ items, const int32_t* __restrict__ vox, int m,
-                const int32_t* __restrict__ col, const float* __restrict__ vD, const float* __restrict__ vL,
+                const void* __restrict__ col, const float* __restrict__ vD, const float* __restrict__ vL,
                 const double* __restrict__ x, float* __restrict__ fD, float* __restrict__ fL, int letd_out)
 {
     constexpr int RPW = 32 / G;                       // rows per warp and trip
@@ -243,7 +254,7 @@ k_forward_short(long long n, const Item* __restrict__ items, const int32_t* __re
             const Item it = ld_item(items + r);
             if (4 * t < it.len) {
                 const long long p = it.start + 4 * t;
-                const int4 c = ld_stream_i4(col + p);
+                const int4 c = ld_idx4<I16>(col, p, 0);
                 const double x0 = __ldg(x + c.x), x1 = __ldg(x + c.y), x2 = __ldg(x + c.z), x3 = __ldg(x + c.w);
                 if (m & 1) fma4(aD, ld_stream_f4(vD + p), x0, x1, x2, x3);
                 if (m & 2) fma4(aL, ld_stream_f4(vL + p), x0, x1, x2, x3);
@@ -267,8 +278,8 @@ enum : int { TEPI_F32 = 0, TEPI_GRAD = 1, TEPI_UPDATE = 2 };
 
 // sum_i D_ij vec[i].x + L_ij vec[i].y over one item by one warp (vec is L2-resident; entries of a spot run over
 // ascending compact row indices, so neighbouring lanes gather neighbouring elements)
-template <int M>
-__device__ __forceinline__ double tr_item(const int32_t* __restrict__ cp, const float* __restrict__ dp,
+template <int M, bool I16>
+__device__ __forceinline__ double tr_item(const void* __restrict__ cbase, long long e0, int add, const float* __restrict__ dp,
                                           const float* __restrict__ lp, int L, int lane, const GatherVec& gv) {
     constexpr int U = 4;
     const double2* __restrict__ vec = gv.pair;
@@ -280,7 +291,7 @@ __device__ __forceinline__ double tr_item(const int32_t* __restrict__ cp, const 
         float4 d[U], l[U];
 #pragma unroll
         for (int u = 0; u < U; ++u) {
-            c[u] = ld_stream_i4(cp + p + 128 * u);
+            c[u] = ld_idx4<I16>(cbase, e0 + p + 128 * u, add);
             if (M & 1) d[u] = ld_stream_f4(dp + p + 128 * u);
             if (M & 2) l[u] = ld_stream_f4(lp + p + 128 * u);
         }
@@ -302,7 +313,7 @@ __device__ __forceinline__ double tr_item(const int32_t* __restrict__ cp, const 
 #pragma unroll
         for (int u = 0; u < U - 1; ++u) {
             const bool ok = p + 128 * u < L;
-            c[u] = ok ? ld_stream_i4(cp + p + 128 * u) : make_int4(0, 0, 0, 0);
+            c[u] = ok ? ld_idx4<I16>(cbase, e0 + p + 128 * u, add) : make_int4(0, 0, 0, 0);
             if (M & 1) d[u] = ok ? ld_stream_f4(dp + p + 128 * u) : make_float4(0.f, 0.f, 0.f, 0.f);
             if (M & 2) l[u] = ok ? ld_stream_f4(lp + p + 128 * u) : make_float4(0.f, 0.f, 0.f, 0.f);
         }
@@ -327,9 +338,10 @@ __device__ __forceinline__ double tr_item(const int32_t* __restrict__ cp, const 
 // of a CTA mostly work on neighbouring spots of one structure and share L1 lines of the gather vector).  Item r
 // stores its partial sum in slot item_slot[r]; k_combine adds the slots of every spot in slot order.  No
 // floating-point atomics, no fences: the result does not depend on the schedule.
+template <bool I16>
 __global__ void __launch_bounds__(FWD_THREADS, 3)
 k_transpose(long long n, const Item* __restrict__ items, const int32_t* __restrict__ item_slot,
-            const uint8_t* __restrict__ mode, const int32_t* __restrict__ t_col, const float* __restrict__ tD,
+            const uint8_t* __restrict__ mode, const void* __restrict__ t_col, const float* __restrict__ tD,
             const float* __restrict__ tL, const GatherVec vec, double* __restrict__ partial)
 {
     const int lane = threadIdx.x & 31;
@@ -341,12 +353,12 @@ k_transpose(long long n, const Item* __restrict__ items, const int32_t* __restri
         const long long rn = r + nwarps;
         Item nx;
         if (rn < n) nx = ld_item(items + rn);
-        const int m = mode[it.seg];
+        const int m = mode[it.seg & 0xFF];
+        const int add = (it.seg >> 8) << 16;              // 16-bit form: the run's 65536-row block
         double tot = 0.0;
-        const int32_t* cp = t_col + it.start;
-        if (m == 3) tot = tr_item<3>(cp, tD + it.start, tL + it.start, it.len, lane, vec);
-        else if (m == 1) tot = tr_item<1>(cp, tD + it.start, nullptr, it.len, lane, vec);
-        else if (m == 2) tot = tr_item<2>(cp, nullptr, tL + it.start, it.len, lane, vec);
+        if (m == 3) tot = tr_item<3, I16>(t_col, it.start, add, tD + it.start, tL + it.start, it.len, lane, vec);
+        else if (m == 1) tot = tr_item<1, I16>(t_col, it.start, add, tD + it.start, nullptr, it.len, lane, vec);
+        else if (m == 2) tot = tr_item<2, I16>(t_col, it.start, add, nullptr, tL + it.start, it.len, lane, vec);
         if (m) tot = warp_sum(tot);
         if (lane == 0) partial[item_slot[r]] = tot;
         r = rn;
