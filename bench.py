@@ -139,6 +139,21 @@ def run_reference(args):
         "gpu_launches": 0}))
 
 
+def max_over_ranks(values, dist, device):
+    """Element-wise MAX of a list of per-rank timings over all ranks (one all-reduce); identity at world size 1."""
+    if dist is None:
+        return [float(v) for v in values]
+    t = torch.tensor(list(values), dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return [float(v) for v in t]
+
+
+def whole_job_rate(units_per_rank, world_size, seconds):
+    """Weak scaling over independent plans: every rank processed `units_per_rank` iterations of its own plan in at most
+    `seconds` (the max over ranks) => whole-job iterations/s."""
+    return world_size * units_per_rank / seconds
+
+
 # ------------------------------------------------------------------------------------------------ our arm
 def run_ours(args):
     ws, rank, lr = _dist_init()
@@ -238,15 +253,12 @@ def run_ours(args):
     spmv = ("forward_x", "transpose_g", "forward_g", "transpose_b")
     four_gbs = sum(pass_bytes[n] for n in spmv) / max(sum(passes[n]["ms"] for n in spmv), 1e-9) / 1e6
 
-    if dist is not None:
-        t = torch.tensor([ms, e2e_s], dtype=torch.float64, device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms, e2e_s = float(t[0]), float(t[1])
+    ms, e2e_s = max_over_ranks([ms, e2e_s], dist, "cuda")
     if rank != 0:
         if dist is not None:
             dist.destroy_process_group()
         return
-    value = ws * K / (ms * 1e-3)
+    value = whole_job_rate(K, ws, ms * 1e-3)
     out = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": ws, "steps": K, "warmup": W, "ms_per_step": ms / K,
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64 accumulate / f32 matrix values",
@@ -260,7 +272,7 @@ def run_ours(args):
                          "inputs larger than L2 (%.2f GB streamed per iteration)" % (iter_bytes / 1e9),
                    "parallelism": "1 plan per GPU"},
         "iter_gbs": iter_bytes * K / (ms * 1e-3) / 1e9,
-        "e2e": {"value": ws * K / e2e_s, "unit": UNIT, "h2d_bytes_per_step": plan.n_cols * 4,
+        "e2e": {"value": whole_job_rate(K, ws, e2e_s), "unit": UNIT, "h2d_bytes_per_step": plan.n_cols * 4,
                 "d2h_bytes_per_step": plan.n_cols * 4 + STATE_BYTES},
         "gpu_launches": int(launches),
         "clocks": clocks,
@@ -302,7 +314,8 @@ def cpu_baseline(plan, spec, args):
 def run_sweep(args):
     """BASELINE.json configs[4]: isolated SpMV passes on configs[2]-geometry matrices with every voxel labelled; spot sigma
     3 -> 10 mm, non-zeros 1e7 -> 1.2e9 (through pitch and layer count); x log-uniform on [1e-3, 1].  One JSON line per
-    (sigma, nnz) point with GB/s (algorithmic bytes: 4 B index + 4 B per value array per non-zero) of every pass, timed
+    (sigma, nnz) point with GB/s (algorithmic bytes: the stored index -- 2 B, or 4 B for columns when there are more than
+    65536 spots -- + 4 B per value array per non-zero) of every pass, timed
     with CUDA events around the C-ABI call (its vector conversions included), median of `--steps` repetitions."""
     import gc
     from paper_2509_20012_b200 import fredopt, plangen as pg
@@ -330,9 +343,17 @@ def run_sweep(args):
         ms = float(np.median(ts))
         return {"ms": ms, "gbs": nbytes / ms / 1e6, "frac_of_measured_peak": nbytes / ms / 1e6 / peak}
 
+    def spec_of(sigma, pitch, layers):
+        # SURVEY sec. 8d labels every voxel so that "active = all"; here the passes run with the ROWS_ALL selector
+        # instead (same rows, same arithmetic) and the ordinary structure labels are kept, so that the plan does not
+        # hold a second, labelled copy of the whole matrix in HBM
+        sp = pg.sweep_spec(sigma, pitch, layers)
+        sp.label_all = False
+        return sp
+
     for sigma in sigmas:
         # probe: non-zeros at a coarse lattice, then scale the spot count (pitch) and layer count to the target
-        probe = pg.build_plan(pg.sweep_spec(sigma, 12.0, 6), device="cuda")
+        probe = pg.build_plan(spec_of(sigma, 12.0, 6), device="cuda")
         nnz0 = probe.nnz
         del probe
         for target in targets:
@@ -340,33 +361,34 @@ def run_sweep(args):
             layers = int(min(40, max(6, round(6 * ratio ** 0.4))))
             pitch = 12.0 / math.sqrt(max(ratio * 6 / layers, 1e-9))
             pitch = min(max(pitch, 0.8), 40.0)
-            plan = pg.build_plan(pg.sweep_spec(sigma, pitch, layers), device="cuda")
+            plan = pg.build_plan(spec_of(sigma, pitch, layers), device="cuda")
             for _ in range(2):                                     # the lattice is discrete: correct the pitch
                 if 0.85 < plan.nnz / target < 1.18 or pitch <= 0.8:
                     break
                 pitch = min(max(pitch * math.sqrt(plan.nnz / target), 0.8), 40.0)
                 del plan
-                plan = pg.build_plan(pg.sweep_spec(sigma, pitch, layers), device="cuda")
+                plan = pg.build_plan(spec_of(sigma, pitch, layers), device="cuda")
             gp = fredopt.from_plan(plan, stream=stream.cuda_stream)
             V, S, nnz = plan.n_rows, plan.n_cols, plan.nnz
             x = torch.from_numpy(pg.log_uniform_weights(5, S)).cuda()
             r = torch.from_numpy(pg.log_uniform_weights(6, V)).cuda()
             d = torch.empty(V, dtype=torch.float32, device="cuda"); l = torch.empty_like(d)
             o = torch.empty(S, dtype=torch.float32, device="cuda")
-            resident = 12 * nnz < 2 * l2
-            # every voxel carries a label here, so the labelled-row transposes built at creation cover the whole
-            # matrix: the transposed passes go through ROWS_ACTIVE (no second transposed copy in HBM)
+            resident = 10 * nnz < 2 * l2
+            gp.spmv_transpose(fredopt.ROWS_ALL, r, None, o)        # builds the transposed copy of the full matrix
+            ibf = 2 if S <= 65536 else 4                           # index bytes as stored (16-bit columns if they fit)
+            ibt = 2                                                # transposed: 16-bit row index inside 65536-row blocks
             res = {
-                "forward_D": timed(lambda: gp.spmv_forward(fredopt.ROWS_ALL, x, d, None), 8 * nnz, resident),
-                "forward_DL_fused": timed(lambda: gp.spmv_forward(fredopt.ROWS_ALL, x, d, l), 12 * nnz, resident),
-                "transpose_D": timed(lambda: gp.spmv_transpose(fredopt.ROWS_ACTIVE, r, None, o), 8 * nnz, resident),
-                "transpose_L": timed(lambda: gp.spmv_transpose(fredopt.ROWS_ACTIVE, None, r, o), 8 * nnz, resident),
-                "transpose_DL_fused": timed(lambda: gp.spmv_transpose(fredopt.ROWS_ACTIVE, r, r, o), 12 * nnz, resident),
+                "forward_D": timed(lambda: gp.spmv_forward(fredopt.ROWS_ALL, x, d, None), (ibf + 4) * nnz, resident),
+                "forward_DL_fused": timed(lambda: gp.spmv_forward(fredopt.ROWS_ALL, x, d, l), (ibf + 8) * nnz, resident),
+                "transpose_D": timed(lambda: gp.spmv_transpose(fredopt.ROWS_ALL, r, None, o), (ibt + 4) * nnz, resident),
+                "transpose_L": timed(lambda: gp.spmv_transpose(fredopt.ROWS_ALL, None, r, o), (ibt + 4) * nnz, resident),
+                "transpose_DL_fused": timed(lambda: gp.spmv_transpose(fredopt.ROWS_ALL, r, r, o), (ibt + 8) * nnz, resident),
             }
             rows_ne = int((plan.row_ptr[1:] > plan.row_ptr[:-1]).sum().item())
             print(json.dumps({"sweep": "configs[4]", "sigma_mm": sigma, "pitch_mm": round(pitch, 3), "layers": layers,
                               "n_voxels": V, "n_spots": S, "nnz": nnz, "mean_row": nnz / max(rows_ne, 1),
-                              "mean_col": nnz / max(S, 1), "l2": "L2 flushed before every repetition" if resident
+                              "mean_col": nnz / max(S, 1), "index_bytes": [ibf, ibt], "l2": "L2 flushed before every repetition" if resident
                               else "larger than L2", "peak_gbs": peak, "passes": res}), flush=True)
             gp.destroy()
             del plan, gp, x, r, d, l, o

@@ -674,7 +674,7 @@ static void ev_end(fredopt_plan* P) {
 }
 
 // grid of the item kernels: one warp per item up to FWD_CTAS_PER_SM resident-CTA-fulls per SM (then round-robin)
-constexpr int FWD_CTAS_PER_SM = 6;   // 2 waves of the 3 CTAs an SM holds (launch bounds of k_forward / k_transpose)
+constexpr int FWD_CTAS_PER_SM = 2 * FWD_MIN_CTAS;   // 2 waves of the CTAs an SM holds (launch bounds of k_forward / k_transpose)
 static int fwd_grid(fredopt_plan* P, long long n) {
     const int cap = P->sm_count * FWD_CTAS_PER_SM < MAX_PARTIALS ? P->sm_count * FWD_CTAS_PER_SM : MAX_PARTIALS;
     return grid_for(n, FWD_WARPS, cap);

@@ -25,6 +25,7 @@ constexpr int FWD_WARPS = FWD_THREADS / 32;
 constexpr int MAX_PARTIALS = 2368;          // 148 SMs x 16 CTAs: upper bound of any partial-sum grid
 constexpr int ROW_THREADS = 256;
 constexpr int TR_ITEM_MAX = 2048;           // entries per transposed work item (multiple of 4)
+constexpr int FWD_MIN_CTAS = 4;             // resident CTAs per SM the item kernels are compiled for (64 registers)
 
 // flags of a structure
 enum : int { F_DOSE_SLAB = 1, F_DL_SLAB = 2, F_LETD = 4, F_DOSE_REF = 8, F_DL_REF = 16 };
@@ -178,7 +179,7 @@ __device__ __forceinline__ void fwd_row(const void* __restrict__ cbase, long lon
 // grid read one contiguous window of the arrays at any time).  The next item's descriptor is fetched one item ahead.
 // mode[seg]: bit 0 = read valD, bit 1 = read valL.
 template <int EPI, bool I16>
-__global__ void __launch_bounds__(FWD_THREADS, 3)
+__global__ void __launch_bounds__(FWD_THREADS, FWD_MIN_CTAS)
 k_forward(long long n, const Item* __restrict__ items, const int32_t* __restrict__ vox, const uint8_t* __restrict__ mode,
           const void* __restrict__ col, const float* __restrict__ vD, const float* __restrict__ vL,
           const double* __restrict__ x,
@@ -339,7 +340,7 @@ __device__ __forceinline__ double tr_item(const void* __restrict__ cbase, long l
 // stores its partial sum in slot item_slot[r]; k_combine adds the slots of every spot in slot order.  No
 // floating-point atomics, no fences: the result does not depend on the schedule.
 template <bool I16>
-__global__ void __launch_bounds__(FWD_THREADS, 3)
+__global__ void __launch_bounds__(FWD_THREADS, FWD_MIN_CTAS)
 k_transpose(long long n, const Item* __restrict__ items, const int32_t* __restrict__ item_slot,
             const uint8_t* __restrict__ mode, const void* __restrict__ t_col, const float* __restrict__ tD,
             const float* __restrict__ tL, const GatherVec vec, double* __restrict__ partial)
