@@ -64,6 +64,9 @@ struct Plan {
     double eta = 1.0;
     int64_t reductionsN = 1, max_trials = 200;
     bool accept_check = true;
+    bool block_sequential = false;     // reading R23: Fig. 2's loop nest, sequential over (kind, ROI) blocks
+    double sweep_prox = 0.0;           // statistics of the last block-sequential sweep (at visit time)
+    int64_t sweep_viol = 0;
 };
 
 // <A_i, x>
@@ -210,6 +213,51 @@ void constraint_pass(const Plan& P, const std::vector<double>& x, std::vector<do
     if (n_viol) *n_viol = nv;
 }
 
+// Block-sequential AMS sweep (reading R23): the loop nest of Fig. 2 -- first the dose kind over all
+// ROIs in label order, then the cDLET kind, then the LETd rows of north_star -- taken block by block: SEQUENTIAL over
+// the (kind, ROI) blocks, SIMULTANEOUS inside a block.  For block b = (kind, ROI s) with participating rows
+// P_b = {i in s : |a_i|^2 > 0}, m = |P_b|:
+//     x <- x - relax * min(w_s, 1) * (1/m) * sum_{i in P_b} (r_i / |a_i|^2) a_i,     every r_i taken at the x the block starts from
+// (the per-row step fractions of Fig. 2 averaged over the block; min(w_s, 1) is the structure's priority as a relaxation
+// factor).  The clamp of PAPER.md:149-154 follows the last block.  Statistics: sets found violated when their
+// block is visited, and 1/2 sum w^_s r_i^2/|a_i|^2 over them (global w^ of R3).
+void block_sweep(Plan& P, double relax) {
+    const int64_t V = P.D.n_rows, S = P.D.n_cols;
+    std::vector<double>& x = P.x;
+    std::vector<double> step(S);
+    P.sweep_prox = 0.0; P.sweep_viol = 0;
+    for (int kind = 0; kind < 3; ++kind)
+        for (size_t s = 1; s <= P.bounds.size(); ++s) {
+            const Bounds& b = P.bounds[s - 1];
+            if (kind == 0 ? !has_dose_slab(b) : kind == 1 ? !has_dl_slab(b) : !has_letd(b)) continue;
+            std::fill(step.begin(), step.end(), 0.0);
+            int64_t m = 0;
+            for (int64_t i = 0; i < V; ++i) {
+                if (P.label[i] != (int32_t)s) continue;
+                double r, n;
+                if (kind == 0) { r = slab_residual(row_dot(P.D, i, x), b.dose_lo, b.dose_hi); n = P.nD[i]; }
+                else if (kind == 1) { r = slab_residual(row_dot(P.L, i, x), b.dl_lo, b.dl_hi); n = P.nL[i]; }
+                else { double val = letd_row_dot(P, i, b.letd_max, x, nullptr); r = val > 0.0 ? val : 0.0; n = P.nT[i]; }
+                if (r != 0.0) ++P.sweep_viol;
+                if (!(n > 0.0)) continue;
+                ++m;
+                if (r == 0.0) continue;
+                P.sweep_prox += 0.5 * P.what[s - 1] * r * r / n;
+                const double c = r / n;
+                if (kind == 0) for (int64_t p = P.D.ptr[i]; p < P.D.ptr[i + 1]; ++p) step[P.D.col[p]] += c * P.D.val[p];
+                else if (kind == 1) for (int64_t p = P.L.ptr[i]; p < P.L.ptr[i + 1]; ++p) step[P.L.col[p]] += c * P.L.val[p];
+                else {
+                    for (int64_t p = P.L.ptr[i]; p < P.L.ptr[i + 1]; ++p) step[P.L.col[p]] += c * P.L.val[p];
+                    for (int64_t p = P.D.ptr[i]; p < P.D.ptr[i + 1]; ++p) step[P.D.col[p]] -= c * b.letd_max * P.D.val[p];
+                }
+            }
+            if (m == 0) continue;
+            const double f = relax * (b.weight < 1.0 ? b.weight : 1.0) / (double)m;
+            for (int64_t j = 0; j < S; ++j) x[j] -= f * step[j];
+        }
+    for (int64_t j = 0; j < S; ++j) if (x[j] < 0.0) x[j] = 0.0;
+}
+
 void fill_csr(Csr& A, int64_t V, int64_t S, const int64_t* ptr, const int32_t* col, const float* val) {
     A.n_rows = V; A.n_cols = S;
     A.ptr.assign(ptr, ptr + V + 1);
@@ -247,7 +295,7 @@ void oracle_set_x(void* h, const float* x) { Plan* P = (Plan*)h; for (size_t j =
 void oracle_set_x64(void* h, const double* x) { Plan* P = (Plan*)h; P->x.assign(x, x + P->x.size()); }
 void oracle_get_x(void* h, double* x) { Plan* P = (Plan*)h; std::memcpy(x, P->x.data(), P->x.size() * sizeof(double)); }
 
-// keys: 0 eta, 1 reductionsN, 2 accept_check, 3 max_trials, 4 reset (k, s, beta)
+// keys: 0 eta, 1 reductionsN, 2 accept_check, 3 max_trials, 4 reset (k, s, beta), 7 block-sequential AMS (R23)
 void oracle_set_option(void* h, int32_t key, double v) {
     Plan* P = (Plan*)h;
     switch (key) {
@@ -256,6 +304,7 @@ void oracle_set_option(void* h, int32_t key, double v) {
         case 2: P->accept_check = v != 0.0; break;
         case 3: P->max_trials = (int64_t)v; break;
         case 4: P->k = 0; P->s = 0; P->trials = 0; P->started = false; P->eta_pow = 1.0; P->last_beta = 0.0; break;
+        case 7: P->block_sequential = v != 0.0; break;
         default: break;
     }
 }
@@ -345,11 +394,14 @@ void oracle_iterate(void* h, int32_t n_iter, float lambda_f, float beta0_f, floa
             }
         }
         // ---- feasibility-seeking step with w_k = eta^k w, simultaneous form (R1)
-        constraint_pass(*P, P->x, &step, nullptr, nullptr);
         const double relax = lambda * P->eta_pow;
-        for (int64_t j = 0; j < S; ++j) {
-            double v = P->x[j] - relax * step[j];
-            P->x[j] = v < 0.0 ? 0.0 : v;                                       // clamp (R6)
+        if (P->block_sequential) block_sweep(*P, relax);                       // R23: Fig. 2's own loop nest, block by block
+        else {
+            constraint_pass(*P, P->x, &step, nullptr, nullptr);
+            for (int64_t j = 0; j < S; ++j) {
+                double v = P->x[j] - relax * step[j];
+                P->x[j] = v < 0.0 ? 0.0 : v;                                   // clamp (R6)
+            }
         }
         P->eta_pow *= P->eta;
         ++P->k;
@@ -361,6 +413,11 @@ void oracle_stats(void* h, int64_t* out, double* dout) {
     Plan* P = (Plan*)h;
     out[0] = P->k; out[1] = P->s; out[2] = P->trials; out[3] = P->n_sets; out[4] = P->n_zero_norm_sets;
     dout[0] = P->last_beta; dout[1] = P->W; dout[2] = P->beta_next;
+}
+
+void oracle_sweep_stats(void* h, double* prox, int64_t* n_viol) {
+    Plan* P = (Plan*)h;
+    *prox = P->sweep_prox; *n_viol = P->sweep_viol;
 }
 
 void oracle_norms(void* h, double* nD, double* nL, double* nT) {

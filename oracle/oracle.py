@@ -16,6 +16,7 @@ _SRC = os.path.join(_HERE, "fredopt_oracle.cpp")
 _LIB = os.path.join(_HERE, "libfredopt_oracle.so")
 
 OPT_ETA, OPT_REDUCTIONS, OPT_ACCEPT_CHECK, OPT_MAX_TRIALS, OPT_RESET = 0, 1, 2, 3, 4
+OPT_BLOCK_SEQUENTIAL = 7
 
 
 def build(force: bool = False) -> str:
@@ -50,6 +51,7 @@ def _load():
         lib.oracle_proximity.argtypes = [vp, vp, vp, vp]
         lib.oracle_iterate.argtypes = [vp, i32, f32, f32, f32]
         lib.oracle_stats.argtypes = [vp, vp, vp]
+        lib.oracle_sweep_stats.argtypes = [vp, vp, vp]
         lib.oracle_norms.argtypes = [vp, vp, vp, vp]
         lib.oracle_what.argtypes = [vp, vp]
         lib.oracle_sequential_sweep.argtypes = [vp, f32]
@@ -156,6 +158,12 @@ class Oracle:
         self._lib.oracle_stats(self._h, _p(o), _p(d))
         return dict(k=int(o[0]), s=int(o[1]), trials=int(o[2]), n_sets=int(o[3]), n_zero_norm_sets=int(o[4]),
                     last_beta=float(d[0]), W=float(d[1]), beta_next=float(d[2]))
+
+    def sweep_stats(self):
+        """(proximity, violated sets) met by the last block-sequential sweep at visit time."""
+        pr = C.c_double(0.0); nv = C.c_int64(0)
+        self._lib.oracle_sweep_stats(self._h, C.byref(pr), C.byref(nv))
+        return pr.value, nv.value
 
     def norms(self):
         a = np.empty(self.V, np.float64); b = np.empty(self.V, np.float64); c = np.empty(self.V, np.float64)

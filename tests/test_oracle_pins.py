@@ -480,3 +480,117 @@ def test_config0_matches_survey_probe_trajectory(plan0):
             assert nv == gold[f"{tag}_viol_{n}"], (tag, n, nv)
         if tag == "sa":
             assert o.stats()["s"] == 50       # single beam: no rejections
+
+
+# ----------------------------------------------------------------------------- block-sequential AMS (reading R23)
+def _dense_block_sweep(Dd, Ld, labels, b, x, lam):
+    """Dense restatement of the block-sequential sweep, written separately from the oracle: Fig. 2's loop nest (dose kind
+    over the ROIs, then cDLET, then the LETd rows), one averaged simultaneous step per (kind, ROI) block, clamp at the end."""
+    b = np.asarray(b, dtype=F32).astype(np.float64)
+    x = x.copy()
+    nviol = 0
+    for kind in range(3):
+        for s in range(1, b.shape[0] + 1):
+            w, dlo, dhi, llo, lhi, tmax = b[s - 1, :6]
+            rows = [i for i, lab in enumerate(labels) if lab == s]
+            if kind == 0:
+                if np.isnan(dlo) and np.isnan(dhi):
+                    continue
+                A, lo, hi = Dd[rows], dlo, dhi
+            elif kind == 1:
+                if np.isnan(llo) and np.isnan(lhi):
+                    continue
+                A, lo, hi = Ld[rows], llo, lhi
+            else:
+                if np.isnan(tmax):
+                    continue
+                A, lo, hi = Ld[rows] - tmax * Dd[rows], NAN, 0.0
+            vals = A @ x
+            r = np.array([DenseReference.resid(v, lo, hi) for v in vals])
+            n2 = np.einsum("ij,ij->i", A, A)
+            nviol += int(np.count_nonzero(r))
+            part = n2 > 0
+            if not part.any():
+                continue
+            step = (r[part] / n2[part]) @ A[part]
+            x = x - lam * min(w, 1.0) / part.sum() * step
+    return np.maximum(x, 0.0), nviol
+
+
+@pytest.mark.parametrize("seed,same", [(11, True), (12, False), (13, True)])
+def test_pin13_block_sequential_dense_brute_force(seed, same):
+    """CSR traversal, block order (kind-major, then ROI), block averaging, priority factor, clamp, sweep statistics."""
+    D, L, labels, x0 = pg.random_small_plan(seed, V=36, S=7, n_struct=3, same_pattern=same)
+    bounds = bounds_rows(dict(weight=1.0, dose_lo=0.8, dose_hi=1.1, dose_ref=1.0),
+                         dict(weight=0.5, dose_hi=0.6, dl_lo=0.5, dl_hi=2.5, letd_max=3.5, dl_ref=2.0),
+                         dict(weight=2.0, dose_hi=0.7, letd_max=4.0))
+    Dd, Ld = csr_to_dense(D, 7), csr_to_dense(L, 7)
+    o = orc.Oracle.create(36, 7, D, L, labels, bounds)
+    o.set_option(orc.OPT_BLOCK_SEQUENTIAL, 1)
+    o.set_x(x0)
+    x = x0.astype(np.float64)
+    for k in range(6):
+        o.iterate(1, 1.3, 0.0, 0.5)
+        x, nv = _dense_block_sweep(Dd, Ld, labels, bounds, x, float(F32(1.3)))
+        assert np.allclose(o.get_x(), x, rtol=1e-12, atol=1e-14)
+        assert o.sweep_stats()[1] == nv
+
+
+def test_pin14_single_block_equals_simultaneous_step():
+    """One structure, one kind => the block sweep IS the simultaneous (Cimmino) step of R1/R3: w^ = 1/|P|."""
+    D, L, labels, x0 = pg.random_small_plan(21, V=30, S=6, n_struct=1)
+    labels = np.where(labels > 0, 1, 0).astype(np.int32)
+    bounds = bounds_rows(dict(weight=1.0, dose_lo=0.9, dose_hi=1.0))
+    a = orc.Oracle.create(30, 6, D, L, labels, bounds)
+    b = orc.Oracle.create(30, 6, D, L, labels, bounds)
+    b.set_option(orc.OPT_BLOCK_SEQUENTIAL, 1)
+    a.set_x(x0); b.set_x(x0)
+    a.iterate(8, 1.5, 0.0, 0.5); b.iterate(8, 1.5, 0.0, 0.5)
+    assert np.allclose(a.get_x(), b.get_x(), rtol=1e-13, atol=1e-15)
+
+
+def test_pin15_one_voxel_blocks_equal_the_sequential_listing():
+    """Every structure holds one voxel => a block is one row and the sweep is Fig. 2 read literally (oracle_sequential_sweep)."""
+    rng = np.random.default_rng(5)
+    V, S = 6, 5
+    Dd = f32mat(rng.uniform(0.1, 1.0, (V, S)))
+    Ld = f32mat(Dd * rng.uniform(2.0, 6.0, (V, S)))
+    labels = np.arange(1, V + 1, dtype=np.int32)
+    bounds = bounds_rows(*[dict(weight=1.0, dose_lo=0.5, dose_hi=0.9, dl_hi=2.0, letd_max=3.0) for _ in range(V)])
+    a, b = make_oracle(Dd, Ld, labels, bounds), make_oracle(Dd, Ld, labels, bounds)
+    x0 = rng.uniform(0.2, 1.0, S).astype(F32)
+    a.set_x(x0); b.set_x(x0)
+    b.set_option(orc.OPT_BLOCK_SEQUENTIAL, 1)
+    for _ in range(5):
+        a.sequential_sweep(1.0)
+        b.iterate(1, 1.0, 0.0, 0.5)
+        assert np.allclose(a.get_x(), b.get_x(), rtol=1e-13, atol=1e-15)
+
+
+def test_pin16_block_sequential_is_fejer_monotone_and_reaches_feasibility():
+    """Sequential relaxed projections (lambda in (0,2)) never move away from a feasible point, and converge to the set."""
+    rng = np.random.default_rng(9)
+    V, S = 40, 8
+    Dd = f32mat(rng.uniform(0.0, 1.0, (V, S)) * (rng.uniform(size=(V, S)) < 0.6))
+    Ld = f32mat(Dd * rng.uniform(2.0, 8.0, (V, S)))
+    xs = rng.uniform(0.2, 1.0, S)
+    labels = (np.arange(V) % 3 + 1).astype(np.int32)
+    d, l = Dd @ xs, Ld @ xs
+    bounds = bounds_rows(dict(weight=1.0, dose_lo=float(d[labels == 1].min()) * 0.98, dose_hi=float(d[labels == 1].max()) * 1.02),
+                         dict(weight=0.7, dose_hi=float(d[labels == 2].max()) * 1.02, dl_hi=float(l[labels == 2].max()) * 1.02),
+                         dict(weight=1.0, dl_lo=float(l[labels == 3].min()) * 0.98, dl_hi=float(l[labels == 3].max()) * 1.02,
+                              letd_max=float((l / np.maximum(d, 1e-9))[labels == 3].max()) * 1.05))
+    o = make_oracle(Dd, Ld, labels, bounds)
+    o.set_option(orc.OPT_BLOCK_SEQUENTIAL, 1)
+    for lam in (0.6, 1.0, 1.8):
+        o.set_option(orc.OPT_RESET, 1)
+        o.set_x((xs * rng.uniform(0.3, 2.0, S)).astype(F32))
+        dist = np.linalg.norm(o.get_x() - xs)
+        p0 = o.proximity(None)[0]
+        for _ in range(400):
+            o.iterate(1, lam, 0.0, 0.5)
+            dn = np.linalg.norm(o.get_x() - xs)
+            assert dn <= dist * (1 + 1e-12)
+            dist = dn
+        p, _ = o.proximity(None)
+        assert p0 > 1e-4 and p < 1e-6 * p0                  # asymptotic convergence to the feasible set
