@@ -100,6 +100,15 @@ typedef struct {
 #define FREDOPT_OPT_TIME_PASSES    6   /* 1: bracket every kernel of fredopt_iterate with CUDA events (implies no */
                                        /*    graph); read with fredopt_get_pass_times; default 0                  */
 
+#define FREDOPT_OPT_BLOCK_SEQUENTIAL 7 /* 1: the feasibility-seeking step follows the loop nest of Fig. 2             */
+                                       /*     block by block: sequential over (kind, structure)     */
+                                       /*    blocks -- dose kind over the structures, then cDLET, then LETd --        */
+                                       /*    simultaneous inside a block: x <- x - lambda eta^k min(w_s,1)/m *        */
+                                       /*    sum_{i in block} (r_i/|a_i|^2) a_i, m = rows of the block with a non-zero */
+                                       /*    norm; clamp after the last block.  fredopt_get_stats then reports the     */
+                                       /*    sets found violated when visited and their proximity share.  Default 0:   */
+                                       /*    one simultaneous step over all sets (R1, R23)                   */
+
 /* Row selectors of the per-pass exports. */
 #define FREDOPT_ROWS_ALL     0
 #define FREDOPT_ROWS_ACTIVE  1

@@ -72,6 +72,12 @@ struct RowSet {
     int32_t* t_item_slot = nullptr;  // [t_n_items] slot of the item's partial sum
     long long* t_item_ptr = nullptr; // [S+1] partial-sum slots of spot j: t_item_ptr[j] .. t_item_ptr[j+1]-1
     double* t_partial = nullptr;     // [t_n_items]
+    // block-sequential AMS: the same items grouped by structure (longest first inside a structure) and the slot
+    // ranges per (spot, structure, 65536-row block)
+    Item* t_items_seg = nullptr;     // [t_n_items]
+    int32_t* t_slot_seg = nullptr;   // [t_n_items]
+    long long* t_slot_ptr = nullptr; // [S * n_seg * t_H + 1]
+    std::vector<long long> t_seg_item_begin;   // host: items of structure s are t_seg_item_begin[s] .. [s+1]-1
     RowList view() const { return RowList{n, start, len, seg, vox}; }
 };
 
@@ -108,14 +114,14 @@ struct fredopt_plan {
     // options / host state
     double eta = 1.0;
     long long reductionsN = 1, max_trials = 200;
-    int accept_check = 1, use_graph = 1, time_passes = 0;
+    int accept_check = 1, use_graph = 1, time_passes = 0, block_sequential = 0;
     bool started = false;
     float latched_beta0 = 0.f;
     long long launches = 0;
     // graphs: [0] = AMS iteration, [1] = SA iteration (for the current reductionsN)
-    cudaGraphExec_t gexec[2] = {nullptr, nullptr};
-    long long gexec_red[2] = {0, 0};
-    int gexec_kernels[2] = {0, 0};
+    cudaGraphExec_t gexec[4] = {nullptr, nullptr, nullptr, nullptr};   // index = 2 * block_sequential + (superiorized ? 1 : 0)
+    long long gexec_red[4] = {0, 0, 0, 0};
+    int gexec_kernels[4] = {0, 0, 0, 0};
     // timing
     std::vector<EventPair> events;
     double pass_ms[FREDOPT_N_PASSES] = {0};
@@ -341,9 +347,9 @@ __global__ void k_count_sets(long long n, const int32_t* seg, const int32_t* ule
         StructInfo& T = tab[seg[a]];
         const int f = T.flags;
         unsigned long long sets = 0, part = 0;
-        if (f & F_DOSE_SLAB) { ++sets; part += nD[a] > 0.0; }
-        if (f & F_DL_SLAB) { ++sets; part += nL[a] > 0.0; }
-        if (f & F_LETD) { ++sets; part += nT[a] > 0.0; }
+        if (f & F_DOSE_SLAB) { ++sets; part += nD[a] > 0.0; if (nD[a] > 0.0) atomicAdd(&T.part_kind[0], 1ULL); }
+        if (f & F_DL_SLAB) { ++sets; part += nL[a] > 0.0; if (nL[a] > 0.0) atomicAdd(&T.part_kind[1], 1ULL); }
+        if (f & F_LETD) { ++sets; part += nT[a] > 0.0; if (nT[a] > 0.0) atomicAdd(&T.part_kind[2], 1ULL); }
         atomicAdd(&T.n_sets, sets);
         atomicAdd(&T.part, part);
         atomicAdd(&T.n_zero, sets - part);
@@ -461,6 +467,14 @@ __global__ void k_tr_item_key(const Item* items, long long n, uint32_t* key, uin
     for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (long long)gridDim.x * blockDim.x) {
         key[i] = (uint32_t)((TR_ITEM_MAX - items[i].len) / 256);
         idx[i] = (uint32_t)i;
+    }
+}
+__global__ void k_tr_item_key_seg(const Item* items, long long n, uint32_t* key, uint32_t* idx, unsigned long long* hist) {
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (long long)gridDim.x * blockDim.x) {
+        const uint32_t sg = (uint32_t)(items[i].seg & 0xFF);
+        key[i] = sg * 16u + (uint32_t)((TR_ITEM_MAX - items[i].len) / 256);
+        idx[i] = (uint32_t)i;
+        atomicAdd(hist + sg, 1ULL);
     }
 }
 __global__ void k_tr_item_permute(const uint32_t* idx, long long n, const Item* items, const int32_t* js, Item* items2, int32_t* js2) {
@@ -590,7 +604,34 @@ static int build_transpose(fredopt_plan* P, RowSet& R) {
     k_tr_item_fill<<<grid_for(K, 256, 4096), 256, 0, st>>>(R.t_ptr, ustart, sbase, S, R.n_seg, H, R.t_items, R.t_item_slot);
     k_tr_item_ptr<<<grid_for(S + 1, 256, 4096), 256, 0, st>>>(sbase, S, (long long)R.n_seg * H, R.t_item_ptr);
     if (cudaGetLastError() != cudaSuccess || cudaStreamSynchronize(st) != cudaSuccess) { cleanup2(); return FREDOPT_CUDA_ERROR; }
-    cudaFree(cnt_sm); cudaFree(sbase);
+    cudaFree(cnt_sm);
+    R.t_slot_ptr = sbase;              // kept: slot ranges per (spot, structure, block) for the block-sequential sweep
+    P->allocs.push_back((void*)sbase);
+    // ---- the same items grouped by structure, longest first inside a structure (block-sequential AMS)
+    R.t_seg_item_begin.assign((size_t)R.n_seg + 1, 0);
+    if (R.t_n_items > 0) {
+        const long long ni = R.t_n_items;
+        uint32_t *ik = nullptr, *ik2 = nullptr, *ii = nullptr, *ii2 = nullptr;
+        unsigned long long* hist = nullptr; void* stmp = nullptr;
+        auto cleanup4 = [&]() { cudaFree(ik); cudaFree(ik2); cudaFree(ii); cudaFree(ii2); cudaFree(hist); cudaFree(stmp); cleanup(); };
+#define CK4(expr) do { cudaError_t e__ = (expr); if (e__ != cudaSuccess) { g_last_cuda_error = std::string(#expr) + ": " + cudaGetErrorString(e__); cudaGetLastError(); cleanup4(); return e__ == cudaErrorMemoryAllocation ? FREDOPT_OUT_OF_MEMORY : FREDOPT_CUDA_ERROR; } } while (0)
+        CK4(cudaMalloc(&ik, ni * 4)); CK4(cudaMalloc(&ik2, ni * 4)); CK4(cudaMalloc(&ii, ni * 4)); CK4(cudaMalloc(&ii2, ni * 4));
+        CK4(cudaMalloc(&hist, 256 * 8));
+        CK4(cudaMemsetAsync(hist, 0, 256 * 8, st));
+        if ((ret = dmalloc(P, &R.t_items_seg, (size_t)ni)) || (ret = dmalloc(P, &R.t_slot_seg, (size_t)ni))) { cleanup4(); return ret; }
+        k_tr_item_key_seg<<<grid_for(ni, 256, 4096), 256, 0, st>>>(R.t_items, ni, ik, ii, hist);
+        size_t sb = 0;
+        CK4(cub::DeviceRadixSort::SortPairs(nullptr, sb, ik, ik2, ii, ii2, ni, 0, 12, st));
+        CK4(cudaMalloc(&stmp, sb ? sb : 1));
+        CK4(cub::DeviceRadixSort::SortPairs(stmp, sb, ik, ik2, ii, ii2, ni, 0, 12, st));
+        k_tr_item_permute<<<grid_for(ni, 256, 4096), 256, 0, st>>>(ii2, ni, R.t_items, R.t_item_slot, R.t_items_seg, R.t_slot_seg);
+        unsigned long long hh[256];
+        CK4(cudaMemcpyAsync(hh, hist, 256 * 8, cudaMemcpyDeviceToHost, st));
+        CK4(cudaStreamSynchronize(st));
+#undef CK4
+        for (int sg = 0; sg < R.n_seg; ++sg) R.t_seg_item_begin[sg + 1] = R.t_seg_item_begin[sg] + (long long)hh[sg];
+        cudaFree(ik); cudaFree(ik2); cudaFree(ii); cudaFree(ii2); cudaFree(hist); cudaFree(stmp);
+    }
     // ---- longest items first: with the static round-robin mapping every round of the grid then holds items of
     //      one length class, so the warps stay balanced to within one class width per round
     if (R.t_n_items > 1) {
@@ -735,6 +776,58 @@ static void launch_finalize(fredopt_plan* P) {
     ++P->launches;
 }
 
+// Block-sequential AMS sweep (reading R23): Fig. 2's loop nest -- dose kind over the structures, then cDLET, then the LETd
+// rows -- one (forward over the block's rows, residual, transposed over the block's items, update) group per block.
+static void enqueue_block_sweep(fredopt_plan* P) {
+    const RowSet& A = P->act;
+    k_sweep_begin<<<1, 1, 0, P->stream>>>(P->st);
+    ++P->launches;
+    std::vector<long long> row_begin((size_t)P->n_struct + 1, 0);
+    for (int s = 0; s < P->n_struct; ++s) row_begin[s + 1] = row_begin[s] + (long long)P->h_tab[s].rows;
+    const int kind_flag[3] = {F_DOSE_SLAB, F_DL_SLAB, F_LETD};
+    const int kind_mode[3] = {1, 2, 3};
+    const GatherVec none{nullptr, nullptr, nullptr};
+    for (int kind = 0; kind < 3; ++kind)
+        for (int s = 0; s < P->n_struct; ++s) {
+            const StructInfo& T = P->h_tab[s];
+            if (!(T.flags & kind_flag[kind])) continue;
+            const long long rb = row_begin[s], re = row_begin[s + 1], nr = re - rb;
+            if (nr == 0) continue;
+            const uint8_t* md = P->mode_fixed + (size_t)kind_mode[kind] * P->max_seg;
+            ev_begin(P, FREDOPT_PASS_FORWARD_X);
+            {
+                const int g = fwd_grid(P, nr);
+                if (A.col16) k_forward<EPI_STORE, true><<<g, FWD_THREADS, 0, P->stream>>>(nr, A.items + rb, A.vox + rb, md, A.col16, A.valD, A.valL, P->x, P->d + rb, P->l + rb, none, nullptr, nullptr, nullptr, nullptr, 0);
+                else k_forward<EPI_STORE, false><<<g, FWD_THREADS, 0, P->stream>>>(nr, A.items + rb, A.vox + rb, md, A.col, A.valD, A.valL, P->x, P->d + rb, P->l + rb, none, nullptr, nullptr, nullptr, nullptr, 0);
+                ++P->launches;
+            }
+            ev_end(P);
+            ev_begin(P, FREDOPT_PASS_RESIDUAL);
+            const int gr = grid_for(nr, ROW_THREADS, P->sm_count * 4 < MAX_PARTIALS ? P->sm_count * 4 : MAX_PARTIALS);
+            k_block_residual<<<gr, ROW_THREADS, 0, P->stream>>>(rb, re, s, kind, P->tab, P->st, P->d, P->l, P->nD, P->nL, P->nT, P->uv,
+                                                               P->part_prox);
+            ++P->launches;
+            ev_end(P);
+            const long long m = (long long)T.part_kind[kind];
+            const long long ib = A.t_seg_item_begin.empty() ? 0 : A.t_seg_item_begin[s], ie = A.t_seg_item_begin.empty() ? 0 : A.t_seg_item_begin[s + 1];
+            if (m == 0) continue;                      // no row of the block has a non-zero norm: violations counted, no step
+            ev_begin(P, FREDOPT_PASS_TRANSPOSE_B);
+            if (ie > ib) {
+                const int g = fwd_grid(P, ie - ib);
+                if (A.t_col16) k_transpose<true><<<g, FWD_THREADS, 0, P->stream>>>(ie - ib, A.t_items_seg + ib, A.t_slot_seg + ib, md, A.t_col16, A.t_valD, A.t_valL, P->uv, A.t_partial);
+                else k_transpose<false><<<g, FWD_THREADS, 0, P->stream>>>(ie - ib, A.t_items_seg + ib, A.t_slot_seg + ib, md, A.t_col, A.t_valD, A.t_valL, P->uv, A.t_partial);
+                ++P->launches;
+            }
+            const double factor = (T.w < 1.0 ? T.w : 1.0) / (double)m;
+            k_combine_block<<<grid_for(P->S, 256, 1 << 30), 256, 0, P->stream>>>(P->S, A.t_slot_ptr, s, A.n_seg, A.t_H, A.t_partial, P->x, P->st,
+                                                                                 factor, P->part_prox, gr);
+            ++P->launches;
+            ev_end(P);
+        }
+    k_sweep_end<<<grid_for(P->S, 256, 1 << 30), 256, 0, P->stream>>>(P->S, P->x, P->st);
+    ++P->launches;
+}
+
 // one iteration of Fig. 3 around the simultaneous Fig. 2 step; returns the number of kernels enqueued
 static int enqueue_iteration(fredopt_plan* P, bool sa) {
     const long long before = P->launches;
@@ -754,17 +847,21 @@ static int enqueue_iteration(fredopt_plan* P, bool sa) {
             ++P->launches;
             ev_end(P);
             ev_begin(P, FREDOPT_PASS_RESIDUAL);
-            const int last = t == P->reductionsN - 1;
+            const int last = t == P->reductionsN - 1 && !P->block_sequential;
             launch_residual(P, P->d, P->l, 1, last, last);                                             // x', d', l'; a7
             ev_end(P);
         }
-    } else {
+    } else if (!P->block_sequential) {
         ev_begin(P, FREDOPT_PASS_FORWARD_X);
         launch_forward(P, P->act, P->mode_con, P->x, P->d, P->l, EPI_STORE);
         ev_end(P);
         ev_begin(P, FREDOPT_PASS_RESIDUAL);
         launch_residual(P, P->d, P->l, 0, 1, 1);
         ev_end(P);
+    }
+    if (P->block_sequential) {
+        enqueue_block_sweep(P);
+        return (int)(P->launches - before);
     }
     ev_begin(P, FREDOPT_PASS_TRANSPOSE_B);
     launch_transpose<TEPI_UPDATE>(P, P->act, P->mode_con, P->uv, nullptr, P->x, nullptr);              // a8, a9
@@ -792,7 +889,7 @@ void fredopt_destroy(fredopt_plan* P) {
     if (!P) return;
     cudaStreamSynchronize(P->stream);
     for (auto& ep : P->events) { cudaEventDestroy(ep.a); cudaEventDestroy(ep.b); }
-    for (int i = 0; i < 2; ++i) if (P->gexec[i]) cudaGraphExecDestroy(P->gexec[i]);
+    for (int i = 0; i < 4; ++i) if (P->gexec[i]) cudaGraphExecDestroy(P->gexec[i]);
     for (void* p : P->allocs) cudaFree(p);
     if (P->owns_stream) cudaStreamDestroy(P->stream);
     delete P;
@@ -1036,6 +1133,7 @@ int fredopt_create(const fredopt_csr* D, const fredopt_csr* L, const int32_t* vo
     if (!out) return FREDOPT_INVALID_ARG;
     *out = nullptr;
     if (!D || !L || n_struct < 0 || (n_struct > 0 && !bounds)) return FREDOPT_INVALID_ARG;
+    if (n_struct > 255) return FREDOPT_UNSUPPORTED;          // work items carry the structure in 8 bits
     if (D->n_rows != L->n_rows || D->n_cols != L->n_cols || D->n_rows < 0 || D->n_cols < 0 || D->nnz < 0 || L->nnz < 0)
         return FREDOPT_INVALID_ARG;
     if (D->n_rows >= (1LL << 31) - 1 || D->n_cols >= (1LL << 31) - 1 || D->nnz >= (1LL << 32) || L->nnz >= (1LL << 32))
@@ -1247,6 +1345,7 @@ int fredopt_set_option(fredopt_plan* P, int32_t key, double value) {
             break;
         }
         case FREDOPT_OPT_USE_GRAPH: P->use_graph = value != 0.0; break;
+        case FREDOPT_OPT_BLOCK_SEQUENTIAL: P->block_sequential = value != 0.0; break;
         case FREDOPT_OPT_TIME_PASSES:
             P->time_passes = value != 0.0;
             if (P->time_passes) {
@@ -1272,7 +1371,7 @@ int fredopt_iterate(fredopt_plan* P, int32_t n_iter, float lambda, float beta0, 
     if (n_iter > 0) {
         const bool graph = P->use_graph && !P->time_passes && n_iter > 1;
         if (graph) {
-            const int gi = sa ? 1 : 0;
+            const int gi = 2 * P->block_sequential + (sa ? 1 : 0);
             if (!P->gexec[gi] || P->gexec_red[gi] != P->reductionsN) {
                 if (P->gexec[gi]) { cudaGraphExecDestroy(P->gexec[gi]); P->gexec[gi] = nullptr; }
                 cudaGraph_t gr = nullptr;
@@ -1293,7 +1392,7 @@ int fredopt_iterate(fredopt_plan* P, int32_t n_iter, float lambda, float beta0, 
         } else {
             for (int it = 0; it < n_iter; ++it) enqueue_iteration(P, sa);
         }
-        launch_finalize(P);
+        if (!P->block_sequential) launch_finalize(P);     // block mode keeps its sweep statistics in the state already
     }
     CK(cudaGetLastError());
     return FREDOPT_OK;

@@ -35,6 +35,7 @@ struct StructInfo {
     double dose_lo, dose_hi, dl_lo, dl_hi, letd_max, dose_ref, dl_ref;
     int flags, pad;
     unsigned long long part, n_sets, n_zero, rows, nnz;   // participating sets, declared sets, zero-norm sets, rows, nnz
+    unsigned long long part_kind[3];                      // participating sets per kind: dose slab, cDL slab, LETd
 };
 
 struct DevState {
@@ -515,6 +516,78 @@ k_residual(long long n, const Item* __restrict__ items, const StructInfo* __rest
             }
         }
     }
+}
+
+// ------------------------------------------------------------------------------------------ block-sequential AMS (R23)
+// Residual pass of ONE (kind, structure) block over its rows [rb, re) of the labelled list, at the x the block starts
+// from: coefficient c_i = r_i / |a_i|^2 (0 where the norm is 0) into the gather vector (kind 0: D; 1: L; 2: L - LETmax D),
+// the block's violated sets (integer atomics: order-independent) and partial sums of its proximity share.
+__global__ void __launch_bounds__(ROW_THREADS)
+k_block_residual(long long rb, long long re, int seg, int kind, const StructInfo* __restrict__ tab, DevState* st,
+                 const double* __restrict__ d, const double* __restrict__ l, const double* __restrict__ nD,
+                 const double* __restrict__ nL, const double* __restrict__ nT, const GatherVec uv,
+                 double* __restrict__ part_prox) {
+    __shared__ double sm[ROW_THREADS / 32];
+    __shared__ unsigned long long smc[ROW_THREADS / 32];
+    const StructInfo& T = tab[seg];
+    const double w = T.what;
+    double prox = 0.0;
+    unsigned long long cnt = 0;
+    for (long long a = rb + (long long)blockIdx.x * blockDim.x + threadIdx.x; a < re; a += (long long)gridDim.x * blockDim.x) {
+        double r, nn;
+        if (kind == 0) { r = slab_residual(d[a], T.dose_lo, T.dose_hi); nn = nD[a]; }
+        else if (kind == 1) { r = slab_residual(l[a], T.dl_lo, T.dl_hi); nn = nL[a]; }
+        else { const double val = l[a] - T.letd_max * d[a]; r = val > 0.0 ? val : 0.0; nn = nT[a]; }
+        if (r != 0.0) ++cnt;
+        double c = 0.0;
+        if (nn > 0.0 && r != 0.0) { c = r / nn; prox += 0.5 * w * r * r / nn; }
+        if (kind == 0) gv_store(uv, a, c, 0.0);
+        else if (kind == 1) gv_store(uv, a, 0.0, c);
+        else gv_store(uv, a, -T.letd_max * c, c);
+    }
+    const double p = block_sum(prox, sm);
+    for (int o = 16; o > 0; o >>= 1) cnt += __shfl_down_sync(0xffffffffu, cnt, o);
+    __syncthreads();
+    if ((threadIdx.x & 31) == 0) smc[threadIdx.x >> 5] = cnt;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        unsigned long long t = 0;
+        for (int i = 0; i < ROW_THREADS / 32; ++i) t += smc[i];
+        part_prox[blockIdx.x] = p;
+        if (t) atomicAdd((unsigned long long*)&st->n_viol, t);
+    }
+}
+
+// Second stage of a block's transposed pass: x_j <- x_j - lambda eta^k min(w_s, 1) / m * (sum of the block's slots of
+// spot j); block 0 also adds the block's proximity share (fixed order) to the sweep statistics.
+__global__ void __launch_bounds__(256)
+k_combine_block(long long S, const long long* __restrict__ slot_ptr, int seg, int n_seg, int H,
+                const double* __restrict__ partial, double* __restrict__ x, DevState* st, double factor,
+                const double* __restrict__ part_prox, int n_part) {
+    if (blockIdx.x == 0 && threadIdx.x < 32) {
+        double p = 0.0;
+        for (int i = threadIdx.x; i < n_part; i += 32) p += part_prox[i];
+        p = warp_sum(p);
+        if (threadIdx.x == 0) st->prox += p;
+    }
+    const long long j = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (j >= S) return;
+    const long long ib = slot_ptr[(j * n_seg + seg) * H], ie = slot_ptr[(j * n_seg + seg + 1) * H];
+    if (ib == ie) return;
+    double tot = 0.0;
+    for (long long i = ib; i < ie; ++i) tot += partial[i];
+    x[j] -= st->lambda * st->eta_pow * factor * tot;
+}
+
+// Start of a block-sequential sweep: the sweep statistics restart.
+__global__ void k_sweep_begin(DevState* st) { st->prox = 0.0; st->n_viol = 0; }
+
+// End of a block-sequential sweep: clamp, w_{k+1} = eta * w_k, k <- k + 1.
+__global__ void __launch_bounds__(256)
+k_sweep_end(long long S, double* __restrict__ x, DevState* st) {
+    const long long j = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (j < S && x[j] < 0.0) x[j] = 0.0;
+    if (j == 0) { st->relax = st->lambda * st->eta_pow; st->eta_pow *= st->eta; st->k += 1; }
 }
 
 __global__ void __launch_bounds__(1024)

@@ -299,6 +299,62 @@ def test_invalid_arguments(fredopt):
         gp.set_option(99, 1.0)
 
 
+# ------------------------------------------------------------------------------------------ block-sequential AMS (R23)
+def _assert_block_state(gp, orc):
+    po, no = orc.sweep_stats()
+    sg = gp.stats()                      # before _assert_state: fredopt_proximity overwrites these two statistics
+    assert sg["n_violated"] == no, f"sets violated when visited: {sg['n_violated']} vs oracle {no}"
+    assert abs(sg["prox"] - po) <= 1e-9 * abs(po) + 1e-300
+    _assert_state(gp, orc)
+
+
+@pytest.mark.parametrize("beta0", [0.0, 1.0])
+@pytest.mark.parametrize("lam", [1.0, 1.7])
+def test_block_sequential_config0(fredopt, plan0, beta0, lam):
+    """Fig. 2's loop nest block by block (option BLOCK_SEQUENTIAL), pure and superiorized, 20 iterations."""
+    from oracle import oracle as om
+    gp = fredopt.from_plan(plan0); orc = _oracle(plan0)
+    gp.set_option(fredopt.OPT_BLOCK_SEQUENTIAL, 1); orc.set_option(om.OPT_BLOCK_SEQUENTIAL, 1)
+    gp.set_weights(plan0.x0); orc.set_x(plan0.x0)
+    for n in (1, 19):                                          # one plain launch sequence, then graph replays
+        gp.iterate(n, lam, beta0, 0.99); orc.iterate(n, lam, beta0, 0.99)
+        _assert_block_state(gp, orc)
+    # and back to the simultaneous step on the same plan
+    gp.set_option(fredopt.OPT_BLOCK_SEQUENTIAL, 0); orc.set_option(om.OPT_BLOCK_SEQUENTIAL, 0)
+    gp.iterate(3, lam, beta0, 0.99); orc.iterate(3, lam, beta0, 0.99)
+    _assert_state(gp, orc)
+
+
+@pytest.mark.parametrize("seed,same", [(3, True), (4, False)])
+def test_block_sequential_random_small_plans(fredopt, seed, same):
+    from oracle import oracle as om
+    V, S = 300, 37
+    D, L, lab, x0 = pg.random_small_plan(seed, V=V, S=S, n_struct=4, density=0.3, same_pattern=same)
+    nan = np.nan
+    bounds = np.array([[1.0, 0.5, 0.9, nan, nan, nan, 0.7, nan],
+                       [2.0, nan, 0.4, nan, 1.5, 3.0, nan, 1.5],
+                       [0.5, 0.1, nan, 0.2, 2.0, nan, 0.3, 1.0],
+                       [0.25, nan, nan, nan, nan, 2.5, nan, nan]], np.float32)
+    orc = _oracle_np(V, S, D, L, lab, bounds)
+    gp = fredopt.Plan(V, S, D, L, lab, bounds)
+    gp.set_option(fredopt.OPT_BLOCK_SEQUENTIAL, 1); orc.set_option(om.OPT_BLOCK_SEQUENTIAL, 1)
+    gp.set_option(fredopt.OPT_ETA, 0.97); orc.set_option(om.OPT_ETA, 0.97)
+    orc.set_x(x0); gp.set_weights(x0)
+    orc.iterate(20, 1.5, 0.5, 0.8); gp.iterate(20, 1.5, 0.5, 0.8)
+    _assert_block_state(gp, orc)
+
+
+def test_block_sequential_three_beam_plan(fredopt):
+    """A scaled configs[2] plan (three beams, four structures, all three kinds): 20 superiorized block-sequential iterations."""
+    from oracle import oracle as om
+    plan = pg.build_plan(pg.config_spec(2, scale=0.25), device="cuda")
+    gp = fredopt.from_plan(plan, stream=torch.cuda.current_stream().cuda_stream); orc = _oracle(plan)
+    gp.set_option(fredopt.OPT_BLOCK_SEQUENTIAL, 1); orc.set_option(om.OPT_BLOCK_SEQUENTIAL, 1)
+    gp.set_weights(plan.x0); orc.set_x(plan.x0)
+    gp.iterate(20, 1.0, 1.0, 0.99); orc.iterate(20, 1.0, 1.0, 0.99)
+    _assert_block_state(gp, orc)
+
+
 # ------------------------------------------------------------------------------------------ full-size configurations
 def _full_size_parity(fredopt, plan, n_sample_rows):
     """20 superiorized iterations in the launch configuration bench.py times (one fredopt_iterate call = graph replay),
