@@ -176,6 +176,8 @@ def run_ours(args):
     gp = fredopt.from_plan(plan, stream=stream.cuda_stream)
     torch.cuda.synchronize()
     t_create = time.perf_counter() - t0
+    if args.block_sequential:
+        gp.set_option(fredopt.OPT_BLOCK_SEQUENTIAL, 1)
     st0 = gp.stats()
     K, W = args.steps, args.warmup
     lam, beta0, a = spec.lam, spec.beta0, spec.a
@@ -266,6 +268,7 @@ def run_ours(args):
         "config": {"workload": f"configs[{args.config}] {spec.name}", "n_voxels": plan.n_rows, "n_spots": plan.n_cols,
                    "nnz_per_matrix": plan.nnz, "nnz_active": stats["nnz_active"], "n_active_rows": stats["n_active_rows"],
                    "n_sets": stats["n_sets"], "lambda": lam, "beta0": beta0, "a": a,
+                   "ams_form": "block-sequential (Fig. 2 loop nest, R23)" if args.block_sequential else "simultaneous (R1)",
                    "passes_per_iteration": 4, "alg_bytes_per_iteration": iter_bytes,
                    "l2": ("L2-resident working set (%.1f MB < 2 x L2): L2 flushed once before the timed region; "
                           "HBM fraction not meaningful" % (iter_bytes / 1e6)) if flush is not None else
@@ -403,6 +406,8 @@ def main():
     ap.add_argument("--config", type=int, default=DEFAULT_CONFIG)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--block-sequential", action="store_true",
+                    help="feasibility-seeking step in the block-sequential form of Fig. 2's loop nest (DESIGN.md R23)")
     ap.add_argument("--sweep", action="store_true", help="BASELINE.json configs[4]: isolated-pass sweep (1 GPU)")
     ap.add_argument("--quick", action="store_true", help="with --sweep: two points only")
     args = ap.parse_args()
