@@ -41,8 +41,8 @@ DEFAULT_STEPS = {0: 50, 1: 200, 2: 100, 3: 50}
 NOMINAL_HBM_GBS = 8000.0    # north_star's "~8 TB/s peak" (context; the roofline denominator is the measured copy figure)
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel from the committed `ncu --set full`
 # capture (profiles/r01_ncu_full_config3.md); keyed by (config, pass); a transposed pass = k_transpose + k_combine
-NCU_TRAFFIC = {(3, "forward_x"): 1246998776, (3, "transpose_g"): 1192556112, (3, "forward_g"): 1247750520,
-               (3, "transpose_b"): 1261692064}
+NCU_TRAFFIC = {(3, "forward_x"): 955060480, (3, "transpose_g"): 902283776, (3, "forward_g"): 952695296,
+               (3, "transpose_b"): 970808832}
 
 
 def _peaks():
