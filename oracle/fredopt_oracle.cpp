@@ -64,6 +64,8 @@ struct Plan {
     double eta = 1.0;
     int64_t reductionsN = 1, max_trials = 200;
     bool accept_check = true;
+    bool normalize_grad = false;       // reading R9 option: step along g / |g|_2
+    bool one_sided_cost = false;       // reading R11 option: OAR term (cDL - cDLref)_+^2
     bool block_sequential = false;     // reading R23: Fig. 2's loop nest, sequential over (kind, ROI) blocks
     double sweep_prox = 0.0;           // statistics of the last block-sequential sweep (at visit time)
     int64_t sweep_viol = 0;
@@ -143,7 +145,8 @@ double cost(const Plan& P, const std::vector<double>& x) {
         if (s == 0) continue;
         const Bounds& b = P.bounds[s - 1];
         if (present(b.dose_ref)) { double e = b.dose_ref - row_dot(P.D, i, x); phi += P.what[s - 1] * e * e; }
-        if (present(b.dl_ref))   { double e = b.dl_ref - row_dot(P.L, i, x);   phi += P.what[s - 1] * e * e; }
+        if (present(b.dl_ref))   { double e = b.dl_ref - row_dot(P.L, i, x);
+                                   if (!(P.one_sided_cost && e > 0.0)) phi += P.what[s - 1] * e * e; }   // one-sided: only cDL above cDLref
     }
     return phi;
 }
@@ -161,6 +164,7 @@ void grad_cost(const Plan& P, const std::vector<double>& x, std::vector<double>&
         }
         if (present(b.dl_ref)) {
             double c = 2.0 * P.what[s - 1] * (row_dot(P.L, i, x) - b.dl_ref);
+            if (P.one_sided_cost && c < 0.0) c = 0.0;
             for (int64_t p = P.L.ptr[i]; p < P.L.ptr[i + 1]; ++p) g[P.L.col[p]] += c * P.L.val[p];
         }
     }
@@ -295,7 +299,7 @@ void oracle_set_x(void* h, const float* x) { Plan* P = (Plan*)h; for (size_t j =
 void oracle_set_x64(void* h, const double* x) { Plan* P = (Plan*)h; P->x.assign(x, x + P->x.size()); }
 void oracle_get_x(void* h, double* x) { Plan* P = (Plan*)h; std::memcpy(x, P->x.data(), P->x.size() * sizeof(double)); }
 
-// keys: 0 eta, 1 reductionsN, 2 accept_check, 3 max_trials, 4 reset (k, s, beta), 7 block-sequential AMS (R23)
+// keys: 0 eta, 1 reductionsN, 2 accept_check, 3 max_trials, 4 reset (k, s, beta), 7 block-sequential AMS (R23), 8 normalised gradient (R9), 9 one-sided cDL cost (R11)
 void oracle_set_option(void* h, int32_t key, double v) {
     Plan* P = (Plan*)h;
     switch (key) {
@@ -305,6 +309,8 @@ void oracle_set_option(void* h, int32_t key, double v) {
         case 3: P->max_trials = (int64_t)v; break;
         case 4: P->k = 0; P->s = 0; P->trials = 0; P->started = false; P->eta_pow = 1.0; P->last_beta = 0.0; break;
         case 7: P->block_sequential = v != 0.0; break;
+        case 8: P->normalize_grad = v != 0.0; break;
+        case 9: P->one_sided_cost = v != 0.0; break;
         default: break;
     }
 }
@@ -383,6 +389,12 @@ void oracle_iterate(void* h, int32_t n_iter, float lambda_f, float beta0_f, floa
                 bool zero = true;
                 for (int64_t j = 0; j < S; ++j) if (g[j] != 0.0) { zero = false; break; }
                 if (zero) break;                                              // R10: nothing to reduce
+                if (P->normalize_grad) {                                      // R9 option: unit direction g / |g|_2
+                    double n2 = 0.0;
+                    for (int64_t j = 0; j < S; ++j) n2 += g[j] * g[j];
+                    const double inv = 1.0 / std::sqrt(n2);
+                    for (int64_t j = 0; j < S; ++j) g[j] *= inv;
+                }
                 for (int64_t trial = 0; trial < P->max_trials; ++trial) {     // `while loop do`; R10 cap
                     const double beta = P->beta_next;                        // s = s + 1; beta = alpha^s (R8: beta0 * a^s)
                     P->beta_next *= a; ++P->s; ++P->trials;

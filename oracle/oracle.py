@@ -16,7 +16,7 @@ _SRC = os.path.join(_HERE, "fredopt_oracle.cpp")
 _LIB = os.path.join(_HERE, "libfredopt_oracle.so")
 
 OPT_ETA, OPT_REDUCTIONS, OPT_ACCEPT_CHECK, OPT_MAX_TRIALS, OPT_RESET = 0, 1, 2, 3, 4
-OPT_BLOCK_SEQUENTIAL = 7
+OPT_BLOCK_SEQUENTIAL, OPT_NORMALIZE_GRAD, OPT_ONE_SIDED_COST = 7, 8, 9
 
 
 def build(force: bool = False) -> str:

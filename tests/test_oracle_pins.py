@@ -594,3 +594,51 @@ def test_pin16_block_sequential_is_fejer_monotone_and_reaches_feasibility():
             dist = dn
         p, _ = o.proximity(None)
         assert p0 > 1e-4 and p < 1e-6 * p0                  # asymptotic convergence to the feasible set
+
+
+# ----------------------------------------------------------------------------- option variants of Fig. 3 / Eq. (2) (R9, R11)
+def _small_cost_plan():
+    D, L, labels, x0 = pg.random_small_plan(31, V=40, S=8, n_struct=2)
+    bounds = bounds_rows(dict(weight=1.0, dose_lo=0.6, dose_hi=1.0, dose_ref=0.8),
+                         dict(weight=1.5, dose_hi=0.7, dl_hi=2.0, dl_ref=1.2))
+    return D, L, labels, x0, bounds
+
+
+def test_pin17_one_sided_cost_and_its_gradient():
+    """(cDL - cDLref)_+^2: only rows above the reference contribute; gradient vs central differences; cost <= two-sided cost."""
+    D, L, labels, x0, _ = _small_cost_plan()
+    Dd, Ld = csr_to_dense(D, 8), csr_to_dense(L, 8)
+    lref = float(F32(np.median((Ld @ x0.astype(np.float64))[labels == 2])))     # some OAR rows above, some below
+    bounds = bounds_rows(dict(weight=1.0, dose_lo=0.6, dose_hi=1.0, dose_ref=0.8),
+                         dict(weight=1.5, dose_hi=0.7, dl_hi=2.0, dl_ref=lref))
+    ref = DenseReference(Dd, Ld, labels, bounds)
+    o = orc.Oracle.create(40, 8, D, L, labels, bounds)
+    two = o.cost(x0.astype(np.float64))
+    o.set_option(orc.OPT_ONE_SIDED_COST, 1)
+    x = x0.astype(np.float64)
+    # dense restatement
+    d, l = Dd @ x, Ld @ x
+    phi = sum(ref.what[0] * (float(F32(0.8)) - d[i]) ** 2 for i in range(40) if labels[i] == 1) + \
+        sum(ref.what[1] * max(l[i] - lref, 0.0) ** 2 for i in range(40) if labels[i] == 2)
+    assert abs(o.cost(x) - phi) <= 1e-13 * phi and o.cost(x) < two
+    assert any(l[i] < lref for i in range(40) if labels[i] == 2) and any(l[i] > lref for i in range(40) if labels[i] == 2)
+    g = o.grad(x)
+    for j in range(8):
+        e = np.zeros(8); e[j] = 1e-6
+        fd = (o.cost(x + e) - o.cost(x - e)) / 2e-6
+        assert abs(fd - g[j]) <= 1e-6 * max(1.0, abs(g[j]))
+
+
+def test_pin18_normalised_gradient_step_has_length_beta():
+    """R9 option: x' = x - beta g/|g|  =>  |x' - x|_2 = beta for the accepted beta (projection step switched off by a slack plan)."""
+    D, L, labels, x0, _ = _small_cost_plan()
+    bounds = bounds_rows(dict(weight=1.0, dose_hi=1e6, dose_ref=0.8), dict(weight=1.5, dose_hi=1e6, dl_ref=1.2))
+    o = orc.Oracle.create(40, 8, D, L, labels, bounds)
+    o.set_option(orc.OPT_NORMALIZE_GRAD, 1)
+    o.set_x(x0)
+    phi0 = o.cost(None)
+    o.iterate(1, 1.0, 0.25, 0.5)                      # nothing is violated: the AMS step is the identity, x stays >= 0
+    st = o.stats()
+    step = np.linalg.norm(o.get_x() - x0.astype(np.float64))
+    assert st["last_beta"] > 0 and abs(step - st["last_beta"]) <= 1e-14
+    assert o.cost(None) < phi0 and st["trials"] == st["s"] >= 1
