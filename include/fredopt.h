@@ -109,6 +109,11 @@ typedef struct {
                                        /*    sets found violated when visited and their proximity share.  Default 0:   */
                                        /*    one simultaneous step over all sets (R1, R23)                   */
 
+#define FREDOPT_OPT_NORMALIZE_GRAD   8 /* 1: the perturbation steps along grad chi^2 / |grad chi^2|_2 (Fig. 3 prints the  */
+                                       /*    un-normalised gradient: default 0; R9)             */
+#define FREDOPT_OPT_ONE_SIDED_COST   9 /* 1: the OAR term of Eq. (2) penalises only cDL above cDLref: w (cDL - cDLref)_+^2 */
+                                       /*    (Eq. (2) as printed is two-sided: default 0; R11)   */
+
 /* Row selectors of the per-pass exports. */
 #define FREDOPT_ROWS_ALL     0
 #define FREDOPT_ROWS_ACTIVE  1

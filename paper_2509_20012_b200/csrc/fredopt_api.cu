@@ -114,7 +114,7 @@ struct fredopt_plan {
     // options / host state
     double eta = 1.0;
     long long reductionsN = 1, max_trials = 200;
-    int accept_check = 1, use_graph = 1, time_passes = 0, block_sequential = 0;
+    int accept_check = 1, use_graph = 1, time_passes = 0, block_sequential = 0, normalize_grad = 0, one_sided_cost = 0;
     bool started = false;
     float latched_beta0 = 0.f;
     long long launches = 0;
@@ -728,7 +728,7 @@ static void launch_forward(fredopt_plan* P, const RowSet& R, const uint8_t* mode
     const GatherVec none{nullptr, nullptr, nullptr};
 #define FWD_LAUNCH(E, I16, COL, PQ, TAB, CP)                                                                                   \
     k_forward<E, I16><<<g, FWD_THREADS, 0, P->stream>>>(R.n, R.items, R.vox, mode, COL, R.valD, R.valL, x, oD, oL, PQ, TAB, CP, \
-                                                       nullptr, nullptr, 0)
+                                                       P->st, nullptr, nullptr, 0)
     if (R.col16) {
         if (epi == EPI_CPART) FWD_LAUNCH(EPI_CPART, true, R.col16, none, P->tab, P->cpart);
         else if (epi == EPI_STORE_PQ) FWD_LAUNCH(EPI_STORE_PQ, true, R.col16, P->pq, P->tab, nullptr);
@@ -797,8 +797,8 @@ static void enqueue_block_sweep(fredopt_plan* P) {
             ev_begin(P, FREDOPT_PASS_FORWARD_X);
             {
                 const int g = fwd_grid(P, nr);
-                if (A.col16) k_forward<EPI_STORE, true><<<g, FWD_THREADS, 0, P->stream>>>(nr, A.items + rb, A.vox + rb, md, A.col16, A.valD, A.valL, P->x, P->d + rb, P->l + rb, none, nullptr, nullptr, nullptr, nullptr, 0);
-                else k_forward<EPI_STORE, false><<<g, FWD_THREADS, 0, P->stream>>>(nr, A.items + rb, A.vox + rb, md, A.col, A.valD, A.valL, P->x, P->d + rb, P->l + rb, none, nullptr, nullptr, nullptr, nullptr, 0);
+                if (A.col16) k_forward<EPI_STORE, true><<<g, FWD_THREADS, 0, P->stream>>>(nr, A.items + rb, A.vox + rb, md, A.col16, A.valD, A.valL, P->x, P->d + rb, P->l + rb, none, nullptr, nullptr, nullptr, nullptr, nullptr, 0);
+                else k_forward<EPI_STORE, false><<<g, FWD_THREADS, 0, P->stream>>>(nr, A.items + rb, A.vox + rb, md, A.col, A.valD, A.valL, P->x, P->d + rb, P->l + rb, none, nullptr, nullptr, nullptr, nullptr, nullptr, 0);
                 ++P->launches;
             }
             ev_end(P);
@@ -843,7 +843,8 @@ static int enqueue_iteration(fredopt_plan* P, bool sa) {
             launch_forward(P, P->act, P->mode_union, P->g, P->Dg, P->Lg, EPI_CPART);                   // a5: Dg, Lg, c
             ev_end(P);
             ev_begin(P, FREDOPT_PASS_SELECT);
-            k_select<<<1, 1024, 0, P->stream>>>(P->st, P->g, P->S, P->cpart, cpart_count(P));          // a4, a6: beta
+            k_select<<<1, 1024, 0, P->stream>>>(P->st, P->g, P->S, P->cpart, cpart_count(P), P->act.n, P->act.items, P->tab, P->d, P->l,
+                                               P->Dg, P->Lg);                                             // a4, a6: beta
             ++P->launches;
             ev_end(P);
             ev_begin(P, FREDOPT_PASS_RESIDUAL);
@@ -1105,7 +1106,7 @@ static int create_impl(fredopt_plan* P, const fredopt_csr* D, const fredopt_csr*
         k_count_sets<<<grid_for(n_act, 256, 4096), 256, 0, st>>>(n_act, A.seg, A.ulen, P->nD, P->nL, P->nT, P->tab);
     }
     k_finish_tables<<<1, 1, 0, st>>>(P->tab, n_struct, P->st, P->mode_union, P->mode_con, P->mode_cost, P->mode_fixed, ns);
-    k_set_params<<<1, 1, 0, st>>>(P->st, 1.0, 0.0, 0.5, 1.0, 200, 1, 1);
+    k_set_params<<<1, 1, 0, st>>>(P->st, 1.0, 0.0, 0.5, 1.0, 200, 1, 0, 1);
     CK(cudaMemcpyAsync(P->h_tab.data(), P->tab, sizeof(StructInfo) * ns, cudaMemcpyDeviceToHost, st));
     CK(cudaStreamSynchronize(st));
     CK(cudaGetLastError());
@@ -1251,8 +1252,8 @@ static int forward_f32(fredopt_plan* P, const RowSet& R, int m, const double* xd
 #undef SHORT_LAUNCH
         }
         if (n_long) {
-            if (i16) k_forward<EPI_F32VOX, true><<<fwd_grid(P, n_long), FWD_THREADS, 0, P->stream>>>(n_long, R.items, R.vox, md, colp, R.valD, R.valL, xd, nullptr, nullptr, none, nullptr, nullptr, dd, dl, letd_out);
-            else k_forward<EPI_F32VOX, false><<<fwd_grid(P, n_long), FWD_THREADS, 0, P->stream>>>(n_long, R.items, R.vox, md, colp, R.valD, R.valL, xd, nullptr, nullptr, none, nullptr, nullptr, dd, dl, letd_out);
+            if (i16) k_forward<EPI_F32VOX, true><<<fwd_grid(P, n_long), FWD_THREADS, 0, P->stream>>>(n_long, R.items, R.vox, md, colp, R.valD, R.valL, xd, nullptr, nullptr, none, nullptr, nullptr, nullptr, dd, dl, letd_out);
+            else k_forward<EPI_F32VOX, false><<<fwd_grid(P, n_long), FWD_THREADS, 0, P->stream>>>(n_long, R.items, R.vox, md, colp, R.valD, R.valL, xd, nullptr, nullptr, none, nullptr, nullptr, nullptr, dd, dl, letd_out);
             ++P->launches;
         }
     }
@@ -1346,6 +1347,8 @@ int fredopt_set_option(fredopt_plan* P, int32_t key, double value) {
         }
         case FREDOPT_OPT_USE_GRAPH: P->use_graph = value != 0.0; break;
         case FREDOPT_OPT_BLOCK_SEQUENTIAL: P->block_sequential = value != 0.0; break;
+        case FREDOPT_OPT_NORMALIZE_GRAD: P->normalize_grad = value != 0.0; break;
+        case FREDOPT_OPT_ONE_SIDED_COST: P->one_sided_cost = value != 0.0; break;
         case FREDOPT_OPT_TIME_PASSES:
             P->time_passes = value != 0.0;
             if (P->time_passes) {
@@ -1365,11 +1368,12 @@ int fredopt_iterate(fredopt_plan* P, int32_t n_iter, float lambda, float beta0, 
         return FREDOPT_INVALID_ARG;
     const int latch = !P->started;
     if (latch) { P->latched_beta0 = beta0; P->started = true; }
-    k_set_params<<<1, 1, 0, P->stream>>>(P->st, (double)lambda, (double)beta0, (double)a, P->eta, P->max_trials, P->accept_check, latch);
+    k_set_params<<<1, 1, 0, P->stream>>>(P->st, (double)lambda, (double)beta0, (double)a, P->eta, P->max_trials, P->accept_check,
+                                           (P->normalize_grad ? SF_NORMALIZE_GRAD : 0) | (P->one_sided_cost ? SF_ONE_SIDED : 0), latch);
     ++P->launches;
     const bool sa = beta0 != 0.f;
     if (n_iter > 0) {
-        const bool graph = P->use_graph && !P->time_passes && n_iter > 1;
+        const bool graph = P->use_graph && !P->time_passes;
         if (graph) {
             const int gi = 2 * P->block_sequential + (sa ? 1 : 0);
             if (!P->gexec[gi] || P->gexec_red[gi] != P->reductionsN) {

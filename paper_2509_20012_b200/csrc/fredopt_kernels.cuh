@@ -29,6 +29,16 @@ constexpr int FWD_MIN_CTAS = 4;             // resident CTAs per SM the item ker
 
 // flags of a structure
 enum : int { F_DOSE_SLAB = 1, F_DL_SLAB = 2, F_LETD = 4, F_DOSE_REF = 8, F_DL_REF = 16 };
+enum : int { SF_NORMALIZE_GRAD = 1, SF_ONE_SIDED = 2 };
+
+struct DevState;
+// cost residuals of Eq. (2) at (d, l): p = 2 w^ (d - Dref), q = 2 w^ (l - cDLref) [one-sided: only where l > cDLref]
+__device__ __forceinline__ void cost_residuals(int f, double w, double dref, double lref, int one_sided, double dv, double lv,
+                                               double& p, double& q) {
+    p = (f & F_DOSE_REF) ? 2.0 * w * (dv - dref) : 0.0;
+    q = (f & F_DL_REF) ? 2.0 * w * (lv - lref) : 0.0;
+    if (one_sided && q < 0.0) q = 0.0;
+}
 
 struct StructInfo {
     double w, what;
@@ -44,7 +54,8 @@ struct DevState {
     double phi, prox, gg, c, W;
     long long k, s, trials, n_viol, max_trials;
     long long n_sets, n_zero;
-    int accept_check, pad;
+    int accept_check;
+    int flags;                 // bit 0: step along g/|g| (R9 option); bit 1: one-sided cDL cost (R11 option)
 };
 
 // One work item: `len` entries (multiple of 4) starting at entry `start` (multiple of 4) of the index / value
@@ -187,6 +198,7 @@ k_forward(long long n, const Item* __restrict__ items, const int32_t* __restrict
           double* __restrict__ oD, double* __restrict__ oL,                // EPI_STORE*, EPI_CPART: item-indexed
           const GatherVec pq,                                              // EPI_STORE_PQ: cost residuals (Eq. 2)
           const StructInfo* __restrict__ tab, double* __restrict__ cpart,  // EPI_STORE_PQ / EPI_CPART
+          const DevState* __restrict__ st,                                 // EPI_STORE_PQ (cost form)
           float* __restrict__ fD, float* __restrict__ fL, int letd_out)    // EPI_F32VOX: voxel-indexed
 {
     const int lane = threadIdx.x & 31;
@@ -216,8 +228,9 @@ k_forward(long long n, const Item* __restrict__ items, const int32_t* __restrict
                 oL[r] = aL;
                 if (EPI == EPI_STORE_PQ) {      // p_i = 2 w^ (d_i - Dref), q_i = 2 w^ (l_i - cDLref): grad chi^2 = D^T p + L^T q
                     const StructInfo& T = tab[it.seg];
-                    gv_store(pq, r, (T.flags & F_DOSE_REF) ? 2.0 * T.what * (aD - T.dose_ref) : 0.0,
-                             (T.flags & F_DL_REF) ? 2.0 * T.what * (aL - T.dl_ref) : 0.0);
+                    double pv, qv;
+                    cost_residuals(T.flags, T.what, T.dose_ref, T.dl_ref, st->flags & SF_ONE_SIDED, aD, aL, pv, qv);
+                    gv_store(pq, r, pv, qv);
                 }
                 if (EPI == EPI_CPART) {
                     const StructInfo& T = tab[it.seg];
@@ -391,7 +404,8 @@ k_combine(long long S, const long long* __restrict__ item_ptr, const double* __r
 
 // ------------------------------------------------------------------------------------------ scalar kernels
 __global__ void k_set_params(DevState* st, double lambda, double beta0, double a, double eta, long long max_trials,
-                             int accept_check, int latch) {
+                             int accept_check, int flags, int latch) {
+    st->flags = flags;
     st->lambda = lambda;
     st->eta = eta;
     st->max_trials = max_trials;
@@ -399,12 +413,34 @@ __global__ void k_set_params(DevState* st, double lambda, double beta0, double a
     if (latch) { st->beta0 = beta0; st->a = a; st->beta_next = beta0; st->eta_pow = 1.0; }
 }
 
-// |g|^2 and c by fixed-order sums, then the `while loop` of Fig. 3 on scalars:
-// chi^2(x - beta g) = chi^2(x) - beta |g|^2 + beta^2 c   =>   accept  <=>  beta c < |g|^2.
-// The accepted beta (0 if none) goes to st->beta_acc; k_residual applies it.  One CTA.
+// chi^2 of Eq. (2) at x - b g from the stored products: d - b Dg, l - b Lg (exact: the products are linear in x).  All
+// threads of the CTA take part; the value is valid in thread 0.
+__device__ __forceinline__ double cost_along(double b, long long n, const Item* __restrict__ items,
+                                             const StructInfo* __restrict__ tab, const double* __restrict__ d,
+                                             const double* __restrict__ l, const double* __restrict__ Dg,
+                                             const double* __restrict__ Lg, int one_sided, double* sm) {
+    double phi = 0.0;
+    for (long long a = threadIdx.x; a < n; a += blockDim.x) {
+        const StructInfo& T = tab[items[a].seg];
+        if (T.flags & F_DOSE_REF) { const double e = T.dose_ref - fma(-b, Dg[a], d[a]); phi += T.what * e * e; }
+        if (T.flags & F_DL_REF) { const double e = T.dl_ref - fma(-b, Lg[a], l[a]); if (!(one_sided && e > 0.0)) phi += T.what * e * e; }
+    }
+    return block_sum(phi, sm);
+}
+
+// |g|^2 and c by fixed-order sums, then the `while loop` of Fig. 3 on device scalars.  The step is
+// b = beta (or beta / |g| with the normalised-gradient option).  Two-sided cost (Eq. 2 as printed):
+//     chi^2(x - b g) = chi^2(x) - b |g|^2 + b^2 c   =>   accept  <=>  b c < |g|^2       (no pass per trial).
+// One-sided cost option: chi^2 is piecewise quadratic, so every trial evaluates chi^2(x - b g) from d - b Dg, l - b Lg
+// (a pass over the labelled rows' vectors, not over the matrix).  The accepted step (0 if none) goes to st->beta_acc;
+// k_residual applies it.  One CTA.
 __global__ void __launch_bounds__(1024)
-k_select(DevState* st, const double* __restrict__ g, long long S, const double* __restrict__ cpart, int n_part) {
+k_select(DevState* st, const double* __restrict__ g, long long S, const double* __restrict__ cpart, int n_part,
+         long long n, const Item* __restrict__ items, const StructInfo* __restrict__ tab, const double* __restrict__ d,
+         const double* __restrict__ l, const double* __restrict__ Dg, const double* __restrict__ Lg) {
     __shared__ double sm[32];
+    __shared__ double s_b;
+    __shared__ int s_go;
     double a0 = 0.0, a1 = 0.0, a2 = 0.0, a3 = 0.0;
     long long j = threadIdx.x;
     for (; j + 3 * 1024 < S; j += 4 * 1024) {       // 4 independent loads in flight; fixed order of addition
@@ -416,22 +452,54 @@ k_select(DevState* st, const double* __restrict__ g, long long S, const double* 
     double c = 0.0;
     for (int i = threadIdx.x; i < n_part; i += blockDim.x) c += cpart[i];
     const double cc = block_sum(c, sm);
-    if (threadIdx.x == 0) {
-        double acc = 0.0;
-        if (gg > 0.0) {                                        // g == 0: nothing to reduce (reading R10)
-            const double aa = st->a;
-            double bn = st->beta_next;
-            long long s = st->s, tr = st->trials;
-            const long long mt = st->max_trials;
-            const int chk = st->accept_check;
-            for (long long t = 0; t < mt; ++t) {
-                const double beta = bn;
-                bn *= aa; ++s; ++tr;
-                if (!chk || beta * cc < gg) { acc = beta; st->last_beta = beta; break; }
+    const int flags = st->flags;
+    if (!(flags & SF_ONE_SIDED)) {
+        if (threadIdx.x == 0) {
+            double acc = 0.0;
+            if (gg > 0.0) {                                        // g == 0: nothing to reduce (reading R10)
+                const double norm = (flags & SF_NORMALIZE_GRAD) ? sqrt(gg) : 1.0;
+                const double aa = st->a;
+                double bn = st->beta_next;
+                long long s = st->s, tr = st->trials;
+                const long long mt = st->max_trials;
+                const int chk = st->accept_check;
+                for (long long t = 0; t < mt; ++t) {
+                    const double beta = bn;
+                    bn *= aa; ++s; ++tr;
+                    const double b = beta / norm;
+                    if (!chk || b * cc < gg) { acc = b; st->last_beta = beta; break; }
+                }
+                st->beta_next = bn; st->s = s; st->trials = tr;
             }
-            st->beta_next = bn; st->s = s; st->trials = tr;
+            st->beta_acc = acc; st->gg = gg; st->c = cc;
         }
-        st->beta_acc = acc; st->gg = gg; st->c = cc;
+        return;
+    }
+    // ---- one-sided cost: literal trials on the stored products
+    if (threadIdx.x == 0) { s_go = gg > 0.0; st->gg = gg; st->c = cc; st->beta_acc = 0.0; }
+    __syncthreads();
+    if (!s_go) return;
+    const double phi0 = cost_along(0.0, n, items, tab, d, l, Dg, Lg, 1, sm);     // valid in thread 0
+    const long long mt = st->max_trials;
+    for (long long t = 0; t < mt; ++t) {
+        __syncthreads();
+        if (threadIdx.x == 0) {
+            const double beta = st->beta_next;
+            st->beta_next = beta * st->a; st->s += 1; st->trials += 1;
+            s_b = (flags & SF_NORMALIZE_GRAD) ? beta / sqrt(gg) : beta;
+        }
+        __syncthreads();
+        const double b = s_b;
+        double phi = 0.0;
+        const int chk = st->accept_check;
+        if (chk) phi = cost_along(b, n, items, tab, d, l, Dg, Lg, 1, sm);
+        if (threadIdx.x == 0) {
+            const int ok = !chk || phi < phi0;
+            if (ok) { st->beta_acc = b; st->last_beta = (flags & SF_NORMALIZE_GRAD) ? b * sqrt(gg) : b; }
+            s_go = !ok;
+        }
+        __syncthreads();
+        if (!s_go) break;
     }
 }
 
@@ -473,7 +541,9 @@ k_residual(long long n, const Item* __restrict__ items, const StructInfo* __rest
         const int f = T.flags;
         const double w = T.what;
         if (!final) {
-            gv_store(pq, a, (f & F_DOSE_REF) ? 2.0 * w * (dv - T.dose_ref) : 0.0, (f & F_DL_REF) ? 2.0 * w * (lv - T.dl_ref) : 0.0);
+            double pv, qv;
+            cost_residuals(f, w, T.dose_ref, T.dl_ref, st->flags & SF_ONE_SIDED, dv, lv, pv, qv);
+            gv_store(pq, a, pv, qv);
             continue;
         }
         double cD = 0.0, cL = 0.0, cT = 0.0;
@@ -490,7 +560,7 @@ k_residual(long long n, const Item* __restrict__ items, const StructInfo* __rest
             if (val > 0.0) { ++cnt; const double nn = nT[a]; if (nn > 0.0) { cT = w * val / nn; prox += 0.5 * w * val * val / nn; } }
         }
         if (f & F_DOSE_REF) { const double e = T.dose_ref - dv; phi += w * e * e; }
-        if (f & F_DL_REF) { const double e = T.dl_ref - lv; phi += w * e * e; }
+        if (f & F_DL_REF) { const double e = T.dl_ref - lv; if (!((st->flags & SF_ONE_SIDED) && e > 0.0)) phi += w * e * e; }
         if (write_uv) {
             gv_store(uv, a, (f & F_LETD) ? cD - T.letd_max * cT : cD,      // row of the LETd set is L_i - LETmax D_i
                      cL + cT);

@@ -17,7 +17,7 @@ LIB_PATH = os.path.join(_HERE, "libfredopt.so")
 
 OK, INVALID_ARG, OUT_OF_MEMORY, CUDA_ERROR, UNSUPPORTED_ARCH, UNSUPPORTED = 0, -1, -2, -3, -4, -5
 OPT_ETA, OPT_REDUCTIONS, OPT_ACCEPT_CHECK, OPT_MAX_TRIALS, OPT_RESET, OPT_USE_GRAPH, OPT_TIME_PASSES, \
-    OPT_BLOCK_SEQUENTIAL = range(8)
+    OPT_BLOCK_SEQUENTIAL, OPT_NORMALIZE_GRAD, OPT_ONE_SIDED_COST = range(10)
 ROWS_ALL, ROWS_ACTIVE = 0, 1
 PASS_NAMES = ("forward_x", "transpose_g", "forward_g", "select", "residual", "transpose_b")
 N_PASSES = len(PASS_NAMES)

@@ -299,6 +299,37 @@ def test_invalid_arguments(fredopt):
         gp.set_option(99, 1.0)
 
 
+# ------------------------------------------------------------------------------------------ options of Fig. 3 / Eq. (2)
+@pytest.mark.parametrize("norm,one_sided", [(1, 0), (0, 1), (1, 1)])
+def test_options_normalised_gradient_and_one_sided_cost(fredopt, norm, one_sided):
+    """R9 / R11 options on a plan with both cost terms; the one-sided accept loop runs its trials on the stored products."""
+    from oracle import oracle as om
+    V, S = 300, 37
+    D, L, lab, x0 = pg.random_small_plan(8, V=V, S=S, n_struct=3, density=0.3)
+    nan = np.nan
+    bounds = np.array([[1.0, 0.5, 0.9, nan, nan, nan, 0.7, nan],
+                       [2.0, nan, 0.4, nan, 1.5, 3.0, nan, 1.0],
+                       [0.5, 0.1, nan, 0.2, 2.0, nan, 0.3, 0.8]], np.float32)
+    orc = _oracle_np(V, S, D, L, lab, bounds)
+    gp = fredopt.Plan(V, S, D, L, lab, bounds)
+    for g_, o_, v in ((fredopt.OPT_NORMALIZE_GRAD, om.OPT_NORMALIZE_GRAD, norm), (fredopt.OPT_ONE_SIDED_COST, om.OPT_ONE_SIDED_COST, one_sided)):
+        gp.set_option(g_, v); orc.set_option(o_, v)
+    orc.set_x(x0); gp.set_weights(x0)
+    orc.iterate(20, 1.2, 2.0, 0.7); gp.iterate(20, 1.2, 2.0, 0.7)       # beta0 = 2: the first trials are rejected
+    assert orc.stats()["trials"] > 20
+    _assert_state(gp, orc)
+
+
+def test_options_on_three_beam_plan(fredopt):
+    from oracle import oracle as om
+    plan = pg.build_plan(pg.config_spec(2, scale=0.25), device="cuda")
+    gp = fredopt.from_plan(plan, stream=torch.cuda.current_stream().cuda_stream); orc = _oracle(plan)
+    gp.set_option(fredopt.OPT_ONE_SIDED_COST, 1); orc.set_option(om.OPT_ONE_SIDED_COST, 1)
+    gp.set_weights(plan.x0); orc.set_x(plan.x0)
+    gp.iterate(20, 1.0, 1.0, 0.99); orc.iterate(20, 1.0, 1.0, 0.99)
+    _assert_state(gp, orc)
+
+
 # ------------------------------------------------------------------------------------------ block-sequential AMS (R23)
 def _assert_block_state(gp, orc):
     po, no = orc.sweep_stats()
