@@ -104,10 +104,12 @@ struct fredopt_plan {
     DevState* st = nullptr;
     // vectors (fp64)
     double *x = nullptr, *g = nullptr, *xtmp = nullptr;                       // [S]
+    float* xstage = nullptr;                                                   // [S] staging of host spot-weight vectors
     double *d = nullptr, *l = nullptr, *Dg = nullptr, *Lg = nullptr;          // [VA]
     GatherVec pq{nullptr, nullptr, nullptr}, uv{nullptr, nullptr, nullptr};    // [VA] gather vectors of the transposed passes
     GatherVec fullUV{nullptr, nullptr, nullptr};                               // lazily: [full.n] gather vector for ROWS_ALL transposes
     double* cpart = nullptr;
+    double* gpart = nullptr;                                                   // [ceil(S/256)] partial sums of |g|^2
     double *part_prox = nullptr, *part_phi = nullptr;
     long long* part_cnt = nullptr;
     int* sink = nullptr;
@@ -753,7 +755,7 @@ static void launch_transpose(fredopt_plan* P, const RowSet& R, const uint8_t* mo
     else
         k_transpose<false><<<fwd_grid(P, R.t_n_items), FWD_THREADS, 0, P->stream>>>(R.t_n_items, R.t_items, R.t_item_slot, mode, R.t_col,
                                                                                       R.t_valD, R.t_valL, vec, R.t_partial);
-    k_combine<EPI><<<grid_for(P->S, 256, 1 << 30), 256, 0, P->stream>>>(P->S, R.t_item_ptr, R.t_partial, g_out, x, P->st, f_out);
+    k_combine<EPI><<<grid_for(P->S, 256, 1 << 30), 256, 0, P->stream>>>(P->S, R.t_item_ptr, R.t_partial, g_out, P->gpart, x, P->st, f_out);
     P->launches += 2;
 }
 
@@ -843,7 +845,7 @@ static int enqueue_iteration(fredopt_plan* P, bool sa) {
             launch_forward(P, P->act, P->mode_union, P->g, P->Dg, P->Lg, EPI_CPART);                   // a5: Dg, Lg, c
             ev_end(P);
             ev_begin(P, FREDOPT_PASS_SELECT);
-            k_select<<<1, 1024, 0, P->stream>>>(P->st, P->g, P->S, P->cpart, cpart_count(P), P->act.n, P->act.items, P->tab, P->d, P->l,
+            k_select<<<1, 1024, 0, P->stream>>>(P->st, P->gpart, P->act.t_n_items ? grid_for(P->S, 256, 1 << 30) : 0, P->cpart, cpart_count(P), P->act.n, P->act.items, P->tab, P->d, P->l,
                                                P->Dg, P->Lg);                                             // a4, a6: beta
             ++P->launches;
             ev_end(P);
@@ -1112,11 +1114,14 @@ static int create_impl(fredopt_plan* P, const fredopt_csr* D, const fredopt_csr*
     CK(cudaGetLastError());
     // ---- vectors
     CKR(dmalloc(P, &P->x, (size_t)S)); CKR(dmalloc(P, &P->g, (size_t)S)); CKR(dmalloc(P, &P->xtmp, (size_t)S));
+    CKR(dmalloc(P, &P->xstage, (size_t)S));
     CK(cudaMemsetAsync(P->x, 0, (S ? S : 1) * 8, st)); CK(cudaMemsetAsync(P->g, 0, (S ? S : 1) * 8, st));
     double** vecs[] = {&P->d, &P->l, &P->Dg, &P->Lg};
     for (auto pp : vecs) { CKR(dmalloc(P, pp, (size_t)n_act)); CK(cudaMemsetAsync(*pp, 0, (n_act ? n_act : 1) * 8, st)); }
     CKR(gv_alloc(P, &P->pq, (size_t)n_act)); CKR(gv_alloc(P, &P->uv, (size_t)n_act));
-    CKR(dmalloc(P, &P->cpart, (size_t)MAX_PARTIALS)); CKR(dmalloc(P, &P->part_prox, (size_t)MAX_PARTIALS));
+    CKR(dmalloc(P, &P->cpart, (size_t)MAX_PARTIALS));
+    CKR(dmalloc(P, &P->gpart, (size_t)(S / 256 + 2)));
+    CK(cudaMemsetAsync(P->gpart, 0, (size_t)(S / 256 + 2) * 8, st)); CKR(dmalloc(P, &P->part_prox, (size_t)MAX_PARTIALS));
     CKR(dmalloc(P, &P->part_phi, (size_t)MAX_PARTIALS)); CKR(dmalloc(P, &P->part_cnt, (size_t)MAX_PARTIALS));
     CKR(dmalloc(P, &P->sink, 4));
     CK(cudaMemsetAsync(P->cpart, 0, MAX_PARTIALS * 8, st));
@@ -1174,13 +1179,22 @@ static int stage_in_f32(fredopt_plan* P, const float* src, size_t n, const float
     return FREDOPT_OK;
 }
 
+// spot-weight vectors (n_cols floats) from the host go through a staging buffer the plan owns (no allocation per call);
+// the copy is complete on return (the caller's array is borrowed for the call only)
+static int stage_x(fredopt_plan* P, const float* x, const float** dev) {
+    if (is_device_ptr(x)) { *dev = x; return FREDOPT_OK; }
+    CK(cudaMemcpyAsync(P->xstage, x, (size_t)P->S * 4, cudaMemcpyHostToDevice, P->stream));
+    CK(cudaStreamSynchronize(P->stream));
+    *dev = P->xstage;
+    return FREDOPT_OK;
+}
+
 int fredopt_set_weights(fredopt_plan* P, const float* x) {
     if (!P || !x) return FREDOPT_INVALID_ARG;
-    const float* dx; void* fr;
-    CKR(stage_in_f32(P, x, P->S, &dx, &fr));
+    const float* dx;
+    CKR(stage_x(P, x, &dx));
     k_f32_to_f64<<<grid_for(P->S, 256, 1024), 256, 0, P->stream>>>(dx, P->x, P->S);
     ++P->launches;
-    if (fr) { cudaStreamSynchronize(P->stream); cudaFree(fr); }
     CK(cudaGetLastError());
     return FREDOPT_OK;
 }
@@ -1212,11 +1226,10 @@ int fredopt_get_weights(fredopt_plan* P, float* x) {
 // x argument of dose_let / proximity / spmv_forward: NULL = plan's x, else widened into xtmp
 static int resolve_x(fredopt_plan* P, const float* x, const double** xd) {
     if (!x) { *xd = P->x; return FREDOPT_OK; }
-    const float* dx; void* fr;
-    CKR(stage_in_f32(P, x, P->S, &dx, &fr));
+    const float* dx;
+    CKR(stage_x(P, x, &dx));
     k_f32_to_f64<<<grid_for(P->S, 256, 1024), 256, 0, P->stream>>>(dx, P->xtmp, P->S);
     ++P->launches;
-    if (fr) { cudaStreamSynchronize(P->stream); cudaFree(fr); }
     *xd = P->xtmp;
     return FREDOPT_OK;
 }

@@ -388,15 +388,27 @@ k_transpose(long long n, const Item* __restrict__ items, const int32_t* __restri
 template <int EPI>
 __global__ void __launch_bounds__(256)
 k_combine(long long S, const long long* __restrict__ item_ptr, const double* __restrict__ partial,
-          double* __restrict__ g_out, double* __restrict__ x, const DevState* __restrict__ st, float* __restrict__ f_out) {
+          double* __restrict__ g_out, double* __restrict__ gpart, double* __restrict__ x, const DevState* __restrict__ st,
+          float* __restrict__ f_out) {
     const long long j = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (EPI == TEPI_GRAD) {   // also the CTA's share of |g|^2 (fixed order), summed by k_select
+        __shared__ double sm[8];
+        double tot = 0.0;
+        if (j < S) {
+            const long long ib = item_ptr[j], ie = item_ptr[j + 1];
+            for (long long i = ib; i < ie; ++i) tot += partial[i];
+            if (ie > ib) g_out[j] = tot;
+        }
+        const double q = block_sum(tot * tot, sm);
+        if (threadIdx.x == 0) gpart[blockIdx.x] = q;
+        return;
+    }
     if (j >= S) return;
     const long long ib = item_ptr[j], ie = item_ptr[j + 1];
     if (ib == ie) return;
     double tot = 0.0;
     for (long long i = ib; i < ie; ++i) tot += partial[i];
-    if (EPI == TEPI_GRAD) g_out[j] = tot;
-    else if (EPI == TEPI_UPDATE) {
+    if (EPI == TEPI_UPDATE) {
         const double v = x[j] - st->relax * tot;          // x <- x' - lambda eta^k * sum w^ (r/|a|^2) a
         x[j] = v < 0.0 ? 0.0 : v;                          // clamp
     } else f_out[j] = (float)tot;
@@ -428,27 +440,23 @@ __device__ __forceinline__ double cost_along(double b, long long n, const Item* 
     return block_sum(phi, sm);
 }
 
-// |g|^2 and c by fixed-order sums, then the `while loop` of Fig. 3 on device scalars.  The step is
+// |g|^2 (partial sums of k_combine) and c (partial sums of F2) in fixed order, then the `while loop` of Fig. 3
+// on device scalars.  The step is
 // b = beta (or beta / |g| with the normalised-gradient option).  Two-sided cost (Eq. 2 as printed):
 //     chi^2(x - b g) = chi^2(x) - b |g|^2 + b^2 c   =>   accept  <=>  b c < |g|^2       (no pass per trial).
 // One-sided cost option: chi^2 is piecewise quadratic, so every trial evaluates chi^2(x - b g) from d - b Dg, l - b Lg
 // (a pass over the labelled rows' vectors, not over the matrix).  The accepted step (0 if none) goes to st->beta_acc;
 // k_residual applies it.  One CTA.
 __global__ void __launch_bounds__(1024)
-k_select(DevState* st, const double* __restrict__ g, long long S, const double* __restrict__ cpart, int n_part,
+k_select(DevState* st, const double* __restrict__ gpart, int n_gpart, const double* __restrict__ cpart, int n_part,
          long long n, const Item* __restrict__ items, const StructInfo* __restrict__ tab, const double* __restrict__ d,
          const double* __restrict__ l, const double* __restrict__ Dg, const double* __restrict__ Lg) {
     __shared__ double sm[32];
     __shared__ double s_b;
     __shared__ int s_go;
-    double a0 = 0.0, a1 = 0.0, a2 = 0.0, a3 = 0.0;
-    long long j = threadIdx.x;
-    for (; j + 3 * 1024 < S; j += 4 * 1024) {       // 4 independent loads in flight; fixed order of addition
-        const double g0 = g[j], g1 = g[j + 1024], g2 = g[j + 2048], g3 = g[j + 3072];
-        a0 = fma(g0, g0, a0); a1 = fma(g1, g1, a1); a2 = fma(g2, g2, a2); a3 = fma(g3, g3, a3);
-    }
-    for (; j < S; j += 1024) a0 = fma(g[j], g[j], a0);
-    const double gg = block_sum((a0 + a1) + (a2 + a3), sm);
+    double a0 = 0.0;
+    for (int i = threadIdx.x; i < n_gpart; i += blockDim.x) a0 += gpart[i];
+    const double gg = block_sum(a0, sm);
     double c = 0.0;
     for (int i = threadIdx.x; i < n_part; i += blockDim.x) c += cpart[i];
     const double cc = block_sum(c, sm);
