@@ -27,6 +27,7 @@
 // and never states lambda, alpha, eta, reductionsN or the matrix sizes, so parity with the PAPER'S OWN
 // RUNS is unpinned; the algorithmic content is pinned by those mathematical checks.
 
+#include <algorithm>
 #include <cmath>
 #include <cstdint>
 #include <cstring>
@@ -430,6 +431,59 @@ void oracle_stats(void* h, int64_t* out, double* dout) {
 void oracle_sweep_stats(void* h, double* prox, int64_t* n_viol) {
     Plan* P = (Plan*)h;
     *prox = P->sweep_prox; *n_viol = P->sweep_viol;
+}
+
+// ---- evaluation quantities of PAPER.md:110 (DVH, LVH, cDLVH, cDL30) and Table 1 -- SURVEY sec. 8f-3.
+// Values of one voxel quantity over the voxels of structure `label`, in voxel order:
+// quantity 0: dose d_i = <D_i, x>; 1: cDL l_i = <L_i, x>; 2: LETd l_i / d_i (0 where d_i = 0, R15).
+static std::vector<double> structure_values(const Plan& P, const std::vector<double>& x, int quantity, int label) {
+    std::vector<double> v;
+    for (int64_t i = 0; i < P.D.n_rows; ++i) {
+        if (P.label[i] != label) continue;
+        const double d = row_dot(P.D, i, x), l = row_dot(P.L, i, x);
+        v.push_back(quantity == 0 ? d : quantity == 1 ? l : (d > 0.0 ? l / d : 0.0));
+    }
+    return v;
+}
+
+// min, mean, max over the structure's voxels (Table 1's columns) and the voxel count; all 0 for an empty structure
+void oracle_structure_stats(void* h, const double* xin, int32_t quantity, int32_t label, double* out3, int64_t* n) {
+    Plan* P = (Plan*)h;
+    std::vector<double> x = xin ? std::vector<double>(xin, xin + P->x.size()) : P->x;
+    std::vector<double> v = structure_values(*P, x, quantity, label);
+    *n = (int64_t)v.size();
+    out3[0] = out3[1] = out3[2] = 0.0;
+    if (v.empty()) return;
+    double mn = v[0], mx = v[0], sum = 0.0;
+    for (double t : v) { mn = t < mn ? t : mn; mx = t > mx ? t : mx; sum += t; }
+    out3[0] = mn; out3[1] = sum / (double)v.size(); out3[2] = mx;
+}
+
+// cumulative volume histogram: hist[b] = fraction of the structure's voxels with value >= b * vmax / n_bins
+void oracle_volume_histogram(void* h, const double* xin, int32_t quantity, int32_t label, int32_t n_bins, double vmax, double* hist) {
+    Plan* P = (Plan*)h;
+    std::vector<double> x = xin ? std::vector<double>(xin, xin + P->x.size()) : P->x;
+    std::vector<double> v = structure_values(*P, x, quantity, label);
+    for (int32_t b = 0; b < n_bins; ++b) {
+        int64_t c = 0;
+        const double edge = (double)b * vmax / (double)n_bins;
+        for (double t : v) if (t >= edge) ++c;
+        hist[b] = v.empty() ? 0.0 : (double)c / (double)v.size();
+    }
+}
+
+// "the value received by `fraction` of the structure volume" (cDL30: fraction 0.3): the smallest of the
+// ceil(fraction * n) largest values, i.e. the largest t such that at least fraction * n voxels have a value >= t
+double oracle_percentile_value(void* h, const double* xin, int32_t quantity, int32_t label, double fraction) {
+    Plan* P = (Plan*)h;
+    std::vector<double> x = xin ? std::vector<double>(xin, xin + P->x.size()) : P->x;
+    std::vector<double> v = structure_values(*P, x, quantity, label);
+    if (v.empty()) return 0.0;
+    std::sort(v.begin(), v.end(), [](double a, double b) { return a > b; });
+    int64_t k = (int64_t)std::ceil(fraction * (double)v.size());
+    if (k < 1) k = 1;
+    if (k > (int64_t)v.size()) k = (int64_t)v.size();
+    return v[k - 1];
 }
 
 void oracle_norms(void* h, double* nD, double* nL, double* nT) {

@@ -52,6 +52,10 @@ def _load():
         lib.oracle_iterate.argtypes = [vp, i32, f32, f32, f32]
         lib.oracle_stats.argtypes = [vp, vp, vp]
         lib.oracle_sweep_stats.argtypes = [vp, vp, vp]
+        lib.oracle_structure_stats.argtypes = [vp, vp, i32, i32, vp, vp]
+        lib.oracle_volume_histogram.argtypes = [vp, vp, i32, i32, i32, f64, vp]
+        lib.oracle_percentile_value.restype = f64
+        lib.oracle_percentile_value.argtypes = [vp, vp, i32, i32, f64]
         lib.oracle_norms.argtypes = [vp, vp, vp, vp]
         lib.oracle_what.argtypes = [vp, vp]
         lib.oracle_sequential_sweep.argtypes = [vp, f32]
@@ -164,6 +168,23 @@ class Oracle:
         pr = C.c_double(0.0); nv = C.c_int64(0)
         self._lib.oracle_sweep_stats(self._h, C.byref(pr), C.byref(nv))
         return pr.value, nv.value
+
+    # ---- evaluation quantities (DVH / LVH / cDLVH, cDL30, Table 1)
+    def structure_stats(self, quantity, label, x=None):
+        xx = None if x is None else np.ascontiguousarray(x, np.float64)
+        o = np.zeros(3, np.float64); n = C.c_int64(0)
+        self._lib.oracle_structure_stats(self._h, _p(xx), int(quantity), int(label), _p(o), C.byref(n))
+        return float(o[0]), float(o[1]), float(o[2]), n.value
+
+    def volume_histogram(self, quantity, label, n_bins, vmax, x=None):
+        xx = None if x is None else np.ascontiguousarray(x, np.float64)
+        hst = np.zeros(n_bins, np.float64)
+        self._lib.oracle_volume_histogram(self._h, _p(xx), int(quantity), int(label), int(n_bins), float(vmax), _p(hst))
+        return hst
+
+    def percentile_value(self, quantity, label, fraction, x=None):
+        xx = None if x is None else np.ascontiguousarray(x, np.float64)
+        return float(self._lib.oracle_percentile_value(self._h, _p(xx), int(quantity), int(label), float(fraction)))
 
     def norms(self):
         a = np.empty(self.V, np.float64); b = np.empty(self.V, np.float64); c = np.empty(self.V, np.float64)

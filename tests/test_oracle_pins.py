@@ -642,3 +642,34 @@ def test_pin18_normalised_gradient_step_has_length_beta():
     step = np.linalg.norm(o.get_x() - x0.astype(np.float64))
     assert st["last_beta"] > 0 and abs(step - st["last_beta"]) <= 1e-14
     assert o.cost(None) < phi0 and st["trials"] == st["s"] >= 1
+
+
+# ----------------------------------------------------------------------------- evaluation quantities
+def test_pin19_volume_histogram_percentile_and_table1_statistics():
+    """DVH / cDLVH / cDL30 and Table 1's columns on a hand example and against numpy."""
+    # hand example: D = identity on 10 voxels of one structure => d_i = x_i = 1..10; "value received by 30% of the volume" = 8
+    V = S = 10
+    Dd = np.eye(V); Ld = 2.0 * np.eye(V)
+    labels = np.ones(V, np.int32)
+    bounds = bounds_rows(dict(weight=1.0, dose_hi=100.0))
+    o = make_oracle(Dd, Ld, labels, bounds)
+    x = np.arange(1.0, 11.0)
+    assert o.percentile_value(0, 1, 0.3, x) == 8.0 and o.percentile_value(1, 1, 0.3, x) == 16.0
+    assert o.percentile_value(0, 1, 1.0, x) == 1.0 and o.percentile_value(0, 1, 0.05, x) == 10.0
+    assert o.structure_stats(0, 1, x) == (1.0, 5.5, 10.0, 10)
+    assert o.structure_stats(2, 1, x)[:3] == (2.0, 2.0, 2.0)                       # LETd = l/d = 2 everywhere
+    assert np.array_equal(o.volume_histogram(0, 1, 5, 10.0, x), [1.0, 0.9, 0.7, 0.5, 0.3])   # edges 0, 2, 4, 6, 8
+    # against numpy on a random plan
+    D, L, lab, x0 = pg.random_small_plan(41, V=60, S=9, n_struct=2)
+    Dd, Ld = csr_to_dense(D, 9), csr_to_dense(L, 9)
+    o = orc.Oracle.create(60, 9, D, L, lab, bounds_rows(dict(weight=1.0, dose_hi=1.0), dict(weight=1.0, dl_hi=1.0)))
+    xx = x0.astype(np.float64)
+    for s_ in (1, 2):
+        d, l = (Dd @ xx)[lab == s_], (Ld @ xx)[lab == s_]
+        for q, v in ((0, d), (1, l), (2, np.where(d > 0, l / np.where(d > 0, d, 1.0), 0.0))):
+            mn, mean, mx, n = o.structure_stats(q, s_, xx)
+            assert n == len(v) and np.allclose([mn, mean, mx], [v.min(), v.mean(), v.max()], rtol=1e-13)
+            pv = o.percentile_value(q, s_, 0.3, xx)
+            assert np.mean(v >= pv * (1 - 1e-13)) >= 0.3 and np.mean(v > pv * (1 + 1e-13)) < 0.3
+            hst = o.volume_histogram(q, s_, 16, float(v.max()) * 1.01, xx)
+            assert hst[0] == 1.0 and np.all(np.diff(hst) <= 0) and hst[-1] > 0
