@@ -160,6 +160,22 @@ int fredopt_proximity(fredopt_plan *plan, const float *x, double *prox, int64_t 
 int fredopt_set_option(fredopt_plan *plan, int32_t key, double value);
 int fredopt_get_stats(fredopt_plan *plan, fredopt_stats *out);
 
+/* ---- evaluation quantities of the paper's constraint selection and plan comparison (Table 1,
+ * PAPER.md:228-236): the dose / LETd / c x D x LETd volume histograms (DVH, LVH, cDLVH), the "value received by a
+ * fraction of the structure volume" (cDL30) and a structure's min / mean / max.  quantity: 0 = dose <D_i, x>,
+ * 1 = cDL <L_i, x>, 2 = LETd = cDL / dose (0 where the dose is 0); label in 1..n_struct; x: n_cols floats or NULL = the
+ * plan's x.  All three synchronise.  An empty structure gives zeros. */
+int fredopt_structure_stats(fredopt_plan *plan, const float *x, int32_t quantity, int32_t label,
+                            double *vmin, double *vmean, double *vmax, int64_t *n_voxels);   /* HOST pointers, may be NULL */
+/* hist[b] = fraction of the structure's voxels whose value is >= b * vmax / n_bins, b = 0..n_bins-1 (cumulative volume
+ * histogram; hist: n_bins floats, host or device; 1 <= n_bins <= 2368; vmax > 0). */
+int fredopt_volume_histogram(fredopt_plan *plan, const float *x, int32_t quantity, int32_t label, int32_t n_bins,
+                             double vmax, float *hist);
+/* The smallest of the ceil(fraction * n) largest values of the structure's n voxels: at least `fraction` of the volume
+ * receives this value or more (cDL30: quantity 1, fraction 0.3).  0 < fraction <= 1; value: HOST pointer. */
+int fredopt_percentile_value(fredopt_plan *plan, const float *x, int32_t quantity, int32_t label, double fraction,
+                             double *value);
+
 /* ---- per-pass exports: per-SpMV parity tests and the isolated-pass sweep (BASELINE.json configs[4]) ----
  * forward:   d = D x, l = L x over the selected rows; d, l: n_rows floats, voxel-indexed (rows outside the
  *            selection are written as 0); either may be NULL (that matrix's values are then not read).

@@ -1338,6 +1338,91 @@ int fredopt_proximity(fredopt_plan* P, const float* x, double* prox, int64_t* n_
     return FREDOPT_OK;
 }
 
+// ---- evaluation quantities: values of one voxel quantity over the rows of structure `label` into uv.cD[rb .. rb+nr)
+static int structure_values(fredopt_plan* P, const float* x, int32_t quantity, int32_t label, long long* rb_out, long long* nr_out) {
+    if (!P || quantity < 0 || quantity > 2 || label < 1 || label > P->n_struct) return FREDOPT_INVALID_ARG;
+    const double* xd;
+    CKR(resolve_x(P, x, &xd));
+    long long rb = 0;
+    for (int s = 0; s < label - 1; ++s) rb += (long long)P->h_tab[s].rows;
+    const long long nr = (long long)P->h_tab[label - 1].rows;
+    *rb_out = rb; *nr_out = nr;
+    if (nr == 0) return FREDOPT_OK;
+    const RowSet& A = P->act;
+    const int m = quantity == 0 ? 1 : quantity == 1 ? 2 : 3;
+    const uint8_t* md = P->mode_fixed + (size_t)m * P->max_seg;
+    const GatherVec none{nullptr, nullptr, nullptr};
+    const int g = fwd_grid(P, nr);
+    if (A.col16) k_forward<EPI_STORE, true><<<g, FWD_THREADS, 0, P->stream>>>(nr, A.items + rb, A.vox + rb, md, A.col16, A.valD, A.valL, xd, P->Dg + rb, P->Lg + rb, none, nullptr, nullptr, nullptr, nullptr, nullptr, 0);
+    else k_forward<EPI_STORE, false><<<g, FWD_THREADS, 0, P->stream>>>(nr, A.items + rb, A.vox + rb, md, A.col, A.valD, A.valL, xd, P->Dg + rb, P->Lg + rb, none, nullptr, nullptr, nullptr, nullptr, nullptr, 0);
+    k_quantity<<<grid_for(nr, 256, 1024), 256, 0, P->stream>>>(nr, quantity, P->Dg + rb, P->Lg + rb, P->uv.cD + rb);
+    P->launches += 2;
+    CK(cudaGetLastError());
+    return FREDOPT_OK;
+}
+
+int fredopt_structure_stats(fredopt_plan* P, const float* x, int32_t quantity, int32_t label, double* vmin, double* vmean,
+                            double* vmax, int64_t* n_voxels) {
+    long long rb, nr;
+    CKR(structure_values(P, x, quantity, label, &rb, &nr));
+    double h[3] = {0.0, 0.0, 0.0};
+    if (nr) {
+        k_value_stats<<<1, 1024, 0, P->stream>>>(nr, P->uv.cD + rb, P->part_prox);
+        ++P->launches;
+        CK(cudaMemcpyAsync(h, P->part_prox, 3 * sizeof(double), cudaMemcpyDeviceToHost, P->stream));
+        CK(cudaStreamSynchronize(P->stream));
+        h[1] /= (double)nr;
+    }
+    if (vmin) *vmin = h[0];
+    if (vmean) *vmean = h[1];
+    if (vmax) *vmax = h[2];
+    if (n_voxels) *n_voxels = nr;
+    return FREDOPT_OK;
+}
+
+int fredopt_volume_histogram(fredopt_plan* P, const float* x, int32_t quantity, int32_t label, int32_t n_bins, double vmax,
+                             float* hist) {
+    if (!hist || n_bins < 1 || n_bins > MAX_PARTIALS || !(vmax > 0.0) || !std::isfinite(vmax)) return FREDOPT_INVALID_ARG;
+    long long rb, nr;
+    CKR(structure_values(P, x, quantity, label, &rb, &nr));
+    std::vector<unsigned long long> c((size_t)n_bins, 0ULL);
+    if (nr) {
+        CK(cudaMemsetAsync(P->part_cnt, 0, (size_t)n_bins * 8, P->stream));
+        k_value_hist<<<grid_for(nr, 256, 1024), 256, 0, P->stream>>>(nr, P->uv.cD + rb, n_bins, vmax, (unsigned long long*)P->part_cnt);
+        ++P->launches;
+        CK(cudaMemcpyAsync(c.data(), P->part_cnt, (size_t)n_bins * 8, cudaMemcpyDeviceToHost, P->stream));
+        CK(cudaStreamSynchronize(P->stream));
+    }
+    std::vector<float> hh((size_t)n_bins, 0.f);
+    unsigned long long cum = 0;
+    for (int b = n_bins - 1; b >= 0; --b) { cum += c[b]; hh[b] = nr ? (float)((double)cum / (double)nr) : 0.f; }
+    if (is_device_ptr(hist)) { CK(cudaMemcpyAsync(hist, hh.data(), (size_t)n_bins * 4, cudaMemcpyHostToDevice, P->stream)); CK(cudaStreamSynchronize(P->stream)); }
+    else memcpy(hist, hh.data(), (size_t)n_bins * 4);
+    return FREDOPT_OK;
+}
+
+int fredopt_percentile_value(fredopt_plan* P, const float* x, int32_t quantity, int32_t label, double fraction, double* value) {
+    if (!value || !(fraction > 0.0) || !(fraction <= 1.0)) return FREDOPT_INVALID_ARG;
+    long long rb, nr;
+    CKR(structure_values(P, x, quantity, label, &rb, &nr));
+    *value = 0.0;
+    if (nr == 0) return FREDOPT_OK;
+    size_t tb = 0;
+    CK(cub::DeviceRadixSort::SortKeysDescending(nullptr, tb, P->uv.cD + rb, P->uv.cL + rb, nr, 0, 64, P->stream));
+    void* tmp = nullptr;
+    CK(cudaMalloc(&tmp, tb ? tb : 1));
+    cudaError_t e = cub::DeviceRadixSort::SortKeysDescending(tmp, tb, P->uv.cD + rb, P->uv.cL + rb, nr, 0, 64, P->stream);
+    long long k = (long long)std::ceil(fraction * (double)nr);
+    if (k < 1) k = 1;
+    if (k > nr) k = nr;
+    if (e == cudaSuccess) e = cudaMemcpyAsync(value, P->uv.cL + rb + (k - 1), sizeof(double), cudaMemcpyDeviceToHost, P->stream);
+    cudaError_t e2 = cudaStreamSynchronize(P->stream);
+    cudaFree(tmp);
+    ++P->launches;
+    CK(e); CK(e2);
+    return FREDOPT_OK;
+}
+
 int fredopt_set_option(fredopt_plan* P, int32_t key, double value) {
     if (!P) return FREDOPT_INVALID_ARG;
     switch (key) {

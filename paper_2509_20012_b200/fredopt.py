@@ -28,6 +28,7 @@ SYMBOLS = (
     "fredopt_dose_let", "fredopt_iterate", "fredopt_proximity", "fredopt_set_option", "fredopt_get_stats",
     "fredopt_spmv_forward", "fredopt_spmv_transpose", "fredopt_get_pass_times", "fredopt_get_pass_bytes",
     "fredopt_launch_count", "fredopt_stream_read", "fredopt_strerror", "fredopt_last_cuda_error",
+    "fredopt_structure_stats", "fredopt_volume_histogram", "fredopt_percentile_value",
 )
 
 
@@ -77,6 +78,9 @@ def _load():
     lib.fredopt_get_stats.argtypes = [vp, C.POINTER(Stats)]
     lib.fredopt_spmv_forward.argtypes = [vp, i32, vp, vp, vp]
     lib.fredopt_spmv_transpose.argtypes = [vp, i32, vp, vp, vp]
+    lib.fredopt_structure_stats.argtypes = [vp, vp, i32, i32, C.POINTER(f64), C.POINTER(f64), C.POINTER(f64), C.POINTER(i64)]
+    lib.fredopt_volume_histogram.argtypes = [vp, vp, i32, i32, i32, f64, vp]
+    lib.fredopt_percentile_value.argtypes = [vp, vp, i32, i32, f64, C.POINTER(f64)]
     lib.fredopt_get_pass_times.argtypes = [vp, C.POINTER(f64), C.POINTER(i64)]
     lib.fredopt_get_pass_bytes.argtypes = [vp, C.POINTER(i64)]
     lib.fredopt_launch_count.argtypes = [vp]
@@ -183,6 +187,24 @@ class Plan:
         _check(_lib.fredopt_proximity(self._h, _ptr(x, np.float32, self.n_cols), C.byref(p), C.byref(n)),
                "fredopt_proximity")
         return p.value, n.value
+
+    # ---- evaluation quantities (DVH / LVH / cDLVH, cDL30, Table 1)
+    def structure_stats(self, quantity, label, x=None):
+        mn, mean, mx, n = C.c_double(0.0), C.c_double(0.0), C.c_double(0.0), C.c_int64(0)
+        _check(_lib.fredopt_structure_stats(self._h, _ptr(x, np.float32, self.n_cols), int(quantity), int(label), C.byref(mn),
+                                            C.byref(mean), C.byref(mx), C.byref(n)), "fredopt_structure_stats")
+        return mn.value, mean.value, mx.value, n.value
+
+    def volume_histogram(self, quantity, label, n_bins, vmax, hist, x=None):
+        _check(_lib.fredopt_volume_histogram(self._h, _ptr(x, np.float32, self.n_cols), int(quantity), int(label), int(n_bins),
+                                             float(vmax), _ptr(hist, np.float32, n_bins)), "fredopt_volume_histogram")
+        return hist
+
+    def percentile_value(self, quantity, label, fraction, x=None):
+        v = C.c_double(0.0)
+        _check(_lib.fredopt_percentile_value(self._h, _ptr(x, np.float32, self.n_cols), int(quantity), int(label),
+                                             float(fraction), C.byref(v)), "fredopt_percentile_value")
+        return v.value
 
     # ---- options, stats
     def set_option(self, key, value):

@@ -330,6 +330,48 @@ def test_options_on_three_beam_plan(fredopt):
     _assert_state(gp, orc)
 
 
+# ------------------------------------------------------------------------------------------ evaluation quantities
+def _assert_evaluation(gp, orc, n_struct, x):
+    x64 = x.astype(np.float64)
+    for label in range(1, n_struct + 1):
+        for q in (0, 1, 2):
+            mn, mean, mx, n = gp.structure_stats(q, label, x)
+            omn, omean, omx, on = orc.structure_stats(q, label, x64)
+            assert n == on
+            assert np.allclose([mn, mean, mx], [omn, omean, omx], rtol=1e-12, atol=1e-300)
+            if n == 0 or omx <= 0:
+                continue
+            for frac in (0.02, 0.3, 0.5, 1.0):
+                assert abs(gp.percentile_value(q, label, frac, x) - orc.percentile_value(q, label, frac, x64)) <= 1e-12 * omx
+            hist = np.empty(64, np.float32)
+            gp.volume_histogram(q, label, 64, omx * 1.05, hist, x)
+            ref = orc.volume_histogram(q, label, 64, omx * 1.05, x64)
+            assert np.all(np.abs(hist - ref) <= 1.5 / n + 1e-6)      # a value within rounding of a bin edge may move one voxel
+            assert hist[0] == 1.0
+
+
+def test_evaluation_quantities_config0(fredopt, plan0):
+    gp = fredopt.from_plan(plan0); orc = _oracle(plan0)
+    _assert_evaluation(gp, orc, 2, plan0.x0)
+    # and at the plan's own x after some iterations (x = NULL)
+    gp.set_weights(plan0.x0); gp.iterate(10, 1.0, 1.0, 0.99)
+    orc.set_x(plan0.x0); orc.iterate(10, 1.0, 1.0, 0.99)
+    v = gp.percentile_value(0, 2, 0.3)
+    assert abs(v - orc.percentile_value(0, 2, 0.3)) <= 1e-12 * max(abs(v), 1e-30)
+    with pytest.raises(fredopt.FredoptError):
+        gp.percentile_value(0, 3, 0.3)
+    with pytest.raises(fredopt.FredoptError):
+        gp.percentile_value(3, 1, 0.3)
+    with pytest.raises(fredopt.FredoptError):
+        gp.percentile_value(0, 1, 0.0)
+
+
+def test_evaluation_quantities_three_beam_plan(fredopt):
+    plan = pg.build_plan(pg.config_spec(2, scale=0.25), device="cuda")
+    gp = fredopt.from_plan(plan, stream=torch.cuda.current_stream().cuda_stream); orc = _oracle(plan)
+    _assert_evaluation(gp, orc, 4, pg.log_uniform_weights(3, plan.n_cols))
+
+
 # ------------------------------------------------------------------------------------------ block-sequential AMS (R23)
 def _assert_block_state(gp, orc):
     po, no = orc.sweep_stats()
