@@ -25,6 +25,12 @@ constexpr int FWD_WARPS = FWD_THREADS / 32;
 constexpr int MAX_PARTIALS = 2368;          // 148 SMs x 16 CTAs: upper bound of any partial-sum grid
 constexpr int ROW_THREADS = 256;
 constexpr int TR_ITEM_MAX = 2048;           // entries per transposed work item (multiple of 4)
+#ifndef FWD_U1
+#define FWD_U1 6   /* 128-entry chunks in flight per trip for rows that read one matrix ... */
+#endif
+#ifndef FWD_U3
+#define FWD_U3 4   /* ... and for rows that read both (measured: 6/4 beats 4/4 by 2 %, 8/4 and 6/3 are slower) */
+#endif
 constexpr int FWD_MIN_CTAS = 4;             // resident CTAs per SM the item kernels are compiled for (64 registers)
 
 // flags of a structure
@@ -147,7 +153,7 @@ template <int M, bool I16>
 __device__ __forceinline__ void fwd_row(const void* __restrict__ cbase, long long e0, const float* __restrict__ dp,
                                         const float* __restrict__ lp, int L, int lane, const double* __restrict__ x,
                                         double& aD, double& aL) {
-    constexpr int U = 4;
+    constexpr int U = (M == 3) ? FWD_U3 : FWD_U1;
     int p = lane * 4;
     for (; p + 128 * (U - 1) < L; p += 128 * U) {
         int4 c[U];
@@ -296,7 +302,7 @@ enum : int { TEPI_F32 = 0, TEPI_GRAD = 1, TEPI_UPDATE = 2 };
 template <int M, bool I16>
 __device__ __forceinline__ double tr_item(const void* __restrict__ cbase, long long e0, int add, const float* __restrict__ dp,
                                           const float* __restrict__ lp, int L, int lane, const GatherVec& gv) {
-    constexpr int U = 4;
+    constexpr int U = (M == 3) ? FWD_U3 : FWD_U1;
     const double2* __restrict__ vec = gv.pair;
     const double* __restrict__ vs = (M == 2) ? gv.cL : gv.cD;
     double aD = 0.0, aL = 0.0;
