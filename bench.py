@@ -171,7 +171,9 @@ def run_ours(args):
     plan = pg.build_plan(spec, device="cuda")
     torch.cuda.synchronize()
     t_gen = time.perf_counter() - t0
-    stream = torch.cuda.current_stream()
+    torch.cuda.synchronize()
+    stream = torch.cuda.Stream()          # the plan's stream: every kernel and every timing event of this run is on it
+    torch.cuda.set_stream(stream)
     t0 = time.perf_counter()
     gp = fredopt.from_plan(plan, stream=stream.cuda_stream)
     torch.cuda.synchronize()
@@ -323,7 +325,8 @@ def run_sweep(args):
     import gc
     from paper_2509_20012_b200 import fredopt, plangen as pg
     torch.cuda.set_device(0)
-    stream = torch.cuda.current_stream()
+    stream = torch.cuda.Stream()          # the plans' stream: kernels and timing events are on it
+    torch.cuda.set_stream(stream)
     peak, peak_src = _peaks()
     l2 = torch.cuda.get_device_properties(0).L2_cache_size
     flush = torch.empty(int(1.5 * l2), dtype=torch.uint8, device="cuda")

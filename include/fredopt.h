@@ -26,7 +26,8 @@
  *     cudaStreamDefault flags, i.e. ordered against the legacy default stream as any blocking stream is -- the
  *     legacy stream itself cannot be captured into a CUDA graph).  Calls enqueue on that stream; a call that writes host memory synchronises the stream before returning, a call with
  *     device outputs only does not.
- *   - arithmetic: matrix values are stored as given (fp32), indices int32, offsets int64; every vector the
+ *   - arithmetic: matrix values are stored as given (fp32), indices as 16 bits where that is exact (n_cols <= 65536;
+ *     row indices of the transposes inside 65536-row blocks) and int32 otherwise, offsets int64; every vector the
  *     iteration keeps (x, d, l, g, u, v) and every accumulator / scalar / decision is fp64 on the device.
  *     fp32 scalars cross the ABI as their bit patterns and are widened, never recomputed.
  *   - every function returns FREDOPT_OK (0) or a negative error code; no exception or abort crosses the ABI;

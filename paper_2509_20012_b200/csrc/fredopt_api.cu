@@ -140,12 +140,6 @@ static int dmalloc(fredopt_plan* P, T** p, size_t n) {
     P->allocs.push_back((void*)*p);
     return FREDOPT_OK;
 }
-static void dfree(fredopt_plan* P, void* p) {
-    if (!p) return;
-    for (size_t i = 0; i < P->allocs.size(); ++i)
-        if (P->allocs[i] == p) { P->allocs[i] = P->allocs.back(); P->allocs.pop_back(); break; }
-    cudaFree(p);
-}
 
 static int gv_alloc(fredopt_plan* P, GatherVec* g, size_t n) {
     CKR(dmalloc(P, &g->pair, n)); CKR(dmalloc(P, &g->cD, n)); CKR(dmalloc(P, &g->cL, n));

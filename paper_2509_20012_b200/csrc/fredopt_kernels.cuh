@@ -13,7 +13,7 @@
 //   k_select     |g|^2, c = sum w^ (Dg)^2 + w^ (Lg)^2 and the accept loop of Fig. 3 on device scalars.
 //   k_residual   d' = d - beta Dg, l' = l - beta Lg, x' = x - beta g, residuals / violations of Fig. 2 -> u, v,
 //                partial sums of proximity, cost and violation count.
-// All vectors and accumulators are fp64; matrix values fp32; indices int32; offsets int64.
+// All vectors and accumulators are fp64; matrix values fp32; indices 16-bit where they fit, else int32; offsets int64.
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>
@@ -147,8 +147,8 @@ __device__ __forceinline__ void fma4(double& acc, const float4& a, double x0, do
 // ------------------------------------------------------------------------------------------ forward
 enum : int { EPI_STORE = 0, EPI_STORE_PQ = 1, EPI_CPART = 2, EPI_F32VOX = 3 };
 
-// <D_i, x> and / or <L_i, x> of one row by one warp.  M: bit 0 = D, bit 1 = L.  Four 128-entry chunks per trip:
-// up to 12 independent 128-bit loads per lane in flight before the first gather.
+// <D_i, x> and / or <L_i, x> of one row by one warp.  M: bit 0 = D, bit 1 = L.  U 128-entry chunks per trip (6 for a
+// single matrix, 4 for both): up to 12 independent vector loads per lane in flight before the first gather.
 template <int M, bool I16>
 __device__ __forceinline__ void fwd_row(const void* __restrict__ cbase, long long e0, const float* __restrict__ dp,
                                         const float* __restrict__ lp, int L, int lane, const double* __restrict__ x,
