@@ -717,21 +717,36 @@ static int fwd_grid(fredopt_plan* P, long long n) {
     return grid_for(n, FWD_WARPS, cap);
 }
 
-// epi: EPI_STORE (d, l), EPI_STORE_PQ (d, l and the cost residuals p, q), EPI_CPART (Dg, Lg and partial sums of c)
-static void launch_forward(fredopt_plan* P, const RowSet& R, const uint8_t* mode, const double* x, double* oD, double* oL, int epi) {
-    if (R.n == 0) { if (epi == EPI_CPART) cudaMemsetAsync(P->cpart, 0, sizeof(double) * MAX_PARTIALS, P->stream); return; }
+static const ResidArgs NO_RESID{nullptr, nullptr, nullptr, GatherVec{nullptr, nullptr, nullptr}, nullptr, nullptr, nullptr, nullptr};
+
+// epi: EPI_STORE (d, l), EPI_STORE_PQ (d, l and the cost residuals p, q), EPI_CPART (Dg, Lg and partial sums of c),
+// EPI_RESID (d, l and the residual / violation epilogue: step coefficients u, v if write_uv, statistics partials)
+static void launch_forward(fredopt_plan* P, const RowSet& R, const uint8_t* mode, const double* x, double* oD, double* oL, int epi,
+                           int write_uv = 0) {
+    if (R.n == 0) {
+        if (epi == EPI_CPART) cudaMemsetAsync(P->cpart, 0, sizeof(double) * MAX_PARTIALS, P->stream);
+        if (epi == EPI_RESID) {   // nothing to visit: zero statistics (finalize reads one partial)
+            cudaMemsetAsync(P->part_prox, 0, 8, P->stream); cudaMemsetAsync(P->part_phi, 0, 8, P->stream); cudaMemsetAsync(P->part_cnt, 0, 8, P->stream);
+            if (write_uv) { k_sweep_end<<<grid_for(P->S, 256, 1 << 30), 256, 0, P->stream>>>(P->S, P->x, P->st); ++P->launches; }   // k, eta^k still advance
+        }
+        return;
+    }
     const int g = fwd_grid(P, R.n);
     const GatherVec none{nullptr, nullptr, nullptr};
+    ResidArgs ra = NO_RESID;
+    if (epi == EPI_RESID) ra = ResidArgs{P->nD, P->nL, P->nT, write_uv ? P->uv : none, P->part_prox, P->part_phi, P->part_cnt, P->st};
 #define FWD_LAUNCH(E, I16, COL, PQ, TAB, CP)                                                                                   \
     k_forward<E, I16><<<g, FWD_THREADS, 0, P->stream>>>(R.n, R.items, R.vox, mode, COL, R.valD, R.valL, x, oD, oL, PQ, TAB, CP, \
-                                                       P->st, nullptr, nullptr, 0)
+                                                       P->st, nullptr, nullptr, 0, ra)
     if (R.col16) {
         if (epi == EPI_CPART) FWD_LAUNCH(EPI_CPART, true, R.col16, none, P->tab, P->cpart);
         else if (epi == EPI_STORE_PQ) FWD_LAUNCH(EPI_STORE_PQ, true, R.col16, P->pq, P->tab, nullptr);
+        else if (epi == EPI_RESID) FWD_LAUNCH(EPI_RESID, true, R.col16, none, P->tab, nullptr);
         else FWD_LAUNCH(EPI_STORE, true, R.col16, none, nullptr, nullptr);
     } else {
         if (epi == EPI_CPART) FWD_LAUNCH(EPI_CPART, false, R.col, none, P->tab, P->cpart);
         else if (epi == EPI_STORE_PQ) FWD_LAUNCH(EPI_STORE_PQ, false, R.col, P->pq, P->tab, nullptr);
+        else if (epi == EPI_RESID) FWD_LAUNCH(EPI_RESID, false, R.col, none, P->tab, nullptr);
         else FWD_LAUNCH(EPI_STORE, false, R.col, none, nullptr, nullptr);
     }
 #undef FWD_LAUNCH
@@ -767,8 +782,9 @@ static void launch_residual(fredopt_plan* P, double* d, double* l, int use_beta,
     ++P->launches;
 }
 
-static void launch_finalize(fredopt_plan* P) {
-    k_finalize_stats<<<1, 1024, 0, P->stream>>>(P->st, P->part_prox, P->part_phi, P->part_cnt, res_grid(P));
+// n_part: how many per-CTA partial sums the last residual pass wrote (k_residual: res_grid; forward epilogue: fwd_grid)
+static void launch_finalize(fredopt_plan* P, int n_part) {
+    k_finalize_stats<<<1, 1024, 0, P->stream>>>(P->st, P->part_prox, P->part_phi, P->part_cnt, n_part);
     ++P->launches;
 }
 
@@ -793,8 +809,8 @@ static void enqueue_block_sweep(fredopt_plan* P) {
             ev_begin(P, FREDOPT_PASS_FORWARD_X);
             {
                 const int g = fwd_grid(P, nr);
-                if (A.col16) k_forward<EPI_STORE, true><<<g, FWD_THREADS, 0, P->stream>>>(nr, A.items + rb, A.vox + rb, md, A.col16, A.valD, A.valL, P->x, P->d + rb, P->l + rb, none, nullptr, nullptr, nullptr, nullptr, nullptr, 0);
-                else k_forward<EPI_STORE, false><<<g, FWD_THREADS, 0, P->stream>>>(nr, A.items + rb, A.vox + rb, md, A.col, A.valD, A.valL, P->x, P->d + rb, P->l + rb, none, nullptr, nullptr, nullptr, nullptr, nullptr, 0);
+                if (A.col16) k_forward<EPI_STORE, true><<<g, FWD_THREADS, 0, P->stream>>>(nr, A.items + rb, A.vox + rb, md, A.col16, A.valD, A.valL, P->x, P->d + rb, P->l + rb, none, nullptr, nullptr, nullptr, nullptr, nullptr, 0, NO_RESID);
+                else k_forward<EPI_STORE, false><<<g, FWD_THREADS, 0, P->stream>>>(nr, A.items + rb, A.vox + rb, md, A.col, A.valD, A.valL, P->x, P->d + rb, P->l + rb, none, nullptr, nullptr, nullptr, nullptr, nullptr, 0, NO_RESID);
                 ++P->launches;
             }
             ev_end(P);
@@ -848,12 +864,9 @@ static int enqueue_iteration(fredopt_plan* P, bool sa) {
             launch_residual(P, P->d, P->l, 1, last, last);                                             // x', d', l'; a7
             ev_end(P);
         }
-    } else if (!P->block_sequential) {
+    } else if (!P->block_sequential) {      // pure feasibility-seeking: the residual / violation work is the forward pass's epilogue
         ev_begin(P, FREDOPT_PASS_FORWARD_X);
-        launch_forward(P, P->act, P->mode_con, P->x, P->d, P->l, EPI_STORE);
-        ev_end(P);
-        ev_begin(P, FREDOPT_PASS_RESIDUAL);
-        launch_residual(P, P->d, P->l, 0, 1, 1);
+        launch_forward(P, P->act, P->mode_con, P->x, P->d, P->l, EPI_RESID, 1);                       // a1 + a7
         ev_end(P);
     }
     if (P->block_sequential) {
@@ -1259,8 +1272,8 @@ static int forward_f32(fredopt_plan* P, const RowSet& R, int m, const double* xd
 #undef SHORT_LAUNCH
         }
         if (n_long) {
-            if (i16) k_forward<EPI_F32VOX, true><<<fwd_grid(P, n_long), FWD_THREADS, 0, P->stream>>>(n_long, R.items, R.vox, md, colp, R.valD, R.valL, xd, nullptr, nullptr, none, nullptr, nullptr, nullptr, dd, dl, letd_out);
-            else k_forward<EPI_F32VOX, false><<<fwd_grid(P, n_long), FWD_THREADS, 0, P->stream>>>(n_long, R.items, R.vox, md, colp, R.valD, R.valL, xd, nullptr, nullptr, none, nullptr, nullptr, nullptr, dd, dl, letd_out);
+            if (i16) k_forward<EPI_F32VOX, true><<<fwd_grid(P, n_long), FWD_THREADS, 0, P->stream>>>(n_long, R.items, R.vox, md, colp, R.valD, R.valL, xd, nullptr, nullptr, none, nullptr, nullptr, nullptr, dd, dl, letd_out, NO_RESID);
+            else k_forward<EPI_F32VOX, false><<<fwd_grid(P, n_long), FWD_THREADS, 0, P->stream>>>(n_long, R.items, R.vox, md, colp, R.valD, R.valL, xd, nullptr, nullptr, none, nullptr, nullptr, nullptr, dd, dl, letd_out, NO_RESID);
             ++P->launches;
         }
     }
@@ -1320,9 +1333,8 @@ int fredopt_proximity(fredopt_plan* P, const float* x, double* prox, int64_t* n_
     const double* xd;
     CKR(resolve_x(P, x, &xd));
     // scratch: Dg / Lg hold the products so that the iteration's d, l are left alone
-    launch_forward(P, P->act, P->mode_con, xd, P->Dg, P->Lg, EPI_STORE);
-    launch_residual(P, P->Dg, P->Lg, 0, 1, 0);
-    launch_finalize(P);
+    launch_forward(P, P->act, P->mode_con, xd, P->Dg, P->Lg, EPI_RESID, 0);     // a11: one pass, statistics only
+    launch_finalize(P, P->act.n ? fwd_grid(P, P->act.n) : 1);
     DevState h;
     CK(cudaMemcpyAsync(&h, P->st, sizeof(DevState), cudaMemcpyDeviceToHost, P->stream));
     CK(cudaStreamSynchronize(P->stream));
@@ -1347,8 +1359,8 @@ static int structure_values(fredopt_plan* P, const float* x, int32_t quantity, i
     const uint8_t* md = P->mode_fixed + (size_t)m * P->max_seg;
     const GatherVec none{nullptr, nullptr, nullptr};
     const int g = fwd_grid(P, nr);
-    if (A.col16) k_forward<EPI_STORE, true><<<g, FWD_THREADS, 0, P->stream>>>(nr, A.items + rb, A.vox + rb, md, A.col16, A.valD, A.valL, xd, P->Dg + rb, P->Lg + rb, none, nullptr, nullptr, nullptr, nullptr, nullptr, 0);
-    else k_forward<EPI_STORE, false><<<g, FWD_THREADS, 0, P->stream>>>(nr, A.items + rb, A.vox + rb, md, A.col, A.valD, A.valL, xd, P->Dg + rb, P->Lg + rb, none, nullptr, nullptr, nullptr, nullptr, nullptr, 0);
+    if (A.col16) k_forward<EPI_STORE, true><<<g, FWD_THREADS, 0, P->stream>>>(nr, A.items + rb, A.vox + rb, md, A.col16, A.valD, A.valL, xd, P->Dg + rb, P->Lg + rb, none, nullptr, nullptr, nullptr, nullptr, nullptr, 0, NO_RESID);
+    else k_forward<EPI_STORE, false><<<g, FWD_THREADS, 0, P->stream>>>(nr, A.items + rb, A.vox + rb, md, A.col, A.valD, A.valL, xd, P->Dg + rb, P->Lg + rb, none, nullptr, nullptr, nullptr, nullptr, nullptr, 0, NO_RESID);
     k_quantity<<<grid_for(nr, 256, 1024), 256, 0, P->stream>>>(nr, quantity, P->Dg + rb, P->Lg + rb, P->uv.cD + rb);
     P->launches += 2;
     CK(cudaGetLastError());
@@ -1488,7 +1500,8 @@ int fredopt_iterate(fredopt_plan* P, int32_t n_iter, float lambda, float beta0, 
         } else {
             for (int it = 0; it < n_iter; ++it) enqueue_iteration(P, sa);
         }
-        if (!P->block_sequential) launch_finalize(P);     // block mode keeps its sweep statistics in the state already
+        if (!P->block_sequential)                         // block mode keeps its sweep statistics in the state already
+            launch_finalize(P, sa ? res_grid(P) : (P->act.n ? fwd_grid(P, P->act.n) : 1));
     }
     CK(cudaGetLastError());
     return FREDOPT_OK;

@@ -4,8 +4,8 @@
 //   k_forward    d = D x, l = L x over a list of work items (one item = one voxel row; one warp per item,
 //                round-robin, 128-bit streamed index/value loads kept out of L1, fp64 accumulation, shuffle
 //                reduction).  A row reads only the value arrays its structure needs.  Epilogues: store d, l
-//                (+ the cost residuals p, q of Eq. 2), the quadratic coefficient c of the accept test, or fp32
-//                dose / LETd per voxel.
+//                (+ the cost residuals p, q of Eq. 2), the quadratic coefficient c of the accept test, the residuals /
+//                violations of Fig. 2 with their statistics (pure feasibility-seeking), or fp32 dose / LETd per voxel.
 //   k_transpose  out_j = sum_i D_ij u_i + L_ij v_i over the stored CSR of the transposes (one item = at most
 //                TR_ITEM_MAX entries of one (structure, spot) run; one warp per item; every item writes its
 //                partial sum to a fixed slot: no atomics, no fences).
@@ -144,8 +144,61 @@ __device__ __forceinline__ void fma4(double& acc, const float4& a, double x0, do
     acc = fma((double)a.w, x3, acc);
 }
 
+// signed residual of a hyperslab lo <= val <= hi (NaN = absent): upper violations > 0, lower < 0
+__device__ __forceinline__ double slab_residual(double val, double lo, double hi) {
+    if (val > hi) return val - hi;      // false when hi is NaN
+    if (val < lo) return val - lo;      // false when lo is NaN
+    return 0.0;
+}
+
+// Residuals of Fig. 2 for one labelled row at (dv, lv) in simultaneous form: the coefficients of D_i and L_i in the step,
+//   u_i = w^ r_dose/|D_i|^2 - LETmax w^ r_letd/|L_i - LETmax D_i|^2 ,  v_i = w^ r_dl/|L_i|^2 + w^ r_letd/|...|^2 ,
+// and the row's share of the violated-set count, the proximity and chi^2.
+__device__ __forceinline__ void row_residual(const StructInfo& T, int one_sided, double dv, double lv, double nD, double nL,
+                                             double nT, double& u, double& v, long long& cnt, double& prox, double& phi) {
+    const int f = T.flags;
+    const double w = T.what;
+    double cD = 0.0, cL = 0.0, cT = 0.0;
+    if (f & F_DOSE_SLAB) {
+        const double r = slab_residual(dv, T.dose_lo, T.dose_hi);
+        if (r != 0.0) { ++cnt; if (nD > 0.0) { cD = w * r / nD; prox += 0.5 * w * r * r / nD; } }
+    }
+    if (f & F_DL_SLAB) {
+        const double r = slab_residual(lv, T.dl_lo, T.dl_hi);
+        if (r != 0.0) { ++cnt; if (nL > 0.0) { cL = w * r / nL; prox += 0.5 * w * r * r / nL; } }
+    }
+    if (f & F_LETD) {
+        const double val = lv - T.letd_max * dv;
+        if (val > 0.0) { ++cnt; if (nT > 0.0) { cT = w * val / nT; prox += 0.5 * w * val * val / nT; } }
+    }
+    if (f & F_DOSE_REF) { const double e = T.dose_ref - dv; phi += w * e * e; }
+    if (f & F_DL_REF) { const double e = T.dl_ref - lv; if (!(one_sided && e > 0.0)) phi += w * e * e; }
+    u = (f & F_LETD) ? cD - T.letd_max * cT : cD;     // row of the LETd set is L_i - LETmax D_i
+    v = cL + cT;
+}
+
+// fixed-order block sum of an integer; result valid in thread 0
+__device__ __forceinline__ long long block_sum_ll(long long c, long long* smc) {
+    for (int o = 16; o > 0; o >>= 1) c += __shfl_down_sync(0xffffffffu, c, o);
+    __syncthreads();
+    if ((threadIdx.x & 31) == 0) smc[threadIdx.x >> 5] = c;
+    __syncthreads();
+    long long t = 0;
+    if (threadIdx.x == 0) for (int i = 0; i < (int)(blockDim.x >> 5); ++i) t += smc[i];
+    return t;
+}
+
+// what the residual epilogue of the forward kernel needs (EPI_RESID)
+struct ResidArgs {
+    const double *nD, *nL, *nT;          // squared norms per labelled row
+    GatherVec uv;                        // out: step coefficients (null pointers: statistics only)
+    double *part_prox, *part_phi;        // out: per-CTA partial sums
+    long long* part_cnt;
+    DevState* st;                        // relax = lambda eta^k, eta^k and k advance when uv is written
+};
+
 // ------------------------------------------------------------------------------------------ forward
-enum : int { EPI_STORE = 0, EPI_STORE_PQ = 1, EPI_CPART = 2, EPI_F32VOX = 3 };
+enum : int { EPI_STORE = 0, EPI_STORE_PQ = 1, EPI_CPART = 2, EPI_F32VOX = 3, EPI_RESID = 4 };
 
 // <D_i, x> and / or <L_i, x> of one row by one warp.  M: bit 0 = D, bit 1 = L.  U 128-entry chunks per trip (6 for a
 // single matrix, 4 for both): up to 12 independent vector loads per lane in flight before the first gather.
@@ -205,12 +258,14 @@ k_forward(long long n, const Item* __restrict__ items, const int32_t* __restrict
           const GatherVec pq,                                              // EPI_STORE_PQ: cost residuals (Eq. 2)
           const StructInfo* __restrict__ tab, double* __restrict__ cpart,  // EPI_STORE_PQ / EPI_CPART
           const DevState* __restrict__ st,                                 // EPI_STORE_PQ (cost form)
-          float* __restrict__ fD, float* __restrict__ fL, int letd_out)    // EPI_F32VOX: voxel-indexed
+          float* __restrict__ fD, float* __restrict__ fL, int letd_out,    // EPI_F32VOX: voxel-indexed
+          const ResidArgs ra)                                              // EPI_RESID: residual / violation epilogue (a7)
 {
     const int lane = threadIdx.x & 31;
     const long long nwarps = (long long)gridDim.x * FWD_WARPS;
     long long r = (long long)blockIdx.x * FWD_WARPS + (threadIdx.x >> 5);
-    double csum = 0.0;
+    double csum = 0.0, rprox = 0.0, rphi = 0.0;
+    long long rcnt = 0;
     Item it;
     if (r < n) it = ld_item(items + r);
     while (r < n) {
@@ -243,6 +298,11 @@ k_forward(long long n, const Item* __restrict__ items, const int32_t* __restrict
                     if (T.flags & F_DOSE_REF) csum += T.what * aD * aD;
                     if (T.flags & F_DL_REF) csum += T.what * aL * aL;
                 }
+                if (EPI == EPI_RESID) {         // residuals / violations of Fig. 2 at x, in the epilogue of the fused pass
+                    double u, v;
+                    row_residual(tab[it.seg], ra.st->flags & SF_ONE_SIDED, aD, aL, ra.nD[r], ra.nL[r], ra.nT[r], u, v, rcnt, rprox, rphi);
+                    if (ra.uv.pair) gv_store(ra.uv, r, u, v);
+                }
             }
         }
         r = rn;
@@ -253,6 +313,21 @@ k_forward(long long n, const Item* __restrict__ items, const int32_t* __restrict
         // lane 0 of each warp carries that warp's sum; other lanes carry 0
         const double t = block_sum(csum, sm);
         if (threadIdx.x == 0) cpart[blockIdx.x] = t;
+    }
+    if (EPI == EPI_RESID) {
+        __shared__ double sm[FWD_WARPS];
+        __shared__ long long smc[FWD_WARPS];
+        const double p = block_sum(rprox, sm);
+        const double q = block_sum(rphi, sm);
+        const long long c = block_sum_ll(rcnt, smc);
+        if (threadIdx.x == 0) {
+            ra.part_prox[blockIdx.x] = p; ra.part_phi[blockIdx.x] = q; ra.part_cnt[blockIdx.x] = c;
+            if (blockIdx.x == 0 && ra.uv.pair) {               // w_k = eta^k w: relax for this step
+                ra.st->relax = ra.st->lambda * ra.st->eta_pow;
+                ra.st->eta_pow *= ra.st->eta;
+                ra.st->k += 1;
+            }
+        }
     }
 }
 
@@ -517,13 +592,6 @@ k_select(DevState* st, const double* __restrict__ gpart, int n_gpart, const doub
     }
 }
 
-// signed residual of a hyperslab lo <= val <= hi (NaN = absent): upper violations > 0, lower < 0
-__device__ __forceinline__ double slab_residual(double val, double lo, double hi) {
-    if (val > hi) return val - hi;      // false when hi is NaN
-    if (val < lo) return val - lo;      // false when lo is NaN
-    return 0.0;
-}
-
 // Per active row: apply the accepted perturbation to the stored products (d' = d - beta Dg, l' = l - beta Lg) and
 // per spot to the weights (x' = x - beta g); then, if `final`, the residuals of Fig. 2 in simultaneous form at x':
 //   u_i = w^ r_dose/|D_i|^2 - LETmax w^ r_letd/|L_i - LETmax D_i|^2 ,  v_i = w^ r_dl/|L_i|^2 + w^ r_letd/|...|^2
@@ -560,25 +628,9 @@ k_residual(long long n, const Item* __restrict__ items, const StructInfo* __rest
             gv_store(pq, a, pv, qv);
             continue;
         }
-        double cD = 0.0, cL = 0.0, cT = 0.0;
-        if (f & (F_DOSE_SLAB)) {
-            const double r = slab_residual(dv, T.dose_lo, T.dose_hi);
-            if (r != 0.0) { ++cnt; const double nn = nD[a]; if (nn > 0.0) { cD = w * r / nn; prox += 0.5 * w * r * r / nn; } }
-        }
-        if (f & (F_DL_SLAB)) {
-            const double r = slab_residual(lv, T.dl_lo, T.dl_hi);
-            if (r != 0.0) { ++cnt; const double nn = nL[a]; if (nn > 0.0) { cL = w * r / nn; prox += 0.5 * w * r * r / nn; } }
-        }
-        if (f & (F_LETD)) {
-            const double val = lv - T.letd_max * dv;
-            if (val > 0.0) { ++cnt; const double nn = nT[a]; if (nn > 0.0) { cT = w * val / nn; prox += 0.5 * w * val * val / nn; } }
-        }
-        if (f & F_DOSE_REF) { const double e = T.dose_ref - dv; phi += w * e * e; }
-        if (f & F_DL_REF) { const double e = T.dl_ref - lv; if (!((st->flags & SF_ONE_SIDED) && e > 0.0)) phi += w * e * e; }
-        if (write_uv) {
-            gv_store(uv, a, (f & F_LETD) ? cD - T.letd_max * cT : cD,      // row of the LETd set is L_i - LETmax D_i
-                     cL + cT);
-        }
+        double uu, vv;
+        row_residual(T, st->flags & SF_ONE_SIDED, dv, lv, nD[a], nL[a], nT[a], uu, vv, cnt, prox, phi);
+        if (write_uv) gv_store(uv, a, uu, vv);
     }
     if (final) {
         const double p = block_sum(prox, sm);
