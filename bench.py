@@ -254,10 +254,10 @@ def run_ours(args):
     peak, peak_src = _peaks()
     achieved = pass_bytes[top] / (top_ms * 1e-3) / 1e9
     passes = {n: {"ms": pt[n][0] / max(pt[n][1], 1), "alg_bytes": pass_bytes[n],
-                  "gbs": pass_bytes[n] / max(pt[n][0] / max(pt[n][1], 1), 1e-9) / 1e6} for n in pt}
+                  "gbs": pass_bytes[n] / max(pt[n][0] / max(pt[n][1], 1), 1e-9) / 1e6} for n in pt if pt[n][1] > 0}
     stats = gp.stats()
     spmv = ("forward_x", "transpose_b") if args.ams else ("forward_x", "transpose_g", "forward_g", "transpose_b")
-    four_gbs = sum(pass_bytes[n] for n in spmv) / max(sum(passes[n]["ms"] for n in spmv), 1e-9) / 1e6
+    four_gbs = sum(pass_bytes[n] for n in spmv if n in passes) / max(sum(passes[n]["ms"] for n in spmv if n in passes), 1e-9) / 1e6
 
     ms, e2e_s = max_over_ranks([ms, e2e_s], dist, "cuda")
     if rank != 0:
