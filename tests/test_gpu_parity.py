@@ -225,6 +225,32 @@ def test_random_small_plans_union_pattern(fredopt, seed, same):
     _assert_state(gp, orc)
 
 
+def test_more_than_65536_spots_uses_32_bit_columns(fredopt):
+    """n_cols > 65536: the forward kernels read int32 column indices while the transposes keep 16-bit row indices."""
+    V, S, per_row = 500, 70000, 40
+    u = pg.uniform01_array(77, V * per_row * 3 + V)
+    cols = np.sort((u[:V * per_row].reshape(V, per_row) * (S // per_row)).astype(np.int64) + np.arange(per_row) * (S // per_row), axis=1)
+    rp = np.arange(V + 1, dtype=np.int64) * per_row
+    ci = cols.reshape(-1).astype(np.int32)
+    vd = (0.05 + u[V * per_row:2 * V * per_row]).astype(np.float32)
+    vl = (vd * (2.0 + 6.0 * u[2 * V * per_row:3 * V * per_row])).astype(np.float32)
+    lab = (np.floor(u[3 * V * per_row:] * 3)).astype(np.int32)
+    nan = np.nan
+    bounds = np.array([[1.0, 8.0, 11.0, nan, nan, nan, 10.0, nan],
+                       [1.0, nan, 9.0, nan, 40.0, 4.5, nan, 35.0]], np.float32)
+    assert ci.max() > 65536
+    orc = _oracle_np(V, S, (rp, ci, vd), (rp, ci, vl), lab, bounds)
+    gp = fredopt.Plan(V, S, (rp, ci, vd), (rp, ci, vl), lab, bounds)
+    x0 = (0.2 + 0.5 * pg.uniform01_array(78, S)).astype(np.float32)
+    d_ref, l_ref, _ = orc.dose_let(x0.astype(np.float64))
+    d = np.empty(V, np.float32); l = np.empty(V, np.float32)
+    gp.spmv_forward(fredopt.ROWS_ALL, x0, d, l)
+    _assert_fwd(d, d_ref, "D x"); _assert_fwd(l, l_ref, "L x")
+    orc.set_x(x0); gp.set_weights(x0)
+    orc.iterate(20, 1.0, 1.0, 0.9); gp.iterate(20, 1.0, 1.0, 0.9)
+    _assert_state(gp, orc)
+
+
 def test_degenerate_inputs(fredopt):
     f = fredopt
     nan = np.nan
@@ -464,6 +490,14 @@ def _full_size_parity(fredopt, plan, n_sample_rows):
                                      None if vv is None else vv.astype(np.float64), active_only=True)
         gp.spmv_transpose(fredopt.ROWS_ACTIVE, uu, vv, out)
         assert np.all(np.abs(out - ref) <= TOL_SPMV * ref_abs)
+    # block-sequential form (R23) from the same state, and the evaluation quantities of the PTV and one OAR
+    from oracle import oracle as om
+    gp.set_option(fredopt.OPT_BLOCK_SEQUENTIAL, 1); orc.set_option(om.OPT_BLOCK_SEQUENTIAL, 1)
+    gp.iterate(5, sp.lam, sp.beta0, sp.a); orc.iterate(5, sp.lam, sp.beta0, sp.a)
+    _assert_block_state(gp, orc)
+    for label, q in ((1, 0), (2, 1), (2, 2)):
+        v, vo = gp.percentile_value(q, label, 0.3), orc.percentile_value(q, label, 0.3)
+        assert abs(v - vo) <= 1e-12 * max(abs(vo), 1e-30)
     gp.destroy()
 
 
