@@ -86,7 +86,8 @@ typedef struct {
     int64_t nnz_active;         /* non-zeros in active rows                                                */
     int64_t alg_bytes_iter;     /* algorithmic bytes of ONE superiorized iteration ("Bytes")    */
     double  last_beta;          /* last accepted beta (0 if none)                                          */
-    double  phi;                /* chi^2 at the perturbed point of the last iteration                      */
+    double  phi;                /* chi^2 at the perturbed point of the last iteration (superiorized,       */
+                                /*   simultaneous form; otherwise over the rows the last pass visited)     */
     double  prox;               /* proximity 1/2 sum w^ r^2/|a|^2 at that same point / last proximity call */
     double  weight_sum;         /* W: sum of the weights of the participating sets                         */
 } fredopt_stats;
