@@ -61,8 +61,13 @@ class Stats(C.Structure):
 
 def _load():
     if not os.path.exists(LIB_PATH):
-        raise ImportError(f"{LIB_PATH} is missing: build it with `python -m paper_2509_20012_b200.build` "
-                          "(there is no CPU fallback)")
+        # a fresh checkout has no built library (it is git-ignored): compile it in-tree with nvcc, or fail loudly
+        try:
+            from . import build as _build
+            _build.build_library()
+        except Exception as e:
+            raise ImportError(f"{LIB_PATH} is missing and could not be built ({e}); build it with "
+                              "`python -m paper_2509_20012_b200.build` (there is no CPU fallback)") from e
     lib = C.CDLL(LIB_PATH)
     vp, i64, i32, f32, f64 = C.c_void_p, C.c_int64, C.c_int32, C.c_float, C.c_double
     lib.fredopt_create.argtypes = [C.POINTER(_Csr), C.POINTER(_Csr), vp, C.POINTER(_Bounds), i32, vp, C.POINTER(vp)]
