@@ -93,7 +93,7 @@ struct fredopt_plan {
     // full: all non-empty rows of the padded matrix (union pattern); act: a compact copy of the rows with a label,
     // ordered by (structure, voxel)
     RowSet full, act;
-    long long full_class[5] = {0, 0, 0, 0, 0};   // rows of length class c of `full`: full_class[c] .. full_class[c+1]-1
+    long long full_class[9] = {0, 0, 0, 0, 0, 0, 0, 0, 0};   // rows of length class c of `full`: full_class[c] .. full_class[c+1]-1
     // per active row
     double *nD = nullptr, *nL = nullptr, *nT = nullptr;
     // tables
@@ -260,9 +260,13 @@ __global__ void k_compact_rows(const int32_t* flag, const int32_t* pos, const lo
     }
 }
 
-// length class of a row of the full set: 0 = more than 64 entries (whole warp per row), 1 = 33..64 (16 lanes per row),
-// 2 = 17..32 (8 lanes), 3 = at most 16 (4 lanes)
-__host__ __device__ inline int len_class(long long padded) { return padded > 64 ? 0 : padded > 32 ? 1 : padded > 16 ? 2 : 3; }
+// length class of a row of the full set, longest first: 0..4 = more than 1024 / 512 / 256 / 128 / 64 entries (whole warp
+// per row; the classes keep the static round-robin balanced), 5 = 33..64 (16 lanes per row), 6 = 17..32 (8 lanes),
+// 7 = at most 16 (4 lanes)
+constexpr int N_LEN_CLASS = 8, FIRST_SHORT_CLASS = 5;
+__host__ __device__ inline int len_class(long long padded) {
+    return padded > 1024 ? 0 : padded > 512 ? 1 : padded > 256 ? 2 : padded > 128 ? 3 : padded > 64 ? 4 : padded > 32 ? 5 : padded > 16 ? 6 : 7;
+}
 __global__ void k_class_keys(const int32_t* vox, const long long* ptr, long long n, int32_t* key, unsigned long long* hist) {
     for (long long a = (long long)blockIdx.x * blockDim.x + threadIdx.x; a < n; a += (long long)gridDim.x * blockDim.x) {
         const long long i = vox[a];
@@ -1033,23 +1037,23 @@ static int create_impl(fredopt_plan* P, const fredopt_csr* D, const fredopt_csr*
         CK(cudaMalloc(&key1, ((size_t)n_ne + 1) * 4)); tmp.push_back(key1);
         CK(cudaMalloc(&flen64, ((size_t)n_ne + 1) * 8)); tmp.push_back(flen64);
         CK(cudaMalloc(&fstart, ((size_t)n_ne + 1) * 8)); tmp.push_back(fstart);
-        CK(cudaMalloc(&hist, 4 * 8)); tmp.push_back(hist);
-        CK(cudaMemsetAsync(hist, 0, 4 * 8, st));
+        CK(cudaMalloc(&hist, N_LEN_CLASS * 8)); tmp.push_back(hist);
+        CK(cudaMemsetAsync(hist, 0, N_LEN_CLASS * 8, st));
         if (V) k_compact_rows<<<grid_for(V, 256, 1 << 16), 256, 0, st>>>(f_ne, pos_ne, pU, pstart, lab, V, vox0, nullptr, nullptr, nullptr, nullptr);
         if (n_ne) k_class_keys<<<grid_for(n_ne, 256, 1 << 16), 256, 0, st>>>(vox0, pU, n_ne, key0, hist);
         size_t tb = 0;
-        CK(cub::DeviceRadixSort::SortPairs(nullptr, tb, key0, key1, vox0, F.vox, n_ne, 0, 2, st));
+        CK(cub::DeviceRadixSort::SortPairs(nullptr, tb, key0, key1, vox0, F.vox, n_ne, 0, 3, st));
         void* t2; CK(cudaMalloc(&t2, tb ? tb : 1)); tmp.push_back(t2);
-        CK(cub::DeviceRadixSort::SortPairs(t2, tb, key0, key1, vox0, F.vox, n_ne, 0, 2, st));   // stable: voxel order inside a class
+        CK(cub::DeviceRadixSort::SortPairs(t2, tb, key0, key1, vox0, F.vox, n_ne, 0, 3, st));   // stable: voxel order inside a class
         if (n_ne) k_fill_active<<<grid_for(n_ne, 256, 1 << 16), 256, 0, st>>>(F.vox, nullptr, pU, pstart, n_ne, fstart, F.len, F.ulen, nullptr);
         CK(cudaMemsetAsync(flen64, 0, ((size_t)n_ne + 1) * 8, st));
         if (n_ne) k_i32_to_i64<<<grid_for(n_ne, 256, 4096), 256, 0, st>>>(F.len, flen64, n_ne);
         CKR(scan_exclusive(P, flen64, F.start, (long long)n_ne + 1));
-        unsigned long long hh[4];
-        CK(cudaMemcpyAsync(hh, hist, 4 * 8, cudaMemcpyDeviceToHost, st));
+        unsigned long long hh[N_LEN_CLASS];
+        CK(cudaMemcpyAsync(hh, hist, N_LEN_CLASS * 8, cudaMemcpyDeviceToHost, st));
         CK(cudaStreamSynchronize(st));
         P->full_class[0] = 0;
-        for (int c = 0; c < 4; ++c) P->full_class[c + 1] = P->full_class[c] + (long long)hh[c];
+        for (int c = 0; c < N_LEN_CLASS; ++c) P->full_class[c + 1] = P->full_class[c] + (long long)hh[c];
         if (n_ne) {
             k_copy_padded<<<grid_for((long long)n_ne * 32, 256, 1 << 16), 256, 0, st>>>(F.n, F.vox, F.start, pU, cU, uD, uL, F.col, F.valD, F.valL);
             k_pack_items<<<grid_for(n_ne, 256, 4096), 256, 0, st>>>(n_ne, F.start, F.len, nullptr, F.items);
@@ -1257,8 +1261,9 @@ static int forward_f32(fredopt_plan* P, const RowSet& R, int m, const double* xd
         const void* colp = i16 ? (const void*)R.col16 : (const void*)R.col;
         long long n_long = R.n;
         if (&R == &P->full) {   // short rows by sub-warps (4 / 8 / 16 lanes per row), long rows by whole warps
-            n_long = P->full_class[1];
-            const long long b[4] = {P->full_class[1], P->full_class[2], P->full_class[3], P->full_class[4]};
+            n_long = P->full_class[FIRST_SHORT_CLASS];
+            const long long b[4] = {P->full_class[FIRST_SHORT_CLASS], P->full_class[FIRST_SHORT_CLASS + 1], P->full_class[FIRST_SHORT_CLASS + 2],
+                                    P->full_class[FIRST_SHORT_CLASS + 3]};
 #define SHORT_LAUNCH(G, LO, HI)                                                                                                  \
     if (HI > LO) {                                                                                                               \
         const int gg = fwd_grid(P, ((HI) - (LO) + (32 / G) - 1) / (32 / G));                                                    \
