@@ -503,7 +503,7 @@ def sweep_spec(sigma: float, pitch: float, n_layers: int, seed: int = 0, scale: 
 def random_small_plan(seed: int, V: int = 40, S: int = 8, n_struct: int = 3, density: float = 0.4,
                       same_pattern: bool = True):
     """Tiny random CSR problem for brute-force checks (numpy arrays).  Not plan-shaped on purpose."""
-    u = uniform01_array(seed, 4 * V * S + V + 64)
+    u = uniform01_array(seed, 4 * V * S + V + S + 64)
     k = 0
     mask = (u[k:k + V * S] < density).reshape(V, S); k += V * S
     Dd = (0.05 + u[k:k + V * S]).reshape(V, S) * mask; k += V * S

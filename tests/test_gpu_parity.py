@@ -225,6 +225,38 @@ def test_random_small_plans_union_pattern(fredopt, seed, same):
     _assert_state(gp, orc)
 
 
+@pytest.mark.parametrize("seed", list(range(20, 32)))
+def test_random_bound_combinations(fredopt, seed):
+    """Random presence / absence of every bound and cost reference per structure, random weights, both AMS forms, ragged
+    shapes (V, S not multiples of anything), differing D / L patterns on odd seeds."""
+    from oracle import oracle as om
+    u = pg.uniform01_array(1000 + seed, 64)
+    V, S, ns = 150 + int(u[0] * 400), 5 + int(u[1] * 90), 1 + int(u[2] * 5)
+    D, L, lab, x0 = pg.random_small_plan(seed, V=V, S=S, n_struct=ns, density=0.15 + 0.5 * u[3], same_pattern=seed % 2 == 0)
+    nan = np.nan
+    rows = []
+    for s_ in range(ns):
+        r = pg.uniform01_array(2000 + seed * 16 + s_, 12)
+        lo, hi = 0.2 + 0.6 * r[0], 1.0 + 0.8 * r[1]
+        rows.append([0.25 + 2.0 * r[2],
+                     lo if r[3] < 0.5 else nan, hi if r[4] < 0.6 else nan,
+                     2.0 * lo if r[5] < 0.3 else nan, 3.0 * hi if r[6] < 0.5 else nan,
+                     2.0 + 3.0 * r[7] if r[8] < 0.5 else nan,
+                     0.5 * (lo + hi) if r[9] < 0.6 else nan, 2.5 * hi if r[10] < 0.5 else nan])
+    bounds = np.array(rows, np.float32)
+    for block in (0, 1):
+        orc = _oracle_np(V, S, D, L, lab, bounds)
+        gp = fredopt.Plan(V, S, D, L, lab, bounds)
+        gp.set_option(fredopt.OPT_BLOCK_SEQUENTIAL, block); orc.set_option(om.OPT_BLOCK_SEQUENTIAL, block)
+        orc.set_x(x0); gp.set_weights(x0)
+        orc.iterate(20, 1.3, 0.8, 0.85); gp.iterate(20, 1.3, 0.8, 0.85)
+        if block:
+            _assert_block_state(gp, orc)
+        else:
+            _assert_state(gp, orc)
+        gp.destroy()
+
+
 def test_more_than_65536_spots_uses_32_bit_columns(fredopt):
     """n_cols > 65536: the forward kernels read int32 column indices while the transposes keep 16-bit row indices."""
     V, S, per_row = 500, 70000, 40
