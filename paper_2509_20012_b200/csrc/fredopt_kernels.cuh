@@ -24,7 +24,10 @@ constexpr int FWD_THREADS = 256;
 constexpr int FWD_WARPS = FWD_THREADS / 32;
 constexpr int MAX_PARTIALS = 2368;          // 148 SMs x 16 CTAs: upper bound of any partial-sum grid
 constexpr int ROW_THREADS = 256;
-constexpr int TR_ITEM_MAX = 2048;           // entries per transposed work item (multiple of 4)
+#ifndef TR_ITEM_MAX_ENTRIES
+#define TR_ITEM_MAX_ENTRIES 2048   /* measured on configs[3]: 1024 -> -3 %, 4096 -> -0.3 %; on configs[1]: 4096 -> -7 % */
+#endif
+constexpr int TR_ITEM_MAX = TR_ITEM_MAX_ENTRIES;   // entries per transposed work item (multiple of 128)
 #ifndef FWD_U1
 #define FWD_U1 6   /* 128-entry chunks in flight per trip for rows that read one matrix ... */
 #endif
