@@ -117,6 +117,7 @@ struct fredopt_plan {
     double eta = 1.0;
     long long reductionsN = 1, max_trials = 200;
     int accept_check = 1, use_graph = 1, time_passes = 0, block_sequential = 0, normalize_grad = 0, one_sided_cost = 0;
+    int use_pdl = 1;
     bool started = false;
     float latched_beta0 = 0.f;
     long long launches = 0;
@@ -714,6 +715,20 @@ static void ev_end(fredopt_plan* P) {
     cudaEventRecord(P->events.back().b, P->stream);
 }
 
+// Launch one kernel of an iteration on the plan's stream.  With programmatic dependent launch (default) the kernel may be
+// scheduled while its predecessor drains; it waits (griddepcontrol.wait at its top) before touching any data.
+template <typename... KA, typename... A>
+static void klaunch(fredopt_plan* P, void (*kern)(KA...), int grid, int block, A... args) {
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3((unsigned)grid); cfg.blockDim = dim3((unsigned)block); cfg.dynamicSmemBytes = 0; cfg.stream = P->stream;
+    cudaLaunchAttribute at;
+    at.id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    at.val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = &at; cfg.numAttrs = P->use_pdl ? 1 : 0;
+    cudaLaunchKernelEx(&cfg, kern, KA(args)...);
+    ++P->launches;
+}
+
 // grid of the item kernels: one warp per item up to FWD_CTAS_PER_SM resident-CTA-fulls per SM (then round-robin)
 constexpr int FWD_CTAS_PER_SM = 2 * FWD_MIN_CTAS;   // 2 waves of the CTAs an SM holds (launch bounds of k_forward / k_transpose)
 static int fwd_grid(fredopt_plan* P, long long n) {
@@ -731,7 +746,7 @@ static void launch_forward(fredopt_plan* P, const RowSet& R, const uint8_t* mode
         if (epi == EPI_CPART) cudaMemsetAsync(P->cpart, 0, sizeof(double) * MAX_PARTIALS, P->stream);
         if (epi == EPI_RESID) {   // nothing to visit: zero statistics (finalize reads one partial)
             cudaMemsetAsync(P->part_prox, 0, 8, P->stream); cudaMemsetAsync(P->part_phi, 0, 8, P->stream); cudaMemsetAsync(P->part_cnt, 0, 8, P->stream);
-            if (write_uv) { k_sweep_end<<<grid_for(P->S, 256, 1 << 30), 256, 0, P->stream>>>(P->S, P->x, P->st); ++P->launches; }   // k, eta^k still advance
+            if (write_uv) klaunch(P, k_sweep_end, grid_for(P->S, 256, 1 << 30), 256, P->S, P->x, P->st);   // k, eta^k still advance
         }
         return;
     }
@@ -740,8 +755,8 @@ static void launch_forward(fredopt_plan* P, const RowSet& R, const uint8_t* mode
     ResidArgs ra = NO_RESID;
     if (epi == EPI_RESID) ra = ResidArgs{P->nD, P->nL, P->nT, write_uv ? P->uv : none, P->part_prox, P->part_phi, P->part_cnt, P->st};
 #define FWD_LAUNCH(E, I16, COL, PQ, TAB, CP)                                                                                   \
-    k_forward<E, I16><<<g, FWD_THREADS, 0, P->stream>>>(R.n, R.items, R.vox, mode, COL, R.valD, R.valL, x, oD, oL, PQ, TAB, CP, \
-                                                       P->st, nullptr, nullptr, 0, ra)
+    klaunch(P, k_forward<E, I16>, g, FWD_THREADS, R.n, R.items, R.vox, mode, COL, R.valD, R.valL, x, oD, oL, PQ, TAB, CP, P->st, \
+            nullptr, nullptr, 0, ra)
     if (R.col16) {
         if (epi == EPI_CPART) FWD_LAUNCH(EPI_CPART, true, R.col16, none, P->tab, P->cpart);
         else if (epi == EPI_STORE_PQ) FWD_LAUNCH(EPI_STORE_PQ, true, R.col16, P->pq, P->tab, nullptr);
@@ -754,7 +769,6 @@ static void launch_forward(fredopt_plan* P, const RowSet& R, const uint8_t* mode
         else FWD_LAUNCH(EPI_STORE, false, R.col, none, nullptr, nullptr);
     }
 #undef FWD_LAUNCH
-    ++P->launches;
 }
 static int cpart_count(fredopt_plan* P) { return P->act.n ? fwd_grid(P, P->act.n) : MAX_PARTIALS; }
 
@@ -763,13 +777,12 @@ static void launch_transpose(fredopt_plan* P, const RowSet& R, const uint8_t* mo
                              float* f_out) {
     if (R.t_n_items == 0) return;
     if (R.t_col16)
-        k_transpose<true><<<fwd_grid(P, R.t_n_items), FWD_THREADS, 0, P->stream>>>(R.t_n_items, R.t_items, R.t_item_slot, mode, R.t_col16,
-                                                                                     R.t_valD, R.t_valL, vec, R.t_partial);
+        klaunch(P, k_transpose<true>, fwd_grid(P, R.t_n_items), FWD_THREADS, R.t_n_items, R.t_items, R.t_item_slot, mode, R.t_col16,
+                R.t_valD, R.t_valL, vec, R.t_partial);
     else
-        k_transpose<false><<<fwd_grid(P, R.t_n_items), FWD_THREADS, 0, P->stream>>>(R.t_n_items, R.t_items, R.t_item_slot, mode, R.t_col,
-                                                                                      R.t_valD, R.t_valL, vec, R.t_partial);
-    k_combine<EPI><<<grid_for(P->S, 256, 1 << 30), 256, 0, P->stream>>>(P->S, R.t_item_ptr, R.t_partial, g_out, P->gpart, x, P->st, f_out);
-    P->launches += 2;
+        klaunch(P, k_transpose<false>, fwd_grid(P, R.t_n_items), FWD_THREADS, R.t_n_items, R.t_items, R.t_item_slot, mode, R.t_col,
+                R.t_valD, R.t_valL, vec, R.t_partial);
+    klaunch(P, k_combine<EPI>, grid_for(P->S, 256, 1 << 30), 256, P->S, R.t_item_ptr, R.t_partial, g_out, P->gpart, x, P->st, f_out);
 }
 
 static int res_grid(fredopt_plan* P) {
@@ -780,24 +793,20 @@ static int res_grid(fredopt_plan* P) {
 
 static void launch_residual(fredopt_plan* P, double* d, double* l, int use_beta, int final, int write_uv) {
     const int g = res_grid(P);
-    k_residual<<<g, ROW_THREADS, 0, P->stream>>>(P->act.n, P->act.items, P->tab, P->st, d, l, P->Dg, P->Lg, P->nD, P->nL, P->nT, P->uv,
-                                                 P->pq, P->x, P->g, P->S, P->part_prox, P->part_phi, P->part_cnt, use_beta, final,
-                                                 write_uv);
-    ++P->launches;
+    klaunch(P, k_residual, g, ROW_THREADS, P->act.n, P->act.items, P->tab, P->st, d, l, P->Dg, P->Lg, P->nD, P->nL, P->nT, P->uv, P->pq,
+            P->x, P->g, P->S, P->part_prox, P->part_phi, P->part_cnt, use_beta, final, write_uv);
 }
 
 // n_part: how many per-CTA partial sums the last residual pass wrote (k_residual: res_grid; forward epilogue: fwd_grid)
 static void launch_finalize(fredopt_plan* P, int n_part) {
-    k_finalize_stats<<<1, 1024, 0, P->stream>>>(P->st, P->part_prox, P->part_phi, P->part_cnt, n_part);
-    ++P->launches;
+    klaunch(P, k_finalize_stats, 1, 1024, P->st, P->part_prox, P->part_phi, P->part_cnt, n_part);
 }
 
 // Block-sequential AMS sweep (reading R23): Fig. 2's loop nest -- dose kind over the structures, then cDLET, then the LETd
 // rows -- one (forward over the block's rows, residual, transposed over the block's items, update) group per block.
 static void enqueue_block_sweep(fredopt_plan* P) {
     const RowSet& A = P->act;
-    k_sweep_begin<<<1, 1, 0, P->stream>>>(P->st);
-    ++P->launches;
+    klaunch(P, k_sweep_begin, 1, 1, P->st);
     std::vector<long long> row_begin((size_t)P->n_struct + 1, 0);
     for (int s = 0; s < P->n_struct; ++s) row_begin[s + 1] = row_begin[s] + (long long)P->h_tab[s].rows;
     const int kind_flag[3] = {F_DOSE_SLAB, F_DL_SLAB, F_LETD};
@@ -813,16 +822,13 @@ static void enqueue_block_sweep(fredopt_plan* P) {
             ev_begin(P, FREDOPT_PASS_FORWARD_X);
             {
                 const int g = fwd_grid(P, nr);
-                if (A.col16) k_forward<EPI_STORE, true><<<g, FWD_THREADS, 0, P->stream>>>(nr, A.items + rb, A.vox + rb, md, A.col16, A.valD, A.valL, P->x, P->d + rb, P->l + rb, none, nullptr, nullptr, nullptr, nullptr, nullptr, 0, NO_RESID);
-                else k_forward<EPI_STORE, false><<<g, FWD_THREADS, 0, P->stream>>>(nr, A.items + rb, A.vox + rb, md, A.col, A.valD, A.valL, P->x, P->d + rb, P->l + rb, none, nullptr, nullptr, nullptr, nullptr, nullptr, 0, NO_RESID);
-                ++P->launches;
+                if (A.col16) klaunch(P, k_forward<EPI_STORE, true>, g, FWD_THREADS, nr, A.items + rb, A.vox + rb, md, A.col16, A.valD, A.valL, P->x, P->d + rb, P->l + rb, none, nullptr, nullptr, nullptr, nullptr, nullptr, 0, NO_RESID);
+                else klaunch(P, k_forward<EPI_STORE, false>, g, FWD_THREADS, nr, A.items + rb, A.vox + rb, md, A.col, A.valD, A.valL, P->x, P->d + rb, P->l + rb, none, nullptr, nullptr, nullptr, nullptr, nullptr, 0, NO_RESID);
             }
             ev_end(P);
             ev_begin(P, FREDOPT_PASS_RESIDUAL);
             const int gr = grid_for(nr, ROW_THREADS, P->sm_count * 4 < MAX_PARTIALS ? P->sm_count * 4 : MAX_PARTIALS);
-            k_block_residual<<<gr, ROW_THREADS, 0, P->stream>>>(rb, re, s, kind, P->tab, P->st, P->d, P->l, P->nD, P->nL, P->nT, P->uv,
-                                                               P->part_prox);
-            ++P->launches;
+            klaunch(P, k_block_residual, gr, ROW_THREADS, rb, re, s, kind, P->tab, P->st, P->d, P->l, P->nD, P->nL, P->nT, P->uv, P->part_prox);
             ev_end(P);
             const long long m = (long long)T.part_kind[kind];
             const long long ib = A.t_seg_item_begin.empty() ? 0 : A.t_seg_item_begin[s], ie = A.t_seg_item_begin.empty() ? 0 : A.t_seg_item_begin[s + 1];
@@ -830,18 +836,15 @@ static void enqueue_block_sweep(fredopt_plan* P) {
             ev_begin(P, FREDOPT_PASS_TRANSPOSE_B);
             if (ie > ib) {
                 const int g = fwd_grid(P, ie - ib);
-                if (A.t_col16) k_transpose<true><<<g, FWD_THREADS, 0, P->stream>>>(ie - ib, A.t_items_seg + ib, A.t_slot_seg + ib, md, A.t_col16, A.t_valD, A.t_valL, P->uv, A.t_partial);
-                else k_transpose<false><<<g, FWD_THREADS, 0, P->stream>>>(ie - ib, A.t_items_seg + ib, A.t_slot_seg + ib, md, A.t_col, A.t_valD, A.t_valL, P->uv, A.t_partial);
-                ++P->launches;
+                if (A.t_col16) klaunch(P, k_transpose<true>, g, FWD_THREADS, ie - ib, A.t_items_seg + ib, A.t_slot_seg + ib, md, A.t_col16, A.t_valD, A.t_valL, P->uv, A.t_partial);
+                else klaunch(P, k_transpose<false>, g, FWD_THREADS, ie - ib, A.t_items_seg + ib, A.t_slot_seg + ib, md, A.t_col, A.t_valD, A.t_valL, P->uv, A.t_partial);
             }
             const double factor = (T.w < 1.0 ? T.w : 1.0) / (double)m;
-            k_combine_block<<<grid_for(P->S, 256, 1 << 30), 256, 0, P->stream>>>(P->S, A.t_slot_ptr, s, A.n_seg, A.t_H, A.t_partial, P->x, P->st,
-                                                                                 factor, P->part_prox, gr);
-            ++P->launches;
+            klaunch(P, k_combine_block, grid_for(P->S, 256, 1 << 30), 256, P->S, A.t_slot_ptr, s, A.n_seg, A.t_H, A.t_partial, P->x, P->st, factor,
+                    P->part_prox, gr);
             ev_end(P);
         }
-    k_sweep_end<<<grid_for(P->S, 256, 1 << 30), 256, 0, P->stream>>>(P->S, P->x, P->st);
-    ++P->launches;
+    klaunch(P, k_sweep_end, grid_for(P->S, 256, 1 << 30), 256, P->S, P->x, P->st);
 }
 
 // one iteration of Fig. 3 around the simultaneous Fig. 2 step; returns the number of kernels enqueued
@@ -859,9 +862,8 @@ static int enqueue_iteration(fredopt_plan* P, bool sa) {
             launch_forward(P, P->act, P->mode_union, P->g, P->Dg, P->Lg, EPI_CPART);                   // a5: Dg, Lg, c
             ev_end(P);
             ev_begin(P, FREDOPT_PASS_SELECT);
-            k_select<<<1, 1024, 0, P->stream>>>(P->st, P->gpart, P->act.t_n_items ? grid_for(P->S, 256, 1 << 30) : 0, P->cpart, cpart_count(P), P->act.n, P->act.items, P->tab, P->d, P->l,
-                                               P->Dg, P->Lg);                                             // a4, a6: beta
-            ++P->launches;
+            klaunch(P, k_select, 1, 1024, P->st, P->gpart, P->act.t_n_items ? grid_for(P->S, 256, 1 << 30) : 0, P->cpart, cpart_count(P), P->act.n,
+                    P->act.items, P->tab, P->d, P->l, P->Dg, P->Lg);                                     // a4, a6: beta
             ev_end(P);
             ev_begin(P, FREDOPT_PASS_RESIDUAL);
             const int last = t == P->reductionsN - 1 && !P->block_sequential;
@@ -1172,6 +1174,7 @@ int fredopt_create(const fredopt_csr* D, const fredopt_csr* L, const int32_t* vo
     }
     P->device = dev;
     P->sm_count = prop.multiProcessorCount;
+    if (getenv("FREDOPT_NO_PDL")) P->use_pdl = 0;
     int rc = create_impl(P, D, L, voxel_labels, bounds, n_struct);
     if (rc != FREDOPT_OK) { fredopt_destroy(P); return rc; }
     *out = P;

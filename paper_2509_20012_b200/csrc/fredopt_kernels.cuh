@@ -88,6 +88,14 @@ __device__ __forceinline__ void gv_store(const GatherVec& g, long long a, double
     g.pair[a] = v; g.cD[a] = vd; g.cL[a] = vl;
 }
 
+// Programmatic dependent launch (griddepcontrol, sm_90+): the kernels of one iteration are launched with programmatic
+// stream serialization, so a kernel's CTAs may be scheduled while its predecessor drains.  pdl_wait() returns when the
+// predecessor grid has completed and its writes are visible (a no-op for an ordinary launch); pdl_trigger() lets the
+// successor start being scheduled.  Every kernel waits before it touches anything another kernel writes, and triggers
+// only after its own wait, so kernel N+2 can never run ahead of kernel N.
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+__device__ __forceinline__ void pdl_trigger() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+
 // ------------------------------------------------------------------------------------------ loads
 // streamed arrays (index / value): read once, keep them out of L1 so that L1 holds the gathered vector
 __device__ __forceinline__ int4 ld_stream_i4(const int32_t* p) {
@@ -270,7 +278,9 @@ k_forward(long long n, const Item* __restrict__ items, const int32_t* __restrict
     double csum = 0.0, rprox = 0.0, rphi = 0.0;
     long long rcnt = 0;
     Item it;
-    if (r < n) it = ld_item(items + r);
+    if (r < n) it = ld_item(items + r);          // static data: fetched before the dependency wait
+    pdl_wait();
+    pdl_trigger();
     while (r < n) {
         const long long rn = r + nwarps;
         Item nx;
@@ -448,6 +458,8 @@ k_transpose(long long n, const Item* __restrict__ items, const int32_t* __restri
     long long r = (long long)blockIdx.x * FWD_WARPS + (threadIdx.x >> 5);
     Item it;
     if (r < n) it = ld_item(items + r);
+    pdl_wait();
+    pdl_trigger();
     while (r < n) {
         const long long rn = r + nwarps;
         Item nx;
@@ -474,6 +486,8 @@ __global__ void __launch_bounds__(256)
 k_combine(long long S, const long long* __restrict__ item_ptr, const double* __restrict__ partial,
           double* __restrict__ g_out, double* __restrict__ gpart, double* __restrict__ x, const DevState* __restrict__ st,
           float* __restrict__ f_out) {
+    pdl_wait();
+    pdl_trigger();
     const long long j = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (EPI == TEPI_GRAD) {   // also the CTA's share of |g|^2 (fixed order), summed by k_select
         __shared__ double sm[8];
@@ -535,6 +549,8 @@ __global__ void __launch_bounds__(1024)
 k_select(DevState* st, const double* __restrict__ gpart, int n_gpart, const double* __restrict__ cpart, int n_part,
          long long n, const Item* __restrict__ items, const StructInfo* __restrict__ tab, const double* __restrict__ d,
          const double* __restrict__ l, const double* __restrict__ Dg, const double* __restrict__ Lg) {
+    pdl_wait();
+    pdl_trigger();
     __shared__ double sm[32];
     __shared__ double s_b;
     __shared__ int s_go;
@@ -607,6 +623,8 @@ k_residual(long long n, const Item* __restrict__ items, const StructInfo* __rest
            const GatherVec uv, const GatherVec pq, double* __restrict__ x, const double* __restrict__ g, long long S,
            double* __restrict__ part_prox, double* __restrict__ part_phi, long long* __restrict__ part_cnt,
            int use_beta, int final, int write_uv) {
+    pdl_wait();
+    pdl_trigger();
     __shared__ double sm[ROW_THREADS / 32];
     __shared__ long long smc[ROW_THREADS / 32];
     const double beta = use_beta ? st->beta_acc : 0.0;
@@ -666,6 +684,8 @@ k_block_residual(long long rb, long long re, int seg, int kind, const StructInfo
                  const double* __restrict__ d, const double* __restrict__ l, const double* __restrict__ nD,
                  const double* __restrict__ nL, const double* __restrict__ nT, const GatherVec uv,
                  double* __restrict__ part_prox) {
+    pdl_wait();
+    pdl_trigger();
     __shared__ double sm[ROW_THREADS / 32];
     __shared__ unsigned long long smc[ROW_THREADS / 32];
     const StructInfo& T = tab[seg];
@@ -703,6 +723,8 @@ __global__ void __launch_bounds__(256)
 k_combine_block(long long S, const long long* __restrict__ slot_ptr, int seg, int n_seg, int H,
                 const double* __restrict__ partial, double* __restrict__ x, DevState* st, double factor,
                 const double* __restrict__ part_prox, int n_part) {
+    pdl_wait();
+    pdl_trigger();
     if (blockIdx.x == 0 && threadIdx.x < 32) {
         double p = 0.0;
         for (int i = threadIdx.x; i < n_part; i += 32) p += part_prox[i];
@@ -719,11 +741,13 @@ k_combine_block(long long S, const long long* __restrict__ slot_ptr, int seg, in
 }
 
 // Start of a block-sequential sweep: the sweep statistics restart.
-__global__ void k_sweep_begin(DevState* st) { st->prox = 0.0; st->n_viol = 0; }
+__global__ void k_sweep_begin(DevState* st) { pdl_wait(); pdl_trigger(); st->prox = 0.0; st->n_viol = 0; }
 
 // End of a block-sequential sweep: clamp, w_{k+1} = eta * w_k, k <- k + 1.
 __global__ void __launch_bounds__(256)
 k_sweep_end(long long S, double* __restrict__ x, DevState* st) {
+    pdl_wait();
+    pdl_trigger();
     const long long j = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (j < S && x[j] < 0.0) x[j] = 0.0;
     if (j == 0) { st->relax = st->lambda * st->eta_pow; st->eta_pow *= st->eta; st->k += 1; }
@@ -732,6 +756,8 @@ k_sweep_end(long long S, double* __restrict__ x, DevState* st) {
 __global__ void __launch_bounds__(1024)
 k_finalize_stats(DevState* st, const double* __restrict__ part_prox, const double* __restrict__ part_phi,
                  const long long* __restrict__ part_cnt, int n_part) {
+    pdl_wait();
+    pdl_trigger();
     __shared__ double sm[32];
     __shared__ long long smc[32];
     double p = 0.0, q = 0.0;
