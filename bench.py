@@ -41,8 +41,8 @@ DEFAULT_STEPS = {0: 50, 1: 200, 2: 100, 3: 50}
 NOMINAL_HBM_GBS = 8000.0    # north_star's "~8 TB/s peak" (context; the roofline denominator is the measured copy figure)
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel from the committed `ncu --set full`
 # capture (profiles/r01_ncu_full_config3.md); keyed by (config, pass); a transposed pass = k_transpose + k_combine
-NCU_TRAFFIC = {(3, "forward_x"): 956105728, (3, "transpose_g"): 901090816, (3, "forward_g"): 952477696,
-               (3, "transpose_b"): 970961152}
+NCU_TRAFFIC = {(3, "forward_x"): 957143296, (3, "transpose_g"): 901036288, (3, "forward_g"): 953572608,
+               (3, "transpose_b"): 971151616}
 
 
 def _peaks():
