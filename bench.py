@@ -249,6 +249,9 @@ def run_ours(args):
     torch.cuda.synchronize()
     read_gbs = 10 * nb / (r0.elapsed_time(r1) * 1e-3) / 1e9
     del buf
+    PASS_KERNELS = {"forward_x": "k_forward<EPI_STORE_PQ> (k_forward<EPI_RESID> with --ams)", "transpose_g": "k_transpose + k_combine<GRAD>",
+                    "forward_g": "k_forward<EPI_CPART>", "select": "k_select", "residual": "k_residual",
+                    "transpose_b": "k_transpose + k_combine<UPDATE>"}
     top = max(pt, key=lambda n: pt[n][0])
     top_ms = pt[top][0] / max(pt[top][1], 1)
     peak, peak_src = _peaks()
@@ -284,7 +287,7 @@ def run_ours(args):
                 "d2h_bytes_per_step": plan.n_cols * 4 + STATE_BYTES},
         "gpu_launches": int(launches),
         "clocks": clocks,
-        "roofline": {"bound": "hbm", "kernel": top, "achieved": achieved, "peak": peak, "unit": "GB/s",
+        "roofline": {"bound": "hbm", "kernel": top, "kernel_names": PASS_KERNELS.get(top, top), "achieved": achieved, "peak": peak, "unit": "GB/s",
                      "frac": achieved / peak, "traffic": NCU_TRAFFIC.get((args.config, top)), "peak_source": peak_src,
                      "alg_bytes_per_launch": pass_bytes[top], "ms_per_launch": top_ms,
                      "frac_of_nominal_8TBs": achieved / NOMINAL_HBM_GBS, "read_ceiling_gbs": read_gbs,
