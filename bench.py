@@ -270,11 +270,12 @@ def run_ours(args):
     value = whole_job_rate(K, ws, ms * 1e-3)
     out = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": ws, "steps": K, "warmup": W, "ms_per_step": ms / K,
-        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64 accumulate / f32 matrix values",
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
         "data": "synthetic",
         "config": {"workload": f"configs[{args.config}] {spec.name}", "n_voxels": plan.n_rows, "n_spots": plan.n_cols,
                    "nnz_per_matrix": plan.nnz, "nnz_active": stats["nnz_active"], "n_active_rows": stats["n_active_rows"],
                    "n_sets": stats["n_sets"], "lambda": lam, "beta0": beta0, "a": a,
+                   "storage": "fp32 matrix values, 16-bit indices where exact (else int32), fp64 vectors and accumulators",
                    "ams_form": "block-sequential (Fig. 2 loop nest, R23)" if args.block_sequential else "simultaneous (R1)",
                    "passes_per_iteration": 2 if args.ams else 4, "alg_bytes_per_iteration": iter_bytes,
                    "form": "pure feasibility-seeking (beta0 = 0)" if args.ams else "superiorized",
