@@ -538,6 +538,20 @@ def test_config1_20_iterations_full_size(fredopt):
     _full_size_parity(fredopt, pg.build_plan(pg.config_spec(1), device="cuda"), 4000)
 
 
+def test_config1_all_200_iterations(fredopt):
+    """BASELINE.json configs[1] over its full iteration count: the violation count is compared every 25 iterations (SURVEY
+    sec. 7.5: all-fp32 arithmetic flips it at 3 of 200 iterations here; fp64 vectors must not)."""
+    plan = pg.build_plan(pg.config_spec(1), device="cuda")
+    gp = fredopt.from_plan(plan, stream=torch.cuda.current_stream().cuda_stream)
+    orc = _oracle(plan)
+    sp = plan.spec
+    orc.set_x(plan.x0); gp.set_weights(plan.x0)
+    for _ in range(8):
+        orc.iterate(25, sp.lam, sp.beta0, sp.a); gp.iterate(25, sp.lam, sp.beta0, sp.a)
+        _assert_state(gp, orc)
+    assert gp.stats()["k"] == sp.n_iter == 200
+
+
 def test_config3_20_iterations_in_bench_configuration(fredopt):
     """BASELINE.json configs[3]: the workload bench.py times (1.15e9 non-zeros per matrix), at full size."""
     plan = pg.build_plan(pg.config_spec(3), device="cuda")
