@@ -538,6 +538,11 @@ def test_config1_20_iterations_full_size(fredopt):
     _full_size_parity(fredopt, pg.build_plan(pg.config_spec(1), device="cuda"), 4000)
 
 
+def test_config2_20_iterations_full_size(fredopt):
+    """BASELINE.json configs[2] (three beams: the first iteration rejects ~200 step sizes), at full size."""
+    _full_size_parity(fredopt, pg.build_plan(pg.config_spec(2), device="cuda"), 8000)
+
+
 def test_config1_all_200_iterations(fredopt):
     """BASELINE.json configs[1] over its full iteration count: the violation count is compared every 25 iterations (SURVEY
     sec. 7.5: all-fp32 arithmetic flips it at 3 of 200 iterations here; fp64 vectors must not)."""
