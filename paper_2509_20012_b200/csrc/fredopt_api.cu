@@ -1492,7 +1492,7 @@ int fredopt_iterate(fredopt_plan* P, int32_t n_iter, float lambda, float beta0, 
             // small plans, whose iteration lasts about as long as a graph launch costs)
             const int form = 2 * P->block_sequential + (sa ? 1 : 0);
             int left = n_iter;
-            // (measured: +3 % on configs[0]-[1], +1 % on configs[2], -0.7 % on configs[3]: long graph only below 5e7 non-zeros)
+            // (measured: +3 % on configs[0]-[1], +1 % on configs[2], nothing at configs[3]: long graph only below 5e7 non-zeros)
             for (int u = P->act.nnz < 50000000LL ? 1 : 0; u >= 0; --u) {
                 const int per = u ? GRAPH_UNROLL : 1, gi = 2 * form + u;
                 // both graphs are built at the first call of a form, so that no later (timed) call pays for a capture
