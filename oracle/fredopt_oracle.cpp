@@ -59,7 +59,8 @@ struct Plan {
     std::vector<double> x;             // fluence
     // state of Fig. 3
     int64_t k = 0, s = 0, trials = 0;
-    bool started = false;
+    bool started = false;              // beta0, a latched (first superiorized call after create / reset)
+    double latched_beta0 = 0.0, latched_a = 0.0;
     double beta_next = 0.0, eta_pow = 1.0, last_beta = 0.0;
     // options
     double eta = 1.0;
@@ -375,11 +376,17 @@ void oracle_proximity(void* h, const double* xin, double* prox, int64_t* n_viol)
 
 // SuperiorDLET (Fig. 3) around the simultaneous AMSrelaxDLET step (Fig. 2).
 // lambda, beta0, a arrive as the fp32 bit patterns the caller passes to the C-ABI and are widened here.
-void oracle_iterate(void* h, int32_t n_iter, float lambda_f, float beta0_f, float a_f) {
+// The step-size sequence beta_s = beta0 a^s (R8) belongs to the plan: beta0 and a are latched by the first call with
+// beta0 > 0 and n_iter > 0 after create / reset; a later call with beta0 > 0 must pass the same pair (else -1 and nothing
+// is done); calls with beta0 == 0 (pure feasibility-seeking) neither latch nor consume the sequence.  Returns 0 / -1.
+int32_t oracle_iterate(void* h, int32_t n_iter, float lambda_f, float beta0_f, float a_f) {
     Plan* P = (Plan*)h;
     const double lambda = (double)lambda_f, beta0 = (double)beta0_f, a = (double)a_f;
     const int64_t S = P->D.n_cols;
-    if (!P->started) { P->beta_next = beta0; P->eta_pow = 1.0; P->started = true; }   // beta_0 = beta0; eta^0 = 1
+    if (beta0 != 0.0 && n_iter > 0) {
+        if (!P->started) { P->beta_next = beta0; P->latched_beta0 = beta0; P->latched_a = a; P->started = true; }   // beta_0 = beta0
+        else if (beta0 != P->latched_beta0 || a != P->latched_a) return -1;
+    }
     std::vector<double> g, xn(S), step;
     for (int32_t it = 0; it < n_iter; ++it) {
         // ---- perturbation phase; skipped entirely when beta0 == 0 (pure AMS)
@@ -419,6 +426,7 @@ void oracle_iterate(void* h, int32_t n_iter, float lambda_f, float beta0_f, floa
         P->eta_pow *= P->eta;
         ++P->k;
     }
+    return 0;
 }
 
 // out: k, s, trials, n_sets, n_zero_norm_sets ; dout: last_beta, W, beta_next

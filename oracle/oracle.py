@@ -49,6 +49,7 @@ def _load():
         lib.oracle_cost.argtypes = [vp, vp]
         lib.oracle_grad.argtypes = [vp, vp, vp]
         lib.oracle_proximity.argtypes = [vp, vp, vp, vp]
+        lib.oracle_iterate.restype = i32
         lib.oracle_iterate.argtypes = [vp, i32, f32, f32, f32]
         lib.oracle_stats.argtypes = [vp, vp, vp]
         lib.oracle_sweep_stats.argtypes = [vp, vp, vp]
@@ -155,7 +156,8 @@ class Oracle:
         return pr.value, nv.value
 
     def iterate(self, n_iter, lam, beta0, a):
-        self._lib.oracle_iterate(self._h, int(n_iter), float(lam), float(beta0), float(a))
+        if self._lib.oracle_iterate(self._h, int(n_iter), float(lam), float(beta0), float(a)) != 0:
+            raise ValueError("beta0 / a differ from the pair latched by the first superiorized call (reset first)")
 
     def stats(self):
         o = np.zeros(5, np.int64); d = np.zeros(3, np.float64)

@@ -509,7 +509,8 @@ def random_small_plan(seed: int, V: int = 40, S: int = 8, n_struct: int = 3, den
     Dd = (0.05 + u[k:k + V * S]).reshape(V, S) * mask; k += V * S
     let = 2.0 + 8.0 * u[k:k + V * S].reshape(V, S); k += V * S
     Ld = Dd * let
-    maskL = mask if same_pattern else ((u[k:k + V * S] < density).reshape(V, S) | mask)
+    # different patterns: L's mask is drawn INDEPENDENTLY of D's, so rows hold entries in D only, in L only and in both
+    maskL = mask if same_pattern else (u[k:k + V * S] < density).reshape(V, S)
     k += V * S
     if not same_pattern:
         Ld = np.where(maskL, np.where(mask, Ld, 0.3 * let), 0.0)

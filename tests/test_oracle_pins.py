@@ -108,14 +108,20 @@ class DenseReference:
                 g += 2 * self.what[s - 1] * (l[i] - lref) * self.L[i]
         return g
 
-    def iterate(self, x, n, lam, beta0, a, max_trials=200):
+    def iterate(self, x, n, lam, beta0, a, max_trials=200, reductions=1, eta=1.0):
+        """Fig. 3 around the simultaneous Fig. 2 step: `while t < reductionsN` holds the
+        `while loop` over step sizes; w_k = eta^k w multiplies the projection step."""
         lam, beta0, a = float(F32(lam)), float(F32(beta0)), float(F32(a))
         beta = beta0
         s_count = 0
+        eta_k = 1.0
         for _ in range(n):
             if beta0 != 0:
-                phi0, g = self.cost(x), self.grad(x)
-                if np.any(g != 0):
+                t = 0
+                while t < reductions:
+                    phi0, g = self.cost(x), self.grad(x)
+                    if not np.any(g != 0):
+                        break
                     for _t in range(max_trials):
                         b = beta
                         beta *= a
@@ -124,12 +130,14 @@ class DenseReference:
                         if self.cost(xn) < phi0:
                             x = xn
                             break
+                    t += 1
             step = np.zeros_like(x)
             for av, lo, hi, s in self.sets:
                 n2 = av @ av
                 if n2 > 0:
                     step += self.what[s - 1] * self.resid(av @ x, lo, hi) / n2 * av
-            x = np.maximum(x - lam * step, 0.0)
+            x = np.maximum(x - lam * eta_k * step, 0.0)
+            eta_k *= eta
         return x, s_count
 
 
@@ -673,3 +681,178 @@ def test_pin19_volume_histogram_percentile_and_table1_statistics():
             assert np.mean(v >= pv * (1 - 1e-13)) >= 0.3 and np.mean(v > pv * (1 + 1e-13)) < 0.3
             hst = o.volume_histogram(q, s_, 16, float(v.max()) * 1.01, xx)
             assert hst[0] == 1.0 and np.all(np.diff(hst) <= 0) and hst[-1] > 0
+
+
+# ----------------------------------------------------------------------------- options of Fig. 3: eta, reductionsN, trial cap
+@pytest.mark.parametrize("eta", [0.9, 0.5])
+def test_pin20_eta_decay_diagonal_closed_form(eta):
+    """w_k = eta^k w (Fig. 3; reading R12): on pin 3's diagonal system the residual after k iterations is
+    prod_{j<k} (1 - lambda eta^j / S) * residual(0).  Guards `relax = lambda * eta_pow` and `eta_pow *= eta` in
+    oracle_iterate (a decay applied cumulatively, one iteration late, or to the wrong factor fails)."""
+    S = 6
+    I = np.eye(S)
+    o = make_oracle(I, 2 * I, [1] * S, bounds_rows(dict(weight=7.0, dose_hi=1.0)))
+    o.set_option(orc.OPT_ETA, eta)
+    x0 = (2.0 + np.arange(S)).astype(F32)
+    r0 = x0.astype(np.float64) - 1.0
+    lam = float(F32(1.5))
+    o.set_x(x0)
+    fac = 1.0
+    for k in range(1, 9):
+        o.iterate(1, 1.5, 0.0, 0.5)
+        fac *= 1.0 - lam * eta ** (k - 1) / S
+        np.testing.assert_allclose(o.get_x() - 1.0, fac * r0, rtol=1e-13)
+    # RESET restarts the decay at eta^0
+    o.set_option(orc.OPT_RESET, 1); o.set_x(x0); o.iterate(1, 1.5, 0.0, 0.5)
+    np.testing.assert_allclose(o.get_x() - 1.0, (1.0 - lam / S) * r0, rtol=1e-13)
+
+
+@pytest.mark.parametrize("reductions", [2, 3])
+@pytest.mark.parametrize("seed,same", [(1, True), (3, False)])
+def test_pin21_reductions_loop_dense_brute_force(reductions, seed, same):
+    """`while t < reductionsN` (Fig. 3): N cost-reducing steps, each with a fresh chi^2 and gradient, before
+    one AMS step.  Guards the `for t < reductionsN` loop of oracle_iterate (phi0 / g not refreshed, or the AMS step inside the
+    loop, fails); x, s and the violation count are compared with the separate dense restatement, with eta < 1 on top."""
+    D, L, labels, x0 = pg.random_small_plan(seed, V=45, S=9, n_struct=3, same_pattern=same)
+    Dd, Ld = csr_to_dense(D, 9), csr_to_dense(L, 9)
+    b = bounds_rows(dict(weight=1.0, dose_lo=1.2, dose_hi=1.6, dose_ref=1.4),
+                    dict(weight=2.5, dose_hi=0.9, dl_hi=4.0, dl_lo=0.5, letd_max=5.0, dl_ref=3.0),
+                    dict(weight=0.5, letd_max=4.0, dose_lo=0.3))
+    o = orc.Oracle.create(45, 9, D, L, labels, b)
+    ref = DenseReference(Dd, Ld, labels, b)
+    o.set_option(orc.OPT_REDUCTIONS, reductions); o.set_option(orc.OPT_ETA, 0.95)
+    o.set_x(x0)
+    o.iterate(7, 1.3, 2.0, 0.8)                      # beta0 = 2: the first trials are rejected
+    xr, s_ref = ref.iterate(x0.astype(np.float64), 7, 1.3, 2.0, 0.8, reductions=reductions, eta=0.95)
+    np.testing.assert_allclose(o.get_x(), xr, rtol=1e-10, atol=1e-13)
+    st = o.stats()
+    assert st["s"] == s_ref and st["trials"] == s_ref and s_ref > 7 * reductions
+    assert o.proximity()[1] == ref.proximity(xr)[1]
+    # one reduction per iteration gives a different trajectory (the loop is not a no-op)
+    o1 = orc.Oracle.create(45, 9, D, L, labels, b)
+    o1.set_option(orc.OPT_ETA, 0.95); o1.set_x(x0); o1.iterate(7, 1.3, 2.0, 0.8)
+    assert np.max(np.abs(o1.get_x() - o.get_x())) > 1e-6
+
+
+def test_pin22_trial_cap_keeps_x_and_still_advances_s():
+    """Reading R10 (Fig. 3's `while loop`, never ends if chi^2 cannot decrease): after `max_trials`
+    rejections x is kept and s has still advanced.  beta0 = 1e6 with a = 0.999 rejects every trial, so with a cap of 5 the
+    trajectory is that of pure feasibility-seeking bit for bit and s grows by exactly 5 per iteration.  Guards the
+    `trial < max_trials` bound and the keep-x fall-through of oracle_iterate."""
+    D, L, labels, x0 = pg.random_small_plan(2, V=45, S=9, n_struct=2)
+    b = bounds_rows(dict(weight=1.0, dose_lo=1.2, dose_hi=1.6, dose_ref=1.4), dict(weight=2.0, dose_hi=0.9, dl_ref=3.0))
+    a = orc.Oracle.create(45, 9, D, L, labels, b)
+    c = orc.Oracle.create(45, 9, D, L, labels, b)
+    a.set_option(orc.OPT_MAX_TRIALS, 5)
+    a.set_x(x0); c.set_x(x0)
+    for k in range(1, 5):
+        a.iterate(1, 1.1, 1.0e6, 0.999); c.iterate(1, 1.1, 0.0, 0.999)
+        assert np.array_equal(a.get_x(), c.get_x())
+        st = a.stats()
+        assert st["s"] == 5 * k and st["trials"] == 5 * k and st["last_beta"] == 0.0 and st["k"] == k
+    # beta_next = beta0 a^(5k) by repeated multiplication
+    bn = float(F32(1.0e6))
+    for _ in range(20):
+        bn *= float(F32(0.999))
+    assert a.stats()["beta_next"] == bn
+
+
+def test_pin23_letd_row_over_entries_in_D_only_and_L_only():
+    """The LETd row a = L_i - LETmax D_i over the UNION pattern (north_star; reading R18): independent D / L masks give entries
+    in D only (a_j = -LETmax D_ij), in L only (a_j = L_ij) and in both.  Guards all three branches of letd_row_dot (the
+    `cd < cl` branch had no test before: a dropped -LETmax D_ij term changes the norm, the residual and the step)."""
+    D, L, labels, x0 = pg.random_small_plan(6, V=40, S=10, n_struct=2, density=0.45, same_pattern=False)
+    Dd, Ld = csr_to_dense(D, 10), csr_to_dense(L, 10)
+    only_d = (Dd != 0) & (Ld == 0) & (labels[:, None] != 0)
+    only_l = (Dd == 0) & (Ld != 0) & (labels[:, None] != 0)
+    assert only_d.sum() > 20 and only_l.sum() > 20 and ((Dd != 0) & (Ld != 0)).sum() > 20
+    b = bounds_rows(dict(weight=1.0, letd_max=1.5), dict(weight=3.0, letd_max=0.7, dose_hi=1.0))
+    o = orc.Oracle.create(40, 10, D, L, labels, b)
+    ref = DenseReference(Dd, Ld, labels, b)
+    # norms of the LETd rows over the union pattern
+    _, _, nT = o.norms()
+    for i in range(40):
+        if labels[i]:
+            a = Ld[i] - float(b[labels[i] - 1, 5]) * Dd[i]
+            assert abs(nT[i] - a @ a) <= 1e-14 * max(a @ a, 1e-300)
+    x = x0.astype(np.float64)
+    p, nv = o.proximity(x)
+    pr, nvr = ref.proximity(x)
+    assert nv == nvr and nv > 5 and abs(p - pr) <= 1e-13 * pr
+    o.set_x(x0)
+    o.iterate(9, 1.4, 0.0, 0.5)
+    xr, _ = ref.iterate(x.copy(), 9, 1.4, 0.0, 0.5)
+    np.testing.assert_allclose(o.get_x(), xr, rtol=1e-11, atol=1e-14)
+    # block-sequential form over the same rows
+    ob = orc.Oracle.create(40, 10, D, L, labels, b)
+    ob.set_option(orc.OPT_BLOCK_SEQUENTIAL, 1); ob.set_x(x0)
+    xb = x.copy()
+    for _ in range(4):
+        ob.iterate(1, 1.2, 0.0, 0.5)
+        xb, _ = _dense_block_sweep(Dd, Ld, labels, b, xb, float(F32(1.2)))
+    np.testing.assert_allclose(ob.get_x(), xb, rtol=1e-11, atol=1e-14)
+
+
+def test_pin24_dose_let_rows_equals_dose_let(plan0):
+    """oracle_dose_let_rows (the checker of the full-size sampled forward parity) returns exactly the listed rows of
+    oracle_dose_let (Eq. 1) -- bit for bit, repeated and unordered rows included."""
+    o = orc.from_plan(plan0)
+    x = pg.log_uniform_weights(5, plan0.n_cols).astype(np.float64)
+    d, l, t = o.dose_let(x)
+    rows = (pg.uniform01_array(8, 3000) * plan0.n_rows).astype(np.int64)
+    rows[:3] = [0, plan0.n_rows - 1, rows[5]]
+    dr, lr, tr = o.dose_let_rows(rows, x)
+    assert np.array_equal(dr, d[rows]) and np.array_equal(lr, l[rows]) and np.array_equal(tr, t[rows])
+    assert np.count_nonzero(dr) > 100
+    # and at the oracle's own x (x = NULL)
+    o.set_x(plan0.x0)
+    d0, l0, t0 = o.dose_let(None)
+    dr0, _, tr0 = o.dose_let_rows(rows, None)
+    assert np.array_equal(dr0, d0[rows]) and np.array_equal(tr0, t0[rows])
+
+
+def test_pin25_transpose_abs_scale_is_the_dense_abs_product():
+    """oracle_transpose's second output (the scale of the per-element tolerance of the transposed GPU passes, SURVEY sec. 8c
+    parity rule) is sum_i |D_ij u_i| + |L_ij v_i| -- no more (a too-large scale would loosen the tolerance), no less."""
+    D, L, labels, _ = pg.random_small_plan(9, V=50, S=11, n_struct=2, density=0.35, same_pattern=False)
+    Dd, Ld = csr_to_dense(D, 11), csr_to_dense(L, 11)
+    o = orc.Oracle.create(50, 11, D, L, labels, bounds_rows(dict(dose_hi=1.0), dict(dl_hi=1.0)))
+    u = pg.uniform01_array(12, 50) - 0.5
+    v = pg.uniform01_array(13, 50) - 0.4
+    for uu, vv in ((u, v), (u, None), (None, v)):
+        for act in (False, True):
+            m = (labels != 0) if act else np.ones(50, bool)
+            out, oabs = o.transpose(uu, vv, active_only=act)
+            ref = np.zeros(11); refa = np.zeros(11)
+            if uu is not None:
+                ref += Dd[m].T @ uu[m]; refa += np.abs(Dd[m]).T @ np.abs(uu[m])
+            if vv is not None:
+                ref += Ld[m].T @ vv[m]; refa += np.abs(Ld[m]).T @ np.abs(vv[m])
+            np.testing.assert_allclose(out, ref, rtol=1e-13, atol=1e-16)
+            np.testing.assert_allclose(oabs, refa, rtol=1e-13)
+
+
+def test_pin26_step_size_sequence_belongs_to_the_plan():
+    """Reading R8: beta_s = beta0 a^s is ONE sequence per plan.  beta0, a are latched by the first superiorized call; calls
+    with beta0 = 0 in between are pure AMS steps that neither latch nor consume it; another (beta0, a) needs a RESET."""
+    D, L, labels, x0 = pg.random_small_plan(2, V=45, S=9, n_struct=2)
+    b = bounds_rows(dict(weight=1.0, dose_lo=1.2, dose_hi=1.6, dose_ref=1.4), dict(weight=2.0, dose_hi=0.9, dl_ref=3.0))
+    o = orc.Oracle.create(45, 9, D, L, labels, b)
+    o.set_x(x0)
+    o.iterate(0, 1.0, 0.7, 0.5)                     # n_iter = 0 latches nothing
+    o.iterate(2, 1.0, 0.0, 0.5)                     # pure AMS first: nothing latched, s stays 0
+    assert o.stats()["s"] == 0 and o.stats()["k"] == 2
+    o.iterate(1, 1.0, 0.5, 0.9)                     # first superiorized call latches (0.5, 0.9)
+    s1 = o.stats()["s"]
+    bn = float(F32(0.5))
+    for _ in range(s1):
+        bn *= float(F32(0.9))
+    assert s1 >= 1 and o.stats()["beta_next"] == bn
+    o.iterate(1, 1.0, 0.0, 0.9)                     # AMS step in between: s unchanged
+    assert o.stats()["s"] == s1
+    with pytest.raises(ValueError):
+        o.iterate(1, 1.0, 0.25, 0.9)
+    with pytest.raises(ValueError):
+        o.iterate(1, 1.0, 0.5, 0.8)
+    o.iterate(1, 1.0, 0.5, 0.9)
+    assert o.stats()["s"] > s1 and o.stats()["k"] == 5
