@@ -113,6 +113,8 @@ typedef struct {
 
 #define FREDOPT_OPT_NORMALIZE_GRAD   8 /* 1: the perturbation steps along grad chi^2 / |grad chi^2|_2 (Fig. 3 prints the  */
                                        /*    un-normalised gradient: default 0; R9)             */
+#define FREDOPT_OPT_USE_PDL         10 /* 1 (default): the kernels of an iteration are launched with programmatic dependent    */
+                                       /*    launch (a kernel's CTAs are scheduled while its predecessor drains); 0: plain launches */
 #define FREDOPT_OPT_ONE_SIDED_COST   9 /* 1: the OAR term of Eq. (2) penalises only cDL above cDLref: w (cDL - cDLref)_+^2 */
                                        /*    (Eq. (2) as printed is two-sided: default 0; R11)   */
 
@@ -137,6 +139,19 @@ typedef struct {
  * OUT_OF_MEMORY, CUDA_ERROR, UNSUPPORTED_ARCH. */
 int fredopt_create(const fredopt_csr *D, const fredopt_csr *L, const int32_t *voxel_labels,
                    const fredopt_bounds *bounds, int32_t n_struct, void *cuda_stream, fredopt_plan **out);
+
+/* Storage choices of a plan, fixed at creation ("optimized method for storing the Dij and LETij matrices", PAPER.md:282;
+ * SURVEY sec. 8f-2).  They change the bytes a pass moves, never a result: index work is exact, and every sum runs over the
+ * same terms plus exact zeros.  struct_size = sizeof(fredopt_create_options) of the caller (the struct may grow). */
+typedef struct {
+    int32_t struct_size;
+    int32_t index_width;        /* 0 = automatic: 16-bit indices where exact (n_cols <= 65536; row indices of the      */
+                                /*     transposes inside 65536-row blocks), int32 otherwise; 32 = int32 everywhere      */
+} fredopt_create_options;
+/* fredopt_create with options (opt = NULL: the defaults, identical to fredopt_create).  INVALID_ARG on an unknown value. */
+int fredopt_create_ex(const fredopt_csr *D, const fredopt_csr *L, const int32_t *voxel_labels,
+                      const fredopt_bounds *bounds, int32_t n_struct, void *cuda_stream,
+                      const fredopt_create_options *opt, fredopt_plan **out);
 void fredopt_destroy(fredopt_plan *plan);
 
 /* Spot weights x (n_cols floats).  set: widened to fp64; get: the plan's fp64 x rounded to fp32.

@@ -8,9 +8,9 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libfredopt.so")
-SOURCES = [os.path.join(CSRC, "fredopt_api.cu")]
-DEPS = SOURCES + [os.path.join(CSRC, "fredopt_kernels.cuh"),
-                  os.path.join(os.path.dirname(HERE), "include", "fredopt.h")]
+SOURCES = [os.path.join(CSRC, f) for f in ("plan_build.cu", "iterate.cu", "passes.cu")]
+DEPS = SOURCES + [os.path.join(CSRC, f) for f in ("fredopt_kernels.cuh", "kernels_iter.cuh", "kernels_eval.cuh", "fredopt_plan.cuh")] + \
+    [os.path.join(os.path.dirname(HERE), "include", "fredopt.h")]
 
 
 def nvcc_path() -> str:
@@ -23,7 +23,7 @@ def nvcc_path() -> str:
 def build_library(force: bool = False, verbose: bool = False) -> str:
     if not force and os.path.exists(LIB) and all(os.path.getmtime(LIB) >= os.path.getmtime(d) for d in DEPS):
         return LIB
-    cmd = [nvcc_path(), "-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
+    cmd = [nvcc_path(), "-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "--threads", "0",
            "-Xcompiler", "-fPIC", "-shared", "-o", LIB] + SOURCES
     if verbose:
         cmd.insert(1, "-Xptxas=-v")

@@ -1,0 +1,200 @@
+// fredopt_plan.cuh -- internal declarations shared by the translation units of libfredopt.so:
+//   plan_build.cu   fredopt_create: validation, row sets, CSR of the transposes, tables (create time, not hot)
+//   iterate.cu      launches of the hot kernels, one iteration of Fig. 3 around Fig. 2, fredopt_iterate, options, state
+//   passes.cu       the other calls of include/fredopt.h: weights, dose_let, proximity, per-pass exports, evaluation
+// Nothing here touches the CPU oracle; there is no CPU fallback.
+#pragma once
+#include "../../include/fredopt.h"
+#include "fredopt_kernels.cuh"
+
+#include <cmath>
+#include <cstdio>
+#include <cstdlib>
+#include <cstring>
+#include <string>
+#include <vector>
+
+using namespace fredopt;
+
+// ============================================================================================ errors
+extern thread_local std::string g_last_cuda_error;      // defined in passes.cu
+
+#define CK(expr)                                                                                   \
+    do {                                                                                           \
+        cudaError_t e__ = (expr);                                                                  \
+        if (e__ != cudaSuccess) {                                                                  \
+            g_last_cuda_error = std::string(#expr) + ": " + cudaGetErrorString(e__);               \
+            cudaGetLastError();                                                                    \
+            return e__ == cudaErrorMemoryAllocation ? FREDOPT_OUT_OF_MEMORY : FREDOPT_CUDA_ERROR;  \
+        }                                                                                          \
+    } while (0)
+#define CKR(expr)                         \
+    do {                                  \
+        int r__ = (expr);                 \
+        if (r__ != FREDOPT_OK) return r__; \
+    } while (0)
+
+// ============================================================================================ plan
+// view of a row set for the create-time kernels
+struct RowList {
+    long long n;                 // rows in the list
+    const long long* start;      // [n] offset of the row in the set's padded arrays (multiple of 4)
+    const int32_t* len;          // [n] padded length (multiple of 4)
+    const int32_t* seg;          // [n] segment (structure - 1), or nullptr = segment 0
+    const int32_t* vox;          // [n] voxel index of the row
+};
+
+struct RowSet {
+    long long n = 0;                 // rows
+    int n_seg = 1;
+    // padded index / value arrays of the set (rows stored back to back in list order)
+    int32_t* col = nullptr;          // int32 column indices (kept for transposition; the hot kernels read col16 if set)
+    uint16_t* col16 = nullptr;       // the same indices as 16 bits when n_cols <= 65536 (2 B instead of 4 B per non-zero)
+    float* valD = nullptr;
+    float* valL = nullptr;
+    int32_t* vox = nullptr;          // [n]
+    int32_t* seg = nullptr;          // [n] or nullptr
+    long long* start = nullptr;      // [n]
+    int32_t* len = nullptr;          // [n] padded
+    int32_t* ulen = nullptr;         // [n] unpadded
+    Item* items = nullptr;           // [n] {start, len, seg}: what the forward kernel reads
+    long long nnz = 0;               // unpadded entries in the set
+    // CSR of the transposes restricted to this set, SEGMENT-major: run k = seg*S + spot; columns = list index
+    bool t_built = false;
+    long long* t_ptr = nullptr;      // [n_seg*S + 1]
+    int32_t* t_col = nullptr;        // compact row index (32-bit form: only if the 16-bit form does not apply)
+    uint16_t* t_col16 = nullptr;     // low 16 bits of the compact row index; runs are cut where the high bits change
+    int t_H = 1;                     // number of 65536-row blocks of the list (1 in the 32-bit form)
+    float* t_valD = nullptr;
+    float* t_valL = nullptr;
+    long long t_nnz_padded = 0;
+    // work items of the transposed pass: runs cut into pieces of at most TR_ITEM_MAX entries
+    long long t_n_items = 0;
+    Item* t_items = nullptr;         // [t_n_items]
+    int32_t* t_item_slot = nullptr;  // [t_n_items] slot of the item's partial sum
+    long long* t_item_ptr = nullptr; // [S+1] partial-sum slots of spot j: t_item_ptr[j] .. t_item_ptr[j+1]-1
+    double* t_partial = nullptr;     // [t_n_items]
+    // block-sequential AMS: the same items grouped by structure (longest first inside a structure) and the slot
+    // ranges per (spot, structure, 65536-row block)
+    Item* t_items_seg = nullptr;     // [t_n_items]
+    int32_t* t_slot_seg = nullptr;   // [t_n_items]
+    long long* t_slot_ptr = nullptr; // [S * n_seg * t_H + 1]
+    std::vector<long long> t_seg_item_begin;   // host: items of structure s are t_seg_item_begin[s] .. [s+1]-1
+    RowList view() const { return RowList{n, start, len, seg, vox}; }
+};
+
+struct EventPair { cudaEvent_t a, b; int pass; };
+
+struct fredopt_plan {
+    cudaStream_t stream = nullptr;
+    bool owns_stream = false;
+    int device = 0;
+    long long V = 0, S = 0, nnz = 0, nnz_padded = 0;
+    int n_struct = 0;
+    std::vector<void*> allocs;
+    // full: all non-empty rows of the padded matrix (union pattern); act: a compact copy of the rows with a label,
+    // ordered by (structure, voxel)
+    RowSet full, act;
+    long long full_class[9] = {0, 0, 0, 0, 0, 0, 0, 0, 0};   // rows of length class c of `full`: full_class[c] .. full_class[c+1]-1
+    // per active row
+    double *nD = nullptr, *nL = nullptr, *nT = nullptr;
+    // tables
+    StructInfo* tab = nullptr;             // [n_struct]
+    std::vector<StructInfo> h_tab;
+    uint8_t *mode_union = nullptr, *mode_con = nullptr, *mode_cost = nullptr, *mode_fixed = nullptr;  // mode_fixed: [4][max_seg]
+    int max_seg = 1;
+    DevState* st = nullptr;
+    // vectors (fp64)
+    double *x = nullptr, *g = nullptr, *xtmp = nullptr;                       // [S]
+    float* xstage = nullptr;                                                   // [S] staging of host spot-weight vectors
+    double *d = nullptr, *l = nullptr, *Dg = nullptr, *Lg = nullptr;          // [VA]
+    GatherVec pq{nullptr, nullptr, nullptr}, uv{nullptr, nullptr, nullptr};    // [VA] gather vectors of the transposed passes
+    GatherVec fullUV{nullptr, nullptr, nullptr};                               // lazily: [full.n] gather vector for ROWS_ALL transposes
+    double* cpart = nullptr;
+    double* gpart = nullptr;                                                   // [ceil(S/256)] partial sums of |g|^2
+    double *part_prox = nullptr, *part_phi = nullptr;
+    long long* part_cnt = nullptr;
+    int* sink = nullptr;
+    // options / host state
+    double eta = 1.0;
+    long long reductionsN = 1, max_trials = 200;
+    int accept_check = 1, use_graph = 1, time_passes = 0, block_sequential = 0, normalize_grad = 0, one_sided_cost = 0;
+    int use_pdl = 1;
+    bool force_idx32 = false;          // create option: int32 indices in both orientations
+    bool started = false;
+    float latched_beta0 = 0.f, latched_a = 0.f;
+    cudaError_t launch_err = cudaSuccess;   // first error of a kernel launch since the last check (klaunch)
+    long long launches = 0;
+    // graphs: [0] = AMS iteration, [1] = SA iteration (for the current reductionsN)
+    cudaGraphExec_t gexec[8] = {};       // index = 2 * (2 * block_sequential + (superiorized ? 1 : 0)) + (GRAPH_UNROLL iterations ? 1 : 0)
+    long long gexec_red[8] = {};
+    int gexec_kernels[8] = {};
+    // timing
+    std::vector<EventPair> events;
+    double pass_ms[FREDOPT_N_PASSES] = {0};
+    long long pass_launches[FREDOPT_N_PASSES] = {0};
+    long long pass_bytes[FREDOPT_N_PASSES] = {0};
+    int sm_count = 148;
+};
+
+
+template <class T>
+static inline int dmalloc(fredopt_plan* P, T** p, size_t n) {
+    *p = nullptr;
+    if (n == 0) n = 1;
+    CK(cudaMalloc((void**)p, n * sizeof(T)));
+    P->allocs.push_back((void*)*p);
+    return FREDOPT_OK;
+}
+
+static inline int gv_alloc(fredopt_plan* P, GatherVec* g, size_t n) {
+    CKR(dmalloc(P, &g->pair, n)); CKR(dmalloc(P, &g->cD, n)); CKR(dmalloc(P, &g->cL, n));
+    CK(cudaMemsetAsync(g->pair, 0, (n ? n : 1) * 16, P->stream));
+    CK(cudaMemsetAsync(g->cD, 0, (n ? n : 1) * 8, P->stream));
+    CK(cudaMemsetAsync(g->cL, 0, (n ? n : 1) * 8, P->stream));
+    return FREDOPT_OK;
+}
+
+static inline bool is_device_ptr(const void* p) {
+    cudaPointerAttributes at;
+    if (cudaPointerGetAttributes(&at, p) != cudaSuccess) { cudaGetLastError(); return false; }
+    return at.type == cudaMemoryTypeDevice || at.type == cudaMemoryTypeManaged;
+}
+
+static inline int grid_for(long long n, int threads, int cap) {
+    long long g = (n + threads - 1) / threads;
+    if (g < 1) g = 1;
+    if (g > cap) g = cap;
+    return (int)g;
+}
+
+// length classes of the full row set (plan_build.cu orders the rows by class; passes.cu launches per class)
+constexpr int N_LEN_CLASS = 8, FIRST_SHORT_CLASS = 5;
+
+// ============================================================================================ launches
+// Launch one kernel of an iteration on the plan's stream.  With programmatic dependent launch (default) the kernel may be
+// scheduled while its predecessor drains; it waits (griddepcontrol.wait at its top) before touching any data.
+template <typename... KA, typename... A>
+static void klaunch(fredopt_plan* P, void (*kern)(KA...), int grid, int block, A... args) {
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3((unsigned)grid); cfg.blockDim = dim3((unsigned)block); cfg.dynamicSmemBytes = 0; cfg.stream = P->stream;
+    cudaLaunchAttribute at;
+    at.id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    at.val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = &at; cfg.numAttrs = P->use_pdl ? 1 : 0;
+    const cudaError_t e = cudaLaunchKernelEx(&cfg, kern, KA(args)...);
+    if (e != cudaSuccess && P->launch_err == cudaSuccess) P->launch_err = e;
+    ++P->launches;
+}
+
+// ---- plan_build.cu
+int build_transpose(fredopt_plan* P, RowSet& R);                 // CSR of the transposes of a row set (lazily for ROWS_ALL)
+// ---- iterate.cu
+int fwd_grid(fredopt_plan* P, long long n);                      // grid of the item kernels (one warp per item, round-robin)
+void state_init(fredopt_plan* P);                                // device state at creation
+extern const ResidArgs NO_RESID;
+void launch_forward(fredopt_plan* P, const RowSet& R, const uint8_t* mode, const double* x, double* oD, double* oL, int epi,
+                    int write_uv = 0);
+void launch_transpose(fredopt_plan* P, int tepi, const RowSet& R, const uint8_t* mode, const GatherVec& vec, double* g_out,
+                      double* x, float* f_out);
+void launch_finalize(fredopt_plan* P, int n_part);

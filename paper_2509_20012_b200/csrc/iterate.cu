@@ -1,0 +1,338 @@
+// iterate.cu -- launches of the hot kernels and the orchestration of fredopt_iterate: one iteration of SuperiorDLET (Fig. 3,
+// PAPER.md:165-199) around the AMSrelaxDLET step (Fig. 2) as a replayed CUDA graph; options, statistics,
+// per-pass timing.
+#include "fredopt_plan.cuh"
+#include "kernels_iter.cuh"
+
+// ============================================================================================ launches
+static void ev_begin(fredopt_plan* P, int pass) {
+    if (!P->time_passes) return;
+    EventPair ep;
+    cudaEventCreate(&ep.a); cudaEventCreate(&ep.b);
+    ep.pass = pass;
+    cudaEventRecord(ep.a, P->stream);
+    P->events.push_back(ep);
+}
+static void ev_end(fredopt_plan* P) {
+    if (!P->time_passes) return;
+    cudaEventRecord(P->events.back().b, P->stream);
+}
+
+// grid of the item kernels: one warp per item up to FWD_CTAS_PER_SM resident-CTA-fulls per SM (then round-robin)
+constexpr int GRAPH_UNROLL = 8;       // iterations captured into the long graph
+constexpr int FWD_CTAS_PER_SM = 2 * FWD_MIN_CTAS;   // 2 waves of the CTAs an SM holds (launch bounds of k_forward / k_transpose)
+int fwd_grid(fredopt_plan* P, long long n) {
+    const int cap = P->sm_count * FWD_CTAS_PER_SM < MAX_PARTIALS ? P->sm_count * FWD_CTAS_PER_SM : MAX_PARTIALS;
+    return grid_for(n, FWD_WARPS, cap);
+}
+
+
+const ResidArgs NO_RESID{nullptr, nullptr, nullptr, GatherVec{nullptr, nullptr, nullptr}, nullptr, nullptr, nullptr, nullptr};
+
+// epi: EPI_STORE (d, l), EPI_STORE_PQ (d, l and the cost residuals p, q), EPI_CPART (Dg, Lg and partial sums of c),
+// EPI_RESID (d, l and the residual / violation epilogue: step coefficients u, v if write_uv, statistics partials)
+void launch_forward(fredopt_plan* P, const RowSet& R, const uint8_t* mode, const double* x, double* oD, double* oL, int epi,
+                    int write_uv) {
+    if (R.n == 0) {
+        if (epi == EPI_CPART) cudaMemsetAsync(P->cpart, 0, sizeof(double) * MAX_PARTIALS, P->stream);
+        if (epi == EPI_RESID) {   // nothing to visit: zero statistics (finalize reads one partial)
+            cudaMemsetAsync(P->part_prox, 0, 8, P->stream); cudaMemsetAsync(P->part_phi, 0, 8, P->stream); cudaMemsetAsync(P->part_cnt, 0, 8, P->stream);
+            if (write_uv) klaunch(P, k_sweep_end, grid_for(P->S, 256, 1 << 30), 256, P->S, P->x, P->st);   // k, eta^k still advance
+        }
+        return;
+    }
+    const int g = fwd_grid(P, R.n);
+    const GatherVec none{nullptr, nullptr, nullptr};
+    ResidArgs ra = NO_RESID;
+    if (epi == EPI_RESID) ra = ResidArgs{P->nD, P->nL, P->nT, write_uv ? P->uv : none, P->part_prox, P->part_phi, P->part_cnt, P->st};
+#define FWD_LAUNCH(E, I16, COL, PQ, TAB, CP)                                                                                   \
+    klaunch(P, k_forward<E, I16>, g, FWD_THREADS, R.n, R.items, R.vox, mode, COL, R.valD, R.valL, x, oD, oL, PQ, TAB, CP, P->st, \
+            nullptr, nullptr, 0, ra)
+    if (R.col16) {
+        if (epi == EPI_CPART) FWD_LAUNCH(EPI_CPART, true, R.col16, none, P->tab, P->cpart);
+        else if (epi == EPI_STORE_PQ) FWD_LAUNCH(EPI_STORE_PQ, true, R.col16, P->pq, P->tab, P->part_phi);
+        else if (epi == EPI_RESID) FWD_LAUNCH(EPI_RESID, true, R.col16, none, P->tab, nullptr);
+        else FWD_LAUNCH(EPI_STORE, true, R.col16, none, nullptr, nullptr);
+    } else {
+        if (epi == EPI_CPART) FWD_LAUNCH(EPI_CPART, false, R.col, none, P->tab, P->cpart);
+        else if (epi == EPI_STORE_PQ) FWD_LAUNCH(EPI_STORE_PQ, false, R.col, P->pq, P->tab, P->part_phi);
+        else if (epi == EPI_RESID) FWD_LAUNCH(EPI_RESID, false, R.col, none, P->tab, nullptr);
+        else FWD_LAUNCH(EPI_STORE, false, R.col, none, nullptr, nullptr);
+    }
+#undef FWD_LAUNCH
+}
+static int cpart_count(fredopt_plan* P) { return P->act.n ? fwd_grid(P, P->act.n) : MAX_PARTIALS; }
+
+void launch_transpose(fredopt_plan* P, int tepi, const RowSet& R, const uint8_t* mode, const GatherVec& vec, double* g_out, double* x,
+                      float* f_out) {
+    if (R.t_n_items == 0 && tepi != TEPI_UPDATE) return;          // nothing to add; the update still clamps (R6)
+    if (R.t_n_items > 0) {
+        if (R.t_col16)
+            klaunch(P, k_transpose<true>, fwd_grid(P, R.t_n_items), FWD_THREADS, R.t_n_items, R.t_items, R.t_item_slot, mode, R.t_col16,
+                    R.t_valD, R.t_valL, vec, R.t_partial);
+        else
+            klaunch(P, k_transpose<false>, fwd_grid(P, R.t_n_items), FWD_THREADS, R.t_n_items, R.t_items, R.t_item_slot, mode, R.t_col,
+                    R.t_valD, R.t_valL, vec, R.t_partial);
+    }
+    const int gc = grid_for(P->S, 256, 1 << 30);
+    if (tepi == TEPI_GRAD) klaunch(P, k_combine<TEPI_GRAD>, gc, 256, P->S, R.t_item_ptr, R.t_partial, g_out, P->gpart, x, P->st, f_out);
+    else if (tepi == TEPI_UPDATE) klaunch(P, k_combine<TEPI_UPDATE>, gc, 256, P->S, R.t_item_ptr, R.t_partial, g_out, P->gpart, x, P->st, f_out);
+    else klaunch(P, k_combine<TEPI_F32>, gc, 256, P->S, R.t_item_ptr, R.t_partial, g_out, P->gpart, x, P->st, f_out);
+}
+
+static int res_grid(fredopt_plan* P) {
+    const int cap = P->sm_count * 4 < MAX_PARTIALS ? P->sm_count * 4 : MAX_PARTIALS;
+    const long long n = P->act.n > P->S ? P->act.n : P->S;
+    return grid_for(n, ROW_THREADS, cap);
+}
+
+static void launch_residual(fredopt_plan* P, double* d, double* l, int use_beta, int final, int write_uv) {
+    const int g = res_grid(P);
+    klaunch(P, k_residual, g, ROW_THREADS, P->act.n, P->act.items, P->tab, P->st, d, l, P->Dg, P->Lg, P->nD, P->nL, P->nT, P->uv, P->pq,
+            P->x, P->g, P->S, P->part_prox, P->part_phi, P->part_cnt, use_beta, final, write_uv);
+}
+
+// n_part: how many per-CTA partial sums the last residual pass wrote (k_residual: res_grid; forward epilogue: fwd_grid)
+void launch_finalize(fredopt_plan* P, int n_part) {
+    klaunch(P, k_finalize_stats, 1, 1024, P->st, P->part_prox, P->part_phi, P->part_cnt, n_part);
+}
+
+// Block-sequential AMS sweep (reading R23): Fig. 2's loop nest -- dose kind over the structures, then cDLET, then the LETd
+// rows -- one (forward over the block's rows, residual, transposed over the block's items, update) group per block.
+static void enqueue_block_sweep(fredopt_plan* P) {
+    const RowSet& A = P->act;
+    klaunch(P, k_sweep_begin, 1, 1, P->st);
+    std::vector<long long> row_begin((size_t)P->n_struct + 1, 0);
+    for (int s = 0; s < P->n_struct; ++s) row_begin[s + 1] = row_begin[s] + (long long)P->h_tab[s].rows;
+    const int kind_flag[3] = {F_DOSE_SLAB, F_DL_SLAB, F_LETD};
+    const int kind_mode[3] = {1, 2, 3};
+    const GatherVec none{nullptr, nullptr, nullptr};
+    for (int kind = 0; kind < 3; ++kind)
+        for (int s = 0; s < P->n_struct; ++s) {
+            const StructInfo& T = P->h_tab[s];
+            if (!(T.flags & kind_flag[kind])) continue;
+            const long long rb = row_begin[s], re = row_begin[s + 1], nr = re - rb;
+            if (nr == 0) continue;
+            const uint8_t* md = P->mode_fixed + (size_t)kind_mode[kind] * P->max_seg;
+            ev_begin(P, FREDOPT_PASS_FORWARD_X);
+            {
+                const int g = fwd_grid(P, nr);
+                if (A.col16) klaunch(P, k_forward<EPI_STORE, true>, g, FWD_THREADS, nr, A.items + rb, A.vox + rb, md, A.col16, A.valD, A.valL, P->x, P->d + rb, P->l + rb, none, nullptr, nullptr, nullptr, nullptr, nullptr, 0, NO_RESID);
+                else klaunch(P, k_forward<EPI_STORE, false>, g, FWD_THREADS, nr, A.items + rb, A.vox + rb, md, A.col, A.valD, A.valL, P->x, P->d + rb, P->l + rb, none, nullptr, nullptr, nullptr, nullptr, nullptr, 0, NO_RESID);
+            }
+            ev_end(P);
+            ev_begin(P, FREDOPT_PASS_RESIDUAL);
+            const int gr = grid_for(nr, ROW_THREADS, P->sm_count * 4 < MAX_PARTIALS ? P->sm_count * 4 : MAX_PARTIALS);
+            klaunch(P, k_block_residual, gr, ROW_THREADS, rb, re, s, kind, P->tab, P->st, P->d, P->l, P->nD, P->nL, P->nT, P->uv, P->part_prox);
+            ev_end(P);
+            const long long m = (long long)T.part_kind[kind];
+            const long long ib = A.t_seg_item_begin.empty() ? 0 : A.t_seg_item_begin[s], ie = A.t_seg_item_begin.empty() ? 0 : A.t_seg_item_begin[s + 1];
+            if (m == 0) continue;                      // no row of the block has a non-zero norm: violations counted, no step
+            ev_begin(P, FREDOPT_PASS_TRANSPOSE_B);
+            if (ie > ib) {
+                const int g = fwd_grid(P, ie - ib);
+                if (A.t_col16) klaunch(P, k_transpose<true>, g, FWD_THREADS, ie - ib, A.t_items_seg + ib, A.t_slot_seg + ib, md, A.t_col16, A.t_valD, A.t_valL, P->uv, A.t_partial);
+                else klaunch(P, k_transpose<false>, g, FWD_THREADS, ie - ib, A.t_items_seg + ib, A.t_slot_seg + ib, md, A.t_col, A.t_valD, A.t_valL, P->uv, A.t_partial);
+            }
+            const double factor = (T.w < 1.0 ? T.w : 1.0) / (double)m;
+            klaunch(P, k_combine_block, grid_for(P->S, 256, 1 << 30), 256, P->S, A.t_slot_ptr, s, A.n_seg, A.t_H, A.t_partial, P->x, P->st, factor,
+                    P->part_prox, gr);
+            ev_end(P);
+        }
+    klaunch(P, k_sweep_end, grid_for(P->S, 256, 1 << 30), 256, P->S, P->x, P->st);
+}
+
+// one iteration of Fig. 3 around the simultaneous Fig. 2 step; returns the number of kernels enqueued
+static int enqueue_iteration(fredopt_plan* P, bool sa) {
+    const long long before = P->launches;
+    if (sa) {
+        ev_begin(P, FREDOPT_PASS_FORWARD_X);
+        launch_forward(P, P->act, P->mode_union, P->x, P->d, P->l, EPI_STORE_PQ);                      // a1, a2: d, l, p, q
+        ev_end(P);
+        for (long long t = 0; t < P->reductionsN; ++t) {
+            ev_begin(P, FREDOPT_PASS_TRANSPOSE_G);
+            launch_transpose(P, TEPI_GRAD, P->act, P->mode_cost, P->pq, P->g, nullptr, nullptr);       // a3: g = D^T p + L^T q
+            ev_end(P);
+            ev_begin(P, FREDOPT_PASS_FORWARD_G);
+            launch_forward(P, P->act, P->mode_union, P->g, P->Dg, P->Lg, EPI_CPART);                   // a5: Dg, Lg, c
+            ev_end(P);
+            ev_begin(P, FREDOPT_PASS_SELECT);
+            klaunch(P, k_select, 1, 1024, P->st, P->gpart, P->act.t_n_items ? grid_for(P->S, 256, 1 << 30) : 0, P->cpart, cpart_count(P),
+                    P->part_phi, P->act.n == 0 ? 0 : t == 0 ? fwd_grid(P, P->act.n) : res_grid(P), P->act.n,
+                    P->act.items, P->tab, P->d, P->l, P->Dg, P->Lg);                                     // a4, a6: beta
+            ev_end(P);
+            ev_begin(P, FREDOPT_PASS_RESIDUAL);
+            const int last = t == P->reductionsN - 1 && !P->block_sequential;
+            launch_residual(P, P->d, P->l, 1, last, last);                                             // x', d', l'; a7
+            ev_end(P);
+        }
+    } else if (!P->block_sequential) {      // pure feasibility-seeking: the residual / violation work is the forward pass's epilogue
+        ev_begin(P, FREDOPT_PASS_FORWARD_X);
+        launch_forward(P, P->act, P->mode_con, P->x, P->d, P->l, EPI_RESID, 1);                       // a1 + a7
+        ev_end(P);
+    }
+    if (P->block_sequential) {
+        enqueue_block_sweep(P);
+        return (int)(P->launches - before);
+    }
+    ev_begin(P, FREDOPT_PASS_TRANSPOSE_B);
+    launch_transpose(P, TEPI_UPDATE, P->act, P->mode_con, P->uv, nullptr, P->x, nullptr);              // a8, a9
+    ev_end(P);
+    return (int)(P->launches - before);
+}
+
+
+void state_init(fredopt_plan* P) {
+    k_set_params<<<1, 1, 0, P->stream>>>(P->st, 1.0, 0.0, 0.5, 1.0, 200, 1, 0, 2);
+}
+
+// ============================================================================================ API
+extern "C" {
+
+int fredopt_set_option(fredopt_plan* P, int32_t key, double value) {
+    if (!P) return FREDOPT_INVALID_ARG;
+    switch (key) {
+        case FREDOPT_OPT_ETA: if (!(value > 0.0) || value > 1.0) return FREDOPT_INVALID_ARG; P->eta = value; break;
+        case FREDOPT_OPT_REDUCTIONS:
+            if (value < 1.0 || value > 1000.0) return FREDOPT_INVALID_ARG;
+            P->reductionsN = (long long)value;
+            break;
+        case FREDOPT_OPT_ACCEPT_CHECK: P->accept_check = value != 0.0; break;
+        case FREDOPT_OPT_MAX_TRIALS: if (value < 1.0) return FREDOPT_INVALID_ARG; P->max_trials = (long long)value; break;
+        case FREDOPT_OPT_RESET: {
+            P->started = false;
+            DevState h;
+            CK(cudaMemcpyAsync(&h, P->st, sizeof(DevState), cudaMemcpyDeviceToHost, P->stream));
+            CK(cudaStreamSynchronize(P->stream));
+            h.k = 0; h.s = 0; h.trials = 0; h.last_beta = 0.0; h.eta_pow = 1.0; h.beta_acc = 0.0;
+            CK(cudaMemcpyAsync(P->st, &h, sizeof(DevState), cudaMemcpyHostToDevice, P->stream));
+            CK(cudaStreamSynchronize(P->stream));
+            break;
+        }
+        case FREDOPT_OPT_USE_GRAPH: P->use_graph = value != 0.0; break;
+        case FREDOPT_OPT_USE_PDL:
+            if (P->use_pdl != (value != 0.0)) {            // the launch attribute is part of a captured graph: capture again
+                P->use_pdl = value != 0.0;
+                for (int i = 0; i < 8; ++i) if (P->gexec[i]) { cudaGraphExecDestroy(P->gexec[i]); P->gexec[i] = nullptr; }
+            }
+            break;
+        case FREDOPT_OPT_BLOCK_SEQUENTIAL: P->block_sequential = value != 0.0; break;
+        case FREDOPT_OPT_NORMALIZE_GRAD: P->normalize_grad = value != 0.0; break;
+        case FREDOPT_OPT_ONE_SIDED_COST: P->one_sided_cost = value != 0.0; break;
+        case FREDOPT_OPT_TIME_PASSES:
+            P->time_passes = value != 0.0;
+            if (P->time_passes) {
+                for (auto& ep : P->events) { cudaEventDestroy(ep.a); cudaEventDestroy(ep.b); }
+                P->events.clear();
+                for (int i = 0; i < FREDOPT_N_PASSES; ++i) { P->pass_ms[i] = 0; P->pass_launches[i] = 0; }
+            }
+            break;
+        default: return FREDOPT_INVALID_ARG;
+    }
+    return FREDOPT_OK;
+}
+
+int fredopt_iterate(fredopt_plan* P, int32_t n_iter, float lambda, float beta0, float a) {
+    if (!P || n_iter < 0) return FREDOPT_INVALID_ARG;
+    if (!(lambda > 0.f) || !(lambda <= 2.f) || !(beta0 >= 0.f) || !std::isfinite(beta0) || !(a > 0.f) || !(a < 1.f))
+        return FREDOPT_INVALID_ARG;
+    // the step-size sequence beta0 a^s belongs to the plan (R8): the first superiorized call latches (beta0, a); calls with
+    // beta0 = 0 neither latch nor consume it; a different pair needs FREDOPT_OPT_RESET
+    int latch = 0;
+    if (beta0 != 0.f && n_iter > 0) {
+        if (!P->started) { latch = 1; P->latched_beta0 = beta0; P->latched_a = a; P->started = true; }
+        else if (beta0 != P->latched_beta0 || a != P->latched_a) return FREDOPT_INVALID_ARG;
+    }
+    k_set_params<<<1, 1, 0, P->stream>>>(P->st, (double)lambda, (double)beta0, (double)a, P->eta, P->max_trials, P->accept_check,
+                                           (P->normalize_grad ? SF_NORMALIZE_GRAD : 0) | (P->one_sided_cost ? SF_ONE_SIDED : 0), latch);
+    ++P->launches;
+    const bool sa = beta0 != 0.f;
+    if (n_iter > 0) {
+        const bool graph = P->use_graph && !P->time_passes;
+        if (graph) {
+            // two graphs per form: one iteration, and GRAPH_UNROLL iterations back to back (fewer graph launches for the
+            // small plans, whose iteration lasts about as long as a graph launch costs)
+            const int form = 2 * P->block_sequential + (sa ? 1 : 0);
+            int left = n_iter;
+            // (measured: +3 % on configs[0]-[1], +1 % on configs[2], nothing at configs[3]: long graph only below 5e7 non-zeros)
+            for (int u = P->act.nnz < 50000000LL ? 1 : 0; u >= 0; --u) {
+                const int per = u ? GRAPH_UNROLL : 1, gi = 2 * form + u;
+                // both graphs are built at the first call of a form, so that no later (timed) call pays for a capture
+                if (!P->gexec[gi] || P->gexec_red[gi] != P->reductionsN) {
+                    if (P->gexec[gi]) { cudaGraphExecDestroy(P->gexec[gi]); P->gexec[gi] = nullptr; }
+                    cudaGraph_t gr = nullptr;
+                    CK(cudaStreamBeginCapture(P->stream, cudaStreamCaptureModeThreadLocal));
+                    const long long l0 = P->launches;
+                    int nk = 0;
+                    P->launch_err = cudaSuccess;
+                    for (int r = 0; r < per; ++r) nk += enqueue_iteration(P, sa);
+                    P->launches = l0;
+                    cudaError_t e = cudaStreamEndCapture(P->stream, &gr);      // always ends the capture, also after a failed launch
+                    if (e == cudaSuccess && P->launch_err != cudaSuccess) e = P->launch_err;
+                    if (e != cudaSuccess) {                                    // nothing was enqueued: the plan's x, k, s are untouched
+                        if (gr) cudaGraphDestroy(gr);
+                        if (latch) P->started = false;
+                        CK(e);
+                    }
+                    e = cudaGraphInstantiate(&P->gexec[gi], gr, 0);
+                    cudaGraphDestroy(gr);
+                    if (e != cudaSuccess) { P->gexec[gi] = nullptr; if (latch) P->started = false; }
+                    CK(e);
+                    P->gexec_red[gi] = P->reductionsN;
+                    P->gexec_kernels[gi] = nk;
+                }
+                for (; left >= per; left -= per) { CK(cudaGraphLaunch(P->gexec[gi], P->stream)); P->launches += P->gexec_kernels[gi]; }
+            }
+        } else {
+            P->launch_err = cudaSuccess;
+            for (int it = 0; it < n_iter && P->launch_err == cudaSuccess; ++it) enqueue_iteration(P, sa);
+            CK(P->launch_err);
+        }
+        if (!P->block_sequential)                         // block mode keeps its sweep statistics in the state already
+            launch_finalize(P, sa ? res_grid(P) : (P->act.n ? fwd_grid(P, P->act.n) : 1));
+    }
+    CK(cudaGetLastError());
+    return FREDOPT_OK;
+}
+
+int fredopt_get_stats(fredopt_plan* P, fredopt_stats* out) {
+    if (!P || !out) return FREDOPT_INVALID_ARG;
+    DevState h;
+    CK(cudaMemcpyAsync(&h, P->st, sizeof(DevState), cudaMemcpyDeviceToHost, P->stream));
+    CK(cudaStreamSynchronize(P->stream));
+    out->k = h.k; out->s = h.s; out->trials = h.trials; out->n_violated = h.n_viol;
+    out->n_sets = h.n_sets; out->n_zero_norm_sets = h.n_zero;
+    out->n_active_rows = P->act.n; out->nnz = P->nnz; out->nnz_active = P->act.nnz;
+    long long b = 0;
+    const int sa_passes[] = {FREDOPT_PASS_FORWARD_X, FREDOPT_PASS_TRANSPOSE_G, FREDOPT_PASS_FORWARD_G, FREDOPT_PASS_SELECT,
+                             FREDOPT_PASS_RESIDUAL, FREDOPT_PASS_TRANSPOSE_B};
+    for (int p : sa_passes) b += P->pass_bytes[p];
+    out->alg_bytes_iter = b;
+    out->last_beta = h.last_beta; out->phi = h.phi; out->prox = h.prox; out->weight_sum = h.W;
+    return FREDOPT_OK;
+}
+
+int fredopt_get_pass_times(fredopt_plan* P, double* ms, int64_t* launches) {
+    if (!P || !ms || !launches) return FREDOPT_INVALID_ARG;
+    CK(cudaStreamSynchronize(P->stream));
+    for (auto& ep : P->events) {
+        float t = 0.f;
+        if (cudaEventElapsedTime(&t, ep.a, ep.b) == cudaSuccess) { P->pass_ms[ep.pass] += t; P->pass_launches[ep.pass] += 1; }
+        cudaEventDestroy(ep.a); cudaEventDestroy(ep.b);
+    }
+    cudaGetLastError();
+    P->events.clear();
+    for (int i = 0; i < FREDOPT_N_PASSES; ++i) { ms[i] = P->pass_ms[i]; launches[i] = P->pass_launches[i]; }
+    return FREDOPT_OK;
+}
+
+int fredopt_get_pass_bytes(fredopt_plan* P, int64_t* bytes) {
+    if (!P || !bytes) return FREDOPT_INVALID_ARG;
+    for (int i = 0; i < FREDOPT_N_PASSES; ++i) bytes[i] = P->pass_bytes[i];
+    return FREDOPT_OK;
+}
+
+int64_t fredopt_launch_count(fredopt_plan* P) { return P ? P->launches : 0; }
+
+
+}  // extern "C"

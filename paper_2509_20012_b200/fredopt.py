@@ -17,14 +17,14 @@ LIB_PATH = os.path.join(_HERE, "libfredopt.so")
 
 OK, INVALID_ARG, OUT_OF_MEMORY, CUDA_ERROR, UNSUPPORTED_ARCH, UNSUPPORTED = 0, -1, -2, -3, -4, -5
 OPT_ETA, OPT_REDUCTIONS, OPT_ACCEPT_CHECK, OPT_MAX_TRIALS, OPT_RESET, OPT_USE_GRAPH, OPT_TIME_PASSES, \
-    OPT_BLOCK_SEQUENTIAL, OPT_NORMALIZE_GRAD, OPT_ONE_SIDED_COST = range(10)
+    OPT_BLOCK_SEQUENTIAL, OPT_NORMALIZE_GRAD, OPT_ONE_SIDED_COST, OPT_USE_PDL = range(11)
 ROWS_ALL, ROWS_ACTIVE = 0, 1
 PASS_NAMES = ("forward_x", "transpose_g", "forward_g", "select", "residual", "transpose_b")
 N_PASSES = len(PASS_NAMES)
 
 # every symbol include/fredopt.h declares (tests check the library exports exactly these)
 SYMBOLS = (
-    "fredopt_create", "fredopt_destroy", "fredopt_set_weights", "fredopt_get_weights", "fredopt_get_weights_f64",
+    "fredopt_create", "fredopt_create_ex", "fredopt_destroy", "fredopt_set_weights", "fredopt_get_weights", "fredopt_get_weights_f64",
     "fredopt_dose_let", "fredopt_iterate", "fredopt_proximity", "fredopt_set_option", "fredopt_get_stats",
     "fredopt_spmv_forward", "fredopt_spmv_transpose", "fredopt_get_pass_times", "fredopt_get_pass_bytes",
     "fredopt_launch_count", "fredopt_stream_read", "fredopt_strerror", "fredopt_last_cuda_error",
@@ -50,6 +50,10 @@ class _Bounds(C.Structure):
                                          "dose_ref", "dl_ref")]
 
 
+class _CreateOptions(C.Structure):
+    _fields_ = [("struct_size", C.c_int32), ("index_width", C.c_int32)]
+
+
 class Stats(C.Structure):
     _fields_ = [(n, C.c_int64) for n in ("k", "s", "trials", "n_violated", "n_sets", "n_zero_norm_sets",
                                          "n_active_rows", "nnz", "nnz_active", "alg_bytes_iter")] + \
@@ -71,6 +75,8 @@ def _load():
     lib = C.CDLL(LIB_PATH)
     vp, i64, i32, f32, f64 = C.c_void_p, C.c_int64, C.c_int32, C.c_float, C.c_double
     lib.fredopt_create.argtypes = [C.POINTER(_Csr), C.POINTER(_Csr), vp, C.POINTER(_Bounds), i32, vp, C.POINTER(vp)]
+    lib.fredopt_create_ex.argtypes = [C.POINTER(_Csr), C.POINTER(_Csr), vp, C.POINTER(_Bounds), i32, vp, C.POINTER(_CreateOptions),
+                                      C.POINTER(vp)]
     lib.fredopt_destroy.argtypes = [vp]
     lib.fredopt_destroy.restype = None
     lib.fredopt_set_weights.argtypes = [vp, vp]
@@ -131,10 +137,11 @@ def _check(rc, where):
 class Plan:
     """One plan = one GPU, one stream.  Mirrors the C calls one to one."""
 
-    def __init__(self, n_rows, n_cols, D, L, voxel_labels, bounds, stream=None):
+    def __init__(self, n_rows, n_cols, D, L, voxel_labels, bounds, stream=None, **create_options):
         """D, L: (row_ptr int64, col_idx int32, values float32) triples; bounds: float32 [n_struct, 8] rows of
         (weight, dose_lo, dose_hi, dl_lo, dl_hi, letd_max, dose_ref, dl_ref), NaN = absent;
-        stream: a raw cudaStream_t integer (e.g. torch.cuda.current_stream().cuda_stream) or None."""
+        stream: a raw cudaStream_t integer (e.g. torch.cuda.current_stream().cuda_stream) or None;
+        create_options: fields of fredopt_create_options (index_width=...): fredopt_create_ex is called when given."""
         self._h = None
         self.n_rows, self.n_cols = int(n_rows), int(n_cols)
 
@@ -151,8 +158,13 @@ class Plan:
         for s in range(n_struct):
             barr[s] = _Bounds(*[float(t) for t in b[s]])
         h = C.c_void_p()
-        rc = _lib.fredopt_create(C.byref(cD), C.byref(cL), _ptr(voxel_labels, np.int32, self.n_rows), barr, n_struct,
-                                 C.c_void_p(stream or 0), C.byref(h))
+        if create_options:
+            opt = _CreateOptions(struct_size=C.sizeof(_CreateOptions), **{k: int(v) for k, v in create_options.items()})
+            rc = _lib.fredopt_create_ex(C.byref(cD), C.byref(cL), _ptr(voxel_labels, np.int32, self.n_rows), barr, n_struct,
+                                        C.c_void_p(stream or 0), C.byref(opt), C.byref(h))
+        else:
+            rc = _lib.fredopt_create(C.byref(cD), C.byref(cL), _ptr(voxel_labels, np.int32, self.n_rows), barr, n_struct,
+                                     C.c_void_p(stream or 0), C.byref(h))
         _check(rc, "fredopt_create")
         self._h = h
 
@@ -249,7 +261,7 @@ class Plan:
         _check(_lib.fredopt_stream_read(self._h, _ptr(device_buf), int(nbytes), int(reps)), "fredopt_stream_read")
 
 
-def from_plan(plan, stream=None) -> Plan:
+def from_plan(plan, stream=None, **create_options) -> Plan:
     """Plan over a plangen.Plan; tensors are passed where they live (host or device)."""
     return Plan(plan.n_rows, plan.n_cols, (plan.row_ptr, plan.col_idx, plan.val_D),
-                (plan.row_ptr, plan.col_idx, plan.val_L), plan.labels, plan.bounds, stream=stream)
+                (plan.row_ptr, plan.col_idx, plan.val_L), plan.labels, plan.bounds, stream=stream, **create_options)

@@ -41,6 +41,10 @@ def _rel_l2(a, b):
     return float(np.linalg.norm(a - b) / max(np.linalg.norm(b), 1e-300))
 
 
+# both stored index forms of a plan: automatic (16-bit where exact) and int32 everywhere (fredopt_create_options.index_width)
+INDEX_FORMS = [pytest.param({}, id="idx16"), pytest.param({"index_width": 32}, id="idx32")]
+
+
 def _assert_fwd(got, ref, what):
     got = got.astype(np.float64)
     # fp32 output rounding: half an ulp = 6e-8 relative; the bar is 1e-5
@@ -89,10 +93,11 @@ def test_forward_active_rows_config0(fredopt, plan0):
     _assert_fwd(l, np.where(lab != 0, l_ref, 0.0), "L x (active)")
 
 
+@pytest.mark.parametrize("copt", INDEX_FORMS)
 @pytest.mark.parametrize("rows", ["all", "active"])
-def test_transpose_config0(fredopt, plan0, rows):
+def test_transpose_config0(fredopt, plan0, rows, copt):
     orc = _oracle(plan0)
-    gp = fredopt.from_plan(plan0)
+    gp = fredopt.from_plan(plan0, **copt)
     V = plan0.n_rows
     # signed, dense coefficient vectors (lower-bound violations are negative)
     u = (pg.uniform01_array(11, V) - 0.4).astype(np.float32)
@@ -124,9 +129,9 @@ def test_proximity_config0(fredopt, plan0):
 
 
 # ------------------------------------------------------------------------------------------ iteration
-def _run_pair(fredopt, plan, n_iter, lam, beta0, a, opts=(), gp=None, orc=None):
+def _run_pair(fredopt, plan, n_iter, lam, beta0, a, opts=(), gp=None, orc=None, copt=None):
     orc = orc or _oracle(plan)
-    gp = gp or fredopt.from_plan(plan)
+    gp = gp or fredopt.from_plan(plan, **(copt or {}))
     for k, v in opts:
         orc.set_option(k, v); gp.set_option(k, v)
     orc.set_x(plan.x0); gp.set_weights(plan.x0)
@@ -147,10 +152,11 @@ def _assert_state(gp, orc, tol=TOL_X20):
         assert abs(sg["last_beta"] - so["last_beta"]) <= 1e-15 * so["last_beta"]
 
 
+@pytest.mark.parametrize("copt", INDEX_FORMS)
 @pytest.mark.parametrize("n_iter", [1, 20, 50])
-def test_superiorized_iterations_config0(fredopt, plan0, n_iter):
+def test_superiorized_iterations_config0(fredopt, plan0, n_iter, copt):
     sp = plan0.spec
-    gp, orc = _run_pair(fredopt, plan0, n_iter, sp.lam, sp.beta0, sp.a)
+    gp, orc = _run_pair(fredopt, plan0, n_iter, sp.lam, sp.beta0, sp.a, copt=copt)
     _assert_state(gp, orc)
     assert (_gpu_x(gp) >= 0).all()
 
@@ -176,6 +182,14 @@ def test_options_eta_reductions_accept_maxtrials(fredopt, plan0):
                  [(f.OPT_ETA, 0.95), (f.OPT_REDUCTIONS, 2)]):
         gp, orc = _run_pair(fredopt, plan0, 12, 1.3, 1.0, 0.9, opts)
         _assert_state(gp, orc)
+    # block-sequential sweep after two reductions (the residual pass of the last reduction writes no u, v there)
+    from oracle import oracle as om
+    gp = f.from_plan(plan0); orc = _oracle(plan0)
+    for o_, m_ in ((gp, f), (orc, om)):
+        o_.set_option(m_.OPT_BLOCK_SEQUENTIAL, 1); o_.set_option(m_.OPT_REDUCTIONS, 2)
+    gp.set_weights(plan0.x0); orc.set_x(plan0.x0)
+    gp.iterate(12, 1.3, 1.0, 0.9); orc.iterate(12, 1.3, 1.0, 0.9)
+    _assert_block_state(gp, orc)
     # a cost step far too large: every trial up to the cap is rejected, x is kept, s still advances (R10)
     gp, orc = _run_pair(fredopt, plan0, 2, 1.0, 1.0e6, 0.999, [(f.OPT_MAX_TRIALS, 5)])
     _assert_state(gp, orc)
@@ -187,8 +201,11 @@ def test_state_two_calls_equal_one_and_graph_equals_launches(fredopt, plan0):
     a = f.from_plan(plan0); a.set_weights(plan0.x0); a.iterate(20, 1.0, 1.0, 0.99)
     b = f.from_plan(plan0); b.set_weights(plan0.x0); b.iterate(10, 1.0, 1.0, 0.99); b.iterate(10, 1.0, 1.0, 0.99)
     c = f.from_plan(plan0); c.set_option(f.OPT_USE_GRAPH, 0); c.set_weights(plan0.x0); c.iterate(20, 1.0, 1.0, 0.99)
+    d = f.from_plan(plan0); d.set_option(f.OPT_USE_PDL, 0); d.set_weights(plan0.x0); d.iterate(20, 1.0, 1.0, 0.99)
+    e = f.from_plan(plan0); e.set_weights(plan0.x0); e.iterate(8, 1.0, 1.0, 0.99); e.set_option(f.OPT_USE_PDL, 0); e.iterate(12, 1.0, 1.0, 0.99)
     xa, xb, xc = _gpu_x(a), _gpu_x(b), _gpu_x(c)
     assert np.array_equal(xa, xb) and np.array_equal(xa, xc)      # no atomics: bitwise reproducible
+    assert np.array_equal(xa, _gpu_x(d)) and np.array_equal(xa, _gpu_x(e))     # with and without programmatic dependent launch
     # RESET restarts beta at beta0
     a.set_option(f.OPT_RESET, 1); a.set_weights(plan0.x0); a.iterate(20, 1.0, 1.0, 0.99)
     assert np.array_equal(_gpu_x(a), xa)
@@ -439,12 +456,13 @@ def _assert_block_state(gp, orc):
     _assert_state(gp, orc)
 
 
+@pytest.mark.parametrize("copt", INDEX_FORMS)
 @pytest.mark.parametrize("beta0", [0.0, 1.0])
 @pytest.mark.parametrize("lam", [1.0, 1.7])
-def test_block_sequential_config0(fredopt, plan0, beta0, lam):
+def test_block_sequential_config0(fredopt, plan0, beta0, lam, copt):
     """Fig. 2's loop nest block by block (option BLOCK_SEQUENTIAL), pure and superiorized, 20 iterations."""
     from oracle import oracle as om
-    gp = fredopt.from_plan(plan0); orc = _oracle(plan0)
+    gp = fredopt.from_plan(plan0, **copt); orc = _oracle(plan0)
     gp.set_option(fredopt.OPT_BLOCK_SEQUENTIAL, 1); orc.set_option(om.OPT_BLOCK_SEQUENTIAL, 1)
     gp.set_weights(plan0.x0); orc.set_x(plan0.x0)
     for n in (1, 19):                                          # one plain launch sequence, then graph replays
@@ -487,10 +505,10 @@ def test_block_sequential_three_beam_plan(fredopt):
 
 
 # ------------------------------------------------------------------------------------------ full-size configurations
-def _full_size_parity(fredopt, plan, n_sample_rows):
+def _full_size_parity(fredopt, plan, n_sample_rows, copt=None):
     """20 superiorized iterations in the launch configuration bench.py times (one fredopt_iterate call = graph replay),
     sampled outputs of the full forward pass computed one by one by the oracle, and the full transposed pass."""
-    gp = fredopt.from_plan(plan, stream=torch.cuda.current_stream().cuda_stream)
+    gp = fredopt.from_plan(plan, stream=torch.cuda.current_stream().cuda_stream, **(copt or {}))
     orc = _oracle(plan)
     sp = plan.spec
     orc.set_x(plan.x0); gp.set_weights(plan.x0)
@@ -533,9 +551,10 @@ def _full_size_parity(fredopt, plan, n_sample_rows):
     gp.destroy()
 
 
-def test_config1_20_iterations_full_size(fredopt):
-    """BASELINE.json configs[1] (mid-size phantom, L2-resident working set)."""
-    _full_size_parity(fredopt, pg.build_plan(pg.config_spec(1), device="cuda"), 4000)
+@pytest.mark.parametrize("copt", INDEX_FORMS)
+def test_config1_20_iterations_full_size(fredopt, copt):
+    """BASELINE.json configs[1] (mid-size phantom, L2-resident working set), both stored index forms."""
+    _full_size_parity(fredopt, pg.build_plan(pg.config_spec(1), device="cuda"), 4000, copt)
 
 
 def test_config2_20_iterations_full_size(fredopt):
@@ -562,3 +581,124 @@ def test_config3_20_iterations_in_bench_configuration(fredopt):
     plan = pg.build_plan(pg.config_spec(3), device="cuda")
     assert plan.nnz > 1.0e9
     _full_size_parity(fredopt, plan, 20000)
+
+
+# ------------------------------------------------------------------------------------------ horizons, state, limits
+def test_500_iterations_three_beam_plan(fredopt):
+    """The horizon BASELINE.json configs[2] states (500 iterations) on the scaled three-beam plan, which rejects step sizes:
+    s, trials, the violation count and x are compared with the oracle's from-definition accept test every 50 iterations."""
+    plan = pg.build_plan(pg.config_spec(2, scale=0.25), device="cuda")
+    gp = fredopt.from_plan(plan, stream=torch.cuda.current_stream().cuda_stream); orc = _oracle(plan)
+    sp = plan.spec
+    gp.set_weights(plan.x0); orc.set_x(plan.x0)
+    for _ in range(10):
+        gp.iterate(50, sp.lam, sp.beta0, sp.a); orc.iterate(50, sp.lam, sp.beta0, sp.a)
+        _assert_state(gp, orc)
+    st = gp.stats()
+    assert st["k"] == 500 and st["trials"] > 500
+
+
+def test_step_sizes_below_the_resolution_of_the_cost(fredopt, plan0):
+    """a = 0.5: after ~60 trials beta |g|^2 falls below the fp64 resolution of chi^2.  Fig. 3 accepts iff chi^2(x - beta g) <
+    chi^2(x) AS EVALUATED, so from then on every trial is rejected and s advances by max_trials per iteration; the closed form
+    beta c < |g|^2 alone would accept them all.  Identical s while the decrease is far above the resolution; the same
+    per-iteration advance far below it (in the few-ulp zone between, the two summation orders may decide differently)."""
+    gp = fredopt.from_plan(plan0); orc = _oracle(plan0)
+    gp.set_weights(plan0.x0); orc.set_x(plan0.x0)
+    gp.iterate(30, 1.0, 1.0, 0.5); orc.iterate(30, 1.0, 1.0, 0.5)          # beta >= 2^-30: decrease ~1e-9 chi^2
+    _assert_state(gp, orc)
+    gp.iterate(50, 1.0, 1.0, 0.5); orc.iterate(50, 1.0, 1.0, 0.5)          # through the zone
+    sg0, so0 = gp.stats()["s"], orc.stats()["s"]
+    gp.iterate(5, 1.0, 1.0, 0.5); orc.iterate(5, 1.0, 1.0, 0.5)
+    assert gp.stats()["s"] - sg0 == 5 * 200 and orc.stats()["s"] - so0 == 5 * 200
+    xg, xo = _gpu_x(gp), orc.get_x()
+    assert _rel_l2(xg, xo) <= TOL_X20
+    assert gp.proximity(None)[1] == orc.proximity(None)[1]
+
+
+def test_step_size_sequence_belongs_to_the_plan(fredopt, plan0):
+    """GPU twin of oracle pin 26 (reading R8): AMS calls neither latch nor consume beta0 a^s; another pair needs a RESET."""
+    f = fredopt
+    gp = f.from_plan(plan0); orc = _oracle(plan0)
+    gp.set_weights(plan0.x0); orc.set_x(plan0.x0)
+    for n, b0, a in ((0, 0.7, 0.5), (2, 0.0, 0.5), (3, 0.5, 0.9), (2, 0.0, 0.9), (3, 0.5, 0.9)):
+        gp.iterate(n, 1.0, b0, a); orc.iterate(n, 1.0, b0, a)
+    _assert_state(gp, orc)
+    for b0, a in ((0.25, 0.9), (0.5, 0.8)):
+        with pytest.raises(f.FredoptError) as e:
+            gp.iterate(1, 1.0, b0, a)
+        assert e.value.code == f.INVALID_ARG
+    from oracle import oracle as om
+    gp.set_option(f.OPT_RESET, 1); orc.set_option(om.OPT_RESET, 1)
+    gp.iterate(2, 1.0, 0.25, 0.8); orc.iterate(2, 1.0, 0.25, 0.8)
+    _assert_state(gp, orc)
+
+
+def test_negative_weight_on_a_spot_no_labelled_row_touches(fredopt):
+    """Reading R6: the clamp runs over EVERY spot, also one that no labelled row reaches (x stays >= 0 at the ABI)."""
+    nan = np.nan
+    rp = np.array([0, 2, 4, 5], np.int64); ci = np.array([0, 1, 0, 1, 3], np.int32); vv = np.array([1, 2, 3, 1, 5], np.float32)
+    lab = np.array([1, 1, 0], np.int32)                       # spot 2 is in no row at all, spot 3 only in an unlabelled row
+    b = np.array([[1.0, nan, 1.0, nan, nan, nan, 0.5, nan]], np.float32)
+    x0 = np.array([1.0, 1.0, -2.0, -3.0], np.float32)
+    for beta0 in (0.0, 0.5):
+        for block in (0, 1):
+            gp = fredopt.Plan(3, 4, (rp, ci, vv), (rp, ci, vv), lab, b)
+            orc = _oracle_np(3, 4, (rp, ci, vv), (rp, ci, vv), lab, b)
+            from oracle import oracle as om
+            gp.set_option(fredopt.OPT_BLOCK_SEQUENTIAL, block); orc.set_option(om.OPT_BLOCK_SEQUENTIAL, block)
+            gp.set_weights(x0); orc.set_x(x0)
+            gp.iterate(1, 1.0, beta0, 0.5); orc.iterate(1, 1.0, beta0, 0.5)
+            xg = _gpu_x(gp)
+            assert xg[2] == 0.0 and xg[3] == 0.0 and (xg >= 0).all()
+            assert _rel_l2(xg, orc.get_x()) <= 1e-14
+
+
+def test_more_structures_than_the_work_items_can_carry(fredopt):
+    """n_struct > 255: FREDOPT_UNSUPPORTED (documented limit), never a wrong result."""
+    nan = np.nan
+    rp = np.array([0, 1], np.int64); ci = np.array([0], np.int32); vv = np.array([1.0], np.float32)
+    b = np.tile(np.array([[1.0, nan, 1.0, nan, nan, nan, nan, nan]], np.float32), (256, 1))
+    with pytest.raises(fredopt.FredoptError) as e:
+        fredopt.Plan(1, 1, (rp, ci, vv), (rp, ci, vv), np.array([1], np.int32), b)
+    assert e.value.code == fredopt.UNSUPPORTED
+    gp = fredopt.Plan(1, 1, (rp, ci, vv), (rp, ci, vv), np.array([255], np.int32), b[:255])     # 255 structures are fine
+    gp.set_weights(np.array([3.0], np.float32)); gp.iterate(1, 1.0, 0.0, 0.5)
+    assert abs(_gpu_x(gp)[0] - 1.0) < 1e-15
+    with pytest.raises(fredopt.FredoptError):
+        fredopt.Plan(1, 1, (rp, ci, vv), (rp, ci, vv), np.array([1], np.int32), b[:1], index_width=8)
+
+
+@pytest.mark.parametrize("copt", INDEX_FORMS)
+def test_more_than_65536_labelled_rows(fredopt, copt):
+    """More labelled rows than one 16-bit block of the transposes holds (several 65536-row blocks per spot run), cheaply: short
+    random rows, two structures, both stored index forms."""
+    V, S, per_row = 150000, 300, 6
+    u = pg.uniform01_array(91, V * per_row * 3 + V)
+    cols = np.sort((u[:V * per_row].reshape(V, per_row) * (S // per_row)).astype(np.int64) + np.arange(per_row) * (S // per_row), axis=1)
+    rp = np.arange(V + 1, dtype=np.int64) * per_row
+    ci = cols.reshape(-1).astype(np.int32)
+    vd = (0.05 + u[V * per_row:2 * V * per_row]).astype(np.float32)
+    vl = (vd * (2.0 + 6.0 * u[2 * V * per_row:3 * V * per_row])).astype(np.float32)
+    lab = (1 + np.floor(u[3 * V * per_row:] * 2)).astype(np.int32)         # every row labelled: 150 000 > 2 x 65 536
+    nan = np.nan
+    bounds = np.array([[1.0, 0.8, 1.1, nan, nan, nan, 1.0, nan],
+                       [1.0, nan, 0.9, nan, 4.0, 4.5, nan, 3.5]], np.float32)
+    orc = _oracle_np(V, S, (rp, ci, vd), (rp, ci, vl), lab, bounds)
+    gp = fredopt.Plan(V, S, (rp, ci, vd), (rp, ci, vl), lab, bounds, **copt)
+    x0 = (0.2 + 0.5 * pg.uniform01_array(92, S)).astype(np.float32)
+    uu = (pg.uniform01_array(93, V) - 0.4).astype(np.float32); vv_ = (pg.uniform01_array(94, V) - 0.6).astype(np.float32)
+    ref, ref_abs = orc.transpose(uu.astype(np.float64), vv_.astype(np.float64), active_only=True)
+    out = np.empty(S, np.float32)
+    gp.spmv_transpose(fredopt.ROWS_ACTIVE, uu, vv_, out)
+    assert np.all(np.abs(out - ref) <= TOL_SPMV * ref_abs)
+    from oracle import oracle as om
+    for block in (0, 1):
+        gp.set_option(fredopt.OPT_RESET, 1); orc.set_option(om.OPT_RESET, 1)
+        gp.set_option(fredopt.OPT_BLOCK_SEQUENTIAL, block); orc.set_option(om.OPT_BLOCK_SEQUENTIAL, block)
+        orc.set_x(x0); gp.set_weights(x0)
+        orc.iterate(10, 1.0, 1.0, 0.9); gp.iterate(10, 1.0, 1.0, 0.9)
+        if block:
+            _assert_block_state(gp, orc)
+        else:
+            _assert_state(gp, orc)
