@@ -175,11 +175,20 @@ def run_ours(args):
     stream = torch.cuda.Stream()          # the plan's stream: every kernel and every timing event of this run is on it
     torch.cuda.set_stream(stream)
     t0 = time.perf_counter()
-    gp = fredopt.from_plan(plan, stream=stream.cuda_stream)
+    copt = {}
+    if args.block_rows:
+        copt["block_rows"] = args.block_rows
+    if args.index_width:
+        copt["index_width"] = args.index_width
+    gp = fredopt.from_plan(plan, stream=stream.cuda_stream, **copt)
     torch.cuda.synchronize()
     t_create = time.perf_counter() - t0
     if args.block_sequential:
         gp.set_option(fredopt.OPT_BLOCK_SEQUENTIAL, 1)
+    if args.work_queue is not None:
+        gp.set_option(fredopt.OPT_WORK_QUEUE, args.work_queue)
+    if args.no_pdl:
+        gp.set_option(fredopt.OPT_USE_PDL, 0)
     st0 = gp.stats()
     K, W = args.steps, args.warmup
     lam, beta0, a = spec.lam, (0.0 if args.ams else spec.beta0), spec.a
@@ -275,6 +284,8 @@ def run_ours(args):
         "config": {"workload": f"configs[{args.config}] {spec.name}", "n_voxels": plan.n_rows, "n_spots": plan.n_cols,
                    "nnz_per_matrix": plan.nnz, "nnz_active": stats["nnz_active"], "n_active_rows": stats["n_active_rows"],
                    "n_sets": stats["n_sets"], "lambda": lam, "beta0": beta0, "a": a,
+                   "block_rows": stats["block_rows"], "entries_active": stats["entries_active"],
+                   "fill_in": stats["entries_active"] * stats["block_rows"] / max(stats["nnz_active"], 1),
                    "storage": "fp32 matrix values, 16-bit indices where exact (else int32), fp64 vectors and accumulators",
                    "ams_form": "block-sequential (Fig. 2 loop nest, R23)" if args.block_sequential else "simultaneous (R1)",
                    "passes_per_iteration": 2 if args.ams else 4, "alg_bytes_per_iteration": iter_bytes,
@@ -420,6 +431,10 @@ def main():
                     help="feasibility-seeking step in the block-sequential form of Fig. 2's loop nest (DESIGN.md R23)")
     ap.add_argument("--ams", action="store_true",
                     help="pure feasibility-seeking (beta0 = 0, the paper's 'AMS' runs, PAPER.md:120): two passes per iteration")
+    ap.add_argument("--block-rows", type=int, default=0, help="fredopt_create_options.block_rows (0 = automatic)")
+    ap.add_argument("--index-width", type=int, default=0, help="fredopt_create_options.index_width (0 = automatic, 32)")
+    ap.add_argument("--no-pdl", action="store_true", help="FREDOPT_OPT_USE_PDL = 0 (plain launches)")
+    ap.add_argument("--work-queue", type=int, default=None, help="FREDOPT_OPT_WORK_QUEUE (bit 0 forward, bit 1 transposed passes)")
     ap.add_argument("--sweep", action="store_true", help="BASELINE.json configs[4]: isolated-pass sweep (1 GPU)")
     ap.add_argument("--quick", action="store_true", help="with --sweep: two points only")
     args = ap.parse_args()

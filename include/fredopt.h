@@ -85,6 +85,9 @@ typedef struct {
     int64_t nnz;                /* non-zeros per matrix (union pattern)                                    */
     int64_t nnz_active;         /* non-zeros in active rows                                                */
     int64_t alg_bytes_iter;     /* algorithmic bytes of ONE superiorized iteration ("Bytes")    */
+    int64_t block_rows;         /* rows per stored block row of the labelled voxels (1, 2 or 4)            */
+    int64_t entries_active;     /* stored entries of the labelled rows: (block row, spot) pairs of the     */
+                                /*   union patterns; entries_active * block_rows >= nnz_active values      */
     double  last_beta;          /* last accepted beta (0 if none)                                          */
     double  phi;                /* chi^2 at the perturbed point of the last iteration (superiorized,       */
                                 /*   simultaneous form; otherwise over the rows the last pass visited)     */
@@ -113,6 +116,11 @@ typedef struct {
 
 #define FREDOPT_OPT_NORMALIZE_GRAD   8 /* 1: the perturbation steps along grad chi^2 / |grad chi^2|_2 (Fig. 3 prints the  */
                                        /*    un-normalised gradient: default 0; R9)             */
+#define FREDOPT_OPT_WORK_QUEUE      11 /* how the matrix passes deal their work items to the warps (tuning; never changes a result: */
+                                       /*    an item's sum is formed by one warp in a fixed order and stored to a place of its own). */
+                                       /*    bit 0 / bit 1: forward / transposed passes take items from a queue (a warp that         */
+                                       /*    finishes early takes more) instead of a static round-robin deal; bit 2 / bit 3: forward  */
+                                       /*    / transposed items are taken longest first instead of in storage order.  Default 13      */
 #define FREDOPT_OPT_USE_PDL         10 /* 1 (default): the kernels of an iteration are launched with programmatic dependent    */
                                        /*    launch (a kernel's CTAs are scheduled while its predecessor drains); 0: plain launches */
 #define FREDOPT_OPT_ONE_SIDED_COST   9 /* 1: the OAR term of Eq. (2) penalises only cDL above cDLref: w (cDL - cDLref)_+^2 */
@@ -145,8 +153,12 @@ int fredopt_create(const fredopt_csr *D, const fredopt_csr *L, const int32_t *vo
  * same terms plus exact zeros.  struct_size = sizeof(fredopt_create_options) of the caller (the struct may grow). */
 typedef struct {
     int32_t struct_size;
-    int32_t index_width;        /* 0 = automatic: 16-bit indices where exact (n_cols <= 65536; row indices of the      */
-                                /*     transposes inside 65536-row blocks), int32 otherwise; 32 = int32 everywhere      */
+    int32_t index_width;        /* 0 = automatic: 16-bit indices where exact (n_cols <= 65536; block-row indices of the */
+                                /*     transposes inside groups of 65536), int32 otherwise; 32 = int32 everywhere       */
+    int32_t block_rows;         /* rows per stored block row of the labelled voxels: consecutive voxels of one          */
+                                /*     structure share one stored index per spot over the union of their patterns       */
+                                /*     (neighbouring voxels see almost the same spots), in both orientations.           */
+                                /*     0 = automatic (the height that stores the fewest bytes), or 1, 2, 4              */
 } fredopt_create_options;
 /* fredopt_create with options (opt = NULL: the defaults, identical to fredopt_create).  INVALID_ARG on an unknown value. */
 int fredopt_create_ex(const fredopt_csr *D, const fredopt_csr *L, const int32_t *voxel_labels,

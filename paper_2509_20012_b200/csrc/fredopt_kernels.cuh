@@ -1,7 +1,11 @@
 // fredopt_kernels.cuh -- the hot kernels of the superiorized feasibility-seeking iteration (sm_100a).
 //
+// Storage: the labelled rows are kept as BLOCK ROWS of R = 1, 2 or 4 consecutive voxels of one
+// structure over the union of their column patterns (neighbouring voxels see almost the same spots): one stored index and
+// one gathered weight serve R values, in both orientations -- an ENTRY is one (block row, spot) pair with R values per matrix.
+//
 // Passes of one iteration:
-//   k_forward    d = D x, l = L x over a list of work items (one item = one voxel row; one warp per item,
+//   k_forward    d = D x, l = L x over a list of work items (one item = one block row; one warp per item,
 //                round-robin, 128-bit streamed index/value loads kept out of L1, fp64 accumulation, shuffle
 //                reduction).  A row reads only the value arrays its structure needs.  Epilogues: store d, l
 //                (+ the cost residuals p, q of Eq. 2), the quadratic coefficient c of the accept test, the residuals /
@@ -34,7 +38,10 @@ constexpr int TR_ITEM_MAX = TR_ITEM_MAX_ENTRIES;   // entries per transposed wor
 #ifndef FWD_U3
 #define FWD_U3 4   /* ... and for rows that read both (measured: 6/4 beats 4/4 by 2 %, 8/4 and 6/3 are slower) */
 #endif
-constexpr int FWD_MIN_CTAS = 4;             // resident CTAs per SM the item kernels are compiled for (64 registers)
+#ifndef FWD_MIN_CTAS_PER_SM
+#define FWD_MIN_CTAS_PER_SM 4
+#endif
+constexpr int FWD_MIN_CTAS = FWD_MIN_CTAS_PER_SM;   // resident CTAs per SM the item kernels are compiled for (4: 64 registers)
 
 // flags of a structure
 enum : int { F_DOSE_SLAB = 1, F_DL_SLAB = 2, F_LETD = 4, F_DOSE_REF = 8, F_DL_REF = 16 };
@@ -54,6 +61,7 @@ struct StructInfo {
     double dose_lo, dose_hi, dl_lo, dl_hi, letd_max, dose_ref, dl_ref;
     int flags, pad;
     unsigned long long part, n_sets, n_zero, rows, nnz;   // participating sets, declared sets, zero-norm sets, rows, nnz
+    unsigned long long entries;                           // stored entries (union patterns of the structure's block rows)
     unsigned long long part_kind[3];                      // participating sets per kind: dose slab, cDL slab, LETd
 };
 
@@ -67,9 +75,11 @@ struct DevState {
     int flags;                 // bit 0: step along g/|g| (R9 option); bit 1: one-sided cDL cost (R11 option)
 };
 
-// One work item: `len` entries (multiple of 4) starting at entry `start` (multiple of 4) of the index / value
-// arrays; `seg` = structure - 1 (selects which value arrays are read); transposed items carry the 65536-row block of
-// their 16-bit row indices in seg >> 8.  16 bytes: fetched with one 128-bit load.
+// One work item: `len` VALUES per matrix (multiple of 4) starting at value `start` (multiple of 4) of the value arrays,
+// i.e. len / R entries starting at entry start / R of the index array; `seg` & 0xFF = structure - 1 (selects which value
+// arrays are read).  Forward items (one block row) carry the number of real rows of the block (1..R; the last block of a
+// structure may be ragged) in bits 8-10; transposed items carry the 65536-block group of their 16-bit block indices in
+// seg >> 8.  16 bytes: fetched with one 128-bit load.
 struct __align__(16) Item {
     long long start;
     int32_t len;
@@ -97,6 +107,11 @@ __device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;"
 __device__ __forceinline__ void pdl_trigger() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
 
 // ------------------------------------------------------------------------------------------ loads
+#ifdef EXP_NO_GATHER          /* timing experiment only (results are wrong): the gathered value is replaced by the index */
+#define FWD_GATHER(x, c) ((double)(c))
+#else
+#define FWD_GATHER(x, c) __ldg((x) + (c))
+#endif
 // streamed arrays (index / value): read once, keep them out of L1 so that L1 holds the gathered vector
 __device__ __forceinline__ int4 ld_stream_i4(const int32_t* p) {
     int4 r;
@@ -110,15 +125,39 @@ __device__ __forceinline__ float4 ld_stream_f4(const float* p) {
                  : "=f"(r.x), "=f"(r.y), "=f"(r.z), "=f"(r.w) : "l"(p));
     return r;
 }
-// four consecutive stored indices starting at entry e (multiple of 4): 32-bit form or 16-bit form (+ `add`)
-template <bool I16>
-__device__ __forceinline__ int4 ld_idx4(const void* __restrict__ base, long long e, int add) {
+// C consecutive stored indices starting at index position i (a multiple of C): 16-bit form (+ `add`) or 32-bit form.
+// C = 4 / R is the number of entries a lane's 128-bit value load covers.
+template <bool I16, int C>
+__device__ __forceinline__ void ld_idx(const void* __restrict__ base, long long i, int add, int (&c)[C]) {
     if (I16) {
-        unsigned int lo, hi;
-        asm volatile("ld.global.nc.L1::no_allocate.v2.u32 {%0,%1}, [%2];" : "=r"(lo), "=r"(hi) : "l"((const uint16_t*)base + e));
-        return make_int4((int)(lo & 0xFFFFu) + add, (int)(lo >> 16) + add, (int)(hi & 0xFFFFu) + add, (int)(hi >> 16) + add);
+        const uint16_t* p = (const uint16_t*)base + i;
+        if (C == 4) {
+            unsigned int lo, hi;
+            asm volatile("ld.global.nc.L1::no_allocate.v2.u32 {%0,%1}, [%2];" : "=r"(lo), "=r"(hi) : "l"(p));
+            c[0] = (int)(lo & 0xFFFFu) + add; c[1 % C] = (int)(lo >> 16) + add; c[2 % C] = (int)(hi & 0xFFFFu) + add; c[3 % C] = (int)(hi >> 16) + add;
+        } else if (C == 2) {
+            unsigned int lo;
+            asm volatile("ld.global.nc.L1::no_allocate.u32 %0, [%1];" : "=r"(lo) : "l"(p));
+            c[0] = (int)(lo & 0xFFFFu) + add; c[1 % C] = (int)(lo >> 16) + add;
+        } else {
+            unsigned short lo;
+            asm volatile("ld.global.nc.L1::no_allocate.u16 %0, [%1];" : "=h"(lo) : "l"(p));
+            c[0] = (int)lo + add;
+        }
     } else {
-        return ld_stream_i4((const int32_t*)base + e);
+        const int32_t* p = (const int32_t*)base + i;
+        if (C == 4) {
+            const int4 v = ld_stream_i4(p);
+            c[0] = v.x; c[1 % C] = v.y; c[2 % C] = v.z; c[3 % C] = v.w;
+        } else if (C == 2) {
+            int a, b;
+            asm volatile("ld.global.nc.L1::no_allocate.v2.s32 {%0,%1}, [%2];" : "=r"(a), "=r"(b) : "l"(p));
+            c[0] = a; c[1 % C] = b;
+        } else {
+            int a;
+            asm volatile("ld.global.nc.L1::no_allocate.s32 %0, [%1];" : "=r"(a) : "l"(p));
+            c[0] = a;
+        }
     }
 }
 __device__ __forceinline__ Item ld_item(const Item* p) {
@@ -128,6 +167,38 @@ __device__ __forceinline__ Item ld_item(const Item* p) {
     it.len = v.z;
     it.seg = v.w;
     return it;
+}
+// R consecutive fp64 coefficients starting at element R * b of a gathered vector (cached: neighbouring entries reuse lines)
+template <int R>
+__device__ __forceinline__ void ld_coef(const double* __restrict__ v, int b, double (&g)[R]) {
+#ifdef EXP_NO_GATHER
+    for (int k = 0; k < R; ++k) g[k] = (double)b;
+    return;
+#endif
+    if (R == 1) g[0] = __ldg(v + b);
+    else if (R == 2) { const double2 t = __ldg((const double2*)v + b); g[0] = t.x; g[1 % R] = t.y; }
+    else {   // 32 bytes, 32-byte aligned: one 256-bit load (sm_100+)
+        double a0, a1, a2, a3;
+        asm volatile("ld.global.nc.v4.f64 {%0,%1,%2,%3}, [%4];" : "=d"(a0), "=d"(a1), "=d"(a2), "=d"(a3) : "l"(v + 4 * (long long)b));
+        g[0] = a0; g[1 % R] = a1; g[2 % R] = a2; g[3 % R] = a3;
+    }
+}
+// R consecutive {coefficient of D_i, coefficient of L_i} pairs starting at pair R * b
+template <int R>
+__device__ __forceinline__ void ld_coef_pair(const double2* __restrict__ v, int b, double (&gd)[R], double (&gl)[R]) {
+#ifdef EXP_NO_GATHER
+    for (int k = 0; k < R; ++k) { gd[k] = (double)b; gl[k] = (double)b; }
+    return;
+#endif
+    if (R == 1) { const double2 t = __ldg(v + b); gd[0] = t.x; gl[0] = t.y; }
+    else {
+#pragma unroll
+        for (int h = 0; h < R / 2; ++h) {   // 32 bytes (two pairs) per 256-bit load
+            double a0, a1, a2, a3;
+            asm volatile("ld.global.nc.v4.f64 {%0,%1,%2,%3}, [%4];" : "=d"(a0), "=d"(a1), "=d"(a2), "=d"(a3) : "l"(v + (long long)R * b + 2 * h));
+            gd[(2 * h) % R] = a0; gl[(2 * h) % R] = a1; gd[(2 * h + 1) % R] = a2; gl[(2 * h + 1) % R] = a3;
+        }
+    }
 }
 
 __device__ __forceinline__ double warp_sum(double v) {
@@ -148,12 +219,7 @@ __device__ __forceinline__ double block_sum(double v, double* sm) {
     return r;
 }
 
-__device__ __forceinline__ void fma4(double& acc, const float4& a, double x0, double x1, double x2, double x3) {
-    acc = fma((double)a.x, x0, acc);
-    acc = fma((double)a.y, x1, acc);
-    acc = fma((double)a.z, x2, acc);
-    acc = fma((double)a.w, x3, acc);
-}
+__device__ __forceinline__ float f4_get(const float4& a, int i) { return i == 0 ? a.x : i == 1 ? a.y : i == 2 ? a.z : a.w; }
 
 // signed residual of a hyperslab lo <= val <= hi (NaN = absent): upper violations > 0, lower < 0
 __device__ __forceinline__ double slab_residual(double val, double lo, double hi) {
@@ -208,149 +274,195 @@ struct ResidArgs {
     DevState* st;                        // relax = lambda eta^k, eta^k and k advance when uv is written
 };
 
+// ------------------------------------------------------------------------------------------ work distribution
+// The items of a pass are dealt to the warps of a persistent grid (one CTA per resident slot) from a queue: the first two
+// items of a warp are static (warp, warp + W), the others come from an integer counter, longest items first -- a warp that
+// finishes early takes more work, so the pass ends when the work ends, not when the unluckiest warp of a static deal does.
+// Which warp computes an item never changes a result: an item's sum is formed by one warp in a fixed lane order and stored
+// to a place that belongs to the item (row, slot, per-item partial sums), so the passes stay bitwise reproducible.  The last
+// warp to leave resets the queue for the next launch (launches of a plan are serialised on its stream).
+struct WorkQueue {
+    unsigned int next;           // items handed out beyond the static ones
+    unsigned int done;           // warps that have left
+};
+__device__ __forceinline__ void queue_leave(WorkQueue* q, int lane, unsigned int n_warps) {
+    if (lane == 0) {
+        const unsigned int old = atomicAdd(&q->done, 1u);
+        if (old == n_warps - 1) { q->next = 0u; q->done = 0u; }          // everyone else has stopped fetching
+    }
+}
+__device__ __forceinline__ void prefetch_l1(const void* p) { asm volatile("prefetch.global.L1 [%0];" ::"l"(p)); }
+
 // ------------------------------------------------------------------------------------------ forward
 enum : int { EPI_STORE = 0, EPI_STORE_PQ = 1, EPI_CPART = 2, EPI_F32VOX = 3, EPI_RESID = 4 };
 
-// <D_i, x> and / or <L_i, x> of one row by one warp.  M: bit 0 = D, bit 1 = L.  U 128-entry chunks per trip (6 for a
-// single matrix, 4 for both): up to 12 independent vector loads per lane in flight before the first gather.
-template <int M, bool I16>
-__device__ __forceinline__ void fwd_row(const void* __restrict__ cbase, long long e0, const float* __restrict__ dp,
-                                        const float* __restrict__ lp, int L, int lane, const double* __restrict__ x,
-                                        double& aD, double& aL) {
+// <D_i, x> and / or <L_i, x> of the R rows of one block row by one warp.  M: bit 0 = D, bit 1 = L.  Lv values per matrix
+// (multiple of 4) starting at value v0: a lane's 128-bit load holds C = 4 / R entries (R values each); inside every chunk of
+// 128 values the entries are stored interleaved so that the j-th gather of the warp covers CONSECUTIVE entries (few lines of
+// x per instruction).  U chunks per trip (6 for a single matrix, 4 for both): up to 12 independent vector loads per lane in
+// flight before the first gather.
+template <int M, int R, bool I16>
+__device__ __forceinline__ void fwd_row(const void* __restrict__ cbase, long long v0, const float* __restrict__ dp,
+                                        const float* __restrict__ lp, int Lv, int lane, const double* __restrict__ x,
+                                        double (&aD)[R], double (&aL)[R]) {
+    constexpr int C = 4 / R;
     constexpr int U = (M == 3) ? FWD_U3 : FWD_U1;
+    const long long i0 = v0 / R;                 // first stored index of the block row
     int p = lane * 4;
-    for (; p + 128 * (U - 1) < L; p += 128 * U) {
-        int4 c[U];
+    for (; p + 128 * (U - 1) < Lv; p += 128 * U) {
+        int c[U][C];
         float4 d[U], l[U];
 #pragma unroll
         for (int u = 0; u < U; ++u) {
-            c[u] = ld_idx4<I16>(cbase, e0 + p + 128 * u, 0);
+            ld_idx<I16, C>(cbase, i0 + (p + 128 * u) / R, 0, c[u]);
             if (M & 1) d[u] = ld_stream_f4(dp + p + 128 * u);
             if (M & 2) l[u] = ld_stream_f4(lp + p + 128 * u);
         }
 #pragma unroll
         for (int u = 0; u < U; ++u) {
-            const double x0 = __ldg(x + c[u].x), x1 = __ldg(x + c[u].y), x2 = __ldg(x + c[u].z), x3 = __ldg(x + c[u].w);
-            if (M & 1) fma4(aD, d[u], x0, x1, x2, x3);
-            if (M & 2) fma4(aL, l[u], x0, x1, x2, x3);
+            double xv[C];
+#pragma unroll
+            for (int j = 0; j < C; ++j) xv[j] = FWD_GATHER(x, c[u][j]);
+#pragma unroll
+            for (int j = 0; j < C; ++j)
+#pragma unroll
+                for (int k = 0; k < R; ++k) {
+                    if (M & 1) aD[k] = fma((double)f4_get(d[u], j * R + k), xv[j], aD[k]);
+                    if (M & 2) aL[k] = fma((double)f4_get(l[u], j * R + k), xv[j], aL[k]);
+                }
         }
     }
-    if (p < L) {   // remainder (fewer than U chunks): ONE predicated trip, all loads in flight together; a lane without
-                   // an entry behaves like padding (column 0, value 0)
-        int4 c[U - 1];
+    if (p < Lv) {   // remainder (fewer than U chunks): ONE predicated trip, all loads in flight together; a lane without
+                    // an entry behaves like padding (column 0, value 0)
+        int c[U - 1][C];
         float4 d[U - 1], l[U - 1];
 #pragma unroll
         for (int u = 0; u < U - 1; ++u) {
-            const bool ok = p + 128 * u < L;
-            c[u] = ok ? ld_idx4<I16>(cbase, e0 + p + 128 * u, 0) : make_int4(0, 0, 0, 0);
+            const bool ok = p + 128 * u < Lv;
+            if (ok) ld_idx<I16, C>(cbase, i0 + (p + 128 * u) / R, 0, c[u]);
+            else {
+#pragma unroll
+                for (int j = 0; j < C; ++j) c[u][j] = 0;
+            }
             if (M & 1) d[u] = ok ? ld_stream_f4(dp + p + 128 * u) : make_float4(0.f, 0.f, 0.f, 0.f);
             if (M & 2) l[u] = ok ? ld_stream_f4(lp + p + 128 * u) : make_float4(0.f, 0.f, 0.f, 0.f);
         }
 #pragma unroll
         for (int u = 0; u < U - 1; ++u) {
-            if (p + 128 * u < L) {
-                const double x0 = __ldg(x + c[u].x), x1 = __ldg(x + c[u].y), x2 = __ldg(x + c[u].z), x3 = __ldg(x + c[u].w);
-                if (M & 1) fma4(aD, d[u], x0, x1, x2, x3);
-                if (M & 2) fma4(aL, l[u], x0, x1, x2, x3);
+            if (p + 128 * u < Lv) {
+                double xv[C];
+#pragma unroll
+                for (int j = 0; j < C; ++j) xv[j] = FWD_GATHER(x, c[u][j]);
+#pragma unroll
+                for (int j = 0; j < C; ++j)
+#pragma unroll
+                    for (int k = 0; k < R; ++k) {
+                        if (M & 1) aD[k] = fma((double)f4_get(d[u], j * R + k), xv[j], aD[k]);
+                        if (M & 2) aL[k] = fma((double)f4_get(l[u], j * R + k), xv[j], aL[k]);
+                    }
             }
         }
     }
 }
 
-// One warp per item, items r = warp, warp + W, ... (static mapping: deterministic partial sums; the warps of the
-// grid read one contiguous window of the arrays at any time).  The next item's descriptor is fetched one item ahead.
-// mode[seg]: bit 0 = read valD, bit 1 = read valL.
-template <int EPI, bool I16>
+// One warp per item (block row) from the work queue (items in longest-first order; item_blk[e] = block row of item e, or null
+// = e).  The descriptor of the next item is fetched while the current one is processed.  mode[seg]: bit 0 = read valD, bit 1 =
+// read valL.  Row r = R * b + k (k < rows of the block) indexes every per-row array; partial sums of the epilogues (c, chi^2,
+// proximity, count) are stored per block row and added in a fixed order by the kernel that consumes them.
+template <int EPI, int R, bool I16>
 __global__ void __launch_bounds__(FWD_THREADS, FWD_MIN_CTAS)
-k_forward(long long n, const Item* __restrict__ items, const int32_t* __restrict__ vox, const uint8_t* __restrict__ mode,
+k_forward(long long n, const Item* __restrict__ items, const int32_t* __restrict__ item_blk, WorkQueue* __restrict__ wq,
+          const int32_t* __restrict__ vox, const uint8_t* __restrict__ mode,
           const void* __restrict__ col, const float* __restrict__ vD, const float* __restrict__ vL,
           const double* __restrict__ x,
-          double* __restrict__ oD, double* __restrict__ oL,                // EPI_STORE*, EPI_CPART: item-indexed
+          double* __restrict__ oD, double* __restrict__ oL,                // EPI_STORE*, EPI_CPART, EPI_RESID: row-indexed
           const GatherVec pq,                                              // EPI_STORE_PQ: cost residuals (Eq. 2)
-          const StructInfo* __restrict__ tab, double* __restrict__ cpart,  // EPI_STORE_PQ / EPI_CPART
+          const StructInfo* __restrict__ tab, double* __restrict__ cpart,  // EPI_STORE_PQ / EPI_CPART: per block row
           const DevState* __restrict__ st,                                 // EPI_STORE_PQ (cost form)
           float* __restrict__ fD, float* __restrict__ fL, int letd_out,    // EPI_F32VOX: voxel-indexed
           const ResidArgs ra)                                              // EPI_RESID: residual / violation epilogue (a7)
 {
     const int lane = threadIdx.x & 31;
-    const long long nwarps = (long long)gridDim.x * FWD_WARPS;
-    long long r = (long long)blockIdx.x * FWD_WARPS + (threadIdx.x >> 5);
-    double csum = 0.0, rprox = 0.0, rphi = 0.0;
-    long long rcnt = 0;
-    Item it;
-    if (r < n) it = ld_item(items + r);          // static data: fetched before the dependency wait
+    const int nwarps = gridDim.x * FWD_WARPS, ni = (int)n;      // items < 2^31
+    int e0 = blockIdx.x * FWD_WARPS + (threadIdx.x >> 5), e1 = e0 + nwarps;
+    if (e0 < ni) prefetch_l1(items + e0);                       // static data: touched before the dependency wait
     pdl_wait();
     pdl_trigger();
-    while (r < n) {
-        const long long rn = r + nwarps;
-        Item nx;
-        if (rn < n) nx = ld_item(items + rn);
-        const int m = mode[it.seg];
-        double aD = 0.0, aL = 0.0;
-        if (m == 3) fwd_row<3, I16>(col, it.start, vD + it.start, vL + it.start, it.len, lane, x, aD, aL);
-        else if (m == 1) fwd_row<1, I16>(col, it.start, vD + it.start, nullptr, it.len, lane, x, aD, aL);
-        else if (m == 2) fwd_row<2, I16>(col, it.start, nullptr, vL + it.start, it.len, lane, x, aD, aL);
-        if (m & 1) aD = warp_sum(aD);
-        if (m & 2) aL = warp_sum(aL);
+    while (e0 < ni) {
+        const Item it = ld_item(items + e0);
+        const int blk = item_blk ? item_blk[e0] : e0;
+        unsigned int e2 = 0;
+        if (wq && lane == 0) e2 = atomicAdd(&wq->next, 1u);     // in flight while this item is processed
+        if (e1 < ni) { prefetch_l1(items + e1); if (item_blk) prefetch_l1(item_blk + e1); }
+        const long long b = blk;
+        const int seg = it.seg & 0xFF, nrow = (it.seg >> 8) & 7;
+        const int m = mode[seg];
+        double aD[R], aL[R];
+#pragma unroll
+        for (int k = 0; k < R; ++k) { aD[k] = 0.0; aL[k] = 0.0; }
+        if (m == 3) fwd_row<3, R, I16>(col, it.start, vD + it.start, vL + it.start, it.len, lane, x, aD, aL);
+        else if (m == 1) fwd_row<1, R, I16>(col, it.start, vD + it.start, nullptr, it.len, lane, x, aD, aL);
+        else if (m == 2) fwd_row<2, R, I16>(col, it.start, nullptr, vL + it.start, it.len, lane, x, aD, aL);
+#pragma unroll
+        for (int k = 0; k < R; ++k) {
+            if (m & 1) aD[k] = warp_sum(aD[k]);
+            if (m & 2) aL[k] = warp_sum(aL[k]);
+        }
         if (lane == 0) {
-            if (EPI == EPI_F32VOX) {
-                const int v = vox[r];
-                if (fD) fD[v] = (float)aD;
-                if (fL) fL[v] = letd_out ? (aD > 0.0 ? (float)(aL / aD) : 0.0f) : (float)aL;
-            } else {
-                oD[r] = aD;
-                oL[r] = aL;
-                if (EPI == EPI_STORE_PQ) {      // p_i = 2 w^ (d_i - Dref), q_i = 2 w^ (l_i - cDLref): grad chi^2 = D^T p + L^T q
-                    const StructInfo& T = tab[it.seg];
-                    const int one_sided = st->flags & SF_ONE_SIDED;
-                    double pv, qv;
-                    cost_residuals(T.flags, T.what, T.dose_ref, T.dl_ref, one_sided, aD, aL, pv, qv);
-                    gv_store(pq, r, pv, qv);
-                    // the row's share of chi^2(x) (Eq. 2): the accept test of Fig. 3 compares against it
-                    if (T.flags & F_DOSE_REF) { const double e = T.dose_ref - aD; csum += T.what * e * e; }
-                    if (T.flags & F_DL_REF) { const double e = T.dl_ref - aL; if (!(one_sided && e > 0.0)) csum += T.what * e * e; }
-                }
-                if (EPI == EPI_CPART) {
-                    const StructInfo& T = tab[it.seg];
-                    if (T.flags & F_DOSE_REF) csum += T.what * aD * aD;
-                    if (T.flags & F_DL_REF) csum += T.what * aL * aL;
-                }
-                if (EPI == EPI_RESID) {         // residuals / violations of Fig. 2 at x, in the epilogue of the fused pass
-                    double u, v;
-                    row_residual(tab[it.seg], ra.st->flags & SF_ONE_SIDED, aD, aL, ra.nD[r], ra.nL[r], ra.nT[r], u, v, rcnt, rprox, rphi);
-                    if (ra.uv.pair) gv_store(ra.uv, r, u, v);
+            double csum = 0.0, rprox = 0.0, rphi = 0.0;
+            long long rcnt = 0;
+#pragma unroll
+            for (int k = 0; k < R; ++k) {
+                if (k >= nrow) break;
+                const long long r = b * R + k;
+                const double dv = aD[k], lv = aL[k];
+                if (EPI == EPI_F32VOX) {
+                    const int v = vox[r];
+                    if (fD) fD[v] = (float)dv;
+                    if (fL) fL[v] = letd_out ? (dv > 0.0 ? (float)(lv / dv) : 0.0f) : (float)lv;
+                } else {
+                    oD[r] = dv;
+                    oL[r] = lv;
+                    if (EPI == EPI_STORE_PQ) {      // p_i = 2 w^ (d_i - Dref), q_i = 2 w^ (l_i - cDLref): grad chi^2 = D^T p + L^T q
+                        const StructInfo& T = tab[seg];
+                        const int one_sided = st->flags & SF_ONE_SIDED;
+                        double pv, qv;
+                        cost_residuals(T.flags, T.what, T.dose_ref, T.dl_ref, one_sided, dv, lv, pv, qv);
+                        gv_store(pq, r, pv, qv);
+                        // the row's share of chi^2(x) (Eq. 2): the accept test of Fig. 3 compares against it
+                        if (T.flags & F_DOSE_REF) { const double e = T.dose_ref - dv; csum += T.what * e * e; }
+                        if (T.flags & F_DL_REF) { const double e = T.dl_ref - lv; if (!(one_sided && e > 0.0)) csum += T.what * e * e; }
+                    }
+                    if (EPI == EPI_CPART) {
+                        const StructInfo& T = tab[seg];
+                        if (T.flags & F_DOSE_REF) csum += T.what * dv * dv;
+                        if (T.flags & F_DL_REF) csum += T.what * lv * lv;
+                    }
+                    if (EPI == EPI_RESID) {         // residuals / violations of Fig. 2 at x, in the epilogue of the fused pass
+                        double u, v;
+                        row_residual(tab[seg], ra.st->flags & SF_ONE_SIDED, dv, lv, ra.nD[r], ra.nL[r], ra.nT[r], u, v, rcnt, rprox, rphi);
+                        if (ra.uv.pair) gv_store(ra.uv, r, u, v);
+                    }
                 }
             }
+            if (EPI == EPI_CPART || EPI == EPI_STORE_PQ) cpart[b] = csum;
+            if (EPI == EPI_RESID) { ra.part_prox[b] = rprox; ra.part_phi[b] = rphi; ra.part_cnt[b] = rcnt; }
         }
-        r = rn;
-        it = nx;
+        e0 = e1;
+        e1 = wq ? 2 * nwarps + (int)__shfl_sync(0xffffffffu, e2, 0) : e1 + nwarps;      // no queue: static round-robin
     }
-    if (EPI == EPI_CPART || EPI == EPI_STORE_PQ) {
-        __shared__ double sm[FWD_WARPS];
-        // lane 0 of each warp carries that warp's sum; other lanes carry 0
-        const double t = block_sum(csum, sm);
-        if (threadIdx.x == 0) cpart[blockIdx.x] = t;
-    }
-    if (EPI == EPI_RESID) {
-        __shared__ double sm[FWD_WARPS];
-        __shared__ long long smc[FWD_WARPS];
-        const double p = block_sum(rprox, sm);
-        const double q = block_sum(rphi, sm);
-        const long long c = block_sum_ll(rcnt, smc);
-        if (threadIdx.x == 0) {
-            ra.part_prox[blockIdx.x] = p; ra.part_phi[blockIdx.x] = q; ra.part_cnt[blockIdx.x] = c;
-            if (blockIdx.x == 0 && ra.uv.pair) {               // w_k = eta^k w: relax for this step
-                ra.st->relax = ra.st->lambda * ra.st->eta_pow;
-                ra.st->eta_pow *= ra.st->eta;
-                ra.st->k += 1;
-            }
-        }
+    if (wq) queue_leave(wq, lane, (unsigned int)nwarps);
+    if (EPI == EPI_RESID && blockIdx.x == 0 && threadIdx.x == 0 && ra.uv.pair) {   // w_k = eta^k w: relax for this step
+        ra.st->relax = ra.st->lambda * ra.st->eta_pow;
+        ra.st->eta_pow *= ra.st->eta;
+        ra.st->k += 1;
     }
 }
 
-// Short rows (at most 4*G entries, G = 4, 8 or 16): G lanes per row, 32/G rows per warp at a time, one 128-bit load per
-// lane and array, shuffle reduction inside the lane group.  Rows of one length class are stored back to back, so the
-// warp's loads are contiguous.  fp32 voxel-indexed outputs only (fredopt_dose_let / fredopt_spmv_forward over all rows).
+// Short rows of the full row set (R = 1; at most 4*G entries, G = 4, 8 or 16): G lanes per row, 32/G rows per warp at a time,
+// one 128-bit load per lane and array, shuffle reduction inside the lane group.  Rows of one length class are stored back to
+// back, so the warp's loads are contiguous.  fp32 voxel-indexed outputs only (fredopt_dose_let / fredopt_spmv_forward over
+// all rows).
 template <int G, bool I16>
 __global__ void __launch_bounds__(FWD_THREADS)
 k_forward_short(long long n, const Item* __restrict__ items, const int32_t* __restrict__ vox, int m,
@@ -367,10 +479,11 @@ k_forward_short(long long n, const Item* __restrict__ items, const int32_t* __re
             const Item it = ld_item(items + r);
             if (4 * t < it.len) {
                 const long long p = it.start + 4 * t;
-                const int4 c = ld_idx4<I16>(col, p, 0);
-                const double x0 = __ldg(x + c.x), x1 = __ldg(x + c.y), x2 = __ldg(x + c.z), x3 = __ldg(x + c.w);
-                if (m & 1) fma4(aD, ld_stream_f4(vD + p), x0, x1, x2, x3);
-                if (m & 2) fma4(aL, ld_stream_f4(vL + p), x0, x1, x2, x3);
+                int c[4];
+                ld_idx<I16, 4>(col, p, 0, c);
+                const double x0 = __ldg(x + c[0]), x1 = __ldg(x + c[1]), x2 = __ldg(x + c[2]), x3 = __ldg(x + c[3]);
+                if (m & 1) { const float4 a = ld_stream_f4(vD + p); aD = fma((double)a.x, x0, aD); aD = fma((double)a.y, x1, aD); aD = fma((double)a.z, x2, aD); aD = fma((double)a.w, x3, aD); }
+                if (m & 2) { const float4 a = ld_stream_f4(vL + p); aL = fma((double)a.x, x0, aL); aL = fma((double)a.y, x1, aL); aL = fma((double)a.z, x2, aL); aL = fma((double)a.w, x3, aL); }
             }
         }
 #pragma unroll
@@ -389,96 +502,105 @@ k_forward_short(long long n, const Item* __restrict__ items, const int32_t* __re
 // ------------------------------------------------------------------------------------------ transposed
 enum : int { TEPI_F32 = 0, TEPI_GRAD = 1, TEPI_UPDATE = 2 };
 
-// sum_i D_ij vec[i].x + L_ij vec[i].y over one item by one warp (vec is L2-resident; entries of a spot run over
-// ascending compact row indices, so neighbouring lanes gather neighbouring elements)
-template <int M, bool I16>
-__device__ __forceinline__ double tr_item(const void* __restrict__ cbase, long long e0, int add, const float* __restrict__ dp,
-                                          const float* __restrict__ lp, int L, int lane, const GatherVec& gv) {
+// sum over one item of D_ij cD[i] + L_ij cL[i] by one warp: an entry is one (spot run, block row b) pair with R values per
+// matrix and gathers the R coefficients of rows R b .. R b + R - 1 with one vector load (the gathered vectors are L2 / L1
+// resident; entries of a run ascend in b, so neighbouring lanes gather neighbouring elements)
+template <int M, int R, bool I16>
+__device__ __forceinline__ double tr_item(const void* __restrict__ cbase, long long v0, int add, const float* __restrict__ dp,
+                                          const float* __restrict__ lp, int Lv, int lane, const GatherVec& gv) {
+    constexpr int C = 4 / R;
     constexpr int U = (M == 3) ? FWD_U3 : FWD_U1;
     const double2* __restrict__ vec = gv.pair;
     const double* __restrict__ vs = (M == 2) ? gv.cL : gv.cD;
+    const long long i0 = v0 / R;
     double aD = 0.0, aL = 0.0;
     int p = lane * 4;
-    for (; p + 128 * (U - 1) < L; p += 128 * U) {
-        int4 c[U];
+#define TR_CONSUME(u)                                                                                     \
+    _Pragma("unroll") for (int j = 0; j < C; ++j) {                                                        \
+        if (M == 3) {                                                                                      \
+            double gd[R], gl[R];                                                                           \
+            ld_coef_pair<R>(vec, c[u][j], gd, gl);                                                         \
+            _Pragma("unroll") for (int k = 0; k < R; ++k) {                                                \
+                aD = fma((double)f4_get(d[u], j * R + k), gd[k], aD);                                      \
+                aL = fma((double)f4_get(l[u], j * R + k), gl[k], aL);                                      \
+            }                                                                                              \
+        } else {                                                                                           \
+            double g[R];                                                                                   \
+            ld_coef<R>(vs, c[u][j], g);                                                                    \
+            _Pragma("unroll") for (int k = 0; k < R; ++k) {                                                \
+                if (M == 1) aD = fma((double)f4_get(d[u], j * R + k), g[k], aD);                           \
+                else aL = fma((double)f4_get(l[u], j * R + k), g[k], aL);                                  \
+            }                                                                                              \
+        }                                                                                                  \
+    }
+    for (; p + 128 * (U - 1) < Lv; p += 128 * U) {
+        int c[U][C];
         float4 d[U], l[U];
 #pragma unroll
         for (int u = 0; u < U; ++u) {
-            c[u] = ld_idx4<I16>(cbase, e0 + p + 128 * u, add);
+            ld_idx<I16, C>(cbase, i0 + (p + 128 * u) / R, add, c[u]);
             if (M & 1) d[u] = ld_stream_f4(dp + p + 128 * u);
             if (M & 2) l[u] = ld_stream_f4(lp + p + 128 * u);
         }
 #pragma unroll
-        for (int u = 0; u < U; ++u) {
-            if (M == 3) {
-                const double2 g0 = __ldg(vec + c[u].x), g1 = __ldg(vec + c[u].y), g2 = __ldg(vec + c[u].z), g3 = __ldg(vec + c[u].w);
-                fma4(aD, d[u], g0.x, g1.x, g2.x, g3.x);
-                fma4(aL, l[u], g0.y, g1.y, g2.y, g3.y);
-            } else {
-                const double g0 = __ldg(vs + c[u].x), g1 = __ldg(vs + c[u].y), g2 = __ldg(vs + c[u].z), g3 = __ldg(vs + c[u].w);
-                if (M == 1) fma4(aD, d[u], g0, g1, g2, g3); else fma4(aL, l[u], g0, g1, g2, g3);
-            }
-        }
+        for (int u = 0; u < U; ++u) { TR_CONSUME(u) }
     }
-    if (p < L) {   // remainder: one predicated trip (see fwd_row)
-        int4 c[U - 1];
+    if (p < Lv) {   // remainder: one predicated trip (see fwd_row)
+        int c[U - 1][C];
         float4 d[U - 1], l[U - 1];
 #pragma unroll
         for (int u = 0; u < U - 1; ++u) {
-            const bool ok = p + 128 * u < L;
-            c[u] = ok ? ld_idx4<I16>(cbase, e0 + p + 128 * u, add) : make_int4(0, 0, 0, 0);
+            const bool ok = p + 128 * u < Lv;
+            if (ok) ld_idx<I16, C>(cbase, i0 + (p + 128 * u) / R, add, c[u]);
+            else {
+#pragma unroll
+                for (int j = 0; j < C; ++j) c[u][j] = 0;
+            }
             if (M & 1) d[u] = ok ? ld_stream_f4(dp + p + 128 * u) : make_float4(0.f, 0.f, 0.f, 0.f);
             if (M & 2) l[u] = ok ? ld_stream_f4(lp + p + 128 * u) : make_float4(0.f, 0.f, 0.f, 0.f);
         }
 #pragma unroll
         for (int u = 0; u < U - 1; ++u) {
-            if (p + 128 * u < L) {
-                if (M == 3) {
-                    const double2 g0 = __ldg(vec + c[u].x), g1 = __ldg(vec + c[u].y), g2 = __ldg(vec + c[u].z), g3 = __ldg(vec + c[u].w);
-                    fma4(aD, d[u], g0.x, g1.x, g2.x, g3.x);
-                    fma4(aL, l[u], g0.y, g1.y, g2.y, g3.y);
-                } else {
-                    const double g0 = __ldg(vs + c[u].x), g1 = __ldg(vs + c[u].y), g2 = __ldg(vs + c[u].z), g3 = __ldg(vs + c[u].w);
-                    if (M == 1) fma4(aD, d[u], g0, g1, g2, g3); else fma4(aL, l[u], g0, g1, g2, g3);
-                }
-            }
+            if (p + 128 * u < Lv) { TR_CONSUME(u) }
         }
     }
+#undef TR_CONSUME
     return aD + aL;
 }
 
-// One warp per item, round-robin.  Items are in longest-first order (ties in (structure, spot) order, so the warps
-// of a CTA mostly work on neighbouring spots of one structure and share L1 lines of the gather vector).  Item r
-// stores its partial sum in slot item_slot[r]; k_combine adds the slots of every spot in slot order.  No
-// floating-point atomics, no fences: the result does not depend on the schedule.
-template <bool I16>
+// One warp per item from the work queue; items are in longest-first order (ties in (structure, spot) order, so the warps of
+// a CTA mostly work on neighbouring spots of one structure and share L1 lines of the gather vector).  Item e stores its
+// partial sum in slot item_slot[e]; k_combine adds the slots of every spot in slot order.  No floating-point atomics, no
+// fences: the result does not depend on the schedule.
+template <int R, bool I16>
 __global__ void __launch_bounds__(FWD_THREADS, FWD_MIN_CTAS)
-k_transpose(long long n, const Item* __restrict__ items, const int32_t* __restrict__ item_slot,
+k_transpose(long long n, const Item* __restrict__ items, const int32_t* __restrict__ item_slot, WorkQueue* __restrict__ wq,
             const uint8_t* __restrict__ mode, const void* __restrict__ t_col, const float* __restrict__ tD,
             const float* __restrict__ tL, const GatherVec vec, double* __restrict__ partial)
 {
     const int lane = threadIdx.x & 31;
-    const long long nwarps = (long long)gridDim.x * FWD_WARPS;
-    long long r = (long long)blockIdx.x * FWD_WARPS + (threadIdx.x >> 5);
-    Item it;
-    if (r < n) it = ld_item(items + r);
+    const int nwarps = gridDim.x * FWD_WARPS, ni = (int)n;
+    int e0 = blockIdx.x * FWD_WARPS + (threadIdx.x >> 5), e1 = e0 + nwarps;
+    if (e0 < ni) prefetch_l1(items + e0);
     pdl_wait();
     pdl_trigger();
-    while (r < n) {
-        const long long rn = r + nwarps;
-        Item nx;
-        if (rn < n) nx = ld_item(items + rn);
+    while (e0 < ni) {
+        const Item it = ld_item(items + e0);
+        unsigned int e2 = 0;
+        if (wq && lane == 0) e2 = atomicAdd(&wq->next, 1u);
+        if (e1 < ni) prefetch_l1(items + e1);
         const int m = mode[it.seg & 0xFF];
-        const int add = (it.seg >> 8) << 16;              // 16-bit form: the run's 65536-row block
+        const int add = (it.seg >> 8) << 16;              // 16-bit form: the run's group of 65536 block rows
         double tot = 0.0;
-        if (m == 3) tot = tr_item<3, I16>(t_col, it.start, add, tD + it.start, tL + it.start, it.len, lane, vec);
-        else if (m == 1) tot = tr_item<1, I16>(t_col, it.start, add, tD + it.start, nullptr, it.len, lane, vec);
-        else if (m == 2) tot = tr_item<2, I16>(t_col, it.start, add, nullptr, tL + it.start, it.len, lane, vec);
+        if (m == 3) tot = tr_item<3, R, I16>(t_col, it.start, add, tD + it.start, tL + it.start, it.len, lane, vec);
+        else if (m == 1) tot = tr_item<1, R, I16>(t_col, it.start, add, tD + it.start, nullptr, it.len, lane, vec);
+        else if (m == 2) tot = tr_item<2, R, I16>(t_col, it.start, add, nullptr, tL + it.start, it.len, lane, vec);
         if (m) tot = warp_sum(tot);
-        if (lane == 0) partial[item_slot[r]] = tot;
-        r = rn;
-        it = nx;
+        if (lane == 0) partial[item_slot[e0]] = tot;
+        e0 = e1;
+        e1 = wq ? 2 * nwarps + (int)__shfl_sync(0xffffffffu, e2, 0) : e1 + nwarps;
     }
+    if (wq) queue_leave(wq, lane, (unsigned int)nwarps);
 }
 
 // Second stage of a transposed pass: one thread per spot adds the spot's partial sums in slot order (ascending
@@ -513,6 +635,5 @@ k_combine(long long S, const long long* __restrict__ item_ptr, const double* __r
         x[j] = v < 0.0 ? 0.0 : v;                          // clamp
     } else if (ie > ib) f_out[j] = (float)tot;
 }
-
 
 }  // namespace fredopt

@@ -35,52 +35,60 @@ extern thread_local std::string g_last_cuda_error;      // defined in passes.cu
     } while (0)
 
 // ============================================================================================ plan
-// view of a row set for the create-time kernels
-struct RowList {
-    long long n;                 // rows in the list
-    const long long* start;      // [n] offset of the row in the set's padded arrays (multiple of 4)
-    const int32_t* len;          // [n] padded length (multiple of 4)
-    const int32_t* seg;          // [n] segment (structure - 1), or nullptr = segment 0
-    const int32_t* vox;          // [n] voxel index of the row
-};
-
+// A row set in the blocked storage of DESIGN.md "Data layout": n BLOCK ROWS of R consecutive rows each (rows R b + k; the last
+// block of a structure may hold fewer than R real rows -- its other rows are padding: vox = -1, rseg = -1).  An ENTRY is one
+// (block row, column) pair over the union of the block's column patterns, with R values per matrix (zeros where a row has no
+// entry there).  C = 4 / R entries share one 128-bit value load; every block row holds a multiple of C entries (padding:
+// column 0, values 0) and starts at a multiple of C; inside every chunk of 32 C entries the entries are interleaved
+// (perm_pos in plan_build.cu).
 struct RowSet {
-    long long n = 0;                 // rows
+    int R = 1;                       // rows per block row (1, 2 or 4)
+    long long n = 0;                 // block rows = work items of the forward pass
+    long long n_rows = 0;            // n * R: length of every per-row array (d, l, norms, gather vectors, vox, rseg)
+    long long n_true = 0;            // real rows
     int n_seg = 1;
-    // padded index / value arrays of the set (rows stored back to back in list order)
-    int32_t* col = nullptr;          // int32 column indices (kept for transposition; the hot kernels read col16 if set)
-    uint16_t* col16 = nullptr;       // the same indices as 16 bits when n_cols <= 65536 (2 B instead of 4 B per non-zero)
-    float* valD = nullptr;
+    // index / value arrays of the set (block rows stored back to back in list order); exactly one of col / col16 is set
+    int32_t* col = nullptr;          // int32 column index per entry
+    uint16_t* col16 = nullptr;       // 16-bit form when n_cols <= 65536 (2 B instead of 4 B per entry)
+    float* valD = nullptr;           // R values per entry: value k of entry position p at p * R + k
     float* valL = nullptr;
-    int32_t* vox = nullptr;          // [n]
-    int32_t* seg = nullptr;          // [n] or nullptr
-    long long* start = nullptr;      // [n]
-    int32_t* len = nullptr;          // [n] padded
-    int32_t* ulen = nullptr;         // [n] unpadded
-    Item* items = nullptr;           // [n] {start, len, seg}: what the forward kernel reads
-    long long nnz = 0;               // unpadded entries in the set
-    // CSR of the transposes restricted to this set, SEGMENT-major: run k = seg*S + spot; columns = list index
+    int32_t* vox = nullptr;          // [n_rows] voxel of the row, -1 = padding
+    int16_t* rseg = nullptr;         // [n_rows] structure - 1 of the row, -1 = padding (labelled set only)
+    int32_t* seg = nullptr;          // [n] structure - 1 of the block row, or nullptr (one segment)
+    long long* start = nullptr;      // [n + 1] first entry position of the block row (multiple of C)
+    int32_t* len = nullptr;          // [n] entries, padded to a multiple of C
+    int32_t* ulen = nullptr;         // [n] entries of the union pattern
+    Item* items = nullptr;           // [n] {start * R, len * R, seg | real rows << 8}: what the forward kernel reads
+    Item* items_x = nullptr;         // [n] the same items in execution order (longest first), or nullptr = list order
+    int32_t* item_blk = nullptr;     // [n] block row of items_x[e]
+    long long nnz = 0;               // non-zeros of the real rows
+    long long entries = 0;           // entries of the union patterns (= nnz when R = 1)
+    long long entries_padded = 0;
+    // CSR of the transposes restricted to this set, SEGMENT-major: run k = (seg * S + spot) * H + group; an entry of a run is
+    // one block row (ascending) with its R values per matrix; index = block row (low 16 bits in the 16-bit form)
     bool t_built = false;
-    long long* t_ptr = nullptr;      // [n_seg*S + 1]
-    int32_t* t_col = nullptr;        // compact row index (32-bit form: only if the 16-bit form does not apply)
-    uint16_t* t_col16 = nullptr;     // low 16 bits of the compact row index; runs are cut where the high bits change
-    int t_H = 1;                     // number of 65536-row blocks of the list (1 in the 32-bit form)
+    long long* t_ptr = nullptr;      // [n_seg * S * H + 1] entry positions
+    int32_t* t_col = nullptr;        // block-row index (32-bit form: only if the 16-bit form does not apply)
+    uint16_t* t_col16 = nullptr;     // low 16 bits of the block-row index; runs are cut where the high bits change
+    int t_H = 1;                     // number of 65536-block-row groups of the list (1 in the 32-bit form)
     float* t_valD = nullptr;
     float* t_valL = nullptr;
-    long long t_nnz_padded = 0;
-    // work items of the transposed pass: runs cut into pieces of at most TR_ITEM_MAX entries
+    long long t_entries_padded = 0;
+    // work items of the transposed pass: runs cut into pieces of at most TR_ITEM_MAX values per matrix
     long long t_n_items = 0;
-    Item* t_items = nullptr;         // [t_n_items]
+    Item* t_items = nullptr;         // [t_n_items] longest first
     int32_t* t_item_slot = nullptr;  // [t_n_items] slot of the item's partial sum
+    Item* t_items_run = nullptr;     // [t_n_items] the same items in run (= storage) order
+    int32_t* t_slot_run = nullptr;
     long long* t_item_ptr = nullptr; // [S+1] partial-sum slots of spot j: t_item_ptr[j] .. t_item_ptr[j+1]-1
     double* t_partial = nullptr;     // [t_n_items]
     // block-sequential AMS: the same items grouped by structure (longest first inside a structure) and the slot
-    // ranges per (spot, structure, 65536-row block)
+    // ranges per (spot, structure, group)
     Item* t_items_seg = nullptr;     // [t_n_items]
     int32_t* t_slot_seg = nullptr;   // [t_n_items]
     long long* t_slot_ptr = nullptr; // [S * n_seg * t_H + 1]
     std::vector<long long> t_seg_item_begin;   // host: items of structure s are t_seg_item_begin[s] .. [s+1]-1
-    RowList view() const { return RowList{n, start, len, seg, vox}; }
+    const void* colp() const { return col16 ? (const void*)col16 : (const void*)col; }
 };
 
 struct EventPair { cudaEvent_t a, b; int pass; };
@@ -95,6 +103,7 @@ struct fredopt_plan {
     // full: all non-empty rows of the padded matrix (union pattern); act: a compact copy of the rows with a label,
     // ordered by (structure, voxel)
     RowSet full, act;
+    std::vector<long long> row_base;       // host: rows of structure s are row_base[s] .. row_base[s] + h_tab[s].rows - 1 of `act`
     long long full_class[9] = {0, 0, 0, 0, 0, 0, 0, 0, 0};   // rows of length class c of `full`: full_class[c] .. full_class[c+1]-1
     // per active row
     double *nD = nullptr, *nL = nullptr, *nT = nullptr;
@@ -115,12 +124,17 @@ struct fredopt_plan {
     double *part_prox = nullptr, *part_phi = nullptr;
     long long* part_cnt = nullptr;
     int* sink = nullptr;
+    WorkQueue* wq = nullptr;                                                   // work queue of the item kernels (one launch at a time)
     // options / host state
     double eta = 1.0;
     long long reductionsN = 1, max_trials = 200;
     int accept_check = 1, use_graph = 1, time_passes = 0, block_sequential = 0, normalize_grad = 0, one_sided_cost = 0;
     int use_pdl = 1;
+    int fwd_dynamic = 1, tr_dynamic = 0;   // item kernels fed from the work queue (else static round-robin, two waves)
+    int fwd_sorted = 1, tr_sorted = 1;     // items taken longest first (else in storage order)
     bool force_idx32 = false;          // create option: int32 indices in both orientations
+    int block_rows_opt = 0;            // create option: rows per block row of the labelled set (0 = chosen by stored bytes)
+    float* out_stage = nullptr;        // lazily: 2 x n_rows floats staging host outputs of dose_let / spmv_forward
     bool started = false;
     float latched_beta0 = 0.f, latched_a = 0.f;
     cudaError_t launch_err = cudaSuccess;   // first error of a kernel launch since the last check (klaunch)
@@ -193,6 +207,9 @@ int build_transpose(fredopt_plan* P, RowSet& R);                 // CSR of the t
 int fwd_grid(fredopt_plan* P, long long n);                      // grid of the item kernels (one warp per item, round-robin)
 void state_init(fredopt_plan* P);                                // device state at creation
 extern const ResidArgs NO_RESID;
+void launch_fwd_kernel(fredopt_plan* P, int epi, const RowSet& R, long long b0, long long n, const uint8_t* mode, const double* x,
+                       double* oD, double* oL, const GatherVec& pq, const StructInfo* tab, double* cpart, float* fD, float* fL,
+                       int letd_out, const ResidArgs& ra);
 void launch_forward(fredopt_plan* P, const RowSet& R, const uint8_t* mode, const double* x, double* oD, double* oL, int epi,
                     int write_uv = 0);
 void launch_transpose(fredopt_plan* P, int tepi, const RowSet& R, const uint8_t* mode, const GatherVec& vec, double* g_out,

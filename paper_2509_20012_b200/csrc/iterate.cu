@@ -18,62 +18,88 @@ static void ev_end(fredopt_plan* P) {
     cudaEventRecord(P->events.back().b, P->stream);
 }
 
-// grid of the item kernels: one warp per item up to FWD_CTAS_PER_SM resident-CTA-fulls per SM (then round-robin)
+// grid of the item kernels: persistent, one CTA per resident slot (launch bounds of k_forward / k_transpose); the items come
+// from the work queue
 constexpr int GRAPH_UNROLL = 8;       // iterations captured into the long graph
-constexpr int FWD_CTAS_PER_SM = 2 * FWD_MIN_CTAS;   // 2 waves of the CTAs an SM holds (launch bounds of k_forward / k_transpose)
 int fwd_grid(fredopt_plan* P, long long n) {
-    const int cap = P->sm_count * FWD_CTAS_PER_SM < MAX_PARTIALS ? P->sm_count * FWD_CTAS_PER_SM : MAX_PARTIALS;
-    return grid_for(n, FWD_WARPS, cap);
+    return grid_for(n, FWD_WARPS, P->sm_count * FWD_MIN_CTAS);
 }
+// static round-robin form of the item kernels (no queue): two waves of the resident CTAs
+static int static_grid(fredopt_plan* P, long long n) { return grid_for(n, FWD_WARPS, P->sm_count * FWD_MIN_CTAS * 2); }
 
 
 const ResidArgs NO_RESID{nullptr, nullptr, nullptr, GatherVec{nullptr, nullptr, nullptr}, nullptr, nullptr, nullptr, nullptr};
 
-// epi: EPI_STORE (d, l), EPI_STORE_PQ (d, l and the cost residuals p, q), EPI_CPART (Dg, Lg and partial sums of c),
-// EPI_RESID (d, l and the residual / violation epilogue: step coefficients u, v if write_uv, statistics partials)
+// k_forward<EPI, R, I16> over n block rows of R starting at block row b0 (per-row arguments are passed already offset by the
+// caller: oD, oL, vox point at row b0 * R)
+#define FREDOPT_DISPATCH(RB, I16, CALL)                                             \
+    switch (RB) {                                                                   \
+        case 1: if (I16) { CALL(1, true); } else { CALL(1, false); } break;         \
+        case 2: if (I16) { CALL(2, true); } else { CALL(2, false); } break;         \
+        default: if (I16) { CALL(4, true); } else { CALL(4, false); } break;        \
+    }
+void launch_fwd_kernel(fredopt_plan* P, int epi, const RowSet& R, long long b0, long long n, const uint8_t* mode, const double* x,
+                       double* oD, double* oL, const GatherVec& pq, const StructInfo* tab, double* cpart, float* fD, float* fL,
+                       int letd_out, const ResidArgs& ra) {
+    if (n <= 0) return;
+    WorkQueue* wq = P->fwd_dynamic ? P->wq : nullptr;
+    const int g = wq ? fwd_grid(P, n) : static_grid(P, n);
+    const bool whole = P->fwd_sorted && b0 == 0 && n == R.n && R.items_x;   // whole set: longest-first execution order
+    const Item* items = whole ? R.items_x : R.items + b0;
+    const int32_t* iblk = whole ? R.item_blk : nullptr;
+    const int32_t* vox = R.vox ? R.vox + b0 * R.R : nullptr;
+    const void* col = R.colp();
+    const bool i16 = R.col16 != nullptr;
+#define FWD_CALL(RB, I16)                                                                                                        \
+    switch (epi) {                                                                                                               \
+        case EPI_STORE: klaunch(P, k_forward<EPI_STORE, RB, I16>, g, FWD_THREADS, n, items, iblk, wq, vox, mode, col, R.valD, R.valL, x, oD, oL, pq, tab, cpart, P->st, fD, fL, letd_out, ra); break;       \
+        case EPI_STORE_PQ: klaunch(P, k_forward<EPI_STORE_PQ, RB, I16>, g, FWD_THREADS, n, items, iblk, wq, vox, mode, col, R.valD, R.valL, x, oD, oL, pq, tab, cpart, P->st, fD, fL, letd_out, ra); break; \
+        case EPI_CPART: klaunch(P, k_forward<EPI_CPART, RB, I16>, g, FWD_THREADS, n, items, iblk, wq, vox, mode, col, R.valD, R.valL, x, oD, oL, pq, tab, cpart, P->st, fD, fL, letd_out, ra); break;       \
+        case EPI_F32VOX: klaunch(P, k_forward<EPI_F32VOX, RB, I16>, g, FWD_THREADS, n, items, iblk, wq, vox, mode, col, R.valD, R.valL, x, oD, oL, pq, tab, cpart, P->st, fD, fL, letd_out, ra); break;     \
+        default: klaunch(P, k_forward<EPI_RESID, RB, I16>, g, FWD_THREADS, n, items, iblk, wq, vox, mode, col, R.valD, R.valL, x, oD, oL, pq, tab, cpart, P->st, fD, fL, letd_out, ra); break;              \
+    }
+    FREDOPT_DISPATCH(R.R, i16, FWD_CALL)
+#undef FWD_CALL
+}
+
+// k_transpose<R, I16> over n work items
+void launch_tr_kernel(fredopt_plan* P, const RowSet& R, const Item* items, const int32_t* slots, long long n, const uint8_t* mode,
+                      const GatherVec& vec) {
+    if (n <= 0) return;
+    WorkQueue* wq = P->tr_dynamic ? P->wq : nullptr;
+    const int g = wq ? fwd_grid(P, n) : static_grid(P, n);
+    const void* tc = R.t_col16 ? (const void*)R.t_col16 : (const void*)R.t_col;
+    const bool i16 = R.t_col16 != nullptr;
+#define TR_CALL(RB, I16) klaunch(P, k_transpose<RB, I16>, g, FWD_THREADS, n, items, slots, wq, mode, tc, R.t_valD, R.t_valL, vec, R.t_partial)
+    FREDOPT_DISPATCH(R.R, i16, TR_CALL)
+#undef TR_CALL
+}
+
+// epi: EPI_STORE (d, l), EPI_STORE_PQ (d, l, the cost residuals p, q and partial sums of chi^2), EPI_CPART (Dg, Lg and partial
+// sums of c), EPI_RESID (d, l and the residual / violation epilogue: step coefficients u, v if write_uv, statistics partials)
 void launch_forward(fredopt_plan* P, const RowSet& R, const uint8_t* mode, const double* x, double* oD, double* oL, int epi,
                     int write_uv) {
     if (R.n == 0) {
-        if (epi == EPI_CPART) cudaMemsetAsync(P->cpart, 0, sizeof(double) * MAX_PARTIALS, P->stream);
+        if (epi == EPI_CPART) cudaMemsetAsync(P->cpart, 0, 8, P->stream);
         if (epi == EPI_RESID) {   // nothing to visit: zero statistics (finalize reads one partial)
             cudaMemsetAsync(P->part_prox, 0, 8, P->stream); cudaMemsetAsync(P->part_phi, 0, 8, P->stream); cudaMemsetAsync(P->part_cnt, 0, 8, P->stream);
             if (write_uv) klaunch(P, k_sweep_end, grid_for(P->S, 256, 1 << 30), 256, P->S, P->x, P->st);   // k, eta^k still advance
         }
         return;
     }
-    const int g = fwd_grid(P, R.n);
     const GatherVec none{nullptr, nullptr, nullptr};
     ResidArgs ra = NO_RESID;
     if (epi == EPI_RESID) ra = ResidArgs{P->nD, P->nL, P->nT, write_uv ? P->uv : none, P->part_prox, P->part_phi, P->part_cnt, P->st};
-#define FWD_LAUNCH(E, I16, COL, PQ, TAB, CP)                                                                                   \
-    klaunch(P, k_forward<E, I16>, g, FWD_THREADS, R.n, R.items, R.vox, mode, COL, R.valD, R.valL, x, oD, oL, PQ, TAB, CP, P->st, \
-            nullptr, nullptr, 0, ra)
-    if (R.col16) {
-        if (epi == EPI_CPART) FWD_LAUNCH(EPI_CPART, true, R.col16, none, P->tab, P->cpart);
-        else if (epi == EPI_STORE_PQ) FWD_LAUNCH(EPI_STORE_PQ, true, R.col16, P->pq, P->tab, P->part_phi);
-        else if (epi == EPI_RESID) FWD_LAUNCH(EPI_RESID, true, R.col16, none, P->tab, nullptr);
-        else FWD_LAUNCH(EPI_STORE, true, R.col16, none, nullptr, nullptr);
-    } else {
-        if (epi == EPI_CPART) FWD_LAUNCH(EPI_CPART, false, R.col, none, P->tab, P->cpart);
-        else if (epi == EPI_STORE_PQ) FWD_LAUNCH(EPI_STORE_PQ, false, R.col, P->pq, P->tab, P->part_phi);
-        else if (epi == EPI_RESID) FWD_LAUNCH(EPI_RESID, false, R.col, none, P->tab, nullptr);
-        else FWD_LAUNCH(EPI_STORE, false, R.col, none, nullptr, nullptr);
-    }
-#undef FWD_LAUNCH
+    launch_fwd_kernel(P, epi, R, 0, R.n, mode, x, oD, oL, epi == EPI_STORE_PQ ? P->pq : none, epi == EPI_STORE ? nullptr : P->tab,
+                      epi == EPI_CPART ? P->cpart : epi == EPI_STORE_PQ ? P->part_phi : nullptr, nullptr, nullptr, 0, ra);
 }
-static int cpart_count(fredopt_plan* P) { return P->act.n ? fwd_grid(P, P->act.n) : MAX_PARTIALS; }
+static int cpart_count(fredopt_plan* P) { return P->act.n ? (int)P->act.n : 1; }     // partial sums per block row
 
 void launch_transpose(fredopt_plan* P, int tepi, const RowSet& R, const uint8_t* mode, const GatherVec& vec, double* g_out, double* x,
                       float* f_out) {
     if (R.t_n_items == 0 && tepi != TEPI_UPDATE) return;          // nothing to add; the update still clamps (R6)
-    if (R.t_n_items > 0) {
-        if (R.t_col16)
-            klaunch(P, k_transpose<true>, fwd_grid(P, R.t_n_items), FWD_THREADS, R.t_n_items, R.t_items, R.t_item_slot, mode, R.t_col16,
-                    R.t_valD, R.t_valL, vec, R.t_partial);
-        else
-            klaunch(P, k_transpose<false>, fwd_grid(P, R.t_n_items), FWD_THREADS, R.t_n_items, R.t_items, R.t_item_slot, mode, R.t_col,
-                    R.t_valD, R.t_valL, vec, R.t_partial);
-    }
+    if (P->tr_sorted) launch_tr_kernel(P, R, R.t_items, R.t_item_slot, R.t_n_items, mode, vec);
+    else launch_tr_kernel(P, R, R.t_items_run, R.t_slot_run, R.t_n_items, mode, vec);
     const int gc = grid_for(P->S, 256, 1 << 30);
     if (tepi == TEPI_GRAD) klaunch(P, k_combine<TEPI_GRAD>, gc, 256, P->S, R.t_item_ptr, R.t_partial, g_out, P->gpart, x, P->st, f_out);
     else if (tepi == TEPI_UPDATE) klaunch(P, k_combine<TEPI_UPDATE>, gc, 256, P->S, R.t_item_ptr, R.t_partial, g_out, P->gpart, x, P->st, f_out);
@@ -82,13 +108,13 @@ void launch_transpose(fredopt_plan* P, int tepi, const RowSet& R, const uint8_t*
 
 static int res_grid(fredopt_plan* P) {
     const int cap = P->sm_count * 4 < MAX_PARTIALS ? P->sm_count * 4 : MAX_PARTIALS;
-    const long long n = P->act.n > P->S ? P->act.n : P->S;
+    const long long n = P->act.n_rows > P->S ? P->act.n_rows : P->S;
     return grid_for(n, ROW_THREADS, cap);
 }
 
 static void launch_residual(fredopt_plan* P, double* d, double* l, int use_beta, int final, int write_uv) {
     const int g = res_grid(P);
-    klaunch(P, k_residual, g, ROW_THREADS, P->act.n, P->act.items, P->tab, P->st, d, l, P->Dg, P->Lg, P->nD, P->nL, P->nT, P->uv, P->pq,
+    klaunch(P, k_residual, g, ROW_THREADS, P->act.n_rows, P->act.rseg, P->tab, P->st, d, l, P->Dg, P->Lg, P->nD, P->nL, P->nT, P->uv, P->pq,
             P->x, P->g, P->S, P->part_prox, P->part_phi, P->part_cnt, use_beta, final, write_uv);
 }
 
@@ -102,8 +128,6 @@ void launch_finalize(fredopt_plan* P, int n_part) {
 static void enqueue_block_sweep(fredopt_plan* P) {
     const RowSet& A = P->act;
     klaunch(P, k_sweep_begin, 1, 1, P->st);
-    std::vector<long long> row_begin((size_t)P->n_struct + 1, 0);
-    for (int s = 0; s < P->n_struct; ++s) row_begin[s + 1] = row_begin[s] + (long long)P->h_tab[s].rows;
     const int kind_flag[3] = {F_DOSE_SLAB, F_DL_SLAB, F_LETD};
     const int kind_mode[3] = {1, 2, 3};
     const GatherVec none{nullptr, nullptr, nullptr};
@@ -111,15 +135,13 @@ static void enqueue_block_sweep(fredopt_plan* P) {
         for (int s = 0; s < P->n_struct; ++s) {
             const StructInfo& T = P->h_tab[s];
             if (!(T.flags & kind_flag[kind])) continue;
-            const long long rb = row_begin[s], re = row_begin[s + 1], nr = re - rb;
+            const long long rb = P->row_base[s], nr = (long long)T.rows, re = rb + nr;     // real rows: padding rows follow them
             if (nr == 0) continue;
+            const int RB = A.R;
             const uint8_t* md = P->mode_fixed + (size_t)kind_mode[kind] * P->max_seg;
             ev_begin(P, FREDOPT_PASS_FORWARD_X);
-            {
-                const int g = fwd_grid(P, nr);
-                if (A.col16) klaunch(P, k_forward<EPI_STORE, true>, g, FWD_THREADS, nr, A.items + rb, A.vox + rb, md, A.col16, A.valD, A.valL, P->x, P->d + rb, P->l + rb, none, nullptr, nullptr, nullptr, nullptr, nullptr, 0, NO_RESID);
-                else klaunch(P, k_forward<EPI_STORE, false>, g, FWD_THREADS, nr, A.items + rb, A.vox + rb, md, A.col, A.valD, A.valL, P->x, P->d + rb, P->l + rb, none, nullptr, nullptr, nullptr, nullptr, nullptr, 0, NO_RESID);
-            }
+            launch_fwd_kernel(P, EPI_STORE, A, rb / RB, (nr + RB - 1) / RB, md, P->x, P->d + rb, P->l + rb, none, nullptr, nullptr, nullptr, nullptr, 0,
+                              NO_RESID);
             ev_end(P);
             ev_begin(P, FREDOPT_PASS_RESIDUAL);
             const int gr = grid_for(nr, ROW_THREADS, P->sm_count * 4 < MAX_PARTIALS ? P->sm_count * 4 : MAX_PARTIALS);
@@ -129,11 +151,7 @@ static void enqueue_block_sweep(fredopt_plan* P) {
             const long long ib = A.t_seg_item_begin.empty() ? 0 : A.t_seg_item_begin[s], ie = A.t_seg_item_begin.empty() ? 0 : A.t_seg_item_begin[s + 1];
             if (m == 0) continue;                      // no row of the block has a non-zero norm: violations counted, no step
             ev_begin(P, FREDOPT_PASS_TRANSPOSE_B);
-            if (ie > ib) {
-                const int g = fwd_grid(P, ie - ib);
-                if (A.t_col16) klaunch(P, k_transpose<true>, g, FWD_THREADS, ie - ib, A.t_items_seg + ib, A.t_slot_seg + ib, md, A.t_col16, A.t_valD, A.t_valL, P->uv, A.t_partial);
-                else klaunch(P, k_transpose<false>, g, FWD_THREADS, ie - ib, A.t_items_seg + ib, A.t_slot_seg + ib, md, A.t_col, A.t_valD, A.t_valL, P->uv, A.t_partial);
-            }
+            launch_tr_kernel(P, A, A.t_items_seg + ib, A.t_slot_seg + ib, ie - ib, md, P->uv);
             const double factor = (T.w < 1.0 ? T.w : 1.0) / (double)m;
             klaunch(P, k_combine_block, grid_for(P->S, 256, 1 << 30), 256, P->S, A.t_slot_ptr, s, A.n_seg, A.t_H, A.t_partial, P->x, P->st, factor,
                     P->part_prox, gr);
@@ -158,8 +176,8 @@ static int enqueue_iteration(fredopt_plan* P, bool sa) {
             ev_end(P);
             ev_begin(P, FREDOPT_PASS_SELECT);
             klaunch(P, k_select, 1, 1024, P->st, P->gpart, P->act.t_n_items ? grid_for(P->S, 256, 1 << 30) : 0, P->cpart, cpart_count(P),
-                    P->part_phi, P->act.n == 0 ? 0 : t == 0 ? fwd_grid(P, P->act.n) : res_grid(P), P->act.n,
-                    P->act.items, P->tab, P->d, P->l, P->Dg, P->Lg);                                     // a4, a6: beta
+                    P->part_phi, P->act.n == 0 ? 0 : t == 0 ? (int)P->act.n : res_grid(P), P->act.n_rows,
+                    P->act.rseg, P->tab, P->d, P->l, P->Dg, P->Lg);                                     // a4, a6: beta
             ev_end(P);
             ev_begin(P, FREDOPT_PASS_RESIDUAL);
             const int last = t == P->reductionsN - 1 && !P->block_sequential;
@@ -210,6 +228,13 @@ int fredopt_set_option(fredopt_plan* P, int32_t key, double value) {
             break;
         }
         case FREDOPT_OPT_USE_GRAPH: P->use_graph = value != 0.0; break;
+        case FREDOPT_OPT_WORK_QUEUE: {
+            const int v = (int)value;
+            if (v < 0 || v > 15) return FREDOPT_INVALID_ARG;
+            P->fwd_dynamic = v & 1; P->tr_dynamic = (v >> 1) & 1; P->fwd_sorted = (v >> 2) & 1; P->tr_sorted = (v >> 3) & 1;
+            for (int i = 0; i < 8; ++i) if (P->gexec[i]) { cudaGraphExecDestroy(P->gexec[i]); P->gexec[i] = nullptr; }
+            break;
+        }
         case FREDOPT_OPT_USE_PDL:
             if (P->use_pdl != (value != 0.0)) {            // the launch attribute is part of a captured graph: capture again
                 P->use_pdl = value != 0.0;
@@ -289,7 +314,7 @@ int fredopt_iterate(fredopt_plan* P, int32_t n_iter, float lambda, float beta0, 
             CK(P->launch_err);
         }
         if (!P->block_sequential)                         // block mode keeps its sweep statistics in the state already
-            launch_finalize(P, sa ? res_grid(P) : (P->act.n ? fwd_grid(P, P->act.n) : 1));
+            launch_finalize(P, sa ? res_grid(P) : (P->act.n ? (int)P->act.n : 1));
     }
     CK(cudaGetLastError());
     return FREDOPT_OK;
@@ -302,7 +327,8 @@ int fredopt_get_stats(fredopt_plan* P, fredopt_stats* out) {
     CK(cudaStreamSynchronize(P->stream));
     out->k = h.k; out->s = h.s; out->trials = h.trials; out->n_violated = h.n_viol;
     out->n_sets = h.n_sets; out->n_zero_norm_sets = h.n_zero;
-    out->n_active_rows = P->act.n; out->nnz = P->nnz; out->nnz_active = P->act.nnz;
+    out->n_active_rows = P->act.n_true; out->nnz = P->nnz; out->nnz_active = P->act.nnz;
+    out->block_rows = P->act.R; out->entries_active = P->act.entries;
     long long b = 0;
     const int sa_passes[] = {FREDOPT_PASS_FORWARD_X, FREDOPT_PASS_TRANSPOSE_G, FREDOPT_PASS_FORWARD_G, FREDOPT_PASS_SELECT,
                              FREDOPT_PASS_RESIDUAL, FREDOPT_PASS_TRANSPOSE_B};

@@ -56,8 +56,8 @@ __global__ void k_f64_to_f32(const double* __restrict__ in, float* __restrict__ 
 __global__ void k_gather_uv(const float* __restrict__ u, const float* __restrict__ v, const int32_t* __restrict__ vox,
                             const GatherVec out, long long n) {
     for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (long long)gridDim.x * blockDim.x) {
-        const int vx = vox[i];
-        gv_store(out, i, u ? (double)u[vx] : 0.0, v ? (double)v[vx] : 0.0);
+        const int vx = vox[i];                                       // -1: padding row of a ragged block
+        gv_store(out, i, (u && vx >= 0) ? (double)u[vx] : 0.0, (v && vx >= 0) ? (double)v[vx] : 0.0);
     }
 }
 

@@ -19,17 +19,36 @@ __global__ void k_set_params(DevState* st, double lambda, double beta0, double a
 
 // chi^2 of Eq. (2) at x - b g from the stored products: d - b Dg, l - b Lg (exact: the products are linear in x).  All
 // threads of the CTA take part; the value is valid in thread 0.
-__device__ __forceinline__ double cost_along(double b, long long n, const Item* __restrict__ items,
+__device__ __forceinline__ double cost_along(double b, long long n, const int16_t* __restrict__ rseg,
                                              const StructInfo* __restrict__ tab, const double* __restrict__ d,
                                              const double* __restrict__ l, const double* __restrict__ Dg,
                                              const double* __restrict__ Lg, int one_sided, double* sm) {
     double phi = 0.0;
     for (long long a = threadIdx.x; a < n; a += blockDim.x) {
-        const StructInfo& T = tab[items[a].seg];
+        const int sg = rseg[a];
+        if (sg < 0) continue;                                          // padding row of a ragged block
+        const StructInfo& T = tab[sg];
         if (T.flags & F_DOSE_REF) { const double e = T.dose_ref - fma(-b, Dg[a], d[a]); phi += T.what * e * e; }
         if (T.flags & F_DL_REF) { const double e = T.dl_ref - fma(-b, Lg[a], l[a]); if (!(one_sided && e > 0.0)) phi += T.what * e * e; }
     }
     return block_sum(phi, sm);
+}
+
+// A thread's share of a fixed-order sum of n partial sums: elements t, t + T, t + 2T, ... (T threads), eight loads in flight
+// at a time, added in index order.
+__device__ __forceinline__ double strided_sum(const double* __restrict__ v, int n) {
+    double acc = 0.0;
+    const int T = blockDim.x;
+    int i = threadIdx.x;
+    for (; i + 7 * T < n; i += 8 * T) {
+        double t[8];
+#pragma unroll
+        for (int u = 0; u < 8; ++u) t[u] = v[i + u * T];
+#pragma unroll
+        for (int u = 0; u < 8; ++u) acc += t[u];
+    }
+    for (; i < n; i += T) acc += v[i];
+    return acc;
 }
 
 // |g|^2 (partial sums of k_combine) and c (partial sums of F2) in fixed order, then the `while loop` of Fig. 3
@@ -42,22 +61,16 @@ __device__ __forceinline__ double cost_along(double b, long long n, const Item* 
 __global__ void __launch_bounds__(1024)
 k_select(DevState* st, const double* __restrict__ gpart, int n_gpart, const double* __restrict__ cpart, int n_part,
          const double* __restrict__ phipart, int n_phipart,
-         long long n, const Item* __restrict__ items, const StructInfo* __restrict__ tab, const double* __restrict__ d,
+         long long n, const int16_t* __restrict__ rseg, const StructInfo* __restrict__ tab, const double* __restrict__ d,
          const double* __restrict__ l, const double* __restrict__ Dg, const double* __restrict__ Lg) {
     pdl_wait();
     pdl_trigger();
     __shared__ double sm[32];
     __shared__ double s_b;
     __shared__ int s_go;
-    double a0 = 0.0;
-    for (int i = threadIdx.x; i < n_gpart; i += blockDim.x) a0 += gpart[i];
-    const double gg = block_sum(a0, sm);
-    double c = 0.0;
-    for (int i = threadIdx.x; i < n_part; i += blockDim.x) c += cpart[i];
-    const double cc = block_sum(c, sm);
-    double f0 = 0.0;
-    for (int i = threadIdx.x; i < n_phipart; i += blockDim.x) f0 += phipart[i];
-    const double phi_x = block_sum(f0, sm);                    // chi^2(x) (partial sums of the pass that wrote p, q)
+    const double gg = block_sum(strided_sum(gpart, n_gpart), sm);
+    const double cc = block_sum(strided_sum(cpart, n_part), sm);
+    const double phi_x = block_sum(strided_sum(phipart, n_phipart), sm);   // chi^2(x) (partial sums of the pass that wrote p, q)
     const int flags = st->flags;
     if (!(flags & SF_ONE_SIDED)) {
         if (threadIdx.x == 0) {
@@ -88,7 +101,7 @@ k_select(DevState* st, const double* __restrict__ gpart, int n_gpart, const doub
     if (threadIdx.x == 0) { s_go = gg > 0.0; st->gg = gg; st->c = cc; st->beta_acc = 0.0; }
     __syncthreads();
     if (!s_go) return;
-    const double phi0 = cost_along(0.0, n, items, tab, d, l, Dg, Lg, 1, sm);     // valid in thread 0
+    const double phi0 = cost_along(0.0, n, rseg, tab, d, l, Dg, Lg, 1, sm);     // valid in thread 0
     const long long mt = st->max_trials;
     for (long long t = 0; t < mt; ++t) {
         __syncthreads();
@@ -101,7 +114,7 @@ k_select(DevState* st, const double* __restrict__ gpart, int n_gpart, const doub
         const double b = s_b;
         double phi = 0.0;
         const int chk = st->accept_check;
-        if (chk) phi = cost_along(b, n, items, tab, d, l, Dg, Lg, 1, sm);
+        if (chk) phi = cost_along(b, n, rseg, tab, d, l, Dg, Lg, 1, sm);
         if (threadIdx.x == 0) {
             const int ok = !chk || phi < phi0;
             if (ok) { st->beta_acc = b; st->last_beta = (flags & SF_NORMALIZE_GRAD) ? b * sqrt(gg) : b; }
@@ -118,7 +131,7 @@ k_select(DevState* st, const double* __restrict__ gpart, int n_gpart, const doub
 // plus partial sums of the proximity, chi^2 and the violation count (fixed grid, fixed order); if not final
 // (another reduction of Fig. 3 follows), the cost residuals p, q at x'.
 __global__ void __launch_bounds__(ROW_THREADS)
-k_residual(long long n, const Item* __restrict__ items, const StructInfo* __restrict__ tab, DevState* st,
+k_residual(long long n, const int16_t* __restrict__ rseg, const StructInfo* __restrict__ tab, DevState* st,
            double* __restrict__ d, double* __restrict__ l, const double* __restrict__ Dg, const double* __restrict__ Lg,
            const double* __restrict__ nD, const double* __restrict__ nL, const double* __restrict__ nT,
            const GatherVec uv, const GatherVec pq, double* __restrict__ x, const double* __restrict__ g, long long S,
@@ -135,13 +148,15 @@ k_residual(long long n, const Item* __restrict__ items, const StructInfo* __rest
     double prox = 0.0, phi = 0.0;
     long long cnt = 0;
     for (long long a = tid; a < n; a += nth) {
+        const int sg = rseg[a];
+        if (sg < 0) continue;                                          // padding row of a ragged block: no sets, no cost term
         double dv = d[a], lv = l[a];
         if (beta != 0.0) {
             dv = fma(-beta, Dg[a], dv);
             lv = fma(-beta, Lg[a], lv);
             d[a] = dv; l[a] = lv;
         }
-        const StructInfo& T = tab[items[a].seg];
+        const StructInfo& T = tab[sg];
         const int f = T.flags;
         const double w = T.what;
         if (!final) {
@@ -269,7 +284,9 @@ k_finalize_stats(DevState* st, const double* __restrict__ part_prox, const doubl
     __shared__ long long smc[32];
     double p = 0.0, q = 0.0;
     long long c = 0;
-    for (int i = threadIdx.x; i < n_part; i += blockDim.x) { p += part_prox[i]; q += part_phi[i]; c += part_cnt[i]; }
+    p = strided_sum(part_prox, n_part);
+    q = strided_sum(part_phi, n_part);
+    for (int i = threadIdx.x; i < n_part; i += blockDim.x) c += part_cnt[i];
     const double P = block_sum(p, sm);
     const double Q = block_sum(q, sm);
     for (int o = 16; o > 0; o >>= 1) c += __shfl_down_sync(0xffffffffu, c, o);

@@ -91,19 +91,20 @@ static int resolve_x(fredopt_plan* P, const float* x, const double** xd) {
 }
 
 static int forward_f32(fredopt_plan* P, const RowSet& R, int m, const double* xd, float* d, float* l, int letd_out) {
-    // d, l: caller outputs (host or device), voxel-indexed, n_rows floats; rows outside R are 0
+    // d, l: caller outputs (host or device), voxel-indexed, n_rows floats; rows outside R are 0.  Host outputs are staged through a
+    // buffer the plan owns (allocated at the first such call, kept)
     float *dd = d, *dl = l;
-    void *fr_d = nullptr, *fr_l = nullptr;
-    const size_t nb = (size_t)(P->V ? P->V : 1) * 4;
-    if (d && !is_device_ptr(d)) { CK(cudaMalloc(&fr_d, nb)); dd = (float*)fr_d; }
-    if (l && !is_device_ptr(l)) { cudaError_t e = cudaMalloc(&fr_l, nb); if (e != cudaSuccess) { cudaFree(fr_d); CK(e); } dl = (float*)fr_l; }
+    const bool hd = d && !is_device_ptr(d), hl = l && !is_device_ptr(l);
+    if ((hd || hl) && !P->out_stage) CKR(dmalloc(P, &P->out_stage, 2 * (size_t)(P->V ? P->V : 1)));
+    if (hd) dd = P->out_stage;
+    if (hl) dl = P->out_stage + (P->V ? P->V : 1);
     if (dd) cudaMemsetAsync(dd, 0, (size_t)P->V * 4, P->stream);
     if (dl) cudaMemsetAsync(dl, 0, (size_t)P->V * 4, P->stream);
     if (R.n) {
         const uint8_t* md = P->mode_fixed + (size_t)m * P->max_seg;
         const GatherVec none{nullptr, nullptr, nullptr};
         const bool i16 = R.col16 != nullptr;
-        const void* colp = i16 ? (const void*)R.col16 : (const void*)R.col;
+        const void* colp = R.colp();
         long long n_long = R.n;
         if (&R == &P->full) {   // short rows by sub-warps (4 / 8 / 16 lanes per row), long rows by whole warps
             n_long = P->full_class[FIRST_SHORT_CLASS];
@@ -121,18 +122,13 @@ static int forward_f32(fredopt_plan* P, const RowSet& R, int m, const double* xd
             SHORT_LAUNCH(4, b[2], b[3])
 #undef SHORT_LAUNCH
         }
-        if (n_long) {
-            if (i16) k_forward<EPI_F32VOX, true><<<fwd_grid(P, n_long), FWD_THREADS, 0, P->stream>>>(n_long, R.items, R.vox, md, colp, R.valD, R.valL, xd, nullptr, nullptr, none, nullptr, nullptr, nullptr, dd, dl, letd_out, NO_RESID);
-            else k_forward<EPI_F32VOX, false><<<fwd_grid(P, n_long), FWD_THREADS, 0, P->stream>>>(n_long, R.items, R.vox, md, colp, R.valD, R.valL, xd, nullptr, nullptr, none, nullptr, nullptr, nullptr, dd, dl, letd_out, NO_RESID);
-            ++P->launches;
-        }
+        launch_fwd_kernel(P, EPI_F32VOX, R, 0, n_long, md, xd, nullptr, nullptr, none, nullptr, nullptr, dd, dl, letd_out, NO_RESID);
     }
     int rc = FREDOPT_OK;
     cudaError_t e = cudaGetLastError();
-    if (e == cudaSuccess && fr_d) e = cudaMemcpyAsync(d, dd, (size_t)P->V * 4, cudaMemcpyDeviceToHost, P->stream);
-    if (e == cudaSuccess && fr_l) e = cudaMemcpyAsync(l, dl, (size_t)P->V * 4, cudaMemcpyDeviceToHost, P->stream);
-    if (fr_d || fr_l) { cudaError_t e2 = cudaStreamSynchronize(P->stream); if (e == cudaSuccess) e = e2; }
-    cudaFree(fr_d); cudaFree(fr_l);
+    if (e == cudaSuccess && hd) e = cudaMemcpyAsync(d, dd, (size_t)P->V * 4, cudaMemcpyDeviceToHost, P->stream);
+    if (e == cudaSuccess && hl) e = cudaMemcpyAsync(l, dl, (size_t)P->V * 4, cudaMemcpyDeviceToHost, P->stream);
+    if (hd || hl) { cudaError_t e2 = cudaStreamSynchronize(P->stream); if (e == cudaSuccess) e = e2; }
     if (e != cudaSuccess) { g_last_cuda_error = cudaGetErrorString(e); cudaGetLastError(); rc = FREDOPT_CUDA_ERROR; }
     return rc;
 }
@@ -158,13 +154,13 @@ int fredopt_spmv_transpose(fredopt_plan* P, int32_t rows, const float* u, const 
     GatherVec vec = P->uv;
     if (rows == FREDOPT_ROWS_ALL) {
         if (!R.t_built) CKR(build_transpose(P, R));
-        if (!P->fullUV.pair) CKR(gv_alloc(P, &P->fullUV, (size_t)R.n));
+        if (!P->fullUV.pair) CKR(gv_alloc(P, &P->fullUV, (size_t)R.n_rows));
         vec = P->fullUV;
     }
     const float *du = nullptr, *dv = nullptr; void *fu = nullptr, *fv = nullptr;
     if (u) CKR(stage_in_f32(P, u, P->V, &du, &fu));
     if (v) { int rc = stage_in_f32(P, v, P->V, &dv, &fv); if (rc) { cudaFree(fu); return rc; } }
-    if (R.n) { k_gather_uv<<<grid_for(R.n, 256, 4096), 256, 0, P->stream>>>(du, dv, R.vox, vec, R.n); ++P->launches; }
+    if (R.n_rows) { k_gather_uv<<<grid_for(R.n_rows, 256, 4096), 256, 0, P->stream>>>(du, dv, R.vox, vec, R.n_rows); ++P->launches; }
     float* dout = out; void* fo = nullptr;
     if (!is_device_ptr(out)) { cudaError_t e = cudaMalloc(&fo, (P->S ? P->S : 1) * 4); if (e != cudaSuccess) { cudaFree(fu); cudaFree(fv); CK(e); } dout = (float*)fo; }
     const int m = (u ? 1 : 0) | (v ? 2 : 0);
@@ -184,7 +180,7 @@ int fredopt_proximity(fredopt_plan* P, const float* x, double* prox, int64_t* n_
     CKR(resolve_x(P, x, &xd));
     // scratch: Dg / Lg hold the products so that the iteration's d, l are left alone
     launch_forward(P, P->act, P->mode_con, xd, P->Dg, P->Lg, EPI_RESID, 0);     // a11: one pass, statistics only
-    launch_finalize(P, P->act.n ? fwd_grid(P, P->act.n) : 1);
+    launch_finalize(P, P->act.n ? (int)P->act.n : 1);
     DevState h;
     CK(cudaMemcpyAsync(&h, P->st, sizeof(DevState), cudaMemcpyDeviceToHost, P->stream));
     CK(cudaStreamSynchronize(P->stream));
@@ -199,8 +195,7 @@ static int structure_values(fredopt_plan* P, const float* x, int32_t quantity, i
     if (!P || quantity < 0 || quantity > 2 || label < 1 || label > P->n_struct) return FREDOPT_INVALID_ARG;
     const double* xd;
     CKR(resolve_x(P, x, &xd));
-    long long rb = 0;
-    for (int s = 0; s < label - 1; ++s) rb += (long long)P->h_tab[s].rows;
+    const long long rb = P->row_base[label - 1];                 // the structure's real rows; padding rows follow them
     const long long nr = (long long)P->h_tab[label - 1].rows;
     *rb_out = rb; *nr_out = nr;
     if (nr == 0) return FREDOPT_OK;
@@ -208,11 +203,10 @@ static int structure_values(fredopt_plan* P, const float* x, int32_t quantity, i
     const int m = quantity == 0 ? 1 : quantity == 1 ? 2 : 3;
     const uint8_t* md = P->mode_fixed + (size_t)m * P->max_seg;
     const GatherVec none{nullptr, nullptr, nullptr};
-    const int g = fwd_grid(P, nr);
-    if (A.col16) k_forward<EPI_STORE, true><<<g, FWD_THREADS, 0, P->stream>>>(nr, A.items + rb, A.vox + rb, md, A.col16, A.valD, A.valL, xd, P->Dg + rb, P->Lg + rb, none, nullptr, nullptr, nullptr, nullptr, nullptr, 0, NO_RESID);
-    else k_forward<EPI_STORE, false><<<g, FWD_THREADS, 0, P->stream>>>(nr, A.items + rb, A.vox + rb, md, A.col, A.valD, A.valL, xd, P->Dg + rb, P->Lg + rb, none, nullptr, nullptr, nullptr, nullptr, nullptr, 0, NO_RESID);
+    launch_fwd_kernel(P, EPI_STORE, A, rb / A.R, (nr + A.R - 1) / A.R, md, xd, P->Dg + rb, P->Lg + rb, none, nullptr, nullptr, nullptr, nullptr, 0,
+                      NO_RESID);
     k_quantity<<<grid_for(nr, 256, 1024), 256, 0, P->stream>>>(nr, quantity, P->Dg + rb, P->Lg + rb, P->uv.cD + rb);
-    P->launches += 2;
+    ++P->launches;
     CK(cudaGetLastError());
     return FREDOPT_OK;
 }

@@ -74,31 +74,20 @@ __global__ void k_union_fill(const long long* pD, const int32_t* cD, const float
     }
 }
 
-// per voxel: unpadded length, padded length (as int64 for the scan), flags
-__global__ void k_row_lengths(const long long* ptr, const int32_t* lab, long long V, long long* plen64, int32_t* nonempty,
-                              int32_t* active) {
+// per voxel: padded length of the row as a block row of its own (multiple of 4; int64 for the scan), flags
+__global__ void k_row_lengths(const long long* ptr, const int32_t* lab, long long V, int32_t* nonempty, int32_t* active) {
     for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < V; i += (long long)gridDim.x * blockDim.x) {
-        const long long n = ptr[i + 1] - ptr[i];
-        plen64[i] = (n + 3) & ~3LL;
-        nonempty[i] = n > 0;
+        nonempty[i] = ptr[i + 1] > ptr[i];
         active[i] = lab[i] != 0;
     }
 }
 
-// compact the flagged voxels (pos = exclusive scan of flag) into a row list
-__global__ void k_compact_rows(const int32_t* flag, const int32_t* pos, const long long* ptr, const long long* pstart,
-                               const int32_t* lab, long long V, int32_t* vox, long long* start, int32_t* len, int32_t* ulen,
-                               int32_t* key) {
+// compact the flagged voxels (pos = exclusive scan of flag) into a list; key = label (optional)
+__global__ void k_compact_rows(const int32_t* flag, const int32_t* pos, const int32_t* lab, long long V, int32_t* vox, int32_t* key) {
     for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < V; i += (long long)gridDim.x * blockDim.x) {
         if (!flag[i]) continue;
         const int o = pos[i];
         vox[o] = (int32_t)i;
-        if (start) {
-            const long long n = ptr[i + 1] - ptr[i];
-            start[o] = pstart[i];
-            len[o] = (int32_t)((n + 3) & ~3LL);
-            ulen[o] = (int32_t)n;
-        }
         if (key) key[o] = lab[i];
     }
 }
@@ -118,75 +107,155 @@ __global__ void k_class_keys(const int32_t* vox, const long long* ptr, long long
     }
 }
 
-// after sorting the active voxels by label: fill the list from the voxel ids
-__global__ void k_fill_active(const int32_t* vox, const int32_t* lab_sorted, const long long* ptr, const long long* pstart,
-                              long long n, long long* start, int32_t* len, int32_t* ulen, int32_t* seg) {
+// rows of a single-row (R = 1) set: entries = the row's non-zeros, padded to a multiple of 4
+__global__ void k_fill_rows1(const int32_t* vox, const long long* ptr, long long n, int32_t* len, int32_t* ulen, long long* len64) {
     for (long long a = (long long)blockIdx.x * blockDim.x + threadIdx.x; a < n; a += (long long)gridDim.x * blockDim.x) {
         const long long i = vox[a];
         const long long m = ptr[i + 1] - ptr[i];
-        start[a] = pstart[i];
         len[a] = (int32_t)((m + 3) & ~3LL);
         ulen[a] = (int32_t)m;
-        if (seg) seg[a] = lab_sorted[a] - 1;
+        len64[a] = (m + 3) & ~3LL;
     }
 }
 
-// Storage order inside a row (or a transposed run) of padded length Lp: every chunk of n <= 128 entries (n a
-// multiple of 4, q = n/4 lanes) is interleaved so that memory position 4t+k of the chunk holds the chunk's logical
-// entry t + q*k.  A lane's 128-bit load then yields entries t, t+q, t+2q, t+3q, and the k-th gather instruction of
-// the warp covers q CONSECUTIVE entries: few cache lines of the gathered vector per instruction.
-__device__ __forceinline__ long long perm_pos(long long e, long long Lp) {
-    const long long cb = e & ~127LL;
-    const long long rem = Lp - cb;
-    const int n = rem < 128 ? (int)rem : 128, q = n >> 2, r = (int)(e - cb);
-    return cb + 4 * (r % q) + r / q;
+// Storage order inside a block row (or a transposed run) of Le entries (a multiple of C): every chunk of n <= 32 C entries
+// (q = n / C lanes) is interleaved so that entry position C t + j of the chunk holds the chunk's logical entry t + q j.  A
+// lane's 128-bit value load then yields the values of entries t, t + q, ..., and the j-th gather instruction of the warp
+// covers q CONSECUTIVE entries: few cache lines of the gathered vector per instruction.  (C = 4: chunks of 128 entries.)
+__host__ __device__ __forceinline__ long long perm_pos(long long e, long long Le, int C) {
+    const int ce = 32 * C;
+    const long long cb = e / ce * ce;
+    const long long rem = Le - cb;
+    const int n = rem < ce ? (int)rem : ce, q = n / C, r = (int)(e - cb);
+    return cb + (long long)C * (r % q) + r / q;
 }
 
-// copy the rows into the padded arrays (warp per non-empty row); padding stays {col 0, value 0}
-__global__ void k_copy_padded(long long n, const int32_t* vox, const long long* start, const long long* ptr, const int32_t* cU,
-                              const float* uD, const float* uL, int32_t* col, float* vD, float* vL) {
+__device__ __forceinline__ void st_col(int32_t* c32, uint16_t* c16, long long i, int v) { if (c16) c16[i] = (uint16_t)v; else c32[i] = v; }
+__device__ __forceinline__ int ld_col(const int32_t* c32, const uint16_t* c16, long long i) { return c16 ? (int)c16[i] : c32[i]; }
+
+// R = 1: copy the rows into the padded arrays (warp per row); padding stays {col 0, value 0}
+__global__ void k_copy_rows1(long long n, const int32_t* vox, const long long* start, const long long* ptr, const int32_t* cU,
+                             const float* uD, const float* uL, int32_t* col, uint16_t* col16, float* vD, float* vL) {
     const int lane = threadIdx.x & 31;
     const long long w0 = ((long long)blockIdx.x * blockDim.x + threadIdx.x) >> 5, nw = ((long long)gridDim.x * blockDim.x) >> 5;
     for (long long r = w0; r < n; r += nw) {
         const long long i = vox[r], b = ptr[i], e = ptr[i + 1], o = start[r];
         const long long Lp = (e - b + 3) & ~3LL;
         for (long long p = b + lane; p < e; p += 32) {
-            const long long m = o + perm_pos(p - b, Lp);
-            col[m] = cU[p];
+            const long long m = o + perm_pos(p - b, Lp, 4);
+            st_col(col, col16, m, cU[p]);
             vD[m] = uD[p];
             vL[m] = uL[p];
         }
     }
 }
 
-// squared norms of D_i, L_i and L_i - LETmax D_i in fp64 (warp per active row)
-__global__ void k_norms(RowList rl, const int32_t* col, const float* vD, const float* vL, const StructInfo* tab, double* nD,
-                        double* nL, double* nT) {
+// ---- block rows of the labelled set
+// padded row index of the a-th labelled row (rows sorted by structure): a + shift[structure]; the other rows stay padding
+__global__ void k_place_rows(long long n_act, const int32_t* vox_s, const int32_t* lab_s, const long long* shift, const long long* ptr,
+                             int32_t* vox, int16_t* rseg, int32_t* rlen) {
+    for (long long a = (long long)blockIdx.x * blockDim.x + threadIdx.x; a < n_act; a += (long long)gridDim.x * blockDim.x) {
+        const int sg = lab_s[a] - 1;
+        const long long pa = a + shift[sg];
+        const long long i = vox_s[a];
+        vox[pa] = (int32_t)i;
+        rseg[pa] = (int16_t)sg;
+        rlen[pa] = (int32_t)(ptr[i + 1] - ptr[i]);
+    }
+}
+
+// Union of the column patterns of the R rows of every block row (thread per block row: an R-way merge of sorted rows).
+// COUNT: entries of the union.  FILL: the index and the R values per matrix of every entry (0 where a row has no entry).
+template <int R, bool FILL>
+__global__ void k_block_union(long long n_blk, const int32_t* __restrict__ vox, const long long* __restrict__ ptr,
+                              const int32_t* __restrict__ cU, const float* __restrict__ uD, const float* __restrict__ uL,
+                              long long* __restrict__ ecount,                                       // COUNT
+                              const long long* __restrict__ start, const int32_t* __restrict__ len,  // FILL
+                              int32_t* __restrict__ col, uint16_t* __restrict__ col16, float* __restrict__ vD, float* __restrict__ vL) {
+    constexpr int C = 4 / R;
+    for (long long b = (long long)blockIdx.x * blockDim.x + threadIdx.x; b < n_blk; b += (long long)gridDim.x * blockDim.x) {
+        long long p[R], pe[R];
+#pragma unroll
+        for (int k = 0; k < R; ++k) {
+            const int v = vox[b * R + k];
+            p[k] = v >= 0 ? ptr[v] : 0;
+            pe[k] = v >= 0 ? ptr[v + 1] : 0;
+        }
+        const long long o = FILL ? start[b] : 0;
+        const long long Le = FILL ? len[b] : 0;
+        long long e = 0;
+        while (true) {
+            int m = INT32_MAX;
+#pragma unroll
+            for (int k = 0; k < R; ++k) if (p[k] < pe[k]) { const int c = cU[p[k]]; m = c < m ? c : m; }
+            if (m == INT32_MAX) break;
+            if (FILL) {
+                const long long pos = o + perm_pos(e, Le, C);
+                st_col(col, col16, pos, m);
+#pragma unroll
+                for (int k = 0; k < R; ++k) {
+                    const bool has = p[k] < pe[k] && cU[p[k]] == m;
+                    vD[pos * R + k] = has ? uD[p[k]] : 0.f;
+                    vL[pos * R + k] = has ? uL[p[k]] : 0.f;
+                    if (has) ++p[k];
+                }
+            } else {
+#pragma unroll
+                for (int k = 0; k < R; ++k) if (p[k] < pe[k] && cU[p[k]] == m) ++p[k];
+            }
+            ++e;
+        }
+        if (!FILL) ecount[b] = e;
+    }
+}
+
+// per block row: structure, real rows, padded length
+__global__ void k_block_meta(long long n_blk, int R, const int16_t* rseg, const long long* ecount, int32_t* seg, int32_t* nreal,
+                             int32_t* ulen, int32_t* len, long long* len64) {
+    const int C = 4 / R;
+    for (long long b = (long long)blockIdx.x * blockDim.x + threadIdx.x; b < n_blk; b += (long long)gridDim.x * blockDim.x) {
+        int nr = 0;
+        for (int k = 0; k < R; ++k) nr += rseg[b * R + k] >= 0;
+        seg[b] = rseg[b * R];                      // row 0 of a block is always real
+        nreal[b] = nr;
+        const long long e = ecount[b], pl = (e + C - 1) / C * C;
+        ulen[b] = (int32_t)e;
+        len[b] = (int32_t)pl;
+        len64[b] = pl;
+    }
+}
+
+// squared norms of D_i, L_i and L_i - LETmax D_i in fp64 (warp per block row of the labelled set)
+__global__ void k_norms(long long n_blk, int R, const long long* start, const int32_t* len, const int32_t* seg, const float* vD,
+                        const float* vL, const StructInfo* tab, double* nD, double* nL, double* nT) {
     const int lane = threadIdx.x & 31;
     const long long w0 = ((long long)blockIdx.x * blockDim.x + threadIdx.x) >> 5, nw = ((long long)gridDim.x * blockDim.x) >> 5;
-    for (long long r = w0; r < rl.n; r += nw) {
-        const long long s = rl.start[r];
-        const int L = rl.len[r];
-        const StructInfo& T = tab[rl.seg[r]];
+    for (long long b = w0; b < n_blk; b += nw) {
+        const long long s = start[b];
+        const int L = len[b];
+        const StructInfo& T = tab[seg[b]];
         const double tm = (T.flags & F_LETD) ? T.letd_max : 0.0;
-        double a = 0.0, b = 0.0, c = 0.0;
-        for (int p = lane; p < L; p += 32) {
-            const double dv = (double)vD[s + p], lv = (double)vL[s + p];
-            a = fma(dv, dv, a);
-            b = fma(lv, lv, b);
-            const double t = lv - tm * dv;
-            c = fma(t, t, c);
+        for (int k = 0; k < R; ++k) {
+            double a = 0.0, bb = 0.0, c = 0.0;
+            for (int p = lane; p < L; p += 32) {
+                const double dv = (double)vD[(s + p) * R + k], lv = (double)vL[(s + p) * R + k];
+                a = fma(dv, dv, a);
+                bb = fma(lv, lv, bb);
+                const double t = lv - tm * dv;
+                c = fma(t, t, c);
+            }
+            a = warp_sum(a); bb = warp_sum(bb); c = warp_sum(c);
+            if (lane == 0) { nD[b * R + k] = a; nL[b * R + k] = bb; nT[b * R + k] = (T.flags & F_LETD) ? c : 0.0; }
         }
-        a = warp_sum(a); b = warp_sum(b); c = warp_sum(c);
-        if (lane == 0) { nD[r] = a; nL[r] = b; nT[r] = (T.flags & F_LETD) ? c : 0.0; }
     }
 }
 
 // integer bookkeeping per structure (atomics on integers: order-independent result)
-__global__ void k_count_sets(long long n, const int32_t* seg, const int32_t* ulen, const double* nD, const double* nL,
+__global__ void k_count_sets(long long n_rows, const int16_t* rseg, const int32_t* rlen, const double* nD, const double* nL,
                              const double* nT, StructInfo* tab) {
-    for (long long a = (long long)blockIdx.x * blockDim.x + threadIdx.x; a < n; a += (long long)gridDim.x * blockDim.x) {
-        StructInfo& T = tab[seg[a]];
+    for (long long a = (long long)blockIdx.x * blockDim.x + threadIdx.x; a < n_rows; a += (long long)gridDim.x * blockDim.x) {
+        if (rseg[a] < 0) continue;
+        StructInfo& T = tab[rseg[a]];
         const int f = T.flags;
         unsigned long long sets = 0, part = 0;
         if (f & F_DOSE_SLAB) { ++sets; part += nD[a] > 0.0; if (nD[a] > 0.0) atomicAdd(&T.part_kind[0], 1ULL); }
@@ -196,8 +265,16 @@ __global__ void k_count_sets(long long n, const int32_t* seg, const int32_t* ule
         atomicAdd(&T.part, part);
         atomicAdd(&T.n_zero, sets - part);
         atomicAdd(&T.rows, 1ULL);
-        atomicAdd(&T.nnz, (unsigned long long)ulen[a]);
+        atomicAdd(&T.nnz, (unsigned long long)rlen[a]);
     }
+}
+__global__ void k_count_entries(long long n_blk, const int32_t* seg, const int32_t* ulen, StructInfo* tab) {
+    for (long long b = (long long)blockIdx.x * blockDim.x + threadIdx.x; b < n_blk; b += (long long)gridDim.x * blockDim.x)
+        atomicAdd(&tab[seg[b]].entries, (unsigned long long)ulen[b]);
+}
+__global__ void k_label_hist(long long n, const int32_t* lab_s, unsigned long long* hist) {
+    for (long long a = (long long)blockIdx.x * blockDim.x + threadIdx.x; a < n; a += (long long)gridDim.x * blockDim.x)
+        atomicAdd(hist + (lab_s[a] - 1), 1ULL);
 }
 
 // W = sum_s w_s * part_s (s ascending), w^_s = w_s / W; pass modes and transposed-pass coefficients
@@ -223,62 +300,66 @@ __global__ void k_finish_tables(StructInfo* tab, int n_struct, DevState* st, uin
     st->W = W; st->n_sets = ns; st->n_zero = nz;
 }
 
-// ---- transposition of a row set
-// key of an entry = ((segment * S + spot) * H + block) with block = row index >> 16 (H = 1: no blocks)
-__global__ void k_tr_keys(RowList rl, const int32_t* ulen, const long long* off, const int32_t* col, long long S, int H,
-                          uint32_t* keys, uint32_t* vals) {
+// ---- transposition of a row set (entries = (block row, column) pairs with R values per matrix)
+// key of an entry = ((segment * S + spot) * H + group) with group = block row >> 16 (H = 1: no groups)
+__global__ void k_tr_keys(long long n, int C, const long long* start, const int32_t* len, const int32_t* ulen, const int32_t* seg,
+                          const long long* off, const int32_t* col, const uint16_t* col16, long long S, int H, uint32_t* keys,
+                          uint32_t* vals) {
     const int lane = threadIdx.x & 31;
     const long long w0 = ((long long)blockIdx.x * blockDim.x + threadIdx.x) >> 5, nw = ((long long)gridDim.x * blockDim.x) >> 5;
-    for (long long r = w0; r < rl.n; r += nw) {
-        const long long s = rl.start[r], o = off[r];
-        const int L = ulen[r];
-        const int sg = rl.seg ? rl.seg[r] : 0;
-        const int Lp = rl.len[r];
+    for (long long r = w0; r < n; r += nw) {
+        const long long s = start[r], o = off[r];
+        const int L = ulen[r], Lp = len[r];
+        const int sg = seg ? seg[r] : 0;
         for (int p = lane; p < L; p += 32) {
-            keys[o + p] = ((uint32_t)sg * (uint32_t)S + (uint32_t)col[s + perm_pos(p, Lp)]) * (uint32_t)H + (H > 1 ? (uint32_t)(r >> 16) : 0u);
+            keys[o + p] = ((uint32_t)sg * (uint32_t)S + (uint32_t)ld_col(col, col16, s + perm_pos(p, Lp, C))) * (uint32_t)H + (H > 1 ? (uint32_t)(r >> 16) : 0u);
             vals[o + p] = (uint32_t)(o + p);
         }
     }
 }
 // ustart[k] = first sorted position with key >= k, k = 0..K
-__global__ void k_tr_bounds(const uint32_t* keys, long long E, long long K, long long* ustart, long long* pcount) {
+__global__ void k_tr_bounds(const uint32_t* keys, long long E, long long K, long long* ustart) {
     for (long long k = (long long)blockIdx.x * blockDim.x + threadIdx.x; k <= K; k += (long long)gridDim.x * blockDim.x) {
         long long lo = 0, hi = E;
         while (lo < hi) { const long long mid = (lo + hi) >> 1; if ((long long)keys[mid] < k) lo = mid + 1; else hi = mid; }
         ustart[k] = lo;
     }
 }
-__global__ void k_tr_pcount(const long long* ustart, long long K, long long* pcount) {
+__global__ void k_tr_pcount(const long long* ustart, long long K, int C, long long* pcount) {
     for (long long k = (long long)blockIdx.x * blockDim.x + threadIdx.x; k < K; k += (long long)gridDim.x * blockDim.x)
-        pcount[k] = (ustart[k + 1] - ustart[k] + 3) & ~3LL;
+        pcount[k] = (ustart[k + 1] - ustart[k] + C - 1) / C * C;
 }
-__global__ void k_tr_fill(const uint32_t* keys, const uint32_t* vals, long long E, const long long* ustart, const long long* t_ptr,
+__global__ void k_tr_fill(const uint32_t* keys, const uint32_t* vals, long long E, int R, const long long* ustart, const long long* t_ptr,
                           const long long* off, long long n_rows, const long long* start, const int32_t* len, const float* vD,
                           const float* vL, int32_t* t_col, uint16_t* t_col16, float* tD, float* tL) {
+    const int C = 4 / R;
     for (long long r = (long long)blockIdx.x * blockDim.x + threadIdx.x; r < E; r += (long long)gridDim.x * blockDim.x) {
         const long long k = keys[r], e = vals[r];
-        // row a with off[a] <= e < off[a+1]
+        // block row a with off[a] <= e < off[a+1]
         long long lo = 0, hi = n_rows;
         while (lo < hi) { const long long mid = (lo + hi) >> 1; if (off[mid + 1] <= e) lo = mid + 1; else hi = mid; }
-        const long long a = lo, p = start[a] + perm_pos(e - off[a], len[a]);
-        const long long dst = t_ptr[k] + perm_pos(r - ustart[k], t_ptr[k + 1] - t_ptr[k]);
+        const long long a = lo, p = start[a] + perm_pos(e - off[a], len[a], C);
+        const long long dst = t_ptr[k] + perm_pos(r - ustart[k], t_ptr[k + 1] - t_ptr[k], C);
         if (t_col16) t_col16[dst] = (uint16_t)(a & 0xFFFF); else t_col[dst] = (int32_t)a;
-        tD[dst] = vD[p];
-        tL[dst] = vL[p];
+        for (int kk = 0; kk < R; ++kk) {
+            tD[dst * R + kk] = vD[p * R + kk];
+            tL[dst * R + kk] = vL[p * R + kk];
+        }
     }
 }
-// {start, len, seg} -> the 16-byte item the hot kernels read
-__global__ void k_pack_items(long long n, const long long* start, const int32_t* len, const int32_t* seg, Item* items) {
+// {start, len, seg, real rows} -> the 16-byte item the forward kernel reads (start / len in values per matrix)
+__global__ void k_pack_items(long long n, int R, const long long* start, const int32_t* len, const int32_t* seg, const int32_t* nreal,
+                             Item* items) {
     for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (long long)gridDim.x * blockDim.x) {
         Item it;
-        it.start = start[i]; it.len = len[i]; it.seg = seg ? seg[i] : 0;
+        it.start = start[i] * R; it.len = len[i] * R; it.seg = (seg ? seg[i] : 0) | ((nreal ? nreal[i] : 1) << 8);
         items[i] = it;
     }
 }
-// items per (spot, segment) run: ceil(padded length / TR_ITEM_MAX)
-__global__ void k_tr_item_count(const long long* t_ptr, long long K, long long* cnt) {
+// items per (spot, segment, group) run: ceil(values / TR_ITEM_MAX)
+__global__ void k_tr_item_count(const long long* t_ptr, long long K, int R, long long* cnt) {
     for (long long k = (long long)blockIdx.x * blockDim.x + threadIdx.x; k < K; k += (long long)gridDim.x * blockDim.x)
-        cnt[k] = (t_ptr[k + 1] - t_ptr[k] + TR_ITEM_MAX - 1) / TR_ITEM_MAX;
+        cnt[k] = ((t_ptr[k + 1] - t_ptr[k]) * R + TR_ITEM_MAX - 1) / TR_ITEM_MAX;
 }
 // the same counts in spot-major order (the order of a spot's partial-sum slots)
 __global__ void k_tr_item_count_sm(const long long* cnt, long long S, int n_seg, int H, long long* cnt_sm) {
@@ -287,11 +368,11 @@ __global__ void k_tr_item_count_sm(const long long* cnt, long long S, int n_seg,
         cnt_sm[(j * n_seg + sg) * H + hi] = cnt[k];
     }
 }
-// item.seg = segment | (block << 8): the kernel adds block << 16 to the 16-bit row indices
-__global__ void k_tr_item_fill(const long long* t_ptr, const long long* ibase, const long long* sbase, long long S, int n_seg, int H,
+// item.seg = segment | (group << 8): the kernel adds group << 16 to the 16-bit block-row indices
+__global__ void k_tr_item_fill(const long long* t_ptr, const long long* ibase, const long long* sbase, long long S, int n_seg, int H, int R,
                                Item* items, int32_t* item_slot) {
     for (long long k = (long long)blockIdx.x * blockDim.x + threadIdx.x; k < S * n_seg * H; k += (long long)gridDim.x * blockDim.x) {
-        const long long b = t_ptr[k], e = t_ptr[k + 1];
+        const long long b = t_ptr[k] * R, e = t_ptr[k + 1] * R;          // in values per matrix
         const long long hi = k % H, js = k / H, j = js % S, sg0 = js / S;
         const long long sg = sg0 | (hi << 8);
         long long i = ibase[k], slot = sbase[(j * n_seg + sg0) * H + hi];
@@ -303,7 +384,7 @@ __global__ void k_tr_item_fill(const long long* t_ptr, const long long* ibase, c
         }
     }
 }
-// longest-first execution order: key = length class (256-entry bins, longest = 0); a stable sort keeps the
+// longest-first execution order: key = length class (256-value bins, longest = 0); a stable sort keeps the
 // (structure, spot) order inside a class
 __global__ void k_tr_item_key(const Item* items, long long n, uint32_t* key, uint32_t* idx) {
     for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (long long)gridDim.x * blockDim.x) {
@@ -329,9 +410,18 @@ __global__ void k_tr_item_ptr(const long long* sbase, long long S, long long run
     for (long long j = (long long)blockIdx.x * blockDim.x + threadIdx.x; j <= S; j += (long long)gridDim.x * blockDim.x)
         item_ptr[j] = sbase[j * runs_per_spot];
 }
-__global__ void k_narrow_u16(const int32_t* in, uint16_t* out, long long n) {
-    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (long long)gridDim.x * blockDim.x)
-        out[i] = (uint16_t)in[i];
+// execution order of the forward items: longest first (stable: list order among equal lengths)
+__global__ void k_item_len_key(const Item* items, long long n, uint32_t* key, uint32_t* idx) {
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (long long)gridDim.x * blockDim.x) {
+        key[i] = 0xFFFFFFFFu - (uint32_t)items[i].len;
+        idx[i] = (uint32_t)i;
+    }
+}
+__global__ void k_item_gather(const uint32_t* idx, long long n, const Item* items, Item* items_x, int32_t* item_blk) {
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (long long)gridDim.x * blockDim.x) {
+        items_x[i] = items[idx[i]];
+        item_blk[i] = (int32_t)idx[i];
+    }
 }
 __global__ void k_i32_to_i64(const int32_t* in, long long* out, long long n) {
     for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (long long)gridDim.x * blockDim.x) out[i] = in[i];
@@ -354,185 +444,175 @@ static int scan_exclusive(fredopt_plan* P, const T* in, T* out, long long n) {
     return FREDOPT_OK;
 }
 
+// temporaries of a create-time routine: freed when the routine returns, whatever the path
+struct TmpPool {
+    std::vector<void*> v;
+    ~TmpPool() { for (void* p : v) cudaFree(p); }
+    template <class T>
+    int get(T** p, size_t n) {
+        *p = nullptr;
+        CK(cudaMalloc((void**)p, (n ? n : 1) * sizeof(T)));
+        v.push_back((void*)*p);
+        return FREDOPT_OK;
+    }
+};
+
 int build_transpose(fredopt_plan* P, RowSet& R) {
     cudaStream_t st = P->stream;
     const long long n = R.n, S = P->S;
-    // 16-bit row indices: cut every (segment, spot) run where the row index crosses a multiple of 65536
+    const int RB = R.R, C = 4 / RB;
+    TmpPool T;
+    // 16-bit block-row indices: cut every (segment, spot) run where the index crosses a multiple of 65536
     int H = (int)((n + 65535) >> 16);
     if (H < 1) H = 1;
-    bool idx16 = R.n_seg < 256 && H < (1 << 23) && (double)S * R.n_seg * H < 4.0e9 && !P->force_idx32;
+    const bool idx16 = R.n_seg < 256 && H < (1 << 23) && (double)S * R.n_seg * H < 4.0e9 && !P->force_idx32;
     if (!idx16) H = 1;
     R.t_H = H;
     const long long K = S * R.n_seg * H;
-    // unpadded offsets
+    // offsets of the block rows in the enumeration of the (unpadded) entries
     long long *len64 = nullptr, *off = nullptr;
-    CK(cudaMalloc(&len64, (n + 1) * sizeof(long long)));
-    CK(cudaMalloc(&off, (n + 2) * sizeof(long long)));
+    CKR(T.get(&len64, (size_t)n + 1)); CKR(T.get(&off, (size_t)n + 2));
     CK(cudaMemsetAsync(len64, 0, (n + 1) * sizeof(long long), st));
     if (n) k_i32_to_i64<<<grid_for(n, 256, 4096), 256, 0, st>>>(R.ulen, len64, n);
-    int rc = scan_exclusive(P, len64, off, n + 1);
-    cudaFree(len64);
-    if (rc) { cudaFree(off); return rc; }
+    CKR(scan_exclusive(P, len64, off, n + 1));
     long long E = 0;
     CK(cudaMemcpyAsync(&E, off + n, sizeof(long long), cudaMemcpyDeviceToHost, st));
     CK(cudaStreamSynchronize(st));
-    R.nnz = E;
-    if (E >= (1LL << 32) || K >= (1LL << 32)) { cudaFree(off); return FREDOPT_INVALID_ARG; }
+    R.entries = E;
+    if (E >= (1LL << 32) || K >= (1LL << 32)) return FREDOPT_INVALID_ARG;
     uint32_t *keys = nullptr, *vals = nullptr, *keys2 = nullptr, *vals2 = nullptr;
     long long *ustart = nullptr, *pcount = nullptr;
-    void* tmp = nullptr;
-    int ret = FREDOPT_OK;
-    auto cleanup = [&]() {
-        cudaFree(keys); cudaFree(vals); cudaFree(keys2); cudaFree(vals2); cudaFree(ustart); cudaFree(pcount); cudaFree(tmp); cudaFree(off);
-    };
-#define CKC(expr)                                                                                   \
-    do {                                                                                            \
-        cudaError_t e__ = (expr);                                                                   \
-        if (e__ != cudaSuccess) {                                                                   \
-            g_last_cuda_error = std::string(#expr) + ": " + cudaGetErrorString(e__);                \
-            cudaGetLastError();                                                                     \
-            cleanup();                                                                              \
-            return e__ == cudaErrorMemoryAllocation ? FREDOPT_OUT_OF_MEMORY : FREDOPT_CUDA_ERROR;   \
-        }                                                                                           \
-    } while (0)
     const size_t En = E ? (size_t)E : 1;
-    CKC(cudaMalloc(&keys, En * 4)); CKC(cudaMalloc(&vals, En * 4));
-    CKC(cudaMalloc(&keys2, En * 4)); CKC(cudaMalloc(&vals2, En * 4));
-    CKC(cudaMalloc(&ustart, (K + 2) * sizeof(long long))); CKC(cudaMalloc(&pcount, (K + 2) * sizeof(long long)));
-    if (n) k_tr_keys<<<grid_for(n * 32, 256, 1 << 16), 256, 0, st>>>(R.view(), R.ulen, off, R.col, S, H, keys, vals);
+    CKR(T.get(&keys, En)); CKR(T.get(&vals, En)); CKR(T.get(&keys2, En)); CKR(T.get(&vals2, En));
+    CKR(T.get(&ustart, (size_t)K + 2)); CKR(T.get(&pcount, (size_t)K + 2));
+    if (n) k_tr_keys<<<grid_for(n * 32, 256, 1 << 16), 256, 0, st>>>(n, C, R.start, R.len, R.ulen, R.seg, off, R.col, R.col16, S, H, keys, vals);
     int bits = 1;
     while ((1LL << bits) < K) ++bits;
-    size_t tb = 0;
-    CKC(cub::DeviceRadixSort::SortPairs(nullptr, tb, keys, keys2, vals, vals2, E, 0, bits, st));
-    CKC(cudaMalloc(&tmp, tb ? tb : 1));
-    CKC(cub::DeviceRadixSort::SortPairs(tmp, tb, keys, keys2, vals, vals2, E, 0, bits, st));   // stable: list order kept inside a key
-    k_tr_bounds<<<grid_for(K + 1, 256, 4096), 256, 0, st>>>(keys2, E, K, ustart, pcount);
-    CKC(cudaMemsetAsync(pcount, 0, (K + 2) * sizeof(long long), st));
-    k_tr_pcount<<<grid_for(K, 256, 4096), 256, 0, st>>>(ustart, K, pcount);
-    CKC(cudaGetLastError());
-    ret = dmalloc(P, &R.t_ptr, (size_t)K + 2);
-    if (ret) { cleanup(); return ret; }
-    ret = scan_exclusive(P, pcount, R.t_ptr, K + 1);
-    if (ret) { cleanup(); return ret; }
-    CKC(cudaMemcpyAsync(&R.t_nnz_padded, R.t_ptr + K, sizeof(long long), cudaMemcpyDeviceToHost, st));
-    CKC(cudaStreamSynchronize(st));
-    const size_t Tn = R.t_nnz_padded ? (size_t)R.t_nnz_padded : 4;
-    if ((ret = idx16 ? dmalloc(P, &R.t_col16, Tn) : dmalloc(P, &R.t_col, Tn)) || (ret = dmalloc(P, &R.t_valD, Tn)) ||
-        (ret = dmalloc(P, &R.t_valL, Tn))) { cleanup(); return ret; }
-    if (idx16) CKC(cudaMemsetAsync(R.t_col16, 0, Tn * 2, st)); else
-    CKC(cudaMemsetAsync(R.t_col, 0, Tn * 4, st));
-    CKC(cudaMemsetAsync(R.t_valD, 0, Tn * 4, st));
-    CKC(cudaMemsetAsync(R.t_valL, 0, Tn * 4, st));
-    if (E) k_tr_fill<<<grid_for(E, 256, 1 << 16), 256, 0, st>>>(keys2, vals2, E, ustart, R.t_ptr, off, n, R.start, R.len, R.valD, R.valL,
+    {
+        size_t tb = 0;
+        void* tmp = nullptr;
+        CK(cub::DeviceRadixSort::SortPairs(nullptr, tb, keys, keys2, vals, vals2, E, 0, bits, st));
+        CKR(T.get((char**)&tmp, tb));
+        CK(cub::DeviceRadixSort::SortPairs(tmp, tb, keys, keys2, vals, vals2, E, 0, bits, st));   // stable: list order kept inside a key
+    }
+    k_tr_bounds<<<grid_for(K + 1, 256, 4096), 256, 0, st>>>(keys2, E, K, ustart);
+    CK(cudaMemsetAsync(pcount, 0, (K + 2) * sizeof(long long), st));
+    k_tr_pcount<<<grid_for(K, 256, 4096), 256, 0, st>>>(ustart, K, C, pcount);
+    CK(cudaGetLastError());
+    CKR(dmalloc(P, &R.t_ptr, (size_t)K + 2));
+    CKR(scan_exclusive(P, pcount, R.t_ptr, K + 1));
+    CK(cudaMemcpyAsync(&R.t_entries_padded, R.t_ptr + K, sizeof(long long), cudaMemcpyDeviceToHost, st));
+    CK(cudaStreamSynchronize(st));
+    const size_t Tn = R.t_entries_padded ? (size_t)R.t_entries_padded : 4;
+    if (idx16) CKR(dmalloc(P, &R.t_col16, Tn)); else CKR(dmalloc(P, &R.t_col, Tn));
+    CKR(dmalloc(P, &R.t_valD, Tn * RB)); CKR(dmalloc(P, &R.t_valL, Tn * RB));
+    if (idx16) CK(cudaMemsetAsync(R.t_col16, 0, Tn * 2, st)); else CK(cudaMemsetAsync(R.t_col, 0, Tn * 4, st));
+    CK(cudaMemsetAsync(R.t_valD, 0, Tn * RB * 4, st));
+    CK(cudaMemsetAsync(R.t_valL, 0, Tn * RB * 4, st));
+    if (E) k_tr_fill<<<grid_for(E, 256, 1 << 16), 256, 0, st>>>(keys2, vals2, E, RB, ustart, R.t_ptr, off, n, R.start, R.len, R.valD, R.valL,
                                                              R.t_col, R.t_col16, R.t_valD, R.t_valL);
-    CKC(cudaGetLastError());
-    // ---- work items: every (segment, spot) run cut into pieces of at most TR_ITEM_MAX entries, in run order
+    CK(cudaGetLastError());
+    // ---- work items: every (segment, spot, group) run cut into pieces of at most TR_ITEM_MAX values, in run order
     //      (neighbouring items = neighbouring spots of one structure: overlapping voxel footprints share L1 lines)
-    CKC(cudaMemsetAsync(pcount, 0, (K + 2) * sizeof(long long), st));
-    k_tr_item_count<<<grid_for(K, 256, 4096), 256, 0, st>>>(R.t_ptr, K, pcount);
-    long long *cnt_sm = nullptr, *sbase = nullptr;
-    CKC(cudaMalloc(&cnt_sm, (K + 2) * sizeof(long long)));
-    { cudaError_t e_ = cudaMalloc(&sbase, (K + 2) * sizeof(long long)); if (e_ != cudaSuccess) { cudaFree(cnt_sm); CKC(e_); } }
-    auto cleanup2 = [&]() { cudaFree(cnt_sm); cudaFree(sbase); cleanup(); };
-    cudaMemsetAsync(cnt_sm, 0, (K + 2) * sizeof(long long), st);
+    CK(cudaMemsetAsync(pcount, 0, (K + 2) * sizeof(long long), st));
+    k_tr_item_count<<<grid_for(K, 256, 4096), 256, 0, st>>>(R.t_ptr, K, RB, pcount);
+    long long* cnt_sm = nullptr;
+    CKR(T.get(&cnt_sm, (size_t)K + 2));
+    CKR(dmalloc(P, &R.t_slot_ptr, (size_t)K + 2));       // kept: slot ranges per (spot, structure, group) for the block-sequential sweep
+    long long* sbase = R.t_slot_ptr;
+    CK(cudaMemsetAsync(cnt_sm, 0, (K + 2) * sizeof(long long), st));
     k_tr_item_count_sm<<<grid_for(K, 256, 4096), 256, 0, st>>>(pcount, S, R.n_seg, H, cnt_sm);
-    ret = scan_exclusive(P, pcount, ustart, K + 1);      // ustart now = first item of each run (execution order)
-    if (!ret) ret = scan_exclusive(P, cnt_sm, sbase, K + 1);   // first partial-sum slot of each (spot, segment)
-    if (ret) { cleanup2(); return ret; }
-    if (cudaMemcpyAsync(&R.t_n_items, ustart + K, sizeof(long long), cudaMemcpyDeviceToHost, st) != cudaSuccess ||
-        cudaStreamSynchronize(st) != cudaSuccess) { cleanup2(); return FREDOPT_CUDA_ERROR; }
-    if ((ret = dmalloc(P, &R.t_items, (size_t)R.t_n_items)) || (ret = dmalloc(P, &R.t_item_slot, (size_t)R.t_n_items)) ||
-        (ret = dmalloc(P, &R.t_item_ptr, (size_t)S + 1)) || (ret = dmalloc(P, &R.t_partial, (size_t)R.t_n_items))) { cleanup2(); return ret; }
-    k_tr_item_fill<<<grid_for(K, 256, 4096), 256, 0, st>>>(R.t_ptr, ustart, sbase, S, R.n_seg, H, R.t_items, R.t_item_slot);
+    CKR(scan_exclusive(P, pcount, ustart, K + 1));       // ustart now = first item of each run (execution order)
+    CKR(scan_exclusive(P, cnt_sm, sbase, K + 1));        // first partial-sum slot of each (spot, segment, group)
+    CK(cudaMemcpyAsync(&R.t_n_items, ustart + K, sizeof(long long), cudaMemcpyDeviceToHost, st));
+    CK(cudaStreamSynchronize(st));
+    CKR(dmalloc(P, &R.t_items, (size_t)R.t_n_items)); CKR(dmalloc(P, &R.t_item_slot, (size_t)R.t_n_items));
+    CKR(dmalloc(P, &R.t_item_ptr, (size_t)S + 1)); CKR(dmalloc(P, &R.t_partial, (size_t)R.t_n_items));
+    k_tr_item_fill<<<grid_for(K, 256, 4096), 256, 0, st>>>(R.t_ptr, ustart, sbase, S, R.n_seg, H, RB, R.t_items, R.t_item_slot);
     k_tr_item_ptr<<<grid_for(S + 1, 256, 4096), 256, 0, st>>>(sbase, S, (long long)R.n_seg * H, R.t_item_ptr);
-    if (cudaGetLastError() != cudaSuccess || cudaStreamSynchronize(st) != cudaSuccess) { cleanup2(); return FREDOPT_CUDA_ERROR; }
-    cudaFree(cnt_sm);
-    R.t_slot_ptr = sbase;              // kept: slot ranges per (spot, structure, block) for the block-sequential sweep
-    P->allocs.push_back((void*)sbase);
+    CK(cudaGetLastError());
+    CK(cudaStreamSynchronize(st));
     // ---- the same items grouped by structure, longest first inside a structure (block-sequential AMS)
     R.t_seg_item_begin.assign((size_t)R.n_seg + 1, 0);
     if (R.t_n_items > 0) {
         const long long ni = R.t_n_items;
         uint32_t *ik = nullptr, *ik2 = nullptr, *ii = nullptr, *ii2 = nullptr;
-        unsigned long long* hist = nullptr; void* stmp = nullptr;
-        auto cleanup4 = [&]() { cudaFree(ik); cudaFree(ik2); cudaFree(ii); cudaFree(ii2); cudaFree(hist); cudaFree(stmp); cleanup(); };
-#define CK4(expr) do { cudaError_t e__ = (expr); if (e__ != cudaSuccess) { g_last_cuda_error = std::string(#expr) + ": " + cudaGetErrorString(e__); cudaGetLastError(); cleanup4(); return e__ == cudaErrorMemoryAllocation ? FREDOPT_OUT_OF_MEMORY : FREDOPT_CUDA_ERROR; } } while (0)
-        CK4(cudaMalloc(&ik, ni * 4)); CK4(cudaMalloc(&ik2, ni * 4)); CK4(cudaMalloc(&ii, ni * 4)); CK4(cudaMalloc(&ii2, ni * 4));
-        CK4(cudaMalloc(&hist, 256 * 8));
-        CK4(cudaMemsetAsync(hist, 0, 256 * 8, st));
-        if ((ret = dmalloc(P, &R.t_items_seg, (size_t)ni)) || (ret = dmalloc(P, &R.t_slot_seg, (size_t)ni))) { cleanup4(); return ret; }
+        unsigned long long* hist = nullptr;
+        CKR(T.get(&ik, (size_t)ni)); CKR(T.get(&ik2, (size_t)ni)); CKR(T.get(&ii, (size_t)ni)); CKR(T.get(&ii2, (size_t)ni));
+        CKR(T.get(&hist, 256));
+        CK(cudaMemsetAsync(hist, 0, 256 * 8, st));
+        CKR(dmalloc(P, &R.t_items_seg, (size_t)ni)); CKR(dmalloc(P, &R.t_slot_seg, (size_t)ni));
         k_tr_item_key_seg<<<grid_for(ni, 256, 4096), 256, 0, st>>>(R.t_items, ni, ik, ii, hist);
         size_t sb = 0;
-        CK4(cub::DeviceRadixSort::SortPairs(nullptr, sb, ik, ik2, ii, ii2, ni, 0, 12, st));
-        CK4(cudaMalloc(&stmp, sb ? sb : 1));
-        CK4(cub::DeviceRadixSort::SortPairs(stmp, sb, ik, ik2, ii, ii2, ni, 0, 12, st));
+        void* stmp = nullptr;
+        CK(cub::DeviceRadixSort::SortPairs(nullptr, sb, ik, ik2, ii, ii2, ni, 0, 12, st));
+        CKR(T.get((char**)&stmp, sb));
+        CK(cub::DeviceRadixSort::SortPairs(stmp, sb, ik, ik2, ii, ii2, ni, 0, 12, st));
         k_tr_item_permute<<<grid_for(ni, 256, 4096), 256, 0, st>>>(ii2, ni, R.t_items, R.t_item_slot, R.t_items_seg, R.t_slot_seg);
         unsigned long long hh[256];
-        CK4(cudaMemcpyAsync(hh, hist, 256 * 8, cudaMemcpyDeviceToHost, st));
-        CK4(cudaStreamSynchronize(st));
-#undef CK4
+        CK(cudaMemcpyAsync(hh, hist, 256 * 8, cudaMemcpyDeviceToHost, st));
+        CK(cudaStreamSynchronize(st));
         for (int sg = 0; sg < R.n_seg; ++sg) R.t_seg_item_begin[sg + 1] = R.t_seg_item_begin[sg] + (long long)hh[sg];
-        cudaFree(ik); cudaFree(ik2); cudaFree(ii); cudaFree(ii2); cudaFree(hist); cudaFree(stmp);
+    }
+    // ---- the items in run order (= storage order) are kept beside the longest-first list
+    if (R.t_n_items > 0) {
+        CKR(dmalloc(P, &R.t_items_run, (size_t)R.t_n_items)); CKR(dmalloc(P, &R.t_slot_run, (size_t)R.t_n_items));
+        CK(cudaMemcpyAsync(R.t_items_run, R.t_items, R.t_n_items * sizeof(Item), cudaMemcpyDeviceToDevice, st));
+        CK(cudaMemcpyAsync(R.t_slot_run, R.t_item_slot, R.t_n_items * sizeof(int32_t), cudaMemcpyDeviceToDevice, st));
     }
     // ---- longest items first: with the static round-robin mapping every round of the grid then holds items of
     //      one length class, so the warps stay balanced to within one class width per round
     if (R.t_n_items > 1) {
         const long long ni = R.t_n_items;
         uint32_t *ik = nullptr, *ik2 = nullptr, *ii = nullptr, *ii2 = nullptr;
-        Item* it2 = nullptr; int32_t* js2 = nullptr; void* stmp = nullptr;
-        auto cleanup3 = [&]() { cudaFree(ik); cudaFree(ik2); cudaFree(ii); cudaFree(ii2); cudaFree(it2); cudaFree(js2); cudaFree(stmp); cleanup(); };
-#define CK3(expr) do { cudaError_t e__ = (expr); if (e__ != cudaSuccess) { g_last_cuda_error = std::string(#expr) + ": " + cudaGetErrorString(e__); cudaGetLastError(); cleanup3(); return e__ == cudaErrorMemoryAllocation ? FREDOPT_OUT_OF_MEMORY : FREDOPT_CUDA_ERROR; } } while (0)
-        CK3(cudaMalloc(&ik, ni * 4)); CK3(cudaMalloc(&ik2, ni * 4)); CK3(cudaMalloc(&ii, ni * 4)); CK3(cudaMalloc(&ii2, ni * 4));
-        CK3(cudaMalloc(&it2, ni * sizeof(Item))); CK3(cudaMalloc(&js2, ni * sizeof(int32_t)));
+        Item* it2 = nullptr; int32_t* js2 = nullptr;
+        CKR(T.get(&ik, (size_t)ni)); CKR(T.get(&ik2, (size_t)ni)); CKR(T.get(&ii, (size_t)ni)); CKR(T.get(&ii2, (size_t)ni));
+        CKR(T.get(&it2, (size_t)ni)); CKR(T.get(&js2, (size_t)ni));
         k_tr_item_key<<<grid_for(ni, 256, 4096), 256, 0, st>>>(R.t_items, ni, ik, ii);
         size_t sb = 0;
-        CK3(cub::DeviceRadixSort::SortPairs(nullptr, sb, ik, ik2, ii, ii2, ni, 0, 4, st));
-        CK3(cudaMalloc(&stmp, sb ? sb : 1));
-        CK3(cub::DeviceRadixSort::SortPairs(stmp, sb, ik, ik2, ii, ii2, ni, 0, 4, st));
+        void* stmp = nullptr;
+        CK(cub::DeviceRadixSort::SortPairs(nullptr, sb, ik, ik2, ii, ii2, ni, 0, 4, st));
+        CKR(T.get((char**)&stmp, sb));
+        CK(cub::DeviceRadixSort::SortPairs(stmp, sb, ik, ik2, ii, ii2, ni, 0, 4, st));
         k_tr_item_permute<<<grid_for(ni, 256, 4096), 256, 0, st>>>(ii2, ni, R.t_items, R.t_item_slot, it2, js2);
-        CK3(cudaMemcpyAsync(R.t_items, it2, ni * sizeof(Item), cudaMemcpyDeviceToDevice, st));
-        CK3(cudaMemcpyAsync(R.t_item_slot, js2, ni * sizeof(int32_t), cudaMemcpyDeviceToDevice, st));
-        CK3(cudaStreamSynchronize(st));
-#undef CK3
-        cudaFree(ik); cudaFree(ik2); cudaFree(ii); cudaFree(ii2); cudaFree(it2); cudaFree(js2); cudaFree(stmp);
+        CK(cudaMemcpyAsync(R.t_items, it2, ni * sizeof(Item), cudaMemcpyDeviceToDevice, st));
+        CK(cudaMemcpyAsync(R.t_item_slot, js2, ni * sizeof(int32_t), cudaMemcpyDeviceToDevice, st));
+        CK(cudaStreamSynchronize(st));
     }
-    CKC(cudaGetLastError());
-    CKC(cudaStreamSynchronize(st));
-    cleanup();
-#undef CKC
+    CK(cudaGetLastError());
+    CK(cudaStreamSynchronize(st));
     R.t_built = true;
     return FREDOPT_OK;
 }
 
-// bytes the method must move in one launch of a pass: per non-zero 4 B index + 4 B per value array
-// the row needs; 8 B per row offset; fp64 vectors read / written once.
+// Bytes the method must move in one launch of a pass: per non-zero of a row 4 B for every value array the
+// row's structure needs in that pass; per stored entry (one per block row and column of the union pattern) the stored index
+// (2 B, or 4 B in the 32-bit form); 8 B per row offset; the fp64 vectors read / written once.  The zeros a block row stores
+// where one of its rows has no entry are NOT counted (they show up as DRAM traffic above this figure).
 static void compute_pass_bytes(fredopt_plan* P) {
-    long long fwd_union = 0, fwd_con = 0, tr_cost = 0, tr_con = 0, rows_union = 0, rows_con = 0, rows_cost = 0;
+    long long fwd_union = 0, tr_cost = 0, tr_con = 0, rows_union = 0, rows_con = 0, rows_cost = 0;
+    const int ibf = P->act.col16 ? 2 : 4, ibt = P->act.t_col16 ? 2 : 4;     // index bytes as stored
     for (int s = 0; s < P->n_struct; ++s) {
         const StructInfo& T = P->h_tab[s];
         const int f = T.flags;
         const int cost = ((f & F_DOSE_REF) ? 1 : 0) | ((f & F_DL_REF) ? 2 : 0);
         const int con = ((f & (F_DOSE_SLAB | F_LETD)) ? 1 : 0) | ((f & (F_DL_SLAB | F_LETD)) ? 2 : 0);
-        auto per = [](int m, int ib) { return m ? ib + 4 * ((m & 1) + ((m >> 1) & 1)) : 0; };
-        const int ibf = P->act.col16 ? 2 : 4, ibt = P->act.t_col16 ? 2 : 4;     // index bytes as stored
-        fwd_union += (long long)T.nnz * per(cost | con, ibf);
-        fwd_con += (long long)T.nnz * per(con, ibf);
-        tr_cost += (long long)T.nnz * per(cost, ibt);
-        tr_con += (long long)T.nnz * per(con, ibt);
+        auto per = [&](int m, int ib) { return m ? (long long)T.entries * ib + (long long)T.nnz * 4 * ((m & 1) + ((m >> 1) & 1)) : 0LL; };
+        fwd_union += per(cost | con, ibf);
+        tr_cost += per(cost, ibt);
+        tr_con += per(con, ibt);
         if (cost | con) rows_union += T.rows;
         if (con) rows_con += T.rows;
         if (cost) rows_cost += T.rows;
     }
-    const long long S = P->S, VA = P->act.n;
+    const long long S = P->S, VA = P->act.n_true;
     P->pass_bytes[FREDOPT_PASS_FORWARD_X] = fwd_union + rows_union * (8 + 16) + S * 8;
     P->pass_bytes[FREDOPT_PASS_FORWARD_G] = fwd_union + rows_union * (8 + 16) + S * 8;
     P->pass_bytes[FREDOPT_PASS_TRANSPOSE_G] = tr_cost + S * P->act.n_seg * 8 + rows_cost * 16 + S * 8;
     P->pass_bytes[FREDOPT_PASS_TRANSPOSE_B] = tr_con + S * P->act.n_seg * 8 + rows_con * 16 + S * 16;
     P->pass_bytes[FREDOPT_PASS_SELECT] = S * 24;
     P->pass_bytes[FREDOPT_PASS_RESIDUAL] = VA * (4 + 8 * 9);
-    (void)fwd_con;
 }
-
 
 // ============================================================================================ API
 extern "C" {
@@ -545,6 +625,28 @@ void fredopt_destroy(fredopt_plan* P) {
     for (void* p : P->allocs) cudaFree(p);
     if (P->owns_stream) cudaStreamDestroy(P->stream);
     delete P;
+}
+
+}  // extern "C"
+
+// union-pattern entries of the labelled rows grouped R at a time (rows placed in `vox`, n_blk block rows)
+template <int R>
+static int count_union(fredopt_plan* P, long long n_blk, const int32_t* vox, const long long* pU, const int32_t* cU, long long* ecount,
+                       long long* total) {
+    if (n_blk) k_block_union<R, false><<<grid_for(n_blk, 128, 1 << 16), 128, 0, P->stream>>>(n_blk, vox, pU, cU, nullptr, nullptr, ecount, nullptr,
+                                                                                       nullptr, nullptr, nullptr, nullptr, nullptr);
+    size_t tb = 0;
+    long long* dsum = nullptr;
+    void* tmp = nullptr;
+    TmpPool T;
+    CKR(T.get(&dsum, 1));
+    CK(cub::DeviceReduce::Sum(nullptr, tb, ecount, dsum, n_blk, P->stream));
+    CKR(T.get((char**)&tmp, tb));
+    CK(cub::DeviceReduce::Sum(tmp, tb, ecount, dsum, n_blk, P->stream));
+    CK(cudaMemcpyAsync(total, dsum, 8, cudaMemcpyDeviceToHost, P->stream));
+    CK(cudaStreamSynchronize(P->stream));
+    CK(cudaGetLastError());
+    return FREDOPT_OK;
 }
 
 static int create_impl(fredopt_plan* P, const fredopt_csr* D, const fredopt_csr* L, const int32_t* labels,
@@ -572,15 +674,12 @@ static int create_impl(fredopt_plan* P, const fredopt_csr* D, const fredopt_csr*
         P->h_tab[s] = T;
     }
     // ---- inputs on the device (borrowed if already there)
-    std::vector<void*> tmp;   // temporaries of this call
-    auto tfree = [&]() { for (void* p : tmp) cudaFree(p); tmp.clear(); };
-    struct Guard { decltype(tfree)& f; ~Guard() { f(); } } guard{tfree};
+    TmpPool tmp;   // temporaries of this call
     auto to_dev = [&](const void* src, size_t bytes, const void** out) -> int {
-        if (bytes == 0) { void* p; CK(cudaMalloc(&p, 16)); tmp.push_back(p); *out = p; return FREDOPT_OK; }
+        if (bytes == 0) { char* p; CKR(tmp.get(&p, 16)); *out = p; return FREDOPT_OK; }
         if (is_device_ptr(src)) { *out = src; return FREDOPT_OK; }
-        void* p = nullptr;
-        CK(cudaMalloc(&p, bytes));
-        tmp.push_back(p);
+        char* p = nullptr;
+        CKR(tmp.get(&p, bytes));
         CK(cudaMemcpyAsync(p, src, bytes, cudaMemcpyHostToDevice, st));
         *out = p;
         return FREDOPT_OK;
@@ -595,7 +694,7 @@ static int create_impl(fredopt_plan* P, const fredopt_csr* D, const fredopt_csr*
     CKR(to_dev(labels, V * 4, (const void**)&lab));
     // ---- validate
     int* flag = nullptr;
-    CK(cudaMalloc(&flag, 2 * sizeof(int))); tmp.push_back(flag);
+    CKR(tmp.get(&flag, 2));
     CK(cudaMemsetAsync(flag, 0, 2 * sizeof(int), st));
     k_check_ptr<<<grid_for(V + 1, 256, 4096), 256, 0, st>>>(pD, V, D->nnz, flag);
     k_check_ptr<<<grid_for(V + 1, 256, 4096), 256, 0, st>>>(pL, V, L->nnz, flag);
@@ -621,167 +720,242 @@ static int create_impl(fredopt_plan* P, const fredopt_csr* D, const fredopt_csr*
     long long nnzU = D->nnz;
     if (!same) {   // union pattern (rare path)
         long long *cnt = nullptr, *pu = nullptr;
-        CK(cudaMalloc(&cnt, (V + 1) * 8)); tmp.push_back(cnt);
-        CK(cudaMalloc(&pu, (V + 2) * 8)); tmp.push_back(pu);
+        CKR(tmp.get(&cnt, (size_t)V + 1)); CKR(tmp.get(&pu, (size_t)V + 2));
         CK(cudaMemsetAsync(cnt, 0, (V + 1) * 8, st));
         k_union_count<<<grid_for(V, 128, 1 << 16), 128, 0, st>>>(pD, cD, pL, cL, V, cnt);
         CKR(scan_exclusive(P, cnt, pu, V + 1));
         CK(cudaMemcpyAsync(&nnzU, pu + V, 8, cudaMemcpyDeviceToHost, st));
         CK(cudaStreamSynchronize(st));
         int32_t* cu; float *ud, *ul;
-        CK(cudaMalloc(&cu, (nnzU ? nnzU : 1) * 4)); tmp.push_back(cu);
-        CK(cudaMalloc(&ud, (nnzU ? nnzU : 1) * 4)); tmp.push_back(ud);
-        CK(cudaMalloc(&ul, (nnzU ? nnzU : 1) * 4)); tmp.push_back(ul);
+        CKR(tmp.get(&cu, (size_t)nnzU)); CKR(tmp.get(&ud, (size_t)nnzU)); CKR(tmp.get(&ul, (size_t)nnzU));
         k_union_fill<<<grid_for(V, 128, 1 << 16), 128, 0, st>>>(pD, cD, vD, pL, cL, vL, V, pu, cu, ud, ul);
         pU = pu; cU = cu; uD = ud; uL = ul;
     }
     if (nnzU >= (1LL << 32)) return FREDOPT_INVALID_ARG;
     P->nnz = nnzU;
-    // ---- row lengths, non-empty list, active list
-    long long *plen64, *pstart; int32_t *f_ne, *f_act, *pos_ne, *pos_act;
-    CK(cudaMalloc(&plen64, (V + 1) * 8)); tmp.push_back(plen64);
-    CK(cudaMalloc(&pstart, (V + 2) * 8)); tmp.push_back(pstart);
-    CK(cudaMalloc(&f_ne, (V + 1) * 4)); tmp.push_back(f_ne);
-    CK(cudaMalloc(&f_act, (V + 1) * 4)); tmp.push_back(f_act);
-    CK(cudaMalloc(&pos_ne, (V + 2) * 4)); tmp.push_back(pos_ne);
-    CK(cudaMalloc(&pos_act, (V + 2) * 4)); tmp.push_back(pos_act);
-    CK(cudaMemsetAsync(plen64, 0, (V + 1) * 8, st));
+    const bool idx16 = S <= 65536 && !P->force_idx32;       // 16-bit column indices for the hot kernels
+    // ---- non-empty list, labelled list
+    int32_t *f_ne, *f_act, *pos_ne, *pos_act;
+    CKR(tmp.get(&f_ne, (size_t)V + 1)); CKR(tmp.get(&f_act, (size_t)V + 1));
+    CKR(tmp.get(&pos_ne, (size_t)V + 2)); CKR(tmp.get(&pos_act, (size_t)V + 2));
     CK(cudaMemsetAsync(f_ne, 0, (V + 1) * 4, st));
     CK(cudaMemsetAsync(f_act, 0, (V + 1) * 4, st));
-    if (V) k_row_lengths<<<grid_for(V, 256, 1 << 16), 256, 0, st>>>(pU, lab, V, plen64, f_ne, f_act);
-    CKR(scan_exclusive(P, plen64, pstart, V + 1));
+    if (V) k_row_lengths<<<grid_for(V, 256, 1 << 16), 256, 0, st>>>(pU, lab, V, f_ne, f_act);
     CKR(scan_exclusive(P, f_ne, pos_ne, V + 1));
     CKR(scan_exclusive(P, f_act, pos_act, V + 1));
     int32_t n_ne = 0, n_act = 0;
-    CK(cudaMemcpyAsync(&P->nnz_padded, pstart + V, 8, cudaMemcpyDeviceToHost, st));
     CK(cudaMemcpyAsync(&n_ne, pos_ne + V, 4, cudaMemcpyDeviceToHost, st));
     CK(cudaMemcpyAsync(&n_act, pos_act + V, 4, cudaMemcpyDeviceToHost, st));
     CK(cudaStreamSynchronize(st));
-    // ---- full row set: non-empty rows ordered by (length class, voxel) and stored in that order, so that short rows
+    // ---- full row set (R = 1): non-empty rows ordered by (length class, voxel) and stored in that order, so that short rows
     //      (entrance channels, few spots per voxel) are handled by sub-warps over contiguous memory
     RowSet& F = P->full;
-    F.n = n_ne; F.n_seg = 1; F.nnz = nnzU;
+    F.R = 1; F.n = n_ne; F.n_rows = n_ne; F.n_true = n_ne; F.n_seg = 1; F.nnz = nnzU; F.entries = nnzU;
     CKR(dmalloc(P, &F.vox, (size_t)n_ne)); CKR(dmalloc(P, &F.start, (size_t)n_ne + 1));
     CKR(dmalloc(P, &F.len, (size_t)n_ne)); CKR(dmalloc(P, &F.ulen, (size_t)n_ne)); CKR(dmalloc(P, &F.items, (size_t)n_ne));
-    const size_t np = P->nnz_padded ? (size_t)P->nnz_padded : 4;
-    CKR(dmalloc(P, &F.col, np)); CKR(dmalloc(P, &F.valD, np)); CKR(dmalloc(P, &F.valL, np));
-    CK(cudaMemsetAsync(F.col, 0, np * 4, st)); CK(cudaMemsetAsync(F.valD, 0, np * 4, st)); CK(cudaMemsetAsync(F.valL, 0, np * 4, st));
     {
+        TmpPool t2;
         int32_t *vox0, *key0, *key1;
-        long long *flen64, *fstart;
+        long long* flen64;
         unsigned long long* hist;
-        CK(cudaMalloc(&vox0, ((size_t)n_ne + 1) * 4)); tmp.push_back(vox0);
-        CK(cudaMalloc(&key0, ((size_t)n_ne + 1) * 4)); tmp.push_back(key0);
-        CK(cudaMalloc(&key1, ((size_t)n_ne + 1) * 4)); tmp.push_back(key1);
-        CK(cudaMalloc(&flen64, ((size_t)n_ne + 1) * 8)); tmp.push_back(flen64);
-        CK(cudaMalloc(&fstart, ((size_t)n_ne + 1) * 8)); tmp.push_back(fstart);
-        CK(cudaMalloc(&hist, N_LEN_CLASS * 8)); tmp.push_back(hist);
+        CKR(t2.get(&vox0, (size_t)n_ne + 1)); CKR(t2.get(&key0, (size_t)n_ne + 1)); CKR(t2.get(&key1, (size_t)n_ne + 1));
+        CKR(t2.get(&flen64, (size_t)n_ne + 1)); CKR(t2.get(&hist, N_LEN_CLASS));
         CK(cudaMemsetAsync(hist, 0, N_LEN_CLASS * 8, st));
-        if (V) k_compact_rows<<<grid_for(V, 256, 1 << 16), 256, 0, st>>>(f_ne, pos_ne, pU, pstart, lab, V, vox0, nullptr, nullptr, nullptr, nullptr);
+        if (V) k_compact_rows<<<grid_for(V, 256, 1 << 16), 256, 0, st>>>(f_ne, pos_ne, lab, V, vox0, nullptr);
         if (n_ne) k_class_keys<<<grid_for(n_ne, 256, 1 << 16), 256, 0, st>>>(vox0, pU, n_ne, key0, hist);
         size_t tb = 0;
         CK(cub::DeviceRadixSort::SortPairs(nullptr, tb, key0, key1, vox0, F.vox, n_ne, 0, 3, st));
-        void* t2; CK(cudaMalloc(&t2, tb ? tb : 1)); tmp.push_back(t2);
-        CK(cub::DeviceRadixSort::SortPairs(t2, tb, key0, key1, vox0, F.vox, n_ne, 0, 3, st));   // stable: voxel order inside a class
-        if (n_ne) k_fill_active<<<grid_for(n_ne, 256, 1 << 16), 256, 0, st>>>(F.vox, nullptr, pU, pstart, n_ne, fstart, F.len, F.ulen, nullptr);
+        char* ts; CKR(t2.get(&ts, tb));
+        CK(cub::DeviceRadixSort::SortPairs(ts, tb, key0, key1, vox0, F.vox, n_ne, 0, 3, st));   // stable: voxel order inside a class
         CK(cudaMemsetAsync(flen64, 0, ((size_t)n_ne + 1) * 8, st));
-        if (n_ne) k_i32_to_i64<<<grid_for(n_ne, 256, 4096), 256, 0, st>>>(F.len, flen64, n_ne);
+        if (n_ne) k_fill_rows1<<<grid_for(n_ne, 256, 1 << 16), 256, 0, st>>>(F.vox, pU, n_ne, F.len, F.ulen, flen64);
         CKR(scan_exclusive(P, flen64, F.start, (long long)n_ne + 1));
         unsigned long long hh[N_LEN_CLASS];
         CK(cudaMemcpyAsync(hh, hist, N_LEN_CLASS * 8, cudaMemcpyDeviceToHost, st));
+        CK(cudaMemcpyAsync(&F.entries_padded, F.start + n_ne, 8, cudaMemcpyDeviceToHost, st));
         CK(cudaStreamSynchronize(st));
+        P->nnz_padded = F.entries_padded;
         P->full_class[0] = 0;
         for (int c = 0; c < N_LEN_CLASS; ++c) P->full_class[c + 1] = P->full_class[c] + (long long)hh[c];
+        const size_t np = F.entries_padded ? (size_t)F.entries_padded : 4;
+        if (idx16) { CKR(dmalloc(P, &F.col16, np)); CK(cudaMemsetAsync(F.col16, 0, np * 2, st)); }
+        else { CKR(dmalloc(P, &F.col, np)); CK(cudaMemsetAsync(F.col, 0, np * 4, st)); }
+        CKR(dmalloc(P, &F.valD, np)); CKR(dmalloc(P, &F.valL, np));
+        CK(cudaMemsetAsync(F.valD, 0, np * 4, st)); CK(cudaMemsetAsync(F.valL, 0, np * 4, st));
         if (n_ne) {
-            k_copy_padded<<<grid_for((long long)n_ne * 32, 256, 1 << 16), 256, 0, st>>>(F.n, F.vox, F.start, pU, cU, uD, uL, F.col, F.valD, F.valL);
-            k_pack_items<<<grid_for(n_ne, 256, 4096), 256, 0, st>>>(n_ne, F.start, F.len, nullptr, F.items);
+            k_copy_rows1<<<grid_for((long long)n_ne * 32, 256, 1 << 16), 256, 0, st>>>(F.n, F.vox, F.start, pU, cU, uD, uL, F.col, F.col16, F.valD, F.valL);
+            k_pack_items<<<grid_for(n_ne, 256, 4096), 256, 0, st>>>(n_ne, 1, F.start, F.len, nullptr, nullptr, F.items);
         }
-        if (S <= 65536 && !P->force_idx32) {   // 16-bit column indices for the hot kernels
-            CKR(dmalloc(P, &F.col16, np));
-            k_narrow_u16<<<grid_for((long long)np, 256, 1 << 16), 256, 0, st>>>(F.col, F.col16, (long long)np);
-        }
-    }
-    // ---- active row set, ordered by (label, voxel), with its own compact copy of the rows: the iteration then
-    //      streams contiguous arrays (no unconstrained rows in between)
-    RowSet& A = P->act;
-    A.n = n_act; A.n_seg = n_struct > 0 ? n_struct : 1;
-    CKR(dmalloc(P, &A.vox, (size_t)n_act)); CKR(dmalloc(P, &A.start, (size_t)n_act + 1)); CKR(dmalloc(P, &A.len, (size_t)n_act));
-    CKR(dmalloc(P, &A.ulen, (size_t)n_act)); CKR(dmalloc(P, &A.seg, (size_t)n_act)); CKR(dmalloc(P, &A.items, (size_t)n_act));
-    {
-        int32_t *vox0, *key0, *key1;
-        long long *alen64, *fstart;
-        CK(cudaMalloc(&vox0, (n_act + 1) * 4)); tmp.push_back(vox0);
-        CK(cudaMalloc(&key0, (n_act + 1) * 4)); tmp.push_back(key0);
-        CK(cudaMalloc(&key1, (n_act + 1) * 4)); tmp.push_back(key1);
-        CK(cudaMalloc(&alen64, ((size_t)n_act + 1) * 8)); tmp.push_back(alen64);
-        CK(cudaMalloc(&fstart, ((size_t)n_act + 1) * 8)); tmp.push_back(fstart);
-        if (V) k_compact_rows<<<grid_for(V, 256, 1 << 16), 256, 0, st>>>(f_act, pos_act, pU, pstart, lab, V, vox0, nullptr, nullptr, nullptr, key0);
-        int bits = 1;
-        while ((1 << bits) <= n_struct) ++bits;
-        size_t tb = 0;
-        CK(cub::DeviceRadixSort::SortPairs(nullptr, tb, key0, key1, vox0, A.vox, n_act, 0, bits, st));
-        void* t2; CK(cudaMalloc(&t2, tb ? tb : 1)); tmp.push_back(t2);
-        CK(cub::DeviceRadixSort::SortPairs(t2, tb, key0, key1, vox0, A.vox, n_act, 0, bits, st));
-        // fstart = the row's offset in the full arrays (unused afterwards), A.len / A.ulen / A.seg; then A.start by a scan
-        if (n_act) k_fill_active<<<grid_for(n_act, 256, 1 << 16), 256, 0, st>>>(A.vox, key1, pU, pstart, n_act, fstart, A.len, A.ulen, A.seg);
-        CK(cudaMemsetAsync(alen64, 0, ((size_t)n_act + 1) * 8, st));
-        if (n_act) k_i32_to_i64<<<grid_for(n_act, 256, 4096), 256, 0, st>>>(A.len, alen64, n_act);
-        CKR(scan_exclusive(P, alen64, A.start, (long long)n_act + 1));
-        long long a_padded = 0;
-        CK(cudaMemcpyAsync(&a_padded, A.start + n_act, 8, cudaMemcpyDeviceToHost, st));
         CK(cudaStreamSynchronize(st));
-        const size_t na = a_padded ? (size_t)a_padded : 4;
-        CKR(dmalloc(P, &A.col, na)); CKR(dmalloc(P, &A.valD, na)); CKR(dmalloc(P, &A.valL, na));
-        CK(cudaMemsetAsync(A.col, 0, na * 4, st)); CK(cudaMemsetAsync(A.valD, 0, na * 4, st)); CK(cudaMemsetAsync(A.valL, 0, na * 4, st));
-        if (n_act) {
-            k_copy_padded<<<grid_for((long long)n_act * 32, 256, 1 << 16), 256, 0, st>>>(A.n, A.vox, A.start, pU, cU, uD, uL, A.col, A.valD, A.valL);
-            k_pack_items<<<grid_for(n_act, 256, 4096), 256, 0, st>>>(n_act, A.start, A.len, A.seg, A.items);
-        }
-        if (S <= 65536 && !P->force_idx32) {
-            CKR(dmalloc(P, &A.col16, na));
-            k_narrow_u16<<<grid_for((long long)na, 256, 1 << 16), 256, 0, st>>>(A.col, A.col16, (long long)na);
-        }
+        CK(cudaGetLastError());
     }
-    // ---- tables, norms, w^
+    // ---- labelled row set, ordered by (label, voxel), as block rows of R consecutive rows of one structure with its own
+    //      compact copy of the entries: the iteration streams contiguous arrays (no unconstrained rows in between)
+    RowSet& A = P->act;
     const int ns = n_struct > 0 ? n_struct : 1;
+    A.n_seg = ns; A.n_true = n_act;
     P->max_seg = ns;
     CKR(dmalloc(P, &P->tab, (size_t)ns));
     CK(cudaMemcpyAsync(P->tab, P->h_tab.data(), sizeof(StructInfo) * ns, cudaMemcpyHostToDevice, st));
-    CKR(dmalloc(P, &P->nD, (size_t)n_act)); CKR(dmalloc(P, &P->nL, (size_t)n_act)); CKR(dmalloc(P, &P->nT, (size_t)n_act));
-    CKR(dmalloc(P, &P->mode_union, (size_t)ns)); CKR(dmalloc(P, &P->mode_con, (size_t)ns)); CKR(dmalloc(P, &P->mode_cost, (size_t)ns));
-    CKR(dmalloc(P, &P->mode_fixed, (size_t)ns * 4));
-    CKR(dmalloc(P, &P->st, 1));
-    CK(cudaMemsetAsync(P->st, 0, sizeof(DevState), st));
-    if (n_act) {
-        k_norms<<<grid_for((long long)n_act * 32, 256, 1 << 16), 256, 0, st>>>(A.view(), A.col, A.valD, A.valL, P->tab, P->nD, P->nL, P->nT);
-        k_count_sets<<<grid_for(n_act, 256, 4096), 256, 0, st>>>(n_act, A.seg, A.ulen, P->nD, P->nL, P->nT, P->tab);
+    {
+        TmpPool t2;
+        int32_t *vox0, *key0, *lab_s, *vox_s;
+        unsigned long long* hist;
+        CKR(t2.get(&vox0, (size_t)n_act + 1)); CKR(t2.get(&key0, (size_t)n_act + 1)); CKR(t2.get(&lab_s, (size_t)n_act + 1));
+        CKR(t2.get(&vox_s, (size_t)n_act + 1)); CKR(t2.get(&hist, (size_t)ns));
+        CK(cudaMemsetAsync(hist, 0, (size_t)ns * 8, st));
+        if (V) k_compact_rows<<<grid_for(V, 256, 1 << 16), 256, 0, st>>>(f_act, pos_act, lab, V, vox0, key0);
+        int bits = 1;
+        while ((1 << bits) <= n_struct) ++bits;
+        size_t tb = 0;
+        CK(cub::DeviceRadixSort::SortPairs(nullptr, tb, key0, lab_s, vox0, vox_s, n_act, 0, bits, st));
+        char* ts; CKR(t2.get(&ts, tb));
+        CK(cub::DeviceRadixSort::SortPairs(ts, tb, key0, lab_s, vox0, vox_s, n_act, 0, bits, st));
+        if (n_act) k_label_hist<<<grid_for(n_act, 256, 4096), 256, 0, st>>>(n_act, lab_s, hist);
+        std::vector<unsigned long long> hrows((size_t)ns, 0ULL);
+        CK(cudaMemcpyAsync(hrows.data(), hist, (size_t)ns * 8, cudaMemcpyDeviceToHost, st));
+        CK(cudaStreamSynchronize(st));
+        // rows of a structure padded to a multiple of R, so that no block row straddles two structures
+        long long* shift_d; CKR(t2.get(&shift_d, (size_t)ns));
+        std::vector<long long> shift((size_t)ns, 0);
+        auto layout = [&](int R, long long* n_rows_out) {
+            long long base = 0, base_pad = 0;
+            P->row_base.assign((size_t)ns + 1, 0);
+            for (int s = 0; s < ns; ++s) {
+                P->row_base[s] = base_pad;
+                shift[s] = base_pad - base;
+                base += (long long)hrows[s];
+                base_pad += ((long long)hrows[s] + R - 1) / R * R;
+            }
+            P->row_base[ns] = base_pad;
+            *n_rows_out = base_pad;
+        };
+        int32_t *rlen = nullptr;
+        long long* ecount = nullptr;
+        auto place = [&](int R, long long* n_rows_out) -> int {      // A.vox / A.rseg / rlen for block height R
+            layout(R, n_rows_out);
+            const long long nr = *n_rows_out;
+            CK(cudaMemcpyAsync(shift_d, shift.data(), (size_t)ns * 8, cudaMemcpyHostToDevice, st));
+            CK(cudaMemsetAsync(A.vox, 0xFF, (size_t)(nr ? nr : 1) * 4, st));
+            CK(cudaMemsetAsync(A.rseg, 0xFF, (size_t)(nr ? nr : 1) * 2, st));
+            CK(cudaMemsetAsync(rlen, 0, (size_t)(nr ? nr : 1) * 4, st));
+            if (n_act) k_place_rows<<<grid_for(n_act, 256, 4096), 256, 0, st>>>(n_act, vox_s, lab_s, shift_d, pU, A.vox, A.rseg, rlen);
+            CK(cudaStreamSynchronize(st));          // `shift` is reused by the next call
+            return FREDOPT_OK;
+        };
+        const size_t max_rows = (size_t)n_act + 4 * (size_t)ns + 4;
+        CKR(dmalloc(P, &A.vox, max_rows)); CKR(dmalloc(P, &A.rseg, max_rows));
+        CKR(t2.get(&rlen, max_rows)); CKR(t2.get(&ecount, max_rows));
+        // block height: the one that stores the fewest bytes (an index per entry + R values); a forced value wins
+        long long nnzA = 0;
+        int Rb = P->block_rows_opt;
+        {
+            long long nr1 = 0;
+            CKR(place(1, &nr1));
+            CKR(count_union<1>(P, nr1, A.vox, pU, cU, ecount, &nnzA));
+        }
+        A.nnz = nnzA;
+        if (Rb == 0) {
+            const double ib = idx16 ? 2.0 : 4.0;
+            double best = (double)nnzA * (4.0 + ib);
+            Rb = 1;
+            for (int R : {2, 4}) {
+                long long nr = 0, ent = 0;
+                CKR(place(R, &nr));
+                if (R == 2) CKR(count_union<2>(P, nr / R, A.vox, pU, cU, ecount, &ent));
+                else CKR(count_union<4>(P, nr / R, A.vox, pU, cU, ecount, &ent));
+                const double bytes = (double)ent * (4.0 * R + ib);
+                if (bytes < 0.97 * best) { best = bytes; Rb = R; }      // a taller block must save at least 3 %
+            }
+        }
+        A.R = Rb;
+        long long n_rows = 0;
+        CKR(place(Rb, &n_rows));
+        A.n_rows = n_rows;
+        A.n = n_rows / Rb;
+        const long long n_blk = A.n;
+        long long ent = 0;
+        if (Rb == 1) CKR(count_union<1>(P, n_blk, A.vox, pU, cU, ecount, &ent));
+        else if (Rb == 2) CKR(count_union<2>(P, n_blk, A.vox, pU, cU, ecount, &ent));
+        else CKR(count_union<4>(P, n_blk, A.vox, pU, cU, ecount, &ent));
+        A.entries = ent;
+        CKR(dmalloc(P, &A.start, (size_t)n_blk + 1)); CKR(dmalloc(P, &A.len, (size_t)n_blk)); CKR(dmalloc(P, &A.ulen, (size_t)n_blk));
+        CKR(dmalloc(P, &A.seg, (size_t)n_blk)); CKR(dmalloc(P, &A.items, (size_t)n_blk));
+        int32_t* nreal; long long* len64;
+        CKR(t2.get(&nreal, (size_t)n_blk)); CKR(t2.get(&len64, (size_t)n_blk + 1));
+        CK(cudaMemsetAsync(len64, 0, ((size_t)n_blk + 1) * 8, st));
+        if (n_blk) k_block_meta<<<grid_for(n_blk, 256, 4096), 256, 0, st>>>(n_blk, Rb, A.rseg, ecount, A.seg, nreal, A.ulen, A.len, len64);
+        CKR(scan_exclusive(P, len64, A.start, n_blk + 1));
+        CK(cudaMemcpyAsync(&A.entries_padded, A.start + n_blk, 8, cudaMemcpyDeviceToHost, st));
+        CK(cudaStreamSynchronize(st));
+        const size_t na = A.entries_padded ? (size_t)A.entries_padded : 4;
+        if (idx16) { CKR(dmalloc(P, &A.col16, na)); CK(cudaMemsetAsync(A.col16, 0, na * 2, st)); }
+        else { CKR(dmalloc(P, &A.col, na)); CK(cudaMemsetAsync(A.col, 0, na * 4, st)); }
+        CKR(dmalloc(P, &A.valD, na * Rb)); CKR(dmalloc(P, &A.valL, na * Rb));
+        CK(cudaMemsetAsync(A.valD, 0, na * Rb * 4, st)); CK(cudaMemsetAsync(A.valL, 0, na * Rb * 4, st));
+        if (n_blk) {
+            const int g = grid_for(n_blk, 128, 1 << 16);
+            if (Rb == 1) k_block_union<1, true><<<g, 128, 0, st>>>(n_blk, A.vox, pU, cU, uD, uL, nullptr, A.start, A.len, A.col, A.col16, A.valD, A.valL);
+            else if (Rb == 2) k_block_union<2, true><<<g, 128, 0, st>>>(n_blk, A.vox, pU, cU, uD, uL, nullptr, A.start, A.len, A.col, A.col16, A.valD, A.valL);
+            else k_block_union<4, true><<<g, 128, 0, st>>>(n_blk, A.vox, pU, cU, uD, uL, nullptr, A.start, A.len, A.col, A.col16, A.valD, A.valL);
+            k_pack_items<<<grid_for(n_blk, 256, 4096), 256, 0, st>>>(n_blk, Rb, A.start, A.len, A.seg, nreal, A.items);
+            // execution order of the whole-set passes: longest block rows first (the queue then ends with the short ones)
+            uint32_t *ik, *ik2, *ii, *ii2;
+            CKR(t2.get(&ik, (size_t)n_blk)); CKR(t2.get(&ik2, (size_t)n_blk)); CKR(t2.get(&ii, (size_t)n_blk)); CKR(t2.get(&ii2, (size_t)n_blk));
+            CKR(dmalloc(P, &A.items_x, (size_t)n_blk)); CKR(dmalloc(P, &A.item_blk, (size_t)n_blk));
+            k_item_len_key<<<grid_for(n_blk, 256, 4096), 256, 0, st>>>(A.items, n_blk, ik, ii);
+            size_t sb = 0;
+            CK(cub::DeviceRadixSort::SortPairs(nullptr, sb, ik, ik2, ii, ii2, n_blk, 0, 32, st));
+            char* stmp; CKR(t2.get(&stmp, sb));
+            CK(cub::DeviceRadixSort::SortPairs(stmp, sb, ik, ik2, ii, ii2, n_blk, 0, 32, st));
+            k_item_gather<<<grid_for(n_blk, 256, 4096), 256, 0, st>>>(ii2, n_blk, A.items, A.items_x, A.item_blk);
+        }
+        // ---- norms, tables, w^
+        CKR(dmalloc(P, &P->nD, (size_t)n_rows)); CKR(dmalloc(P, &P->nL, (size_t)n_rows)); CKR(dmalloc(P, &P->nT, (size_t)n_rows));
+        CK(cudaMemsetAsync(P->nD, 0, (size_t)(n_rows ? n_rows : 1) * 8, st)); CK(cudaMemsetAsync(P->nL, 0, (size_t)(n_rows ? n_rows : 1) * 8, st));
+        CK(cudaMemsetAsync(P->nT, 0, (size_t)(n_rows ? n_rows : 1) * 8, st));
+        CKR(dmalloc(P, &P->mode_union, (size_t)ns)); CKR(dmalloc(P, &P->mode_con, (size_t)ns)); CKR(dmalloc(P, &P->mode_cost, (size_t)ns));
+        CKR(dmalloc(P, &P->mode_fixed, (size_t)ns * 4));
+        CKR(dmalloc(P, &P->st, 1));
+        CK(cudaMemsetAsync(P->st, 0, sizeof(DevState), st));
+        if (n_blk) {
+            k_norms<<<grid_for(n_blk * 32, 256, 1 << 16), 256, 0, st>>>(n_blk, Rb, A.start, A.len, A.seg, A.valD, A.valL, P->tab, P->nD, P->nL, P->nT);
+            k_count_sets<<<grid_for(n_rows, 256, 4096), 256, 0, st>>>(n_rows, A.rseg, rlen, P->nD, P->nL, P->nT, P->tab);
+            k_count_entries<<<grid_for(n_blk, 256, 4096), 256, 0, st>>>(n_blk, A.seg, A.ulen, P->tab);
+        }
+        k_finish_tables<<<1, 1, 0, st>>>(P->tab, n_struct, P->st, P->mode_union, P->mode_con, P->mode_cost, P->mode_fixed, ns);
+        state_init(P);
+        CK(cudaMemcpyAsync(P->h_tab.data(), P->tab, sizeof(StructInfo) * ns, cudaMemcpyDeviceToHost, st));
+        CK(cudaStreamSynchronize(st));
+        CK(cudaGetLastError());
     }
-    k_finish_tables<<<1, 1, 0, st>>>(P->tab, n_struct, P->st, P->mode_union, P->mode_con, P->mode_cost, P->mode_fixed, ns);
-    state_init(P);
-    CK(cudaMemcpyAsync(P->h_tab.data(), P->tab, sizeof(StructInfo) * ns, cudaMemcpyDeviceToHost, st));
-    CK(cudaStreamSynchronize(st));
-    CK(cudaGetLastError());
     // ---- vectors
+    const long long NR = A.n_rows;
     CKR(dmalloc(P, &P->x, (size_t)S)); CKR(dmalloc(P, &P->g, (size_t)S)); CKR(dmalloc(P, &P->xtmp, (size_t)S));
     CKR(dmalloc(P, &P->xstage, (size_t)S));
     CK(cudaMemsetAsync(P->x, 0, (S ? S : 1) * 8, st)); CK(cudaMemsetAsync(P->g, 0, (S ? S : 1) * 8, st));
     double** vecs[] = {&P->d, &P->l, &P->Dg, &P->Lg};
-    for (auto pp : vecs) { CKR(dmalloc(P, pp, (size_t)n_act)); CK(cudaMemsetAsync(*pp, 0, (n_act ? n_act : 1) * 8, st)); }
-    CKR(gv_alloc(P, &P->pq, (size_t)n_act)); CKR(gv_alloc(P, &P->uv, (size_t)n_act));
-    CKR(dmalloc(P, &P->cpart, (size_t)MAX_PARTIALS));
+    for (auto pp : vecs) { CKR(dmalloc(P, pp, (size_t)NR)); CK(cudaMemsetAsync(*pp, 0, (NR ? NR : 1) * 8, st)); }
+    CKR(gv_alloc(P, &P->pq, (size_t)NR)); CKR(gv_alloc(P, &P->uv, (size_t)NR));
+    const size_t npart = (size_t)(A.n > MAX_PARTIALS ? A.n : MAX_PARTIALS);     // per block row (forward epilogues) or per CTA
+    CKR(dmalloc(P, &P->cpart, npart));
+    CKR(dmalloc(P, &P->wq, 1));
+    CK(cudaMemsetAsync(P->wq, 0, sizeof(WorkQueue), st));
     CKR(dmalloc(P, &P->gpart, (size_t)(S / 256 + 2)));
-    CK(cudaMemsetAsync(P->gpart, 0, (size_t)(S / 256 + 2) * 8, st)); CKR(dmalloc(P, &P->part_prox, (size_t)MAX_PARTIALS));
-    CKR(dmalloc(P, &P->part_phi, (size_t)MAX_PARTIALS)); CKR(dmalloc(P, &P->part_cnt, (size_t)MAX_PARTIALS));
+    CK(cudaMemsetAsync(P->gpart, 0, (size_t)(S / 256 + 2) * 8, st)); CKR(dmalloc(P, &P->part_prox, npart));
+    CKR(dmalloc(P, &P->part_phi, npart)); CKR(dmalloc(P, &P->part_cnt, npart));
     CKR(dmalloc(P, &P->sink, 4));
-    CK(cudaMemsetAsync(P->cpart, 0, MAX_PARTIALS * 8, st));
-    CK(cudaMemsetAsync(P->part_prox, 0, MAX_PARTIALS * 8, st)); CK(cudaMemsetAsync(P->part_phi, 0, MAX_PARTIALS * 8, st));
-    CK(cudaMemsetAsync(P->part_cnt, 0, MAX_PARTIALS * 8, st));
-    // ---- CSR of the transposes restricted to the active rows
+    CK(cudaMemsetAsync(P->cpart, 0, npart * 8, st));
+    CK(cudaMemsetAsync(P->part_prox, 0, npart * 8, st)); CK(cudaMemsetAsync(P->part_phi, 0, npart * 8, st));
+    CK(cudaMemsetAsync(P->part_cnt, 0, npart * 8, st));
+    // ---- CSR of the transposes restricted to the labelled rows
     CKR(build_transpose(P, A));
     compute_pass_bytes(P);
     CK(cudaStreamSynchronize(st));
     return FREDOPT_OK;
 }
+
+extern "C" {
 
 int fredopt_create(const fredopt_csr* D, const fredopt_csr* L, const int32_t* voxel_labels, const fredopt_bounds* bounds,
                    int32_t n_struct, void* cuda_stream, fredopt_plan** out) {
@@ -799,6 +973,7 @@ int fredopt_create_ex(const fredopt_csr* D, const fredopt_csr* L, const int32_t*
         memcpy(&o, opt, (size_t)opt->struct_size);
     }
     if (o.index_width != 0 && o.index_width != 32) return FREDOPT_INVALID_ARG;
+    if (o.block_rows != 0 && o.block_rows != 1 && o.block_rows != 2 && o.block_rows != 4) return FREDOPT_INVALID_ARG;
     if (!D || !L || n_struct < 0 || (n_struct > 0 && !bounds)) return FREDOPT_INVALID_ARG;
     if (n_struct > 255) return FREDOPT_UNSUPPORTED;          // work items carry the structure in 8 bits
     if (D->n_rows != L->n_rows || D->n_cols != L->n_cols || D->n_rows < 0 || D->n_cols < 0 || D->nnz < 0 || L->nnz < 0)
@@ -823,6 +998,7 @@ int fredopt_create_ex(const fredopt_csr* D, const fredopt_csr* L, const int32_t*
     P->device = dev;
     P->sm_count = prop.multiProcessorCount;
     P->force_idx32 = o.index_width == 32;
+    P->block_rows_opt = o.block_rows;
     int rc = create_impl(P, D, L, voxel_labels, bounds, n_struct);
     if (rc != FREDOPT_OK) { fredopt_destroy(P); return rc; }
     *out = P;

@@ -17,7 +17,7 @@ LIB_PATH = os.path.join(_HERE, "libfredopt.so")
 
 OK, INVALID_ARG, OUT_OF_MEMORY, CUDA_ERROR, UNSUPPORTED_ARCH, UNSUPPORTED = 0, -1, -2, -3, -4, -5
 OPT_ETA, OPT_REDUCTIONS, OPT_ACCEPT_CHECK, OPT_MAX_TRIALS, OPT_RESET, OPT_USE_GRAPH, OPT_TIME_PASSES, \
-    OPT_BLOCK_SEQUENTIAL, OPT_NORMALIZE_GRAD, OPT_ONE_SIDED_COST, OPT_USE_PDL = range(11)
+    OPT_BLOCK_SEQUENTIAL, OPT_NORMALIZE_GRAD, OPT_ONE_SIDED_COST, OPT_USE_PDL, OPT_WORK_QUEUE = range(12)
 ROWS_ALL, ROWS_ACTIVE = 0, 1
 PASS_NAMES = ("forward_x", "transpose_g", "forward_g", "select", "residual", "transpose_b")
 N_PASSES = len(PASS_NAMES)
@@ -51,12 +51,12 @@ class _Bounds(C.Structure):
 
 
 class _CreateOptions(C.Structure):
-    _fields_ = [("struct_size", C.c_int32), ("index_width", C.c_int32)]
+    _fields_ = [("struct_size", C.c_int32), ("index_width", C.c_int32), ("block_rows", C.c_int32)]
 
 
 class Stats(C.Structure):
     _fields_ = [(n, C.c_int64) for n in ("k", "s", "trials", "n_violated", "n_sets", "n_zero_norm_sets",
-                                         "n_active_rows", "nnz", "nnz_active", "alg_bytes_iter")] + \
+                                         "n_active_rows", "nnz", "nnz_active", "alg_bytes_iter", "block_rows", "entries_active")] + \
                [(n, C.c_double) for n in ("last_beta", "phi", "prox", "weight_sum")]
 
     def as_dict(self):

@@ -49,7 +49,7 @@ def test_strerror_and_struct_layout(lib_path):
     assert b"invalid" in fredopt._lib.fredopt_strerror(fredopt.INVALID_ARG)
     assert C.sizeof(fredopt._Csr) == 48          # 3 x int64 + 3 pointers
     assert C.sizeof(fredopt._Bounds) == 32       # 8 floats
-    assert C.sizeof(fredopt.Stats) == 10 * 8 + 4 * 8
+    assert C.sizeof(fredopt.Stats) == 12 * 8 + 4 * 8
 
 
 def test_null_arguments_are_rejected_without_touching_a_device(lib_path):

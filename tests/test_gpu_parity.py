@@ -41,8 +41,11 @@ def _rel_l2(a, b):
     return float(np.linalg.norm(a - b) / max(np.linalg.norm(b), 1e-300))
 
 
-# both stored index forms of a plan: automatic (16-bit where exact) and int32 everywhere (fredopt_create_options.index_width)
-INDEX_FORMS = [pytest.param({}, id="idx16"), pytest.param({"index_width": 32}, id="idx32")]
+# the stored forms of a plan (fredopt_create_options): index width automatic (16-bit where exact) or int32 everywhere; rows per
+# stored block row automatic (fewest bytes) or forced to 1, 2, 4
+INDEX_FORMS = [pytest.param({}, id="auto"), pytest.param({"index_width": 32}, id="idx32"),
+               pytest.param({"block_rows": 1}, id="rows1"), pytest.param({"block_rows": 2}, id="rows2"),
+               pytest.param({"block_rows": 4}, id="rows4"), pytest.param({"block_rows": 2, "index_width": 32}, id="rows2-idx32")]
 
 
 def _assert_fwd(got, ref, what):
@@ -222,8 +225,9 @@ def test_rejected_trials_multi_beam(fredopt):
 
 
 # ------------------------------------------------------------------------------------------ small / ragged / degenerate
+@pytest.mark.parametrize("rows", [0, 1, 2, 4])
 @pytest.mark.parametrize("seed,same", [(1, True), (2, False), (5, False)])
-def test_random_small_plans_union_pattern(fredopt, seed, same):
+def test_random_small_plans_union_pattern(fredopt, seed, same, rows):
     V, S = 300, 37
     D, L, lab, x0 = pg.random_small_plan(seed, V=V, S=S, n_struct=3, density=0.3, same_pattern=same)
     nan = np.nan
@@ -231,7 +235,8 @@ def test_random_small_plans_union_pattern(fredopt, seed, same):
                        [2.0, nan, 0.4, nan, 1.5, 3.0, nan, 1.5],
                        [0.5, 0.1, nan, 0.2, 2.0, nan, 0.3, 1.0]], np.float32)
     orc = _oracle_np(V, S, D, L, lab, bounds)
-    gp = fredopt.Plan(V, S, D, L, lab, bounds)
+    gp = fredopt.Plan(V, S, D, L, lab, bounds, block_rows=rows)
+    assert gp.stats()["block_rows"] == rows or rows == 0
     x = x0
     d_ref, l_ref, _ = orc.dose_let(x.astype(np.float64))
     d = np.empty(V, np.float32); l = np.empty(V, np.float32)
@@ -263,7 +268,7 @@ def test_random_bound_combinations(fredopt, seed):
     bounds = np.array(rows, np.float32)
     for block in (0, 1):
         orc = _oracle_np(V, S, D, L, lab, bounds)
-        gp = fredopt.Plan(V, S, D, L, lab, bounds)
+        gp = fredopt.Plan(V, S, D, L, lab, bounds, block_rows=(0, 1, 2, 4)[seed % 4])
         gp.set_option(fredopt.OPT_BLOCK_SEQUENTIAL, block); orc.set_option(om.OPT_BLOCK_SEQUENTIAL, block)
         orc.set_x(x0); gp.set_weights(x0)
         orc.iterate(20, 1.3, 0.8, 0.85); gp.iterate(20, 1.3, 0.8, 0.85)
@@ -702,3 +707,27 @@ def test_more_than_65536_labelled_rows(fredopt, copt):
             _assert_block_state(gp, orc)
         else:
             _assert_state(gp, orc)
+
+
+def test_work_distribution_never_changes_a_result(fredopt, plan0):
+    """FREDOPT_OPT_WORK_QUEUE: items dealt statically or from the queue, in storage order or longest first, in either orientation
+    -- the same bits in x after 20 superiorized + 5 block-sequential iterations (an item's sum is formed by one warp in a fixed
+    order and lands in a place of its own; partial sums are added in a fixed order)."""
+    f = fredopt
+    ref = None
+    for mode in range(16):
+        gp = f.from_plan(plan0)
+        gp.set_option(f.OPT_WORK_QUEUE, mode)
+        gp.set_weights(plan0.x0)
+        gp.iterate(20, 1.0, 1.0, 0.99)
+        gp.set_option(f.OPT_BLOCK_SEQUENTIAL, 1)
+        gp.iterate(5, 1.0, 1.0, 0.99)
+        x = _gpu_x(gp)
+        st = gp.stats()
+        key = (st["k"], st["s"], st["trials"], st["n_violated"], st["prox"])
+        if ref is None:
+            ref = (x, key)
+        assert np.array_equal(x, ref[0]) and key == ref[1], f"mode {mode}"
+        gp.destroy()
+    with pytest.raises(f.FredoptError):
+        gp = f.from_plan(plan0); gp.set_option(f.OPT_WORK_QUEUE, 16)
