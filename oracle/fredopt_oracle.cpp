@@ -48,10 +48,15 @@ struct Bounds {   // all widened from the fp32 bit patterns the caller passed; N
 
 inline bool present(double v) { return !std::isnan(v); }
 
+// fields of the per-voxel bound arrays (bounds "defined for each point in the image space"; Eq. (2),
+// per-voxel Dref_i, cDLref_i)
+enum { VB_DOSE_LO = 0, VB_DOSE_HI, VB_DL_LO, VB_DL_HI, VB_LETD_MAX, VB_DOSE_REF, VB_DL_REF, VB_N };
+
 struct Plan {
     Csr D, L;
     std::vector<int32_t> label;        // per voxel; 0 = unconstrained
     std::vector<Bounds> bounds;        // index s-1 for label s
+    std::vector<double> vb[VB_N];      // optional per-voxel values (empty = none; NaN = the structure's scalar)
     std::vector<double> nD, nL, nT;    // squared norms of D_i, L_i, L_i - letd_max*D_i  (per voxel)
     std::vector<double> what;          // normalised weight per structure (index s-1)
     double W = 0.0;
@@ -72,6 +77,16 @@ struct Plan {
     double sweep_prox = 0.0;           // statistics of the last block-sequential sweep (at visit time)
     int64_t sweep_viol = 0;
 };
+
+// Bounds of voxel i (structure s): the structure's scalars, each replaced by the voxel's own value where a per-voxel array
+// holds one.  Which constraint kinds and cost terms a voxel has is decided by its structure (has_dose_slab(bounds[s-1]), ...).
+inline Bounds voxel_bounds(const Plan& P, int64_t i, int32_t s) {
+    Bounds b = P.bounds[s - 1];
+    double* f[VB_N] = {&b.dose_lo, &b.dose_hi, &b.dl_lo, &b.dl_hi, &b.letd_max, &b.dose_ref, &b.dl_ref};
+    for (int k = 0; k < VB_N; ++k)
+        if (!P.vb[k].empty() && !std::isnan(P.vb[k][i])) *f[k] = P.vb[k][i];
+    return b;
+}
 
 // <A_i, x>
 inline double row_dot(const Csr& A, int64_t i, const std::vector<double>& x) {
@@ -127,7 +142,7 @@ void setup(Plan& P) {
         n = 0.0;
         for (int64_t p = P.L.ptr[i]; p < P.L.ptr[i + 1]; ++p) n += P.L.val[p] * P.L.val[p];
         P.nL[i] = n;
-        if (has_letd(b)) { letd_row_dot(P, i, b.letd_max, zero, &n); P.nT[i] = n; }
+        if (has_letd(b)) { letd_row_dot(P, i, voxel_bounds(P, i, s).letd_max, zero, &n); P.nT[i] = n; }
         if (has_dose_slab(b)) { ++P.n_sets; if (P.nD[i] > 0) ++part[s - 1]; else ++P.n_zero_norm_sets; }
         if (has_dl_slab(b))   { ++P.n_sets; if (P.nL[i] > 0) ++part[s - 1]; else ++P.n_zero_norm_sets; }
         if (has_letd(b))      { ++P.n_sets; if (P.nT[i] > 0) ++part[s - 1]; else ++P.n_zero_norm_sets; }
@@ -145,9 +160,10 @@ double cost(const Plan& P, const std::vector<double>& x) {
     for (int64_t i = 0; i < P.D.n_rows; ++i) {
         int32_t s = P.label[i];
         if (s == 0) continue;
-        const Bounds& b = P.bounds[s - 1];
-        if (present(b.dose_ref)) { double e = b.dose_ref - row_dot(P.D, i, x); phi += P.what[s - 1] * e * e; }
-        if (present(b.dl_ref))   { double e = b.dl_ref - row_dot(P.L, i, x);
+        const Bounds& sb = P.bounds[s - 1];                         // the structure decides which terms exist ...
+        const Bounds b = voxel_bounds(P, i, s);                      // ... the voxel may carry its own reference values
+        if (present(sb.dose_ref)) { double e = b.dose_ref - row_dot(P.D, i, x); phi += P.what[s - 1] * e * e; }
+        if (present(sb.dl_ref))   { double e = b.dl_ref - row_dot(P.L, i, x);
                                    if (!(P.one_sided_cost && e > 0.0)) phi += P.what[s - 1] * e * e; }   // one-sided: only cDL above cDLref
     }
     return phi;
@@ -159,12 +175,13 @@ void grad_cost(const Plan& P, const std::vector<double>& x, std::vector<double>&
     for (int64_t i = 0; i < P.D.n_rows; ++i) {
         int32_t s = P.label[i];
         if (s == 0) continue;
-        const Bounds& b = P.bounds[s - 1];
-        if (present(b.dose_ref)) {
+        const Bounds& sb = P.bounds[s - 1];
+        const Bounds b = voxel_bounds(P, i, s);
+        if (present(sb.dose_ref)) {
             double c = 2.0 * P.what[s - 1] * (row_dot(P.D, i, x) - b.dose_ref);
             for (int64_t p = P.D.ptr[i]; p < P.D.ptr[i + 1]; ++p) g[P.D.col[p]] += c * P.D.val[p];
         }
-        if (present(b.dl_ref)) {
+        if (present(sb.dl_ref)) {
             double c = 2.0 * P.what[s - 1] * (row_dot(P.L, i, x) - b.dl_ref);
             if (P.one_sided_cost && c < 0.0) c = 0.0;
             for (int64_t p = P.L.ptr[i]; p < P.L.ptr[i + 1]; ++p) g[P.L.col[p]] += c * P.L.val[p];
@@ -183,9 +200,10 @@ void constraint_pass(const Plan& P, const std::vector<double>& x, std::vector<do
     for (int64_t i = 0; i < P.D.n_rows; ++i) {
         int32_t s = P.label[i];
         if (s == 0) continue;
-        const Bounds& b = P.bounds[s - 1];
+        const Bounds& sb = P.bounds[s - 1];
+        const Bounds b = voxel_bounds(P, i, s);
         const double w = P.what[s - 1];
-        if (has_dose_slab(b)) {                                   // dose block of Fig. 2 (R4)
+        if (has_dose_slab(sb)) {                                  // dose block of Fig. 2 (R4)
             double r = slab_residual(row_dot(P.D, i, x), b.dose_lo, b.dose_hi);
             if (r != 0.0) ++nv;
             if (P.nD[i] > 0 && r != 0.0) {
@@ -194,7 +212,7 @@ void constraint_pass(const Plan& P, const std::vector<double>& x, std::vector<do
                     for (int64_t p = P.D.ptr[i]; p < P.D.ptr[i + 1]; ++p) (*step)[P.D.col[p]] += c * P.D.val[p]; }
             }
         }
-        if (has_dl_slab(b)) {                                     // cDLET block of Fig. 2
+        if (has_dl_slab(sb)) {                                    // cDLET block of Fig. 2
             double r = slab_residual(row_dot(P.L, i, x), b.dl_lo, b.dl_hi);
             if (r != 0.0) ++nv;
             if (P.nL[i] > 0 && r != 0.0) {
@@ -203,7 +221,7 @@ void constraint_pass(const Plan& P, const std::vector<double>& x, std::vector<do
                     for (int64_t p = P.L.ptr[i]; p < P.L.ptr[i + 1]; ++p) (*step)[P.L.col[p]] += c * P.L.val[p]; }
             }
         }
-        if (has_letd(b)) {                                        // <L_i - LETmax D_i, x> <= 0 (north_star)
+        if (has_letd(sb)) {                                       // <L_i - LETmax D_i, x> <= 0 (north_star)
             double val = letd_row_dot(P, i, b.letd_max, x, nullptr);
             double r = val > 0.0 ? val : 0.0;
             if (r != 0.0) ++nv;
@@ -240,10 +258,11 @@ void block_sweep(Plan& P, double relax) {
             int64_t m = 0;
             for (int64_t i = 0; i < V; ++i) {
                 if (P.label[i] != (int32_t)s) continue;
+                const Bounds vbn = voxel_bounds(P, i, (int32_t)s);
                 double r, n;
-                if (kind == 0) { r = slab_residual(row_dot(P.D, i, x), b.dose_lo, b.dose_hi); n = P.nD[i]; }
-                else if (kind == 1) { r = slab_residual(row_dot(P.L, i, x), b.dl_lo, b.dl_hi); n = P.nL[i]; }
-                else { double val = letd_row_dot(P, i, b.letd_max, x, nullptr); r = val > 0.0 ? val : 0.0; n = P.nT[i]; }
+                if (kind == 0) { r = slab_residual(row_dot(P.D, i, x), vbn.dose_lo, vbn.dose_hi); n = P.nD[i]; }
+                else if (kind == 1) { r = slab_residual(row_dot(P.L, i, x), vbn.dl_lo, vbn.dl_hi); n = P.nL[i]; }
+                else { double val = letd_row_dot(P, i, vbn.letd_max, x, nullptr); r = val > 0.0 ? val : 0.0; n = P.nT[i]; }
                 if (r != 0.0) ++P.sweep_viol;
                 if (!(n > 0.0)) continue;
                 ++m;
@@ -254,7 +273,7 @@ void block_sweep(Plan& P, double relax) {
                 else if (kind == 1) for (int64_t p = P.L.ptr[i]; p < P.L.ptr[i + 1]; ++p) step[P.L.col[p]] += c * P.L.val[p];
                 else {
                     for (int64_t p = P.L.ptr[i]; p < P.L.ptr[i + 1]; ++p) step[P.L.col[p]] += c * P.L.val[p];
-                    for (int64_t p = P.D.ptr[i]; p < P.D.ptr[i + 1]; ++p) step[P.D.col[p]] -= c * b.letd_max * P.D.val[p];
+                    for (int64_t p = P.D.ptr[i]; p < P.D.ptr[i + 1]; ++p) step[P.D.col[p]] -= c * vbn.letd_max * P.D.val[p];
                 }
             }
             if (m == 0) continue;
@@ -315,6 +334,31 @@ void oracle_set_option(void* h, int32_t key, double v) {
         case 9: P->one_sided_cost = v != 0.0; break;
         default: break;
     }
+}
+
+// Per-voxel values of one bound field (V floats, NaN = the structure's scalar; NULL removes the array).  A value applies where
+// the voxel's structure declares that kind of constraint / cost term.  Norms and w^ are set up again (the LETd rows
+// L_i - LETmax_i D_i change with LETmax_i).  Returns 0, or -1 (nothing changed) if a value is infinite or lo > hi on a voxel.
+int32_t oracle_set_voxel_bounds(void* h, int32_t field, const float* values) {
+    Plan* P = (Plan*)h;
+    if (field < 0 || field >= VB_N) return -1;
+    const int64_t V = P->D.n_rows;
+    std::vector<double> old = P->vb[field];
+    if (!values) P->vb[field].clear();
+    else {
+        P->vb[field].resize(V);
+        for (int64_t i = 0; i < V; ++i) P->vb[field][i] = (double)values[i];
+    }
+    bool ok = true;
+    for (int64_t i = 0; i < V && ok; ++i) {
+        if (values && std::isinf(values[i])) ok = false;
+        if (P->label[i] == 0) continue;
+        const Bounds b = voxel_bounds(*P, i, P->label[i]);
+        if (b.dose_lo > b.dose_hi || b.dl_lo > b.dl_hi) ok = false;
+    }
+    if (!ok) { P->vb[field] = old; return -1; }
+    setup(*P);
+    return 0;
 }
 
 // d = D x, l = L x over ALL rows; LETd_i = l_i / d_i where d_i > 0, else 0 (Eq. (1); R15)
@@ -514,19 +558,20 @@ void oracle_sequential_sweep(void* h, float lambda_f) {
         for (int64_t i = 0; i < P->D.n_rows; ++i) {
             int32_t s = P->label[i];
             if (s == 0) continue;
-            const Bounds& b = P->bounds[s - 1];
+            const Bounds& sb = P->bounds[s - 1];
+            const Bounds b = voxel_bounds(*P, i, s);
             const double w = b.weight < 1.0 ? b.weight : 1.0;
-            if (pass == 0 && has_dose_slab(b) && P->nD[i] > 0) {
+            if (pass == 0 && has_dose_slab(sb) && P->nD[i] > 0) {
                 double r = slab_residual(row_dot(P->D, i, x), b.dose_lo, b.dose_hi);
                 if (r != 0.0) { double c = lambda * w * r / P->nD[i];
                     for (int64_t p = P->D.ptr[i]; p < P->D.ptr[i + 1]; ++p) x[P->D.col[p]] -= c * P->D.val[p]; }
             }
-            if (pass == 1 && has_dl_slab(b) && P->nL[i] > 0) {
+            if (pass == 1 && has_dl_slab(sb) && P->nL[i] > 0) {
                 double r = slab_residual(row_dot(P->L, i, x), b.dl_lo, b.dl_hi);
                 if (r != 0.0) { double c = lambda * w * r / P->nL[i];
                     for (int64_t p = P->L.ptr[i]; p < P->L.ptr[i + 1]; ++p) x[P->L.col[p]] -= c * P->L.val[p]; }
             }
-            if (pass == 2 && has_letd(b) && P->nT[i] > 0) {
+            if (pass == 2 && has_letd(sb) && P->nT[i] > 0) {
                 double val = letd_row_dot(*P, i, b.letd_max, x, nullptr);
                 if (val > 0.0) { double c = lambda * w * val / P->nT[i];
                     for (int64_t p = P->L.ptr[i]; p < P->L.ptr[i + 1]; ++p) x[P->L.col[p]] -= c * P->L.val[p];

@@ -17,6 +17,7 @@ _LIB = os.path.join(_HERE, "libfredopt_oracle.so")
 
 OPT_ETA, OPT_REDUCTIONS, OPT_ACCEPT_CHECK, OPT_MAX_TRIALS, OPT_RESET = 0, 1, 2, 3, 4
 OPT_BLOCK_SEQUENTIAL, OPT_NORMALIZE_GRAD, OPT_ONE_SIDED_COST = 7, 8, 9
+VB_DOSE_LO, VB_DOSE_HI, VB_DL_LO, VB_DL_HI, VB_LETD_MAX, VB_DOSE_REF, VB_DL_REF = range(7)
 
 
 def build(force: bool = False) -> str:
@@ -42,6 +43,8 @@ def _load():
         lib.oracle_set_x64.argtypes = [vp, vp]
         lib.oracle_get_x.argtypes = [vp, vp]
         lib.oracle_set_option.argtypes = [vp, i32, f64]
+        lib.oracle_set_voxel_bounds.restype = i32
+        lib.oracle_set_voxel_bounds.argtypes = [vp, i32, vp]
         lib.oracle_dose_let.argtypes = [vp, vp, vp, vp, vp]
         lib.oracle_dose_let_rows.argtypes = [vp, vp, vp, i64, vp, vp, vp]
         lib.oracle_transpose.argtypes = [vp, vp, vp, i32, vp, vp]
@@ -116,6 +119,12 @@ class Oracle:
 
     def set_option(self, key, value):
         self._lib.oracle_set_option(self._h, key, float(value))
+
+    def set_voxel_bounds(self, field, values):
+        """values: V floats (NaN = the structure's scalar) or None (remove the array)."""
+        v = None if values is None else np.ascontiguousarray(values, np.float32)
+        if self._lib.oracle_set_voxel_bounds(self._h, int(field), _p(v)) != 0:
+            raise ValueError("per-voxel bounds: infinite value or lo > hi on a voxel")
 
     # ---- the calls of the boundary
     def dose_let(self, x=None):

@@ -47,20 +47,28 @@ def bounds_rows(*rows):
 class DenseReference:
     """Dense restatement of SURVEY.md sec. 8c, written separately from the oracle (numpy mat-vecs)."""
 
-    def __init__(self, Dd, Ld, labels, bounds):
+    def __init__(self, Dd, Ld, labels, bounds, vb=None):
+        """vb: optional {field index 1..7 of a bounds row: per-voxel float32 array, NaN = the structure's scalar} (PAPER.md:161:
+        bounds "defined for each point in the image space"); the structure's scalars decide which sets / cost terms exist."""
         self.D, self.L, self.lab = Dd, Ld, labels
         self.b = np.asarray(bounds, dtype=F32).astype(np.float64)
+        self.vb = {k: np.asarray(v, dtype=F32).astype(np.float64) for k, v in (vb or {}).items()}
+
+        def val(i, s, k):
+            a = self.vb.get(k)
+            return a[i] if a is not None and not np.isnan(a[i]) else self.b[s - 1, k]
+        self.val = val
         sets = []   # (row vector a, lo, hi, structure)
         for i, s in enumerate(labels):
             if s == 0:
                 continue
             w, dlo, dhi, llo, lhi, tmax, _, _ = self.b[s - 1]
             if not (np.isnan(dlo) and np.isnan(dhi)):
-                sets.append((Dd[i], dlo, dhi, s))
+                sets.append((Dd[i], val(i, s, 1), val(i, s, 2), s))
             if not (np.isnan(llo) and np.isnan(lhi)):
-                sets.append((Ld[i], llo, lhi, s))
+                sets.append((Ld[i], val(i, s, 3), val(i, s, 4), s))
             if not np.isnan(tmax):
-                sets.append((Ld[i] - tmax * Dd[i], NAN, 0.0, s))
+                sets.append((Ld[i] - val(i, s, 5) * Dd[i], NAN, 0.0, s))
         self.sets = sets
         self.W = sum(self.b[s - 1, 0] for a, lo, hi, s in sets if a @ a > 0)
         self.what = self.b[:, 0] / self.W if self.W > 0 else self.b[:, 0] * 0
@@ -90,9 +98,9 @@ class DenseReference:
                 continue
             dref, lref = self.b[s - 1, 6], self.b[s - 1, 7]
             if not np.isnan(dref):
-                phi += self.what[s - 1] * (dref - d[i]) ** 2
+                phi += self.what[s - 1] * (self.val(i, s, 6) - d[i]) ** 2
             if not np.isnan(lref):
-                phi += self.what[s - 1] * (lref - l[i]) ** 2
+                phi += self.what[s - 1] * (self.val(i, s, 7) - l[i]) ** 2
         return phi
 
     def grad(self, x):
@@ -103,9 +111,9 @@ class DenseReference:
                 continue
             dref, lref = self.b[s - 1, 6], self.b[s - 1, 7]
             if not np.isnan(dref):
-                g += 2 * self.what[s - 1] * (d[i] - dref) * self.D[i]
+                g += 2 * self.what[s - 1] * (d[i] - self.val(i, s, 6)) * self.D[i]
             if not np.isnan(lref):
-                g += 2 * self.what[s - 1] * (l[i] - lref) * self.L[i]
+                g += 2 * self.what[s - 1] * (l[i] - self.val(i, s, 7)) * self.L[i]
         return g
 
     def iterate(self, x, n, lam, beta0, a, max_trials=200, reductions=1, eta=1.0):
@@ -856,3 +864,126 @@ def test_pin26_step_size_sequence_belongs_to_the_plan():
         o.iterate(1, 1.0, 0.5, 0.8)
     o.iterate(1, 1.0, 0.5, 0.9)
     assert o.stats()["s"] > s1 and o.stats()["k"] == 5
+
+
+# ----------------------------------------------------------------------------- per-voxel bounds and references
+def _voxel_bound_plan():
+    D, L, labels, x0 = pg.random_small_plan(7, V=48, S=9, n_struct=3, same_pattern=False)
+    b = bounds_rows(dict(weight=1.0, dose_lo=1.2, dose_hi=1.6, dose_ref=1.4),
+                    dict(weight=2.5, dose_hi=0.9, dl_hi=4.0, dl_lo=0.5, letd_max=5.0, dl_ref=3.0),
+                    dict(weight=0.5, letd_max=4.0, dose_lo=0.3))
+    return D, L, labels, x0, b
+
+
+def test_pin27_per_voxel_arrays_of_the_structure_scalars_change_nothing():
+    """Per-voxel arrays filled with the structures' own scalars (or with NaN = "use the scalar") reproduce the trajectory of the
+    scalar plan BIT FOR BIT: the per-voxel path evaluates the same formulas (Eq. (2))."""
+    D, L, labels, x0, b = _voxel_bound_plan()
+    base = orc.Oracle.create(48, 9, D, L, labels, b)
+    full = orc.Oracle.create(48, 9, D, L, labels, b)
+    nan_ = orc.Oracle.create(48, 9, D, L, labels, b)
+    for field in range(7):
+        col = np.where(labels > 0, b[np.maximum(labels, 1) - 1, field + 1], NAN).astype(F32)
+        full.set_voxel_bounds(field, col)
+        nan_.set_voxel_bounds(field, np.full(48, NAN, F32))
+    for o in (base, full, nan_):
+        o.set_x(x0); o.iterate(9, 1.3, 0.7, 0.9)
+    assert np.array_equal(base.get_x(), full.get_x()) and np.array_equal(base.get_x(), nan_.get_x())
+    assert base.stats() == full.stats() == nan_.stats()
+    assert base.proximity() == full.proximity() and base.cost() == full.cost()
+    # removing an array restores the scalar
+    full.set_voxel_bounds(orc.VB_DOSE_HI, np.full(48, 5.0, F32))
+    assert full.proximity() != base.proximity()
+    full.set_voxel_bounds(orc.VB_DOSE_HI, None)
+    assert full.proximity() == base.proximity()
+
+
+@pytest.mark.parametrize("block", [0, 1])
+def test_pin28_per_voxel_bounds_dense_brute_force(block):
+    """Bounds and references that genuinely vary from voxel to voxel against the separate dense restatement: dose / cDL slabs,
+    the LETd limit (its row L_i - LETmax_i D_i and norm change with the voxel's LETmax_i) and both cost references.  Guards
+    voxel_bounds() and every place the oracle reads a bound (a place still reading the structure scalar fails)."""
+    D, L, labels, x0, b = _voxel_bound_plan()
+    Dd, Ld = csr_to_dense(D, 9), csr_to_dense(L, 9)
+    u = pg.uniform01_array(77, 7 * 48).reshape(7, 48)
+    vb = {}
+    for field in range(7):
+        k = field + 1
+        col = b[np.maximum(labels, 1) - 1, k].astype(np.float64)
+        scale = 0.8 + 0.4 * u[field]                                   # +-20 % around the structure's value ...
+        if field in (0, 2):
+            scale = 0.7 + 0.25 * u[field]                              # (lower bounds stay below upper bounds)
+        if field in (1, 3):
+            scale = 1.0 + 0.3 * u[field]
+        arr = np.where(u[(field + 3) % 7] < 0.3, NAN, col * scale)     # ... and NaN (= scalar) on ~30 % of the voxels
+        vb[k] = arr.astype(F32)
+    o = orc.Oracle.create(48, 9, D, L, labels, b)
+    for k, arr in vb.items():
+        o.set_voxel_bounds(k - 1, arr)
+    ref = DenseReference(Dd, Ld, labels, b, vb=vb)
+    x = x0.astype(np.float64)
+    assert abs(o.stats()["W"] - ref.W) <= 1e-13 * ref.W
+    p, nv = o.proximity(x); pr, nvr = ref.proximity(x)
+    assert nv == nvr and nv > 5 and abs(p - pr) <= 1e-12 * pr
+    assert abs(o.cost(x) - ref.cost(x)) <= 1e-12 * ref.cost(x)
+    np.testing.assert_allclose(o.grad(x), ref.grad(x), rtol=1e-11, atol=1e-15)
+    # the scalar plan differs (the arrays are not a no-op)
+    o0 = orc.Oracle.create(48, 9, D, L, labels, b)
+    assert abs(o0.proximity(x)[0] - p) > 1e-3 * p
+    if not block:
+        o.set_x(x0); o.iterate(7, 1.3, 1.0, 0.9)
+        xr, s_ref = ref.iterate(x.copy(), 7, 1.3, 1.0, 0.9)
+        np.testing.assert_allclose(o.get_x(), xr, rtol=1e-10, atol=1e-13)
+        assert o.stats()["s"] == s_ref and o.proximity()[1] == ref.proximity(xr)[1]
+    else:
+        # block-sequential sweep against a dense restatement with per-voxel bounds
+        o.set_option(orc.OPT_BLOCK_SEQUENTIAL, 1); o.set_x(x0)
+        xb = x.copy()
+        for _ in range(4):
+            o.iterate(1, 1.2, 0.0, 0.5)
+            for kind in range(3):
+                for s_ in range(1, 4):
+                    rows = [i for i in range(48) if labels[i] == s_]
+                    if kind == 0 and np.isnan(b[s_ - 1, 1]) and np.isnan(b[s_ - 1, 2]) or kind == 1 and np.isnan(b[s_ - 1, 3]) and np.isnan(b[s_ - 1, 4]) \
+                            or kind == 2 and np.isnan(b[s_ - 1, 5]):
+                        continue
+                    step = np.zeros(9); m = 0
+                    for i in rows:
+                        if kind == 0:
+                            a, lo, hi = Dd[i], ref.val(i, s_, 1), ref.val(i, s_, 2)
+                        elif kind == 1:
+                            a, lo, hi = Ld[i], ref.val(i, s_, 3), ref.val(i, s_, 4)
+                        else:
+                            a, lo, hi = Ld[i] - ref.val(i, s_, 5) * Dd[i], NAN, 0.0
+                        n2 = a @ a
+                        if n2 > 0:
+                            m += 1
+                            step += DenseReference.resid(a @ xb, lo, hi) / n2 * a
+                    if m:
+                        xb = xb - float(F32(1.2)) * min(float(b[s_ - 1, 0]), 1.0) / m * step
+            xb = np.maximum(xb, 0.0)
+        np.testing.assert_allclose(o.get_x(), xb, rtol=1e-11, atol=1e-14)
+
+
+def test_pin29_per_voxel_letd_limit_lands_on_the_voxels_own_boundary():
+    """Single LETd half-space with a per-voxel limit: lambda = 1 lands on <L_i - t_i D_i, x> = 0 for the VOXEL'S t_i (closed
+    form), i.e. LETd_i = t_i afterwards; with the structure scalar it would land elsewhere."""
+    Dd = f32mat(np.array([[0.5, 0.2, 0.9, 0.4]]))
+    Ld = f32mat(np.array([[2.5, 2.2, 1.0, 3.1]]))
+    x0 = np.array([1.0, 1.0, 1.0, 1.0], F32)
+    o = make_oracle(Dd, Ld, [1], bounds_rows(dict(letd_max=3.0)))
+    o.set_voxel_bounds(orc.VB_LETD_MAX, np.array([2.5], F32))
+    o.set_x(x0); o.iterate(1, 1.0, 0.0, 0.5)
+    d, l, t = o.dose_let()
+    assert abs(t[0] - 2.5) < 1e-12
+    _, _, nT = o.norms()
+    a = Ld[0] - 2.5 * Dd[0]
+    assert abs(nT[0] - a @ a) <= 1e-15 * (a @ a)
+    # invalid: lo > hi on a voxel, infinite value -> refused, state unchanged
+    o2 = make_oracle(Dd, Ld, [1], bounds_rows(dict(dose_lo=1.0, dose_hi=2.0)))
+    with pytest.raises(ValueError):
+        o2.set_voxel_bounds(orc.VB_DOSE_LO, np.array([2.5], F32))
+    with pytest.raises(ValueError):
+        o2.set_voxel_bounds(orc.VB_DOSE_HI, np.array([np.inf], F32))
+    o2.set_x(x0)
+    assert o2.proximity()[1] == 0 or o2.proximity()[1] == 1
