@@ -182,6 +182,22 @@ int fredopt_dose_let(fredopt_plan *plan, const float *x, float *dose, float *let
  * beta0 and a are latched at the first call after create / RESET.  Asynchronous (device work only). */
 int fredopt_iterate(fredopt_plan *plan, int32_t n_iter, float lambda, float beta0, float a);
 
+/* Per-voxel bounds and references (bounds are "upper and lower constraints for all organs or defined for each
+ * point in the image space"; Eq. (2): per-voxel Dref_i, cDLref_i).  values: n_rows floats, voxel-indexed,
+ * host or device; NaN = the voxel keeps its structure's scalar; NULL removes the field's array.  A value applies where the
+ * voxel's structure declares that kind of constraint (dose slab: dose_lo or dose_hi; cDL slab; LETd limit) or that cost term
+ * (dose_ref, dl_ref): which sets and terms exist stays with the structure.  With FREDOPT_VB_LETD_MAX the norms of the rows
+ * L_i - LETmax_i D_i, the participating sets and the normalised weights are set up again.  Errors: INVALID_ARG (infinite value,
+ * lo > hi on a voxel; the plan is unchanged).  Synchronises. */
+#define FREDOPT_VB_DOSE_LO   0
+#define FREDOPT_VB_DOSE_HI   1
+#define FREDOPT_VB_DL_LO     2
+#define FREDOPT_VB_DL_HI     3
+#define FREDOPT_VB_LETD_MAX  4
+#define FREDOPT_VB_DOSE_REF  5
+#define FREDOPT_VB_DL_REF    6
+int fredopt_set_voxel_bounds(fredopt_plan *plan, int32_t field, const float *values);
+
 /* Proximity p(x) = 1/2 sum_{k in P} w^_k r_k^2 / |a_k|^2 and the number of declared sets with r_k != 0.
  * x: n_cols floats or NULL = the plan's x.  prox, n_violated: HOST pointers.  Synchronises. */
 int fredopt_proximity(fredopt_plan *plan, const float *x, double *prox, int64_t *n_violated);

@@ -75,6 +75,24 @@ struct DevState {
     int flags;                 // bit 0: step along g/|g| (R9 option); bit 1: one-sided cDL cost (R11 option)
 };
 
+// Per-voxel bounds and references (bounds "defined for each point in the image space"; Eq. (2), PAPER.md:207-210:
+// Dref_i, cDLref_i): per field an optional row-indexed array of EFFECTIVE values (the voxel's own value, else the structure's
+// scalar); a null pointer = the structure's scalar everywhere.  Which kinds / cost terms a row has stays with its structure.
+enum : int { VB_DOSE_LO = 0, VB_DOSE_HI, VB_DL_LO, VB_DL_HI, VB_LETD_MAX, VB_DOSE_REF, VB_DL_REF, VB_N };
+struct VoxBounds { const double* f[VB_N]; };
+struct RowBounds { double dose_lo, dose_hi, dl_lo, dl_hi, letd_max, dose_ref, dl_ref; };
+__device__ __forceinline__ RowBounds row_bounds(const StructInfo& T, const VoxBounds& vb, long long r) {
+    RowBounds b;
+    b.dose_lo = vb.f[VB_DOSE_LO] ? vb.f[VB_DOSE_LO][r] : T.dose_lo;
+    b.dose_hi = vb.f[VB_DOSE_HI] ? vb.f[VB_DOSE_HI][r] : T.dose_hi;
+    b.dl_lo = vb.f[VB_DL_LO] ? vb.f[VB_DL_LO][r] : T.dl_lo;
+    b.dl_hi = vb.f[VB_DL_HI] ? vb.f[VB_DL_HI][r] : T.dl_hi;
+    b.letd_max = vb.f[VB_LETD_MAX] ? vb.f[VB_LETD_MAX][r] : T.letd_max;
+    b.dose_ref = vb.f[VB_DOSE_REF] ? vb.f[VB_DOSE_REF][r] : T.dose_ref;
+    b.dl_ref = vb.f[VB_DL_REF] ? vb.f[VB_DL_REF][r] : T.dl_ref;
+    return b;
+}
+
 // One work item: `len` VALUES per matrix (multiple of 4) starting at value `start` (multiple of 4) of the value arrays,
 // i.e. len / R entries starting at entry start / R of the index array; `seg` & 0xFF = structure - 1 (selects which value
 // arrays are read).  Forward items (one block row) carry the number of real rows of the block (1..R; the last block of a
@@ -231,10 +249,10 @@ __device__ __forceinline__ double slab_residual(double val, double lo, double hi
 // Residuals of Fig. 2 for one labelled row at (dv, lv) in simultaneous form: the coefficients of D_i and L_i in the step,
 //   u_i = w^ r_dose/|D_i|^2 - LETmax w^ r_letd/|L_i - LETmax D_i|^2 ,  v_i = w^ r_dl/|L_i|^2 + w^ r_letd/|...|^2 ,
 // and the row's share of the violated-set count, the proximity and chi^2.
-__device__ __forceinline__ void row_residual(const StructInfo& T, int one_sided, double dv, double lv, double nD, double nL,
-                                             double nT, double& u, double& v, long long& cnt, double& prox, double& phi) {
-    const int f = T.flags;
-    const double w = T.what;
+__device__ __forceinline__ void row_residual(const StructInfo& S_, const RowBounds& T, int one_sided, double dv, double lv, double nD,
+                                             double nL, double nT, double& u, double& v, long long& cnt, double& prox, double& phi) {
+    const int f = S_.flags;
+    const double w = S_.what;
     double cD = 0.0, cL = 0.0, cT = 0.0;
     if (f & F_DOSE_SLAB) {
         const double r = slab_residual(dv, T.dose_lo, T.dose_hi);
@@ -377,7 +395,7 @@ k_forward(long long n, const Item* __restrict__ items, const int32_t* __restrict
           const double* __restrict__ x,
           double* __restrict__ oD, double* __restrict__ oL,                // EPI_STORE*, EPI_CPART, EPI_RESID: row-indexed
           const GatherVec pq,                                              // EPI_STORE_PQ: cost residuals (Eq. 2)
-          const StructInfo* __restrict__ tab, double* __restrict__ cpart,  // EPI_STORE_PQ / EPI_CPART: per block row
+          const StructInfo* __restrict__ tab, const VoxBounds vb, double* __restrict__ cpart,  // EPI_STORE_PQ / EPI_CPART: per block row
           const DevState* __restrict__ st,                                 // EPI_STORE_PQ (cost form)
           float* __restrict__ fD, float* __restrict__ fL, int letd_out,    // EPI_F32VOX: voxel-indexed
           const ResidArgs ra)                                              // EPI_RESID: residual / violation epilogue (a7)
@@ -426,12 +444,14 @@ k_forward(long long n, const Item* __restrict__ items, const int32_t* __restrict
                     if (EPI == EPI_STORE_PQ) {      // p_i = 2 w^ (d_i - Dref), q_i = 2 w^ (l_i - cDLref): grad chi^2 = D^T p + L^T q
                         const StructInfo& T = tab[seg];
                         const int one_sided = st->flags & SF_ONE_SIDED;
+                        const double dref = vb.f[VB_DOSE_REF] ? vb.f[VB_DOSE_REF][r] : T.dose_ref;
+                        const double lref = vb.f[VB_DL_REF] ? vb.f[VB_DL_REF][r] : T.dl_ref;
                         double pv, qv;
-                        cost_residuals(T.flags, T.what, T.dose_ref, T.dl_ref, one_sided, dv, lv, pv, qv);
+                        cost_residuals(T.flags, T.what, dref, lref, one_sided, dv, lv, pv, qv);
                         gv_store(pq, r, pv, qv);
                         // the row's share of chi^2(x) (Eq. 2): the accept test of Fig. 3 compares against it
-                        if (T.flags & F_DOSE_REF) { const double e = T.dose_ref - dv; csum += T.what * e * e; }
-                        if (T.flags & F_DL_REF) { const double e = T.dl_ref - lv; if (!(one_sided && e > 0.0)) csum += T.what * e * e; }
+                        if (T.flags & F_DOSE_REF) { const double e = dref - dv; csum += T.what * e * e; }
+                        if (T.flags & F_DL_REF) { const double e = lref - lv; if (!(one_sided && e > 0.0)) csum += T.what * e * e; }
                     }
                     if (EPI == EPI_CPART) {
                         const StructInfo& T = tab[seg];
@@ -440,7 +460,8 @@ k_forward(long long n, const Item* __restrict__ items, const int32_t* __restrict
                     }
                     if (EPI == EPI_RESID) {         // residuals / violations of Fig. 2 at x, in the epilogue of the fused pass
                         double u, v;
-                        row_residual(tab[seg], ra.st->flags & SF_ONE_SIDED, dv, lv, ra.nD[r], ra.nL[r], ra.nT[r], u, v, rcnt, rprox, rphi);
+                        row_residual(tab[seg], row_bounds(tab[seg], vb, r), ra.st->flags & SF_ONE_SIDED, dv, lv, ra.nD[r], ra.nL[r], ra.nT[r], u, v,
+                                     rcnt, rprox, rphi);
                         if (ra.uv.pair) gv_store(ra.uv, r, u, v);
                     }
                 }

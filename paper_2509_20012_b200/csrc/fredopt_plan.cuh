@@ -113,6 +113,8 @@ struct fredopt_plan {
     uint8_t *mode_union = nullptr, *mode_con = nullptr, *mode_cost = nullptr, *mode_fixed = nullptr;  // mode_fixed: [4][max_seg]
     int max_seg = 1;
     DevState* st = nullptr;
+    VoxBounds vb = {};                     // per-voxel bounds: row-indexed effective values per field (null = structure scalars)
+    double* vb_buf[VB_N] = {};             // the arrays behind vb (owned)
     // vectors (fp64)
     double *x = nullptr, *g = nullptr, *xtmp = nullptr;                       // [S]
     float* xstage = nullptr;                                                   // [S] staging of host spot-weight vectors
@@ -215,3 +217,6 @@ void launch_forward(fredopt_plan* P, const RowSet& R, const uint8_t* mode, const
 void launch_transpose(fredopt_plan* P, int tepi, const RowSet& R, const uint8_t* mode, const GatherVec& vec, double* g_out,
                       double* x, float* f_out);
 void launch_finalize(fredopt_plan* P, int n_part);
+void invalidate_graphs(fredopt_plan* P);                         // captured launches hold kernel arguments: capture again
+// ---- plan_build.cu
+int recount_sets(fredopt_plan* P, bool letd_norms);              // norms of the LETd rows (per-voxel limits), set counts, W, w^

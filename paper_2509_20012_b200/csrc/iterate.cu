@@ -52,11 +52,11 @@ void launch_fwd_kernel(fredopt_plan* P, int epi, const RowSet& R, long long b0, 
     const bool i16 = R.col16 != nullptr;
 #define FWD_CALL(RB, I16)                                                                                                        \
     switch (epi) {                                                                                                               \
-        case EPI_STORE: klaunch(P, k_forward<EPI_STORE, RB, I16>, g, FWD_THREADS, n, items, iblk, wq, vox, mode, col, R.valD, R.valL, x, oD, oL, pq, tab, cpart, P->st, fD, fL, letd_out, ra); break;       \
-        case EPI_STORE_PQ: klaunch(P, k_forward<EPI_STORE_PQ, RB, I16>, g, FWD_THREADS, n, items, iblk, wq, vox, mode, col, R.valD, R.valL, x, oD, oL, pq, tab, cpart, P->st, fD, fL, letd_out, ra); break; \
-        case EPI_CPART: klaunch(P, k_forward<EPI_CPART, RB, I16>, g, FWD_THREADS, n, items, iblk, wq, vox, mode, col, R.valD, R.valL, x, oD, oL, pq, tab, cpart, P->st, fD, fL, letd_out, ra); break;       \
-        case EPI_F32VOX: klaunch(P, k_forward<EPI_F32VOX, RB, I16>, g, FWD_THREADS, n, items, iblk, wq, vox, mode, col, R.valD, R.valL, x, oD, oL, pq, tab, cpart, P->st, fD, fL, letd_out, ra); break;     \
-        default: klaunch(P, k_forward<EPI_RESID, RB, I16>, g, FWD_THREADS, n, items, iblk, wq, vox, mode, col, R.valD, R.valL, x, oD, oL, pq, tab, cpart, P->st, fD, fL, letd_out, ra); break;              \
+        case EPI_STORE: klaunch(P, k_forward<EPI_STORE, RB, I16>, g, FWD_THREADS, n, items, iblk, wq, vox, mode, col, R.valD, R.valL, x, oD, oL, pq, tab, P->vb, cpart, P->st, fD, fL, letd_out, ra); break;       \
+        case EPI_STORE_PQ: klaunch(P, k_forward<EPI_STORE_PQ, RB, I16>, g, FWD_THREADS, n, items, iblk, wq, vox, mode, col, R.valD, R.valL, x, oD, oL, pq, tab, P->vb, cpart, P->st, fD, fL, letd_out, ra); break; \
+        case EPI_CPART: klaunch(P, k_forward<EPI_CPART, RB, I16>, g, FWD_THREADS, n, items, iblk, wq, vox, mode, col, R.valD, R.valL, x, oD, oL, pq, tab, P->vb, cpart, P->st, fD, fL, letd_out, ra); break;       \
+        case EPI_F32VOX: klaunch(P, k_forward<EPI_F32VOX, RB, I16>, g, FWD_THREADS, n, items, iblk, wq, vox, mode, col, R.valD, R.valL, x, oD, oL, pq, tab, P->vb, cpart, P->st, fD, fL, letd_out, ra); break;     \
+        default: klaunch(P, k_forward<EPI_RESID, RB, I16>, g, FWD_THREADS, n, items, iblk, wq, vox, mode, col, R.valD, R.valL, x, oD, oL, pq, tab, P->vb, cpart, P->st, fD, fL, letd_out, ra); break;              \
     }
     FREDOPT_DISPATCH(R.R, i16, FWD_CALL)
 #undef FWD_CALL
@@ -114,7 +114,7 @@ static int res_grid(fredopt_plan* P) {
 
 static void launch_residual(fredopt_plan* P, double* d, double* l, int use_beta, int final, int write_uv) {
     const int g = res_grid(P);
-    klaunch(P, k_residual, g, ROW_THREADS, P->act.n_rows, P->act.rseg, P->tab, P->st, d, l, P->Dg, P->Lg, P->nD, P->nL, P->nT, P->uv, P->pq,
+    klaunch(P, k_residual, g, ROW_THREADS, P->act.n_rows, P->act.rseg, P->tab, P->vb, P->st, d, l, P->Dg, P->Lg, P->nD, P->nL, P->nT, P->uv, P->pq,
             P->x, P->g, P->S, P->part_prox, P->part_phi, P->part_cnt, use_beta, final, write_uv);
 }
 
@@ -145,7 +145,7 @@ static void enqueue_block_sweep(fredopt_plan* P) {
             ev_end(P);
             ev_begin(P, FREDOPT_PASS_RESIDUAL);
             const int gr = grid_for(nr, ROW_THREADS, P->sm_count * 4 < MAX_PARTIALS ? P->sm_count * 4 : MAX_PARTIALS);
-            klaunch(P, k_block_residual, gr, ROW_THREADS, rb, re, s, kind, P->tab, P->st, P->d, P->l, P->nD, P->nL, P->nT, P->uv, P->part_prox);
+            klaunch(P, k_block_residual, gr, ROW_THREADS, rb, re, s, kind, P->tab, P->vb, P->st, P->d, P->l, P->nD, P->nL, P->nT, P->uv, P->part_prox);
             ev_end(P);
             const long long m = (long long)T.part_kind[kind];
             const long long ib = A.t_seg_item_begin.empty() ? 0 : A.t_seg_item_begin[s], ie = A.t_seg_item_begin.empty() ? 0 : A.t_seg_item_begin[s + 1];
@@ -177,7 +177,7 @@ static int enqueue_iteration(fredopt_plan* P, bool sa) {
             ev_begin(P, FREDOPT_PASS_SELECT);
             klaunch(P, k_select, 1, 1024, P->st, P->gpart, P->act.t_n_items ? grid_for(P->S, 256, 1 << 30) : 0, P->cpart, cpart_count(P),
                     P->part_phi, P->act.n == 0 ? 0 : t == 0 ? (int)P->act.n : res_grid(P), P->act.n_rows,
-                    P->act.rseg, P->tab, P->d, P->l, P->Dg, P->Lg);                                     // a4, a6: beta
+                    P->act.rseg, P->tab, P->vb, P->d, P->l, P->Dg, P->Lg);                                     // a4, a6: beta
             ev_end(P);
             ev_begin(P, FREDOPT_PASS_RESIDUAL);
             const int last = t == P->reductionsN - 1 && !P->block_sequential;
@@ -199,6 +199,10 @@ static int enqueue_iteration(fredopt_plan* P, bool sa) {
     return (int)(P->launches - before);
 }
 
+
+void invalidate_graphs(fredopt_plan* P) {
+    for (int i = 0; i < 8; ++i) if (P->gexec[i]) { cudaGraphExecDestroy(P->gexec[i]); P->gexec[i] = nullptr; }
+}
 
 void state_init(fredopt_plan* P) {
     k_set_params<<<1, 1, 0, P->stream>>>(P->st, 1.0, 0.0, 0.5, 1.0, 200, 1, 0, 2);

@@ -61,6 +61,33 @@ __global__ void k_gather_uv(const float* __restrict__ u, const float* __restrict
     }
 }
 
+// per-voxel values of one bound field (voxel-indexed fp32, NaN = the structure's scalar) -> row-indexed effective fp64 values;
+// *bad |= 1 on an infinite value
+__global__ void k_vb_fill(long long n_rows, const int32_t* __restrict__ vox, const int16_t* __restrict__ rseg,
+                          const StructInfo* __restrict__ tab, int field, const float* __restrict__ values, double* __restrict__ out,
+                          int* __restrict__ bad) {
+    for (long long a = (long long)blockIdx.x * blockDim.x + threadIdx.x; a < n_rows; a += (long long)gridDim.x * blockDim.x) {
+        const int sg = rseg[a];
+        if (sg < 0) { out[a] = 0.0; continue; }
+        const StructInfo& T = tab[sg];
+        const double sc = field == VB_DOSE_LO ? T.dose_lo : field == VB_DOSE_HI ? T.dose_hi : field == VB_DL_LO ? T.dl_lo
+                        : field == VB_DL_HI ? T.dl_hi : field == VB_LETD_MAX ? T.letd_max : field == VB_DOSE_REF ? T.dose_ref : T.dl_ref;
+        const float v = values[vox[a]];
+        if (isinf(v)) *bad = 1;
+        out[a] = isnan(v) ? sc : (double)v;
+    }
+}
+// lo <= hi on every row (comparisons with NaN = absent are false)
+__global__ void k_vb_check(long long n_rows, const int16_t* __restrict__ rseg, const StructInfo* __restrict__ tab, const VoxBounds vb,
+                           int* __restrict__ bad) {
+    for (long long a = (long long)blockIdx.x * blockDim.x + threadIdx.x; a < n_rows; a += (long long)gridDim.x * blockDim.x) {
+        const int sg = rseg[a];
+        if (sg < 0) continue;
+        const RowBounds B = row_bounds(tab[sg], vb, a);
+        if (B.dose_lo > B.dose_hi || B.dl_lo > B.dl_hi) *bad = 1;
+    }
+}
+
 // read-only streaming sum (practical ceiling of a 100%-read pass): 8 independent 128-bit loads per thread
 __global__ void __launch_bounds__(256)
 k_stream_read(const int4* __restrict__ p, long long n16, int* __restrict__ sink) {

@@ -20,7 +20,7 @@ __global__ void k_set_params(DevState* st, double lambda, double beta0, double a
 // chi^2 of Eq. (2) at x - b g from the stored products: d - b Dg, l - b Lg (exact: the products are linear in x).  All
 // threads of the CTA take part; the value is valid in thread 0.
 __device__ __forceinline__ double cost_along(double b, long long n, const int16_t* __restrict__ rseg,
-                                             const StructInfo* __restrict__ tab, const double* __restrict__ d,
+                                             const StructInfo* __restrict__ tab, const VoxBounds& vb, const double* __restrict__ d,
                                              const double* __restrict__ l, const double* __restrict__ Dg,
                                              const double* __restrict__ Lg, int one_sided, double* sm) {
     double phi = 0.0;
@@ -28,8 +28,10 @@ __device__ __forceinline__ double cost_along(double b, long long n, const int16_
         const int sg = rseg[a];
         if (sg < 0) continue;                                          // padding row of a ragged block
         const StructInfo& T = tab[sg];
-        if (T.flags & F_DOSE_REF) { const double e = T.dose_ref - fma(-b, Dg[a], d[a]); phi += T.what * e * e; }
-        if (T.flags & F_DL_REF) { const double e = T.dl_ref - fma(-b, Lg[a], l[a]); if (!(one_sided && e > 0.0)) phi += T.what * e * e; }
+        const double dref = vb.f[VB_DOSE_REF] ? vb.f[VB_DOSE_REF][a] : T.dose_ref;
+        const double lref = vb.f[VB_DL_REF] ? vb.f[VB_DL_REF][a] : T.dl_ref;
+        if (T.flags & F_DOSE_REF) { const double e = dref - fma(-b, Dg[a], d[a]); phi += T.what * e * e; }
+        if (T.flags & F_DL_REF) { const double e = lref - fma(-b, Lg[a], l[a]); if (!(one_sided && e > 0.0)) phi += T.what * e * e; }
     }
     return block_sum(phi, sm);
 }
@@ -61,8 +63,8 @@ __device__ __forceinline__ double strided_sum(const double* __restrict__ v, int 
 __global__ void __launch_bounds__(1024)
 k_select(DevState* st, const double* __restrict__ gpart, int n_gpart, const double* __restrict__ cpart, int n_part,
          const double* __restrict__ phipart, int n_phipart,
-         long long n, const int16_t* __restrict__ rseg, const StructInfo* __restrict__ tab, const double* __restrict__ d,
-         const double* __restrict__ l, const double* __restrict__ Dg, const double* __restrict__ Lg) {
+         long long n, const int16_t* __restrict__ rseg, const StructInfo* __restrict__ tab, const VoxBounds vb,
+         const double* __restrict__ d, const double* __restrict__ l, const double* __restrict__ Dg, const double* __restrict__ Lg) {
     pdl_wait();
     pdl_trigger();
     __shared__ double sm[32];
@@ -101,7 +103,7 @@ k_select(DevState* st, const double* __restrict__ gpart, int n_gpart, const doub
     if (threadIdx.x == 0) { s_go = gg > 0.0; st->gg = gg; st->c = cc; st->beta_acc = 0.0; }
     __syncthreads();
     if (!s_go) return;
-    const double phi0 = cost_along(0.0, n, rseg, tab, d, l, Dg, Lg, 1, sm);     // valid in thread 0
+    const double phi0 = cost_along(0.0, n, rseg, tab, vb, d, l, Dg, Lg, 1, sm);     // valid in thread 0
     const long long mt = st->max_trials;
     for (long long t = 0; t < mt; ++t) {
         __syncthreads();
@@ -114,7 +116,7 @@ k_select(DevState* st, const double* __restrict__ gpart, int n_gpart, const doub
         const double b = s_b;
         double phi = 0.0;
         const int chk = st->accept_check;
-        if (chk) phi = cost_along(b, n, rseg, tab, d, l, Dg, Lg, 1, sm);
+        if (chk) phi = cost_along(b, n, rseg, tab, vb, d, l, Dg, Lg, 1, sm);
         if (threadIdx.x == 0) {
             const int ok = !chk || phi < phi0;
             if (ok) { st->beta_acc = b; st->last_beta = (flags & SF_NORMALIZE_GRAD) ? b * sqrt(gg) : b; }
@@ -131,7 +133,7 @@ k_select(DevState* st, const double* __restrict__ gpart, int n_gpart, const doub
 // plus partial sums of the proximity, chi^2 and the violation count (fixed grid, fixed order); if not final
 // (another reduction of Fig. 3 follows), the cost residuals p, q at x'.
 __global__ void __launch_bounds__(ROW_THREADS)
-k_residual(long long n, const int16_t* __restrict__ rseg, const StructInfo* __restrict__ tab, DevState* st,
+k_residual(long long n, const int16_t* __restrict__ rseg, const StructInfo* __restrict__ tab, const VoxBounds vb, DevState* st,
            double* __restrict__ d, double* __restrict__ l, const double* __restrict__ Dg, const double* __restrict__ Lg,
            const double* __restrict__ nD, const double* __restrict__ nL, const double* __restrict__ nT,
            const GatherVec uv, const GatherVec pq, double* __restrict__ x, const double* __restrict__ g, long long S,
@@ -159,16 +161,17 @@ k_residual(long long n, const int16_t* __restrict__ rseg, const StructInfo* __re
         const StructInfo& T = tab[sg];
         const int f = T.flags;
         const double w = T.what;
+        const RowBounds B = row_bounds(T, vb, a);
         if (!final) {
             double pv, qv;
-            cost_residuals(f, w, T.dose_ref, T.dl_ref, st->flags & SF_ONE_SIDED, dv, lv, pv, qv);
+            cost_residuals(f, w, B.dose_ref, B.dl_ref, st->flags & SF_ONE_SIDED, dv, lv, pv, qv);
             gv_store(pq, a, pv, qv);
-            if (f & F_DOSE_REF) { const double e = T.dose_ref - dv; phi += w * e * e; }
-            if (f & F_DL_REF) { const double e = T.dl_ref - lv; if (!((st->flags & SF_ONE_SIDED) && e > 0.0)) phi += w * e * e; }
+            if (f & F_DOSE_REF) { const double e = B.dose_ref - dv; phi += w * e * e; }
+            if (f & F_DL_REF) { const double e = B.dl_ref - lv; if (!((st->flags & SF_ONE_SIDED) && e > 0.0)) phi += w * e * e; }
             continue;
         }
         double uu, vv;
-        row_residual(T, st->flags & SF_ONE_SIDED, dv, lv, nD[a], nL[a], nT[a], uu, vv, cnt, prox, phi);
+        row_residual(T, B, st->flags & SF_ONE_SIDED, dv, lv, nD[a], nL[a], nT[a], uu, vv, cnt, prox, phi);
         if (write_uv) gv_store(uv, a, uu, vv);
     }
     if (!final) {                                                  // chi^2(x') for the next reduction's accept test
@@ -202,7 +205,7 @@ k_residual(long long n, const int16_t* __restrict__ rseg, const StructInfo* __re
 // from: coefficient c_i = r_i / |a_i|^2 (0 where the norm is 0) into the gather vector (kind 0: D; 1: L; 2: L - LETmax D),
 // the block's violated sets (integer atomics: order-independent) and partial sums of its proximity share.
 __global__ void __launch_bounds__(ROW_THREADS)
-k_block_residual(long long rb, long long re, int seg, int kind, const StructInfo* __restrict__ tab, DevState* st,
+k_block_residual(long long rb, long long re, int seg, int kind, const StructInfo* __restrict__ tab, const VoxBounds vb, DevState* st,
                  const double* __restrict__ d, const double* __restrict__ l, const double* __restrict__ nD,
                  const double* __restrict__ nL, const double* __restrict__ nT, const GatherVec uv,
                  double* __restrict__ part_prox) {
@@ -215,16 +218,17 @@ k_block_residual(long long rb, long long re, int seg, int kind, const StructInfo
     double prox = 0.0;
     unsigned long long cnt = 0;
     for (long long a = rb + (long long)blockIdx.x * blockDim.x + threadIdx.x; a < re; a += (long long)gridDim.x * blockDim.x) {
+        const RowBounds B = row_bounds(T, vb, a);
         double r, nn;
-        if (kind == 0) { r = slab_residual(d[a], T.dose_lo, T.dose_hi); nn = nD[a]; }
-        else if (kind == 1) { r = slab_residual(l[a], T.dl_lo, T.dl_hi); nn = nL[a]; }
-        else { const double val = l[a] - T.letd_max * d[a]; r = val > 0.0 ? val : 0.0; nn = nT[a]; }
+        if (kind == 0) { r = slab_residual(d[a], B.dose_lo, B.dose_hi); nn = nD[a]; }
+        else if (kind == 1) { r = slab_residual(l[a], B.dl_lo, B.dl_hi); nn = nL[a]; }
+        else { const double val = l[a] - B.letd_max * d[a]; r = val > 0.0 ? val : 0.0; nn = nT[a]; }
         if (r != 0.0) ++cnt;
         double c = 0.0;
         if (nn > 0.0 && r != 0.0) { c = r / nn; prox += 0.5 * w * r * r / nn; }
         if (kind == 0) gv_store(uv, a, c, 0.0);
         else if (kind == 1) gv_store(uv, a, 0.0, c);
-        else gv_store(uv, a, -T.letd_max * c, c);
+        else gv_store(uv, a, -B.letd_max * c, c);
     }
     const double p = block_sum(prox, sm);
     for (int o = 16; o > 0; o >>= 1) cnt += __shfl_down_sync(0xffffffffu, cnt, o);

@@ -174,6 +174,46 @@ int fredopt_spmv_transpose(fredopt_plan* P, int32_t rows, const float* u, const 
     return FREDOPT_OK;
 }
 
+int fredopt_set_voxel_bounds(fredopt_plan* P, int32_t field, const float* values) {
+    if (!P || field < 0 || field >= VB_N) return FREDOPT_INVALID_ARG;
+    const RowSet& A = P->act;
+    cudaStream_t st = P->stream;
+    VoxBounds nv = P->vb;
+    double* nbuf = nullptr;
+    if (values) {
+        const float* dv; void* fr = nullptr;
+        CKR(stage_in_f32(P, values, P->V, &dv, &fr));
+        cudaError_t e = cudaMalloc((void**)&nbuf, (size_t)(A.n_rows ? A.n_rows : 1) * 8);
+        int* bad = nullptr;
+        if (e == cudaSuccess) e = cudaMalloc((void**)&bad, sizeof(int));
+        int hbad = 0;
+        if (e == cudaSuccess) e = cudaMemsetAsync(bad, 0, sizeof(int), st);
+        if (e == cudaSuccess) {
+            nv.f[field] = nbuf;
+            if (A.n_rows) {
+                k_vb_fill<<<grid_for(A.n_rows, 256, 4096), 256, 0, st>>>(A.n_rows, A.vox, A.rseg, P->tab, field, dv, nbuf, bad);
+                k_vb_check<<<grid_for(A.n_rows, 256, 4096), 256, 0, st>>>(A.n_rows, A.rseg, P->tab, nv, bad);
+                P->launches += 2;
+            }
+            e = cudaMemcpyAsync(&hbad, bad, sizeof(int), cudaMemcpyDeviceToHost, st);
+        }
+        cudaError_t e2 = cudaStreamSynchronize(st);
+        if (e == cudaSuccess) e = e2;
+        if (e == cudaSuccess) e = cudaGetLastError();
+        cudaFree(bad); cudaFree(fr);
+        if (e != cudaSuccess || hbad) { cudaFree(nbuf); if (e != cudaSuccess) CK(e); return FREDOPT_INVALID_ARG; }   // state untouched
+    } else {
+        nv.f[field] = nullptr;
+    }
+    CK(cudaStreamSynchronize(st));                        // nothing in flight reads the old array
+    cudaFree(P->vb_buf[field]);
+    P->vb_buf[field] = nbuf;
+    P->vb = nv;
+    invalidate_graphs(P);                                 // captured launches hold the old pointers
+    if (field == VB_LETD_MAX) CKR(recount_sets(P, true)); // the LETd rows L_i - LETmax_i D_i changed: norms, participating sets, w^
+    return FREDOPT_OK;
+}
+
 int fredopt_proximity(fredopt_plan* P, const float* x, double* prox, int64_t* n_violated) {
     if (!P || (!prox && !n_violated)) return FREDOPT_INVALID_ARG;
     const double* xd;

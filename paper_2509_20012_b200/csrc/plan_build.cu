@@ -268,6 +268,47 @@ __global__ void k_count_sets(long long n_rows, const int16_t* rseg, const int32_
         atomicAdd(&T.nnz, (unsigned long long)rlen[a]);
     }
 }
+// per-voxel LETd limits: |L_i - LETmax_i D_i|^2 of every row of a structure with an LETd limit (warp per block row)
+__global__ void k_norms_letd(long long n_blk, int R, const long long* start, const int32_t* len, const int32_t* seg, const float* vD,
+                             const float* vL, const StructInfo* tab, const double* tmax_row, double* nT) {
+    const int lane = threadIdx.x & 31;
+    const long long w0 = ((long long)blockIdx.x * blockDim.x + threadIdx.x) >> 5, nw = ((long long)gridDim.x * blockDim.x) >> 5;
+    for (long long b = w0; b < n_blk; b += nw) {
+        const StructInfo& T = tab[seg[b]];
+        if (!(T.flags & F_LETD)) continue;
+        const long long s = start[b];
+        const int L = len[b];
+        for (int k = 0; k < R; ++k) {
+            const double tm = tmax_row ? tmax_row[b * R + k] : T.letd_max;
+            double c = 0.0;
+            for (int p = lane; p < L; p += 32) {
+                const double t = (double)vL[(s + p) * R + k] - tm * (double)vD[(s + p) * R + k];
+                c = fma(t, t, c);
+            }
+            c = warp_sum(c);
+            if (lane == 0) nT[b * R + k] = c;
+        }
+    }
+}
+__global__ void k_reset_set_counts(StructInfo* tab, int n) {
+    const int s = blockIdx.x * blockDim.x + threadIdx.x;
+    if (s < n) { tab[s].part = 0; tab[s].n_sets = 0; tab[s].n_zero = 0; tab[s].part_kind[0] = tab[s].part_kind[1] = tab[s].part_kind[2] = 0; }
+}
+// the set bookkeeping of k_count_sets without the row / non-zero counts
+__global__ void k_recount_sets(long long n_rows, const int16_t* rseg, const double* nD, const double* nL, const double* nT, StructInfo* tab) {
+    for (long long a = (long long)blockIdx.x * blockDim.x + threadIdx.x; a < n_rows; a += (long long)gridDim.x * blockDim.x) {
+        if (rseg[a] < 0) continue;
+        StructInfo& T = tab[rseg[a]];
+        const int f = T.flags;
+        unsigned long long sets = 0, part = 0;
+        if (f & F_DOSE_SLAB) { ++sets; part += nD[a] > 0.0; if (nD[a] > 0.0) atomicAdd(&T.part_kind[0], 1ULL); }
+        if (f & F_DL_SLAB) { ++sets; part += nL[a] > 0.0; if (nL[a] > 0.0) atomicAdd(&T.part_kind[1], 1ULL); }
+        if (f & F_LETD) { ++sets; part += nT[a] > 0.0; if (nT[a] > 0.0) atomicAdd(&T.part_kind[2], 1ULL); }
+        atomicAdd(&T.n_sets, sets);
+        atomicAdd(&T.part, part);
+        atomicAdd(&T.n_zero, sets - part);
+    }
+}
 __global__ void k_count_entries(long long n_blk, const int32_t* seg, const int32_t* ulen, StructInfo* tab) {
     for (long long b = (long long)blockIdx.x * blockDim.x + threadIdx.x; b < n_blk; b += (long long)gridDim.x * blockDim.x)
         atomicAdd(&tab[seg[b]].entries, (unsigned long long)ulen[b]);
@@ -585,6 +626,21 @@ int build_transpose(fredopt_plan* P, RowSet& R) {
     return FREDOPT_OK;
 }
 
+int recount_sets(fredopt_plan* P, bool letd_norms) {
+    cudaStream_t st = P->stream;
+    const RowSet& A = P->act;
+    const int ns = P->max_seg;
+    if (A.n && letd_norms)
+        k_norms_letd<<<grid_for(A.n * 32, 256, 1 << 16), 256, 0, st>>>(A.n, A.R, A.start, A.len, A.seg, A.valD, A.valL, P->tab, P->vb.f[VB_LETD_MAX], P->nT);
+    k_reset_set_counts<<<1, 256, 0, st>>>(P->tab, P->n_struct);
+    if (A.n_rows) k_recount_sets<<<grid_for(A.n_rows, 256, 4096), 256, 0, st>>>(A.n_rows, A.rseg, P->nD, P->nL, P->nT, P->tab);
+    k_finish_tables<<<1, 1, 0, st>>>(P->tab, P->n_struct, P->st, P->mode_union, P->mode_con, P->mode_cost, P->mode_fixed, ns);
+    CK(cudaMemcpyAsync(P->h_tab.data(), P->tab, sizeof(StructInfo) * ns, cudaMemcpyDeviceToHost, st));
+    CK(cudaStreamSynchronize(st));
+    CK(cudaGetLastError());
+    return FREDOPT_OK;
+}
+
 // Bytes the method must move in one launch of a pass: per non-zero of a row 4 B for every value array the
 // row's structure needs in that pass; per stored entry (one per block row and column of the union pattern) the stored index
 // (2 B, or 4 B in the 32-bit form); 8 B per row offset; the fp64 vectors read / written once.  The zeros a block row stores
@@ -623,6 +679,7 @@ void fredopt_destroy(fredopt_plan* P) {
     for (auto& ep : P->events) { cudaEventDestroy(ep.a); cudaEventDestroy(ep.b); }
     for (int i = 0; i < 8; ++i) if (P->gexec[i]) cudaGraphExecDestroy(P->gexec[i]);
     for (void* p : P->allocs) cudaFree(p);
+    for (int k = 0; k < VB_N; ++k) cudaFree(P->vb_buf[k]);
     if (P->owns_stream) cudaStreamDestroy(P->stream);
     delete P;
 }

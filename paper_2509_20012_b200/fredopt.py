@@ -19,13 +19,14 @@ OK, INVALID_ARG, OUT_OF_MEMORY, CUDA_ERROR, UNSUPPORTED_ARCH, UNSUPPORTED = 0, -
 OPT_ETA, OPT_REDUCTIONS, OPT_ACCEPT_CHECK, OPT_MAX_TRIALS, OPT_RESET, OPT_USE_GRAPH, OPT_TIME_PASSES, \
     OPT_BLOCK_SEQUENTIAL, OPT_NORMALIZE_GRAD, OPT_ONE_SIDED_COST, OPT_USE_PDL, OPT_WORK_QUEUE = range(12)
 ROWS_ALL, ROWS_ACTIVE = 0, 1
+VB_DOSE_LO, VB_DOSE_HI, VB_DL_LO, VB_DL_HI, VB_LETD_MAX, VB_DOSE_REF, VB_DL_REF = range(7)
 PASS_NAMES = ("forward_x", "transpose_g", "forward_g", "select", "residual", "transpose_b")
 N_PASSES = len(PASS_NAMES)
 
 # every symbol include/fredopt.h declares (tests check the library exports exactly these)
 SYMBOLS = (
     "fredopt_create", "fredopt_create_ex", "fredopt_destroy", "fredopt_set_weights", "fredopt_get_weights", "fredopt_get_weights_f64",
-    "fredopt_dose_let", "fredopt_iterate", "fredopt_proximity", "fredopt_set_option", "fredopt_get_stats",
+    "fredopt_set_voxel_bounds", "fredopt_dose_let", "fredopt_iterate", "fredopt_proximity", "fredopt_set_option", "fredopt_get_stats",
     "fredopt_spmv_forward", "fredopt_spmv_transpose", "fredopt_get_pass_times", "fredopt_get_pass_bytes",
     "fredopt_launch_count", "fredopt_stream_read", "fredopt_strerror", "fredopt_last_cuda_error",
     "fredopt_structure_stats", "fredopt_volume_histogram", "fredopt_percentile_value",
@@ -82,6 +83,7 @@ def _load():
     lib.fredopt_set_weights.argtypes = [vp, vp]
     lib.fredopt_get_weights.argtypes = [vp, vp]
     lib.fredopt_get_weights_f64.argtypes = [vp, vp]
+    lib.fredopt_set_voxel_bounds.argtypes = [vp, i32, vp]
     lib.fredopt_dose_let.argtypes = [vp, vp, vp, vp]
     lib.fredopt_iterate.argtypes = [vp, i32, f32, f32, f32]
     lib.fredopt_proximity.argtypes = [vp, vp, C.POINTER(f64), C.POINTER(i64)]
@@ -190,6 +192,10 @@ class Plan:
     def get_weights_f64(self, out):
         _check(_lib.fredopt_get_weights_f64(self._h, _ptr(out, np.float64, self.n_cols)), "fredopt_get_weights_f64")
         return out
+
+    def set_voxel_bounds(self, field, values):
+        """values: n_rows float32 (NaN = the structure's scalar), host or device, or None (remove the array)."""
+        _check(_lib.fredopt_set_voxel_bounds(self._h, int(field), _ptr(values, np.float32, self.n_rows)), "fredopt_set_voxel_bounds")
 
     # ---- the four calls of north_star
     def dose_let(self, x, dose, letd):

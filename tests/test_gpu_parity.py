@@ -731,3 +731,117 @@ def test_work_distribution_never_changes_a_result(fredopt, plan0):
         gp.destroy()
     with pytest.raises(f.FredoptError):
         gp = f.from_plan(plan0); gp.set_option(f.OPT_WORK_QUEUE, 16)
+
+
+# ------------------------------------------------------------------------------------------ per-voxel bounds
+def _varying_voxel_bounds(plan, bounds, seed):
+    """Per-voxel arrays around the structures' scalars (+-, NaN on ~30 % of the voxels), voxel-indexed float32, for every field."""
+    lab = plan.labels.cpu().numpy() if hasattr(plan.labels, "cpu") else np.asarray(plan.labels)
+    V = len(lab)
+    u = pg.uniform01_array(seed, 8 * V).reshape(8, V)
+    out = {}
+    for field in range(7):
+        col = np.where(lab > 0, bounds[np.maximum(lab, 1) - 1, field + 1], np.nan).astype(np.float64)
+        scale = 0.8 + 0.4 * u[field]
+        if field in (0, 2):
+            scale = 0.7 + 0.25 * u[field]
+        if field in (1, 3):
+            scale = 1.0 + 0.3 * u[field]
+        out[field] = np.where(u[7] < 0.3, np.nan, col * scale).astype(np.float32)
+    return out
+
+
+@pytest.mark.parametrize("copt", [pytest.param({}, id="auto"), pytest.param({"block_rows": 1}, id="rows1"), pytest.param({"block_rows": 4}, id="rows4")])
+def test_per_voxel_bounds_config0(fredopt, plan0, copt):
+    from oracle import oracle as om
+    f = fredopt
+    # arrays of the structures' own scalars: the same bits as the scalar plan
+    a = f.from_plan(plan0, **copt); b = f.from_plan(plan0, **copt)
+    lab = plan0.labels.numpy()
+    for field in range(7):
+        col = np.where(lab > 0, plan0.bounds[np.maximum(lab, 1) - 1, field + 1], np.nan).astype(np.float32)
+        b.set_voxel_bounds(field, col)
+    for g in (a, b):
+        g.set_weights(plan0.x0); g.iterate(20, 1.0, 1.0, 0.99)
+    assert np.array_equal(_gpu_x(a), _gpu_x(b)) and a.stats() == b.stats()
+    # genuinely varying bounds, both AMS forms, against the oracle
+    vb = _varying_voxel_bounds(plan0, plan0.bounds, 5)
+    for block in (0, 1):
+        gp = f.from_plan(plan0, **copt); orc = _oracle(plan0)
+        for field, arr in vb.items():
+            gp.set_voxel_bounds(field, torch.from_numpy(arr).cuda() if field % 2 else arr)     # device and host pointers
+            orc.set_voxel_bounds(field, arr)
+        assert abs(gp.stats()["weight_sum"] - orc.stats()["W"]) <= 1e-12 * orc.stats()["W"]
+        gp.set_option(f.OPT_BLOCK_SEQUENTIAL, block); orc.set_option(om.OPT_BLOCK_SEQUENTIAL, block)
+        gp.set_weights(plan0.x0); orc.set_x(plan0.x0)
+        gp.iterate(20, 1.0, 1.0, 0.99); orc.iterate(20, 1.0, 1.0, 0.99)
+        if block:
+            _assert_block_state(gp, orc)
+        else:
+            _assert_state(gp, orc)
+        # the arrays matter: the scalar plan is elsewhere
+        assert _rel_l2(_gpu_x(gp), _gpu_x(a)) > 1e-4 or block
+    # removing the arrays restores the scalar plan; invalid arrays are refused and change nothing
+    for field in range(7):
+        gp.set_voxel_bounds(field, None)
+    gp.set_option(f.OPT_BLOCK_SEQUENTIAL, 0); gp.set_option(f.OPT_RESET, 1)
+    gp.set_weights(plan0.x0); gp.iterate(20, 1.0, 1.0, 0.99)
+    assert np.array_equal(_gpu_x(gp), _gpu_x(a))
+    with pytest.raises(f.FredoptError) as e:
+        gp.set_voxel_bounds(f.VB_DOSE_LO, np.full(plan0.n_rows, 9.0, np.float32))          # above the PTV's dose_hi
+    assert e.value.code == f.INVALID_ARG
+    with pytest.raises(f.FredoptError):
+        gp.set_voxel_bounds(f.VB_DOSE_HI, np.full(plan0.n_rows, np.inf, np.float32))
+    with pytest.raises(f.FredoptError):
+        gp.set_voxel_bounds(7, np.zeros(plan0.n_rows, np.float32))
+    gp.set_option(f.OPT_RESET, 1); gp.set_weights(plan0.x0); gp.iterate(20, 1.0, 1.0, 0.99)
+    assert np.array_equal(_gpu_x(gp), _gpu_x(a))
+
+
+@pytest.mark.parametrize("seed", [3, 4])
+def test_per_voxel_bounds_random_plans_one_sided_cost(fredopt, seed):
+    """Differing D / L patterns, every field varying per voxel, reductionsN = 2 and the one-sided cost (its accept loop reads
+    the per-voxel cDL references from the stored products)."""
+    from oracle import oracle as om
+    V, S = 300, 37
+    D, L, lab, x0 = pg.random_small_plan(seed, V=V, S=S, n_struct=3, density=0.3, same_pattern=False)
+    nan = np.nan
+    bounds = np.array([[1.0, 0.5, 0.9, nan, nan, nan, 0.7, nan],
+                       [2.0, nan, 0.4, nan, 1.5, 3.0, nan, 1.0],
+                       [0.5, 0.1, nan, 0.2, 2.0, 2.5, 0.3, 0.8]], np.float32)
+
+    class _P:
+        labels = lab
+    vb = _varying_voxel_bounds(_P, bounds, 100 + seed)
+    for one_sided in (0, 1):
+        orc = _oracle_np(V, S, D, L, lab, bounds)
+        gp = fredopt.Plan(V, S, D, L, lab, bounds, block_rows=(2, 4)[seed % 2])
+        for field, arr in vb.items():
+            gp.set_voxel_bounds(field, arr); orc.set_voxel_bounds(field, arr)
+        for g_, o_, v in ((fredopt.OPT_ONE_SIDED_COST, om.OPT_ONE_SIDED_COST, one_sided), (fredopt.OPT_REDUCTIONS, om.OPT_REDUCTIONS, 2)):
+            gp.set_option(g_, v); orc.set_option(o_, v)
+        orc.set_x(x0); gp.set_weights(x0)
+        orc.iterate(20, 1.2, 2.0, 0.7); gp.iterate(20, 1.2, 2.0, 0.7)
+        _assert_state(gp, orc)
+
+
+def test_oar_bound_from_the_cdl30_of_the_forward_plan(fredopt):
+    """The paper's constraint selection: the cDL value that 30 % of an OAR's volume receives in the forward
+    (starting) plan becomes that OAR's upper cDL bound -- here per voxel, through fredopt_percentile_value and
+    fredopt_set_voxel_bounds, end to end on the scaled three-beam plan, against the oracle doing the same."""
+    from oracle import oracle as om
+    plan = pg.build_plan(pg.config_spec(2, scale=0.25), device="cuda")
+    gp = fredopt.from_plan(plan, stream=torch.cuda.current_stream().cuda_stream); orc = _oracle(plan)
+    lab = plan.labels.cpu().numpy()
+    hi_g = np.full(plan.n_rows, np.nan, np.float32); hi_o = hi_g.copy()
+    for label in (2, 3):                                        # brainstem-like and chiasm-like OARs carry a cDL slab
+        cg = gp.percentile_value(1, label, 0.3, plan.x0)
+        co = orc.percentile_value(1, label, 0.3, plan.x0.astype(np.float64))
+        assert abs(cg - co) <= 1e-12 * max(abs(co), 1e-30)
+        hi_g[lab == label] = np.float32(cg); hi_o[lab == label] = np.float32(co)
+    assert np.array_equal(hi_g, hi_o, equal_nan=True) and np.isfinite(hi_g[lab == 2]).all()
+    gp.set_voxel_bounds(fredopt.VB_DL_HI, hi_g); orc.set_voxel_bounds(om.VB_DL_HI, hi_o)
+    gp.set_voxel_bounds(fredopt.VB_DL_REF, hi_g); orc.set_voxel_bounds(om.VB_DL_REF, hi_o)
+    gp.set_weights(plan.x0); orc.set_x(plan.x0)
+    gp.iterate(20, 1.0, 1.0, 0.99); orc.iterate(20, 1.0, 1.0, 0.99)
+    _assert_state(gp, orc)
