@@ -159,6 +159,11 @@ typedef struct {
                                 /*     structure share one stored index per spot over the union of their patterns       */
                                 /*     (neighbouring voxels see almost the same spots), in both orientations.           */
                                 /*     0 = automatic (the height that stores the fewest bytes), or 1, 2, 4              */
+    int32_t shard_rank;         /* ONE plan on several GPUs: the labelled voxels are cut into          */
+    int32_t shard_world;        /*     shard_world contiguous voxel ranges balanced by labelled non-zeros                */
+                                /*     (fredopt_shard_range); this plan keeps range shard_rank of them.  x is replicated;  */
+                                /*     the sums over voxels are completed through fredopt_set_reduce.  0 / 0 or 0 / 1:     */
+                                /*     the whole plan.  fredopt_dose_let and the ROWS_ALL exports always cover all voxels  */
 } fredopt_create_options;
 /* fredopt_create with options (opt = NULL: the defaults, identical to fredopt_create).  INVALID_ARG on an unknown value. */
 int fredopt_create_ex(const fredopt_csr *D, const fredopt_csr *L, const int32_t *voxel_labels,
@@ -171,6 +176,7 @@ void fredopt_destroy(fredopt_plan *plan);
 int fredopt_set_weights(fredopt_plan *plan, const float *x);
 int fredopt_get_weights(fredopt_plan *plan, float *x);
 int fredopt_get_weights_f64(fredopt_plan *plan, double *x);
+int fredopt_set_weights_f64(fredopt_plan *plan, const double *x);   /* the fp64 state itself (checkpoint / resume) */
 
 /* dose = D x, LETd_i = (L x)_i / (D x)_i (0 where dose_i = 0) over ALL n_rows voxels (Eq. 1).
  * x: n_cols floats or NULL = the plan's x.  dose, letd: n_rows floats each; either may be NULL. */
@@ -204,6 +210,42 @@ int fredopt_proximity(fredopt_plan *plan, const float *x, double *prox, int64_t 
 
 int fredopt_set_option(fredopt_plan *plan, int32_t key, double value);
 int fredopt_get_stats(fredopt_plan *plan, fredopt_stats *out);
+
+/* ---- one plan on several GPUs (the paper's optimizer is single-GPU) ----
+ * Voxel range [*v_begin, *v_end) of shard `rank` of `world`: cuts at the voxel indices where the running count of
+ * (non-zeros of D + 1) over LABELLED voxels crosses rank / world of its total.  HOST arrays; pure host code (no GPU
+ * needed): every rank computes the same cuts.  INVALID_ARG on bad arguments. */
+int fredopt_shard_range(const int64_t *row_ptr, const int32_t *voxel_labels, int64_t n_rows, int32_t rank, int32_t world,
+                        int64_t *v_begin, int64_t *v_end);
+/* The reduction a sharded plan calls where a sum runs over all voxels: fn must replace buf[0..n) (DEVICE memory, fp64) by its
+ * element-wise sum over all ranks -- the same bits on every rank -- ordered on `cuda_stream` (e.g. ncclAllReduce on that
+ * stream), and return 0.  It is called once inside fredopt_set_reduce (set counts -> the normalised weights w^ of the WHOLE
+ * plan) and then, per superiorized iteration, three times: after the transposed pass of the gradient (n_cols + 1 values: the
+ * partial gradient and chi^2), after the forward pass on g (1 value: c) and after the transposed pass of the step (n_cols + 3
+ * values: the partial step, proximity, chi^2, violated sets); once per pure feasibility-seeking iteration; once per
+ * fredopt_proximity.  The spot weights stay replicated bit for bit because every rank applies the same arithmetic to the same
+ * reduced values.  A sharded plan launches its kernels directly (no graph replay) and supports the simultaneous form
+ * (FREDOPT_OPT_BLOCK_SEQUENTIAL and the evaluation quantities return FREDOPT_UNSUPPORTED).  fredopt_iterate on a sharded plan
+ * without a reduction returns FREDOPT_INVALID_ARG. */
+typedef int (*fredopt_reduce_fn)(void *ctx, double *buf, int64_t n, void *cuda_stream);
+int fredopt_set_reduce(fredopt_plan *plan, fredopt_reduce_fn fn, void *ctx);
+
+/* The state of Fig. 3 that fredopt_iterate carries from call to call, beside the spot weights: with fredopt_get_weights_f64 /
+ * fredopt_set_weights_f64 it is everything a run needs to be resumed -- in another plan, another process -- and to continue
+ * bit for bit as if it had not been interrupted (options are the caller's to set again).  Plain data; both calls synchronise. */
+typedef struct {
+    int64_t k;                  /* iterations done                                          */
+    int64_t s;                  /* step-size exponent consumed so far                   */
+    int64_t trials;             /* perturbation trials evaluated so far                                    */
+    double  beta_next;          /* beta0 * a^s, built by repeated multiplication                           */
+    double  eta_pow;            /* eta^k, likewise                                          */
+    double  last_beta;          /* last accepted beta                                                      */
+    float   beta0, a;           /* the latched pair (reading R8), 0 if none                                */
+    int32_t latched;            /* 1 if a superiorized call has latched (beta0, a)                         */
+    int32_t reserved;
+} fredopt_state;
+int fredopt_get_state(fredopt_plan *plan, fredopt_state *out);
+int fredopt_set_state(fredopt_plan *plan, const fredopt_state *in);
 
 /* ---- evaluation quantities of the paper's constraint selection and plan comparison (Table 1,
  * PAPER.md:228-236): the dose / LETd / c x D x LETd volume histograms (DVH, LVH, cDLVH), the "value received by a

@@ -136,6 +136,11 @@ struct fredopt_plan {
     int fwd_sorted = 1, tr_sorted = 1;     // items taken longest first (else in storage order)
     bool force_idx32 = false;          // create option: int32 indices in both orientations
     int block_rows_opt = 0;            // create option: rows per block row of the labelled set (0 = chosen by stored bytes)
+    int shard_rank = 0, shard_world = 1;   // create option: this plan keeps one voxel range of the labelled rows
+    long long shard_begin = 0, shard_end = 0;
+    fredopt_reduce_fn reduce_fn = nullptr; // sums a device buffer over all ranks (sharded plans)
+    void* reduce_ctx = nullptr;
+    double* rbuf = nullptr;            // [S + 8] reduction buffer of the step pass; g has the same 8 spare values
     float* out_stage = nullptr;        // lazily: 2 x n_rows floats staging host outputs of dose_let / spmv_forward
     bool started = false;
     float latched_beta0 = 0.f, latched_a = 0.f;
@@ -146,7 +151,7 @@ struct fredopt_plan {
     long long gexec_red[8] = {};
     int gexec_kernels[8] = {};
     // timing
-    std::vector<EventPair> events;
+    std::vector<EventPair> events, event_pool;
     double pass_ms[FREDOPT_N_PASSES] = {0};
     long long pass_launches[FREDOPT_N_PASSES] = {0};
     long long pass_bytes[FREDOPT_N_PASSES] = {0};
@@ -214,9 +219,13 @@ void launch_fwd_kernel(fredopt_plan* P, int epi, const RowSet& R, long long b0, 
                        int letd_out, const ResidArgs& ra);
 void launch_forward(fredopt_plan* P, const RowSet& R, const uint8_t* mode, const double* x, double* oD, double* oL, int epi,
                     int write_uv = 0);
+void launch_tr_kernel(fredopt_plan* P, const RowSet& R, const Item* items, const int32_t* slots, long long n, const uint8_t* mode,
+                      const GatherVec& vec);
 void launch_transpose(fredopt_plan* P, int tepi, const RowSet& R, const uint8_t* mode, const GatherVec& vec, double* g_out,
                       double* x, float* f_out);
 void launch_finalize(fredopt_plan* P, int n_part);
-void invalidate_graphs(fredopt_plan* P);                         // captured launches hold kernel arguments: capture again
+void launch_sum_to(fredopt_plan* P, double* out, const double* in, const long long* in_ll, int n);   // out[0] = fixed-order sum
+void invalidate_graphs(fredopt_plan* P);
+int reduce_call(fredopt_plan* P, double* buf, long long n);      // the caller's reduction on the plan's stream (sharded plans)                         // captured launches hold kernel arguments: capture again
 // ---- plan_build.cu
 int recount_sets(fredopt_plan* P, bool letd_norms);              // norms of the LETd rows (per-voxel limits), set counts, W, w^

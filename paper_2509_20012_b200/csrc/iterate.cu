@@ -4,16 +4,25 @@
 #include "fredopt_plan.cuh"
 #include "kernels_iter.cuh"
 
+#include <nvtx3/nvToolsExt.h>
+
 // ============================================================================================ launches
+// Every pass is bracketed by an NVTX range (visible in a timeline tool; a few nanoseconds without one) and, with
+// FREDOPT_OPT_TIME_PASSES, by a pair of CUDA events taken from a pool the plan keeps.
+static const char* const PASS_LABEL[FREDOPT_N_PASSES] = {"fredopt F1 forward_x", "fredopt T1 transpose_g", "fredopt F2 forward_g",
+                                                         "fredopt select", "fredopt residual", "fredopt T2 transpose_b"};
 static void ev_begin(fredopt_plan* P, int pass) {
+    nvtxRangePushA(PASS_LABEL[pass]);
     if (!P->time_passes) return;
     EventPair ep;
-    cudaEventCreate(&ep.a); cudaEventCreate(&ep.b);
+    if (!P->event_pool.empty()) { ep = P->event_pool.back(); P->event_pool.pop_back(); }
+    else { cudaEventCreate(&ep.a); cudaEventCreate(&ep.b); }
     ep.pass = pass;
     cudaEventRecord(ep.a, P->stream);
     P->events.push_back(ep);
 }
 static void ev_end(fredopt_plan* P) {
+    nvtxRangePop();
     if (!P->time_passes) return;
     cudaEventRecord(P->events.back().b, P->stream);
 }
@@ -200,6 +209,53 @@ static int enqueue_iteration(fredopt_plan* P, bool sa) {
 }
 
 
+void launch_sum_to(fredopt_plan* P, double* out, const double* in, const long long* in_ll, int n) {
+    if (in_ll) klaunch(P, k_sum_to_ll, 1, 1024, out, in_ll, n);
+    else klaunch(P, k_sum_to, 1, 1024, out, in, n);
+}
+
+int reduce_call(fredopt_plan* P, double* buf, long long n) {
+    if (!P->reduce_fn) return FREDOPT_INVALID_ARG;
+    return P->reduce_fn(P->reduce_ctx, buf, (int64_t)n, (void*)P->stream) == 0 ? FREDOPT_OK : FREDOPT_CUDA_ERROR;
+}
+
+// One iteration of a SHARDED plan (simultaneous form): the local passes of enqueue_iteration with the sums over voxels completed
+// by the caller's reduction -- the partial gradient (+ chi^2), c, and the partial step (+ statistics).  Launched directly.
+static int enqueue_iteration_sharded(fredopt_plan* P, bool sa) {
+    const RowSet& A = P->act;
+    const long long S = P->S;
+    const int gS = grid_for(S, 256, 1 << 30);
+    if (sa) {
+        launch_forward(P, A, P->mode_union, P->x, P->d, P->l, EPI_STORE_PQ);
+        for (long long t = 0; t < P->reductionsN; ++t) {
+            // local partial gradient into g (slots of the local rows), chi^2 of the local rows into g[S]
+            if (A.t_n_items) launch_tr_kernel(P, A, A.t_items, A.t_item_slot, A.t_n_items, P->mode_cost, P->pq);
+            klaunch(P, k_slots_sum, gS, 256, S, A.t_item_ptr, A.t_partial, P->g);
+            klaunch(P, k_sum_to, 1, 1024, P->g + S, P->part_phi, A.n == 0 ? 0 : t == 0 ? (int)A.n : res_grid(P));
+            CKR(reduce_call(P, P->g, S + 1));
+            klaunch(P, k_gnorm, gS, 256, S, P->g, P->gpart);
+            launch_forward(P, A, P->mode_union, P->g, P->Dg, P->Lg, EPI_CPART);
+            klaunch(P, k_sum_to, 1, 1024, P->rbuf, P->cpart, A.n ? (int)A.n : 0);
+            CKR(reduce_call(P, P->rbuf, 1));
+            klaunch(P, k_select, 1, 1024, P->st, P->gpart, gS, P->rbuf, 1, P->g + S, 1, A.n_rows, A.rseg, P->tab, P->vb, P->d, P->l, P->Dg, P->Lg);
+            const int last = t == P->reductionsN - 1;
+            launch_residual(P, P->d, P->l, 1, last, last);
+        }
+    } else {
+        launch_forward(P, A, P->mode_con, P->x, P->d, P->l, EPI_RESID, 1);
+    }
+    // local partial step and statistics -> reduction -> update + clamp on every rank
+    if (A.t_n_items) launch_tr_kernel(P, A, A.t_items, A.t_item_slot, A.t_n_items, P->mode_con, P->uv);
+    klaunch(P, k_slots_sum, gS, 256, S, A.t_item_ptr, A.t_partial, P->rbuf);
+    const int np = A.n == 0 ? 0 : sa ? res_grid(P) : (int)A.n;
+    klaunch(P, k_sum_to, 1, 1024, P->rbuf + S, P->part_prox, np);
+    klaunch(P, k_sum_to, 1, 1024, P->rbuf + S + 1, P->part_phi, np);
+    klaunch(P, k_sum_to_ll, 1, 1024, P->rbuf + S + 2, P->part_cnt, np);
+    CKR(reduce_call(P, P->rbuf, S + 3));
+    klaunch(P, k_update_from, gS, 256, S, P->rbuf, P->x, P->st);
+    return FREDOPT_OK;
+}
+
 void invalidate_graphs(fredopt_plan* P) {
     for (int i = 0; i < 8; ++i) if (P->gexec[i]) { cudaGraphExecDestroy(P->gexec[i]); P->gexec[i] = nullptr; }
 }
@@ -251,7 +307,7 @@ int fredopt_set_option(fredopt_plan* P, int32_t key, double value) {
         case FREDOPT_OPT_TIME_PASSES:
             P->time_passes = value != 0.0;
             if (P->time_passes) {
-                for (auto& ep : P->events) { cudaEventDestroy(ep.a); cudaEventDestroy(ep.b); }
+                for (auto& ep : P->events) P->event_pool.push_back(ep);
                 P->events.clear();
                 for (int i = 0; i < FREDOPT_N_PASSES; ++i) { P->pass_ms[i] = 0; P->pass_launches[i] = 0; }
             }
@@ -265,6 +321,8 @@ int fredopt_iterate(fredopt_plan* P, int32_t n_iter, float lambda, float beta0, 
     if (!P || n_iter < 0) return FREDOPT_INVALID_ARG;
     if (!(lambda > 0.f) || !(lambda <= 2.f) || !(beta0 >= 0.f) || !std::isfinite(beta0) || !(a > 0.f) || !(a < 1.f))
         return FREDOPT_INVALID_ARG;
+    if (P->shard_world > 1 && !P->reduce_fn) return FREDOPT_INVALID_ARG;
+    if (P->shard_world > 1 && P->block_sequential) return FREDOPT_UNSUPPORTED;
     // the step-size sequence beta0 a^s belongs to the plan (R8): the first superiorized call latches (beta0, a); calls with
     // beta0 = 0 neither latch nor consume it; a different pair needs FREDOPT_OPT_RESET
     int latch = 0;
@@ -276,6 +334,15 @@ int fredopt_iterate(fredopt_plan* P, int32_t n_iter, float lambda, float beta0, 
                                            (P->normalize_grad ? SF_NORMALIZE_GRAD : 0) | (P->one_sided_cost ? SF_ONE_SIDED : 0), latch);
     ++P->launches;
     const bool sa = beta0 != 0.f;
+    if (P->shard_world > 1) {                                   // one plan on several GPUs: direct launches + the caller's reduction
+        if (n_iter > 0) {
+            P->launch_err = cudaSuccess;
+            for (int it = 0; it < n_iter; ++it) CKR(enqueue_iteration_sharded(P, sa));
+            CK(P->launch_err);
+        }
+        CK(cudaGetLastError());
+        return FREDOPT_OK;
+    }
     if (n_iter > 0) {
         const bool graph = P->use_graph && !P->time_passes;
         if (graph) {
@@ -324,6 +391,39 @@ int fredopt_iterate(fredopt_plan* P, int32_t n_iter, float lambda, float beta0, 
     return FREDOPT_OK;
 }
 
+int fredopt_get_state(fredopt_plan* P, fredopt_state* out) {
+    if (!P || !out) return FREDOPT_INVALID_ARG;
+    DevState h;
+    CK(cudaMemcpyAsync(&h, P->st, sizeof(DevState), cudaMemcpyDeviceToHost, P->stream));
+    CK(cudaStreamSynchronize(P->stream));
+    out->k = h.k; out->s = h.s; out->trials = h.trials;
+    out->beta_next = h.beta_next; out->eta_pow = h.eta_pow; out->last_beta = h.last_beta;
+    out->beta0 = P->started ? P->latched_beta0 : 0.f; out->a = P->started ? P->latched_a : 0.f;
+    out->latched = P->started ? 1 : 0;
+    out->reserved = 0;
+    return FREDOPT_OK;
+}
+
+int fredopt_set_state(fredopt_plan* P, const fredopt_state* in) {
+    if (!P || !in) return FREDOPT_INVALID_ARG;
+    if (in->k < 0 || in->s < 0 || in->trials < 0 || !(in->eta_pow >= 0.0) || !std::isfinite(in->eta_pow) || !(in->beta_next >= 0.0) ||
+        !std::isfinite(in->beta_next) || !(in->last_beta >= 0.0) || !std::isfinite(in->last_beta) || (in->latched != 0 && in->latched != 1))
+        return FREDOPT_INVALID_ARG;
+    if (in->latched && (!(in->beta0 > 0.f) || !std::isfinite(in->beta0) || !(in->a > 0.f) || !(in->a < 1.f))) return FREDOPT_INVALID_ARG;
+    DevState h;
+    CK(cudaMemcpyAsync(&h, P->st, sizeof(DevState), cudaMemcpyDeviceToHost, P->stream));
+    CK(cudaStreamSynchronize(P->stream));
+    h.k = in->k; h.s = in->s; h.trials = in->trials;
+    h.beta_next = in->beta_next; h.eta_pow = in->eta_pow; h.last_beta = in->last_beta;
+    if (in->latched) { h.beta0 = (double)in->beta0; h.a = (double)in->a; }
+    CK(cudaMemcpyAsync(P->st, &h, sizeof(DevState), cudaMemcpyHostToDevice, P->stream));
+    CK(cudaStreamSynchronize(P->stream));
+    P->started = in->latched != 0;
+    P->latched_beta0 = in->latched ? in->beta0 : 0.f;
+    P->latched_a = in->latched ? in->a : 0.f;
+    return FREDOPT_OK;
+}
+
 int fredopt_get_stats(fredopt_plan* P, fredopt_stats* out) {
     if (!P || !out) return FREDOPT_INVALID_ARG;
     DevState h;
@@ -348,7 +448,7 @@ int fredopt_get_pass_times(fredopt_plan* P, double* ms, int64_t* launches) {
     for (auto& ep : P->events) {
         float t = 0.f;
         if (cudaEventElapsedTime(&t, ep.a, ep.b) == cudaSuccess) { P->pass_ms[ep.pass] += t; P->pass_launches[ep.pass] += 1; }
-        cudaEventDestroy(ep.a); cudaEventDestroy(ep.b);
+        P->event_pool.push_back(ep);
     }
     cudaGetLastError();
     P->events.clear();

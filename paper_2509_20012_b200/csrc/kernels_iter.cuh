@@ -53,6 +53,56 @@ __device__ __forceinline__ double strided_sum(const double* __restrict__ v, int 
     return acc;
 }
 
+// ---- sharded plans: local sums that go through the caller's reduction
+// out[0] = fixed-order sum of in[0..n)   (one CTA)
+__global__ void __launch_bounds__(1024) k_sum_to(double* __restrict__ out, const double* __restrict__ in, int n) {
+    pdl_wait();
+    pdl_trigger();
+    __shared__ double sm[32];
+    const double t = block_sum(strided_sum(in, n), sm);
+    if (threadIdx.x == 0) out[0] = t;
+}
+__global__ void __launch_bounds__(1024) k_sum_to_ll(double* __restrict__ out, const long long* __restrict__ in, int n) {
+    pdl_wait();
+    pdl_trigger();
+    __shared__ long long smc[32];
+    long long c = 0;
+    for (int i = threadIdx.x; i < n; i += blockDim.x) c += in[i];
+    const long long t = block_sum_ll(c, smc);
+    if (threadIdx.x == 0) out[0] = (double)t;
+}
+// per-CTA partial sums of |g|^2 from the (reduced) gradient, in the layout k_select reads
+__global__ void __launch_bounds__(256) k_gnorm(long long S, const double* __restrict__ g, double* __restrict__ gpart) {
+    pdl_wait();
+    pdl_trigger();
+    __shared__ double sm[8];
+    const long long j = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    const double v = j < S ? g[j] : 0.0;
+    const double q = block_sum(v * v, sm);
+    if (threadIdx.x == 0) gpart[blockIdx.x] = q;
+}
+// out[j] = sum of the local partial-sum slots of spot j (0 for a spot without slots)
+__global__ void __launch_bounds__(256) k_slots_sum(long long S, const long long* __restrict__ item_ptr, const double* __restrict__ partial,
+                                                   double* __restrict__ out) {
+    pdl_wait();
+    pdl_trigger();
+    const long long j = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (j >= S) return;
+    double tot = 0.0;
+    for (long long i = item_ptr[j]; i < item_ptr[j + 1]; ++i) tot += partial[i];
+    out[j] = tot;
+}
+// x_j <- max(0, x_j - lambda eta^k * (reduced step)_j); the reduced statistics follow the step in the buffer
+__global__ void __launch_bounds__(256) k_update_from(long long S, const double* __restrict__ rbuf, double* __restrict__ x, DevState* st) {
+    pdl_wait();
+    pdl_trigger();
+    const long long j = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (j == 0) { st->prox = rbuf[S]; st->phi = rbuf[S + 1]; st->n_viol = (long long)rbuf[S + 2]; }
+    if (j >= S) return;
+    const double v = x[j] - st->relax * rbuf[j];
+    x[j] = v < 0.0 ? 0.0 : v;
+}
+
 // |g|^2 (partial sums of k_combine) and c (partial sums of F2) in fixed order, then the `while loop` of Fig. 3
 // on device scalars.  The step is
 // b = beta (or beta / |g| with the normalised-gradient option).  Two-sided cost (Eq. 2 as printed):

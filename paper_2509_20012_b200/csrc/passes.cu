@@ -55,6 +55,14 @@ int fredopt_set_weights(fredopt_plan* P, const float* x) {
     return FREDOPT_OK;
 }
 
+int fredopt_set_weights_f64(fredopt_plan* P, const double* x) {
+    if (!P || !x) return FREDOPT_INVALID_ARG;
+    const bool dev = is_device_ptr(x);
+    CK(cudaMemcpyAsync(P->x, x, P->S * 8, dev ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice, P->stream));
+    if (!dev) CK(cudaStreamSynchronize(P->stream));       // the caller's array is borrowed for the call only
+    return FREDOPT_OK;
+}
+
 int fredopt_get_weights_f64(fredopt_plan* P, double* x) {
     if (!P || !x) return FREDOPT_INVALID_ARG;
     const bool dev = is_device_ptr(x);
@@ -220,6 +228,20 @@ int fredopt_proximity(fredopt_plan* P, const float* x, double* prox, int64_t* n_
     CKR(resolve_x(P, x, &xd));
     // scratch: Dg / Lg hold the products so that the iteration's d, l are left alone
     launch_forward(P, P->act, P->mode_con, xd, P->Dg, P->Lg, EPI_RESID, 0);     // a11: one pass, statistics only
+    if (P->shard_world > 1) {      // local statistics -> the caller's reduction
+        if (!P->reduce_fn) return FREDOPT_INVALID_ARG;
+        const int np = P->act.n ? (int)P->act.n : 0;
+        launch_sum_to(P, P->rbuf, P->part_prox, nullptr, np);
+        launch_sum_to(P, P->rbuf + 1, nullptr, P->part_cnt, np);
+        CKR(reduce_call(P, P->rbuf, 2));
+        double h2[2];
+        CK(cudaMemcpyAsync(h2, P->rbuf, 16, cudaMemcpyDeviceToHost, P->stream));
+        CK(cudaStreamSynchronize(P->stream));
+        CK(cudaGetLastError());
+        if (prox) *prox = h2[0];
+        if (n_violated) *n_violated = (int64_t)h2[1];
+        return FREDOPT_OK;
+    }
     launch_finalize(P, P->act.n ? (int)P->act.n : 1);
     DevState h;
     CK(cudaMemcpyAsync(&h, P->st, sizeof(DevState), cudaMemcpyDeviceToHost, P->stream));
@@ -233,6 +255,7 @@ int fredopt_proximity(fredopt_plan* P, const float* x, double* prox, int64_t* n_
 // ---- evaluation quantities: values of one voxel quantity over the rows of structure `label` into uv.cD[rb .. rb+nr)
 static int structure_values(fredopt_plan* P, const float* x, int32_t quantity, int32_t label, long long* rb_out, long long* nr_out) {
     if (!P || quantity < 0 || quantity > 2 || label < 1 || label > P->n_struct) return FREDOPT_INVALID_ARG;
+    if (P->shard_world > 1) return FREDOPT_UNSUPPORTED;          // a structure's voxels are spread over the ranks
     const double* xd;
     CKR(resolve_x(P, x, &xd));
     const long long rb = P->row_base[label - 1];                 // the structure's real rows; padding rows follow them

@@ -75,10 +75,11 @@ __global__ void k_union_fill(const long long* pD, const int32_t* cD, const float
 }
 
 // per voxel: padded length of the row as a block row of its own (multiple of 4; int64 for the scan), flags
-__global__ void k_row_lengths(const long long* ptr, const int32_t* lab, long long V, int32_t* nonempty, int32_t* active) {
+__global__ void k_row_lengths(const long long* ptr, const int32_t* lab, long long V, long long vb, long long ve, int32_t* nonempty,
+                              int32_t* active) {
     for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < V; i += (long long)gridDim.x * blockDim.x) {
         nonempty[i] = ptr[i + 1] > ptr[i];
-        active[i] = lab[i] != 0;
+        active[i] = lab[i] != 0 && i >= vb && i < ve;      // a sharded plan keeps the labelled voxels of its range
     }
 }
 
@@ -626,6 +627,41 @@ int build_transpose(fredopt_plan* P, RowSet& R) {
     return FREDOPT_OK;
 }
 
+// Sharded plans: the set counts of the WHOLE plan (participating / declared / zero-norm sets per structure and kind) are the
+// sums of the ranks' local counts -> W, w^.  Call right after a local count.
+static int reduce_set_counts(fredopt_plan* P) {
+    // the set counts of the WHOLE plan: participating / declared / zero-norm sets per structure and kind -> W, w^
+    const int ns = P->n_struct;
+    std::vector<double> h((size_t)ns * 6 + 1, 0.0);
+    CK(cudaMemcpyAsync(P->h_tab.data(), P->tab, sizeof(StructInfo) * P->max_seg, cudaMemcpyDeviceToHost, P->stream));
+    CK(cudaStreamSynchronize(P->stream));
+    for (int s = 0; s < ns; ++s) {
+        const StructInfo& T = P->h_tab[s];
+        h[s * 6 + 0] = (double)T.part; h[s * 6 + 1] = (double)T.n_sets; h[s * 6 + 2] = (double)T.n_zero;
+        h[s * 6 + 3] = (double)T.part_kind[0]; h[s * 6 + 4] = (double)T.part_kind[1]; h[s * 6 + 5] = (double)T.part_kind[2];
+    }
+    double* d = nullptr;
+    CK(cudaMalloc((void**)&d, h.size() * 8));
+    cudaError_t e = cudaMemcpyAsync(d, h.data(), h.size() * 8, cudaMemcpyHostToDevice, P->stream);
+    int rc = e == cudaSuccess ? reduce_call(P, d, (long long)h.size()) : FREDOPT_CUDA_ERROR;
+    if (rc == FREDOPT_OK) e = cudaMemcpyAsync(h.data(), d, h.size() * 8, cudaMemcpyDeviceToHost, P->stream);
+    cudaError_t e2 = cudaStreamSynchronize(P->stream);
+    cudaFree(d);
+    if (rc != FREDOPT_OK) return rc;
+    CK(e); CK(e2);
+    for (int s = 0; s < ns; ++s) {
+        StructInfo& T = P->h_tab[s];
+        T.part = (unsigned long long)h[s * 6 + 0]; T.n_sets = (unsigned long long)h[s * 6 + 1]; T.n_zero = (unsigned long long)h[s * 6 + 2];
+        T.part_kind[0] = (unsigned long long)h[s * 6 + 3]; T.part_kind[1] = (unsigned long long)h[s * 6 + 4]; T.part_kind[2] = (unsigned long long)h[s * 6 + 5];
+    }
+    CK(cudaMemcpyAsync(P->tab, P->h_tab.data(), sizeof(StructInfo) * P->max_seg, cudaMemcpyHostToDevice, P->stream));
+    k_finish_tables<<<1, 1, 0, P->stream>>>(P->tab, P->n_struct, P->st, P->mode_union, P->mode_con, P->mode_cost, P->mode_fixed, P->max_seg);
+    CK(cudaMemcpyAsync(P->h_tab.data(), P->tab, sizeof(StructInfo) * P->max_seg, cudaMemcpyDeviceToHost, P->stream));
+    CK(cudaStreamSynchronize(P->stream));
+    CK(cudaGetLastError());
+    return FREDOPT_OK;
+}
+
 int recount_sets(fredopt_plan* P, bool letd_norms) {
     cudaStream_t st = P->stream;
     const RowSet& A = P->act;
@@ -638,6 +674,7 @@ int recount_sets(fredopt_plan* P, bool letd_norms) {
     CK(cudaMemcpyAsync(P->h_tab.data(), P->tab, sizeof(StructInfo) * ns, cudaMemcpyDeviceToHost, st));
     CK(cudaStreamSynchronize(st));
     CK(cudaGetLastError());
+    if (P->shard_world > 1 && P->reduce_fn) CKR(reduce_set_counts(P));
     return FREDOPT_OK;
 }
 
@@ -677,6 +714,7 @@ void fredopt_destroy(fredopt_plan* P) {
     if (!P) return;
     cudaStreamSynchronize(P->stream);
     for (auto& ep : P->events) { cudaEventDestroy(ep.a); cudaEventDestroy(ep.b); }
+    for (auto& ep : P->event_pool) { cudaEventDestroy(ep.a); cudaEventDestroy(ep.b); }
     for (int i = 0; i < 8; ++i) if (P->gexec[i]) cudaGraphExecDestroy(P->gexec[i]);
     for (void* p : P->allocs) cudaFree(p);
     for (int k = 0; k < VB_N; ++k) cudaFree(P->vb_buf[k]);
@@ -797,7 +835,18 @@ static int create_impl(fredopt_plan* P, const fredopt_csr* D, const fredopt_csr*
     CKR(tmp.get(&pos_ne, (size_t)V + 2)); CKR(tmp.get(&pos_act, (size_t)V + 2));
     CK(cudaMemsetAsync(f_ne, 0, (V + 1) * 4, st));
     CK(cudaMemsetAsync(f_act, 0, (V + 1) * 4, st));
-    if (V) k_row_lengths<<<grid_for(V, 256, 1 << 16), 256, 0, st>>>(pU, lab, V, f_ne, f_act);
+    P->shard_begin = 0; P->shard_end = V;
+    if (P->shard_world > 1) {      // the cuts are computed on the host from D's row offsets and the labels (every rank: the same cuts)
+        std::vector<long long> hp((size_t)V + 1);
+        std::vector<int32_t> hl((size_t)(V ? V : 1));
+        CK(cudaMemcpyAsync(hp.data(), pD, (V + 1) * 8, cudaMemcpyDefault, st));
+        CK(cudaMemcpyAsync(hl.data(), lab, V * 4, cudaMemcpyDefault, st));
+        CK(cudaStreamSynchronize(st));
+        int64_t b = 0, e = 0;
+        CKR(fredopt_shard_range((const int64_t*)hp.data(), hl.data(), V, P->shard_rank, P->shard_world, &b, &e));
+        P->shard_begin = b; P->shard_end = e;
+    }
+    if (V) k_row_lengths<<<grid_for(V, 256, 1 << 16), 256, 0, st>>>(pU, lab, V, P->shard_begin, P->shard_end, f_ne, f_act);
     CKR(scan_exclusive(P, f_ne, pos_ne, V + 1));
     CKR(scan_exclusive(P, f_act, pos_act, V + 1));
     int32_t n_ne = 0, n_act = 0;
@@ -988,9 +1037,11 @@ static int create_impl(fredopt_plan* P, const fredopt_csr* D, const fredopt_csr*
     }
     // ---- vectors
     const long long NR = A.n_rows;
-    CKR(dmalloc(P, &P->x, (size_t)S)); CKR(dmalloc(P, &P->g, (size_t)S)); CKR(dmalloc(P, &P->xtmp, (size_t)S));
+    CKR(dmalloc(P, &P->x, (size_t)S)); CKR(dmalloc(P, &P->g, (size_t)S + 8)); CKR(dmalloc(P, &P->xtmp, (size_t)S));
+    CKR(dmalloc(P, &P->rbuf, (size_t)S + 8));
+    CK(cudaMemsetAsync(P->rbuf, 0, ((size_t)S + 8) * 8, st));
     CKR(dmalloc(P, &P->xstage, (size_t)S));
-    CK(cudaMemsetAsync(P->x, 0, (S ? S : 1) * 8, st)); CK(cudaMemsetAsync(P->g, 0, (S ? S : 1) * 8, st));
+    CK(cudaMemsetAsync(P->x, 0, (S ? S : 1) * 8, st)); CK(cudaMemsetAsync(P->g, 0, ((size_t)S + 8) * 8, st));
     double** vecs[] = {&P->d, &P->l, &P->Dg, &P->Lg};
     for (auto pp : vecs) { CKR(dmalloc(P, pp, (size_t)NR)); CK(cudaMemsetAsync(*pp, 0, (NR ? NR : 1) * 8, st)); }
     CKR(gv_alloc(P, &P->pq, (size_t)NR)); CKR(gv_alloc(P, &P->uv, (size_t)NR));
@@ -1014,6 +1065,37 @@ static int create_impl(fredopt_plan* P, const fredopt_csr* D, const fredopt_csr*
 
 extern "C" {
 
+int fredopt_shard_range(const int64_t* row_ptr, const int32_t* voxel_labels, int64_t n_rows, int32_t rank, int32_t world,
+                        int64_t* v_begin, int64_t* v_end) {
+    if (!row_ptr || (n_rows > 0 && !voxel_labels) || n_rows < 0 || world < 1 || rank < 0 || rank >= world || !v_begin || !v_end)
+        return FREDOPT_INVALID_ARG;
+    long long total = 0;
+    for (int64_t i = 0; i < n_rows; ++i) if (voxel_labels[i] != 0) total += row_ptr[i + 1] - row_ptr[i] + 1;
+    // cut r: the first voxel at which the running weight reaches ceil(r * total / world); cut 0 = 0, cut world = n_rows
+    auto cut = [&](int r) -> int64_t {
+        if (r <= 0) return 0;
+        if (r >= world) return n_rows;
+        const long long target = (long long)(((__int128)total * r + world - 1) / world);
+        long long run = 0;
+        for (int64_t i = 0; i < n_rows; ++i) {
+            if (run >= target) return i;
+            if (voxel_labels[i] != 0) run += row_ptr[i + 1] - row_ptr[i] + 1;
+        }
+        return n_rows;
+    };
+    *v_begin = cut(rank);
+    *v_end = cut(rank + 1);
+    return FREDOPT_OK;
+}
+
+int fredopt_set_reduce(fredopt_plan* P, fredopt_reduce_fn fn, void* ctx) {
+    if (!P) return FREDOPT_INVALID_ARG;
+    P->reduce_fn = fn; P->reduce_ctx = ctx;
+    invalidate_graphs(P);
+    if (!fn || P->shard_world <= 1) return FREDOPT_OK;
+    return recount_sets(P, false);        // local counts, then (sharded) their sum over the ranks -> W, w^ of the whole plan
+}
+
 int fredopt_create(const fredopt_csr* D, const fredopt_csr* L, const int32_t* voxel_labels, const fredopt_bounds* bounds,
                    int32_t n_struct, void* cuda_stream, fredopt_plan** out) {
     return fredopt_create_ex(D, L, voxel_labels, bounds, n_struct, cuda_stream, nullptr, out);
@@ -1031,6 +1113,8 @@ int fredopt_create_ex(const fredopt_csr* D, const fredopt_csr* L, const int32_t*
     }
     if (o.index_width != 0 && o.index_width != 32) return FREDOPT_INVALID_ARG;
     if (o.block_rows != 0 && o.block_rows != 1 && o.block_rows != 2 && o.block_rows != 4) return FREDOPT_INVALID_ARG;
+    if (o.shard_world < 0 || o.shard_rank < 0 || (o.shard_world == 0 && o.shard_rank != 0) || (o.shard_world > 0 && o.shard_rank >= o.shard_world))
+        return FREDOPT_INVALID_ARG;
     if (!D || !L || n_struct < 0 || (n_struct > 0 && !bounds)) return FREDOPT_INVALID_ARG;
     if (n_struct > 255) return FREDOPT_UNSUPPORTED;          // work items carry the structure in 8 bits
     if (D->n_rows != L->n_rows || D->n_cols != L->n_cols || D->n_rows < 0 || D->n_cols < 0 || D->nnz < 0 || L->nnz < 0)
@@ -1056,6 +1140,7 @@ int fredopt_create_ex(const fredopt_csr* D, const fredopt_csr* L, const int32_t*
     P->sm_count = prop.multiProcessorCount;
     P->force_idx32 = o.index_width == 32;
     P->block_rows_opt = o.block_rows;
+    P->shard_rank = o.shard_rank; P->shard_world = o.shard_world > 1 ? o.shard_world : 1;
     int rc = create_impl(P, D, L, voxel_labels, bounds, n_struct);
     if (rc != FREDOPT_OK) { fredopt_destroy(P); return rc; }
     *out = P;

@@ -26,6 +26,7 @@ N_PASSES = len(PASS_NAMES)
 # every symbol include/fredopt.h declares (tests check the library exports exactly these)
 SYMBOLS = (
     "fredopt_create", "fredopt_create_ex", "fredopt_destroy", "fredopt_set_weights", "fredopt_get_weights", "fredopt_get_weights_f64",
+    "fredopt_set_weights_f64", "fredopt_get_state", "fredopt_set_state", "fredopt_shard_range", "fredopt_set_reduce",
     "fredopt_set_voxel_bounds", "fredopt_dose_let", "fredopt_iterate", "fredopt_proximity", "fredopt_set_option", "fredopt_get_stats",
     "fredopt_spmv_forward", "fredopt_spmv_transpose", "fredopt_get_pass_times", "fredopt_get_pass_bytes",
     "fredopt_launch_count", "fredopt_stream_read", "fredopt_strerror", "fredopt_last_cuda_error",
@@ -52,7 +53,17 @@ class _Bounds(C.Structure):
 
 
 class _CreateOptions(C.Structure):
-    _fields_ = [("struct_size", C.c_int32), ("index_width", C.c_int32), ("block_rows", C.c_int32)]
+    _fields_ = [("struct_size", C.c_int32), ("index_width", C.c_int32), ("block_rows", C.c_int32), ("shard_rank", C.c_int32),
+                ("shard_world", C.c_int32)]
+
+
+REDUCE_FN = C.CFUNCTYPE(C.c_int, C.c_void_p, C.c_void_p, C.c_int64, C.c_void_p)   # fredopt_reduce_fn
+
+
+class State(C.Structure):
+    """fredopt_state: plain data, e.g. bytes(state) / State.from_buffer_copy(b) for a checkpoint file."""
+    _fields_ = [("k", C.c_int64), ("s", C.c_int64), ("trials", C.c_int64), ("beta_next", C.c_double), ("eta_pow", C.c_double),
+                ("last_beta", C.c_double), ("beta0", C.c_float), ("a", C.c_float), ("latched", C.c_int32), ("reserved", C.c_int32)]
 
 
 class Stats(C.Structure):
@@ -83,6 +94,11 @@ def _load():
     lib.fredopt_set_weights.argtypes = [vp, vp]
     lib.fredopt_get_weights.argtypes = [vp, vp]
     lib.fredopt_get_weights_f64.argtypes = [vp, vp]
+    lib.fredopt_set_weights_f64.argtypes = [vp, vp]
+    lib.fredopt_shard_range.argtypes = [vp, vp, i64, i32, i32, C.POINTER(i64), C.POINTER(i64)]
+    lib.fredopt_set_reduce.argtypes = [vp, REDUCE_FN, vp]
+    lib.fredopt_get_state.argtypes = [vp, C.POINTER(State)]
+    lib.fredopt_set_state.argtypes = [vp, C.POINTER(State)]
     lib.fredopt_set_voxel_bounds.argtypes = [vp, i32, vp]
     lib.fredopt_dose_let.argtypes = [vp, vp, vp, vp]
     lib.fredopt_iterate.argtypes = [vp, i32, f32, f32, f32]
@@ -189,6 +205,17 @@ class Plan:
         _check(_lib.fredopt_get_weights(self._h, _ptr(out, np.float32, self.n_cols)), "fredopt_get_weights")
         return out
 
+    def set_weights_f64(self, x):
+        _check(_lib.fredopt_set_weights_f64(self._h, _ptr(x, np.float64, self.n_cols)), "fredopt_set_weights_f64")
+
+    def get_state(self):
+        st = State()
+        _check(_lib.fredopt_get_state(self._h, C.byref(st)), "fredopt_get_state")
+        return st
+
+    def set_state(self, st):
+        _check(_lib.fredopt_set_state(self._h, C.byref(st)), "fredopt_set_state")
+
     def get_weights_f64(self, out):
         _check(_lib.fredopt_get_weights_f64(self._h, _ptr(out, np.float64, self.n_cols)), "fredopt_get_weights_f64")
         return out
@@ -229,6 +256,20 @@ class Plan:
                                              float(fraction), C.byref(v)), "fredopt_percentile_value")
         return v.value
 
+    def set_reduce(self, fn):
+        """fn(device_pointer: int, n: int, cuda_stream: int) -> None must sum the n doubles at device_pointer over all ranks in
+        place, ordered on cuda_stream (sharded plans; fredopt_set_reduce).  Exceptions are reported as a failed reduction."""
+        def tramp(_ctx, buf, n, stream):
+            try:
+                fn(int(buf), int(n), int(stream or 0))
+                return 0
+            except Exception:                                    # never let an exception cross the C boundary
+                import traceback
+                traceback.print_exc()
+                return 1
+        self._reduce_cb = REDUCE_FN(tramp)                         # keep the callback object alive as long as the plan
+        _check(_lib.fredopt_set_reduce(self._h, self._reduce_cb, None), "fredopt_set_reduce")
+
     # ---- options, stats
     def set_option(self, key, value):
         _check(_lib.fredopt_set_option(self._h, int(key), float(value)), "fredopt_set_option")
@@ -265,6 +306,23 @@ class Plan:
 
     def stream_read(self, device_buf, nbytes, reps=1):
         _check(_lib.fredopt_stream_read(self._h, _ptr(device_buf), int(nbytes), int(reps)), "fredopt_stream_read")
+
+
+def shard_range(row_ptr, voxel_labels, rank, world):
+    """fredopt_shard_range on host numpy arrays: the voxel range [begin, end) of shard `rank` of `world` (pure host code)."""
+    rp = np.ascontiguousarray(row_ptr, np.int64); lab = np.ascontiguousarray(voxel_labels, np.int32)
+    b, e = C.c_int64(0), C.c_int64(0)
+    _check(_lib.fredopt_shard_range(rp.ctypes.data, lab.ctypes.data, len(lab), int(rank), int(world), C.byref(b), C.byref(e)),
+           "fredopt_shard_range")
+    return b.value, e.value
+
+
+class DeviceDoubles:
+    """A view of n doubles of device memory for torch.as_tensor(view, device="cuda") (CUDA array interface, zero copy): how a
+    reduction callback hands the library's buffer to torch.distributed."""
+
+    def __init__(self, ptr, n):
+        self.__cuda_array_interface__ = {"shape": (int(n),), "typestr": "<f8", "data": (int(ptr), False), "version": 3}
 
 
 def from_plan(plan, stream=None, **create_options) -> Plan:

@@ -845,3 +845,35 @@ def test_oar_bound_from_the_cdl30_of_the_forward_plan(fredopt):
     gp.set_weights(plan.x0); orc.set_x(plan.x0)
     gp.iterate(20, 1.0, 1.0, 0.99); orc.iterate(20, 1.0, 1.0, 0.99)
     _assert_state(gp, orc)
+
+
+def test_checkpoint_and_resume_in_a_new_plan(fredopt, plan0, tmp_path):
+    """fredopt_get_state + fredopt_get_weights_f64 written to a file, read into a NEW plan (as another process would): the
+    resumed run continues bit for bit as the uninterrupted one, in both AMS forms with eta < 1 and two reductions."""
+    f = fredopt
+    for block in (0, 1):
+        def mk():
+            g = f.from_plan(plan0)
+            g.set_option(f.OPT_ETA, 0.97); g.set_option(f.OPT_REDUCTIONS, 2); g.set_option(f.OPT_BLOCK_SEQUENTIAL, block)
+            return g
+        a = mk(); a.set_weights(plan0.x0); a.iterate(4, 1.2, 0.0, 0.9); a.iterate(16, 1.2, 1.0, 0.9)
+        b = mk(); b.set_weights(plan0.x0); b.iterate(4, 1.2, 0.0, 0.9); b.iterate(6, 1.2, 1.0, 0.9)
+        path = tmp_path / f"ckpt{block}.bin"
+        with open(path, "wb") as fh:
+            fh.write(bytes(b.get_state())); fh.write(_gpu_x(b).tobytes())
+        b.destroy()
+        raw = open(path, "rb").read()
+        n = C_sizeof_state = len(bytes(f.State()))
+        c = mk()
+        c.set_weights_f64(np.frombuffer(raw[n:], np.float64).copy())
+        c.set_state(f.State.from_buffer_copy(raw[:n]))
+        c.iterate(10, 1.2, 1.0, 0.9)
+        assert np.array_equal(_gpu_x(c), _gpu_x(a))
+        sa, sc = a.stats(), c.stats()
+        assert all(sa[k] == sc[k] for k in ("k", "s", "trials", "last_beta", "n_violated", "prox"))
+        assert bytes(a.get_state()) == bytes(c.get_state())
+        with pytest.raises(f.FredoptError):                      # the latched pair came back with the state
+            c.iterate(1, 1.2, 0.5, 0.9)
+    bad = f.State(); bad.k = -1
+    with pytest.raises(f.FredoptError):
+        c.set_state(bad)
