@@ -27,13 +27,54 @@
 // and never states lambda, alpha, eta, reductionsN or the matrix sizes, so parity with the PAPER'S OWN
 // RUNS is unpinned; the algorithmic content is pinned by those mathematical checks.
 
+// Timing build: the same source compiled with -fopenmp (oracle.py build(omp=True)) runs the row loops of the simultaneous form
+// on all host cores -- rows in static contiguous chunks, back-projections into per-thread private S-vectors that are added
+// in thread order (SURVEY.md sec. 8d "Oracle timing").  Without -fopenmp the pragmas vanish and every loop is the plain
+// index-order loop; with one thread the two builds give the same bits (tests/test_oracle_pins.py::test_openmp_*).
 #include <algorithm>
 #include <cmath>
 #include <cstdint>
 #include <cstring>
 #include <vector>
+#ifdef _OPENMP
+#include <omp.h>
+#endif
 
 namespace {
+
+// Row loop of a pass: body(i, acc, t) handles row i, adding its S-vector contribution into acc (null if the pass has none) and
+// its scalar contributions into slot t of the caller's per-slot accumulators.  Plain build: one pass in index order, acc = out,
+// t = 0.  OpenMP build: static contiguous chunks of rows, per-thread private vectors added to `out` in thread order.
+inline int row_slots() {
+#ifdef _OPENMP
+    return omp_get_max_threads();
+#else
+    return 1;
+#endif
+}
+template <class Body>
+void for_rows(int64_t V, int64_t S, std::vector<double>* out, Body body) {
+    if (out) out->assign(S, 0.0);
+#ifdef _OPENMP
+    const int nt = omp_get_max_threads();
+    if (nt > 1) {
+        std::vector<std::vector<double>> priv(out ? nt : 0);
+#pragma omp parallel num_threads(nt)
+        {
+            const int t = omp_get_thread_num();
+            std::vector<double>* acc = nullptr;
+            if (out) { priv[t].assign(S, 0.0); acc = &priv[t]; }
+#pragma omp for schedule(static)
+            for (int64_t i = 0; i < V; ++i) body(i, acc, t);
+        }
+        if (out)
+            for (int t = 0; t < nt; ++t)
+                for (int64_t j = 0; j < S; ++j) (*out)[j] += priv[t][j];
+        return;
+    }
+#endif
+    for (int64_t i = 0; i < V; ++i) body(i, out, 0);
+}
 
 struct Csr {
     int64_t n_rows = 0, n_cols = 0;
@@ -157,6 +198,7 @@ void setup(Plan& P) {
 // chi^2(x), Eq. (2): sum_i w^_i (Dref_i - D(x)_i)^2 + sum_i w^_i (cDLref_i - cDL(x)_i)^2
 double cost(const Plan& P, const std::vector<double>& x) {
     double phi = 0.0;
+#pragma omp parallel for schedule(static) reduction(+ : phi)
     for (int64_t i = 0; i < P.D.n_rows; ++i) {
         int32_t s = P.label[i];
         if (s == 0) continue;
@@ -171,10 +213,10 @@ double cost(const Plan& P, const std::vector<double>& x) {
 
 // grad chi^2(x) = 2 [ sum_i w^_i (D(x)_i - Dref_i) D_i + sum_i w^_i (cDL(x)_i - cDLref_i) L_i ]
 void grad_cost(const Plan& P, const std::vector<double>& x, std::vector<double>& g) {
-    g.assign(P.D.n_cols, 0.0);
-    for (int64_t i = 0; i < P.D.n_rows; ++i) {
+    for_rows(P.D.n_rows, P.D.n_cols, &g, [&](int64_t i, std::vector<double>* gp, int) {
+        std::vector<double>& g = *gp;
         int32_t s = P.label[i];
-        if (s == 0) continue;
+        if (s == 0) return;
         const Bounds& sb = P.bounds[s - 1];
         const Bounds b = voxel_bounds(P, i, s);
         if (present(sb.dose_ref)) {
@@ -186,7 +228,7 @@ void grad_cost(const Plan& P, const std::vector<double>& x, std::vector<double>&
             if (P.one_sided_cost && c < 0.0) c = 0.0;
             for (int64_t p = P.L.ptr[i]; p < P.L.ptr[i + 1]; ++p) g[P.L.col[p]] += c * P.L.val[p];
         }
-    }
+    });
 }
 
 // One pass over all declared sets at x.  If `step` is non-null it receives
@@ -194,12 +236,13 @@ void grad_cost(const Plan& P, const std::vector<double>& x, std::vector<double>&
 // prox = 1/2 sum_{k in P} w^_k r_k^2 / n_k ;  n_viol = #{declared sets with r_k != 0}.
 void constraint_pass(const Plan& P, const std::vector<double>& x, std::vector<double>* step,
                      double* prox, int64_t* n_viol) {
-    if (step) step->assign(P.D.n_cols, 0.0);
-    double pr = 0.0;
-    int64_t nv = 0;
-    for (int64_t i = 0; i < P.D.n_rows; ++i) {
+    std::vector<double> prs(row_slots(), 0.0);      // one slot in the plain build: the sums run in index order
+    std::vector<int64_t> nvs(row_slots(), 0);
+    for_rows(P.D.n_rows, P.D.n_cols, step, [&](int64_t i, std::vector<double>* step, int t) {
+        double& pr = prs[t];
+        int64_t& nv = nvs[t];
         int32_t s = P.label[i];
-        if (s == 0) continue;
+        if (s == 0) return;
         const Bounds& sb = P.bounds[s - 1];
         const Bounds b = voxel_bounds(P, i, s);
         const double w = P.what[s - 1];
@@ -232,7 +275,10 @@ void constraint_pass(const Plan& P, const std::vector<double>& x, std::vector<do
                     for (int64_t p = P.D.ptr[i]; p < P.D.ptr[i + 1]; ++p) (*step)[P.D.col[p]] -= c * b.letd_max * P.D.val[p]; }
             }
         }
-    }
+    });
+    double pr = 0.0;
+    int64_t nv = 0;
+    for (size_t t = 0; t < prs.size(); ++t) { pr += prs[t]; nv += nvs[t]; }
     if (prox) *prox = pr;
     if (n_viol) *n_viol = nv;
 }
@@ -315,6 +361,16 @@ void* oracle_create(int64_t V, int64_t S, const int64_t* ptrD, const int32_t* co
 }
 
 void oracle_destroy(void* h) { delete (Plan*)h; }
+
+// threads the row loops run on (1 in the plain build)
+int32_t oracle_threads(void) { return (int32_t)row_slots(); }
+void oracle_set_threads(int32_t n) {
+#ifdef _OPENMP
+    if (n >= 1) omp_set_num_threads(n);
+#else
+    (void)n;
+#endif
+}
 
 void oracle_set_x(void* h, const float* x) { Plan* P = (Plan*)h; for (size_t j = 0; j < P->x.size(); ++j) P->x[j] = (double)x[j]; }
 void oracle_set_x64(void* h, const double* x) { Plan* P = (Plan*)h; P->x.assign(x, x + P->x.size()); }
@@ -478,6 +534,19 @@ void oracle_stats(void* h, int64_t* out, double* dout) {
     Plan* P = (Plan*)h;
     out[0] = P->k; out[1] = P->s; out[2] = P->trials; out[3] = P->n_sets; out[4] = P->n_zero_norm_sets;
     dout[0] = P->last_beta; dout[1] = P->W; dout[2] = P->beta_next;
+}
+
+// The state of Fig. 3 carried from call to call (checkpoint / resume): iout = k, s, trials, latched; dout = beta_next, eta_pow,
+// last_beta, latched beta0, latched a.
+void oracle_get_state(void* h, int64_t* iout, double* dout) {
+    Plan* P = (Plan*)h;
+    iout[0] = P->k; iout[1] = P->s; iout[2] = P->trials; iout[3] = P->started ? 1 : 0;
+    dout[0] = P->beta_next; dout[1] = P->eta_pow; dout[2] = P->last_beta; dout[3] = P->latched_beta0; dout[4] = P->latched_a;
+}
+void oracle_set_state(void* h, const int64_t* iin, const double* din) {
+    Plan* P = (Plan*)h;
+    P->k = iin[0]; P->s = iin[1]; P->trials = iin[2]; P->started = iin[3] != 0;
+    P->beta_next = din[0]; P->eta_pow = din[1]; P->last_beta = din[2]; P->latched_beta0 = din[3]; P->latched_a = din[4];
 }
 
 void oracle_sweep_stats(void* h, double* prox, int64_t* n_viol) {

@@ -14,27 +14,29 @@ import numpy as np
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _SRC = os.path.join(_HERE, "fredopt_oracle.cpp")
 _LIB = os.path.join(_HERE, "libfredopt_oracle.so")
+_LIB_OMP = os.path.join(_HERE, "libfredopt_oracle_omp.so")      # timing build: same source, -fopenmp
 
 OPT_ETA, OPT_REDUCTIONS, OPT_ACCEPT_CHECK, OPT_MAX_TRIALS, OPT_RESET = 0, 1, 2, 3, 4
 OPT_BLOCK_SEQUENTIAL, OPT_NORMALIZE_GRAD, OPT_ONE_SIDED_COST = 7, 8, 9
 VB_DOSE_LO, VB_DOSE_HI, VB_DL_LO, VB_DL_HI, VB_LETD_MAX, VB_DOSE_REF, VB_DL_REF = range(7)
 
 
-def build(force: bool = False) -> str:
-    """Compile the oracle with plain g++ -O2 (no OpenMP, no fast-math)."""
-    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
-        subprocess.check_call(["g++", "-O2", "-std=c++17", "-fPIC", "-shared", "-ffp-contract=off",
-                               "-o", _LIB, _SRC])
-    return _LIB
+def build(force: bool = False, omp: bool = False) -> str:
+    """Compile the oracle with plain g++ -O2 (no fast-math); omp=True: the timing build of the same source with -fopenmp (row
+    loops on all host cores)."""
+    lib = _LIB_OMP if omp else _LIB
+    if force or not os.path.exists(lib) or os.path.getmtime(lib) < os.path.getmtime(_SRC):
+        subprocess.check_call(["g++", "-O2", "-std=c++17", "-fPIC", "-shared", "-ffp-contract=off"] + (["-fopenmp"] if omp else []) +
+                              ["-o", lib, _SRC])
+    return lib
 
 
-_lib = None
+_libs = {}
 
 
-def _load():
-    global _lib
-    if _lib is None:
-        lib = C.CDLL(build())
+def _load(omp: bool = False):
+    if omp not in _libs:
+        lib = C.CDLL(build(omp=omp))
         vp, i64, i32, f32, f64 = C.c_void_p, C.c_int64, C.c_int32, C.c_float, C.c_double
         lib.oracle_create.restype = vp
         lib.oracle_create.argtypes = [i64, i64, vp, vp, vp, vp, vp, vp, vp, vp, i32]
@@ -55,6 +57,8 @@ def _load():
         lib.oracle_iterate.restype = i32
         lib.oracle_iterate.argtypes = [vp, i32, f32, f32, f32]
         lib.oracle_stats.argtypes = [vp, vp, vp]
+        lib.oracle_get_state.argtypes = [vp, vp, vp]
+        lib.oracle_set_state.argtypes = [vp, vp, vp]
         lib.oracle_sweep_stats.argtypes = [vp, vp, vp]
         lib.oracle_structure_stats.argtypes = [vp, vp, i32, i32, vp, vp]
         lib.oracle_volume_histogram.argtypes = [vp, vp, i32, i32, i32, f64, vp]
@@ -63,8 +67,8 @@ def _load():
         lib.oracle_norms.argtypes = [vp, vp, vp, vp]
         lib.oracle_what.argtypes = [vp, vp]
         lib.oracle_sequential_sweep.argtypes = [vp, f32]
-        _lib = lib
-    return _lib
+        _libs[omp] = lib
+    return _libs[omp]
 
 
 def _p(a):
@@ -74,8 +78,8 @@ def _p(a):
 class Oracle:
     """fp64 CPU restatement of the hot path.  Inputs are numpy arrays (fp32 values, int32 cols, int64 ptrs)."""
 
-    def __init__(self, D, L, labels, bounds):
-        lib = _load()
+    def __init__(self, D, L, labels, bounds, omp=False):
+        lib = _load(omp)
         rpD, ciD, vD = D
         rpL, ciL, vL = L
         self.V = len(rpD) - 1
@@ -87,8 +91,9 @@ class Oracle:
         self._lib = lib
 
     @classmethod
-    def create(cls, V, S, D, L, labels, bounds):
-        self = cls(D, L, labels, bounds)
+    def create(cls, V, S, D, L, labels, bounds, omp=False):
+        """omp=True: the OpenMP timing build (threads = OMP_NUM_THREADS / all host cores)."""
+        self = cls(D, L, labels, bounds, omp=omp)
         self.V, self.S = int(V), int(S)
         k = self._keep
         assert len(k[0]) == V + 1 and len(k[3]) == V + 1 and len(k[6]) == V
@@ -174,6 +179,15 @@ class Oracle:
         return dict(k=int(o[0]), s=int(o[1]), trials=int(o[2]), n_sets=int(o[3]), n_zero_norm_sets=int(o[4]),
                     last_beta=float(d[0]), W=float(d[1]), beta_next=float(d[2]))
 
+    def get_state(self):
+        i = np.zeros(4, np.int64); d = np.zeros(5, np.float64)
+        self._lib.oracle_get_state(self._h, _p(i), _p(d))
+        return i, d
+
+    def set_state(self, state):
+        i, d = state
+        self._lib.oracle_set_state(self._h, _p(np.ascontiguousarray(i, np.int64)), _p(np.ascontiguousarray(d, np.float64)))
+
     def sweep_stats(self):
         """(proximity, violated sets) met by the last block-sequential sweep at visit time."""
         pr = C.c_double(0.0); nv = C.c_int64(0)
@@ -211,7 +225,17 @@ class Oracle:
         self._lib.oracle_sequential_sweep(self._h, float(lam))
 
 
-def from_plan(plan) -> "Oracle":
+def from_plan(plan, omp=False) -> "Oracle":
     """Oracle over a plangen.Plan (tensors are copied to host numpy)."""
     rp, ci, vd, vl, lab = plan.to_numpy()
-    return Oracle.create(plan.n_rows, plan.n_cols, (rp, ci, vd), (rp, ci, vl), lab, plan.bounds)
+    return Oracle.create(plan.n_rows, plan.n_cols, (rp, ci, vd), (rp, ci, vl), lab, plan.bounds, omp=omp)
+
+
+def omp_threads(n: int = 0) -> int:
+    """Threads the OpenMP timing build runs with (n >= 1: set them first)."""
+    lib = _load(True)
+    lib.oracle_threads.restype = C.c_int32
+    lib.oracle_set_threads.argtypes = [C.c_int32]
+    if n >= 1:
+        lib.oracle_set_threads(int(n))
+    return int(lib.oracle_threads())

@@ -987,3 +987,32 @@ def test_pin29_per_voxel_letd_limit_lands_on_the_voxels_own_boundary():
         o2.set_voxel_bounds(orc.VB_DOSE_HI, np.array([np.inf], F32))
     o2.set_x(x0)
     assert o2.proximity()[1] == 0 or o2.proximity()[1] == 1
+
+
+# ----------------------------------------------------------------------------- the OpenMP timing build
+def test_openmp_timing_build_is_the_same_oracle(plan0):
+    """bench.py's all-cores cpu_baseline runs oracle/fredopt_oracle.cpp compiled with -fopenmp.  With one thread it returns the
+    plain build's bits; with several, static row chunks and per-thread S-vectors added in thread order change the summation
+    order only (1e-13), never a decision (s, trials, violation count)."""
+    plain = orc.from_plan(plan0)
+    plain.set_x(plan0.x0); plain.iterate(12, 1.0, 1.0, 0.99)
+    for nt, tol in ((1, 0.0), (4, 1e-13)):
+        assert orc.omp_threads(nt) == nt
+        o = orc.from_plan(plan0, omp=True)
+        o.set_x(plan0.x0); o.iterate(12, 1.0, 1.0, 0.99)
+        err = np.linalg.norm(o.get_x() - plain.get_x()) / np.linalg.norm(plain.get_x())
+        assert err <= tol, (nt, err)
+        assert o.stats()["s"] == plain.stats()["s"] and o.proximity()[1] == plain.proximity()[1]
+        assert abs(o.proximity()[0] - plain.proximity()[0]) <= max(tol, 0.0) * plain.proximity()[0]
+        assert abs(o.cost() - plain.cost()) <= max(tol, 0.0) * plain.cost()
+
+
+def test_state_snapshot_continues_bit_for_bit(plan0):
+    """get_state / set_state (+ x) carry everything Fig. 3 keeps between calls: a second oracle resumed from the snapshot
+    continues exactly as the first (bench.py times the one-thread oracle from the all-cores oracle's warm state this way)."""
+    a = orc.from_plan(plan0); a.set_option(orc.OPT_ETA, 0.97)
+    a.set_x(plan0.x0); a.iterate(6, 1.0, 1.0, 0.9)
+    b = orc.from_plan(plan0); b.set_option(orc.OPT_ETA, 0.97)
+    b.set_x(a.get_x()); b.set_state(a.get_state())
+    a.iterate(6, 1.0, 1.0, 0.9); b.iterate(6, 1.0, 1.0, 0.9)
+    assert np.array_equal(a.get_x(), b.get_x()) and a.stats() == b.stats()
