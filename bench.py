@@ -39,10 +39,31 @@ UNIT = "iterations/s"
 DEFAULT_CONFIG = 3          # BASELINE.json configs[3]: the clinical-size plan the metric is quoted on (fits one B200)
 DEFAULT_STEPS = {0: 50, 1: 200, 2: 100, 3: 50}
 NOMINAL_HBM_GBS = 8000.0    # north_star's "~8 TB/s peak" (context; the roofline denominator is the measured copy figure)
-# dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel from the committed `ncu --set full`
-# capture (profiles/r01_ncu_full_config3.md); keyed by (config, pass); a transposed pass = k_transpose + k_combine
-NCU_TRAFFIC = {(3, "forward_x"): 957143296, (3, "transpose_g"): 901036288, (3, "forward_g"): 953572608,
-               (3, "transpose_b"): 971151616}
+TRAFFIC_FILE = os.path.join(ROOT, "profiles", "r02_traffic.csv")   # DRAM bytes per launch from the committed ncu capture
+KERNEL_SOURCES = ("fredopt_kernels.cuh", "kernels_iter.cuh")       # the capture is valid for these sources only (hash)
+CPU_BUDGET_S = 25.0         # bound of the all-cores oracle leg of the default run
+
+
+def kernel_source_hash():
+    import hashlib
+    h = hashlib.sha256()
+    for f in KERNEL_SOURCES:
+        h.update(open(os.path.join(ROOT, "paper_2509_20012_b200", "csrc", f), "rb").read())
+    return h.hexdigest()[:16]
+
+
+def captured_traffic(config, pass_name):
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch of `pass_name` from the committed `ncu --set full` capture, or None
+    when there is none for this configuration or the kernel sources have changed since (rows: config,pass,dram_bytes,hash)."""
+    try:
+        cur = kernel_source_hash()
+        for line in open(TRAFFIC_FILE):
+            c = [t.strip() for t in line.split(",")]
+            if len(c) >= 4 and c[0] == str(config) and c[1] == pass_name and c[3] == cur:
+                return int(c[2])
+    except Exception:
+        pass
+    return None
 
 
 def _peaks():
@@ -112,7 +133,8 @@ def _dist_init():
 
 # ------------------------------------------------------------------------------------------------ reference arm
 def run_reference(args):
-    """The oracle, as it stands, on the host cores: a bounded sample of the same workload per step."""
+    """The oracle, as it stands, on the host cores (its OpenMP timing build: the same source, row loops on all cores): the same
+    window as our arm -- W warm-up iterations from x0, then K timed iterations of the full plan."""
     ws, rank, _ = _dist_init()
     if rank != 0:
         return
@@ -120,7 +142,8 @@ def run_reference(args):
     from paper_2509_20012_b200 import plangen as pg
     spec = pg.config_spec(args.config)
     plan = pg.build_plan(spec, device="cuda" if torch.cuda.is_available() else "cpu")
-    orc = oracle.from_plan(plan)
+    cores = oracle.omp_threads()
+    orc = oracle.from_plan(plan, omp=True)
     orc.set_x(plan.x0)
     K, W = args.steps, args.warmup
     orc.iterate(W, spec.lam, spec.beta0, spec.a)
@@ -128,13 +151,14 @@ def run_reference(args):
     orc.iterate(K, spec.lam, spec.beta0, spec.a)
     dt = time.perf_counter() - t0
     v = K / dt
-    sample = f"{K} superiorized iterations of configs[{args.config}] ({spec.name}), full plan, after {W} warm-up iterations"
+    sample = (f"iterations {W}..{W + K - 1} from x0 of configs[{args.config}] ({spec.name}), full plan: the window of our arm; fp64 oracle, "
+              f"OpenMP timing build, {cores} threads")
     print(json.dumps({
         "impl": "reference", "metric": METRIC, "value": v, "unit": UNIT, "n_gpus": args.gpus, "steps": K, "warmup": W,
         "ms_per_step": 1e3 * dt / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
         "data": "synthetic", "config": {"workload": f"configs[{args.config}] {spec.name}", "nnz": plan.nnz,
                                         "n_spots": plan.n_cols, "n_voxels": plan.n_rows},
-        "cpu_baseline": {"value": v, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
+        "cpu_baseline": {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
         "e2e": {"value": v, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0}))
 
@@ -180,7 +204,20 @@ def run_ours(args):
         copt["block_rows"] = args.block_rows
     if args.index_width:
         copt["index_width"] = args.index_width
+    sharded = bool(args.shard) and ws > 1
+    if sharded:                          # ONE plan on all ranks: voxel ranges, x replicated, sums completed by an NCCL all-reduce
+        copt.update(shard_rank=rank, shard_world=ws)
     gp = fredopt.from_plan(plan, stream=stream.cuda_stream, **copt)
+    if sharded:
+        views = {}
+
+        def allreduce(ptr, n, cuda_stream):
+            t = views.get((ptr, n))
+            if t is None:
+                t = views[(ptr, n)] = torch.as_tensor(fredopt.DeviceDoubles(ptr, n), device="cuda")
+            with torch.cuda.stream(stream):                 # the plan's stream: NCCL orders the collective after the work queued on it
+                dist.all_reduce(t)
+        gp.set_reduce(allreduce)
     torch.cuda.synchronize()
     t_create = time.perf_counter() - t0
     if args.block_sequential:
@@ -276,10 +313,10 @@ def run_ours(args):
         if dist is not None:
             dist.destroy_process_group()
         return
-    value = whole_job_rate(K, ws, ms * 1e-3)
+    value = whole_job_rate(K, 1 if sharded else ws, ms * 1e-3)      # sharded: the ranks advance ONE plan together
     out = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": ws, "steps": K, "warmup": W, "ms_per_step": ms / K,
-        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+        "higher_is_better": True, "scaling": "strong" if sharded else "weak", "vs_baseline": None, "dtype": "f64",
         "data": "synthetic",
         "config": {"workload": f"configs[{args.config}] {spec.name}", "n_voxels": plan.n_rows, "n_spots": plan.n_cols,
                    "nnz_per_matrix": plan.nnz, "nnz_active": stats["nnz_active"], "n_active_rows": stats["n_active_rows"],
@@ -293,14 +330,17 @@ def run_ours(args):
                    "l2": ("L2-resident working set (%.1f MB < 2 x L2): L2 flushed once before the timed region; "
                           "HBM fraction not meaningful" % (iter_bytes / 1e6)) if flush is not None else
                          "inputs larger than L2 (%.2f GB streamed per iteration)" % (iter_bytes / 1e9),
-                   "parallelism": "1 plan per GPU"},
+                   "parallelism": ("one plan sharded over %d GPUs by voxel range (x replicated, 3 all-reduces of <= n_spots + 3 doubles per "
+                                   "iteration)" % ws) if sharded else "1 plan per GPU"},
         "iter_gbs": iter_bytes * K / (ms * 1e-3) / 1e9,
-        "e2e": {"value": whole_job_rate(K, ws, e2e_s), "unit": UNIT, "h2d_bytes_per_step": plan.n_cols * 4,
+        "e2e": {"value": whole_job_rate(K, 1 if sharded else ws, e2e_s), "unit": UNIT, "h2d_bytes_per_step": plan.n_cols * 4,
                 "d2h_bytes_per_step": plan.n_cols * 4 + STATE_BYTES},
         "gpu_launches": int(launches),
         "clocks": clocks,
         "roofline": {"bound": "hbm", "kernel": top, "kernel_names": PASS_KERNELS.get(top, top), "achieved": achieved, "peak": peak, "unit": "GB/s",
-                     "frac": achieved / peak, "traffic": NCU_TRAFFIC.get((args.config, top)), "peak_source": peak_src,
+                     "frac": achieved / peak, "traffic": captured_traffic(args.config, top),
+                     "traffic_source": "profiles/r02_traffic.csv (ncu --set full capture; null when the kernel sources changed since)",
+                     "peak_source": peak_src,
                      "alg_bytes_per_launch": pass_bytes[top], "ms_per_launch": top_ms,
                      "frac_of_nominal_8TBs": achieved / NOMINAL_HBM_GBS, "read_ceiling_gbs": read_gbs,
                      "frac_of_read_ceiling": achieved / read_gbs,
@@ -309,28 +349,85 @@ def run_ours(args):
         "setup": {"generate_s": t_gen, "create_s": t_create},
         "final": {"prox": prox, "n_violated": nviol, "trials": stats["trials"]},
     }
+    if ws == 1 and not args.no_forms and not args.ams:
+        out["forms"] = compare_forms(gp, fredopt, plan, K, W, lam, beta0, a, stream)
     if ws == 1 and not args.no_cpu_baseline:
-        out["cpu_baseline"] = cpu_baseline(plan, spec, args)
+        out["cpu_baseline"] = cpu_baseline(plan, spec, args, lam, beta0, a)
     print(json.dumps(out))
     if dist is not None:
         dist.destroy_process_group()
 
 
-def cpu_baseline(plan, spec, args):
-    """The oracle as it stands, single thread, on a bounded sample (about 10-30 s) of the same workload."""
+def compare_forms(gp, fredopt, plan, K, W, lam, beta0, a, stream):
+    """What an iteration buys in each feasibility-seeking form (iterations/s alone favours the form that moves x
+    least).  For the simultaneous step (reading R1, the form `value` times) and the block-sequential sweep (R23, Fig. 2's own loop
+    nest): iterations/s over the same window, proximity and violated sets (fredopt_proximity) after W + K iterations from x0, and
+    the time either form needs to bring the proximity down to what the block-sequential form reaches in that window."""
+    res = {}
+
+    def run(block, n, timed):
+        gp.set_option(fredopt.OPT_BLOCK_SEQUENTIAL, block)
+        gp.set_option(fredopt.OPT_RESET, 1)
+        gp.set_weights(plan.x0)
+        gp.iterate(W, lam, beta0, a)
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(stream); gp.iterate(n, lam, beta0, a); e1.record(stream)
+        torch.cuda.synchronize()
+        return e0.elapsed_time(e1) * 1e-3
+
+    for name, block in (("simultaneous", 0), ("block_sequential", 1)):
+        dt = run(block, K, True)
+        p, nv = gp.proximity(None)
+        res[name] = {"iterations_per_s": K / dt, "prox_after": p, "n_violated_after": nv, "iterations": W + K}
+    target = res["block_sequential"]["prox_after"]
+    for name, block in (("simultaneous", 0), ("block_sequential", 1)):
+        gp.set_option(fredopt.OPT_BLOCK_SEQUENTIAL, block); gp.set_option(fredopt.OPT_RESET, 1); gp.set_weights(plan.x0)
+        done, secs, hit, step, cap = 0, 0.0, None, 25, 2000
+        while done < cap:
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(stream); gp.iterate(step, lam, beta0, a); e1.record(stream)
+            torch.cuda.synchronize()
+            secs += e0.elapsed_time(e1) * 1e-3; done += step
+            if gp.proximity(None)[0] <= target:
+                hit = done
+                break
+        res[name]["to_target"] = {"prox_target": target, "iterations": hit, "seconds": secs if hit else None,
+                                  "note": None if hit else f"not reached within {cap} iterations ({secs:.2f} s)"}
+    gp.set_option(fredopt.OPT_BLOCK_SEQUENTIAL, 0); gp.set_option(fredopt.OPT_RESET, 1)
+    return res
+
+
+def cpu_baseline(plan, spec, args, lam, beta0, a):
+    """The oracle as it stands on the host cores, over the window our arm times: W warm-up iterations from x0, then K timed.
+    All cores = the OpenMP timing build of the same source; the leg is bounded (CPU_BUDGET_S): if the K iterations would not fit,
+    fewer are timed and `sample` says so.  One thread = the plain build, continued from the all-cores oracle's state after the
+    warm-up (same x, k, s, beta), over the first iterations of the same window."""
     from oracle import oracle
-    orc = oracle.from_plan(plan)
+    K, W = args.steps, args.warmup
+    cores = oracle.omp_threads()
+    orc = oracle.from_plan(plan, omp=True)
     orc.set_x(plan.x0)
     t0 = time.perf_counter()
-    orc.iterate(1, spec.lam, spec.beta0, spec.a)
-    t1 = time.perf_counter() - t0
-    n = int(max(1, min(200, 15.0 / max(t1, 1e-6))))
+    orc.iterate(W, lam, beta0, a)
+    t_warm = time.perf_counter() - t0
+    x_w, st_w = orc.get_x(), orc.get_state()
+    per = t_warm / max(W, 1)
+    k_all = int(max(1, min(K, CPU_BUDGET_S / max(per, 1e-9))))
     t0 = time.perf_counter()
-    orc.iterate(n, spec.lam, spec.beta0, spec.a)
+    orc.iterate(k_all, lam, beta0, a)
     dt = time.perf_counter() - t0
-    return {"value": n / dt, "unit": UNIT, "cores": 1, "kind": "oracle",
-            "sample": f"{n} superiorized iterations of the same plan (after 1 warm-up iteration), fp64, single thread"}
-
+    one = oracle.from_plan(plan)
+    one.set_x(x_w); one.set_state(st_w)
+    k_one = int(max(1, min(k_all, 0.5 * CPU_BUDGET_S / max(dt / k_all * cores * 0.5, 1e-9))))
+    t0 = time.perf_counter()
+    one.iterate(k_one, lam, beta0, a)
+    dt1 = time.perf_counter() - t0
+    what = "superiorized" if beta0 else "pure feasibility-seeking"
+    return {"value": k_all / dt, "unit": UNIT, "cores": cores, "kind": "oracle",
+            "sample": f"{what} iterations {W}..{W + k_all - 1} from x0 of the same plan (our arm times {W}..{W + K - 1}), fp64 oracle, "
+                      f"OpenMP timing build, {cores} threads",
+            "one_thread": {"value": k_one / dt1, "unit": UNIT, "cores": 1,
+                           "sample": f"iterations {W}..{W + k_one - 1} of the same window, plain build, continued from the same state"}}
 
 
 # ------------------------------------------------------------------------------------------------ configs[4]: pass sweep
@@ -431,6 +528,9 @@ def main():
                     help="feasibility-seeking step in the block-sequential form of Fig. 2's loop nest (DESIGN.md R23)")
     ap.add_argument("--ams", action="store_true",
                     help="pure feasibility-seeking (beta0 = 0, the paper's 'AMS' runs, PAPER.md:120): two passes per iteration")
+    ap.add_argument("--shard", action="store_true",
+                    help="with --gpus N > 1 (torchrun): ONE plan sharded over the ranks by voxel range (strong scaling; DESIGN.md Multi-GPU)")
+    ap.add_argument("--no-forms", action="store_true", help="skip the comparison of the two feasibility-seeking forms")
     ap.add_argument("--block-rows", type=int, default=0, help="fredopt_create_options.block_rows (0 = automatic)")
     ap.add_argument("--index-width", type=int, default=0, help="fredopt_create_options.index_width (0 = automatic, 32)")
     ap.add_argument("--no-pdl", action="store_true", help="FREDOPT_OPT_USE_PDL = 0 (plain launches)")

@@ -20,11 +20,13 @@ def nvcc_path() -> str:
     return "nvcc"
 
 
-def build_library(force: bool = False, verbose: bool = False) -> str:
-    if not force and os.path.exists(LIB) and all(os.path.getmtime(LIB) >= os.path.getmtime(d) for d in DEPS):
+def build_library(force: bool = False, verbose: bool = False, defines=()) -> str:
+    """defines: extra -D... flags (the compile-time tunables of csrc/fredopt_kernels.cuh, e.g. -DFWD_U1=8; timing experiments
+    such as -DEXP_NO_GATHER give wrong results on purpose).  A build with defines always recompiles."""
+    if not force and not defines and os.path.exists(LIB) and all(os.path.getmtime(LIB) >= os.path.getmtime(d) for d in DEPS):
         return LIB
     cmd = [nvcc_path(), "-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "--threads", "0",
-           "-Xcompiler", "-fPIC", "-shared", "-o", LIB] + SOURCES
+           "-Xcompiler", "-fPIC", "-shared", "-o", LIB] + list(defines) + SOURCES
     if verbose:
         cmd.insert(1, "-Xptxas=-v")
         print(" ".join(cmd), file=sys.stderr)
@@ -33,4 +35,4 @@ def build_library(force: bool = False, verbose: bool = False) -> str:
 
 
 if __name__ == "__main__":
-    print(build_library(force="--force" in sys.argv, verbose="-v" in sys.argv))
+    print(build_library(force="--force" in sys.argv, verbose="-v" in sys.argv, defines=[a for a in sys.argv[1:] if a.startswith("-D")]))
