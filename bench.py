@@ -226,6 +226,8 @@ def run_ours(args):
         gp.set_option(fredopt.OPT_WORK_QUEUE, args.work_queue)
     if args.no_pdl:
         gp.set_option(fredopt.OPT_USE_PDL, 0)
+    if args.skip_satisfied:
+        gp.set_option(fredopt.OPT_SKIP_SATISFIED, 1)
     st0 = gp.stats()
     K, W = args.steps, args.warmup
     lam, beta0, a = spec.lam, (0.0 if args.ams else spec.beta0), spec.a
@@ -284,6 +286,8 @@ def run_ours(args):
     gp.set_option(fredopt.OPT_TIME_PASSES, 1)
     gp.iterate(min(K, 50), lam, beta0, a)
     pt = gp.pass_times()
+    pass_bytes_static = pass_bytes
+    pass_bytes = gp.pass_bytes_timed()     # as the timed launches needed them: the back-projection reads the values of rows with a coefficient only
     gp.set_option(fredopt.OPT_TIME_PASSES, 0)
     # ---- practical ceiling of a 100%-read pass: the library's streaming-read kernel over a buffer larger than L2
     nb = 1 << 31
@@ -302,9 +306,12 @@ def run_ours(args):
     top_ms = pt[top][0] / max(pt[top][1], 1)
     peak, peak_src = _peaks()
     achieved = pass_bytes[top] / (top_ms * 1e-3) / 1e9
-    passes = {n: {"ms": pt[n][0] / max(pt[n][1], 1), "alg_bytes": pass_bytes[n],
+    passes = {n: {"ms": pt[n][0] / max(pt[n][1], 1), "alg_bytes": pass_bytes[n], "alg_bytes_all_rows": pass_bytes_static[n],
                   "gbs": pass_bytes[n] / max(pt[n][0] / max(pt[n][1], 1), 1e-9) / 1e6} for n in pt if pt[n][1] > 0}
     stats = gp.stats()
+    # bytes one iteration needs, with the back-projection as the timed launches needed it (rows with a non-zero coefficient)
+    iter_bytes_all_rows = iter_bytes
+    iter_bytes = sum(pass_bytes[n] for n in (("forward_x", "transpose_b") if args.ams else PASS_KERNELS) if n in pass_bytes)
     spmv = ("forward_x", "transpose_b") if args.ams else ("forward_x", "transpose_g", "forward_g", "transpose_b")
     four_gbs = sum(pass_bytes[n] for n in spmv if n in passes) / max(sum(passes[n]["ms"] for n in spmv if n in passes), 1e-9) / 1e6
 
@@ -326,6 +333,9 @@ def run_ours(args):
                    "storage": "fp32 matrix values, 16-bit indices where exact (else int32), fp64 vectors and accumulators",
                    "ams_form": "block-sequential (Fig. 2 loop nest, R23)" if args.block_sequential else "simultaneous (R1)",
                    "passes_per_iteration": 2 if args.ams else 4, "alg_bytes_per_iteration": iter_bytes,
+                   "alg_bytes_per_iteration_all_rows": iter_bytes_all_rows,
+                   "back_projection": "values of rows with a non-zero coefficient only (--skip-satisfied)" if args.skip_satisfied else
+                                      "every value",
                    "form": "pure feasibility-seeking (beta0 = 0)" if args.ams else "superiorized",
                    "l2": ("L2-resident working set (%.1f MB < 2 x L2): L2 flushed once before the timed region; "
                           "HBM fraction not meaningful" % (iter_bytes / 1e6)) if flush is not None else
@@ -534,6 +544,8 @@ def main():
     ap.add_argument("--block-rows", type=int, default=0, help="fredopt_create_options.block_rows (0 = automatic)")
     ap.add_argument("--index-width", type=int, default=0, help="fredopt_create_options.index_width (0 = automatic, 32)")
     ap.add_argument("--no-pdl", action="store_true", help="FREDOPT_OPT_USE_PDL = 0 (plain launches)")
+    ap.add_argument("--skip-satisfied", action="store_true",
+                    help="FREDOPT_OPT_SKIP_SATISFIED = 1: the back-projection streams the values of rows with a non-zero coefficient only")
     ap.add_argument("--work-queue", type=int, default=None, help="FREDOPT_OPT_WORK_QUEUE (bit 0 forward, bit 1 transposed passes)")
     ap.add_argument("--sweep", action="store_true", help="BASELINE.json configs[4]: isolated-pass sweep (1 GPU)")
     ap.add_argument("--quick", action="store_true", help="with --sweep: two points only")

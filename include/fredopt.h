@@ -123,6 +123,12 @@ typedef struct {
                                        /*    / transposed items are taken longest first instead of in storage order.  Default 13      */
 #define FREDOPT_OPT_USE_PDL         10 /* 1 (default): the kernels of an iteration are launched with programmatic dependent    */
                                        /*    launch (a kernel's CTAs are scheduled while its predecessor drains); 0: plain launches */
+#define FREDOPT_OPT_SKIP_SATISFIED  12 /* 1: the back-projection of the simultaneous step streams the values of a row only if the row   */
+                                       /*    carries a non-zero coefficient (Fig. 2 touches a row only when its test fires,            */
+                                       /*    PAPER.md:129-146); every skipped term is an exact zero: the result has the same bits.     */
+                                       /*    Default 0 (stream every value): on the configs[3] plan 65-75 % of the entries stay live    */
+                                       /*    over the first hundreds of iterations and looking up liveness costs more than the 25-35 %  */
+                                       /*    of values it saves ("Measured dead ends"); it pays close to feasibility         */
 #define FREDOPT_OPT_ONE_SIDED_COST   9 /* 1: the OAR term of Eq. (2) penalises only cDL above cDLref: w (cDL - cDLref)_+^2 */
                                        /*    (Eq. (2) as printed is two-sided: default 0; R11)   */
 
@@ -276,6 +282,12 @@ int fredopt_spmv_transpose(fredopt_plan *plan, int32_t rows, const float *u, con
 int fredopt_get_pass_times(fredopt_plan *plan, double *ms, int64_t *launches);
 /* Algorithmic bytes of ONE launch of each pass ("Bytes"): FREDOPT_N_PASSES entries, HOST pointer. */
 int fredopt_get_pass_bytes(fredopt_plan *plan, int64_t *bytes);
+
+/* The same for the launches timed since TIME_PASSES was set to 1 (mean per launch).  It differs from fredopt_get_pass_bytes in
+ * the back-projection pass, whose need depends on the iterate: every stored index, but the values of those entries only whose
+ * (block) row had a non-zero coefficient in that launch (FREDOPT_OPT_SKIP_SATISFIED; counted on the device by a separate kernel
+ * after each timed launch).  Without timed launches: the static figures.  Synchronises. */
+int fredopt_get_pass_bytes_timed(fredopt_plan *plan, int64_t *bytes);
 
 /* Number of kernels this library has launched on behalf of `plan` since creation. */
 int64_t fredopt_launch_count(fredopt_plan *plan);

@@ -41,6 +41,10 @@ constexpr int TR_ITEM_MAX = TR_ITEM_MAX_ENTRIES;   // entries per transposed wor
 #ifndef FWD_MIN_CTAS_PER_SM
 #define FWD_MIN_CTAS_PER_SM 4
 #endif
+// spare (zeroed) elements behind every stored index array: tr_item_live loads the indices of a trip one trip ahead and may run
+// up to U + 1 chunks of 128 entries past the last item; such words are never used
+constexpr size_t IDX_SLACK = 1024;
+static_assert(128 * (FWD_U1 + 1) <= IDX_SLACK && 128 * (FWD_U3 + 1) <= IDX_SLACK, "index look-ahead stays inside the spare elements");
 constexpr int FWD_MIN_CTAS = FWD_MIN_CTAS_PER_SM;   // resident CTAs per SM the item kernels are compiled for (4: 64 registers)
 
 // flags of a structure
@@ -125,8 +129,10 @@ __device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;"
 __device__ __forceinline__ void pdl_trigger() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
 
 // ------------------------------------------------------------------------------------------ loads
-#ifdef EXP_NO_GATHER          /* timing experiment only (results are wrong): the gathered value is replaced by the index */
-#define FWD_GATHER(x, c) ((double)(c))
+// Timing experiments (results are WRONG on purpose; profiles/r02_ceilings.md): -DEXP_NO_GATHER makes the gathered value from the
+// index without a load, -DEXP_NO_CVT skips the fp32 -> fp64 conversion, -DEXP_NO_FMA replaces the fp64 multiply-add by an xor.
+#ifdef EXP_NO_GATHER
+#define FWD_GATHER(x, c) __hiloint2double(0x3ff00000, (c))
 #else
 #define FWD_GATHER(x, c) __ldg((x) + (c))
 #endif
@@ -178,6 +184,41 @@ __device__ __forceinline__ void ld_idx(const void* __restrict__ base, long long 
         }
     }
 }
+// the same indices as loaded (16-bit form: two per word), unpacked where they are used: tr_item_live keeps the indices of the
+// next trip in registers
+template <bool I16, int C> struct IdxRaw { unsigned int w[I16 ? (C + 1) / 2 : C]; };
+template <bool I16, int C>
+__device__ __forceinline__ void ld_idx_raw(const void* __restrict__ base, long long i, IdxRaw<I16, C>& r) {
+    if (I16) {
+        const uint16_t* p = (const uint16_t*)base + i;
+        if (C == 4) {
+            asm volatile("ld.global.nc.L1::no_allocate.v2.u32 {%0,%1}, [%2];" : "=r"(r.w[0]), "=r"(r.w[(C + 1) / 2 - 1]) : "l"(p));
+        } else if (C == 2) {
+            asm volatile("ld.global.nc.L1::no_allocate.u32 %0, [%1];" : "=r"(r.w[0]) : "l"(p));
+        } else {
+            unsigned short lo;
+            asm volatile("ld.global.nc.L1::no_allocate.u16 %0, [%1];" : "=h"(lo) : "l"(p));
+            r.w[0] = lo;
+        }
+    } else {
+        const int32_t* p = (const int32_t*)base + i;
+        if (C == 4) {
+            asm volatile("ld.global.nc.L1::no_allocate.v4.u32 {%0,%1,%2,%3}, [%4];" : "=r"(r.w[0]), "=r"(r.w[1 % C]), "=r"(r.w[2 % C]), "=r"(r.w[3 % C]) : "l"(p));
+        } else if (C == 2) {
+            asm volatile("ld.global.nc.L1::no_allocate.v2.u32 {%0,%1}, [%2];" : "=r"(r.w[0]), "=r"(r.w[1 % C]) : "l"(p));
+        } else {
+            asm volatile("ld.global.nc.L1::no_allocate.u32 %0, [%1];" : "=r"(r.w[0]) : "l"(p));
+        }
+    }
+}
+template <bool I16, int C>
+__device__ __forceinline__ int idx_get(const IdxRaw<I16, C>& r, int j, int add) {
+    if (I16) {
+        const unsigned int w = r.w[j / 2];
+        return (int)((j & 1) ? (w >> 16) : (w & 0xFFFFu)) + add;
+    }
+    return (int)r.w[j];
+}
 __device__ __forceinline__ Item ld_item(const Item* p) {
     const int4 v = __ldg((const int4*)p);
     Item it;
@@ -190,7 +231,7 @@ __device__ __forceinline__ Item ld_item(const Item* p) {
 template <int R>
 __device__ __forceinline__ void ld_coef(const double* __restrict__ v, int b, double (&g)[R]) {
 #ifdef EXP_NO_GATHER
-    for (int k = 0; k < R; ++k) g[k] = (double)b;
+    for (int k = 0; k < R; ++k) g[k] = __hiloint2double(0x3ff00000, b + k);
     return;
 #endif
     if (R == 1) g[0] = __ldg(v + b);
@@ -205,7 +246,7 @@ __device__ __forceinline__ void ld_coef(const double* __restrict__ v, int b, dou
 template <int R>
 __device__ __forceinline__ void ld_coef_pair(const double2* __restrict__ v, int b, double (&gd)[R], double (&gl)[R]) {
 #ifdef EXP_NO_GATHER
-    for (int k = 0; k < R; ++k) { gd[k] = (double)b; gl[k] = (double)b; }
+    for (int k = 0; k < R; ++k) { gd[k] = __hiloint2double(0x3ff00000, b + k); gl[k] = __hiloint2double(0x3ff00000, b - k); }
     return;
 #endif
     if (R == 1) { const double2 t = __ldg(v + b); gd[0] = t.x; gl[0] = t.y; }
@@ -238,6 +279,21 @@ __device__ __forceinline__ double block_sum(double v, double* sm) {
 }
 
 __device__ __forceinline__ float f4_get(const float4& a, int i) { return i == 0 ? a.x : i == 1 ? a.y : i == 2 ? a.z : a.w; }
+// a stored value as fp64 and the multiply-add of the matrix passes (the experiments above replace them)
+__device__ __forceinline__ double f2d(float v) {
+#ifdef EXP_NO_CVT
+    return __hiloint2double(0x3ff00000, (int)__float_as_uint(v));
+#else
+    return (double)v;
+#endif
+}
+__device__ __forceinline__ double fma_op(double a, double b, double c) {
+#ifdef EXP_NO_FMA
+    return __longlong_as_double(__double_as_longlong(a) ^ __double_as_longlong(b) ^ __double_as_longlong(c));
+#else
+    return fma(a, b, c);
+#endif
+}
 
 // signed residual of a hyperslab lo <= val <= hi (NaN = absent): upper violations > 0, lower < 0
 __device__ __forceinline__ double slab_residual(double val, double lo, double hi) {
@@ -290,6 +346,7 @@ struct ResidArgs {
     double *part_prox, *part_phi;        // out: per-CTA partial sums
     long long* part_cnt;
     DevState* st;                        // relax = lambda eta^k, eta^k and k advance when uv is written
+    uint8_t* live;                       // out: per block row, 1 iff one of its rows has a non-zero step coefficient (with uv)
 };
 
 // ------------------------------------------------------------------------------------------ work distribution
@@ -345,8 +402,8 @@ __device__ __forceinline__ void fwd_row(const void* __restrict__ cbase, long lon
             for (int j = 0; j < C; ++j)
 #pragma unroll
                 for (int k = 0; k < R; ++k) {
-                    if (M & 1) aD[k] = fma((double)f4_get(d[u], j * R + k), xv[j], aD[k]);
-                    if (M & 2) aL[k] = fma((double)f4_get(l[u], j * R + k), xv[j], aL[k]);
+                    if (M & 1) aD[k] = fma_op(f2d(f4_get(d[u], j * R + k)), xv[j], aD[k]);
+                    if (M & 2) aL[k] = fma_op(f2d(f4_get(l[u], j * R + k)), xv[j], aL[k]);
                 }
         }
     }
@@ -375,8 +432,8 @@ __device__ __forceinline__ void fwd_row(const void* __restrict__ cbase, long lon
                 for (int j = 0; j < C; ++j)
 #pragma unroll
                     for (int k = 0; k < R; ++k) {
-                        if (M & 1) aD[k] = fma((double)f4_get(d[u], j * R + k), xv[j], aD[k]);
-                        if (M & 2) aL[k] = fma((double)f4_get(l[u], j * R + k), xv[j], aL[k]);
+                        if (M & 1) aD[k] = fma_op(f2d(f4_get(d[u], j * R + k)), xv[j], aD[k]);
+                        if (M & 2) aL[k] = fma_op(f2d(f4_get(l[u], j * R + k)), xv[j], aL[k]);
                     }
             }
         }
@@ -429,6 +486,7 @@ k_forward(long long n, const Item* __restrict__ items, const int32_t* __restrict
         if (lane == 0) {
             double csum = 0.0, rprox = 0.0, rphi = 0.0;
             long long rcnt = 0;
+            int nzb = 0;
 #pragma unroll
             for (int k = 0; k < R; ++k) {
                 if (k >= nrow) break;
@@ -463,11 +521,15 @@ k_forward(long long n, const Item* __restrict__ items, const int32_t* __restrict
                         row_residual(tab[seg], row_bounds(tab[seg], vb, r), ra.st->flags & SF_ONE_SIDED, dv, lv, ra.nD[r], ra.nL[r], ra.nT[r], u, v,
                                      rcnt, rprox, rphi);
                         if (ra.uv.pair) gv_store(ra.uv, r, u, v);
+                        nzb |= (u != 0.0) | (v != 0.0);
                     }
                 }
             }
             if (EPI == EPI_CPART || EPI == EPI_STORE_PQ) cpart[b] = csum;
-            if (EPI == EPI_RESID) { ra.part_prox[b] = rprox; ra.part_phi[b] = rphi; ra.part_cnt[b] = rcnt; }
+            if (EPI == EPI_RESID) {
+                ra.part_prox[b] = rprox; ra.part_phi[b] = rphi; ra.part_cnt[b] = rcnt;
+                if (ra.uv.pair) ra.live[b] = (uint8_t)nzb;
+            }
         }
         e0 = e1;
         e1 = wq ? 2 * nwarps + (int)__shfl_sync(0xffffffffu, e2, 0) : e1 + nwarps;      // no queue: static round-robin
@@ -542,15 +604,15 @@ __device__ __forceinline__ double tr_item(const void* __restrict__ cbase, long l
             double gd[R], gl[R];                                                                           \
             ld_coef_pair<R>(vec, c[u][j], gd, gl);                                                         \
             _Pragma("unroll") for (int k = 0; k < R; ++k) {                                                \
-                aD = fma((double)f4_get(d[u], j * R + k), gd[k], aD);                                      \
-                aL = fma((double)f4_get(l[u], j * R + k), gl[k], aL);                                      \
+                aD = fma_op(f2d(f4_get(d[u], j * R + k)), gd[k], aD);                                      \
+                aL = fma_op(f2d(f4_get(l[u], j * R + k)), gl[k], aL);                                      \
             }                                                                                              \
         } else {                                                                                           \
             double g[R];                                                                                   \
             ld_coef<R>(vs, c[u][j], g);                                                                    \
             _Pragma("unroll") for (int k = 0; k < R; ++k) {                                                \
-                if (M == 1) aD = fma((double)f4_get(d[u], j * R + k), g[k], aD);                           \
-                else aL = fma((double)f4_get(l[u], j * R + k), g[k], aL);                                  \
+                if (M == 1) aD = fma_op(f2d(f4_get(d[u], j * R + k)), g[k], aD);                           \
+                else aL = fma_op(f2d(f4_get(l[u], j * R + k)), g[k], aL);                                  \
             }                                                                                              \
         }                                                                                                  \
     }
@@ -589,15 +651,101 @@ __device__ __forceinline__ double tr_item(const void* __restrict__ cbase, long l
     return aD + aL;
 }
 
+// The same sum where most coefficients are zero (the back-projection of Fig. 2 touches a row only when its test fires,
+// PAPER.md:129-146; after a few dozen iterations most sets are satisfied): live[b] != 0 iff block row b has a non-zero
+// coefficient (written by the residual pass that wrote the coefficients).  A lane streams its 16 bytes of values per matrix and
+// gathers only where one of its C entries is live; every skipped term is an exact zero, so the sum has the same bits.  The
+// indices are needed BEFORE the values: those of a trip are loaded one trip ahead (a word or two per chunk and lane) and the
+// liveness bytes (L1-resident) are looked up at the start of the trip.
+template <int M, int R, bool I16>
+__device__ __forceinline__ double tr_item_live(const void* __restrict__ cbase, long long v0, int add, const float* __restrict__ dp,
+                                               const float* __restrict__ lp, int Lv, int lane, const GatherVec& gv,
+                                               const uint8_t* __restrict__ live) {
+    constexpr int C = 4 / R;
+    constexpr int U = (M == 3) ? FWD_U3 : FWD_U1;
+    const double2* __restrict__ vec = gv.pair;
+    const double* __restrict__ vs = (M == 2) ? gv.cL : gv.cD;
+    const long long i0 = v0 / R;
+    double aD = 0.0, aL = 0.0;
+    int p = lane * 4;
+#define TRL_CONSUME(cc, u)                                                                                \
+    _Pragma("unroll") for (int j = 0; j < C; ++j) {                                                        \
+        if ((lv >> ((u) * C + j)) & 1u) {                                                                  \
+            const int b = (idx_get<I16, C>(cc[u], j, add));                                                \
+            if (M == 3) {                                                                                  \
+                double gd[R], gl[R];                                                                       \
+                ld_coef_pair<R>(vec, b, gd, gl);                                                           \
+                _Pragma("unroll") for (int k = 0; k < R; ++k) {                                            \
+                    aD = fma_op(f2d(f4_get(d[u], j * R + k)), gd[k], aD);                                  \
+                    aL = fma_op(f2d(f4_get(l[u], j * R + k)), gl[k], aL);                                  \
+                }                                                                                          \
+            } else {                                                                                       \
+                double g[R];                                                                               \
+                ld_coef<R>(vs, b, g);                                                                      \
+                _Pragma("unroll") for (int k = 0; k < R; ++k) {                                            \
+                    if (M == 1) aD = fma_op(f2d(f4_get(d[u], j * R + k)), g[k], aD);                       \
+                    else aL = fma_op(f2d(f4_get(l[u], j * R + k)), g[k], aL);                              \
+                }                                                                                          \
+            }                                                                                              \
+        }                                                                                                  \
+    }
+    IdxRaw<I16, C> cn[U];                        // the indices of the next trip
+#pragma unroll
+    for (int u = 0; u < U; ++u) ld_idx_raw<I16, C>(cbase, i0 + (p + 128 * u) / R, cn[u]);
+    for (; p + 128 * (U - 1) < Lv; p += 128 * U) {
+        IdxRaw<I16, C> c[U];
+        float4 d[U], l[U];
+        unsigned int lv = 0u;                    // bit u * C + j: entry j of chunk u is live
+#pragma unroll
+        for (int u = 0; u < U; ++u) {
+            c[u] = cn[u];
+#pragma unroll
+            for (int j = 0; j < C; ++j) lv |= (__ldg(live + idx_get<I16, C>(c[u], j, add)) ? 1u : 0u) << (u * C + j);
+        }
+#pragma unroll
+        for (int u = 0; u < U; ++u) {
+            const bool any = (lv >> (u * C)) & ((1u << C) - 1u);
+            if (M & 1) d[u] = any ? ld_stream_f4(dp + p + 128 * u) : make_float4(0.f, 0.f, 0.f, 0.f);
+            if (M & 2) l[u] = any ? ld_stream_f4(lp + p + 128 * u) : make_float4(0.f, 0.f, 0.f, 0.f);
+        }
+#pragma unroll
+        for (int u = 0; u < U; ++u) ld_idx_raw<I16, C>(cbase, i0 + (p + 128 * (U + u)) / R, cn[u]);
+#pragma unroll
+        for (int u = 0; u < U; ++u) { TRL_CONSUME(c, u) }
+    }
+    if (p < Lv) {   // remainder: one predicated trip; a lane beyond the item's end holds foreign indices and uses none of them
+        float4 d[U - 1], l[U - 1];
+        unsigned int lv = 0u;
+#pragma unroll
+        for (int u = 0; u < U - 1; ++u) {
+            if (p + 128 * u < Lv) {
+#pragma unroll
+                for (int j = 0; j < C; ++j) lv |= (__ldg(live + idx_get<I16, C>(cn[u], j, add)) ? 1u : 0u) << (u * C + j);
+            }
+        }
+#pragma unroll
+        for (int u = 0; u < U - 1; ++u) {
+            const bool any = (lv >> (u * C)) & ((1u << C) - 1u);
+            if (M & 1) d[u] = any ? ld_stream_f4(dp + p + 128 * u) : make_float4(0.f, 0.f, 0.f, 0.f);
+            if (M & 2) l[u] = any ? ld_stream_f4(lp + p + 128 * u) : make_float4(0.f, 0.f, 0.f, 0.f);
+        }
+#pragma unroll
+        for (int u = 0; u < U - 1; ++u) { TRL_CONSUME(cn, u) }
+    }
+#undef TRL_CONSUME
+    return aD + aL;
+}
+
 // One warp per item from the work queue; items are in longest-first order (ties in (structure, spot) order, so the warps of
 // a CTA mostly work on neighbouring spots of one structure and share L1 lines of the gather vector).  Item e stores its
 // partial sum in slot item_slot[e]; k_combine adds the slots of every spot in slot order.  No floating-point atomics, no
 // fences: the result does not depend on the schedule.
-template <int R, bool I16>
+template <int R, bool I16, bool LIVE>
 __global__ void __launch_bounds__(FWD_THREADS, FWD_MIN_CTAS)
 k_transpose(long long n, const Item* __restrict__ items, const int32_t* __restrict__ item_slot, WorkQueue* __restrict__ wq,
             const uint8_t* __restrict__ mode, const void* __restrict__ t_col, const float* __restrict__ tD,
-            const float* __restrict__ tL, const GatherVec vec, double* __restrict__ partial)
+            const float* __restrict__ tL, const GatherVec vec, double* __restrict__ partial,
+            const uint8_t* __restrict__ live)          // LIVE: liveness byte per block row (tr_item_live)
 {
     const int lane = threadIdx.x & 31;
     const int nwarps = gridDim.x * FWD_WARPS, ni = (int)n;
@@ -613,15 +761,46 @@ k_transpose(long long n, const Item* __restrict__ items, const int32_t* __restri
         const int m = mode[it.seg & 0xFF];
         const int add = (it.seg >> 8) << 16;              // 16-bit form: the run's group of 65536 block rows
         double tot = 0.0;
-        if (m == 3) tot = tr_item<3, R, I16>(t_col, it.start, add, tD + it.start, tL + it.start, it.len, lane, vec);
-        else if (m == 1) tot = tr_item<1, R, I16>(t_col, it.start, add, tD + it.start, nullptr, it.len, lane, vec);
-        else if (m == 2) tot = tr_item<2, R, I16>(t_col, it.start, add, nullptr, tL + it.start, it.len, lane, vec);
+        if (LIVE) {
+            if (m == 3) tot = tr_item_live<3, R, I16>(t_col, it.start, add, tD + it.start, tL + it.start, it.len, lane, vec, live);
+            else if (m == 1) tot = tr_item_live<1, R, I16>(t_col, it.start, add, tD + it.start, nullptr, it.len, lane, vec, live);
+            else if (m == 2) tot = tr_item_live<2, R, I16>(t_col, it.start, add, nullptr, tL + it.start, it.len, lane, vec, live);
+        } else {
+            if (m == 3) tot = tr_item<3, R, I16>(t_col, it.start, add, tD + it.start, tL + it.start, it.len, lane, vec);
+            else if (m == 1) tot = tr_item<1, R, I16>(t_col, it.start, add, tD + it.start, nullptr, it.len, lane, vec);
+            else if (m == 2) tot = tr_item<2, R, I16>(t_col, it.start, add, nullptr, tL + it.start, it.len, lane, vec);
+        }
         if (m) tot = warp_sum(tot);
         if (lane == 0) partial[item_slot[e0]] = tot;
         e0 = e1;
         e1 = wq ? 2 * nwarps + (int)__shfl_sync(0xffffffffu, e2, 0) : e1 + nwarps;
     }
     if (wq) queue_leave(wq, lane, (unsigned int)nwarps);
+}
+
+// Measurement only (FREDOPT_OPT_TIME_PASSES): the values a back-projection with these liveness bytes NEEDS -- entries of the
+// items whose block row is live, times R values, times the matrices the item's structure reads -- added to out[0].
+template <int R, bool I16>
+__global__ void __launch_bounds__(FWD_THREADS)
+k_count_live(long long n, const Item* __restrict__ items, const uint8_t* __restrict__ mode, const void* __restrict__ t_col,
+             const uint8_t* __restrict__ live, unsigned long long* __restrict__ out) {
+    const int lane = threadIdx.x & 31;
+    const long long nwarps = (long long)gridDim.x * FWD_WARPS;
+    unsigned long long tot = 0;
+    for (long long e = (long long)blockIdx.x * FWD_WARPS + (threadIdx.x >> 5); e < n; e += nwarps) {
+        const Item it = ld_item(items + e);
+        const int m = mode[it.seg & 0xFF], add = (it.seg >> 8) << 16;
+        const int nm = (m & 1) + ((m >> 1) & 1);
+        const long long i0 = it.start / R;
+        unsigned int c = 0;
+        for (int i = lane; i < it.len / R; i += 32) {
+            const int b = (I16 ? (int)((const uint16_t*)t_col)[i0 + i] : ((const int32_t*)t_col)[i0 + i]) + (I16 ? add : 0);
+            c += live[b] ? 1u : 0u;
+        }
+        tot += (unsigned long long)c * R * nm;
+    }
+    for (int o = 16; o > 0; o >>= 1) tot += __shfl_down_sync(0xffffffffu, tot, o);
+    if (lane == 0 && tot) atomicAdd(out, tot);
 }
 
 // Second stage of a transposed pass: one thread per spot adds the spot's partial sums in slot order (ascending

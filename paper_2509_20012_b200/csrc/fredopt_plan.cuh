@@ -127,6 +127,9 @@ struct fredopt_plan {
     long long* part_cnt = nullptr;
     int* sink = nullptr;
     WorkQueue* wq = nullptr;                                                   // work queue of the item kernels (one launch at a time)
+    uint8_t* live8 = nullptr;                                                  // [act.n] 1 iff a row of the block row has a non-zero step coefficient
+    unsigned long long* live_count = nullptr;                                  // values the timed back-projections needed (k_count_live)
+    int skip_dead = 0;                                                         // back-projection skips block rows without a coefficient (option)
     // options / host state
     double eta = 1.0;
     long long reductionsN = 1, max_trials = 200;
@@ -155,6 +158,12 @@ struct fredopt_plan {
     double pass_ms[FREDOPT_N_PASSES] = {0};
     long long pass_launches[FREDOPT_N_PASSES] = {0};
     long long pass_bytes[FREDOPT_N_PASSES] = {0};
+    long long tr_con_value_bytes = 0;      // the share of pass_bytes[TRANSPOSE_B] that is matrix values (depends on the iterate)
+    long long live_all = -1;               // what k_count_live returns with every block row live (lazily)
+    long long live_launches = 0;           // timed back-projections counted into *live_count
+    bool count_pending = false;            // a timed back-projection waits for its count (launched by ev_end, outside the bracket)
+    const Item* count_items = nullptr;
+    const uint8_t* count_mode = nullptr;
     int sm_count = 148;
 };
 
@@ -220,9 +229,9 @@ void launch_fwd_kernel(fredopt_plan* P, int epi, const RowSet& R, long long b0, 
 void launch_forward(fredopt_plan* P, const RowSet& R, const uint8_t* mode, const double* x, double* oD, double* oL, int epi,
                     int write_uv = 0);
 void launch_tr_kernel(fredopt_plan* P, const RowSet& R, const Item* items, const int32_t* slots, long long n, const uint8_t* mode,
-                      const GatherVec& vec);
+                      const GatherVec& vec, const uint8_t* live = nullptr);
 void launch_transpose(fredopt_plan* P, int tepi, const RowSet& R, const uint8_t* mode, const GatherVec& vec, double* g_out,
-                      double* x, float* f_out);
+                      double* x, float* f_out, const uint8_t* live = nullptr);
 void launch_finalize(fredopt_plan* P, int n_part);
 void launch_sum_to(fredopt_plan* P, double* out, const double* in, const long long* in_ll, int n);   // out[0] = fixed-order sum
 void invalidate_graphs(fredopt_plan* P);

@@ -21,10 +21,29 @@ static void ev_begin(fredopt_plan* P, int pass) {
     cudaEventRecord(ep.a, P->stream);
     P->events.push_back(ep);
 }
+// values a back-projection over `items` needs with the liveness bytes `live` (added to *live_count)
+static void launch_count_live(fredopt_plan* P, const Item* items, const uint8_t* mode, const uint8_t* live) {
+    const RowSet& R = P->act;
+    const void* tc = R.t_col16 ? (const void*)R.t_col16 : (const void*)R.t_col;
+    const bool i16 = R.t_col16 != nullptr;
+    const long long n = R.t_n_items;
+#define CNT_CALL(RB, I16) k_count_live<RB, I16><<<P->sm_count * 8, FWD_THREADS, 0, P->stream>>>(n, items, mode, tc, live, P->live_count)
+    switch (R.R) {
+        case 1: if (i16) { CNT_CALL(1, true); } else { CNT_CALL(1, false); } break;
+        case 2: if (i16) { CNT_CALL(2, true); } else { CNT_CALL(2, false); } break;
+        default: if (i16) { CNT_CALL(4, true); } else { CNT_CALL(4, false); } break;
+    }
+#undef CNT_CALL
+}
 static void ev_end(fredopt_plan* P) {
     nvtxRangePop();
     if (!P->time_passes) return;
     cudaEventRecord(P->events.back().b, P->stream);
+    if (P->count_pending) {                 // after the bracket: the count is not part of the timed pass
+        P->count_pending = false;
+        launch_count_live(P, P->count_items, P->count_mode, P->live8);
+        ++P->live_launches;
+    }
 }
 
 // grid of the item kernels: persistent, one CTA per resident slot (launch bounds of k_forward / k_transpose); the items come
@@ -37,7 +56,7 @@ int fwd_grid(fredopt_plan* P, long long n) {
 static int static_grid(fredopt_plan* P, long long n) { return grid_for(n, FWD_WARPS, P->sm_count * FWD_MIN_CTAS * 2); }
 
 
-const ResidArgs NO_RESID{nullptr, nullptr, nullptr, GatherVec{nullptr, nullptr, nullptr}, nullptr, nullptr, nullptr, nullptr};
+const ResidArgs NO_RESID{nullptr, nullptr, nullptr, GatherVec{nullptr, nullptr, nullptr}, nullptr, nullptr, nullptr, nullptr, nullptr};
 
 // k_forward<EPI, R, I16> over n block rows of R starting at block row b0 (per-row arguments are passed already offset by the
 // caller: oD, oL, vox point at row b0 * R)
@@ -73,15 +92,22 @@ void launch_fwd_kernel(fredopt_plan* P, int epi, const RowSet& R, long long b0, 
 
 // k_transpose<R, I16> over n work items
 void launch_tr_kernel(fredopt_plan* P, const RowSet& R, const Item* items, const int32_t* slots, long long n, const uint8_t* mode,
-                      const GatherVec& vec) {
+                      const GatherVec& vec, const uint8_t* live) {
     if (n <= 0) return;
     WorkQueue* wq = P->tr_dynamic ? P->wq : nullptr;
     const int g = wq ? fwd_grid(P, n) : static_grid(P, n);
     const void* tc = R.t_col16 ? (const void*)R.t_col16 : (const void*)R.t_col;
     const bool i16 = R.t_col16 != nullptr;
-#define TR_CALL(RB, I16) klaunch(P, k_transpose<RB, I16>, g, FWD_THREADS, n, items, slots, wq, mode, tc, R.t_valD, R.t_valL, vec, R.t_partial)
+    if (!P->skip_dead) live = nullptr;
+#define TR_CALL(RB, I16)                                                                                                                      \
+    if (live) klaunch(P, k_transpose<RB, I16, true>, g, FWD_THREADS, n, items, slots, wq, mode, tc, R.t_valD, R.t_valL, vec, R.t_partial, live);  \
+    else klaunch(P, k_transpose<RB, I16, false>, g, FWD_THREADS, n, items, slots, wq, mode, tc, R.t_valD, R.t_valL, vec, R.t_partial, live)
     FREDOPT_DISPATCH(R.R, i16, TR_CALL)
 #undef TR_CALL
+    if (live && P->time_passes && P->live_count && &R == &P->act && n == R.t_n_items) {
+        // measurement: what this launch needed, counted by a separate kernel; launch_transpose closes the timed bracket first
+        P->count_pending = true; P->count_items = items; P->count_mode = mode;
+    }
 }
 
 // epi: EPI_STORE (d, l), EPI_STORE_PQ (d, l, the cost residuals p, q and partial sums of chi^2), EPI_CPART (Dg, Lg and partial
@@ -98,17 +124,17 @@ void launch_forward(fredopt_plan* P, const RowSet& R, const uint8_t* mode, const
     }
     const GatherVec none{nullptr, nullptr, nullptr};
     ResidArgs ra = NO_RESID;
-    if (epi == EPI_RESID) ra = ResidArgs{P->nD, P->nL, P->nT, write_uv ? P->uv : none, P->part_prox, P->part_phi, P->part_cnt, P->st};
+    if (epi == EPI_RESID) ra = ResidArgs{P->nD, P->nL, P->nT, write_uv ? P->uv : none, P->part_prox, P->part_phi, P->part_cnt, P->st, P->live8};
     launch_fwd_kernel(P, epi, R, 0, R.n, mode, x, oD, oL, epi == EPI_STORE_PQ ? P->pq : none, epi == EPI_STORE ? nullptr : P->tab,
                       epi == EPI_CPART ? P->cpart : epi == EPI_STORE_PQ ? P->part_phi : nullptr, nullptr, nullptr, 0, ra);
 }
 static int cpart_count(fredopt_plan* P) { return P->act.n ? (int)P->act.n : 1; }     // partial sums per block row
 
 void launch_transpose(fredopt_plan* P, int tepi, const RowSet& R, const uint8_t* mode, const GatherVec& vec, double* g_out, double* x,
-                      float* f_out) {
+                      float* f_out, const uint8_t* live) {
     if (R.t_n_items == 0 && tepi != TEPI_UPDATE) return;          // nothing to add; the update still clamps (R6)
-    if (P->tr_sorted) launch_tr_kernel(P, R, R.t_items, R.t_item_slot, R.t_n_items, mode, vec);
-    else launch_tr_kernel(P, R, R.t_items_run, R.t_slot_run, R.t_n_items, mode, vec);
+    if (P->tr_sorted) launch_tr_kernel(P, R, R.t_items, R.t_item_slot, R.t_n_items, mode, vec, live);
+    else launch_tr_kernel(P, R, R.t_items_run, R.t_slot_run, R.t_n_items, mode, vec, live);
     const int gc = grid_for(P->S, 256, 1 << 30);
     if (tepi == TEPI_GRAD) klaunch(P, k_combine<TEPI_GRAD>, gc, 256, P->S, R.t_item_ptr, R.t_partial, g_out, P->gpart, x, P->st, f_out);
     else if (tepi == TEPI_UPDATE) klaunch(P, k_combine<TEPI_UPDATE>, gc, 256, P->S, R.t_item_ptr, R.t_partial, g_out, P->gpart, x, P->st, f_out);
@@ -124,7 +150,7 @@ static int res_grid(fredopt_plan* P) {
 static void launch_residual(fredopt_plan* P, double* d, double* l, int use_beta, int final, int write_uv) {
     const int g = res_grid(P);
     klaunch(P, k_residual, g, ROW_THREADS, P->act.n_rows, P->act.rseg, P->tab, P->vb, P->st, d, l, P->Dg, P->Lg, P->nD, P->nL, P->nT, P->uv, P->pq,
-            P->x, P->g, P->S, P->part_prox, P->part_phi, P->part_cnt, use_beta, final, write_uv);
+            P->x, P->g, P->S, P->part_prox, P->part_phi, P->part_cnt, use_beta, final, write_uv, P->live8, P->act.R);
 }
 
 // n_part: how many per-CTA partial sums the last residual pass wrote (k_residual: res_grid; forward epilogue: fwd_grid)
@@ -203,7 +229,7 @@ static int enqueue_iteration(fredopt_plan* P, bool sa) {
         return (int)(P->launches - before);
     }
     ev_begin(P, FREDOPT_PASS_TRANSPOSE_B);
-    launch_transpose(P, TEPI_UPDATE, P->act, P->mode_con, P->uv, nullptr, P->x, nullptr);              // a8, a9
+    launch_transpose(P, TEPI_UPDATE, P->act, P->mode_con, P->uv, nullptr, P->x, nullptr, P->live8);    // a8, a9 (rows with a coefficient only)
     ev_end(P);
     return (int)(P->launches - before);
 }
@@ -245,7 +271,7 @@ static int enqueue_iteration_sharded(fredopt_plan* P, bool sa) {
         launch_forward(P, A, P->mode_con, P->x, P->d, P->l, EPI_RESID, 1);
     }
     // local partial step and statistics -> reduction -> update + clamp on every rank
-    if (A.t_n_items) launch_tr_kernel(P, A, A.t_items, A.t_item_slot, A.t_n_items, P->mode_con, P->uv);
+    if (A.t_n_items) launch_tr_kernel(P, A, A.t_items, A.t_item_slot, A.t_n_items, P->mode_con, P->uv, P->live8);
     klaunch(P, k_slots_sum, gS, 256, S, A.t_item_ptr, A.t_partial, P->rbuf);
     const int np = A.n == 0 ? 0 : sa ? res_grid(P) : (int)A.n;
     klaunch(P, k_sum_to, 1, 1024, P->rbuf + S, P->part_prox, np);
@@ -304,12 +330,20 @@ int fredopt_set_option(fredopt_plan* P, int32_t key, double value) {
         case FREDOPT_OPT_BLOCK_SEQUENTIAL: P->block_sequential = value != 0.0; break;
         case FREDOPT_OPT_NORMALIZE_GRAD: P->normalize_grad = value != 0.0; break;
         case FREDOPT_OPT_ONE_SIDED_COST: P->one_sided_cost = value != 0.0; break;
+        case FREDOPT_OPT_SKIP_SATISFIED:
+            if (P->skip_dead != (value != 0.0)) {              // another kernel instantiation: capture again
+                P->skip_dead = value != 0.0;
+                invalidate_graphs(P);
+            }
+            break;
         case FREDOPT_OPT_TIME_PASSES:
             P->time_passes = value != 0.0;
             if (P->time_passes) {
                 for (auto& ep : P->events) P->event_pool.push_back(ep);
                 P->events.clear();
                 for (int i = 0; i < FREDOPT_N_PASSES; ++i) { P->pass_ms[i] = 0; P->pass_launches[i] = 0; }
+                P->live_launches = 0;
+                if (P->live_count) cudaMemsetAsync(P->live_count, 0, sizeof(unsigned long long), P->stream);
             }
             break;
         default: return FREDOPT_INVALID_ARG;
@@ -459,6 +493,35 @@ int fredopt_get_pass_times(fredopt_plan* P, double* ms, int64_t* launches) {
 int fredopt_get_pass_bytes(fredopt_plan* P, int64_t* bytes) {
     if (!P || !bytes) return FREDOPT_INVALID_ARG;
     for (int i = 0; i < FREDOPT_N_PASSES; ++i) bytes[i] = P->pass_bytes[i];
+    return FREDOPT_OK;
+}
+
+int fredopt_get_pass_bytes_timed(fredopt_plan* P, int64_t* bytes) {
+    if (!P || !bytes) return FREDOPT_INVALID_ARG;
+    for (int i = 0; i < FREDOPT_N_PASSES; ++i) bytes[i] = P->pass_bytes[i];
+    CK(cudaStreamSynchronize(P->stream));
+    if (P->live_launches > 0 && P->act.t_n_items > 0) {
+        unsigned long long cnt = 0;
+        CK(cudaMemcpy(&cnt, P->live_count, sizeof(cnt), cudaMemcpyDeviceToHost));
+        if (P->live_all < 0) {              // the same count with every block row live
+            uint8_t* ones = nullptr;
+            CK(cudaMalloc((void**)&ones, (size_t)(P->act.n ? P->act.n : 1)));
+            cudaMemsetAsync(ones, 1, (size_t)(P->act.n ? P->act.n : 1), P->stream);
+            cudaMemsetAsync(P->live_count, 0, sizeof(unsigned long long), P->stream);
+            launch_count_live(P, P->tr_sorted ? P->act.t_items : P->act.t_items_run, P->mode_con, ones);
+            unsigned long long all = 0;
+            cudaMemcpyAsync(&all, P->live_count, sizeof(all), cudaMemcpyDeviceToHost, P->stream);
+            cudaMemcpyAsync(P->live_count, &cnt, sizeof(cnt), cudaMemcpyHostToDevice, P->stream);   // put the running sum back
+            CK(cudaStreamSynchronize(P->stream));
+            cudaFree(ones);
+            P->live_all = (long long)all;
+        }
+        if (P->live_all > 0) {
+            const double frac = (double)cnt / ((double)P->live_launches * (double)P->live_all);
+            bytes[FREDOPT_PASS_TRANSPOSE_B] = P->pass_bytes[FREDOPT_PASS_TRANSPOSE_B] - P->tr_con_value_bytes +
+                                               (long long)(frac * (double)P->tr_con_value_bytes);
+        }
+    }
     return FREDOPT_OK;
 }
 

@@ -188,41 +188,51 @@ k_residual(long long n, const int16_t* __restrict__ rseg, const StructInfo* __re
            const double* __restrict__ nD, const double* __restrict__ nL, const double* __restrict__ nT,
            const GatherVec uv, const GatherVec pq, double* __restrict__ x, const double* __restrict__ g, long long S,
            double* __restrict__ part_prox, double* __restrict__ part_phi, long long* __restrict__ part_cnt,
-           int use_beta, int final, int write_uv) {
+           int use_beta, int final, int write_uv, uint8_t* __restrict__ live, int R) {
     pdl_wait();
     pdl_trigger();
     __shared__ double sm[ROW_THREADS / 32];
     __shared__ long long smc[ROW_THREADS / 32];
     const double beta = use_beta ? st->beta_acc : 0.0;
     const long long tid = (long long)blockIdx.x * blockDim.x + threadIdx.x, nth = (long long)gridDim.x * blockDim.x;
+    const int lane = threadIdx.x & 31;
     if (beta != 0.0)
         for (long long j = tid; j < S; j += nth) x[j] = fma(-beta, g[j], x[j]);
     double prox = 0.0, phi = 0.0;
     long long cnt = 0;
-    for (long long a = tid; a < n; a += nth) {
-        const int sg = rseg[a];
-        if (sg < 0) continue;                                          // padding row of a ragged block: no sets, no cost term
-        double dv = d[a], lv = l[a];
-        if (beta != 0.0) {
-            dv = fma(-beta, Dg[a], dv);
-            lv = fma(-beta, Lg[a], lv);
-            d[a] = dv; l[a] = lv;
+    for (long long a0 = tid - lane; a0 < n; a0 += nth) {            // whole warps: the R rows of a block row sit in R neighbouring lanes
+        const long long a = a0 + lane;
+        const int sg = a < n ? rseg[a] : -1;                          // -1: padding row of a ragged block (no sets, no cost term)
+        int nz = 0;
+        if (sg >= 0) {
+            double dv = d[a], lv = l[a];
+            if (beta != 0.0) {
+                dv = fma(-beta, Dg[a], dv);
+                lv = fma(-beta, Lg[a], lv);
+                d[a] = dv; l[a] = lv;
+            }
+            const StructInfo& T = tab[sg];
+            const int f = T.flags;
+            const double w = T.what;
+            const RowBounds B = row_bounds(T, vb, a);
+            if (!final) {
+                double pv, qv;
+                cost_residuals(f, w, B.dose_ref, B.dl_ref, st->flags & SF_ONE_SIDED, dv, lv, pv, qv);
+                gv_store(pq, a, pv, qv);
+                if (f & F_DOSE_REF) { const double e = B.dose_ref - dv; phi += w * e * e; }
+                if (f & F_DL_REF) { const double e = B.dl_ref - lv; if (!((st->flags & SF_ONE_SIDED) && e > 0.0)) phi += w * e * e; }
+            } else {
+                double uu, vv;
+                row_residual(T, B, st->flags & SF_ONE_SIDED, dv, lv, nD[a], nL[a], nT[a], uu, vv, cnt, prox, phi);
+                if (write_uv) gv_store(uv, a, uu, vv);
+                nz = (uu != 0.0) | (vv != 0.0);
+            }
         }
-        const StructInfo& T = tab[sg];
-        const int f = T.flags;
-        const double w = T.what;
-        const RowBounds B = row_bounds(T, vb, a);
-        if (!final) {
-            double pv, qv;
-            cost_residuals(f, w, B.dose_ref, B.dl_ref, st->flags & SF_ONE_SIDED, dv, lv, pv, qv);
-            gv_store(pq, a, pv, qv);
-            if (f & F_DOSE_REF) { const double e = B.dose_ref - dv; phi += w * e * e; }
-            if (f & F_DL_REF) { const double e = B.dl_ref - lv; if (!((st->flags & SF_ONE_SIDED) && e > 0.0)) phi += w * e * e; }
-            continue;
+        if (final && write_uv) {                                       // liveness byte of the block row (read by the back-projection)
+            if (R >= 2) nz |= __shfl_xor_sync(0xffffffffu, nz, 1);
+            if (R == 4) nz |= __shfl_xor_sync(0xffffffffu, nz, 2);
+            if (a < n && (a % R) == 0) live[a / R] = (uint8_t)nz;
         }
-        double uu, vv;
-        row_residual(T, B, st->flags & SF_ONE_SIDED, dv, lv, nD[a], nL[a], nT[a], uu, vv, cnt, prox, phi);
-        if (write_uv) gv_store(uv, a, uu, vv);
     }
     if (!final) {                                                  // chi^2(x') for the next reduction's accept test
         const double q = block_sum(phi, sm);

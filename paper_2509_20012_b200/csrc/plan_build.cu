@@ -546,9 +546,9 @@ int build_transpose(fredopt_plan* P, RowSet& R) {
     CK(cudaMemcpyAsync(&R.t_entries_padded, R.t_ptr + K, sizeof(long long), cudaMemcpyDeviceToHost, st));
     CK(cudaStreamSynchronize(st));
     const size_t Tn = R.t_entries_padded ? (size_t)R.t_entries_padded : 4;
-    if (idx16) CKR(dmalloc(P, &R.t_col16, Tn)); else CKR(dmalloc(P, &R.t_col, Tn));
+    if (idx16) CKR(dmalloc(P, &R.t_col16, Tn + IDX_SLACK)); else CKR(dmalloc(P, &R.t_col, Tn + IDX_SLACK));   // slack: see IDX_SLACK
     CKR(dmalloc(P, &R.t_valD, Tn * RB)); CKR(dmalloc(P, &R.t_valL, Tn * RB));
-    if (idx16) CK(cudaMemsetAsync(R.t_col16, 0, Tn * 2, st)); else CK(cudaMemsetAsync(R.t_col, 0, Tn * 4, st));
+    if (idx16) CK(cudaMemsetAsync(R.t_col16, 0, (Tn + IDX_SLACK) * 2, st)); else CK(cudaMemsetAsync(R.t_col, 0, (Tn + IDX_SLACK) * 4, st));
     CK(cudaMemsetAsync(R.t_valD, 0, Tn * RB * 4, st));
     CK(cudaMemsetAsync(R.t_valL, 0, Tn * RB * 4, st));
     if (E) k_tr_fill<<<grid_for(E, 256, 1 << 16), 256, 0, st>>>(keys2, vals2, E, RB, ustart, R.t_ptr, off, n, R.start, R.len, R.valD, R.valL,
@@ -683,7 +683,7 @@ int recount_sets(fredopt_plan* P, bool letd_norms) {
 // (2 B, or 4 B in the 32-bit form); 8 B per row offset; the fp64 vectors read / written once.  The zeros a block row stores
 // where one of its rows has no entry are NOT counted (they show up as DRAM traffic above this figure).
 static void compute_pass_bytes(fredopt_plan* P) {
-    long long fwd_union = 0, tr_cost = 0, tr_con = 0, rows_union = 0, rows_con = 0, rows_cost = 0;
+    long long fwd_union = 0, tr_cost = 0, tr_con = 0, rows_union = 0, rows_con = 0, rows_cost = 0, con_values = 0;
     const int ibf = P->act.col16 ? 2 : 4, ibt = P->act.t_col16 ? 2 : 4;     // index bytes as stored
     for (int s = 0; s < P->n_struct; ++s) {
         const StructInfo& T = P->h_tab[s];
@@ -694,6 +694,7 @@ static void compute_pass_bytes(fredopt_plan* P) {
         fwd_union += per(cost | con, ibf);
         tr_cost += per(cost, ibt);
         tr_con += per(con, ibt);
+        con_values += (long long)T.nnz * 4 * ((con & 1) + ((con >> 1) & 1));
         if (cost | con) rows_union += T.rows;
         if (con) rows_con += T.rows;
         if (cost) rows_cost += T.rows;
@@ -703,6 +704,7 @@ static void compute_pass_bytes(fredopt_plan* P) {
     P->pass_bytes[FREDOPT_PASS_FORWARD_G] = fwd_union + rows_union * (8 + 16) + S * 8;
     P->pass_bytes[FREDOPT_PASS_TRANSPOSE_G] = tr_cost + S * P->act.n_seg * 8 + rows_cost * 16 + S * 8;
     P->pass_bytes[FREDOPT_PASS_TRANSPOSE_B] = tr_con + S * P->act.n_seg * 8 + rows_con * 16 + S * 16;
+    P->tr_con_value_bytes = con_values;
     P->pass_bytes[FREDOPT_PASS_SELECT] = S * 24;
     P->pass_bytes[FREDOPT_PASS_RESIDUAL] = VA * (4 + 8 * 9);
 }
@@ -884,8 +886,8 @@ static int create_impl(fredopt_plan* P, const fredopt_csr* D, const fredopt_csr*
         P->full_class[0] = 0;
         for (int c = 0; c < N_LEN_CLASS; ++c) P->full_class[c + 1] = P->full_class[c] + (long long)hh[c];
         const size_t np = F.entries_padded ? (size_t)F.entries_padded : 4;
-        if (idx16) { CKR(dmalloc(P, &F.col16, np)); CK(cudaMemsetAsync(F.col16, 0, np * 2, st)); }
-        else { CKR(dmalloc(P, &F.col, np)); CK(cudaMemsetAsync(F.col, 0, np * 4, st)); }
+        if (idx16) { CKR(dmalloc(P, &F.col16, np + IDX_SLACK)); CK(cudaMemsetAsync(F.col16, 0, (np + IDX_SLACK) * 2, st)); }
+        else { CKR(dmalloc(P, &F.col, np + IDX_SLACK)); CK(cudaMemsetAsync(F.col, 0, (np + IDX_SLACK) * 4, st)); }
         CKR(dmalloc(P, &F.valD, np)); CKR(dmalloc(P, &F.valL, np));
         CK(cudaMemsetAsync(F.valD, 0, np * 4, st)); CK(cudaMemsetAsync(F.valL, 0, np * 4, st));
         if (n_ne) {
@@ -995,8 +997,8 @@ static int create_impl(fredopt_plan* P, const fredopt_csr* D, const fredopt_csr*
         CK(cudaMemcpyAsync(&A.entries_padded, A.start + n_blk, 8, cudaMemcpyDeviceToHost, st));
         CK(cudaStreamSynchronize(st));
         const size_t na = A.entries_padded ? (size_t)A.entries_padded : 4;
-        if (idx16) { CKR(dmalloc(P, &A.col16, na)); CK(cudaMemsetAsync(A.col16, 0, na * 2, st)); }
-        else { CKR(dmalloc(P, &A.col, na)); CK(cudaMemsetAsync(A.col, 0, na * 4, st)); }
+        if (idx16) { CKR(dmalloc(P, &A.col16, na + IDX_SLACK)); CK(cudaMemsetAsync(A.col16, 0, (na + IDX_SLACK) * 2, st)); }
+        else { CKR(dmalloc(P, &A.col, na + IDX_SLACK)); CK(cudaMemsetAsync(A.col, 0, (na + IDX_SLACK) * 4, st)); }
         CKR(dmalloc(P, &A.valD, na * Rb)); CKR(dmalloc(P, &A.valL, na * Rb));
         CK(cudaMemsetAsync(A.valD, 0, na * Rb * 4, st)); CK(cudaMemsetAsync(A.valL, 0, na * Rb * 4, st));
         if (n_blk) {
@@ -1049,6 +1051,10 @@ static int create_impl(fredopt_plan* P, const fredopt_csr* D, const fredopt_csr*
     CKR(dmalloc(P, &P->cpart, npart));
     CKR(dmalloc(P, &P->wq, 1));
     CK(cudaMemsetAsync(P->wq, 0, sizeof(WorkQueue), st));
+    CKR(dmalloc(P, &P->live8, (size_t)(P->act.n ? P->act.n : 1)));
+    CK(cudaMemsetAsync(P->live8, 1, (size_t)(P->act.n ? P->act.n : 1), st));      // until a residual pass has written it: every block row
+    CKR(dmalloc(P, &P->live_count, 1));
+    CK(cudaMemsetAsync(P->live_count, 0, sizeof(unsigned long long), st));
     CKR(dmalloc(P, &P->gpart, (size_t)(S / 256 + 2)));
     CK(cudaMemsetAsync(P->gpart, 0, (size_t)(S / 256 + 2) * 8, st)); CKR(dmalloc(P, &P->part_prox, npart));
     CKR(dmalloc(P, &P->part_phi, npart)); CKR(dmalloc(P, &P->part_cnt, npart));

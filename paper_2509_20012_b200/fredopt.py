@@ -17,7 +17,7 @@ LIB_PATH = os.path.join(_HERE, "libfredopt.so")
 
 OK, INVALID_ARG, OUT_OF_MEMORY, CUDA_ERROR, UNSUPPORTED_ARCH, UNSUPPORTED = 0, -1, -2, -3, -4, -5
 OPT_ETA, OPT_REDUCTIONS, OPT_ACCEPT_CHECK, OPT_MAX_TRIALS, OPT_RESET, OPT_USE_GRAPH, OPT_TIME_PASSES, \
-    OPT_BLOCK_SEQUENTIAL, OPT_NORMALIZE_GRAD, OPT_ONE_SIDED_COST, OPT_USE_PDL, OPT_WORK_QUEUE = range(12)
+    OPT_BLOCK_SEQUENTIAL, OPT_NORMALIZE_GRAD, OPT_ONE_SIDED_COST, OPT_USE_PDL, OPT_WORK_QUEUE, OPT_SKIP_SATISFIED = range(13)
 ROWS_ALL, ROWS_ACTIVE = 0, 1
 VB_DOSE_LO, VB_DOSE_HI, VB_DL_LO, VB_DL_HI, VB_LETD_MAX, VB_DOSE_REF, VB_DL_REF = range(7)
 PASS_NAMES = ("forward_x", "transpose_g", "forward_g", "select", "residual", "transpose_b")
@@ -29,6 +29,7 @@ SYMBOLS = (
     "fredopt_set_weights_f64", "fredopt_get_state", "fredopt_set_state", "fredopt_shard_range", "fredopt_set_reduce",
     "fredopt_set_voxel_bounds", "fredopt_dose_let", "fredopt_iterate", "fredopt_proximity", "fredopt_set_option", "fredopt_get_stats",
     "fredopt_spmv_forward", "fredopt_spmv_transpose", "fredopt_get_pass_times", "fredopt_get_pass_bytes",
+    "fredopt_get_pass_bytes_timed",
     "fredopt_launch_count", "fredopt_stream_read", "fredopt_strerror", "fredopt_last_cuda_error",
     "fredopt_structure_stats", "fredopt_volume_histogram", "fredopt_percentile_value",
 )
@@ -112,6 +113,7 @@ def _load():
     lib.fredopt_percentile_value.argtypes = [vp, vp, i32, i32, f64, C.POINTER(f64)]
     lib.fredopt_get_pass_times.argtypes = [vp, C.POINTER(f64), C.POINTER(i64)]
     lib.fredopt_get_pass_bytes.argtypes = [vp, C.POINTER(i64)]
+    lib.fredopt_get_pass_bytes_timed.argtypes = [vp, C.POINTER(i64)]
     lib.fredopt_launch_count.argtypes = [vp]
     lib.fredopt_launch_count.restype = i64
     lib.fredopt_stream_read.argtypes = [vp, vp, i64, i32]
@@ -299,6 +301,11 @@ class Plan:
     def pass_bytes(self):
         b = (C.c_int64 * N_PASSES)()
         _check(_lib.fredopt_get_pass_bytes(self._h, b), "fredopt_get_pass_bytes")
+        return {PASS_NAMES[i]: b[i] for i in range(N_PASSES)}
+
+    def pass_bytes_timed(self):
+        b = (C.c_int64 * N_PASSES)()
+        _check(_lib.fredopt_get_pass_bytes_timed(self._h, b), "fredopt_get_pass_bytes_timed")
         return {PASS_NAMES[i]: b[i] for i in range(N_PASSES)}
 
     def launch_count(self):

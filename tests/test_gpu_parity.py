@@ -733,6 +733,68 @@ def test_work_distribution_never_changes_a_result(fredopt, plan0):
         gp = f.from_plan(plan0); gp.set_option(f.OPT_WORK_QUEUE, 16)
 
 
+@pytest.mark.parametrize("copt", INDEX_FORMS)
+@pytest.mark.parametrize("beta0", [0.0, 1.0])
+def test_skipping_rows_without_a_coefficient_never_changes_a_result(fredopt, plan0, beta0, copt):
+    """FREDOPT_OPT_SKIP_SATISFIED: the back-projection streams the values of a (block) row only if the row has a non-zero step
+    coefficient (Fig. 2 touches a row only when its test fires).  Every skipped term is an exact zero, so x,
+    the counters and the statistics carry the same bits with the option on and off -- superiorized and pure feasibility-seeking
+    (the two kernels that write the liveness bytes), every stored form, reductionsN = 2 -- and both match the oracle."""
+    f = fredopt
+    from oracle import oracle as om
+    res = []
+    for skip in (1, 0):
+        gp = f.from_plan(plan0, **copt)
+        gp.set_option(f.OPT_SKIP_SATISFIED, skip)
+        gp.set_weights(plan0.x0)
+        gp.iterate(30, 1.0, beta0, 0.99)
+        gp.set_option(f.OPT_REDUCTIONS, 2)
+        gp.iterate(5, 1.7, beta0, 0.99)
+        st = gp.stats()
+        res.append((_gpu_x(gp), (st["k"], st["s"], st["trials"], st["n_violated"], st["prox"], st["phi"])))
+        if skip:
+            orc = _oracle(plan0)
+            orc.set_x(plan0.x0)
+            orc.iterate(30, 1.0, beta0, 0.99)
+            orc.set_option(om.OPT_REDUCTIONS, 2)
+            orc.iterate(5, 1.7, beta0, 0.99)
+            _assert_state(gp, orc)
+        gp.destroy()
+    assert np.array_equal(res[0][0], res[1][0]) and res[0][1] == res[1][1]
+
+
+def test_skipping_on_a_plan_where_most_rows_are_satisfied(fredopt):
+    """A three-beam plan driven close to feasibility (block-sequential sweeps first): afterwards few rows carry a coefficient, the
+    timed byte count of the back-projection (fredopt_get_pass_bytes_timed) falls below the static one, and the simultaneous
+    iterations that follow are bit-identical with and without skipping."""
+    f = fredopt
+    spec = pg.config_spec(2, scale=0.2)
+    plan = pg.build_plan(spec, device="cuda")
+    xs = []
+    for skip in (1, 0):
+        gp = f.from_plan(plan)
+        gp.set_option(f.OPT_SKIP_SATISFIED, skip)
+        gp.set_weights(plan.x0)
+        gp.set_option(f.OPT_BLOCK_SEQUENTIAL, 1)
+        gp.iterate(150, 1.0, 0.0, 0.99)
+        gp.set_option(f.OPT_BLOCK_SEQUENTIAL, 0)
+        gp.set_option(f.OPT_TIME_PASSES, 1)
+        gp.iterate(10, 1.0, 0.0, 0.99)
+        static, timed = gp.pass_bytes(), gp.pass_bytes_timed()
+        gp.set_option(f.OPT_TIME_PASSES, 0)
+        gp.iterate(10, 1.0, 1.0, 0.99)
+        xs.append(_gpu_x(gp))
+        st = gp.stats()
+        if skip:
+            assert timed["transpose_b"] < static["transpose_b"], (timed, static)
+            assert timed["forward_x"] == static["forward_x"]
+            assert st["n_violated"] < 0.5 * st["n_sets"]
+        else:
+            assert timed["transpose_b"] == static["transpose_b"]
+        gp.destroy()
+    assert np.array_equal(xs[0], xs[1])
+
+
 # ------------------------------------------------------------------------------------------ per-voxel bounds (SURVEY 8f-4)
 def _varying_voxel_bounds(plan, bounds, seed):
     """Per-voxel arrays around the structures' scalars (+-, NaN on ~30 % of the voxels), voxel-indexed float32, for every field."""
