@@ -21,6 +21,7 @@
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>
+#include <stdio.h>
 
 namespace fredopt {
 
@@ -128,23 +129,57 @@ __device__ __forceinline__ void gv_store(const GatherVec& g, long long a, double
 __device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
 __device__ __forceinline__ void pdl_trigger() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
 
+// ------------------------------------------------------------------------------------------ checked build
+// -DFREDOPT_CHECKED (python paper_2509_20012_b200/build.py -DFREDOPT_CHECKED): every load of the item kernels -- streamed
+// indices and values, item descriptors, gathered weights / coefficients, liveness bytes -- is checked against the extents of
+// the live plans' device allocations and traps with a message when it lies outside all of them.  Slow; for the tests only
+// (compute-sanitizer is closed on this pool: profiles/r02_sanitizer.md).
+#ifdef FREDOPT_CHECKED
+struct ChkRange { const char* b; const char* e; };
+constexpr int CHK_MAX = 2048;
+static __device__ ChkRange g_chk[CHK_MAX];
+static __device__ int g_chk_n;
+static __device__ __noinline__ void chk_fail(const void* p, int bytes, int site) {
+    printf("fredopt checked build: load of %d bytes at %p lies outside every allocation of a plan (site %d, block %d, thread %d)\n", bytes, p, site,
+           (int)blockIdx.x, (int)threadIdx.x);
+    __trap();
+}
+__device__ __forceinline__ void chk(const void* p, int bytes, int site) {
+    const char* a = (const char*)p;
+    const int n = g_chk_n;
+    for (int i = 0; i < n; ++i)
+        if (a >= g_chk[i].b && a + bytes <= g_chk[i].e) return;
+    chk_fail(p, bytes, site);
+}
+// this translation unit's copy of the table
+static inline void chk_upload_tu(const ChkRange* h, int n) {
+    cudaMemcpyToSymbol(g_chk, h, (size_t)n * sizeof(ChkRange));
+    cudaMemcpyToSymbol(g_chk_n, &n, sizeof(int));
+}
+#else
+#define chk(p, bytes, site) ((void)0)
+#endif
+
 // ------------------------------------------------------------------------------------------ loads
 // Timing experiments (results are WRONG on purpose; profiles/r02_ceilings.md): -DEXP_NO_GATHER makes the gathered value from the
 // index without a load, -DEXP_NO_CVT skips the fp32 -> fp64 conversion, -DEXP_NO_FMA replaces the fp64 multiply-add by an xor.
 #ifdef EXP_NO_GATHER
 #define FWD_GATHER(x, c) __hiloint2double(0x3ff00000, (c))
 #else
-#define FWD_GATHER(x, c) __ldg((x) + (c))
+__device__ __forceinline__ double fwd_gather(const double* __restrict__ x, int c) { chk(x + c, 8, 8); return __ldg(x + c); }
+#define FWD_GATHER(x, c) fwd_gather((x), (c))
 #endif
 // streamed arrays (index / value): read once, keep them out of L1 so that L1 holds the gathered vector
 __device__ __forceinline__ int4 ld_stream_i4(const int32_t* p) {
     int4 r;
+    chk(p, 16, 1);
     asm volatile("ld.global.nc.L1::no_allocate.v4.s32 {%0,%1,%2,%3}, [%4];"
                  : "=r"(r.x), "=r"(r.y), "=r"(r.z), "=r"(r.w) : "l"(p));
     return r;
 }
 __device__ __forceinline__ float4 ld_stream_f4(const float* p) {
     float4 r;
+    chk(p, 16, 2);
     asm volatile("ld.global.nc.L1::no_allocate.v4.f32 {%0,%1,%2,%3}, [%4];"
                  : "=f"(r.x), "=f"(r.y), "=f"(r.z), "=f"(r.w) : "l"(p));
     return r;
@@ -153,6 +188,7 @@ __device__ __forceinline__ float4 ld_stream_f4(const float* p) {
 // C = 4 / R is the number of entries a lane's 128-bit value load covers.
 template <bool I16, int C>
 __device__ __forceinline__ void ld_idx(const void* __restrict__ base, long long i, int add, int (&c)[C]) {
+    chk((const char*)base + i * (I16 ? 2 : 4), C * (I16 ? 2 : 4), 3);
     if (I16) {
         const uint16_t* p = (const uint16_t*)base + i;
         if (C == 4) {
@@ -189,6 +225,7 @@ __device__ __forceinline__ void ld_idx(const void* __restrict__ base, long long 
 template <bool I16, int C> struct IdxRaw { unsigned int w[I16 ? (C + 1) / 2 : C]; };
 template <bool I16, int C>
 __device__ __forceinline__ void ld_idx_raw(const void* __restrict__ base, long long i, IdxRaw<I16, C>& r) {
+    chk((const char*)base + i * (I16 ? 2 : 4), C * (I16 ? 2 : 4), 4);
     if (I16) {
         const uint16_t* p = (const uint16_t*)base + i;
         if (C == 4) {
@@ -220,6 +257,7 @@ __device__ __forceinline__ int idx_get(const IdxRaw<I16, C>& r, int j, int add) 
     return (int)r.w[j];
 }
 __device__ __forceinline__ Item ld_item(const Item* p) {
+    chk(p, 16, 5);
     const int4 v = __ldg((const int4*)p);
     Item it;
     it.start = (long long)(((unsigned long long)(unsigned)v.y << 32) | (unsigned)v.x);
@@ -234,6 +272,7 @@ __device__ __forceinline__ void ld_coef(const double* __restrict__ v, int b, dou
     for (int k = 0; k < R; ++k) g[k] = __hiloint2double(0x3ff00000, b + k);
     return;
 #endif
+    chk(v + (long long)R * b, 8 * R, 6);
     if (R == 1) g[0] = __ldg(v + b);
     else if (R == 2) { const double2 t = __ldg((const double2*)v + b); g[0] = t.x; g[1 % R] = t.y; }
     else {   // 32 bytes, 32-byte aligned: one 256-bit load (sm_100+)
@@ -249,6 +288,7 @@ __device__ __forceinline__ void ld_coef_pair(const double2* __restrict__ v, int 
     for (int k = 0; k < R; ++k) { gd[k] = __hiloint2double(0x3ff00000, b + k); gl[k] = __hiloint2double(0x3ff00000, b - k); }
     return;
 #endif
+    chk(v + (long long)R * b, 16 * R, 7);
     if (R == 1) { const double2 t = __ldg(v + b); gd[0] = t.x; gl[0] = t.y; }
     else {
 #pragma unroll
@@ -700,7 +740,7 @@ __device__ __forceinline__ double tr_item_live(const void* __restrict__ cbase, l
         for (int u = 0; u < U; ++u) {
             c[u] = cn[u];
 #pragma unroll
-            for (int j = 0; j < C; ++j) lv |= (__ldg(live + idx_get<I16, C>(c[u], j, add)) ? 1u : 0u) << (u * C + j);
+            for (int j = 0; j < C; ++j) { const int bb = (idx_get<I16, C>(c[u], j, add)); chk(live + bb, 1, 9); lv |= (__ldg(live + bb) ? 1u : 0u) << (u * C + j); }
         }
 #pragma unroll
         for (int u = 0; u < U; ++u) {
@@ -720,7 +760,7 @@ __device__ __forceinline__ double tr_item_live(const void* __restrict__ cbase, l
         for (int u = 0; u < U - 1; ++u) {
             if (p + 128 * u < Lv) {
 #pragma unroll
-                for (int j = 0; j < C; ++j) lv |= (__ldg(live + idx_get<I16, C>(cn[u], j, add)) ? 1u : 0u) << (u * C + j);
+                for (int j = 0; j < C; ++j) { const int bb = (idx_get<I16, C>(cn[u], j, add)); chk(live + bb, 1, 9); lv |= (__ldg(live + bb) ? 1u : 0u) << (u * C + j); }
             }
         }
 #pragma unroll

@@ -168,12 +168,27 @@ struct fredopt_plan {
 };
 
 
+// checked build (fredopt_kernels.cuh, FREDOPT_CHECKED): the extents of every live plan's allocations, mirrored on the device
+#ifdef FREDOPT_CHECKED
+void chk_register(const void* p, size_t bytes);     // plan_build.cu
+void chk_unregister(const void* p);
+void chk_sync(cudaStream_t stream);                 // upload the table if it changed (not during a capture)
+void chk_upload_iterate(const ChkRange* h, int n);  // one per translation unit that instantiates checked kernels
+void chk_upload_passes(const ChkRange* h, int n);
+void chk_upload_build(const ChkRange* h, int n);
+#else
+static inline void chk_register(const void*, size_t) {}
+static inline void chk_unregister(const void*) {}
+static inline void chk_sync(cudaStream_t) {}
+#endif
+
 template <class T>
 static inline int dmalloc(fredopt_plan* P, T** p, size_t n) {
     *p = nullptr;
     if (n == 0) n = 1;
     CK(cudaMalloc((void**)p, n * sizeof(T)));
     P->allocs.push_back((void*)*p);
+    chk_register((const void*)*p, n * sizeof(T));
     return FREDOPT_OK;
 }
 

@@ -66,10 +66,14 @@ const ResidArgs NO_RESID{nullptr, nullptr, nullptr, GatherVec{nullptr, nullptr, 
         case 2: if (I16) { CALL(2, true); } else { CALL(2, false); } break;         \
         default: if (I16) { CALL(4, true); } else { CALL(4, false); } break;        \
     }
+#ifdef FREDOPT_CHECKED
+void chk_upload_iterate(const ChkRange* h, int n) { chk_upload_tu(h, n); }
+#endif
 void launch_fwd_kernel(fredopt_plan* P, int epi, const RowSet& R, long long b0, long long n, const uint8_t* mode, const double* x,
                        double* oD, double* oL, const GatherVec& pq, const StructInfo* tab, double* cpart, float* fD, float* fL,
                        int letd_out, const ResidArgs& ra) {
     if (n <= 0) return;
+    chk_sync(P->stream);
     WorkQueue* wq = P->fwd_dynamic ? P->wq : nullptr;
     const int g = wq ? fwd_grid(P, n) : static_grid(P, n);
     const bool whole = P->fwd_sorted && b0 == 0 && n == R.n && R.items_x;   // whole set: longest-first execution order
@@ -94,6 +98,7 @@ void launch_fwd_kernel(fredopt_plan* P, int epi, const RowSet& R, long long b0, 
 void launch_tr_kernel(fredopt_plan* P, const RowSet& R, const Item* items, const int32_t* slots, long long n, const uint8_t* mode,
                       const GatherVec& vec, const uint8_t* live) {
     if (n <= 0) return;
+    chk_sync(P->stream);
     WorkQueue* wq = P->tr_dynamic ? P->wq : nullptr;
     const int g = wq ? fwd_grid(P, n) : static_grid(P, n);
     const void* tc = R.t_col16 ? (const void*)R.t_col16 : (const void*)R.t_col;
@@ -353,6 +358,7 @@ int fredopt_set_option(fredopt_plan* P, int32_t key, double value) {
 
 int fredopt_iterate(fredopt_plan* P, int32_t n_iter, float lambda, float beta0, float a) {
     if (!P || n_iter < 0) return FREDOPT_INVALID_ARG;
+    chk_sync(P->stream);                 // checked build: before any capture begins
     if (!(lambda > 0.f) || !(lambda <= 2.f) || !(beta0 >= 0.f) || !std::isfinite(beta0) || !(a > 0.f) || !(a < 1.f))
         return FREDOPT_INVALID_ARG;
     if (P->shard_world > 1 && !P->reduce_fn) return FREDOPT_INVALID_ARG;

@@ -8,6 +8,10 @@
 
 thread_local std::string g_last_cuda_error;
 
+#ifdef FREDOPT_CHECKED
+void chk_upload_passes(const ChkRange* h, int n) { chk_upload_tu(h, n); }
+#endif
+
 extern "C" {
 
 const char* fredopt_strerror(int code) {
@@ -104,6 +108,7 @@ static int forward_f32(fredopt_plan* P, const RowSet& R, int m, const double* xd
     float *dd = d, *dl = l;
     const bool hd = d && !is_device_ptr(d), hl = l && !is_device_ptr(l);
     if ((hd || hl) && !P->out_stage) CKR(dmalloc(P, &P->out_stage, 2 * (size_t)(P->V ? P->V : 1)));
+    chk_sync(P->stream);                 // checked build: the allocation table on the device is current
     if (hd) dd = P->out_stage;
     if (hl) dl = P->out_stage + (P->V ? P->V : 1);
     if (dd) cudaMemsetAsync(dd, 0, (size_t)P->V * 4, P->stream);
@@ -163,6 +168,7 @@ int fredopt_spmv_transpose(fredopt_plan* P, int32_t rows, const float* u, const 
     if (rows == FREDOPT_ROWS_ALL) {
         if (!R.t_built) CKR(build_transpose(P, R));
         if (!P->fullUV.pair) CKR(gv_alloc(P, &P->fullUV, (size_t)R.n_rows));
+        chk_sync(P->stream);
         vec = P->fullUV;
     }
     const float *du = nullptr, *dv = nullptr; void *fu = nullptr, *fv = nullptr;

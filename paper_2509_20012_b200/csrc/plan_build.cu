@@ -712,13 +712,44 @@ static void compute_pass_bytes(fredopt_plan* P) {
 // ============================================================================================ API
 extern "C" {
 
+#ifdef FREDOPT_CHECKED
+}   // extern "C"
+#include <mutex>
+static std::mutex g_chk_mu;
+static std::vector<ChkRange> g_chk_host;
+static unsigned long long g_chk_version = 0, g_chk_uploaded = ~0ull;
+void chk_register(const void* p, size_t bytes) {
+    std::lock_guard<std::mutex> lk(g_chk_mu);
+    g_chk_host.push_back(ChkRange{(const char*)p, (const char*)p + bytes});
+    ++g_chk_version;
+}
+void chk_unregister(const void* p) {
+    std::lock_guard<std::mutex> lk(g_chk_mu);
+    for (size_t i = 0; i < g_chk_host.size(); ++i)
+        if (g_chk_host[i].b == (const char*)p) { g_chk_host[i] = g_chk_host.back(); g_chk_host.pop_back(); ++g_chk_version; break; }
+}
+void chk_upload_build(const ChkRange* h, int n) { chk_upload_tu(h, n); }
+void chk_sync(cudaStream_t stream) {
+    std::lock_guard<std::mutex> lk(g_chk_mu);
+    if (g_chk_uploaded == g_chk_version) return;
+    cudaStreamCaptureStatus cs = cudaStreamCaptureStatusNone;
+    if (stream && cudaStreamIsCapturing(stream, &cs) == cudaSuccess && cs != cudaStreamCaptureStatusNone) return;
+    cudaDeviceSynchronize();
+    const int n = (int)(g_chk_host.size() < (size_t)CHK_MAX ? g_chk_host.size() : (size_t)CHK_MAX);
+    chk_upload_iterate(g_chk_host.data(), n); chk_upload_passes(g_chk_host.data(), n); chk_upload_build(g_chk_host.data(), n);
+    cudaDeviceSynchronize();
+    g_chk_uploaded = g_chk_version;
+}
+extern "C" {
+#endif
+
 void fredopt_destroy(fredopt_plan* P) {
     if (!P) return;
     cudaStreamSynchronize(P->stream);
     for (auto& ep : P->events) { cudaEventDestroy(ep.a); cudaEventDestroy(ep.b); }
     for (auto& ep : P->event_pool) { cudaEventDestroy(ep.a); cudaEventDestroy(ep.b); }
     for (int i = 0; i < 8; ++i) if (P->gexec[i]) cudaGraphExecDestroy(P->gexec[i]);
-    for (void* p : P->allocs) cudaFree(p);
+    for (void* p : P->allocs) { chk_unregister(p); cudaFree(p); }
     for (int k = 0; k < VB_N; ++k) cudaFree(P->vb_buf[k]);
     if (P->owns_stream) cudaStreamDestroy(P->stream);
     delete P;

@@ -4,6 +4,8 @@ Tolerances (BASELINE.json north_star): per SpMV relative error <= 1e-5; after 20
 error in w <= 1e-4 and an IDENTICAL constraint-violation count.  Transposed passes carry signed
 coefficients, so they are judged element-wise relative to sum_i |A_ij r_i| (parity rule).
 """
+import os
+
 import numpy as np
 import pytest
 import torch
@@ -586,6 +588,27 @@ def test_config3_20_iterations_in_bench_configuration(fredopt):
     plan = pg.build_plan(pg.config_spec(3), device="cuda")
     assert plan.nnz > 1.0e9
     _full_size_parity(fredopt, plan, 20000)
+
+
+@pytest.mark.skipif(os.environ.get("FREDOPT_LONG") != "1", reason="the full horizons of configs[2] and configs[3] take ~12 min of oracle time: FREDOPT_LONG=1")
+@pytest.mark.parametrize("config", [2, 3])
+def test_full_size_over_the_full_horizon(fredopt, config):
+    """BASELINE.json configs[2] and configs[3] at full size over the 500 iterations they state: x, s, trials and the violation
+    count against the oracle every 100 iterations (the record is profiles/r02_parity_full_horizon.md)."""
+    plan = pg.build_plan(pg.config_spec(config), device="cuda")
+    gp = fredopt.from_plan(plan, stream=torch.cuda.current_stream().cuda_stream); orc = _oracle(plan)
+    sp = plan.spec
+    assert sp.n_iter == 500
+    gp.set_weights(plan.x0); orc.set_x(plan.x0)
+    for k in range(5):
+        gp.iterate(100, sp.lam, sp.beta0, sp.a); orc.iterate(100, sp.lam, sp.beta0, sp.a)
+        xg, xo = _gpu_x(gp), orc.get_x()
+        (pgp, ng), (po, no) = gp.proximity(None), orc.proximity(None)
+        sg, so = gp.stats(), orc.stats()
+        print(f"configs[{config}] after {100 * (k + 1)} iterations: rel L2(x) {_rel_l2(xg, xo):.3e}; violated sets gpu / oracle {ng} / {no}; "
+              f"proximity {pgp:.9e} / {po:.9e}; s {sg['s']} / {so['s']}; trials {sg['trials']} / {so['trials']}")
+        _assert_state(gp, orc)
+    gp.destroy()
 
 
 # ------------------------------------------------------------------------------------------ horizons, state, limits
