@@ -113,6 +113,7 @@ struct fredopt_plan {
     uint8_t *mode_union = nullptr, *mode_con = nullptr, *mode_cost = nullptr, *mode_fixed = nullptr;  // mode_fixed: [4][max_seg]
     int max_seg = 1;
     DevState* st = nullptr;
+    DevState* st_host = nullptr;           // pinned host copy for fredopt_get_stats (a pageable target would make the copy a staged one)
     VoxBounds vb = {};                     // per-voxel bounds: row-indexed effective values per field (null = structure scalars)
     double* vb_buf[VB_N] = {};             // the arrays behind vb (owned)
     // vectors (fp64)

@@ -466,9 +466,10 @@ int fredopt_set_state(fredopt_plan* P, const fredopt_state* in) {
 
 int fredopt_get_stats(fredopt_plan* P, fredopt_stats* out) {
     if (!P || !out) return FREDOPT_INVALID_ARG;
-    DevState h;
-    CK(cudaMemcpyAsync(&h, P->st, sizeof(DevState), cudaMemcpyDeviceToHost, P->stream));
+    if (!P->st_host) CK(cudaMallocHost((void**)&P->st_host, sizeof(DevState)));
+    CK(cudaMemcpyAsync(P->st_host, P->st, sizeof(DevState), cudaMemcpyDeviceToHost, P->stream));
     CK(cudaStreamSynchronize(P->stream));
+    const DevState h = *P->st_host;
     out->k = h.k; out->s = h.s; out->trials = h.trials; out->n_violated = h.n_viol;
     out->n_sets = h.n_sets; out->n_zero_norm_sets = h.n_zero;
     out->n_active_rows = P->act.n_true; out->nnz = P->nnz; out->nnz_active = P->act.nnz;

@@ -750,6 +750,7 @@ void fredopt_destroy(fredopt_plan* P) {
     for (auto& ep : P->event_pool) { cudaEventDestroy(ep.a); cudaEventDestroy(ep.b); }
     for (int i = 0; i < 8; ++i) if (P->gexec[i]) cudaGraphExecDestroy(P->gexec[i]);
     for (void* p : P->allocs) { chk_unregister(p); cudaFree(p); }
+    if (P->st_host) cudaFreeHost(P->st_host);
     for (int k = 0; k < VB_N; ++k) cudaFree(P->vb_buf[k]);
     if (P->owns_stream) cudaStreamDestroy(P->stream);
     delete P;
