@@ -204,6 +204,8 @@ def run_ours(args):
         copt["block_rows"] = args.block_rows
     if args.index_width:
         copt["index_width"] = args.index_width
+    if args.value_bits:
+        copt["value_bits"] = args.value_bits
     sharded = bool(args.shard) and ws > 1
     if sharded:                          # ONE plan on all ranks: voxel ranges, x replicated, sums completed by an NCCL all-reduce
         copt.update(shard_rank=rank, shard_world=ws)
@@ -330,7 +332,9 @@ def run_ours(args):
                    "n_sets": stats["n_sets"], "lambda": lam, "beta0": beta0, "a": a,
                    "block_rows": stats["block_rows"], "entries_active": stats["entries_active"],
                    "fill_in": stats["entries_active"] * stats["block_rows"] / max(stats["nnz_active"], 1),
-                   "storage": "fp32 matrix values, 16-bit indices where exact (else int32), fp64 vectors and accumulators",
+                   "storage": ("matrix values ROUNDED TO IEEE HALF and stored in 16 bits (--value-bits 16: a different input, not the headline "
+                               "configuration)" if args.value_bits == 16 else "fp32 matrix values") +
+                              ", 16-bit indices where exact (else int32), fp64 vectors and accumulators",
                    "ams_form": "block-sequential (Fig. 2 loop nest, R23)" if args.block_sequential else "simultaneous (R1)",
                    "passes_per_iteration": 2 if args.ams else 4, "alg_bytes_per_iteration": iter_bytes,
                    "alg_bytes_per_iteration_all_rows": iter_bytes_all_rows,
@@ -543,6 +547,7 @@ def main():
     ap.add_argument("--no-forms", action="store_true", help="skip the comparison of the two feasibility-seeking forms")
     ap.add_argument("--block-rows", type=int, default=0, help="fredopt_create_options.block_rows (0 = automatic)")
     ap.add_argument("--index-width", type=int, default=0, help="fredopt_create_options.index_width (0 = automatic, 32)")
+    ap.add_argument("--value-bits", type=int, default=0, help="fredopt_create_options.value_bits (0 = fp32 values; 16 = values rounded to half)")
     ap.add_argument("--no-pdl", action="store_true", help="FREDOPT_OPT_USE_PDL = 0 (plain launches)")
     ap.add_argument("--skip-satisfied", action="store_true",
                     help="FREDOPT_OPT_SKIP_SATISFIED = 1: the back-projection streams the values of rows with a non-zero coefficient only")

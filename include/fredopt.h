@@ -26,7 +26,7 @@
  *     cudaStreamDefault flags, i.e. ordered against the legacy default stream as any blocking stream is -- the
  *     legacy stream itself cannot be captured into a CUDA graph).  Calls enqueue on that stream; a call that writes host memory synchronises the stream before returning, a call with
  *     device outputs only does not.
- *   - arithmetic: matrix values are stored as given (fp32), indices as 16 bits where that is exact (n_cols <= 65536;
+ *   - arithmetic: matrix values are stored as given (fp32; as IEEE halves of their roundings with fredopt_create_options.value_bits = 16), indices as 16 bits where that is exact (n_cols <= 65536;
  *     row indices of the transposes inside 65536-row blocks) and int32 otherwise, offsets int64; every vector the
  *     iteration keeps (x, d, l, g, u, v) and every accumulator / scalar / decision is fp64 on the device.
  *     fp32 scalars cross the ABI as their bit patterns and are widened, never recomputed.
@@ -171,6 +171,14 @@ typedef struct {
                                 /*     (fredopt_shard_range); this plan keeps range shard_rank of them.  x is replicated;  */
                                 /*     the sums over voxels are completed through fredopt_set_reduce.  0 / 0 or 0 / 1:     */
                                 /*     the whole plan.  fredopt_dose_let and the ROWS_ALL exports always cover all voxels  */
+    int32_t value_bits;         /* 0 / 32 = the matrix values as given (fp32).  16 = every value of D and L is first replaced */
+                                /*     by the nearest IEEE half (round to nearest even; float -> half -> float) -- the plan then */
+                                /*     IS the plan of those rounded matrices: dose_let, the per-pass exports, norms, every        */
+                                /*     iterate agree with any fp64 evaluation of the rounded matrices as the fp32 plan does with  */
+                                /*     the given ones -- and the iteration streams 2-byte copies ("16-bit        */
+                                /*     values"): fewer bytes, a DIFFERENT input (relative change up to 4.9e-4 per value; values     */
+                                /*     below 6e-8 become 0, above 65504 infinity -> INVALID_ARG).  Not the default, not the        */
+                                /*     configuration bench.py's headline times                                                    */
 } fredopt_create_options;
 /* fredopt_create with options (opt = NULL: the defaults, identical to fredopt_create).  INVALID_ARG on an unknown value. */
 int fredopt_create_ex(const fredopt_csr *D, const fredopt_csr *L, const int32_t *voxel_labels,

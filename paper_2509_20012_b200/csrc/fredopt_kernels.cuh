@@ -20,6 +20,7 @@
 // All vectors and accumulators are fp64; matrix values fp32; indices 16-bit where they fit, else int32; offsets int64.
 #pragma once
 #include <cuda_runtime.h>
+#include <cuda_fp16.h>
 #include <stdint.h>
 #include <stdio.h>
 
@@ -176,6 +177,15 @@ __device__ __forceinline__ int4 ld_stream_i4(const int32_t* p) {
     asm volatile("ld.global.nc.L1::no_allocate.v4.s32 {%0,%1,%2,%3}, [%4];"
                  : "=r"(r.x), "=r"(r.y), "=r"(r.z), "=r"(r.w) : "l"(p));
     return r;
+}
+// four consecutive stored values of a matrix as fp32: stored as fp32 (one 128-bit load) or, with the 16-bit value option of
+// fredopt_create_options, as IEEE half (one 64-bit load; half -> float is exact)
+__device__ __forceinline__ float4 ld_stream_f4(const __half* p) {
+    unsigned int lo, hi;
+    chk(p, 8, 2);
+    asm volatile("ld.global.nc.L1::no_allocate.v2.u32 {%0,%1}, [%2];" : "=r"(lo), "=r"(hi) : "l"(p));
+    const float2 a = __half22float2(*reinterpret_cast<const __half2*>(&lo)), b = __half22float2(*reinterpret_cast<const __half2*>(&hi));
+    return make_float4(a.x, a.y, b.x, b.y);
 }
 __device__ __forceinline__ float4 ld_stream_f4(const float* p) {
     float4 r;
@@ -416,9 +426,9 @@ enum : int { EPI_STORE = 0, EPI_STORE_PQ = 1, EPI_CPART = 2, EPI_F32VOX = 3, EPI
 // 128 values the entries are stored interleaved so that the j-th gather of the warp covers CONSECUTIVE entries (few lines of
 // x per instruction).  U chunks per trip (6 for a single matrix, 4 for both): up to 12 independent vector loads per lane in
 // flight before the first gather.
-template <int M, int R, bool I16>
-__device__ __forceinline__ void fwd_row(const void* __restrict__ cbase, long long v0, const float* __restrict__ dp,
-                                        const float* __restrict__ lp, int Lv, int lane, const double* __restrict__ x,
+template <int M, int R, bool I16, typename VT>
+__device__ __forceinline__ void fwd_row(const void* __restrict__ cbase, long long v0, const VT* __restrict__ dp,
+                                        const VT* __restrict__ lp, int Lv, int lane, const double* __restrict__ x,
                                         double (&aD)[R], double (&aL)[R]) {
     constexpr int C = 4 / R;
     constexpr int U = (M == 3) ? FWD_U3 : FWD_U1;
@@ -484,11 +494,11 @@ __device__ __forceinline__ void fwd_row(const void* __restrict__ cbase, long lon
 // = e).  The descriptor of the next item is fetched while the current one is processed.  mode[seg]: bit 0 = read valD, bit 1 =
 // read valL.  Row r = R * b + k (k < rows of the block) indexes every per-row array; partial sums of the epilogues (c, chi^2,
 // proximity, count) are stored per block row and added in a fixed order by the kernel that consumes them.
-template <int EPI, int R, bool I16>
+template <int EPI, int R, bool I16, typename VT>
 __global__ void __launch_bounds__(FWD_THREADS, FWD_MIN_CTAS)
 k_forward(long long n, const Item* __restrict__ items, const int32_t* __restrict__ item_blk, WorkQueue* __restrict__ wq,
           const int32_t* __restrict__ vox, const uint8_t* __restrict__ mode,
-          const void* __restrict__ col, const float* __restrict__ vD, const float* __restrict__ vL,
+          const void* __restrict__ col, const VT* __restrict__ vD, const VT* __restrict__ vL,
           const double* __restrict__ x,
           double* __restrict__ oD, double* __restrict__ oL,                // EPI_STORE*, EPI_CPART, EPI_RESID: row-indexed
           const GatherVec pq,                                              // EPI_STORE_PQ: cost residuals (Eq. 2)
@@ -516,8 +526,8 @@ k_forward(long long n, const Item* __restrict__ items, const int32_t* __restrict
 #pragma unroll
         for (int k = 0; k < R; ++k) { aD[k] = 0.0; aL[k] = 0.0; }
         if (m == 3) fwd_row<3, R, I16>(col, it.start, vD + it.start, vL + it.start, it.len, lane, x, aD, aL);
-        else if (m == 1) fwd_row<1, R, I16>(col, it.start, vD + it.start, nullptr, it.len, lane, x, aD, aL);
-        else if (m == 2) fwd_row<2, R, I16>(col, it.start, nullptr, vL + it.start, it.len, lane, x, aD, aL);
+        else if (m == 1) fwd_row<1, R, I16>(col, it.start, vD + it.start, (const VT*)nullptr, it.len, lane, x, aD, aL);
+        else if (m == 2) fwd_row<2, R, I16>(col, it.start, (const VT*)nullptr, vL + it.start, it.len, lane, x, aD, aL);
 #pragma unroll
         for (int k = 0; k < R; ++k) {
             if (m & 1) aD[k] = warp_sum(aD[k]);
@@ -628,9 +638,9 @@ enum : int { TEPI_F32 = 0, TEPI_GRAD = 1, TEPI_UPDATE = 2 };
 // sum over one item of D_ij cD[i] + L_ij cL[i] by one warp: an entry is one (spot run, block row b) pair with R values per
 // matrix and gathers the R coefficients of rows R b .. R b + R - 1 with one vector load (the gathered vectors are L2 / L1
 // resident; entries of a run ascend in b, so neighbouring lanes gather neighbouring elements)
-template <int M, int R, bool I16>
-__device__ __forceinline__ double tr_item(const void* __restrict__ cbase, long long v0, int add, const float* __restrict__ dp,
-                                          const float* __restrict__ lp, int Lv, int lane, const GatherVec& gv) {
+template <int M, int R, bool I16, typename VT>
+__device__ __forceinline__ double tr_item(const void* __restrict__ cbase, long long v0, int add, const VT* __restrict__ dp,
+                                          const VT* __restrict__ lp, int Lv, int lane, const GatherVec& gv) {
     constexpr int C = 4 / R;
     constexpr int U = (M == 3) ? FWD_U3 : FWD_U1;
     const double2* __restrict__ vec = gv.pair;
@@ -697,9 +707,9 @@ __device__ __forceinline__ double tr_item(const void* __restrict__ cbase, long l
 // gathers only where one of its C entries is live; every skipped term is an exact zero, so the sum has the same bits.  The
 // indices are needed BEFORE the values: those of a trip are loaded one trip ahead (a word or two per chunk and lane) and the
 // liveness bytes (L1-resident) are looked up at the start of the trip.
-template <int M, int R, bool I16>
-__device__ __forceinline__ double tr_item_live(const void* __restrict__ cbase, long long v0, int add, const float* __restrict__ dp,
-                                               const float* __restrict__ lp, int Lv, int lane, const GatherVec& gv,
+template <int M, int R, bool I16, typename VT>
+__device__ __forceinline__ double tr_item_live(const void* __restrict__ cbase, long long v0, int add, const VT* __restrict__ dp,
+                                               const VT* __restrict__ lp, int Lv, int lane, const GatherVec& gv,
                                                const uint8_t* __restrict__ live) {
     constexpr int C = 4 / R;
     constexpr int U = (M == 3) ? FWD_U3 : FWD_U1;
@@ -780,11 +790,11 @@ __device__ __forceinline__ double tr_item_live(const void* __restrict__ cbase, l
 // a CTA mostly work on neighbouring spots of one structure and share L1 lines of the gather vector).  Item e stores its
 // partial sum in slot item_slot[e]; k_combine adds the slots of every spot in slot order.  No floating-point atomics, no
 // fences: the result does not depend on the schedule.
-template <int R, bool I16, bool LIVE>
+template <int R, bool I16, bool LIVE, typename VT>
 __global__ void __launch_bounds__(FWD_THREADS, FWD_MIN_CTAS)
 k_transpose(long long n, const Item* __restrict__ items, const int32_t* __restrict__ item_slot, WorkQueue* __restrict__ wq,
-            const uint8_t* __restrict__ mode, const void* __restrict__ t_col, const float* __restrict__ tD,
-            const float* __restrict__ tL, const GatherVec vec, double* __restrict__ partial,
+            const uint8_t* __restrict__ mode, const void* __restrict__ t_col, const VT* __restrict__ tD,
+            const VT* __restrict__ tL, const GatherVec vec, double* __restrict__ partial,
             const uint8_t* __restrict__ live)          // LIVE: liveness byte per block row (tr_item_live)
 {
     const int lane = threadIdx.x & 31;
@@ -803,12 +813,12 @@ k_transpose(long long n, const Item* __restrict__ items, const int32_t* __restri
         double tot = 0.0;
         if (LIVE) {
             if (m == 3) tot = tr_item_live<3, R, I16>(t_col, it.start, add, tD + it.start, tL + it.start, it.len, lane, vec, live);
-            else if (m == 1) tot = tr_item_live<1, R, I16>(t_col, it.start, add, tD + it.start, nullptr, it.len, lane, vec, live);
-            else if (m == 2) tot = tr_item_live<2, R, I16>(t_col, it.start, add, nullptr, tL + it.start, it.len, lane, vec, live);
+            else if (m == 1) tot = tr_item_live<1, R, I16>(t_col, it.start, add, tD + it.start, (const VT*)nullptr, it.len, lane, vec, live);
+            else if (m == 2) tot = tr_item_live<2, R, I16>(t_col, it.start, add, (const VT*)nullptr, tL + it.start, it.len, lane, vec, live);
         } else {
             if (m == 3) tot = tr_item<3, R, I16>(t_col, it.start, add, tD + it.start, tL + it.start, it.len, lane, vec);
-            else if (m == 1) tot = tr_item<1, R, I16>(t_col, it.start, add, tD + it.start, nullptr, it.len, lane, vec);
-            else if (m == 2) tot = tr_item<2, R, I16>(t_col, it.start, add, nullptr, tL + it.start, it.len, lane, vec);
+            else if (m == 1) tot = tr_item<1, R, I16>(t_col, it.start, add, tD + it.start, (const VT*)nullptr, it.len, lane, vec);
+            else if (m == 2) tot = tr_item<2, R, I16>(t_col, it.start, add, (const VT*)nullptr, tL + it.start, it.len, lane, vec);
         }
         if (m) tot = warp_sum(tot);
         if (lane == 0) partial[item_slot[e0]] = tot;

@@ -52,6 +52,8 @@ struct RowSet {
     uint16_t* col16 = nullptr;       // 16-bit form when n_cols <= 65536 (2 B instead of 4 B per entry)
     float* valD = nullptr;           // R values per entry: value k of entry position p at p * R + k
     float* valL = nullptr;
+    __half* valD16 = nullptr;        // 16-bit value option: half copies, read by the hot kernels instead of valD / valL
+    __half* valL16 = nullptr;
     int32_t* vox = nullptr;          // [n_rows] voxel of the row, -1 = padding
     int16_t* rseg = nullptr;         // [n_rows] structure - 1 of the row, -1 = padding (labelled set only)
     int32_t* seg = nullptr;          // [n] structure - 1 of the block row, or nullptr (one segment)
@@ -73,6 +75,8 @@ struct RowSet {
     int t_H = 1;                     // number of 65536-block-row groups of the list (1 in the 32-bit form)
     float* t_valD = nullptr;
     float* t_valL = nullptr;
+    __half* t_valD16 = nullptr;
+    __half* t_valL16 = nullptr;
     long long t_entries_padded = 0;
     // work items of the transposed pass: runs cut into pieces of at most TR_ITEM_MAX values per matrix
     long long t_n_items = 0;
@@ -139,6 +143,7 @@ struct fredopt_plan {
     int fwd_dynamic = 1, tr_dynamic = 0;   // item kernels fed from the work queue (else static round-robin, two waves)
     int fwd_sorted = 1, tr_sorted = 1;     // items taken longest first (else in storage order)
     bool force_idx32 = false;          // create option: int32 indices in both orientations
+    int value_bits = 32;               // create option: 16 = matrix values rounded to IEEE half, half copies for the iteration
     int block_rows_opt = 0;            // create option: rows per block row of the labelled set (0 = chosen by stored bytes)
     int shard_rank = 0, shard_world = 1;   // create option: this plan keeps one voxel range of the labelled rows
     long long shard_begin = 0, shard_end = 0;

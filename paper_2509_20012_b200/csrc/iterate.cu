@@ -82,15 +82,21 @@ void launch_fwd_kernel(fredopt_plan* P, int epi, const RowSet& R, long long b0, 
     const int32_t* vox = R.vox ? R.vox + b0 * R.R : nullptr;
     const void* col = R.colp();
     const bool i16 = R.col16 != nullptr;
-#define FWD_CALL(RB, I16)                                                                                                        \
-    switch (epi) {                                                                                                               \
-        case EPI_STORE: klaunch(P, k_forward<EPI_STORE, RB, I16>, g, FWD_THREADS, n, items, iblk, wq, vox, mode, col, R.valD, R.valL, x, oD, oL, pq, tab, P->vb, cpart, P->st, fD, fL, letd_out, ra); break;       \
-        case EPI_STORE_PQ: klaunch(P, k_forward<EPI_STORE_PQ, RB, I16>, g, FWD_THREADS, n, items, iblk, wq, vox, mode, col, R.valD, R.valL, x, oD, oL, pq, tab, P->vb, cpart, P->st, fD, fL, letd_out, ra); break; \
-        case EPI_CPART: klaunch(P, k_forward<EPI_CPART, RB, I16>, g, FWD_THREADS, n, items, iblk, wq, vox, mode, col, R.valD, R.valL, x, oD, oL, pq, tab, P->vb, cpart, P->st, fD, fL, letd_out, ra); break;       \
-        case EPI_F32VOX: klaunch(P, k_forward<EPI_F32VOX, RB, I16>, g, FWD_THREADS, n, items, iblk, wq, vox, mode, col, R.valD, R.valL, x, oD, oL, pq, tab, P->vb, cpart, P->st, fD, fL, letd_out, ra); break;     \
-        default: klaunch(P, k_forward<EPI_RESID, RB, I16>, g, FWD_THREADS, n, items, iblk, wq, vox, mode, col, R.valD, R.valL, x, oD, oL, pq, tab, P->vb, cpart, P->st, fD, fL, letd_out, ra); break;              \
+#define FWD_ARGS(VD, VL) g, FWD_THREADS, n, items, iblk, wq, vox, mode, col, VD, VL, x, oD, oL, pq, tab, P->vb, cpart, P->st, fD, fL, letd_out, ra
+#define FWD_CALL_VT(RB, I16, VT, VD, VL)                                                          \
+    switch (epi) {                                                                                \
+        case EPI_STORE: klaunch(P, k_forward<EPI_STORE, RB, I16, VT>, FWD_ARGS(VD, VL)); break;    \
+        case EPI_STORE_PQ: klaunch(P, k_forward<EPI_STORE_PQ, RB, I16, VT>, FWD_ARGS(VD, VL)); break; \
+        case EPI_CPART: klaunch(P, k_forward<EPI_CPART, RB, I16, VT>, FWD_ARGS(VD, VL)); break;    \
+        case EPI_F32VOX: klaunch(P, k_forward<EPI_F32VOX, RB, I16, VT>, FWD_ARGS(VD, VL)); break;  \
+        default: klaunch(P, k_forward<EPI_RESID, RB, I16, VT>, FWD_ARGS(VD, VL)); break;           \
     }
+#define FWD_CALL(RB, I16)                                                                         \
+    if (R.valD16) { FWD_CALL_VT(RB, I16, __half, (const __half*)R.valD16, (const __half*)R.valL16) } \
+    else { FWD_CALL_VT(RB, I16, float, (const float*)R.valD, (const float*)R.valL) }
     FREDOPT_DISPATCH(R.R, i16, FWD_CALL)
+#undef FWD_CALL_VT
+#undef FWD_ARGS
 #undef FWD_CALL
 }
 
@@ -104,10 +110,14 @@ void launch_tr_kernel(fredopt_plan* P, const RowSet& R, const Item* items, const
     const void* tc = R.t_col16 ? (const void*)R.t_col16 : (const void*)R.t_col;
     const bool i16 = R.t_col16 != nullptr;
     if (!P->skip_dead) live = nullptr;
-#define TR_CALL(RB, I16)                                                                                                                      \
-    if (live) klaunch(P, k_transpose<RB, I16, true>, g, FWD_THREADS, n, items, slots, wq, mode, tc, R.t_valD, R.t_valL, vec, R.t_partial, live);  \
-    else klaunch(P, k_transpose<RB, I16, false>, g, FWD_THREADS, n, items, slots, wq, mode, tc, R.t_valD, R.t_valL, vec, R.t_partial, live)
+#define TR_CALL_VT(RB, I16, VT, TD, TL)                                                                                         \
+    if (live) klaunch(P, k_transpose<RB, I16, true, VT>, g, FWD_THREADS, n, items, slots, wq, mode, tc, TD, TL, vec, R.t_partial, live); \
+    else klaunch(P, k_transpose<RB, I16, false, VT>, g, FWD_THREADS, n, items, slots, wq, mode, tc, TD, TL, vec, R.t_partial, live);
+#define TR_CALL(RB, I16)                                                                                                         \
+    if (R.t_valD16) { TR_CALL_VT(RB, I16, __half, (const __half*)R.t_valD16, (const __half*)R.t_valL16) }                        \
+    else { TR_CALL_VT(RB, I16, float, (const float*)R.t_valD, (const float*)R.t_valL) }
     FREDOPT_DISPATCH(R.R, i16, TR_CALL)
+#undef TR_CALL_VT
 #undef TR_CALL
     if (live && P->time_passes && P->live_count && &R == &P->act && n == R.t_n_items) {
         // measurement: what this launch needed, counted by a separate kernel; launch_transpose closes the timed bracket first

@@ -74,6 +74,19 @@ __global__ void k_union_fill(const long long* pD, const int32_t* cD, const float
     }
 }
 
+// 16-bit value storage (fredopt_create_options.value_bits = 16): every stored value is replaced by the nearest IEEE half (round to
+// nearest even, the conversion numpy and every IEEE library perform), in place in fp32 -- norms, tables and the fp32 row sets then
+// see exactly the values the half copies hold -- and the hot arrays get half copies
+__global__ void k_round_to_half(float* v, size_t n, int* overflow) {
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) {
+        const float r = __half2float(__float2half_rn(v[i]));
+        if (isinf(r)) *overflow = 1;                                 // |value| > 65504 (inputs are finite: checked before)
+        v[i] = r;
+    }
+}
+__global__ void k_to_half(const float* v, __half* h, size_t n) {
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) h[i] = __float2half_rn(v[i]);
+}
 // per voxel: padded length of the row as a block row of its own (multiple of 4; int64 for the scan), flags
 __global__ void k_row_lengths(const long long* ptr, const int32_t* lab, long long V, long long vb, long long ve, int32_t* nonempty,
                               int32_t* active) {
@@ -690,11 +703,12 @@ static void compute_pass_bytes(fredopt_plan* P) {
         const int f = T.flags;
         const int cost = ((f & F_DOSE_REF) ? 1 : 0) | ((f & F_DL_REF) ? 2 : 0);
         const int con = ((f & (F_DOSE_SLAB | F_LETD)) ? 1 : 0) | ((f & (F_DL_SLAB | F_LETD)) ? 2 : 0);
-        auto per = [&](int m, int ib) { return m ? (long long)T.entries * ib + (long long)T.nnz * 4 * ((m & 1) + ((m >> 1) & 1)) : 0LL; };
+        const int vw = P->act.valD16 ? 2 : 4;                                   // value bytes as stored
+        auto per = [&](int m, int ib) { return m ? (long long)T.entries * ib + (long long)T.nnz * vw * ((m & 1) + ((m >> 1) & 1)) : 0LL; };
         fwd_union += per(cost | con, ibf);
         tr_cost += per(cost, ibt);
         tr_con += per(con, ibt);
-        con_values += (long long)T.nnz * 4 * ((con & 1) + ((con >> 1) & 1));
+        con_values += (long long)T.nnz * vw * ((con & 1) + ((con >> 1) & 1));
         if (cost | con) rows_union += T.rows;
         if (con) rows_con += T.rows;
         if (cost) rows_cost += T.rows;
@@ -823,8 +837,8 @@ static int create_impl(fredopt_plan* P, const fredopt_csr* D, const fredopt_csr*
     CKR(to_dev(labels, V * 4, (const void**)&lab));
     // ---- validate
     int* flag = nullptr;
-    CKR(tmp.get(&flag, 2));
-    CK(cudaMemsetAsync(flag, 0, 2 * sizeof(int), st));
+    CKR(tmp.get(&flag, 3));                                      // [0] invalid input, [1] patterns differ, [2] a value beyond the range of a half
+    CK(cudaMemsetAsync(flag, 0, 3 * sizeof(int), st));
     k_check_ptr<<<grid_for(V + 1, 256, 4096), 256, 0, st>>>(pD, V, D->nnz, flag);
     k_check_ptr<<<grid_for(V + 1, 256, 4096), 256, 0, st>>>(pL, V, L->nnz, flag);
     k_check_labels<<<grid_for(V, 256, 4096), 256, 0, st>>>(lab, V, n_struct, flag);
@@ -924,6 +938,10 @@ static int create_impl(fredopt_plan* P, const fredopt_csr* D, const fredopt_csr*
         CK(cudaMemsetAsync(F.valD, 0, np * 4, st)); CK(cudaMemsetAsync(F.valL, 0, np * 4, st));
         if (n_ne) {
             k_copy_rows1<<<grid_for((long long)n_ne * 32, 256, 1 << 16), 256, 0, st>>>(F.n, F.vox, F.start, pU, cU, uD, uL, F.col, F.col16, F.valD, F.valL);
+            if (P->value_bits == 16) {
+                k_round_to_half<<<P->sm_count * 8, 256, 0, st>>>(F.valD, np, flag + 2);
+                k_round_to_half<<<P->sm_count * 8, 256, 0, st>>>(F.valL, np, flag + 2);
+            }
             k_pack_items<<<grid_for(n_ne, 256, 4096), 256, 0, st>>>(n_ne, 1, F.start, F.len, nullptr, nullptr, F.items);
         }
         CK(cudaStreamSynchronize(st));
@@ -1038,6 +1056,10 @@ static int create_impl(fredopt_plan* P, const fredopt_csr* D, const fredopt_csr*
             if (Rb == 1) k_block_union<1, true><<<g, 128, 0, st>>>(n_blk, A.vox, pU, cU, uD, uL, nullptr, A.start, A.len, A.col, A.col16, A.valD, A.valL);
             else if (Rb == 2) k_block_union<2, true><<<g, 128, 0, st>>>(n_blk, A.vox, pU, cU, uD, uL, nullptr, A.start, A.len, A.col, A.col16, A.valD, A.valL);
             else k_block_union<4, true><<<g, 128, 0, st>>>(n_blk, A.vox, pU, cU, uD, uL, nullptr, A.start, A.len, A.col, A.col16, A.valD, A.valL);
+            if (P->value_bits == 16) {      // before the norms: everything that follows sees the rounded values
+                k_round_to_half<<<P->sm_count * 8, 256, 0, st>>>(A.valD, na * Rb, flag + 2);
+                k_round_to_half<<<P->sm_count * 8, 256, 0, st>>>(A.valL, na * Rb, flag + 2);
+            }
             k_pack_items<<<grid_for(n_blk, 256, 4096), 256, 0, st>>>(n_blk, Rb, A.start, A.len, A.seg, nreal, A.items);
             // execution order of the whole-set passes: longest block rows first (the queue then ends with the short ones)
             uint32_t *ik, *ik2, *ii, *ii2;
@@ -1096,6 +1118,17 @@ static int create_impl(fredopt_plan* P, const fredopt_csr* D, const fredopt_csr*
     CK(cudaMemsetAsync(P->part_cnt, 0, npart * 8, st));
     // ---- CSR of the transposes restricted to the labelled rows
     CKR(build_transpose(P, A));
+    if (P->value_bits == 16) {              // half copies of the arrays the iteration streams (the fp32 ones stay for set-up work)
+        const size_t na = (size_t)(A.entries_padded ? A.entries_padded : 4) * A.R, nt = (size_t)(A.t_entries_padded ? A.t_entries_padded : 4) * A.R;
+        CKR(dmalloc(P, &A.valD16, na)); CKR(dmalloc(P, &A.valL16, na)); CKR(dmalloc(P, &A.t_valD16, nt)); CKR(dmalloc(P, &A.t_valL16, nt));
+        k_to_half<<<P->sm_count * 8, 256, 0, st>>>(A.valD, A.valD16, na); k_to_half<<<P->sm_count * 8, 256, 0, st>>>(A.valL, A.valL16, na);
+        k_to_half<<<P->sm_count * 8, 256, 0, st>>>(A.t_valD, A.t_valD16, nt); k_to_half<<<P->sm_count * 8, 256, 0, st>>>(A.t_valL, A.t_valL16, nt);
+        CK(cudaGetLastError());
+        int over = 0;
+        CK(cudaMemcpyAsync(&over, flag + 2, sizeof(int), cudaMemcpyDeviceToHost, st));
+        CK(cudaStreamSynchronize(st));
+        if (over) return FREDOPT_INVALID_ARG;                    // a value beyond the range of a half
+    }
     compute_pass_bytes(P);
     // Forward items from the queue only when there are enough of them to balance: below ~6 items per resident warp the static
     // deal is faster (configs[1] 16.7 k vs 14.0 k iterations/s, configs[2] 6 961 vs 6 174; configs[3], 9.6 items per warp: 1 695
@@ -1155,6 +1188,7 @@ int fredopt_create_ex(const fredopt_csr* D, const fredopt_csr* L, const int32_t*
     }
     if (o.index_width != 0 && o.index_width != 32) return FREDOPT_INVALID_ARG;
     if (o.block_rows != 0 && o.block_rows != 1 && o.block_rows != 2 && o.block_rows != 4) return FREDOPT_INVALID_ARG;
+    if (o.value_bits != 0 && o.value_bits != 32 && o.value_bits != 16) return FREDOPT_INVALID_ARG;
     if (o.shard_world < 0 || o.shard_rank < 0 || (o.shard_world == 0 && o.shard_rank != 0) || (o.shard_world > 0 && o.shard_rank >= o.shard_world))
         return FREDOPT_INVALID_ARG;
     if (!D || !L || n_struct < 0 || (n_struct > 0 && !bounds)) return FREDOPT_INVALID_ARG;
@@ -1182,6 +1216,7 @@ int fredopt_create_ex(const fredopt_csr* D, const fredopt_csr* L, const int32_t*
     P->sm_count = prop.multiProcessorCount;
     P->force_idx32 = o.index_width == 32;
     P->block_rows_opt = o.block_rows;
+    P->value_bits = o.value_bits == 16 ? 16 : 32;
     P->shard_rank = o.shard_rank; P->shard_world = o.shard_world > 1 ? o.shard_world : 1;
     int rc = create_impl(P, D, L, voxel_labels, bounds, n_struct);
     if (rc != FREDOPT_OK) { fredopt_destroy(P); return rc; }

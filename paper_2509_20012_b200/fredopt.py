@@ -55,7 +55,7 @@ class _Bounds(C.Structure):
 
 class _CreateOptions(C.Structure):
     _fields_ = [("struct_size", C.c_int32), ("index_width", C.c_int32), ("block_rows", C.c_int32), ("shard_rank", C.c_int32),
-                ("shard_world", C.c_int32)]
+                ("shard_world", C.c_int32), ("value_bits", C.c_int32)]
 
 
 REDUCE_FN = C.CFUNCTYPE(C.c_int, C.c_void_p, C.c_void_p, C.c_int64, C.c_void_p)   # fredopt_reduce_fn

@@ -51,7 +51,7 @@ def test_strerror_and_struct_layout(lib_path):
     assert C.sizeof(fredopt._Bounds) == 32       # 8 floats
     assert C.sizeof(fredopt.Stats) == 12 * 8 + 4 * 8
     assert C.sizeof(fredopt.State) == 3 * 8 + 3 * 8 + 2 * 4 + 2 * 4
-    assert C.sizeof(fredopt._CreateOptions) == 5 * 4
+    assert C.sizeof(fredopt._CreateOptions) == 6 * 4
 
 
 def test_null_arguments_are_rejected_without_touching_a_device(lib_path):

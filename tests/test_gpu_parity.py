@@ -818,6 +818,92 @@ def test_skipping_on_a_plan_where_most_rows_are_satisfied(fredopt):
     assert np.array_equal(xs[0], xs[1])
 
 
+# ------------------------------------------------------------------------------------------ 16-bit values
+def _rounded_to_half(plan):
+    """The plan of the matrices rounded to IEEE half by numpy (float32 -> float16 -> float32): what value_bits = 16 stores."""
+    import dataclasses
+    rd = lambda t: torch.from_numpy(t.cpu().numpy().astype(np.float16).astype(np.float32)).to(t.device)
+    return dataclasses.replace(plan, val_D=rd(plan.val_D), val_L=rd(plan.val_L))
+
+
+@pytest.mark.parametrize("copt", [pytest.param({}, id="auto"), pytest.param({"block_rows": 1}, id="rows1"),
+                                  pytest.param({"block_rows": 4, "index_width": 32}, id="rows4-idx32")])
+def test_16_bit_values_are_the_plan_of_the_rounded_matrices(fredopt, plan0, copt):
+    """fredopt_create_options.value_bits = 16 (SURVEY sec. 8f-2 "16-bit values ... parity to be re-established"): the library
+    rounds every value of D and L to the nearest IEEE half and streams 2-byte copies.  Parity is re-established against the
+    oracle fed the SAME rounding done independently (numpy's float16 conversion): iterations within the usual bars, and -- since
+    half -> float is exact and the kernels add in the same order -- the same bits in x as the fp32-storage plan of the rounded
+    matrices; forward, transposed, block-sequential and evaluation calls agree too; the fp32 plan of the ORIGINAL matrices
+    differs (the rounding is real); a value beyond the range of a half is refused."""
+    f = fredopt
+    pr = _rounded_to_half(plan0)
+    assert not torch.equal(pr.val_D, plan0.val_D)
+    sp = plan0.spec
+    gp = f.from_plan(plan0, value_bits=16, **copt)               # the library rounds
+    g32 = f.from_plan(pr, **copt)                                # fp32 storage of the rounded matrices
+    orc = _oracle(pr)
+    assert gp.pass_bytes()["forward_x"] < g32.pass_bytes()["forward_x"]
+    for p_ in (gp, g32):
+        p_.set_weights(plan0.x0)
+        p_.iterate(30, sp.lam, sp.beta0, sp.a)
+    orc.set_x(plan0.x0); orc.iterate(30, sp.lam, sp.beta0, sp.a)
+    _assert_state(gp, orc)
+    assert np.array_equal(_gpu_x(gp), _gpu_x(g32))
+    # forward over all rows (fp32 row set of the rounded values) and over the labelled rows (half copies)
+    x = pg.log_uniform_weights(7, plan0.n_cols)
+    d_ref, l_ref, t_ref = orc.dose_let(x.astype(np.float64))
+    dose = np.empty(plan0.n_rows, np.float32); letd = np.empty(plan0.n_rows, np.float32)
+    gp.dose_let(x, dose, letd)
+    _assert_fwd(dose, d_ref, "dose"); _assert_fwd(letd, t_ref, "LETd")
+    d = np.empty(plan0.n_rows, np.float32); l = np.empty(plan0.n_rows, np.float32)
+    gp.spmv_forward(f.ROWS_ACTIVE, x, d, l)
+    lab = plan0.labels.numpy() > 0
+    _assert_fwd(d[lab], d_ref[lab], "D x (labelled)"); _assert_fwd(l[lab], l_ref[lab], "L x (labelled)")
+    # transposed over the labelled rows
+    V = plan0.n_rows
+    u = (pg.uniform01_array(31, V) - 0.4).astype(np.float32); v = (pg.uniform01_array(32, V) - 0.6).astype(np.float32)
+    ref, ref_abs = orc.transpose(u.astype(np.float64), v.astype(np.float64), active_only=True)
+    out = np.empty(plan0.n_cols, np.float32)
+    gp.spmv_transpose(f.ROWS_ACTIVE, u, v, out)
+    assert np.all(np.abs(out - ref) <= TOL_SPMV * ref_abs)
+    # block-sequential form
+    from oracle import oracle as om
+    gp.set_option(f.OPT_BLOCK_SEQUENTIAL, 1); orc.set_option(om.OPT_BLOCK_SEQUENTIAL, 1)
+    gp.iterate(5, sp.lam, sp.beta0, sp.a); orc.iterate(5, sp.lam, sp.beta0, sp.a)
+    _assert_block_state(gp, orc)
+    # the rounding is real: the plan of the original matrices goes elsewhere
+    g0 = f.from_plan(plan0, **copt)
+    g0.set_weights(plan0.x0); g0.iterate(30, sp.lam, sp.beta0, sp.a)
+    g32.set_option(f.OPT_RESET, 1); g32.set_weights(plan0.x0); g32.iterate(30, sp.lam, sp.beta0, sp.a)
+    assert 1e-7 < _rel_l2(_gpu_x(g0), _gpu_x(g32)) < 1e-2
+    for p_ in (gp, g32, g0):
+        p_.destroy()
+    # out of range
+    big = _rounded_to_half(plan0)
+    vd = plan0.val_D.clone(); vd[0] = 7.0e4
+    import dataclasses
+    with pytest.raises(f.FredoptError) as e:
+        f.from_plan(dataclasses.replace(plan0, val_D=vd), value_bits=16)
+    assert e.value.code == f.INVALID_ARG
+    with pytest.raises(f.FredoptError):
+        f.from_plan(plan0, value_bits=8)
+
+
+def test_16_bit_values_three_beam_plan(fredopt):
+    """The same on a three-beam plan (rejected step sizes, LETd rows that read both matrices) with 20 + 5 iterations."""
+    f = fredopt
+    plan = pg.build_plan(pg.config_spec(2, scale=0.2), device="cuda")
+    pr = _rounded_to_half(plan)
+    sp = plan.spec
+    gp = f.from_plan(plan, value_bits=16); orc = _oracle(pr)
+    gp.set_weights(plan.x0); orc.set_x(plan.x0)
+    gp.iterate(20, sp.lam, sp.beta0, sp.a); orc.iterate(20, sp.lam, sp.beta0, sp.a)
+    _assert_state(gp, orc)
+    gp.iterate(5, sp.lam, 0.0, sp.a); orc.iterate(5, sp.lam, 0.0, sp.a)
+    _assert_state(gp, orc)
+    gp.destroy()
+
+
 # ------------------------------------------------------------------------------------------ per-voxel bounds (SURVEY 8f-4)
 def _varying_voxel_bounds(plan, bounds, seed):
     """Per-voxel arrays around the structures' scalars (+-, NaN on ~30 % of the voxels), voxel-indexed float32, for every field."""
