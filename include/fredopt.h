@@ -156,8 +156,8 @@ int fredopt_create(const fredopt_csr *D, const fredopt_csr *L, const int32_t *vo
                    const fredopt_bounds *bounds, int32_t n_struct, void *cuda_stream, fredopt_plan **out);
 
 /* Storage choices of a plan, fixed at creation ("optimized method for storing the Dij and LETij matrices", PAPER.md:282;
- * SURVEY sec. 8f-2).  They change the bytes a pass moves, never a result: index work is exact, and every sum runs over the
- * same terms plus exact zeros.  struct_size = sizeof(fredopt_create_options) of the caller (the struct may grow). */
+ * SURVEY sec. 8f-2).  index_width and block_rows change the bytes a pass moves, never a result: index work is exact, and every
+ * sum runs over the same terms plus exact zeros; value_bits = 16 changes the INPUT (see the field).  struct_size = sizeof(fredopt_create_options) of the caller (the struct may grow). */
 typedef struct {
     int32_t struct_size;
     int32_t index_width;        /* 0 = automatic: 16-bit indices where exact (n_cols <= 65536; block-row indices of the */
