@@ -78,7 +78,7 @@ struct RowSet {
     __half* t_valD16 = nullptr;
     __half* t_valL16 = nullptr;
     long long t_entries_padded = 0;
-    // work items of the transposed pass: runs cut into pieces of at most TR_ITEM_MAX values per matrix
+    // work items of the transposed pass: runs cut into pieces of at most 3 072 (large plans) or TR_ITEM_MAX values per matrix
     long long t_n_items = 0;
     Item* t_items = nullptr;         // [t_n_items] longest first
     int32_t* t_item_slot = nullptr;  // [t_n_items] slot of the item's partial sum

@@ -53,7 +53,10 @@ int fwd_grid(fredopt_plan* P, long long n) {
     return grid_for(n, FWD_WARPS, P->sm_count * FWD_MIN_CTAS);
 }
 // static round-robin form of the item kernels (no queue): two waves of the resident CTAs
-static int static_grid(fredopt_plan* P, long long n) { return grid_for(n, FWD_WARPS, P->sm_count * FWD_MIN_CTAS * 2); }
+#ifndef STATIC_WAVES
+#define STATIC_WAVES 2
+#endif
+static int static_grid(fredopt_plan* P, long long n) { return grid_for(n, FWD_WARPS, P->sm_count * FWD_MIN_CTAS * STATIC_WAVES); }
 
 
 const ResidArgs NO_RESID{nullptr, nullptr, nullptr, GatherVec{nullptr, nullptr, nullptr}, nullptr, nullptr, nullptr, nullptr, nullptr};

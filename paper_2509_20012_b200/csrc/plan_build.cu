@@ -412,9 +412,9 @@ __global__ void k_pack_items(long long n, int R, const long long* start, const i
     }
 }
 // items per (spot, segment, group) run: ceil(values / TR_ITEM_MAX)
-__global__ void k_tr_item_count(const long long* t_ptr, long long K, int R, long long* cnt) {
+__global__ void k_tr_item_count(const long long* t_ptr, long long K, int R, int item_max, long long* cnt) {
     for (long long k = (long long)blockIdx.x * blockDim.x + threadIdx.x; k < K; k += (long long)gridDim.x * blockDim.x)
-        cnt[k] = ((t_ptr[k + 1] - t_ptr[k]) * R + TR_ITEM_MAX - 1) / TR_ITEM_MAX;
+        cnt[k] = ((t_ptr[k + 1] - t_ptr[k]) * R + item_max - 1) / item_max;
 }
 // the same counts in spot-major order (the order of a spot's partial-sum slots)
 __global__ void k_tr_item_count_sm(const long long* cnt, long long S, int n_seg, int H, long long* cnt_sm) {
@@ -425,15 +425,15 @@ __global__ void k_tr_item_count_sm(const long long* cnt, long long S, int n_seg,
 }
 // item.seg = segment | (group << 8): the kernel adds group << 16 to the 16-bit block-row indices
 __global__ void k_tr_item_fill(const long long* t_ptr, const long long* ibase, const long long* sbase, long long S, int n_seg, int H, int R,
-                               Item* items, int32_t* item_slot) {
+                               int item_max, Item* items, int32_t* item_slot) {
     for (long long k = (long long)blockIdx.x * blockDim.x + threadIdx.x; k < S * n_seg * H; k += (long long)gridDim.x * blockDim.x) {
         const long long b = t_ptr[k] * R, e = t_ptr[k + 1] * R;          // in values per matrix
         const long long hi = k % H, js = k / H, j = js % S, sg0 = js / S;
         const long long sg = sg0 | (hi << 8);
         long long i = ibase[k], slot = sbase[(j * n_seg + sg0) * H + hi];
-        for (long long p = b; p < e; p += TR_ITEM_MAX, ++i, ++slot) {
+        for (long long p = b; p < e; p += item_max, ++i, ++slot) {
             Item it;
-            it.start = p; it.len = (int32_t)((e - p) < TR_ITEM_MAX ? (e - p) : TR_ITEM_MAX); it.seg = (int32_t)sg;
+            it.start = p; it.len = (int32_t)((e - p) < item_max ? (e - p) : item_max); it.seg = (int32_t)sg;
             items[i] = it;
             item_slot[i] = (int32_t)slot;
         }
@@ -441,16 +441,16 @@ __global__ void k_tr_item_fill(const long long* t_ptr, const long long* ibase, c
 }
 // longest-first execution order: key = length class (256-value bins, longest = 0); a stable sort keeps the
 // (structure, spot) order inside a class
-__global__ void k_tr_item_key(const Item* items, long long n, uint32_t* key, uint32_t* idx) {
+__global__ void k_tr_item_key(const Item* items, long long n, int item_max, uint32_t* key, uint32_t* idx) {
     for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (long long)gridDim.x * blockDim.x) {
-        key[i] = (uint32_t)((TR_ITEM_MAX - items[i].len) / 256);
+        key[i] = (uint32_t)((item_max - items[i].len) / 256);
         idx[i] = (uint32_t)i;
     }
 }
-__global__ void k_tr_item_key_seg(const Item* items, long long n, uint32_t* key, uint32_t* idx, unsigned long long* hist) {
+__global__ void k_tr_item_key_seg(const Item* items, long long n, int item_max, uint32_t* key, uint32_t* idx, unsigned long long* hist) {
     for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (long long)gridDim.x * blockDim.x) {
         const uint32_t sg = (uint32_t)(items[i].seg & 0xFF);
-        key[i] = sg * 16u + (uint32_t)((TR_ITEM_MAX - items[i].len) / 256);
+        key[i] = sg * 16u + (uint32_t)((item_max - items[i].len) / 256);
         idx[i] = (uint32_t)i;
         atomicAdd(hist + sg, 1ULL);
     }
@@ -570,7 +570,11 @@ int build_transpose(fredopt_plan* P, RowSet& R) {
     // ---- work items: every (segment, spot, group) run cut into pieces of at most TR_ITEM_MAX values, in run order
     //      (neighbouring items = neighbouring spots of one structure: overlapping voxel footprints share L1 lines)
     CK(cudaMemsetAsync(pcount, 0, (K + 2) * sizeof(long long), st));
-    k_tr_item_count<<<grid_for(K, 256, 4096), 256, 0, st>>>(R.t_ptr, K, RB, pcount);
+    // Items of 3 072 values on large plans: 24 chunks are whole trips for both trip sizes (4 x 6 and 6 x 4 chunks), so no item ends on
+    // a ragged trip (configs[3] +1.4 %, configs[2] +1.7 %); small plans keep 2 048 (configs[1] -5 % with 3 072: fewer items than warps).
+    const int item_max = (&R == &P->act && R.nnz >= 50000000LL) ? 3072 : TR_ITEM_MAX;
+    static_assert(3072 % 256 == 0 && 3072 / 256 < 16, "length-class keys");
+    k_tr_item_count<<<grid_for(K, 256, 4096), 256, 0, st>>>(R.t_ptr, K, RB, item_max, pcount);
     long long* cnt_sm = nullptr;
     CKR(T.get(&cnt_sm, (size_t)K + 2));
     CKR(dmalloc(P, &R.t_slot_ptr, (size_t)K + 2));       // kept: slot ranges per (spot, structure, group) for the block-sequential sweep
@@ -583,7 +587,7 @@ int build_transpose(fredopt_plan* P, RowSet& R) {
     CK(cudaStreamSynchronize(st));
     CKR(dmalloc(P, &R.t_items, (size_t)R.t_n_items)); CKR(dmalloc(P, &R.t_item_slot, (size_t)R.t_n_items));
     CKR(dmalloc(P, &R.t_item_ptr, (size_t)S + 1)); CKR(dmalloc(P, &R.t_partial, (size_t)R.t_n_items));
-    k_tr_item_fill<<<grid_for(K, 256, 4096), 256, 0, st>>>(R.t_ptr, ustart, sbase, S, R.n_seg, H, RB, R.t_items, R.t_item_slot);
+    k_tr_item_fill<<<grid_for(K, 256, 4096), 256, 0, st>>>(R.t_ptr, ustart, sbase, S, R.n_seg, H, RB, item_max, R.t_items, R.t_item_slot);
     k_tr_item_ptr<<<grid_for(S + 1, 256, 4096), 256, 0, st>>>(sbase, S, (long long)R.n_seg * H, R.t_item_ptr);
     CK(cudaGetLastError());
     CK(cudaStreamSynchronize(st));
@@ -597,7 +601,7 @@ int build_transpose(fredopt_plan* P, RowSet& R) {
         CKR(T.get(&hist, 256));
         CK(cudaMemsetAsync(hist, 0, 256 * 8, st));
         CKR(dmalloc(P, &R.t_items_seg, (size_t)ni)); CKR(dmalloc(P, &R.t_slot_seg, (size_t)ni));
-        k_tr_item_key_seg<<<grid_for(ni, 256, 4096), 256, 0, st>>>(R.t_items, ni, ik, ii, hist);
+        k_tr_item_key_seg<<<grid_for(ni, 256, 4096), 256, 0, st>>>(R.t_items, ni, item_max, ik, ii, hist);
         size_t sb = 0;
         void* stmp = nullptr;
         CK(cub::DeviceRadixSort::SortPairs(nullptr, sb, ik, ik2, ii, ii2, ni, 0, 12, st));
@@ -623,7 +627,7 @@ int build_transpose(fredopt_plan* P, RowSet& R) {
         Item* it2 = nullptr; int32_t* js2 = nullptr;
         CKR(T.get(&ik, (size_t)ni)); CKR(T.get(&ik2, (size_t)ni)); CKR(T.get(&ii, (size_t)ni)); CKR(T.get(&ii2, (size_t)ni));
         CKR(T.get(&it2, (size_t)ni)); CKR(T.get(&js2, (size_t)ni));
-        k_tr_item_key<<<grid_for(ni, 256, 4096), 256, 0, st>>>(R.t_items, ni, ik, ii);
+        k_tr_item_key<<<grid_for(ni, 256, 4096), 256, 0, st>>>(R.t_items, ni, item_max, ik, ii);
         size_t sb = 0;
         void* stmp = nullptr;
         CK(cub::DeviceRadixSort::SortPairs(nullptr, sb, ik, ik2, ii, ii2, ni, 0, 4, st));
