@@ -62,6 +62,8 @@ def test_null_arguments_are_rejected_without_touching_a_device(lib_path):
     assert L.fredopt_proximity(None, None, None, None) == fredopt.INVALID_ARG
     assert L.fredopt_dose_let(None, None, None, None) == fredopt.INVALID_ARG
     assert L.fredopt_launch_count(None) == 0
+    assert L.fredopt_get_pass_bytes_timed(None, None) == fredopt.INVALID_ARG
+    assert L.fredopt_set_option(None, fredopt.OPT_SKIP_SATISFIED, 1.0) == fredopt.INVALID_ARG
     L.fredopt_destroy(None)
 
 
