@@ -120,8 +120,8 @@ typedef struct {
                                        /*    an item's sum is formed by one warp in a fixed order and stored to a place of its own). */
                                        /*    bit 0 / bit 1: forward / transposed passes take items from a queue (a warp that         */
                                        /*    finishes early takes more) instead of a static round-robin deal; bit 2 / bit 3: forward  */
-                                       /*    / transposed items are taken longest first instead of in storage order.  Default 12, and    */
-                                       /*    13 (forward items from the queue) when the plan has at least 6 block rows per resident warp  */
+                                       /*    / transposed items are taken longest first instead of in storage order.  Default: 12, with    */
+                                       /*    bit 0 decided per forward launch (queue iff >= 6 items per resident warp of >= 2048 values) */
 #define FREDOPT_OPT_USE_PDL         10 /* 1 (default): the kernels of an iteration are launched with programmatic dependent    */
                                        /*    launch (a kernel's CTAs are scheduled while its predecessor drains); 0: plain launches */
 #define FREDOPT_OPT_SKIP_SATISFIED  12 /* 1: the back-projection of the simultaneous step streams the values of a row only if the row   */

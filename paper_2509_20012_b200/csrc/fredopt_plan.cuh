@@ -140,7 +140,8 @@ struct fredopt_plan {
     long long reductionsN = 1, max_trials = 200;
     int accept_check = 1, use_graph = 1, time_passes = 0, block_sequential = 0, normalize_grad = 0, one_sided_cost = 0;
     int use_pdl = 1;
-    int fwd_dynamic = 1, tr_dynamic = 0;   // item kernels fed from the work queue (else static round-robin, two waves)
+    int fwd_dynamic = -1, tr_dynamic = 0;  // item kernels fed from the work queue (else static round-robin, two waves); -1: per launch
+                                           // by item count and length (launch_fwd_kernel)
     int fwd_sorted = 1, tr_sorted = 1;     // items taken longest first (else in storage order)
     bool force_idx32 = false;          // create option: int32 indices in both orientations
     int value_bits = 32;               // create option: 16 = matrix values rounded to IEEE half, half copies for the iteration

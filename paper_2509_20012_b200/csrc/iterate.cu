@@ -77,7 +77,13 @@ void launch_fwd_kernel(fredopt_plan* P, int epi, const RowSet& R, long long b0, 
                        int letd_out, const ResidArgs& ra) {
     if (n <= 0) return;
     chk_sync(P->stream);
-    WorkQueue* wq = P->fwd_dynamic ? P->wq : nullptr;
+    // Items from the queue or dealt statically: FREDOPT_OPT_WORK_QUEUE decides if it was set; otherwise the queue is used where it
+    // pays -- enough items to balance (at least 6 per resident warp) and long ones (2 048 values on average): with short rows the
+    // one counter every warp increments per item becomes the bottleneck (isolated forward pass over all rows, 2.9e8 non-zeros, mean
+    // row 900: 2.5 TB/s from the queue, 5.1 TB/s dealt statically), with few items there is nothing to balance.
+    const bool dyn = P->fwd_dynamic >= 0 ? P->fwd_dynamic != 0
+                                         : (R.n >= 6LL * P->sm_count * FWD_MIN_CTAS * FWD_WARPS && R.entries_padded * R.R >= 2048LL * R.n);
+    WorkQueue* wq = dyn ? P->wq : nullptr;
     const int g = wq ? fwd_grid(P, n) : static_grid(P, n);
     const bool whole = P->fwd_sorted && b0 == 0 && n == R.n && R.items_x;   // whole set: longest-first execution order
     const Item* items = whole ? R.items_x : R.items + b0;

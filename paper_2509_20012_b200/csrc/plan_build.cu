@@ -1134,10 +1134,6 @@ static int create_impl(fredopt_plan* P, const fredopt_csr* D, const fredopt_csr*
         if (over) return FREDOPT_INVALID_ARG;                    // a value beyond the range of a half
     }
     compute_pass_bytes(P);
-    // Forward items from the queue only when there are enough of them to balance: below ~6 items per resident warp the static
-    // deal is faster (configs[1] 16.7 k vs 14.0 k iterations/s, configs[2] 6 961 vs 6 174; configs[3], 9.6 items per warp: 1 695
-    // from the queue vs 1 645 static).  FREDOPT_OPT_WORK_QUEUE overrides.
-    P->fwd_dynamic = P->act.n >= 6LL * P->sm_count * FWD_MIN_CTAS * FWD_WARPS ? 1 : 0;
     CK(cudaStreamSynchronize(st));
     return FREDOPT_OK;
 }
