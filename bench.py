@@ -268,14 +268,13 @@ def run_ours(args):
     xo = torch.empty_like(xh).pin_memory()
     gp.set_option(fredopt.OPT_RESET, 1)
     for _ in range(W):
-        gp.set_weights(xh); gp.iterate(1, lam, beta0, a); gp.get_weights(xo); xh.copy_(xo)
+        gp.iterate_host(1, lam, beta0, a, xh, xo); xh.copy_(xo)
     barrier()
     t0 = time.perf_counter()
     for _ in range(K):
-        gp.set_weights(xh)                    # H2D: S floats from pinned host memory
-        gp.iterate(1, lam, beta0, a)
-        gp.get_weights(xo)                    # D2H: S floats (synchronises)
-        st_e = gp.stats()                     # D2H: the step's metrics (proximity, chi^2, violation count, k, s, beta)
+        # one C-ABI call per step (fredopt_iterate_host): H2D of S floats from pinned host memory, the iteration, D2H of S floats
+        # and of the step's metrics (proximity, chi^2, violation count, k, s, beta), one synchronisation
+        st_e = gp.iterate_host(1, lam, beta0, a, xh, xo)
         xh.copy_(xo)
     prox, nviol = st_e["prox"], st_e["n_violated"]
     barrier()
@@ -348,7 +347,7 @@ def run_ours(args):
                                    "iteration)" % ws) if sharded else "1 plan per GPU"},
         "iter_gbs": iter_bytes * K / (ms * 1e-3) / 1e9,
         "e2e": {"value": whole_job_rate(K, 1 if sharded else ws, e2e_s), "unit": UNIT, "h2d_bytes_per_step": plan.n_cols * 4,
-                "d2h_bytes_per_step": plan.n_cols * 4 + STATE_BYTES},
+                "d2h_bytes_per_step": plan.n_cols * 4 + STATE_BYTES, "call": "fredopt_iterate_host (pinned host buffers, one call per step)"},
         "gpu_launches": int(launches),
         "clocks": clocks,
         "roofline": {"bound": "hbm", "kernel": top, "kernel_names": PASS_KERNELS.get(top, top), "achieved": achieved, "peak": peak, "unit": "GB/s",

@@ -203,6 +203,16 @@ int fredopt_dose_let(fredopt_plan *plan, const float *x, float *dose, float *let
  * beta0 and a are latched at the first call after create / RESET.  Asynchronous (device work only). */
 int fredopt_iterate(fredopt_plan *plan, int32_t n_iter, float lambda, float beta0, float a);
 
+/* The same n_iter iterations as ONE call with the caller's buffers, one synchronisation at its end (the call of an
+ * application that keeps its spot weights on the host; bench.py's end-to-end figure times it).  In stream order:
+ * x_in (n_cols floats, host or device, or NULL = continue from the plan's x) replaces the plan's x as fredopt_set_weights
+ * does; fredopt_iterate(n_iter, lambda, beta0, a); x_out (n_cols floats, host or device, or NULL) receives the plan's x
+ * rounded to fp32 as fredopt_get_weights does; stats (HOST, or NULL) as fredopt_get_stats.  Both arrays are borrowed for
+ * the call only.  Results are those of the four calls made one after the other, bit for bit.  Errors: those of
+ * fredopt_iterate; when the iterations are refused x_in is installed all the same and x_out, stats are untouched. */
+int fredopt_iterate_host(fredopt_plan *plan, int32_t n_iter, float lambda, float beta0, float a,
+                         const float *x_in, float *x_out, fredopt_stats *stats);
+
 /* Per-voxel bounds and references (bounds are "upper and lower constraints for all organs or defined for each
  * point in the image space"; Eq. (2): per-voxel Dref_i, cDLref_i).  values: n_rows floats, voxel-indexed,
  * host or device; NaN = the voxel keeps its structure's scalar; NULL removes the field's array.  A value applies where the

@@ -255,6 +255,7 @@ void launch_tr_kernel(fredopt_plan* P, const RowSet& R, const Item* items, const
 void launch_transpose(fredopt_plan* P, int tepi, const RowSet& R, const uint8_t* mode, const GatherVec& vec, double* g_out,
                       double* x, float* f_out, const uint8_t* live = nullptr);
 void launch_finalize(fredopt_plan* P, int n_part);
+void fill_stats(fredopt_plan* P, const DevState& h, fredopt_stats* out);   // iterate.cu: the public statistics from a host copy of the state
 void launch_sum_to(fredopt_plan* P, double* out, const double* in, const long long* in_ll, int n);   // out[0] = fixed-order sum
 void invalidate_graphs(fredopt_plan* P);
 int reduce_call(fredopt_plan* P, double* buf, long long n);      // the caller's reduction on the plan's stream (sharded plans)                         // captured launches hold kernel arguments: capture again

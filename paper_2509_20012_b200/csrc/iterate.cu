@@ -315,6 +315,19 @@ void state_init(fredopt_plan* P) {
 }
 
 // ============================================================================================ API
+void fill_stats(fredopt_plan* P, const DevState& h, fredopt_stats* out) {
+    out->k = h.k; out->s = h.s; out->trials = h.trials; out->n_violated = h.n_viol;
+    out->n_sets = h.n_sets; out->n_zero_norm_sets = h.n_zero;
+    out->n_active_rows = P->act.n_true; out->nnz = P->nnz; out->nnz_active = P->act.nnz;
+    out->block_rows = P->act.R; out->entries_active = P->act.entries;
+    long long b = 0;
+    const int sa_passes[] = {FREDOPT_PASS_FORWARD_X, FREDOPT_PASS_TRANSPOSE_G, FREDOPT_PASS_FORWARD_G, FREDOPT_PASS_SELECT,
+                             FREDOPT_PASS_RESIDUAL, FREDOPT_PASS_TRANSPOSE_B};
+    for (int p : sa_passes) b += P->pass_bytes[p];
+    out->alg_bytes_iter = b;
+    out->last_beta = h.last_beta; out->phi = h.phi; out->prox = h.prox; out->weight_sum = h.W;
+}
+
 extern "C" {
 
 int fredopt_set_option(fredopt_plan* P, int32_t key, double value) {
@@ -488,17 +501,7 @@ int fredopt_get_stats(fredopt_plan* P, fredopt_stats* out) {
     if (!P->st_host) CK(cudaMallocHost((void**)&P->st_host, sizeof(DevState)));
     CK(cudaMemcpyAsync(P->st_host, P->st, sizeof(DevState), cudaMemcpyDeviceToHost, P->stream));
     CK(cudaStreamSynchronize(P->stream));
-    const DevState h = *P->st_host;
-    out->k = h.k; out->s = h.s; out->trials = h.trials; out->n_violated = h.n_viol;
-    out->n_sets = h.n_sets; out->n_zero_norm_sets = h.n_zero;
-    out->n_active_rows = P->act.n_true; out->nnz = P->nnz; out->nnz_active = P->act.nnz;
-    out->block_rows = P->act.R; out->entries_active = P->act.entries;
-    long long b = 0;
-    const int sa_passes[] = {FREDOPT_PASS_FORWARD_X, FREDOPT_PASS_TRANSPOSE_G, FREDOPT_PASS_FORWARD_G, FREDOPT_PASS_SELECT,
-                             FREDOPT_PASS_RESIDUAL, FREDOPT_PASS_TRANSPOSE_B};
-    for (int p : sa_passes) b += P->pass_bytes[p];
-    out->alg_bytes_iter = b;
-    out->last_beta = h.last_beta; out->phi = h.phi; out->prox = h.prox; out->weight_sum = h.W;
+    fill_stats(P, *P->st_host, out);
     return FREDOPT_OK;
 }
 

@@ -91,6 +91,47 @@ int fredopt_get_weights(fredopt_plan* P, float* x) {
     return FREDOPT_OK;
 }
 
+int fredopt_iterate_host(fredopt_plan* P, int32_t n_iter, float lambda, float beta0, float a, const float* x_in, float* x_out,
+                         fredopt_stats* stats) {
+    if (!P) return FREDOPT_INVALID_ARG;
+    // everything is enqueued on the plan's stream; the caller's arrays are borrowed until the one synchronisation at the end
+    bool pending_host_copy = false;
+    if (x_in) {
+        const float* dx = x_in;
+        if (!is_device_ptr(x_in)) {
+            CK(cudaMemcpyAsync(P->xstage, x_in, (size_t)P->S * 4, cudaMemcpyHostToDevice, P->stream));
+            dx = P->xstage;
+            pending_host_copy = true;
+        }
+        k_f32_to_f64<<<grid_for(P->S, 256, 1024), 256, 0, P->stream>>>(dx, P->x, P->S);
+        ++P->launches;
+    }
+    const int rc = fredopt_iterate(P, n_iter, lambda, beta0, a);
+    if (rc != FREDOPT_OK) {
+        if (pending_host_copy) cudaStreamSynchronize(P->stream);
+        return rc;
+    }
+    if (x_out) {
+        if (is_device_ptr(x_out)) {
+            k_f64_to_f32<<<grid_for(P->S, 256, 1024), 256, 0, P->stream>>>(P->x, x_out, P->S);
+            ++P->launches;
+        } else {
+            float* tmp = (float*)P->xtmp;   // S doubles of scratch hold S floats
+            k_f64_to_f32<<<grid_for(P->S, 256, 1024), 256, 0, P->stream>>>(P->x, tmp, P->S);
+            ++P->launches;
+            CK(cudaMemcpyAsync(x_out, tmp, (size_t)P->S * 4, cudaMemcpyDeviceToHost, P->stream));
+        }
+    }
+    if (stats) {
+        if (!P->st_host) CK(cudaMallocHost((void**)&P->st_host, sizeof(DevState)));
+        CK(cudaMemcpyAsync(P->st_host, P->st, sizeof(DevState), cudaMemcpyDeviceToHost, P->stream));
+    }
+    CK(cudaGetLastError());
+    CK(cudaStreamSynchronize(P->stream));
+    if (stats) fill_stats(P, *P->st_host, stats);
+    return FREDOPT_OK;
+}
+
 // x argument of dose_let / proximity / spmv_forward: NULL = plan's x, else widened into xtmp
 static int resolve_x(fredopt_plan* P, const float* x, const double** xd) {
     if (!x) { *xd = P->x; return FREDOPT_OK; }

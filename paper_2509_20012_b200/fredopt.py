@@ -27,7 +27,7 @@ N_PASSES = len(PASS_NAMES)
 SYMBOLS = (
     "fredopt_create", "fredopt_create_ex", "fredopt_destroy", "fredopt_set_weights", "fredopt_get_weights", "fredopt_get_weights_f64",
     "fredopt_set_weights_f64", "fredopt_get_state", "fredopt_set_state", "fredopt_shard_range", "fredopt_set_reduce",
-    "fredopt_set_voxel_bounds", "fredopt_dose_let", "fredopt_iterate", "fredopt_proximity", "fredopt_set_option", "fredopt_get_stats",
+    "fredopt_set_voxel_bounds", "fredopt_dose_let", "fredopt_iterate", "fredopt_iterate_host", "fredopt_proximity", "fredopt_set_option", "fredopt_get_stats",
     "fredopt_spmv_forward", "fredopt_spmv_transpose", "fredopt_get_pass_times", "fredopt_get_pass_bytes",
     "fredopt_get_pass_bytes_timed",
     "fredopt_launch_count", "fredopt_stream_read", "fredopt_strerror", "fredopt_last_cuda_error",
@@ -103,6 +103,7 @@ def _load():
     lib.fredopt_set_voxel_bounds.argtypes = [vp, i32, vp]
     lib.fredopt_dose_let.argtypes = [vp, vp, vp, vp]
     lib.fredopt_iterate.argtypes = [vp, i32, f32, f32, f32]
+    lib.fredopt_iterate_host.argtypes = [vp, i32, f32, f32, f32, vp, vp, C.POINTER(Stats)]
     lib.fredopt_proximity.argtypes = [vp, vp, C.POINTER(f64), C.POINTER(i64)]
     lib.fredopt_set_option.argtypes = [vp, i32, f64]
     lib.fredopt_get_stats.argtypes = [vp, C.POINTER(Stats)]
@@ -233,6 +234,13 @@ class Plan:
 
     def iterate(self, n_iter, lam, beta0, a):
         _check(_lib.fredopt_iterate(self._h, int(n_iter), float(lam), float(beta0), float(a)), "fredopt_iterate")
+
+    def iterate_host(self, n_iter, lam, beta0, a, x_in=None, x_out=None, stats=True):
+        """set_weights(x_in), iterate, get_weights(x_out), stats as one call with one synchronisation; returns the stats or None."""
+        s = Stats() if stats else None
+        _check(_lib.fredopt_iterate_host(self._h, int(n_iter), float(lam), float(beta0), float(a), _ptr(x_in, np.float32, self.n_cols),
+                                         _ptr(x_out, np.float32, self.n_cols), C.byref(s) if stats else None), "fredopt_iterate_host")
+        return s.as_dict() if stats else None
 
     def proximity(self, x=None):
         p, n = C.c_double(0.0), C.c_int64(0)

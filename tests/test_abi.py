@@ -59,6 +59,7 @@ def test_null_arguments_are_rejected_without_touching_a_device(lib_path):
     L = fredopt._lib
     assert L.fredopt_create(None, None, None, None, 0, None, None) == fredopt.INVALID_ARG
     assert L.fredopt_iterate(None, 1, 1.0, 1.0, 0.5) == fredopt.INVALID_ARG
+    assert L.fredopt_iterate_host(None, 1, 1.0, 1.0, 0.5, None, None, None) == fredopt.INVALID_ARG
     assert L.fredopt_proximity(None, None, None, None) == fredopt.INVALID_ARG
     assert L.fredopt_dose_let(None, None, None, None) == fredopt.INVALID_ARG
     assert L.fredopt_launch_count(None) == 0

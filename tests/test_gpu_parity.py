@@ -1048,3 +1048,38 @@ def test_checkpoint_and_resume_in_a_new_plan(fredopt, plan0, tmp_path):
     bad = f.State(); bad.k = -1
     with pytest.raises(f.FredoptError):
         c.set_state(bad)
+
+
+def test_iterate_host_is_the_four_calls_in_one(fredopt, plan0):
+    """fredopt_iterate_host(x_in, x_out, stats) = set_weights, iterate, get_weights, get_stats made one after the other, bit for
+    bit, over steps that pass x through the caller's fp32 array each time (bench.py's end-to-end loop); with NULL arrays it is
+    fredopt_iterate on the plan's own x; and three such steps stay on the oracle's trajectory fed the same rounded x."""
+    f = fredopt
+    sp = plan0.spec
+    a, b = f.from_plan(plan0), f.from_plan(plan0)
+    xa, xb = plan0.x0.copy(), plan0.x0.copy()
+    out_a, out_b = np.empty_like(xa), np.empty_like(xb)
+    orc = _oracle(plan0)
+    for step in range(3):
+        a.set_weights(xa); a.iterate(2, sp.lam, sp.beta0, sp.a); a.get_weights(out_a); sa = a.stats()
+        sb = b.iterate_host(2, sp.lam, sp.beta0, sp.a, xb, out_b)
+        assert np.array_equal(out_a, out_b)
+        assert sa == sb
+        orc.set_x(xa.astype(np.float64)); orc.iterate(2, sp.lam, sp.beta0, sp.a)
+        assert _rel_l2(out_b.astype(np.float64), orc.get_x()) <= 1e-6            # out is rounded to fp32
+        xa, xb = out_a.copy(), out_b.copy()
+    # device arrays, and no arrays at all
+    import torch
+    xd = torch.from_numpy(plan0.x0).cuda(); od = torch.empty_like(xd)
+    c = f.from_plan(plan0)
+    c.iterate_host(2, sp.lam, sp.beta0, sp.a, xd, od, stats=False)
+    d = f.from_plan(plan0); d.set_weights(plan0.x0); d.iterate_host(2, sp.lam, sp.beta0, sp.a)
+    assert np.array_equal(_gpu_x(c), _gpu_x(d))
+    torch.cuda.synchronize()
+    ref = np.empty_like(plan0.x0); d.get_weights(ref)
+    assert np.array_equal(od.cpu().numpy(), ref)
+    # a refused iteration returns the error of fredopt_iterate
+    with pytest.raises(f.FredoptError):
+        d.iterate_host(1, 3.0, sp.beta0, sp.a, plan0.x0, out_a)
+    for g in (a, b, c, d):
+        g.destroy()
