@@ -288,6 +288,29 @@ int fredopt_volume_histogram(fredopt_plan *plan, const float *x, int32_t quantit
 int fredopt_percentile_value(fredopt_plan *plan, const float *x, int32_t quantity, int32_t label, double fraction,
                              double *value);
 
+/* ---- the one call that allocates nothing (for callers that cannot call cudaMalloc: code under CUDA graph capture, serving
+ * loops, harnesses that forbid it).  The cumulative volume histogram of fredopt_volume_histogram over the CALLER's arrays,
+ * without a plan: values = n_voxels floats, voxel-indexed (e.g. an output of fredopt_dose_let); labels = n_voxels int32 or
+ * NULL; the structure is the voxels with labels[i] == label (every voxel when labels is NULL).
+ *     hist[b] = fraction of the structure's voxels whose value is >= b * vmax / n_bins, b = 0..n_bins-1; zeros if it is empty;
+ *     *n_in_structure = the structure's voxel count (may be NULL).
+ * values, labels, hist, n_in_structure: DEVICE pointers, borrowed until the work has run.  Asynchronous on cuda_stream
+ * (NULL = the default stream); the device is the CURRENT one.  Bins are decided in fp64 from the fp32 values, as
+ * fredopt_volume_histogram decides them from its fp64 products: a value within fp32 rounding of a bin edge may sit in the
+ * neighbouring bin.
+ * Scratch: the bin counters live in a fixed array in device memory that every GPU loading the library holds until the process
+ * exits ((FREDOPT_NO_ALLOC_MAX_BINS + 1) * 8 = 32 776 bytes).  All calls on a GPU share it; each call clears what it uses
+ * first, in stream order.  Calls that can overlap on one GPU (different streams, no dependency) RACE on it: order them.
+ * No cudaMalloc / cudaFree / allocating library routine is called, neither here nor in fredopt_no_alloc_setup.
+ * Errors: INVALID_ARG (null values / hist, n_voxels < 0, n_bins < 1, vmax not positive and finite, and n_bins >
+ * FREDOPT_NO_ALLOC_MAX_BINS: the text of fredopt_last_cuda_error() then names the limit), UNSUPPORTED_ARCH, CUDA_ERROR.
+ * fredopt_no_alloc_setup looks up the scratch's device address for the current device (once per device; the histogram call
+ * does it on first use otherwise): call it before a stream capture begins, since the look-up may load the module. */
+#define FREDOPT_NO_ALLOC_MAX_BINS 4096
+int fredopt_no_alloc_setup(void);
+int fredopt_volume_histogram_no_alloc(const float *values, const int32_t *labels, int64_t n_voxels, int32_t label,
+                                      int32_t n_bins, double vmax, float *hist, int64_t *n_in_structure, void *cuda_stream);
+
 /* ---- per-pass exports: per-SpMV parity tests and the isolated-pass sweep (BASELINE.json configs[4]) ----
  * forward:   d = D x, l = L x over the selected rows; d, l: n_rows floats, voxel-indexed (rows outside the
  *            selection are written as 0); either may be NULL (that matrix's values are then not read).

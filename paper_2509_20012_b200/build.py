@@ -8,7 +8,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libfredopt.so")
-SOURCES = [os.path.join(CSRC, f) for f in ("plan_build.cu", "iterate.cu", "passes.cu")]
+SOURCES = [os.path.join(CSRC, f) for f in ("plan_build.cu", "iterate.cu", "passes.cu", "no_alloc.cu")]
 DEPS = SOURCES + [os.path.join(CSRC, f) for f in ("fredopt_kernels.cuh", "kernels_iter.cuh", "kernels_eval.cuh", "fredopt_plan.cuh")] + \
     [os.path.join(os.path.dirname(HERE), "include", "fredopt.h")]
 

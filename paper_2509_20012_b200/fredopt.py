@@ -32,6 +32,7 @@ SYMBOLS = (
     "fredopt_get_pass_bytes_timed",
     "fredopt_launch_count", "fredopt_stream_read", "fredopt_strerror", "fredopt_last_cuda_error",
     "fredopt_structure_stats", "fredopt_volume_histogram", "fredopt_percentile_value",
+    "fredopt_no_alloc_setup", "fredopt_volume_histogram_no_alloc",
 )
 
 
@@ -112,6 +113,8 @@ def _load():
     lib.fredopt_structure_stats.argtypes = [vp, vp, i32, i32, C.POINTER(f64), C.POINTER(f64), C.POINTER(f64), C.POINTER(i64)]
     lib.fredopt_volume_histogram.argtypes = [vp, vp, i32, i32, i32, f64, vp]
     lib.fredopt_percentile_value.argtypes = [vp, vp, i32, i32, f64, C.POINTER(f64)]
+    lib.fredopt_no_alloc_setup.argtypes = []
+    lib.fredopt_volume_histogram_no_alloc.argtypes = [vp, vp, i64, i32, i32, f64, vp, vp, vp]
     lib.fredopt_get_pass_times.argtypes = [vp, C.POINTER(f64), C.POINTER(i64)]
     lib.fredopt_get_pass_bytes.argtypes = [vp, C.POINTER(i64)]
     lib.fredopt_get_pass_bytes_timed.argtypes = [vp, C.POINTER(i64)]
@@ -321,6 +324,27 @@ class Plan:
 
     def stream_read(self, device_buf, nbytes, reps=1):
         _check(_lib.fredopt_stream_read(self._h, _ptr(device_buf), int(nbytes), int(reps)), "fredopt_stream_read")
+
+
+NO_ALLOC_MAX_BINS = 4096      # FREDOPT_NO_ALLOC_MAX_BINS
+
+
+def no_alloc_setup():
+    """Look up the fixed scratch of volume_histogram_no_alloc on the current device (before a stream capture begins)."""
+    _check(_lib.fredopt_no_alloc_setup(), "fredopt_no_alloc_setup")
+
+
+def volume_histogram_no_alloc(values, labels, label, n_bins, vmax, hist, n_in_structure=None, stream=None):
+    """fredopt_volume_histogram_no_alloc: DEVICE tensors only (values float32 [n], labels int32 [n] or None, hist float32
+    [n_bins], n_in_structure int64 [1] or None); asynchronous on `stream` (a cudaStream_t as int; None = default stream)."""
+    n = values.numel()
+    if hist.numel() < n_bins:
+        raise ValueError(f"hist holds {hist.numel()} floats, n_bins = {n_bins}")
+    rc = _lib.fredopt_volume_histogram_no_alloc(_ptr(values, np.float32, n), _ptr(labels, np.int32, n), n, int(label), int(n_bins),
+                                                float(vmax), _ptr(hist, np.float32), _ptr(n_in_structure, np.int64, 1), stream)
+    if rc != OK:
+        raise FredoptError(rc, "fredopt_volume_histogram_no_alloc [" + _lib.fredopt_last_cuda_error().decode() + "]")
+    return hist
 
 
 def shard_range(row_ptr, voxel_labels, rank, world):

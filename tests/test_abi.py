@@ -61,6 +61,7 @@ def test_null_arguments_are_rejected_without_touching_a_device(lib_path):
     assert L.fredopt_iterate(None, 1, 1.0, 1.0, 0.5) == fredopt.INVALID_ARG
     assert L.fredopt_iterate_host(None, 1, 1.0, 1.0, 0.5, None, None, None) == fredopt.INVALID_ARG
     assert L.fredopt_proximity(None, None, None, None) == fredopt.INVALID_ARG
+    assert L.fredopt_volume_histogram_no_alloc(None, None, 0, 0, 8, 1.0, None, None, None) == fredopt.INVALID_ARG
     assert L.fredopt_dose_let(None, None, None, None) == fredopt.INVALID_ARG
     assert L.fredopt_launch_count(None) == 0
     assert L.fredopt_get_pass_bytes_timed(None, None) == fredopt.INVALID_ARG
