@@ -131,6 +131,29 @@ def _dist_init():
     return ws, rank, lr
 
 
+# ------------------------------------------------------------------------------------------------ the workload, as both arms state it
+L2_RESIDENT_BYTES = 256 * 1024 * 1024      # 2 x the B200's 126 MB L2: below this a pass's matrix bytes can stay in L2
+
+
+def workload_config(args, spec, plan, ws=1, sharded=False):
+    """`config` of the JSON line: what is computed, from the plan and the flags alone (no library call), so that `--impl reference`
+    states the same object.  How OUR arm stores the plan (block rows, index width, bytes) is in its `plan` key."""
+    lab = plan.labels > 0
+    nnz_lab = int((plan.row_ptr[1:] - plan.row_ptr[:-1])[lab].sum())
+    resident = 2 * 4 * nnz_lab < L2_RESIDENT_BYTES               # D and L values of the labelled rows, one pass
+    return {"workload": f"configs[{args.config}] {spec.name}", "n_voxels": plan.n_rows, "n_spots": plan.n_cols,
+            "nnz_per_matrix": plan.nnz, "n_labelled_voxels": int(lab.sum()), "nnz_labelled_per_matrix": nnz_lab,
+            "lambda": spec.lam, "beta0": 0.0 if args.ams else spec.beta0, "a": spec.a,
+            "value_bits": 16 if args.value_bits == 16 else 32,
+            "ams_form": "block-sequential (Fig. 2 loop nest, R23)" if args.block_sequential else "simultaneous (R1)",
+            "form": "pure feasibility-seeking (beta0 = 0)" if args.ams else "superiorized",
+            "l2": ("L2-resident working set (labelled values of one pass %.1f MB < 256 MB): the GPU arm flushes L2 once before the timed "
+                   "region; HBM fraction not meaningful" % (8 * nnz_lab / 1e6)) if resident else
+                  "inputs larger than L2 (labelled values of one pass: %.2f GB)" % (8 * nnz_lab / 1e9),
+            "parallelism": ("one plan sharded over %d GPUs by voxel range (x replicated, 3 all-reduces of <= n_spots + 3 doubles per "
+                            "iteration)" % ws) if sharded else "1 plan per GPU"}
+
+
 # ------------------------------------------------------------------------------------------------ reference arm
 def run_reference(args):
     """The oracle, as it stands, on the host cores (its OpenMP timing build: the same source, row loops on all cores): the same
@@ -142,13 +165,19 @@ def run_reference(args):
     from paper_2509_20012_b200 import plangen as pg
     spec = pg.config_spec(args.config)
     plan = pg.build_plan(spec, device="cuda" if torch.cuda.is_available() else "cpu")
+    if args.value_bits == 16:            # the plan of the matrices rounded to half (round to nearest even), as fredopt_create_options.value_bits = 16 defines it
+        plan.val_D = plan.val_D.half().float()
+        plan.val_L = plan.val_L.half().float()
     cores = oracle.omp_threads()
     orc = oracle.from_plan(plan, omp=True)
+    if args.block_sequential:
+        orc.set_option(oracle.OPT_BLOCK_SEQUENTIAL, 1)
     orc.set_x(plan.x0)
     K, W = args.steps, args.warmup
-    orc.iterate(W, spec.lam, spec.beta0, spec.a)
+    beta0 = 0.0 if args.ams else spec.beta0
+    orc.iterate(W, spec.lam, beta0, spec.a)
     t0 = time.perf_counter()
-    orc.iterate(K, spec.lam, spec.beta0, spec.a)
+    orc.iterate(K, spec.lam, beta0, spec.a)
     dt = time.perf_counter() - t0
     v = K / dt
     sample = (f"iterations {W}..{W + K - 1} from x0 of configs[{args.config}] ({spec.name}), full plan: the window of our arm; fp64 oracle, "
@@ -156,8 +185,7 @@ def run_reference(args):
     print(json.dumps({
         "impl": "reference", "metric": METRIC, "value": v, "unit": UNIT, "n_gpus": args.gpus, "steps": K, "warmup": W,
         "ms_per_step": 1e3 * dt / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
-        "data": "synthetic", "config": {"workload": f"configs[{args.config}] {spec.name}", "nnz": plan.nnz,
-                                        "n_spots": plan.n_cols, "n_voxels": plan.n_rows},
+        "data": "synthetic", "config": workload_config(args, spec, plan, ws=args.gpus, sharded=bool(args.shard) and args.gpus > 1),
         "cpu_baseline": {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
         "e2e": {"value": v, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0}))
@@ -238,8 +266,9 @@ def run_ours(args):
     if args.ams:      # forward over the constraint rows + back-projection; the vector kernels are noise at this size
         iter_bytes = pass_bytes["transpose_b"] * 2
     l2_bytes = torch.cuda.get_device_properties(lr).L2_cache_size
+    config = workload_config(args, spec, plan, ws=ws, sharded=sharded)
     flush = None
-    if iter_bytes < 2 * l2_bytes:
+    if config["l2"].startswith("L2-resident"):
         flush = torch.empty(int(1.5 * l2_bytes), dtype=torch.uint8, device="cuda")
 
     def barrier():
@@ -326,25 +355,17 @@ def run_ours(args):
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": ws, "steps": K, "warmup": W, "ms_per_step": ms / K,
         "higher_is_better": True, "scaling": "strong" if sharded else "weak", "vs_baseline": None, "dtype": "f64",
         "data": "synthetic",
-        "config": {"workload": f"configs[{args.config}] {spec.name}", "n_voxels": plan.n_rows, "n_spots": plan.n_cols,
-                   "nnz_per_matrix": plan.nnz, "nnz_active": stats["nnz_active"], "n_active_rows": stats["n_active_rows"],
-                   "n_sets": stats["n_sets"], "lambda": lam, "beta0": beta0, "a": a,
-                   "block_rows": stats["block_rows"], "entries_active": stats["entries_active"],
-                   "fill_in": stats["entries_active"] * stats["block_rows"] / max(stats["nnz_active"], 1),
-                   "storage": ("matrix values ROUNDED TO IEEE HALF and stored in 16 bits (--value-bits 16: a different input, not the headline "
-                               "configuration)" if args.value_bits == 16 else "fp32 matrix values") +
-                              ", 16-bit indices where exact (else int32), fp64 vectors and accumulators",
-                   "ams_form": "block-sequential (Fig. 2 loop nest, R23)" if args.block_sequential else "simultaneous (R1)",
-                   "passes_per_iteration": 2 if args.ams else 4, "alg_bytes_per_iteration": iter_bytes,
-                   "alg_bytes_per_iteration_all_rows": iter_bytes_all_rows,
-                   "back_projection": "values of rows with a non-zero coefficient only (--skip-satisfied)" if args.skip_satisfied else
-                                      "every value",
-                   "form": "pure feasibility-seeking (beta0 = 0)" if args.ams else "superiorized",
-                   "l2": ("L2-resident working set (%.1f MB < 2 x L2): L2 flushed once before the timed region; "
-                          "HBM fraction not meaningful" % (iter_bytes / 1e6)) if flush is not None else
-                         "inputs larger than L2 (%.2f GB streamed per iteration)" % (iter_bytes / 1e9),
-                   "parallelism": ("one plan sharded over %d GPUs by voxel range (x replicated, 3 all-reduces of <= n_spots + 3 doubles per "
-                                   "iteration)" % ws) if sharded else "1 plan per GPU"},
+        "config": config,
+        "plan": {"nnz_active": stats["nnz_active"], "n_active_rows": stats["n_active_rows"], "n_sets": stats["n_sets"],
+                 "block_rows": stats["block_rows"], "entries_active": stats["entries_active"],
+                 "fill_in": stats["entries_active"] * stats["block_rows"] / max(stats["nnz_active"], 1),
+                 "storage": ("matrix values ROUNDED TO IEEE HALF and stored in 16 bits (--value-bits 16: a different input, not the headline "
+                             "configuration)" if args.value_bits == 16 else "fp32 matrix values") +
+                            ", 16-bit indices where exact (else int32), fp64 vectors and accumulators",
+                 "passes_per_iteration": 2 if args.ams else 4, "alg_bytes_per_iteration": iter_bytes,
+                 "alg_bytes_per_iteration_all_rows": iter_bytes_all_rows,
+                 "back_projection": "values of rows with a non-zero coefficient only (--skip-satisfied)" if args.skip_satisfied else
+                                    "every value"},
         "iter_gbs": iter_bytes * K / (ms * 1e-3) / 1e9,
         "e2e": {"value": whole_job_rate(K, 1 if sharded else ws, e2e_s), "unit": UNIT, "h2d_bytes_per_step": plan.n_cols * 4,
                 "d2h_bytes_per_step": plan.n_cols * 4 + STATE_BYTES, "call": "fredopt_iterate_host (pinned host buffers, one call per step)"},

@@ -5,6 +5,8 @@ import os
 import subprocess
 import sys
 
+import pytest
+
 ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 
 
@@ -19,6 +21,26 @@ def test_reference_arm_prints_the_contract_line():
     assert "iterations 3..5 from x0" in line["cpu_baseline"]["sample"]        # the window our arm times: W warm-up, then K
     assert line["e2e"] == {"value": line["value"], "unit": "iterations/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}
     assert line["config"]["workload"].startswith("configs[0]") and line["vs_baseline"] is None
+    # `config` states the workload from the plan and the flags alone (bench.workload_config): the object our arm prints too
+    for k in ("n_voxels", "n_spots", "nnz_per_matrix", "n_labelled_voxels", "lambda", "beta0", "a", "form", "ams_form", "l2", "parallelism"):
+        assert k in line["config"]
+    assert line["config"]["form"] == "superiorized" and line["config"]["l2"].startswith("L2-resident")
+
+
+@pytest.mark.gpu
+def test_both_arms_state_the_same_config():
+    """The driver divides our arm's value by the reference arm's: both lines must name the same workload, key for key."""
+    lines = []
+    for impl in ("reference", "ours"):
+        out = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--impl", impl, "--config", "0", "--steps", "3", "--warmup", "3",
+                              "--no-cpu-baseline", "--no-forms"], capture_output=True, text=True, timeout=900, cwd=ROOT)
+        assert out.returncode == 0, out.stderr[-2000:]
+        lines.append(json.loads(out.stdout.strip().splitlines()[-1]))
+    ref, ours = lines
+    assert ref["config"] == ours["config"]
+    assert (ref["metric"], ref["unit"], ref["higher_is_better"], ref["steps"], ref["warmup"]) == \
+           (ours["metric"], ours["unit"], ours["higher_is_better"], ours["steps"], ours["warmup"])
+    assert ours["plan"]["block_rows"] in (1, 2, 4) and ours["gpu_launches"] > 0 and ref["gpu_launches"] == 0
 
 
 def test_reference_arm_other_ranks_exit_quietly():
